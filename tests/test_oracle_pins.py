@@ -1,0 +1,242 @@
+"""Pins of the CPU oracle against what the paper's definition and the mathematics fix.
+
+The paper prints no worked numeric example, so the pins are: hand-worked closed forms
+(tests/golden/unit_square_cases.json), regular grids, global invariants (sum of measures,
+first-moment identity, per-simplex conservation, neighbour symmetry), brute-force
+equidistance / no-nearer-site of every output corner (Eq. 1), Qhull
+(scipy.spatial) Voronoi volumes / Delaunay neighbours / circumcentres for interior cells,
+and tier A == tier B.  None of these re-types the oracle's own formulas.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2509_07175_b200 import inputs
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _mesh_centroid(w):
+    p = w.verts[w.simplices]
+    c = p.mean(axis=1)
+    if w.kind == inputs.KIND_TRI_2D:
+        e1, e2 = p[:, 1] - p[:, 0], p[:, 2] - p[:, 0]
+        a = np.abs(e1[:, 0] * e2[:, 1] - e1[:, 1] * e2[:, 0]) * 0.5
+    elif w.kind == inputs.KIND_TRI_SURFACE:
+        a = np.linalg.norm(np.cross(p[:, 1] - p[:, 0], p[:, 2] - p[:, 0]), axis=1) * 0.5
+    else:
+        a = np.abs(np.linalg.det(p[:, 1:] - p[:, :1])) / 6.0
+    return a, (a[:, None] * c).sum(0)
+
+
+def _check_invariants(w, c, corner_sample=4000, seed=0):
+    """Invariants that hold for any correct answer, none using the oracle's code."""
+    n = w.n
+    simplex_measure, first_moment = _mesh_centroid(w)
+    # (1) cells partition the domain
+    assert abs(c.measure.sum() - w.measure) <= 1e-11 * w.measure
+    # (2) first moments add up to the domain's
+    mom = (c.measure[:, None] * c.centroid).sum(0)
+    assert np.abs(mom - first_moment).max() <= 1e-11 * max(1.0, np.abs(first_moment).max())
+    # (3) pieces partition every simplex
+    per_simplex = np.bincount(c.piece_simplex, weights=c.piece_measure, minlength=w.m)
+    assert np.abs(per_simplex - simplex_measure).max() <= 1e-11 * simplex_measure.max()
+    # (4) neighbour symmetry
+    pairs = set()
+    for i in range(n):
+        for j in c.neighbours(i):
+            pairs.add((i, int(j)))
+    for (i, j) in pairs:
+        assert (j, i) in pairs, f"neighbour relation not symmetric: {i}->{j}"
+    # (5) every corner is equidistant from its cell's site and from the sites in its label, and
+    #     no site is nearer (brute force over all n) -- Eq. 1
+    rng = np.random.default_rng(seed)
+    owner = np.repeat(np.repeat(np.arange(n), np.diff(c.piece_off)), np.diff(c.vert_off))
+    nvt = c.vert_xyz.shape[0]
+    pick = rng.choice(nvt, size=min(corner_sample, nvt), replace=False)
+    scale = w.diameter
+    for v in pick:
+        x = c.vert_xyz[v]
+        d = np.linalg.norm(w.sites - x, axis=1)
+        di = d[owner[v]]
+        assert di <= d.min() + 1e-10 * scale
+        for fl in c.vert_flags[v]:
+            if fl >= 0:
+                assert abs(d[fl] - di) <= 1e-10 * scale
+    # (6) 3D pieces are simple polytopes: V = 2F - 4 with F = number of distinct labels
+    if w.kind == inputs.KIND_TET_3D:
+        for p in range(len(c.piece_simplex)):
+            xyz, fl = c.piece_verts(p)
+            if (fl == ~w.m).any():
+                continue  # two boundary faces of one tet share the label ~m: F is not countable from labels
+            F = len(np.unique(fl))
+            assert xyz.shape[0] == 2 * F - 4
+
+
+# ---------------------------------------------------------------------- golden hand cases
+def test_golden_unit_square_cases():
+    with open(os.path.join(HERE, "golden", "unit_square_cases.json")) as f:
+        cases = json.load(f)["cases"]
+    v, t = inputs.unit_square_mesh()
+    for case in cases:
+        s = np.array(case["sites"], dtype=np.float64)
+        c = oracle.compute(s, v, t, inputs.KIND_TRI_2D)
+        assert np.allclose(c.measure, case["area"], rtol=0, atol=1e-12)
+        for i, cen in enumerate(case["centroid"]):
+            if cen is not None:
+                assert np.allclose(c.centroid[i], cen, rtol=0, atol=1e-12)
+        for i, nb in enumerate(case["nbr"]):
+            assert c.neighbours(i).tolist() == nb
+        if case["pieces"] is not None:
+            for i, pcs in enumerate(case["pieces"]):
+                got = [[int(c.piece_simplex[p]), int(c.vert_off[p + 1] - c.vert_off[p])] for p in c.pieces(i)]
+                assert got == pcs
+
+
+def test_three_site_voronoi_vertex_and_flags():
+    # sites (0.5,0.2),(0.2,0.8),(0.8,0.8): the Voronoi vertex is (0.5, 0.575) by hand.
+    v, t = inputs.unit_square_mesh()
+    s = np.array([[0.5, 0.2], [0.2, 0.8], [0.8, 0.8]])
+    c = oracle.compute(s, v, t, inputs.KIND_TRI_2D)
+    hits = 0
+    for vtx, fl in zip(c.vert_xyz, c.vert_flags):
+        if fl[0] >= 0 and fl[1] >= 0:
+            assert np.allclose(vtx, [0.5, 0.575], atol=1e-14)
+            hits += 1
+    assert hits == 3  # one per cell
+    # boundary flags: ~flag == m (=2) on the square's sides, ~flag == other triangle on the diagonal
+    assert set(np.unique(c.vert_flags[c.vert_flags < 0]).tolist()) <= {~0, ~1, ~2}
+    assert c.simplex_adj.tolist() == [[2, 1, 2], [2, 2, 0]]
+
+
+def test_two_sites_in_cube():
+    # bisector x = 1/2: two half cubes, centroids (1/4,1/2,1/2), (3/4,1/2,1/2)
+    v, t = inputs.cube_kuhn_mesh(1)
+    s = np.array([[0.25, 0.5, 0.5], [0.75, 0.5, 0.5]])
+    c = oracle.compute(s, v, t, inputs.KIND_TET_3D)
+    assert np.allclose(c.measure, [0.5, 0.5], atol=1e-15)
+    assert np.allclose(c.centroid, s, atol=1e-15)
+    assert c.neighbours(0).tolist() == [1] and c.neighbours(1).tolist() == [0]
+
+
+@pytest.mark.parametrize("dim,k", [(2, 4), (3, 3)])
+def test_regular_grid_equal_cells(dim, k):
+    # degenerate (cocircular / cospherical) input: only measure and centroid are unique
+    s = inputs.grid_sites(k, dim)
+    if dim == 2:
+        v, t = inputs.unit_square_mesh()
+        kind = inputs.KIND_TRI_2D
+    else:
+        v, t = inputs.cube_kuhn_mesh(2)
+        kind = inputs.KIND_TET_3D
+    c = oracle.compute(s, v, t, kind)
+    assert np.allclose(c.measure, 1.0 / k ** dim, rtol=0, atol=1e-14)
+    assert np.allclose(c.centroid, s, rtol=0, atol=1e-13)
+    # face-adjacent sites must be neighbours
+    for i in range(len(s)):
+        d = np.abs(s - s[i]).sum(1)
+        face_adj = set(np.nonzero(np.isclose(d, 1.0 / k))[0].tolist())
+        assert face_adj <= set(c.neighbours(i).tolist())
+
+
+# ---------------------------------------------------------------------- invariants, full C1 + replicas
+def test_c1_full_invariants():
+    w = inputs.config(1)
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    _check_invariants(w, c)
+    assert (c.measure > 0).all()
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4, 5])
+def test_replica_invariants(idx):
+    w = inputs.config(idx, "small")
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    _check_invariants(w, c, corner_sample=1500)
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 5])
+def test_tier_b_equals_tier_a(idx):
+    w = inputs.config(idx, "small")
+    rng = np.random.default_rng(10 + idx)
+    sub = np.sort(rng.choice(w.n, size=min(w.n, 300), replace=False))
+    a = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=sub, tier="A")
+    b = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=sub, tier="B")
+    assert np.array_equal(a.piece_off, b.piece_off)
+    assert np.array_equal(a.piece_simplex, b.piece_simplex)
+    assert np.array_equal(a.vert_off, b.vert_off)
+    assert np.array_equal(a.vert_flags, b.vert_flags)
+    assert np.array_equal(a.nbr_off, b.nbr_off) and np.array_equal(a.nbr, b.nbr)
+    assert np.abs(a.vert_xyz - b.vert_xyz).max() <= 1e-12 * w.diameter
+    assert np.allclose(a.measure, b.measure, rtol=1e-11, atol=0)
+
+
+# ---------------------------------------------------------------------- library special case (Qhull)
+def test_qhull_interior_cells_3d():
+    """Cells that do not touch the cube boundary are ordinary Voronoi cells: volume = hull of the
+    Qhull Voronoi region, neighbours = Delaunay neighbours, 3-site corners = circumcentres."""
+    from scipy.spatial import ConvexHull, Delaunay, Voronoi
+    w = inputs.config(2, "small")
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    vor = Voronoi(w.sites)
+    tri = Delaunay(w.sites)
+    indptr, indices = tri.vertex_neighbor_vertices
+    m = w.m
+    checked = 0
+    for i in range(w.n):
+        fl = np.concatenate([c.piece_verts(p)[1].ravel() for p in c.pieces(i)])
+        if (fl == ~m).any():
+            continue  # touches the domain boundary
+        region = vor.regions[vor.point_region[i]]
+        assert -1 not in region
+        vol = ConvexHull(vor.vertices[region]).volume
+        assert abs(vol - c.measure[i]) <= 1e-9 * vol
+        assert sorted(indices[indptr[i]:indptr[i + 1]].tolist()) == c.neighbours(i).tolist()
+        # corners labelled by three sites are Voronoi vertices (circumcentres of Delaunay tets)
+        vv = vor.vertices[region]
+        for p in c.pieces(i):
+            xyz, f3 = c.piece_verts(p)
+            for x, f in zip(xyz, f3):
+                if (f >= 0).all():
+                    assert np.linalg.norm(vv - x, axis=1).min() <= 1e-9
+        checked += 1
+    assert checked > 200
+
+
+def test_qhull_interior_cells_2d():
+    from scipy.spatial import Delaunay, Voronoi
+    w = inputs.config(1)
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    vor = Voronoi(w.sites)
+    tri = Delaunay(w.sites)
+    indptr, indices = tri.vertex_neighbor_vertices
+    checked = 0
+    for i in range(w.n):
+        fl = np.concatenate([c.piece_verts(p)[1].ravel() for p in c.pieces(i)])
+        if (fl == ~w.m).any():
+            continue
+        region = vor.regions[vor.point_region[i]]
+        assert -1 not in region
+        P = vor.vertices[region]
+        cx = P[:, 0] * np.roll(P[:, 1], -1) - np.roll(P[:, 0], -1) * P[:, 1]
+        assert abs(abs(cx.sum()) * 0.5 - c.measure[i]) <= 1e-10 * c.measure[i]
+        assert sorted(indices[indptr[i]:indptr[i + 1]].tolist()) == c.neighbours(i).tolist()
+        checked += 1
+    assert checked > 1500
+
+
+def test_surface_pieces_lie_in_their_triangle():
+    w = inputs.config(4, "small")
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    for p in range(len(c.piece_simplex)):
+        tri = w.verts[w.simplices[c.piece_simplex[p]]]
+        nrm = np.cross(tri[1] - tri[0], tri[2] - tri[0])
+        nrm /= np.linalg.norm(nrm)
+        xyz, _ = c.piece_verts(p)
+        assert np.abs((xyz - tri[0]) @ nrm).max() <= 1e-13
+    # cells with an empty restricted cell follow the empty-cell convention
+    empty = c.measure == 0
+    assert empty.any()
+    assert np.array_equal(c.centroid[empty], w.sites[empty])
