@@ -1,0 +1,165 @@
+/* vd.h -- C ABI of libvd.so: clipped / restricted Voronoi cells by point-in-cell clipping on one B200.
+ *
+ * The calls follow the problem statement of "Efficient Computation of Voronoi Diagrams Using
+ * Point-in-Cell Tests" (Xiao, Cao, Chen; /root/reference/PAPER.md, cited below as P:Lnnn):
+ * input sites V = {v_i} in R^d and a domain M = {T_a} of simplices, output the domain-cell
+ * intersections {Omega_i ∩ M}, i = 1..n  (Eq. 1 at P:L77), each the union of
+ * simplex-cell pieces P_{a,i} = T_a ∩ Omega_i whose edges / faces carry flags.
+ *
+ * Everything behind these calls runs in hand-written CUDA kernels for sm_100a, in fp64.  There is
+ * no CPU fallback: every entry point that needs the device returns VD_E_CUDA when it is missing.
+ *
+ * Pointers: every INPUT pointer may be a host pointer or a device pointer (resolved with
+ * cudaPointerGetAttributes); inputs are copied, the caller keeps ownership and may free them as
+ * soon as the call returns.  Every OUTPUT pointer inside vd_cells is a DEVICE pointer owned by the
+ * context, valid until the next vd_compute on that context or vd_destroy.  One context must be
+ * used by one host thread at a time.  Errors are return codes only; a failed call leaves the
+ * context usable; vd_last_error() gives a one-line description.
+ */
+#ifndef VD_H_
+#define VD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vd_ctx vd_ctx; /* opaque; owns all device state */
+
+typedef enum {
+  VD_OK = 0,
+  VD_E_ARG = 1,        /* null pointer, n < 1, m < 1, bad kind                                   */
+  VD_E_DIM = 2,        /* dim not in {2,3} or kind / dim mismatch                                */
+  VD_E_STATE = 3,      /* vd_compute before vd_set_domain, vd_cells_to_host before vd_compute    */
+  VD_E_INPUT = 4,      /* NaN/Inf, index out of range, zero-measure simplex, non-manifold face   */
+  VD_E_CUDA = 5,       /* no device, or a CUDA runtime error                                     */
+  VD_E_NOMEM = 6,
+  VD_E_CAPACITY = 7,   /* a piece outgrew every capacity tier (see vd_options)                   */
+  VD_E_NOCONVERGE = 8  /* an iteration cap was hit (degenerate input: duplicate sites, ...)      */
+} vd_status;
+
+/* Domain kinds.  dim == 2 <=> VD_TRI_2D;  dim == 3 <=> VD_TRI_SURFACE or VD_TET_3D. */
+typedef enum { VD_TRI_2D = 0, VD_TRI_SURFACE = 1, VD_TET_3D = 2 } vd_domain_kind;
+
+/* Result of vd_compute: CSR arrays, 0-based, DEVICE pointers.
+ *
+ * Flags (P:L85, 0-based restatement): flag >= 0 is a site id j (the edge/face lies on the bisector
+ * B_ij); flag < 0 means ~flag is the id of the simplex adjacent across that edge/face of T_a, with
+ * ~flag == m marking a face on the domain boundary.
+ *
+ * cell i:   measure[i] = sum_a |P_{a,i}|,  centroid[i*dim..] = sum_a |P|.c(P) / measure[i];
+ *           an empty cell has measure 0, centroid = the site itself, no pieces, no neighbours.
+ *           nbr[nbr_off[i] .. nbr_off[i+1])   : ascending site ids j, each once, such that some piece
+ *                                               of cell i has an edge/face on B_ij (restricted neighbours).
+ *           pieces piece_off[i] .. piece_off[i+1], ascending simplex id piece_simplex[p].
+ * piece p:  corners vert_off[p] .. vert_off[p+1]: vert_xyz[v*dim..], and vert_flags[v*nfl..] = the
+ *           flags of the nfl edges/faces meeting at the corner, ascending (nfl = 2 for triangle
+ *           kinds, 3 for tets); corners are sorted lexicographically by that flag tuple.
+ */
+typedef struct vd_cells {
+  int64_t n;           /* number of sites = number of cells                                      */
+  int32_t dim, nfl;
+  int64_t n_nonempty, n_pieces, n_verts, n_nbrs;
+  const double* measure;        /* [n]            */
+  const double* centroid;       /* [n*dim]        */
+  const int64_t* nbr_off;       /* [n+1]          */
+  const int32_t* nbr;           /* [n_nbrs]       */
+  const int64_t* piece_off;     /* [n+1]          */
+  const int32_t* piece_simplex; /* [n_pieces]     */
+  const double* piece_measure;  /* [n_pieces]     */
+  const int64_t* vert_off;      /* [n_pieces+1]   */
+  const double* vert_xyz;       /* [n_verts*dim]  */
+  const int32_t* vert_flags;    /* [n_verts*nfl]  */
+} vd_cells;
+
+/* Tunables (P:L383 grid density; P:L369 step-out).  Zero / negative fields mean "default". */
+typedef struct vd_options {
+  double grid_density;    /* average sites per grid cell of the site index (default 4.0; paper 2~4) */
+  int32_t step_out;       /* 1: use the improved search of section VI-A; default 0     */
+  int32_t real_edges;     /* 1 (default): search on a real edge p_s p_t when the outside corner has
+                             a known-inside neighbour (Alg. 1); 0: always the virtual
+                             edge from the pair's witness point (Alg. 3)               */
+  int32_t persistent;     /* 1 (default): device-side work queue; 0: one launch per wave  */
+  int64_t pair_capacity;  /* initial capacity of the (simplex, site) pair list; grows on demand     */
+  int64_t vert_capacity;  /* initial capacity of the corner pool; grows on demand                   */
+  int32_t reserved[8];
+} vd_options;
+
+/* Work counters of the last vd_compute (always collected; a few atomics per pair). */
+typedef struct vd_counters {
+  int64_t pairs;          /* (simplex, site) pairs processed = Alg. 3 runs          */
+  int64_t pieces;         /* non-empty pieces                                                      */
+  int64_t queries;        /* nearest-site queries = point-in-cell tests + seeds     */
+  int64_t dist_evals;     /* site distance evaluations inside those queries                        */
+  int64_t search_iters;   /* iterations of the edge-based bisector search                 */
+  int64_t clips;          /* clippings performed                                    */
+  int64_t waves;          /* wavefronts; 1 in persistent mode                       */
+  int64_t overflow_pairs; /* pairs that needed the large-capacity path                             */
+  int64_t reruns;         /* times the whole compute was repeated after growing a pool            */
+  int64_t reserved[7];
+} vd_counters;
+
+/* vd_create: copy n sites of dimension dim (row-major [n][dim], fp64).  Builds nothing heavy: the
+ * site index (line 1 of Alg. 2/4/5) is built inside vd_compute.
+ * Errors: VD_E_ARG, VD_E_DIM, VD_E_INPUT (non-finite coordinate), VD_E_CUDA, VD_E_NOMEM. */
+vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out);
+
+/* vd_update_sites: replace the coordinates of the n sites (same n, dim) -- for Lloyd iterations
+ * (P:L483-492).  Same errors as vd_create. */
+vd_status vd_update_sites(vd_ctx* ctx, const double* sites);
+
+/* vd_set_domain: copy the domain M = {T_a}: verts [nv][dim] fp64, simplices [m][3]
+ * (both triangle kinds) or [m][4] (tets), int32, 0-based, any orientation.  Derives the simplex
+ * adjacency that initialises the edge/face flags (Fig. 2a).  May be called again.
+ * Errors: VD_E_ARG, VD_E_DIM, VD_E_INPUT (index out of range, zero-measure simplex, an edge/face
+ * shared by more than two simplices), VD_E_CUDA, VD_E_NOMEM. */
+vd_status vd_set_domain(vd_ctx* ctx, const double* verts, int64_t nv, const int32_t* simplices, int64_t m,
+                        vd_domain_kind kind);
+
+/* vd_compute: the whole hot path -- site index, seeds, (simplex, site) clipping by point-in-cell
+ * tests (Alg. 3/4/5), propagation over flags, assembly.  Asynchronous on the context's
+ * stream except for one small read-back of counts at the end.  Fills *out_cells.
+ * Errors: VD_E_ARG, VD_E_STATE, VD_E_CUDA, VD_E_NOMEM, VD_E_CAPACITY, VD_E_NOCONVERGE. */
+vd_status vd_compute(vd_ctx* ctx, vd_cells* out_cells);
+
+void vd_destroy(vd_ctx* ctx);
+
+/* ---- support calls ---- */
+
+/* Stream all later work of this context is issued on (e.g. torch.cuda.current_stream().cuda_stream). */
+vd_status vd_set_stream(vd_ctx* ctx, void* cuda_stream);
+
+/* Device allocator hooks (e.g. the torch caching allocator).  NULL restores cudaMalloc / cudaFree. */
+vd_status vd_set_allocator(vd_ctx* ctx, void* (*alloc)(size_t bytes, void* user, void* stream),
+                           void (*release)(void* ptr, void* user), void* user);
+
+vd_status vd_set_options(vd_ctx* ctx, const vd_options* opt);
+vd_status vd_get_counters(const vd_ctx* ctx, vd_counters* out);
+
+/* Per-stage device times (ms, CUDA events) of the last vd_compute:
+ * [0] site index (S1)  [1] seeds (S3)  [2] clip + propagate (S4+S5)  [3] assemble (S6)  [4] total. */
+vd_status vd_get_stage_ms(const vd_ctx* ctx, double out_ms[5]);
+
+/* Copy the last result into caller HOST buffers (any may be NULL to skip).  Sizes are those of
+ * vd_cells.  Synchronises the context's stream. */
+vd_status vd_cells_to_host(vd_ctx* ctx, double* measure, double* centroid, int64_t* nbr_off, int32_t* nbr,
+                           int64_t* piece_off, int32_t* piece_simplex, double* piece_measure,
+                           int64_t* vert_off, double* vert_xyz, int32_t* vert_flags);
+
+/* Nearest site N_q of nq query points [nq][dim] through the site index (built on demand):
+ * out_index[q] = argmin_j |q - v_j|, ties to the lowest id.  queries / out_index: host or device. */
+vd_status vd_nearest(vd_ctx* ctx, const double* queries, int64_t nq, int32_t* out_index);
+
+/* Simplex adjacency derived by vd_set_domain, [m][3 or 4] int32: adj[a][k] = simplex across the
+ * edge/face opposite local corner k, or m on the domain boundary.  out: host or device. */
+vd_status vd_get_adjacency(vd_ctx* ctx, int32_t* out);
+
+const char* vd_last_error(const vd_ctx* ctx);
+const char* vd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VD_H_ */

@@ -1,0 +1,244 @@
+"""Thin ctypes binding of libvd.so (include/vd.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; this module converts numpy / torch
+arguments to pointers and copies results back on request.  There is no CPU fallback: if
+libvd.so is missing, cannot be loaded, or finds no CUDA device, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D = 0, 1, 2
+STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_INPUT", 5: "VD_E_CUDA",
+          6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
+EXPORTS = ["vd_create", "vd_update_sites", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
+           "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_cells_to_host",
+           "vd_nearest", "vd_get_adjacency", "vd_last_error", "vd_version"]
+
+_LIB_PATH = _build.lib_path()
+_lib = None
+
+
+class VdError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class vd_cells(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int64), ("dim", ctypes.c_int32), ("nfl", ctypes.c_int32),
+                ("n_nonempty", ctypes.c_int64), ("n_pieces", ctypes.c_int64), ("n_verts", ctypes.c_int64),
+                ("n_nbrs", ctypes.c_int64),
+                ("measure", ctypes.c_void_p), ("centroid", ctypes.c_void_p), ("nbr_off", ctypes.c_void_p),
+                ("nbr", ctypes.c_void_p), ("piece_off", ctypes.c_void_p), ("piece_simplex", ctypes.c_void_p),
+                ("piece_measure", ctypes.c_void_p), ("vert_off", ctypes.c_void_p), ("vert_xyz", ctypes.c_void_p),
+                ("vert_flags", ctypes.c_void_p)]
+
+
+class vd_options(ctypes.Structure):
+    _fields_ = [("grid_density", ctypes.c_double), ("step_out", ctypes.c_int32), ("real_edges", ctypes.c_int32),
+                ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
+                ("reserved", ctypes.c_int32 * 8)]
+
+
+class vd_counters(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int64) for k in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips",
+                                               "waves", "overflow_pairs", "reruns")] + [("reserved", ctypes.c_int64 * 7)]
+
+
+def load():
+    """Load libvd.so (raises if it is missing: build it with __graft_entry__.build())."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(f"{_LIB_PATH} not found: the CUDA library is not built (python -m paper_2509_07175_b200.build)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    lib.vd_create.argtypes = [vp, i64, ci, ctypes.POINTER(vp)]
+    lib.vd_update_sites.argtypes = [vp, vp]
+    lib.vd_set_domain.argtypes = [vp, vp, i64, vp, i64, ci]
+    lib.vd_compute.argtypes = [vp, ctypes.POINTER(vd_cells)]
+    lib.vd_destroy.argtypes = [vp]
+    lib.vd_destroy.restype = None
+    lib.vd_set_stream.argtypes = [vp, vp]
+    lib.vd_set_allocator.argtypes = [vp, vp, vp, vp]
+    lib.vd_set_options.argtypes = [vp, ctypes.POINTER(vd_options)]
+    lib.vd_get_counters.argtypes = [vp, ctypes.POINTER(vd_counters)]
+    lib.vd_get_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    lib.vd_cells_to_host.argtypes = [vp] + [vp] * 10
+    lib.vd_nearest.argtypes = [vp, vp, i64, vp]
+    lib.vd_get_adjacency.argtypes = [vp, vp]
+    lib.vd_last_error.argtypes = [vp]
+    lib.vd_last_error.restype = ctypes.c_char_p
+    lib.vd_version.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        if getattr(lib, name).restype is ctypes.c_int and name not in ("vd_destroy",):
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _ptr(x, dtype):
+    """(pointer, keepalive) of a numpy array (host) or a torch tensor (host or CUDA)."""
+    if isinstance(x, np.ndarray):
+        a = np.ascontiguousarray(x, dtype=dtype)
+        return a.ctypes.data, a
+    if hasattr(x, "data_ptr"):  # torch tensor
+        import torch
+        want = {np.float64: torch.float64, np.int32: torch.int32}[dtype]
+        t = x.contiguous()
+        if t.dtype != want:
+            t = t.to(want)
+        return t.data_ptr(), t
+    a = np.ascontiguousarray(np.asarray(x), dtype=dtype)
+    return a.ctypes.data, a
+
+
+@dataclass
+class HostCells:
+    """Result of vd_compute copied to the host (same CSR arrays as include/vd.h's vd_cells)."""
+    n: int
+    dim: int
+    nfl: int
+    n_nonempty: int
+    measure: np.ndarray
+    centroid: np.ndarray
+    nbr_off: np.ndarray
+    nbr: np.ndarray
+    piece_off: np.ndarray
+    piece_simplex: np.ndarray
+    piece_measure: np.ndarray
+    vert_off: np.ndarray
+    vert_xyz: np.ndarray
+    vert_flags: np.ndarray
+
+    def neighbours(self, i):
+        return self.nbr[self.nbr_off[i]:self.nbr_off[i + 1]]
+
+    def pieces(self, i):
+        return range(int(self.piece_off[i]), int(self.piece_off[i + 1]))
+
+    def piece_verts(self, p):
+        a, b = int(self.vert_off[p]), int(self.vert_off[p + 1])
+        return self.vert_xyz[a:b], self.vert_flags[a:b]
+
+
+class Context:
+    """vd_ctx wrapper: vd_create / vd_set_domain / vd_compute / vd_destroy."""
+
+    def __init__(self, sites, dim=None):
+        self._lib = load()
+        self._h = ctypes.c_void_p()
+        shape = tuple(sites.shape)
+        self.n, self.dim = int(shape[0]), int(shape[1] if dim is None else dim)
+        p, keep = _ptr(sites, np.float64)
+        self._check(self._lib.vd_create(p, self.n, self.dim, ctypes.byref(self._h)), create=True)
+        self.cells = vd_cells()
+        self.kind = None
+        self.m = 0
+        self.nc = 0
+
+    def _check(self, rc, create=False):
+        if rc != 0:
+            msg = "" if create else (self._lib.vd_last_error(self._h) or b"").decode()
+            if create and rc == 5:
+                msg = "no CUDA device (this library has no CPU fallback)"
+            raise VdError(rc, msg)
+
+    def set_stream(self, cuda_stream: int):
+        self._check(self._lib.vd_set_stream(self._h, ctypes.c_void_p(cuda_stream)))
+
+    def set_options(self, **kw):
+        o = vd_options()
+        o.real_edges = 1
+        for k, v in kw.items():
+            setattr(o, k, v)
+        self._check(self._lib.vd_set_options(self._h, ctypes.byref(o)))
+
+    def update_sites(self, sites):
+        p, keep = _ptr(sites, np.float64)
+        self._check(self._lib.vd_update_sites(self._h, p))
+
+    def set_domain(self, verts, simplices, kind):
+        pv, k1 = _ptr(verts, np.float64)
+        ps, k2 = _ptr(simplices, np.int32)
+        self.kind, self.m, self.nc = int(kind), int(simplices.shape[0]), int(simplices.shape[1])
+        self._check(self._lib.vd_set_domain(self._h, pv, int(verts.shape[0]), ps, self.m, int(kind)))
+
+    def compute(self) -> vd_cells:
+        self._check(self._lib.vd_compute(self._h, ctypes.byref(self.cells)))
+        return self.cells
+
+    def counters(self) -> dict:
+        c = vd_counters()
+        self._check(self._lib.vd_get_counters(self._h, ctypes.byref(c)))
+        return {k: int(getattr(c, k)) for k, _ in vd_counters._fields_ if k != "reserved"}
+
+    def stage_ms(self):
+        a = (ctypes.c_double * 5)()
+        self._check(self._lib.vd_get_stage_ms(self._h, a))
+        return dict(zip(("index", "seed", "clip", "assemble", "total"), [float(x) for x in a]))
+
+    def to_host(self, full=True) -> HostCells:
+        r = self.cells
+        n, dim, nfl = int(r.n), int(r.dim), int(r.nfl)
+        npc, nvt, nnb = int(r.n_pieces), int(r.n_verts), int(r.n_nbrs)
+        out = HostCells(
+            n=n, dim=dim, nfl=nfl, n_nonempty=int(r.n_nonempty),
+            measure=np.empty(n, np.float64), centroid=np.empty((n, dim), np.float64),
+            nbr_off=np.empty(n + 1, np.int64), nbr=np.empty(nnb, np.int32),
+            piece_off=np.empty(n + 1, np.int64), piece_simplex=np.empty(npc, np.int32),
+            piece_measure=np.empty(npc, np.float64), vert_off=np.empty(npc + 1, np.int64),
+            vert_xyz=np.empty((nvt, dim), np.float64) if full else np.empty((0, dim), np.float64),
+            vert_flags=np.empty((nvt, nfl), np.int32) if full else np.empty((0, nfl), np.int32))
+        d = lambda a: a.ctypes.data if a.size else None
+        self._check(self._lib.vd_cells_to_host(
+            self._h, d(out.measure), d(out.centroid), d(out.nbr_off), d(out.nbr), d(out.piece_off),
+            d(out.piece_simplex), d(out.piece_measure), d(out.vert_off),
+            d(out.vert_xyz) if full else None, d(out.vert_flags) if full else None))
+        return out
+
+    def nearest(self, queries) -> np.ndarray:
+        q = np.ascontiguousarray(queries, dtype=np.float64)
+        out = np.empty(q.shape[0], np.int32)
+        self._check(self._lib.vd_nearest(self._h, q.ctypes.data, q.shape[0], out.ctypes.data))
+        return out
+
+    def adjacency(self) -> np.ndarray:
+        out = np.empty((self.m, self.nc), np.int32)
+        self._check(self._lib.vd_get_adjacency(self._h, out.ctypes.data))
+        return out
+
+    def destroy(self):
+        if self._h:
+            self._lib.vd_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def compute(sites, verts, simplices, kind, **options) -> HostCells:
+    """One-shot: vd_create -> vd_set_domain -> vd_compute -> copy to host -> vd_destroy."""
+    with Context(sites) as ctx:
+        if options:
+            ctx.set_options(**options)
+        ctx.set_domain(verts, simplices, kind)
+        ctx.compute()
+        return ctx.to_host()

@@ -1,0 +1,338 @@
+// vd_api.cu -- the C ABI of include/vd.h: argument marshalling, memory, the stage sequence of
+// vd_compute and the pool-growth / rerun policy.  No geometry happens on the host.
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "vd_internal.h"
+
+namespace vd {
+
+vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return VD_OK;
+  if (c) c->lastError = std::string(what) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? VD_E_NOMEM : VD_E_CUDA;
+}
+
+void release(vd_ctx* c, DevBuf& b) {
+  if (!b.p) return;
+  if (c->freeFn) c->freeFn(b.p, c->allocUser); else cudaFree(b.p);
+  b.p = nullptr;
+  b.cap = 0;
+}
+
+vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
+  if (bytes < 256) bytes = 256;
+  if (b.cap >= bytes) return VD_OK;
+  // pending kernels may still use the old block
+  cudaStreamSynchronize(c->stream);
+  release(c, b);
+  void* p = nullptr;
+  if (c->allocFn) {
+    p = c->allocFn(bytes, c->allocUser, (void*)c->stream);
+    if (!p) { c->lastError = "allocator hook returned NULL"; return VD_E_NOMEM; }
+  } else {
+    const cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); c->lastError = "cudaMalloc failed"; return VD_E_NOMEM; }
+  }
+  b.p = p;
+  b.cap = bytes;
+  return VD_OK;
+}
+
+// [n][dim] (host or device) -> device [n][3], z = 0 for dim 2; flags non-finite values
+__global__ void __launch_bounds__(kBlock) k_pad3(const double* __restrict__ in, int64_t n, int dim, double* __restrict__ out, unsigned int* err) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    bool bad = false;
+    for (int a = 0; a < 3; ++a) {
+      const double v = a < dim ? in[i * dim + a] : 0.0;
+      if (!(v == v) || fabs(v) > 1e150) bad = true;
+      out[i * 3 + a] = v;
+    }
+    if (bad) atomicOr(err, ERR_INPUT);
+  }
+}
+
+static vd_status upload_points(vd_ctx* c, const double* src, int64_t n, int dim, DevBuf& dst, const char* what) {
+  vd_status s;
+  DevBuf tmp;
+  if ((s = ensure(c, dst, sizeof(double) * 3 * n))) return s;
+  if ((s = ensure(c, tmp, sizeof(double) * dim * n))) return s;
+  if ((s = ensure(c, c->control, sizeof(Control)))) { release(c, tmp); return s; }
+  cudaError_t e = cudaMemcpyAsync(tmp.p, src, sizeof(double) * dim * n, cudaMemcpyDefault, c->stream);
+  if (e != cudaSuccess) { release(c, tmp); return cuda_check(c, e, what); }
+  cudaMemsetAsync(c->control.p, 0, sizeof(Control), c->stream);
+  int blocks = (int)((n + kBlock - 1) / kBlock);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  VD_LAUNCH(k_pad3, blocks, kBlock, 0, c->stream)(tmp.as<double>(), n, dim, dst.as<double>(), &c->control.as<Control>()->err);
+  Control h;
+  e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  release(c, tmp);
+  if (e != cudaSuccess) return cuda_check(c, e, what);
+  if (h.err & ERR_INPUT) { c->lastError = std::string(what) + ": non-finite coordinate"; return VD_E_INPUT; }
+  return VD_OK;
+}
+
+static void set_default_options(vd_options& o) {
+  memset(&o, 0, sizeof(o));
+  o.grid_density = 4.0;
+  o.step_out = 0;
+  o.real_edges = 1;
+  o.persistent = 0;
+}
+
+static int64_t next_pow2(int64_t v) {
+  int64_t p = 1;
+  while (p < v) p <<= 1;
+  return p;
+}
+
+static vd_status alloc_pools(vd_ctx* c) {
+  vd_status s;
+  c->hashCap = next_pow2(2 * c->pairCap);
+  c->ovfCap = c->pairCap;
+  if ((s = ensure(c, c->pairs, sizeof(Pair) * c->pairCap))) return s;
+  if ((s = ensure(c, c->pieces, sizeof(Piece) * c->pairCap))) return s;
+  if ((s = ensure(c, c->visited, sizeof(unsigned long long) * c->hashCap))) return s;
+  if ((s = ensure(c, c->ovf, sizeof(int) * c->ovfCap))) return s;
+  if ((s = ensure(c, c->poolXYZ, sizeof(double) * 3 * c->vertCap))) return s;
+  if ((s = ensure(c, c->poolFlags, sizeof(int) * c->nfl * c->vertCap))) return s;
+  if ((s = ensure(c, c->poolNbr, sizeof(int) * c->nbrCap))) return s;
+  if ((s = ensure(c, c->sitePieces, sizeof(int) * c->n))) return s;
+  if ((s = ensure(c, c->siteNbrRaw, sizeof(int) * c->n))) return s;
+  return VD_OK;
+}
+
+}  // namespace vd
+
+using namespace vd;
+
+extern "C" {
+
+const char* vd_version(void) { return "vd-b200 0.1 (sm_100a, fp64)"; }
+
+const char* vd_last_error(const vd_ctx* ctx) { return ctx ? ctx->lastError.c_str() : "null context"; }
+
+vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out) {
+  if (!sites || !out || n < 1) return VD_E_ARG;
+  if (dim != 2 && dim != 3) return VD_E_DIM;
+  if (n > 0x7fffffff) return VD_E_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return VD_E_CUDA; }
+  vd_ctx* c = new (std::nothrow) vd_ctx();
+  if (!c) return VD_E_NOMEM;
+  c->n = n;
+  c->dim = dim;
+  set_default_options(c->opt);
+  for (int k = 0; k < 6; ++k) cudaEventCreate(&c->ev[k]);
+  const vd_status s = upload_points(c, sites, n, dim, c->sites, "vd_create");
+  if (s != VD_OK) { vd_destroy(c); return s; }
+  *out = c;
+  return VD_OK;
+}
+
+vd_status vd_update_sites(vd_ctx* c, const double* sites) {
+  if (!c || !sites) return VD_E_ARG;
+  c->indexValid = false;
+  c->haveResult = false;
+  return upload_points(c, sites, c->n, c->dim, c->sites, "vd_update_sites");
+}
+
+vd_status vd_set_domain(vd_ctx* c, const double* verts, int64_t nv, const int32_t* simplices, int64_t m, vd_domain_kind kind) {
+  if (!c || !verts || !simplices || nv < 1 || m < 1) return VD_E_ARG;
+  if (kind != VD_TRI_2D && kind != VD_TRI_SURFACE && kind != VD_TET_3D) return VD_E_ARG;
+  if ((kind == VD_TRI_2D) != (c->dim == 2)) return VD_E_DIM;
+  if (m > 0x3fffffff || nv > 0x7fffffff) return VD_E_ARG;
+  c->haveDomain = false;
+  c->haveResult = false;
+  c->kind = (int)kind;
+  c->nc = kind == VD_TET_3D ? 4 : 3;
+  c->nfl = kind == VD_TET_3D ? 3 : 2;
+  c->nv = nv;
+  c->m = m;
+  vd_status s = upload_points(c, verts, nv, c->dim, c->verts, "vd_set_domain");
+  if (s != VD_OK) return s;
+  if ((s = ensure(c, c->simp, sizeof(int) * m * c->nc))) return s;
+  cudaError_t e = cudaMemcpyAsync(c->simp.p, simplices, sizeof(int) * m * c->nc, cudaMemcpyDefault, c->stream);
+  if (e != cudaSuccess) return cuda_check(c, e, "vd_set_domain");
+  if ((s = stage_domain(c))) return s;
+  c->haveDomain = true;
+  return VD_OK;
+}
+
+vd_status vd_compute(vd_ctx* c, vd_cells* out) {
+  if (!c || !out) return VD_E_ARG;
+  if (!c->haveDomain) { c->lastError = "vd_compute before vd_set_domain"; return VD_E_STATE; }
+  c->haveResult = false;
+  if (c->pairCap == 0) {
+    c->pairCap = c->opt.pair_capacity > 0 ? c->opt.pair_capacity : (8 * c->m + 4 * c->n + (1 << 16));
+    c->vertCap = c->opt.vert_capacity > 0 ? c->opt.vert_capacity : 12 * c->pairCap;
+    c->nbrCap = 8 * c->pairCap;
+  }
+  memset(&c->counters, 0, sizeof(c->counters));
+  cudaStream_t st = c->stream;
+  vd_status s;
+  for (int attempt = 0;; ++attempt) {
+    if ((s = alloc_pools(c))) return s;
+    if ((s = ensure(c, c->control, sizeof(Control)))) return s;
+    cudaMemsetAsync(c->control.p, 0, sizeof(Control), st);
+    cudaEventRecord(c->ev[0], st);
+    if ((s = stage_index(c))) return s;
+    cudaEventRecord(c->ev[1], st);
+    if ((s = stage_seed(c))) return s;
+    cudaEventRecord(c->ev[2], st);
+    if ((s = stage_clip(c))) return s;
+    cudaEventRecord(c->ev[3], st);
+    const unsigned err = c->hostControl.err;
+    if (err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) {
+      if (attempt >= 6) { c->lastError = "vd_compute: pools still too small after 6 regrowths"; return VD_E_CAPACITY; }
+      if (err & ERR_PAIR_CAP) c->pairCap *= 2;
+      if (err & ERR_VERT_CAP) c->vertCap *= 2;
+      if (err & ERR_NBR_CAP) c->nbrCap *= 2;
+      c->counters.reruns += 1;
+      continue;
+    }
+    if (err & ERR_INPUT) { c->lastError = "vd_compute: non-finite site coordinate"; return VD_E_INPUT; }
+    if (err & ERR_PIECE_CAP) { c->lastError = "vd_compute: a piece outgrew the large-capacity path"; return VD_E_CAPACITY; }
+    if (err & (ERR_NOCONVERGE | ERR_TOPOLOGY)) {
+      c->lastError = (err & ERR_NOCONVERGE) ? "vd_compute: bisector search hit its iteration cap (degenerate input?)"
+                                            : "vd_compute: clip produced a non-simple rim (degenerate input?)";
+      return VD_E_NOCONVERGE;
+    }
+    break;
+  }
+  if ((s = stage_assemble(c))) return s;
+  cudaEventRecord(c->ev[4], st);
+  Control h;
+  cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_check(c, e, "vd_compute");
+  c->hostControl = h;
+  float ms = 0;
+  for (int k = 0; k < 4; ++k) { cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]); c->stageMs[k] = ms; }
+  cudaEventElapsedTime(&ms, c->ev[0], c->ev[4]);
+  c->stageMs[4] = ms;
+  const int64_t reruns = c->counters.reruns, waves = c->counters.waves;
+  c->counters.pairs = (int64_t)h.cnt.pairs; c->counters.pieces = (int64_t)h.cnt.pieces;
+  c->counters.queries = (int64_t)h.cnt.queries; c->counters.dist_evals = (int64_t)h.cnt.dist_evals;
+  c->counters.search_iters = (int64_t)h.cnt.search_iters; c->counters.clips = (int64_t)h.cnt.clips;
+  c->counters.overflow_pairs = (int64_t)h.ovfTail;
+  c->counters.reruns = reruns; c->counters.waves = waves;
+  vd_cells& r = c->cells;
+  r.n = c->n; r.dim = c->dim; r.nfl = c->nfl;
+  r.n_nonempty = (int64_t)h.nNonEmpty; r.n_pieces = (int64_t)h.nPieces; r.n_verts = (int64_t)h.nVerts; r.n_nbrs = (int64_t)h.nNbrs;
+  r.measure = c->oMeasure.as<double>(); r.centroid = c->oCentroid.as<double>();
+  r.nbr_off = c->oNbrOff.as<int64_t>(); r.nbr = c->oNbr.as<int32_t>();
+  r.piece_off = c->oPieceOff.as<int64_t>(); r.piece_simplex = c->oPieceSimplex.as<int32_t>();
+  r.piece_measure = c->oPieceMeasure.as<double>();
+  r.vert_off = c->oVertOff.as<int64_t>(); r.vert_xyz = c->oVertXYZ.as<double>(); r.vert_flags = c->oVertFlags.as<int32_t>();
+  *out = r;
+  c->haveResult = true;
+  return VD_OK;
+}
+
+void vd_destroy(vd_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
+                   &c->scanTmp, &c->vnn, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
+                   &c->poolNbr, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
+                   &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
+                   &c->oPieceMeasure, &c->oVertOff, &c->oVertXYZ, &c->oVertFlags};
+  for (DevBuf* b : all) release(c, *b);
+  for (int k = 0; k < 6; ++k)
+    if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+  delete c;
+}
+
+vd_status vd_set_stream(vd_ctx* c, void* stream) {
+  if (!c) return VD_E_ARG;
+  cudaStreamSynchronize(c->stream);
+  c->stream = (cudaStream_t)stream;
+  return VD_OK;
+}
+
+vd_status vd_set_allocator(vd_ctx* c, void* (*alloc)(size_t, void*, void*), void (*rel)(void*, void*), void* user) {
+  if (!c || ((alloc == nullptr) != (rel == nullptr))) return VD_E_ARG;
+  if (c->pairs.p || c->sorted.p) { c->lastError = "vd_set_allocator must be called before the first vd_compute"; return VD_E_STATE; }
+  c->allocFn = alloc; c->freeFn = rel; c->allocUser = user;
+  return VD_OK;
+}
+
+vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
+  if (!c || !o) return VD_E_ARG;
+  vd_options d;
+  set_default_options(d);
+  c->opt = *o;
+  if (!(c->opt.grid_density > 0)) c->opt.grid_density = d.grid_density;
+  if (c->opt.real_edges < 0) c->opt.real_edges = d.real_edges;
+  return VD_OK;
+}
+
+vd_status vd_get_counters(const vd_ctx* c, vd_counters* out) {
+  if (!c || !out) return VD_E_ARG;
+  *out = c->counters;
+  return VD_OK;
+}
+
+vd_status vd_get_stage_ms(const vd_ctx* c, double out_ms[5]) {
+  if (!c || !out_ms) return VD_E_ARG;
+  for (int k = 0; k < 5; ++k) out_ms[k] = c->stageMs[k];
+  return VD_OK;
+}
+
+#define VD_COPY(dst, src, bytes)                                                                          \
+  if ((dst) && (bytes) > 0) {                                                                             \
+    const cudaError_t e_ = cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDefault, c->stream);          \
+    if (e_ != cudaSuccess) return cuda_check(c, e_, "vd_cells_to_host");                                  \
+  }
+
+vd_status vd_cells_to_host(vd_ctx* c, double* measure, double* centroid, int64_t* nbr_off, int32_t* nbr, int64_t* piece_off,
+                           int32_t* piece_simplex, double* piece_measure, int64_t* vert_off, double* vert_xyz, int32_t* vert_flags) {
+  if (!c) return VD_E_ARG;
+  if (!c->haveResult) { c->lastError = "vd_cells_to_host before a successful vd_compute"; return VD_E_STATE; }
+  const vd_cells& r = c->cells;
+  VD_COPY(measure, r.measure, sizeof(double) * r.n);
+  VD_COPY(centroid, r.centroid, sizeof(double) * r.n * r.dim);
+  VD_COPY(nbr_off, r.nbr_off, sizeof(int64_t) * (r.n + 1));
+  VD_COPY(nbr, r.nbr, sizeof(int32_t) * r.n_nbrs);
+  VD_COPY(piece_off, r.piece_off, sizeof(int64_t) * (r.n + 1));
+  VD_COPY(piece_simplex, r.piece_simplex, sizeof(int32_t) * r.n_pieces);
+  VD_COPY(piece_measure, r.piece_measure, sizeof(double) * r.n_pieces);
+  VD_COPY(vert_off, r.vert_off, sizeof(int64_t) * (r.n_pieces + 1));
+  VD_COPY(vert_xyz, r.vert_xyz, sizeof(double) * r.n_verts * r.dim);
+  VD_COPY(vert_flags, r.vert_flags, sizeof(int32_t) * r.n_verts * r.nfl);
+  return cuda_check(c, cudaStreamSynchronize(c->stream), "vd_cells_to_host");
+}
+
+vd_status vd_nearest(vd_ctx* c, const double* queries, int64_t nq, int32_t* out_index) {
+  if (!c || !queries || !out_index || nq < 1) return VD_E_ARG;
+  vd_status s;
+  if (!c->indexValid) {
+    if ((s = ensure(c, c->control, sizeof(Control)))) return s;
+    cudaMemsetAsync(c->control.p, 0, sizeof(Control), c->stream);
+    if ((s = stage_index(c))) return s;
+  }
+  DevBuf q3, res;
+  if ((s = upload_points(c, queries, nq, c->dim, q3, "vd_nearest"))) return s;
+  if ((s = ensure(c, res, sizeof(int) * nq))) { release(c, q3); return s; }
+  s = stage_nearest_points(c, q3.as<double>(), nq, res.as<int>());
+  cudaError_t e = cudaMemcpyAsync(out_index, res.p, sizeof(int) * nq, cudaMemcpyDefault, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  release(c, q3);
+  release(c, res);
+  if (s != VD_OK) return s;
+  return cuda_check(c, e, "vd_nearest");
+}
+
+vd_status vd_get_adjacency(vd_ctx* c, int32_t* out) {
+  if (!c || !out) return VD_E_ARG;
+  if (!c->haveDomain) return VD_E_STATE;
+  cudaError_t e = cudaMemcpyAsync(out, c->adj.p, sizeof(int) * c->m * c->nc, cudaMemcpyDefault, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  return cuda_check(c, e, "vd_get_adjacency");
+}
+
+}  // extern "C"

@@ -1,0 +1,160 @@
+// vd_clip.cu -- S3 seeds, S4 clip kernels (one warp per (simplex, site) pair), S5 propagation through
+// the pair list.  Alg. 4 / Alg. 5 lines 15-27 as a wavefront over one growing
+// list: wave k processes the pairs pushed by wave k-1.
+#include "vd_clip2d.cuh"
+#include "vd_clip3d.cuh"
+
+namespace vd {
+
+// S3 (Alg. 2 line 4, for every corner instead of the first; Alg. 4 lines 3-6): the nearest site
+// of a corner of T_a owns that corner, so (T_a, N_p) is a non-empty pair and p is its witness.
+__global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc) {
+  for (int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; a < A.m; a += (int64_t)gridDim.x * blockDim.x) {
+    for (int k = 0; k < nc; ++k) {
+      const int v = A.simp[a * nc + k];
+      const int j = A.vnn[v];
+      if (j < 0 || j >= A.n) continue;
+      push_pair(A, (int)a, j, A.verts[(int64_t)v * 3 + 0], A.verts[(int64_t)v * 3 + 1], A.verts[(int64_t)v * 3 + 2]);
+    }
+  }
+}
+
+constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
+constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
+constexpr int K2 = 32, K2B = 256;
+
+// items: pairs[begin .. end) when list == nullptr, else pairs[list[begin .. end)]
+template <int KIND, bool BIG>
+__global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end) {
+  constexpr int W = BIG ? 1 : kWarpsPerBlock;
+  __shared__ GridIndex g;
+  if (threadIdx.x == 0) g = *A.grid;
+  __syncthreads();
+  const int w = (int)threadIdx.x / kLanes;
+  const int64_t warp = (int64_t)blockIdx.x * W + w;
+  const int64_t nwarps = (int64_t)gridDim.x * W;
+  QueryStats st = {0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u};
+  if constexpr (KIND == KIND_TET_3D) {
+    __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
+    for (int64_t k = begin + warp; k < end; k += nwarps) {
+      const int64_t idx = list ? (int64_t)list[k] : k;
+      const int rc = clip_pair_3d(S[w], g, A, idx, st, lc);
+      if (rc == 1) {
+        if (BIG) {
+          if (lane_id() == 0) {
+            atomicOr(&A.ctl->err, ERR_PIECE_CAP);
+            Piece pc = {};
+            pc.site = A.pairs[idx].i; pc.simplex = A.pairs[idx].a;
+            A.pieces[idx] = pc;
+          }
+        } else if (lane_id() == 0) {
+          const unsigned long long slot = atomicAdd(&A.ctl->ovfTail, 1ull);
+          if ((int64_t)slot < A.ovfCap) A.ovf[slot] = (int)idx; else atomicOr(&A.ctl->err, ERR_PAIR_CAP);
+        }
+      }
+      __syncwarp();
+    }
+  } else {
+    __shared__ Poly2<BIG ? K2B : K2> S[W];
+    for (int64_t k = begin + warp; k < end; k += nwarps) {
+      const int64_t idx = list ? (int64_t)list[k] : k;
+      const int rc = clip_pair_2d(S[w], g, A, idx, st, lc);
+      if (rc == 1) {
+        if (BIG) {
+          if (lane_id() == 0) {
+            atomicOr(&A.ctl->err, ERR_PIECE_CAP);
+            Piece pc = {};
+            pc.site = A.pairs[idx].i; pc.simplex = A.pairs[idx].a;
+            A.pieces[idx] = pc;
+          }
+        } else if (lane_id() == 0) {
+          const unsigned long long slot = atomicAdd(&A.ctl->ovfTail, 1ull);
+          if ((int64_t)slot < A.ovfCap) A.ovf[slot] = (int)idx; else atomicOr(&A.ctl->err, ERR_PAIR_CAP);
+        }
+      }
+      __syncwarp();
+    }
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
+static ClipArgs make_args(vd_ctx* c) {
+  ClipArgs A;
+  A.grid = c->grid.as<GridIndex>();
+  A.sites = c->sites.as<double>();
+  A.verts = c->verts.as<double>();
+  A.simp = c->simp.as<int>();
+  A.adj = c->adj.as<int>();
+  A.vnn = c->vnn.as<int>();
+  A.n = (int)c->n; A.m = (int)c->m; A.kind = c->kind;
+  A.realEdges = c->opt.real_edges; A.stepOut = c->opt.step_out;
+  A.ctl = c->control.as<Control>();
+  A.pairs = c->pairs.as<Pair>();
+  A.pieces = c->pieces.as<Piece>();
+  A.visited = c->visited.as<unsigned long long>();
+  A.hashMask = (uint64_t)c->hashCap - 1;
+  A.pairCap = c->pairCap; A.vertCap = c->vertCap; A.nbrCap = c->nbrCap; A.ovfCap = c->ovfCap;
+  A.ovf = c->ovf.as<int>();
+  A.poolXYZ = c->poolXYZ.as<double>();
+  A.poolFlags = c->poolFlags.as<int>();
+  A.poolNbr = c->poolNbr.as<int>();
+  A.sitePieces = c->sitePieces.as<int>();
+  A.siteNbrRaw = c->siteNbrRaw.as<int>();
+  return A;
+}
+
+static int blocks_for(int64_t items, int perBlock, int cap) {
+  int64_t b = (items + perBlock - 1) / perBlock;
+  if (b > cap) b = cap;
+  if (b < 1) b = 1;
+  return (int)b;
+}
+
+vd_status stage_seed(vd_ctx* c) {
+  vd_status s;
+  cudaStream_t st = c->stream;
+  if ((s = ensure(c, c->vnn, sizeof(int) * c->nv))) return s;
+  // nearest site of every mesh vertex: classifies the corners of every T_a and seeds the pair list
+  if ((s = stage_nearest_points(c, c->verts.as<double>(), c->nv, c->vnn.as<int>()))) return s;
+  cudaMemsetAsync(c->visited.p, 0, sizeof(unsigned long long) * c->hashCap, st);
+  cudaMemsetAsync(c->sitePieces.p, 0, sizeof(int) * c->n, st);
+  cudaMemsetAsync(c->siteNbrRaw.p, 0, sizeof(int) * c->n, st);
+  const ClipArgs A = make_args(c);
+  VD_LAUNCH(k_seed, blocks_for(c->m, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
+  return cuda_check(c, cudaGetLastError(), "seed");
+}
+
+template <int KIND>
+static void launch_wave(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, int64_t ob, int64_t oe) {
+  if (e > b) VD_LAUNCH((k_clip<KIND, false>), blocks_for(e - b, kWarpsPerBlock, 148 * 6), kBlock, 0, c->stream)(A, nullptr, b, e);
+  if (oe > ob) VD_LAUNCH((k_clip<KIND, true>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe);
+}
+
+vd_status stage_clip(vd_ctx* c) {
+  const ClipArgs A = make_args(c);
+  cudaStream_t st = c->stream;
+  int64_t begin = 0, obegin = 0;
+  int64_t waves = 0;
+  Control h;
+  for (;;) {
+    cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_check(c, e, "clip wave");
+    if (h.err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) break;   // caller grows the pools and reruns
+    int64_t end = (int64_t)h.pairTail, oend = (int64_t)h.ovfTail;
+    if (end > c->pairCap) end = c->pairCap;
+    if (oend > c->ovfCap) oend = c->ovfCap;
+    if (end == begin && oend == obegin) break;   // "while L1 is not empty"
+    if (c->kind == KIND_TET_3D) launch_wave<KIND_TET_3D>(c, A, begin, end, obegin, oend);
+    else launch_wave<KIND_TRI_2D>(c, A, begin, end, obegin, oend);
+    begin = end;
+    obegin = oend;
+    ++waves;
+  }
+  c->hostControl = h;
+  c->counters.waves = waves;
+  return cuda_check(c, cudaGetLastError(), "clip");
+}
+
+}  // namespace vd

@@ -1,0 +1,274 @@
+// vd_clip2d.cuh -- S4 for triangles (2D domains and surface meshes): one warp computes the
+// polygon P_{a,i} = T_a ∩ Omega_i.  The polygon is an ordered loop of corners, edge c runs from corner
+// c to corner c+1 and carries a flag and its supporting plane (for a surface: the bisector plane,
+// or the plane through a triangle edge perpendicular to the triangle).  Every corner is the solution
+// of (edge plane, edge plane, triangle plane), so coordinates do not depend on the clip order.
+// The nearest-site queries are warp-cooperative; the few-corner loop surgery is done by lane 0.
+#pragma once
+#include "vd_clip3d.cuh"
+
+namespace vd {
+
+template <int K>
+struct Poly2 {
+  double cx[K], cy[K], cz[K];
+  double enx[K], eny[K], enz[K], ed[K];
+  int eflag[K], cnn[K];
+  unsigned char cstate[K];
+  // scratch copy used while rebuilding the loop
+  double tx[K], ty[K], tz[K], tnx[K], tny[K], tnz[K], td[K];
+  int tflag[K], tnn[K];
+  unsigned char tstate[K];
+  int nc;
+};
+
+template <int K>
+__device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+  const int lane = lane_id();
+  const Pair pr = A.pairs[pairIdx];
+  const int a = pr.a, i = pr.i;
+  int tv[3];
+  double tx[3], ty[3], tz[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    tv[k] = __ldg(&A.simp[(int64_t)a * 3 + k]);
+    tx[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 0]);
+    ty[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 1]);
+    tz[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 2]);
+  }
+  const double ox = tx[0], oy = ty[0], oz = tz[0];
+  const double six = __ldg(&A.sites[(int64_t)i * 3 + 0]), siy = __ldg(&A.sites[(int64_t)i * 3 + 1]),
+               siz = __ldg(&A.sites[(int64_t)i * 3 + 2]);
+  const double vix = six - ox, viy = siy - oy, viz = siz - oz;
+  const double wx = pr.wx - ox, wy = pr.wy - oy, wz = pr.wz - oz;
+  // triangle plane (local): unit normal, offset 0 (corner 0 is the origin)
+  double pnx, pny, pnz;
+  {
+    const double ax = tx[1] - ox, ay = ty[1] - oy, az = tz[1] - oz, bx = tx[2] - ox, by = ty[2] - oy, bz = tz[2] - oz;
+    pnx = ay * bz - az * by; pny = az * bx - ax * bz; pnz = ax * by - ay * bx;
+    const double inv = 1.0 / sqrt(pnx * pnx + pny * pny + pnz * pnz);
+    pnx *= inv; pny *= inv; pnz *= inv;
+  }
+  // ---- P <- T: corner k = vertex k, edge k = (k -> k+1) lies opposite vertex k+2
+  if (lane < 3) {
+    const int k = lane, k1 = (k + 1) % 3, k2 = (k + 2) % 3;
+    S.cx[k] = tx[k] - ox; S.cy[k] = ty[k] - oy; S.cz[k] = tz[k] - oz;
+    const double ex = tx[k1] - tx[k], ey = ty[k1] - ty[k], ez = tz[k1] - tz[k];
+    double nx = ey * pnz - ez * pny, ny = ez * pnx - ex * pnz, nz = ex * pny - ey * pnx;   // e x n
+    const double side = nx * (tx[k2] - tx[k]) + ny * (ty[k2] - ty[k]) + nz * (tz[k2] - tz[k]);
+    if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
+    S.enx[k] = nx; S.eny[k] = ny; S.enz[k] = nz;
+    S.ed[k] = nx * (tx[k] - ox) + ny * (ty[k] - oy) + nz * (tz[k] - oz);
+    S.eflag[k] = ~__ldg(&A.adj[(int64_t)a * 3 + k2]);
+    const int nn = __ldg(&A.vnn[tv[k]]);
+    S.cnn[k] = nn;
+    S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
+  }
+  if (lane == 0) S.nc = 3;
+  __syncwarp();
+  bool failed = false;
+#ifdef VD_TRACE
+  {
+    double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0u, 0u};
+    nearest(g, pr.wx, pr.wy, pr.wz, b, bi, s2);
+    const double dx = pr.wx - six, dy = pr.wy - siy, dz = pr.wz - siz;
+    const double di = dx * dx + dy * dy + dz * dz;
+    if (lane == 0 && bi != i && di - b > 1e-13) printf("BAD WITNESS pair(%d,%d) w=(%g,%g) nearest=%d di2=%g best=%g\n", a, i, pr.wx, pr.wy, bi, di, b);
+  }
+#endif
+  for (int guard = 0; guard < 4 * K; ++guard) {
+    const int nc = S.nc;
+    // point-in-cell tests of unclassified corners (section IV-A)
+    for (int c = 0; c < nc; ++c) {
+      if (S.cstate[c] != ST_UNKNOWN) continue;
+      const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
+      const double dx = qx - six, dy = qy - siy, dz = qz - siz;
+      double best = dx * dx + dy * dy + dz * dz;
+      int bestId = i;
+      nearest(g, qx, qy, qz, best, bestId, st);
+      bool inside = bestId == i;
+      if (!inside) {
+        bool own = false;
+        for (int f = lane; f < nc; f += kLanes) own |= (S.eflag[f] == bestId);
+        inside = __any_sync(kFull, own);   // flag rule (reading U6)
+      }
+      __syncwarp();
+      if (lane == 0) { S.cstate[c] = inside ? ST_IN : ST_OUT; S.cnn[c] = bestId; }
+#ifdef VD_TRACE
+      if (lane == 0) printf("pair(%d,%d) classify c=%d q=(%g,%g) best=%g id=%d inside=%d\n", a, i, c, qx, qy, best, bestId, (int)inside);
+#endif
+      __syncwarp();
+    }
+    // select the outside corner p and, if possible, a neighbour p_s in Omega_i (real edge)
+    int p = -1, s = -1;
+    for (int c = 0; c < nc; ++c) {
+      if (S.cstate[c] != ST_OUT) continue;
+      if (p < 0) p = c;
+      if (A.realEdges) {
+        const int pv = (c + nc - 1) % nc, nx = (c + 1) % nc;
+        if (S.cstate[pv] == ST_IN) { p = c; s = pv; break; }
+        if (S.cstate[nx] == ST_IN) { p = c; s = nx; break; }
+      }
+    }
+    if (p < 0) break;
+    double psx = wx, psy = wy, psz = wz;
+    if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
+    double nx, ny, nz, d;
+    const int j = find_bisector(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
+                                nx, ny, nz, d, st, lc);
+    if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
+    bool own = false;
+    for (int c = 0; c < nc; ++c) own |= (S.eflag[c] == j);
+    if (own) {
+      __syncwarp();
+      if (lane == 0) S.cstate[p] = ST_IN;
+      __syncwarp();
+      continue;
+    }
+#ifdef VD_TRACE
+    if (lane == 0) printf("pair(%d,%d) clip p=%d s=%d j=%d nc=%d\n", a, i, p, s, j, nc);
+#endif
+    lc.clips += 1;
+    __syncwarp();
+    int rc = 0;
+    if (lane == 0) {
+      // outside run around p (P:L391's R_p for a loop): corners beyond the line, not known inside
+      int r0 = p, r1 = p, len = 1;
+      while (len < nc) {
+        const int q = (r0 + nc - 1) % nc;
+        const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
+        if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
+        r0 = q; ++len;
+      }
+      while (len < nc) {
+        const int q = (r1 + 1) % nc;
+        const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
+        if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
+        r1 = q; ++len;
+      }
+      if (len >= nc) {
+        S.nc = 0;
+      } else if (nc - len + 2 > K) {
+        rc = 1;
+      } else {
+        const int pv = (r0 + nc - 1) % nc, nxt = (r1 + 1) % nc;
+        int k = 0;
+        for (int c = nxt;; c = (c + 1) % nc) {   // survivors nxt .. pv keep corner and edge
+          S.tx[k] = S.cx[c]; S.ty[k] = S.cy[c]; S.tz[k] = S.cz[c];
+          S.tnx[k] = S.enx[c]; S.tny[k] = S.eny[c]; S.tnz[k] = S.enz[c]; S.td[k] = S.ed[c];
+          S.tflag[k] = S.eflag[c]; S.tnn[k] = S.cnn[c]; S.tstate[k] = S.cstate[c];
+          ++k;
+          if (c == pv) break;
+        }
+        // X = edge(pv) ∩ B_ij : start of the new edge, which takes flag j
+        solve3(S.enx[pv], S.eny[pv], S.enz[pv], S.ed[pv], nx, ny, nz, d, pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]);
+        S.tnx[k] = nx; S.tny[k] = ny; S.tnz[k] = nz; S.td[k] = d; S.tflag[k] = j; S.tnn[k] = -1;
+        S.tstate[k] = (s == pv && p == r0) ? ST_IN : ST_UNKNOWN;   // on the searched real edge
+        ++k;
+        // E = B_ij ∩ edge(r1) : the rest of edge r1 keeps its plane and flag
+        solve3(nx, ny, nz, d, S.enx[r1], S.eny[r1], S.enz[r1], S.ed[r1], pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]);
+        S.tnx[k] = S.enx[r1]; S.tny[k] = S.eny[r1]; S.tnz[k] = S.enz[r1]; S.td[k] = S.ed[r1];
+        S.tflag[k] = S.eflag[r1]; S.tnn[k] = -1;
+        S.tstate[k] = (s == nxt && p == r1) ? ST_IN : ST_UNKNOWN;
+        ++k;
+        for (int c = 0; c < k; ++c) {
+          S.cx[c] = S.tx[c]; S.cy[c] = S.ty[c]; S.cz[c] = S.tz[c];
+          S.enx[c] = S.tnx[c]; S.eny[c] = S.tny[c]; S.enz[c] = S.tnz[c]; S.ed[c] = S.td[c];
+          S.eflag[c] = S.tflag[c]; S.cnn[c] = S.tnn[c]; S.cstate[c] = S.tstate[c];
+        }
+        S.nc = k;
+      }
+    }
+#ifdef VD_TRACE
+    if (lane == 0) { printf("   loop:"); for (int c = 0; c < S.nc; ++c) printf(" (%.4f,%.4f|f%d|s%d)", S.cx[c]+ox, S.cy[c]+oy, S.eflag[c], (int)S.cstate[c]); printf("\n"); }
+#endif
+    rc = shfl(rc, 0);
+    __syncwarp();
+    if (rc) return 1;
+    if (S.nc == 0) break;
+  }
+  // ---- finish
+  const int nc = S.nc;
+  Piece pc;
+  pc.site = i; pc.simplex = a; pc.nverts = 0; pc.nnbr = 0; pc.vbase = 0; pc.nbase = 0;
+  pc.measure = 0; pc.mx = pc.my = pc.mz = 0;
+  lc.pairs += 1;
+  if (failed || nc < 3) {
+    if (lane == 0) A.pieces[pairIdx] = pc;
+    return 0;
+  }
+  // area and first moment: fan from corner 0, signed along the triangle's unit normal
+  double area = 0, mx = 0, my = 0, mz = 0;
+  for (int c = 1; c + 1 < nc; ++c) {
+    const double ux = S.cx[c] - S.cx[0], uy = S.cy[c] - S.cy[0], uz = S.cz[c] - S.cz[0];
+    const double vx = S.cx[c + 1] - S.cx[0], vy = S.cy[c + 1] - S.cy[0], vz = S.cz[c + 1] - S.cz[0];
+    const double ar = 0.5 * ((uy * vz - uz * vy) * pnx + (uz * vx - ux * vz) * pny + (ux * vy - uy * vx) * pnz);
+    area += ar;
+    mx += ar * (S.cx[0] + (ux + vx) * (1.0 / 3.0));
+    my += ar * (S.cy[0] + (uy + vy) * (1.0 / 3.0));
+    mz += ar * (S.cz[0] + (uz + vz) * (1.0 / 3.0));
+  }
+  if (area < 0) { area = -area; mx = -mx; my = -my; mz = -mz; }
+  if (!(area > 0)) {
+    if (lane == 0) A.pieces[pairIdx] = pc;
+    return 0;
+  }
+  int nnbr = 0;
+  for (int c = 0; c < nc; ++c) nnbr += S.eflag[c] >= 0 ? 1 : 0;
+  unsigned long long nb0 = 0, vb0 = 0;
+  if (lane == 0) {
+    nb0 = atomicAdd(&A.ctl->nbrTail, (unsigned long long)nnbr);
+    vb0 = atomicAdd(&A.ctl->vertTail, (unsigned long long)nc);
+  }
+  nb0 = shfl(nb0, 0);
+  vb0 = shfl(vb0, 0);
+  if ((int64_t)(nb0 + nnbr) > A.nbrCap || (int64_t)(vb0 + nc) > A.vertCap) {
+    if (lane == 0) {
+      atomicOr(&A.ctl->err, (int64_t)(vb0 + nc) > A.vertCap ? ERR_VERT_CAP : ERR_NBR_CAP);
+      A.pieces[pairIdx] = pc;
+    }
+    return 0;
+  }
+  if (lane == 0) {
+    int k = 0;
+    for (int c = 0; c < nc; ++c) {
+      if (S.eflag[c] < 0) continue;
+      A.poolNbr[nb0 + k++] = S.eflag[c];
+      const int c1 = (c + 1) % nc;
+      // witness: the edge midpoint lies in T_a ∩ Omega_i ∩ Omega_j
+      push_pair(A, a, S.eflag[c], 0.5 * (S.cx[c] + S.cx[c1]) + ox, 0.5 * (S.cy[c] + S.cy[c1]) + oy,
+                0.5 * (S.cz[c] + S.cz[c1]) + oz);
+    }
+  }
+  // corners with their two edge flags, ascending; ranked lexicographically
+  for (int c = lane; c < nc; c += kLanes) {
+    int f0 = S.eflag[(c + nc - 1) % nc], f1 = S.eflag[c];
+    if (f0 > f1) { const int t = f0; f0 = f1; f1 = t; }
+    S.tflag[c] = f0; S.tnn[c] = f1;
+  }
+  __syncwarp();
+  for (int c = lane; c < nc; c += kLanes) {
+    const int k0 = S.tflag[c], k1 = S.tnn[c];
+    int rank = 0;
+    for (int o = 0; o < nc; ++o) {
+      const int o0 = S.tflag[o], o1 = S.tnn[o];
+      rank += (o0 < k0 || (o0 == k0 && (o1 < k1 || (o1 == k1 && o < c)))) ? 1 : 0;
+    }
+    const int64_t v = (int64_t)vb0 + rank;
+    A.poolXYZ[v * 3 + 0] = S.cx[c] + ox; A.poolXYZ[v * 3 + 1] = S.cy[c] + oy; A.poolXYZ[v * 3 + 2] = S.cz[c] + oz;
+    A.poolFlags[v * 2 + 0] = k0; A.poolFlags[v * 2 + 1] = k1;
+  }
+  if (lane == 0) {
+    pc.nverts = nc; pc.nnbr = nnbr; pc.vbase = (int64_t)vb0; pc.nbase = (int64_t)nb0;
+    pc.measure = area;
+    pc.mx = mx + area * ox; pc.my = my + area * oy; pc.mz = mz + area * oz;
+    A.pieces[pairIdx] = pc;
+    atomicAdd(&A.sitePieces[i], 1);
+    atomicAdd(&A.siteNbrRaw[i], nnbr);
+  }
+  lc.pieces += 1;
+  __syncwarp();
+  return 0;
+}
+
+}  // namespace vd

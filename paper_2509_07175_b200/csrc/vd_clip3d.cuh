@@ -1,0 +1,414 @@
+// vd_clip3d.cuh -- S4 for tetrahedra: one warp computes P_{a,i} = T_a ∩ Omega_i by Alg. 3
+// / Alg. 1 on the cell structure of section VI-C: an array of planes and an
+// array of corners, each corner the intersection of three planes = a triangle of the dual mesh.
+#pragma once
+#include "vd_clip_args.cuh"
+
+namespace vd {
+
+template <int P, int C>
+struct Poly3 {
+  double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
+  int pflag[P];                           // flag of plane f
+  double cx[C], cy[C], cz[C];             // corner coordinates (local)
+  int cnn[C];                             // nearest site of an outside corner
+  int key[C][3];                          // scratch: ascending flag triple of a corner (output order)
+  unsigned short cp[C][3];                // the corner's three planes, cyclically ordered
+  unsigned short cadj[C][3];              // corner across the polytope edge (cp[t], cp[t+1])
+  unsigned short remap[C];                // scratch: index of a surviving corner after the clip
+  unsigned short pa[P], pb[P];            // scratch: new corner whose rim edge starts / ends at a plane
+  unsigned short be[P][4];                // rim edges of R_p: (a, b, inside neighbour, flags)
+  unsigned char cstate[C], cmark[C];
+};
+
+__device__ __forceinline__ void solve3(double ax, double ay, double az, double ad, double bx, double by, double bz, double bd,
+                                       double cx, double cy, double cz, double cd, double& x, double& y, double& z) {
+  // Cramer: x = (ad (b x c) + bd (c x a) + cd (a x b)) / det[a, b, c]
+  const double bcx = by * cz - bz * cy, bcy = bz * cx - bx * cz, bcz = bx * cy - by * cx;
+  const double cax = cy * az - cz * ay, cay = cz * ax - cx * az, caz = cx * ay - cy * ax;
+  const double abx = ay * bz - az * by, aby = az * bx - ax * bz, abz = ax * by - ay * bx;
+  const double det = ax * bcx + ay * bcy + az * bcz;
+  const double inv = 1.0 / det;
+  x = (ad * bcx + bd * cax + cd * abx) * inv;
+  y = (ad * bcy + bd * cay + cd * aby) * inv;
+  z = (ad * bcz + bd * caz + cd * abz) * inv;
+}
+
+// P <- P clipped by the half-space n.x <= d with flag j (Alg. 3 line 4), steps of P:L389: (1) the
+// corners outside the plane, restricted to the connected component R_p that contains the known-outside
+// corner p; (2) the rim of R_p; (3) R_p removed, one new corner per rim edge.
+// np, nc are updated.  Returns 0 ok, 1 capacity, 2 the rim is not a simple loop.
+template <int P, int C>
+__device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, double nx, double ny, double nz, double d, int j) {
+  const int lane = lane_id();
+  const int N = np;   // index of the new plane
+  // (1) candidates: strictly outside the plane and not known to be in Omega_i; p itself always
+  for (int c = lane; c < nc; c += kLanes) {
+    const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+    const bool cand = (c == p) || (sd > 0.0 && S.cstate[c] != ST_IN);
+    S.cmark[c] = (c == p) ? 2 : (cand ? 1 : 0);   // 2 = in R_p, 1 = candidate, 0 = stays
+  }
+  if (lane == 0) {
+    S.pnx[N] = nx; S.pny[N] = ny; S.pnz[N] = nz; S.pd[N] = d; S.pflag[N] = j;
+  }
+  __syncwarp();
+  for (int it = 0; it < C; ++it) {   // flood over polytope edges
+    bool grew = false;
+    for (int c = lane; c < nc; c += kLanes) {
+      if (S.cmark[c] == 1 && (S.cmark[S.cadj[c][0]] == 2 || S.cmark[S.cadj[c][1]] == 2 || S.cmark[S.cadj[c][2]] == 2)) {
+        S.cmark[c] = 2;
+        grew = true;
+      }
+    }
+    __syncwarp();
+    if (!__any_sync(kFull, grew)) break;
+  }
+  // (2) rim edges: edge (cp[t], cp[t+1]) of a removed corner whose neighbour across it stays
+  int L = 0, nRemoved = 0;
+  for (int c0 = 0; c0 < nc; c0 += kLanes) {
+    const int c = c0 + lane;
+    const bool rem = c < nc && S.cmark[c] == 2;
+    int cnt = 0;
+    unsigned short ea[3], eb[3], en[3];
+    if (rem) {
+#pragma unroll
+      for (int t = 0; t < 3; ++t) {
+        const int nb = S.cadj[c][t];
+        if (S.cmark[nb] != 2) { ea[cnt] = S.cp[c][t]; eb[cnt] = S.cp[c][(t + 1) % 3]; en[cnt] = (unsigned short)nb; ++cnt; }
+      }
+    }
+    int incl = cnt;
+#pragma unroll
+    for (int off = 1; off < kLanes; off <<= 1) {
+      const int o = __shfl_up_sync(kFull, incl, off);
+      if (lane >= off) incl += o;
+    }
+    const int base = L + incl - cnt;
+    const int tot = shfl(incl, kLanes - 1);
+    if (L + tot > P) return 1;
+    for (int k = 0; k < cnt; ++k) {
+      S.be[base + k][0] = ea[k]; S.be[base + k][1] = eb[k]; S.be[base + k][2] = en[k];
+      S.be[base + k][3] = (unsigned short)((c == p && (int)en[k] == s) ? 1 : 0);
+      // the surviving neighbour's slot that pointed at c will point at the new corner
+#pragma unroll
+      for (int t = 0; t < 3; ++t)
+        if (S.cadj[en[k]][t] == c) S.cadj[en[k]][t] = (unsigned short)(0x8000 | (base + k));
+    }
+    L += tot;
+    nRemoved += __popc(__ballot_sync(kFull, rem));
+  }
+  __syncwarp();
+  const int nSurv = nc - nRemoved;
+  if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
+  if (nSurv + L > C) return 1;
+  // (3a) compact the surviving corners to the front
+  int run = 0;
+  for (int c0 = 0; c0 < nc; c0 += kLanes) {
+    const int c = c0 + lane;
+    const bool keep = c < nc && S.cmark[c] != 2;
+    const unsigned m = __ballot_sync(kFull, keep);
+    if (keep) S.remap[c] = (unsigned short)(run + __popc(m & ((1u << lane) - 1u)));
+    run += __popc(m);
+  }
+  __syncwarp();
+  for (int c0 = 0; c0 < nc; c0 += kLanes) {
+    const int c = c0 + lane;
+    const bool keep = c < nc && S.cmark[c] != 2;
+    double x = 0, y = 0, z = 0;
+    int nn = 0, st = 0;
+    unsigned short cp0 = 0, cp1 = 0, cp2 = 0, a0 = 0, a1 = 0, a2 = 0;
+    if (keep) {
+      x = S.cx[c]; y = S.cy[c]; z = S.cz[c]; nn = S.cnn[c]; st = S.cstate[c];
+      cp0 = S.cp[c][0]; cp1 = S.cp[c][1]; cp2 = S.cp[c][2];
+      a0 = S.cadj[c][0]; a1 = S.cadj[c][1]; a2 = S.cadj[c][2];
+      a0 = (a0 & 0x8000) ? (unsigned short)(nSurv + (a0 & 0x7fff)) : S.remap[a0];
+      a1 = (a1 & 0x8000) ? (unsigned short)(nSurv + (a1 & 0x7fff)) : S.remap[a1];
+      a2 = (a2 & 0x8000) ? (unsigned short)(nSurv + (a2 & 0x7fff)) : S.remap[a2];
+    }
+    __syncwarp();
+    if (keep) {
+      const int t = S.remap[c];
+      S.cx[t] = x; S.cy[t] = y; S.cz[t] = z; S.cnn[t] = nn; S.cstate[t] = (unsigned char)st;
+      S.cp[t][0] = cp0; S.cp[t][1] = cp1; S.cp[t][2] = cp2;
+      S.cadj[t][0] = a0; S.cadj[t][1] = a1; S.cadj[t][2] = a2;
+    }
+    __syncwarp();
+  }
+  // (3b) new corners: rim edge (a -> b) becomes the corner (a, b, N)
+  for (int f = lane; f <= N; f += kLanes) { S.pa[f] = 0xffff; S.pb[f] = 0xffff; }
+  __syncwarp();
+  bool bad = false;
+  for (int e = lane; e < L; e += kLanes) {
+    const int ea = S.be[e][0], eb = S.be[e][1];
+    if (S.pa[ea] != 0xffff || S.pb[eb] != 0xffff) bad = true;   // (racy duplicates are caught below)
+    S.pa[ea] = (unsigned short)(nSurv + e);
+    S.pb[eb] = (unsigned short)(nSurv + e);
+  }
+  __syncwarp();
+  for (int e = lane; e < L; e += kLanes) {
+    const int t = nSurv + e;
+    const int ea = S.be[e][0], eb = S.be[e][1];
+    S.cp[t][0] = (unsigned short)ea; S.cp[t][1] = (unsigned short)eb; S.cp[t][2] = (unsigned short)N;
+    S.cadj[t][0] = S.remap[S.be[e][2]];
+    const int nxt = S.pa[eb];   // edge (b -> N) is shared with the corner whose rim edge starts at b
+    const int prv = S.pb[ea];   // edge (N -> a) with the corner whose rim edge ends at a
+    if (nxt == 0xffff || prv == 0xffff || S.pa[ea] != t || S.pb[eb] != t) bad = true;
+    S.cadj[t][1] = (unsigned short)nxt;
+    S.cadj[t][2] = (unsigned short)prv;
+    double x, y, z;
+    solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
+    S.cx[t] = x; S.cy[t] = y; S.cz[t] = z;
+    S.cnn[t] = -1;
+    // the new corner on the searched real edge p_s p is in Omega_i ∩ Omega_j
+    S.cstate[t] = S.be[e][3] ? ST_IN : ST_UNKNOWN;
+  }
+  __syncwarp();
+  nc = nSurv + L;
+  np = N + 1;
+  return __any_sync(kFull, bad) ? 2 : 0;
+}
+
+// Record the finished piece: measure and first moment (fan tetrahedra over every face, S6 input),
+// corners with their flag triples in canonical order, face flags, and the propagation of P:L266-273.
+template <int P, int C>
+__device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairIdx, int a, int i, int np, int nc, double ox,
+                               double oy, double oz, bool failed, LocalCnt& lc) {
+  const int lane = lane_id();
+  Piece pc;
+  pc.site = i; pc.simplex = a; pc.nverts = 0; pc.nnbr = 0; pc.vbase = 0; pc.nbase = 0;
+  pc.measure = 0; pc.mx = pc.my = pc.mz = 0;
+  lc.pairs += 1;
+  if (failed || nc < 4) {
+    if (lane == 0) A.pieces[pairIdx] = pc;
+    return 0;
+  }
+  // one corner of every live plane (a plane is live iff some corner lies on it)
+  for (int f = lane; f < np; f += kLanes) S.pa[f] = 0xffff;
+  __syncwarp();
+  for (int c = lane; c < nc; c += kLanes) {
+    S.pa[S.cp[c][0]] = (unsigned short)c; S.pa[S.cp[c][1]] = (unsigned short)c; S.pa[S.cp[c][2]] = (unsigned short)c;
+  }
+  __syncwarp();
+  const double rx = S.cx[0], ry = S.cy[0], rz = S.cz[0];   // reference point of the fan: corner 0
+  double vol = 0, mx = 0, my = 0, mz = 0;
+  int nnbr = 0;
+  for (int f0 = 0; f0 < np; f0 += kLanes) {
+    const int f = f0 + lane;
+    const bool live = f < np && S.pa[f] != 0xffff;
+    double fx = 0, fy = 0, fz = 0;
+    int fk = 0;
+    if (live) {
+      // walk the face loop: from a corner, the edge that starts at plane f leads to the next corner
+      const int c0 = S.pa[f];
+      const double ux = S.cx[c0] - rx, uy = S.cy[c0] - ry, uz = S.cz[c0] - rz;
+      fx = S.cx[c0]; fy = S.cy[c0]; fz = S.cz[c0]; fk = 1;
+      int c = c0;
+      double vx = 0, vy = 0, vz = 0;
+      for (int step = 0; step < nc; ++step) {
+        const int t = (S.cp[c][0] == f) ? 0 : ((S.cp[c][1] == f) ? 1 : 2);
+        c = S.cadj[c][t];
+        if (c == c0) break;
+        const double wx = S.cx[c] - rx, wy = S.cy[c] - ry, wz = S.cz[c] - rz;
+        fx += S.cx[c]; fy += S.cy[c]; fz += S.cz[c]; ++fk;
+        if (step > 0) {
+          const double tv = (ux * (vy * wz - vz * wy) + uy * (vz * wx - vx * wz) + uz * (vx * wy - vy * wx)) * (1.0 / 6.0);
+          vol += tv;
+          mx += tv * (rx + 0.25 * (ux + vx + wx));
+          my += tv * (ry + 0.25 * (uy + vy + wy));
+          mz += tv * (rz + 0.25 * (uz + vz + wz));
+        }
+        vx = wx; vy = wy; vz = wz;
+      }
+    }
+    const bool pos = live && S.pflag[f] >= 0;
+    const unsigned pm = __ballot_sync(kFull, pos);
+    // the face flags travel in key[][] (free until the corners are ranked): flag, then witness
+    if (pos) {
+      const int slot = nnbr + __popc(pm & ((1u << lane) - 1u));
+      if (slot < C) {
+        S.key[slot][0] = S.pflag[f];
+        const double inv = 1.0 / fk;
+        // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
+        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz);
+      }
+    }
+    nnbr += __popc(pm);
+  }
+  vol = warp_sum(vol); mx = warp_sum(mx); my = warp_sum(my); mz = warp_sum(mz);
+  if (vol < 0) { vol = -vol; mx = -mx; my = -my; mz = -mz; }
+  if (!(vol > 0)) {
+    if (lane == 0) A.pieces[pairIdx] = pc;
+    return 0;
+  }
+  if (nnbr > C) nnbr = C;
+  // face flags -> pool
+  unsigned long long nb0 = 0;
+  if (lane == 0) nb0 = atomicAdd(&A.ctl->nbrTail, (unsigned long long)nnbr);
+  nb0 = shfl(nb0, 0);
+  unsigned long long vb0 = 0;
+  if (lane == 0) vb0 = atomicAdd(&A.ctl->vertTail, (unsigned long long)nc);
+  vb0 = shfl(vb0, 0);
+  if ((int64_t)(nb0 + nnbr) > A.nbrCap || (int64_t)(vb0 + nc) > A.vertCap) {
+    if (lane == 0) {
+      atomicOr(&A.ctl->err, (int64_t)(vb0 + nc) > A.vertCap ? ERR_VERT_CAP : ERR_NBR_CAP);
+      A.pieces[pairIdx] = pc;
+    }
+    return 0;
+  }
+  for (int k = lane; k < nnbr; k += kLanes) A.poolNbr[nb0 + k] = S.key[k][0];
+  __syncwarp();
+  // corners: ascending flag triple, corners ranked lexicographically by it
+  for (int c = lane; c < nc; c += kLanes) {
+    int f0 = S.pflag[S.cp[c][0]], f1 = S.pflag[S.cp[c][1]], f2 = S.pflag[S.cp[c][2]];
+    int t;
+    if (f0 > f1) { t = f0; f0 = f1; f1 = t; }
+    if (f1 > f2) { t = f1; f1 = f2; f2 = t; }
+    if (f0 > f1) { t = f0; f0 = f1; f1 = t; }
+    S.key[c][0] = f0; S.key[c][1] = f1; S.key[c][2] = f2;
+  }
+  __syncwarp();
+  for (int c = lane; c < nc; c += kLanes) {
+    const int k0 = S.key[c][0], k1 = S.key[c][1], k2 = S.key[c][2];
+    int rank = 0;
+    for (int o = 0; o < nc; ++o) {
+      const int o0 = S.key[o][0], o1 = S.key[o][1], o2 = S.key[o][2];
+      const bool less = o0 < k0 || (o0 == k0 && (o1 < k1 || (o1 == k1 && (o2 < k2 || (o2 == k2 && o < c)))));
+      rank += less ? 1 : 0;
+    }
+    const int64_t v = (int64_t)vb0 + rank;
+    A.poolXYZ[v * 3 + 0] = S.cx[c] + ox; A.poolXYZ[v * 3 + 1] = S.cy[c] + oy; A.poolXYZ[v * 3 + 2] = S.cz[c] + oz;
+    A.poolFlags[v * 3 + 0] = k0; A.poolFlags[v * 3 + 1] = k1; A.poolFlags[v * 3 + 2] = k2;
+  }
+  if (lane == 0) {
+    pc.nverts = nc; pc.nnbr = nnbr; pc.vbase = (int64_t)vb0; pc.nbase = (int64_t)nb0;
+    pc.measure = vol;
+    pc.mx = mx + vol * ox; pc.my = my + vol * oy; pc.mz = mz + vol * oz;
+    A.pieces[pairIdx] = pc;
+    atomicAdd(&A.sitePieces[i], 1);
+    atomicAdd(&A.siteNbrRaw[i], nnbr);
+  }
+  lc.pieces += 1;
+  return 0;
+}
+
+// returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
+template <int P, int C>
+__device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+  const int lane = lane_id();
+  const Pair pr = A.pairs[pairIdx];
+  const int a = pr.a, i = pr.i;
+  int tv[4];
+  double tx[4], ty[4], tz[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    tv[k] = __ldg(&A.simp[(int64_t)a * 4 + k]);
+    tx[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 0]);
+    ty[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 1]);
+    tz[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 2]);
+  }
+  const double ox = tx[0], oy = ty[0], oz = tz[0];
+  const double six = __ldg(&A.sites[(int64_t)i * 3 + 0]), siy = __ldg(&A.sites[(int64_t)i * 3 + 1]),
+               siz = __ldg(&A.sites[(int64_t)i * 3 + 2]);
+  const double vix = six - ox, viy = siy - oy, viz = siz - oz;
+  const double wx = pr.wx - ox, wy = pr.wy - oy, wz = pr.wz - oz;
+
+  // ---- P <- T (Alg. 3 line 1): 4 planes (flags from the simplex adjacency), 4 corners
+  if (lane < 4) {
+    const int k = lane;
+    const int q0 = (k + 1) & 3, q1 = (k + 2) & 3, q2 = (k + 3) & 3;
+    const double ax = tx[q1] - tx[q0], ay = ty[q1] - ty[q0], az = tz[q1] - tz[q0];
+    const double bx = tx[q2] - tx[q0], by = ty[q2] - ty[q0], bz = tz[q2] - tz[q0];
+    double nx = ay * bz - az * by, ny = az * bx - ax * bz, nz = ax * by - ay * bx;
+    const double side = nx * (tx[k] - tx[q0]) + ny * (ty[k] - ty[q0]) + nz * (tz[k] - tz[q0]);
+    if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
+    S.pnx[k] = nx; S.pny[k] = ny; S.pnz[k] = nz;
+    S.pd[k] = nx * (tx[q0] - ox) + ny * (ty[q0] - oy) + nz * (tz[q0] - oz);
+    S.pflag[k] = ~__ldg(&A.adj[(int64_t)a * 4 + k]);
+    // corner k = tet vertex k = the three faces other than k, in the cyclic order of DESIGN.md
+    const int tri[4][3] = {{1, 3, 2}, {0, 2, 3}, {0, 3, 1}, {0, 1, 2}};
+    S.cx[k] = tx[k] - ox; S.cy[k] = ty[k] - oy; S.cz[k] = tz[k] - oz;
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+      S.cp[k][t] = (unsigned short)tri[k][t];
+      S.cadj[k][t] = (unsigned short)(6 - k - tri[k][t] - tri[k][(t + 1) % 3]);
+    }
+    // corners of T are classified from the per-vertex nearest site (S3): in Omega_i iff N_p = v_i
+    const int nn = __ldg(&A.vnn[tv[k]]);
+    S.cnn[k] = nn;
+    S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
+  }
+  __syncwarp();
+  int np = 4, nc = 4;
+  bool failed = false;
+
+  // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
+  for (int guard = 0; guard < 4 * P + 16; ++guard) {
+    // point-in-cell tests of the unclassified corners (section IV-A)
+    for (int c0 = 0; c0 < nc; c0 += kLanes) {
+      const int c = c0 + lane;
+      unsigned um = __ballot_sync(kFull, c < nc && S.cstate[c] == ST_UNKNOWN);
+      while (um) {
+        const int cc = c0 + __ffs(um) - 1;
+        um &= um - 1;
+        const double qx = S.cx[cc] + ox, qy = S.cy[cc] + oy, qz = S.cz[cc] + oz;
+        const double dx = qx - six, dy = qy - siy, dz = qz - siz;
+        double best = dx * dx + dy * dy + dz * dz;
+        int bestId = i;
+        nearest(g, qx, qy, qz, best, bestId, st);
+        bool inside = bestId == i;
+        if (!inside) {
+          // flag rule in the form of reading U6: N_q already owns a plane of P
+          bool own = false;
+          for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == bestId);
+          inside = __any_sync(kFull, own);
+        }
+        if (lane == 0) {
+          S.cstate[cc] = inside ? ST_IN : ST_OUT;
+          S.cnn[cc] = bestId;
+        }
+      }
+    }
+    __syncwarp();
+    // select an outside corner p; prefer one with a neighbour p_s in Omega_i (a real edge, Alg. 1 line 3)
+    int p = -1, s = -1;
+    for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
+      const int c = c0 + lane;
+      const bool out = c < nc && S.cstate[c] == ST_OUT;
+      int sn = -1;
+      if (out && A.realEdges) {
+#pragma unroll
+        for (int t = 0; t < 3; ++t)
+          if (S.cstate[S.cadj[c][t]] == ST_IN) sn = S.cadj[c][t];
+      }
+      const unsigned mr = __ballot_sync(kFull, sn >= 0);
+      const unsigned mo = __ballot_sync(kFull, out);
+      if (mr) { const int src = __ffs(mr) - 1; p = c0 + src; s = shfl(sn, src); }
+      else if (mo) { p = c0 + __ffs(mo) - 1; }
+    }
+    if (p < 0) break;            // every corner is in Omega_i: P = T ∩ Omega_i
+    if (np >= P) return 1;
+    // find a bisector B_ij on the real edge p_s p or on the virtual edge w p (Alg. 1 line 4 / Alg. 3 line 3)
+    double psx = wx, psy = wy, psz = wz;
+    if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
+    double nx, ny, nz, d;
+    const int j = find_bisector(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
+                                nx, ny, nz, d, st, lc);
+    if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
+    {
+      bool own = false;
+      for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == j);
+      if (__any_sync(kFull, own)) {   // B_ij already bounds P: p lies on it up to rounding
+        if (lane == 0) S.cstate[p] = ST_IN;
+        __syncwarp();
+        continue;
+      }
+    }
+    lc.clips += 1;
+    const int rc = apply_clip_3d(S, np, nc, p, s, nx, ny, nz, d, j);
+    if (rc == 1) return 1;
+    if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); break; }
+  }
+  return finish_piece_3d(S, A, pairIdx, a, i, np, nc, ox, oy, oz, failed, lc);
+}
+
+}  // namespace vd

@@ -1,0 +1,105 @@
+// vd_clip_args.cuh -- kernel arguments and small helpers shared by the 2D/surface and 3D clip kernels.
+#pragma once
+#include "vd_internal.h"
+#include "vd_nearest.cuh"
+
+namespace vd {
+
+struct ClipArgs {
+  const GridIndex* grid;
+  const double* sites;     // [n][3] original order
+  const double* verts;     // [nv][3]
+  const int* simp;         // [m][nc]
+  const int* adj;          // [m][nc]
+  const int* vnn;          // [nv] nearest site of every mesh vertex
+  int n, m, kind;
+  int realEdges, stepOut;
+  Control* ctl;
+  Pair* pairs;
+  Piece* pieces;
+  unsigned long long* visited;
+  uint64_t hashMask;
+  int64_t pairCap, vertCap, nbrCap, ovfCap;
+  int* ovf;
+  double* poolXYZ;
+  int* poolFlags;
+  int* poolNbr;
+  int* sitePieces;
+  int* siteNbrRaw;
+};
+
+enum { ST_UNKNOWN = 0, ST_IN = 1, ST_OUT = 2 };
+
+struct LocalCnt {
+  unsigned pairs, pieces, search_iters, clips;
+};
+
+__device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& st, const LocalCnt& lc) {
+  if (lane_id() == 0) {
+    atomicAdd(&ctl->cnt.pairs, (unsigned long long)lc.pairs);
+    atomicAdd(&ctl->cnt.pieces, (unsigned long long)lc.pieces);
+    atomicAdd(&ctl->cnt.search_iters, (unsigned long long)lc.search_iters);
+    atomicAdd(&ctl->cnt.clips, (unsigned long long)lc.clips);
+    atomicAdd(&ctl->cnt.queries, (unsigned long long)st.queries);
+    atomicAdd(&ctl->cnt.dist_evals, (unsigned long long)st.dist_evals);
+  }
+}
+
+// Propagation (Alg. 4 lines 11-15): a positive flag j on an edge/face of P_{a,i} means
+// Omega_j meets T_a; push (a, j) once, with a witness point on that edge/face.
+__device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, double wx, double wy, double wz) {
+  if (!visit(A.visited, A.hashMask, a, j)) return;
+  const unsigned long long slot = atomicAdd(&A.ctl->pairTail, 1ull);
+  if ((int64_t)slot >= A.pairCap) { atomicOr(&A.ctl->err, ERR_PAIR_CAP); return; }
+  Pair p;
+  p.a = a; p.i = j; p.wx = wx; p.wy = wy; p.wz = wz;
+  A.pairs[slot] = p;
+}
+
+// Edge-based bisector search (section IV-B) on the segment p_s -> p_t, all in coordinates
+// local to the origin o.  p_s is in Omega_i, the nearest site of p_t is j != i.  Iterates
+// q = B_ij ∩ segment, k = N_q, until k is i or j; then B_ij is the target bisector.  Along the segment
+// every g_k(t) = |x-v_k|^2 - |x-v_i|^2 is linear, so this is Newton's iteration on the concave
+// piecewise-linear min_k g_k from t = 1 (reading U7).  flags[0..nflags) are the flags of P's edges/faces:
+// the segment lies in P, and P is inside H_ik for every site k that owns one of them, so N_q = v_k can
+// only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
+// (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
+__device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, double ox, double oy, double oz,
+                                             double vix, double viy, double viz,   // v_i local
+                                             double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
+                                             double& nx, double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
+  for (int it = 0; it < 96; ++it) {
+    lc.search_iters += 1;
+    const double vjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
+                 vjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+    nx = vjx - vix; ny = vjy - viy; nz = vjz - viz;
+    d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz));
+    const double gs = d - (nx * psx + ny * psy + nz * psz);
+    const double gt = d - (nx * ptx + ny * pty + nz * ptz);
+    const double den = gs - gt;
+    double t = den > 0.0 ? gs / den : 1.0;
+    t = fmin(fmax(t, 0.0), 1.0);
+    const double qx = psx + t * (ptx - psx), qy = psy + t * (pty - psy), qz = psz + t * (ptz - psz);
+    // point-in-cell test of the intersecting point: N_q in {i, j} means q is in Omega_i
+    const double ax = qx + ox, ay = qy + oy, az = qz + oz;
+    const double dix = ax - (vix + ox), diy = ay - (viy + oy), diz = az - (viz + oz);
+    const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
+    const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
+    double best = di2;
+    int bestId = i;
+    if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
+    nearest(g, ax, ay, az, best, bestId, st);
+#ifdef VD_TRACE
+    if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
+#endif
+    if (bestId == i || bestId == j) return j;
+    bool own = false;
+    for (int f = lane_id(); f < nflags; f += kLanes) own |= (flags[f] == bestId);
+    if (__any_sync(kFull, own)) return j;
+    j = bestId;
+    ptx = qx; pty = qy; ptz = qz;
+  }
+  return -1;
+}
+
+}  // namespace vd

@@ -1,0 +1,128 @@
+// vd_common.cuh -- shared types and warp helpers of the CUDA path (sm_100a).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#ifndef VD_LANES
+#define VD_LANES 32
+#endif
+#ifndef VD_LAUNCH
+#define VD_LAUNCH(kernel, grid, block, smem, stream) kernel<<<(grid), (block), (smem), (stream)>>>
+#endif
+
+namespace vd {
+
+constexpr int kLanes = VD_LANES;
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kWarpsPerBlock = 8;
+constexpr int kBlock = kWarpsPerBlock * kLanes;
+
+enum { KIND_TRI_2D = 0, KIND_TRI_SURFACE = 1, KIND_TET_3D = 2 };
+
+// device-side sticky error bits (read once at the end of vd_compute)
+enum {
+  ERR_PAIR_CAP = 1,      // pair list / visited set full
+  ERR_VERT_CAP = 2,      // corner pool full
+  ERR_NBR_CAP = 4,       // face-flag pool full
+  ERR_PIECE_CAP = 8,     // a piece outgrew the large-capacity path
+  ERR_NOCONVERGE = 16,   // iteration cap
+  ERR_TOPOLOGY = 32,     // clip produced a non-simple boundary loop
+  ERR_INPUT = 64         // zero-measure simplex / non-manifold face / non-finite coordinate
+};
+
+// Site index: uniform grid over the sites' bounding box; sites sorted by cell key so
+// that a run of cells along x is one contiguous range.
+struct GridIndex {
+  double lo[3];
+  double h[3];      // cell size (0 on a degenerate axis)
+  double inv_h[3];  // 1/h (0 on a degenerate axis)
+  double hi[3];
+  int G[3];
+  int n;
+  const int* __restrict__ cellStart;      // [G0*G1*G2 + 1]
+  const double4* __restrict__ sites;      // sorted; w = original id (as int bits)
+};
+
+// One unit of work: simplex a, site i, and a witness point w in T_a ∩ Ω_i
+// (DESIGN.md "witness"): the start p_s of virtual edges instead of v_i (Alg. 3 line 3).
+struct Pair {
+  int a, i;
+  double wx, wy, wz;
+};
+
+// Per-pair output record.
+struct Piece {
+  int site, simplex;
+  int nverts, nnbr;
+  int64_t vbase;   // first corner in the corner pool
+  int64_t nbase;   // first entry in the face-flag pool
+  double measure;
+  double mx, my, mz;  // first moment (measure * centroid)
+};
+
+struct Counters {
+  unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs;
+};
+
+__device__ __forceinline__ int lane_id() { return (int)(threadIdx.x % kLanes); }
+
+template <typename T>
+__device__ __forceinline__ T shfl(T v, int src) { return __shfl_sync(kFull, v, src); }
+
+__device__ __forceinline__ bool closer(double d2, int id, double best, int bestId) {
+  return d2 < best || (d2 == best && id < bestId);
+}
+
+// Warp argmin of (d2, id) with the tie rule "lowest id" (reading U5); result uniform.
+__device__ __forceinline__ void warp_argmin(double& d2, int& id) {
+#pragma unroll
+  for (int off = kLanes / 2; off > 0; off >>= 1) {
+    const double od = __shfl_xor_sync(kFull, d2, off);
+    const int oi = __shfl_xor_sync(kFull, id, off);
+    if (closer(od, oi, d2, id)) { d2 = od; id = oi; }
+  }
+}
+
+__device__ __forceinline__ int warp_sum(int v) {
+#pragma unroll
+  for (int off = kLanes / 2; off > 0; off >>= 1) v += __shfl_xor_sync(kFull, v, off);
+  return v;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int off = kLanes / 2; off > 0; off >>= 1) v += __shfl_xor_sync(kFull, v, off);
+  return v;
+}
+
+// exclusive prefix of a per-lane flag, and the total
+__device__ __forceinline__ int warp_rank(bool flag, int& total) {
+  const unsigned m = __ballot_sync(kFull, flag);
+  total = __popc(m);
+  return __popc(m & ((1u << lane_id()) - 1u));
+}
+
+__device__ __forceinline__ uint64_t pair_key(int a, int i) {
+  return (((uint64_t)(uint32_t)a) << 32 | (uint32_t)i) + 1ull;   // 0 = empty slot
+}
+
+__device__ __forceinline__ uint64_t hash64(uint64_t x) {
+  x ^= x >> 33; x *= 0xff51afd7ed558ccdull; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ull; x ^= x >> 33;
+  return x;
+}
+
+// "label it in atomic" (Alg. 4 line 5/13): true iff (a, i) was not yet labelled.
+__device__ __forceinline__ bool visit(unsigned long long* table, uint64_t mask, int a, int i) {
+  const unsigned long long key = pair_key(a, i);
+  uint64_t h = hash64(key) & mask;
+  for (uint64_t probe = 0; probe <= mask; ++probe) {
+    const unsigned long long cur = atomicCAS(&table[h], 0ull, key);
+    if (cur == 0ull) return true;
+    if (cur == key) return false;
+    h = (h + 1) & mask;
+  }
+  return false;
+}
+
+}  // namespace vd

@@ -1,0 +1,182 @@
+// vd_index.cu -- S1: the site index ("build a structure S of V", line 1 of Alg. 2/4/5, P:L180/L250/L301;
+// grid structure P:L377-383).  Bounding box -> cell key per site -> counting sort (histogram, exclusive
+// scan, scatter) -> sites gathered in cell order as 32-byte records.  Plus the S2 query as a kernel of
+// its own (vd_nearest, and the per-mesh-vertex nearest site used by S3).
+#include <math.h>
+
+#include "vd_internal.h"
+#include "vd_nearest.cuh"
+#include "vd_scan.cuh"
+
+namespace vd {
+
+constexpr int kBBoxBlocks = 296;   // 2 x 148 SMs
+
+__global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restrict__ sites, int64_t n, double* __restrict__ part) {
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const double v = sites[i * 3 + a];
+      lo[a] = fmin(lo[a], v);
+      hi[a] = fmax(hi[a], v);
+    }
+  }
+  __shared__ double sm[kWarpsPerBlock][6];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    for (int off = kLanes / 2; off > 0; off >>= 1) {
+      lo[a] = fmin(lo[a], __shfl_xor_sync(kFull, lo[a], off));
+      hi[a] = fmax(hi[a], __shfl_xor_sync(kFull, hi[a], off));
+    }
+  }
+  const int w = (int)threadIdx.x / kLanes;
+  if (lane_id() == 0) {
+    for (int a = 0; a < 3; ++a) { sm[w][a] = lo[a]; sm[w][3 + a] = hi[a]; }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < (int)blockDim.x / kLanes; ++k)
+      for (int a = 0; a < 3; ++a) {
+        sm[0][a] = fmin(sm[0][a], sm[k][a]);
+        sm[0][3 + a] = fmax(sm[0][3 + a], sm[k][3 + a]);
+      }
+    for (int a = 0; a < 6; ++a) part[blockIdx.x * 6 + a] = sm[0][a];
+  }
+}
+
+// One thread: final box, grid resolution ("each grid cell contains, on average, 2~3 / 3~4 sites":
+// average over all cells of the sites' box -- reading U9), header written to device memory.
+__global__ void k_grid_params(const double* __restrict__ part, int nparts, int64_t n, double density, int64_t gridCap,
+                              const int* cellStart, const double4* sorted, GridIndex* g, unsigned int* err) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int k = 0; k < nparts; ++k)
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = fmin(lo[a], part[k * 6 + a]);
+      hi[a] = fmax(hi[a], part[k * 6 + 3 + a]);
+    }
+  double ext[3], vol = 1.0;
+  int nd = 0;
+  for (int a = 0; a < 3; ++a) {
+    ext[a] = hi[a] - lo[a];
+    if (!(ext[a] == ext[a]) || ext[a] > 1e300) atomicOr(err, ERR_INPUT);
+    if (ext[a] > 0) { vol *= ext[a]; ++nd; }
+  }
+  double target = (double)n / density;
+  if (target < 1.0) target = 1.0;
+  double h = nd > 0 ? pow(vol / target, 1.0 / nd) : 1.0;
+  int G[3];
+  for (int it = 0; it < 64; ++it) {
+    double prod = 1.0;
+    for (int a = 0; a < 3; ++a) {
+      G[a] = ext[a] > 0 ? (int)fmin(fmax(ceil(ext[a] / h), 1.0), 2047.0) : 1;
+      prod *= G[a];
+    }
+    if (prod <= (double)gridCap) break;
+    h *= 1.1;
+  }
+  GridIndex out;
+  for (int a = 0; a < 3; ++a) {
+    out.lo[a] = lo[a];
+    out.hi[a] = hi[a];
+    out.G[a] = G[a];
+    out.h[a] = ext[a] > 0 ? ext[a] / G[a] : 0.0;
+    out.inv_h[a] = ext[a] > 0 ? G[a] / ext[a] : 0.0;
+  }
+  out.n = (int)n;
+  out.cellStart = cellStart;
+  out.sites = sorted;
+  *g = out;
+}
+
+__global__ void __launch_bounds__(kBlock) k_cell_count(const double* __restrict__ sites, int64_t n, const GridIndex* __restrict__ gp,
+                                                        int* __restrict__ cellOf, int* __restrict__ cellFill) {
+  const GridIndex g = *gp;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int cx = cell_of(g, 0, sites[i * 3 + 0]), cy = cell_of(g, 1, sites[i * 3 + 1]), cz = cell_of(g, 2, sites[i * 3 + 2]);
+    const int c = (cz * g.G[1] + cy) * g.G[0] + cx;
+    cellOf[i] = c;
+    atomicAdd(&cellFill[c], 1);
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_cell_scatter(const double* __restrict__ sites, int64_t n, const int* __restrict__ cellOf,
+                                                          const int* __restrict__ cellStart, int* __restrict__ cellFill,
+                                                          double4* __restrict__ sorted) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int c = cellOf[i];
+    const int pos = cellStart[c] + atomicSub(&cellFill[c], 1) - 1;
+    double4 p;
+    p.x = sites[i * 3 + 0];
+    p.y = sites[i * 3 + 1];
+    p.z = sites[i * 3 + 2];
+    p.w = __longlong_as_double((long long)i);
+    sorted[pos] = p;
+  }
+}
+
+// S2 as a kernel: one warp per query point.
+__global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __restrict__ gp, const double* __restrict__ q3, int64_t nq,
+                                                            int* __restrict__ out, Counters* cnt) {
+  const GridIndex g = *gp;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
+  QueryStats st = {0u, 0u};
+  for (int64_t q = warp; q < nq; q += nwarps) {
+    double best = 2e300;
+    int bestId = 0x7fffffff;
+    nearest(g, q3[q * 3 + 0], q3[q * 3 + 1], q3[q * 3 + 2], best, bestId, st);
+    if (lane_id() == 0) out[q] = bestId;
+  }
+  if (lane_id() == 0 && cnt) {
+    atomicAdd(&cnt->queries, (unsigned long long)st.queries);
+    atomicAdd(&cnt->dist_evals, (unsigned long long)st.dist_evals);
+  }
+}
+
+static int grid_for(int64_t items, int perBlock) {
+  int64_t b = (items + perBlock - 1) / perBlock;
+  const int64_t cap = 148 * 16;
+  if (b > cap) b = cap;
+  if (b < 1) b = 1;
+  return (int)b;
+}
+
+vd_status stage_index(vd_ctx* c) {
+  const int64_t n = c->n;
+  const double density = c->opt.grid_density > 0 ? c->opt.grid_density : 4.0;
+  const int64_t gridCap = (int64_t)((double)n / density) * 2 + 64;
+  c->gridCap = gridCap;
+  vd_status s;
+  if ((s = ensure(c, c->grid, sizeof(GridIndex)))) return s;
+  if ((s = ensure(c, c->bbox, sizeof(double) * 6 * kBBoxBlocks))) return s;
+  if ((s = ensure(c, c->cellOf, sizeof(int) * n))) return s;
+  if ((s = ensure(c, c->cellStart, sizeof(int) * (gridCap + 2)))) return s;
+  if ((s = ensure(c, c->cellFill, sizeof(int) * (gridCap + 2)))) return s;
+  if ((s = ensure(c, c->sorted, sizeof(double4) * n))) return s;
+  if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(n > gridCap ? n : gridCap) * 2))) return s;
+  if ((s = ensure(c, c->control, sizeof(Control)))) return s;
+  cudaStream_t st = c->stream;
+  const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
+  VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
+  VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
+                                         c->sorted.as<double4>(), c->grid.as<GridIndex>(), &c->control.as<Control>()->err);
+  cudaMemsetAsync(c->cellFill.p, 0, sizeof(int) * (gridCap + 2), st);
+  VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
+                                                              c->cellFill.as<int>());
+  exclusive_scan<int, int>(c->cellFill.as<int>(), gridCap + 1, c->cellStart.as<int>(), c->scanTmp.as<int>(), st);
+  VD_LAUNCH(k_cell_scatter, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->cellOf.as<int>(), c->cellStart.as<int>(),
+                                                                c->cellFill.as<int>(), c->sorted.as<double4>());
+  c->indexValid = true;
+  return cuda_check(c, cudaGetLastError(), "site index");
+}
+
+vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out) {
+  if (nq <= 0) return VD_OK;
+  const int blocks = grid_for(nq, kWarpsPerBlock);
+  VD_LAUNCH(k_nearest_points, blocks, kBlock, 0, c->stream)(c->grid.as<GridIndex>(), q3, nq, out, &c->control.as<Control>()->cnt);
+  return cuda_check(c, cudaGetLastError(), "nearest");
+}
+
+}  // namespace vd

@@ -1,0 +1,99 @@
+// vd_internal.h -- the context behind the C ABI (include/vd.h) and the stage entry points.
+#pragma once
+#include <string>
+
+#include "../../include/vd.h"
+#include "vd_common.cuh"
+
+namespace vd {
+
+// Device-side control block: queue tails, pool cursors, sticky error word, work counters.
+struct Control {
+  unsigned long long pairTail;   // pairs pushed so far
+  unsigned long long ovfTail;    // pairs deferred to the large-capacity path
+  unsigned long long vertTail;   // corners allocated in the pool
+  unsigned long long nbrTail;    // face flags allocated in the pool
+  unsigned int err;              // ERR_* bits
+  unsigned int pad;
+  Counters cnt;
+  unsigned long long nPieces, nNonEmpty, nVerts, nNbrs;   // totals written by S6
+};
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+  template <typename T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+}  // namespace vd
+
+struct vd_ctx {
+  int64_t n = 0, nv = 0, m = 0;
+  int dim = 0, kind = -1, nc = 0, nfl = 0;
+  bool haveDomain = false, haveResult = false, indexValid = false;
+  cudaStream_t stream = nullptr;
+  void* (*allocFn)(size_t, void*, void*) = nullptr;
+  void (*freeFn)(void*, void*) = nullptr;
+  void* allocUser = nullptr;
+  vd_options opt{};
+  vd_counters counters{};
+  double stageMs[5] = {0, 0, 0, 0, 0};
+  std::string lastError;
+  cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+
+  int64_t pairCap = 0, vertCap = 0, nbrCap = 0, hashCap = 0, ovfCap = 0, gridCap = 0;
+
+  // inputs
+  vd::DevBuf sites;       // double [n][3] (z = 0 for dim 2)
+  vd::DevBuf verts;       // double [nv][3]
+  vd::DevBuf simp;        // int [m][nc]
+  vd::DevBuf adj;         // int [m][nc]
+  // S1
+  vd::DevBuf grid;        // GridIndex (device copy)
+  vd::DevBuf bbox;        // double partial min/max
+  vd::DevBuf cellOf;      // int [n]
+  vd::DevBuf cellStart;   // int [gridCap+1]
+  vd::DevBuf cellFill;    // int [gridCap+1]
+  vd::DevBuf sorted;      // double4 [n]
+  vd::DevBuf scanTmp;     // scan scratch
+  // S3-S5
+  vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
+  vd::DevBuf control;     // Control
+  vd::DevBuf pairs;       // Pair [pairCap]
+  vd::DevBuf pieces;      // Piece [pairCap]
+  vd::DevBuf visited;     // u64 [hashCap]
+  vd::DevBuf ovf;         // int [ovfCap]
+  vd::DevBuf poolXYZ;     // double [vertCap][3]
+  vd::DevBuf poolFlags;   // int [vertCap][nfl]
+  vd::DevBuf poolNbr;     // int [nbrCap]
+  // S6
+  vd::DevBuf sitePieces;  // int [n]  pieces per site
+  vd::DevBuf siteNbrRaw;  // int [n]  face flags per site (with repeats)
+  vd::DevBuf siteFill;    // int [n]
+  vd::DevBuf order;       // int [pieces]  piece list grouped by site, sorted by simplex
+  vd::DevBuf nbrRawOff;   // int64 [n+1]
+  vd::DevBuf nbrRaw;      // int [sum raw]
+  vd::DevBuf nbrCnt;      // int [n]
+  vd::DevBuf vcount;      // int [pieces]
+  // outputs (vd_cells)
+  vd::DevBuf oMeasure, oCentroid, oNbrOff, oNbr, oPieceOff, oPieceSimplex, oPieceMeasure, oVertOff, oVertXYZ, oVertFlags;
+  vd_cells cells{};
+  vd::Control hostControl{};
+};
+
+namespace vd {
+
+// memory
+vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes);
+void release(vd_ctx* c, DevBuf& b);
+vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what);
+
+// stages (each enqueues kernels on c->stream)
+vd_status stage_domain(vd_ctx* c);                 // S0  vd_domain.cu
+vd_status stage_index(vd_ctx* c);                  // S1  vd_index.cu
+vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out);  // S2 as a kernel (vd_nearest, vnn)
+vd_status stage_seed(vd_ctx* c);                   // S3  vd_clip.cu
+vd_status stage_clip(vd_ctx* c);                   // S4+S5  vd_clip.cu
+vd_status stage_assemble(vd_ctx* c);               // S6  vd_assemble.cu
+
+}  // namespace vd

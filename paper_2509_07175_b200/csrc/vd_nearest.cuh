@@ -1,0 +1,164 @@
+// vd_nearest.cuh -- S2: warp-cooperative nearest-site query over the grid index.
+// All 32 lanes of a warp call these functions with the SAME query point; lanes split the candidate
+// rows / sites; results are warp-uniform.
+#pragma once
+#include "vd_common.cuh"
+
+namespace vd {
+
+struct QueryStats {
+  unsigned queries, dist_evals;
+};
+
+__device__ __forceinline__ int cell_of(const GridIndex& g, int ax, double q) {
+  int c = (int)floor((q - g.lo[ax]) * g.inv_h[ax]);
+  return min(max(c, 0), g.G[ax] - 1);
+}
+
+// squared distance from q to the slab [lo + c0*h, lo + (c1+1)*h] along one axis (slightly widened:
+// conservative against the rounding of the cell assignment)
+__device__ __forceinline__ double slab_d2(const GridIndex& g, int ax, double q, int c0, int c1) {
+  const double a = g.lo[ax] + (c0 - 1e-9) * g.h[ax];
+  const double b = g.lo[ax] + (c1 + 1 + 1e-9) * g.h[ax];
+  const double d = (q < a) ? (a - q) : ((q > b) ? (q - b) : 0.0);
+  return d * d;
+}
+
+// Scan one contiguous site range [s, s+cnt) for sites closer than (best, bestId).  Uniform result.
+__device__ __forceinline__ void scan_range(const GridIndex& g, double qx, double qy, double qz, int s, int cnt,
+                                           double& best, int& bestId, QueryStats& st) {
+  st.dist_evals += (unsigned)cnt;
+  for (int k0 = 0; k0 < cnt; k0 += kLanes) {
+    const int k = k0 + lane_id();
+    double d2 = best;
+    int id = 0x7fffffff;
+    if (k < cnt) {
+      const double4 p = g.sites[s + k];
+      const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
+      d2 = dx * dx + dy * dy + dz * dz;
+      id = __double_as_longlong(p.w) & 0x7fffffff;
+    }
+    const bool better = (k < cnt) && closer(d2, id, best, bestId);
+    if (__any_sync(kFull, better)) {
+      if (!better) { d2 = best; id = bestId; }
+      warp_argmin(d2, id);
+      best = d2;
+      bestId = id;
+    }
+  }
+}
+
+// Scan every cell of the box [x0..x1]x[y0..y1]x[z0..z1] whose row can hold a site closer than best.
+// One lane per row (y,z): box-distance pruning, x-extent tightened to the ball, one contiguous range.
+__device__ __forceinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0,
+                                         int y1, int z0, int z1, double& best, int& bestId, QueryStats& st) {
+  const int ny = y1 - y0 + 1;
+  const int nrows = ny * (z1 - z0 + 1);
+  for (int r0 = 0; r0 < nrows; r0 += kLanes) {
+    const int r = r0 + lane_id();
+    int s = 0, cnt = 0;
+    double rd2 = 0.0;
+    if (r < nrows) {
+      const int y = y0 + r % ny, z = z0 + r / ny;
+      rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
+      if (!(rd2 > best)) {
+        int xa = x0, xb = x1;
+        if (best < 1e300) {
+          const double w = sqrt(best - rd2);
+          xa = max(x0, (int)floor((qx - w - g.lo[0]) * g.inv_h[0] - 1e-6));
+          xb = min(x1, (int)floor((qx + w - g.lo[0]) * g.inv_h[0] + 1e-6));
+        }
+        if (xa <= xb) {
+          const int base = (z * g.G[1] + y) * g.G[0];
+          s = __ldg(&g.cellStart[base + xa]);
+          cnt = __ldg(&g.cellStart[base + xb + 1]) - s;
+          rd2 += slab_d2(g, 0, qx, xa, xb);
+        }
+      }
+    }
+    unsigned m = __ballot_sync(kFull, cnt > 0);
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      const int ss = shfl(s, src), cc = shfl(cnt, src);
+      const double dd = shfl(rd2, src);
+      if (dd > best) continue;
+      scan_range(g, qx, qy, qz, ss, cc, best, bestId, st);
+    }
+  }
+}
+
+// N_q: the site nearest to q among those closer than the incoming (best, bestId); ties to
+// the lowest id (reading U5).  Call with best = +inf, bestId = INT_MAX for an unbounded query, or
+// with best = |q - v_i|^2, bestId = i for a point-in-cell test (Eq. 2).
+__device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
+                                        QueryStats& st) {
+  st.queries += 1;
+  const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);
+  // how far q lies outside the grid box on each axis
+  const double ox = fmax(fmax(g.lo[0] - qx, qx - g.hi[0]), 0.0);
+  const double oy = fmax(fmax(g.lo[1] - qy, qy - g.hi[1]), 0.0);
+  const double oz = fmax(fmax(g.lo[2] - qz, qz - g.hi[2]), 0.0);
+  bool needSeed = !(best < 1e300);  // callers pass best >= 2e300 for "unbounded"
+  if (!needSeed) {
+    // rows of the ball's bounding box; a loose bound is first tightened around the home cell
+    const double r = sqrt(best);
+    const double ry = 2.0 * r * g.inv_h[1] + 2.0, rz = 2.0 * r * g.inv_h[2] + 2.0;
+    needSeed = ry * rz > 16.0;
+  }
+  if (needSeed) {
+    // expanding shells around the (clamped) home cell until some site is known (sb, si); then the
+    // ball's box below decides.  Stops at once when no unscanned cell can beat the bound.
+    double sb = 2e300;
+    int si = 0x7fffffff;
+    bool done = false;
+    const int smax = max(g.G[0], max(g.G[1], g.G[2]));
+    for (int s = 0; s <= smax; ++s) {
+      if (s > 0) {
+        // lower bound of the distance to any cell outside the box of radius s-1 (faces that lie
+        // beyond the grid hold no cells)
+        double lb = 2e300;
+        const int k = s - 1;
+        if (cx - k > 0) lb = fmin(lb, slab_d2(g, 0, qx, 0, cx - k - 1) + oy * oy + oz * oz);
+        if (cx + k < g.G[0] - 1) lb = fmin(lb, slab_d2(g, 0, qx, cx + k + 1, g.G[0] - 1) + oy * oy + oz * oz);
+        if (cy - k > 0) lb = fmin(lb, slab_d2(g, 1, qy, 0, cy - k - 1) + ox * ox + oz * oz);
+        if (cy + k < g.G[1] - 1) lb = fmin(lb, slab_d2(g, 1, qy, cy + k + 1, g.G[1] - 1) + ox * ox + oz * oz);
+        if (cz - k > 0) lb = fmin(lb, slab_d2(g, 2, qz, 0, cz - k - 1) + ox * ox + oy * oy);
+        if (cz + k < g.G[2] - 1) lb = fmin(lb, slab_d2(g, 2, qz, cz + k + 1, g.G[2] - 1) + ox * ox + oy * oy);
+        if (lb > fmin(best, sb)) { done = true; break; }
+        if (sb < 1e300) break;
+      }
+      // shell s: rows with max(|dy|,|dz|) == s take the full x extent, inner rows the two end cells
+      const int y0 = max(cy - s, 0), y1 = min(cy + s, g.G[1] - 1);
+      const int z0 = max(cz - s, 0), z1 = min(cz + s, g.G[2] - 1);
+      const int xl = cx - s, xr = cx + s;
+      const int xa = max(xl, 0), xb = min(xr, g.G[0] - 1);
+      if (s == 0) {
+        scan_box(g, qx, qy, qz, xa, xb, y0, y1, z0, z1, sb, si, st);
+      } else {
+        if (cz - s >= 0) scan_box(g, qx, qy, qz, xa, xb, y0, y1, cz - s, cz - s, sb, si, st);
+        if (cz + s < g.G[2]) scan_box(g, qx, qy, qz, xa, xb, y0, y1, cz + s, cz + s, sb, si, st);
+        const int zi0 = max(cz - s + 1, 0), zi1 = min(cz + s - 1, g.G[2] - 1);
+        if (zi0 <= zi1) {
+          if (cy - s >= 0) scan_box(g, qx, qy, qz, xa, xb, cy - s, cy - s, zi0, zi1, sb, si, st);
+          if (cy + s < g.G[1]) scan_box(g, qx, qy, qz, xa, xb, cy + s, cy + s, zi0, zi1, sb, si, st);
+          const int yi0 = max(cy - s + 1, 0), yi1 = min(cy + s - 1, g.G[1] - 1);
+          if (yi0 <= yi1) {
+            if (xl >= 0) scan_box(g, qx, qy, qz, xl, xl, yi0, yi1, zi0, zi1, sb, si, st);
+            if (xr < g.G[0]) scan_box(g, qx, qy, qz, xr, xr, yi0, yi1, zi0, zi1, sb, si, st);
+          }
+        }
+      }
+    }
+    if (closer(sb, si, best, bestId)) { best = sb; bestId = si; }
+    if (done || !(best < 1e300)) return;
+  }
+  // the ball (q, sqrt(best)) decides: scan its bounding box of cells, rows pruned as best shrinks
+  const double r = sqrt(best);
+  const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
+  const int y0 = cell_of(g, 1, qy - r - 1e-6 * g.h[1]), y1 = cell_of(g, 1, qy + r + 1e-6 * g.h[1]);
+  const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
+  scan_box(g, qx, qy, qz, x0, x1, y0, y1, z0, z1, best, bestId, st);
+}
+
+}  // namespace vd

@@ -1,0 +1,123 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: neighbour sets / piece simplices / corner counts /
+corner flags exact, measure and centroid 1e-9 relative, corners 1e-9 * domain diameter."""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2509_07175_b200 import binding, inputs
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu(w, **opts):
+    with binding.Context(w.sites) as ctx:
+        if opts:
+            ctx.set_options(**opts)
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        ctx.compute()
+        return ctx.to_host(), ctx.counters(), ctx.adjacency()
+
+
+def test_golden_hand_cases_through_the_abi():
+    import json, os
+    here = os.path.dirname(os.path.abspath(__file__))
+    cases = json.load(open(os.path.join(here, "golden", "unit_square_cases.json")))["cases"]
+    v, t = inputs.unit_square_mesh()
+    for case in cases:
+        s = np.array(case["sites"], dtype=np.float64)
+        g = binding.compute(s, v, t, 0)
+        assert np.allclose(g.measure, case["area"], rtol=0, atol=1e-12)
+        for i, nb in enumerate(case["nbr"]):
+            assert g.neighbours(i).tolist() == nb
+        if case["pieces"] is not None:
+            for i, pcs in enumerate(case["pieces"]):
+                got = [[int(g.piece_simplex[p]), int(g.vert_off[p + 1] - g.vert_off[p])] for p in g.pieces(i)]
+                assert got == pcs
+
+
+def test_c1_full_parity():
+    w = inputs.config(1)
+    g, cnt, adj = _gpu(w)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+    assert np.array_equal(adj, o.simplex_adj)
+    assert cnt["pieces"] == len(o.piece_simplex)
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4, 5])
+def test_replica_parity(idx):
+    w = inputs.config(idx, "small")
+    g, cnt, adj = _gpu(w)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+    assert np.array_equal(adj, o.simplex_adj)
+    assert g.n_nonempty == int((o.measure > 0).sum())
+
+
+@pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0)])
+def test_options_do_not_change_the_result(opts):
+    w = inputs.config(2, "small")
+    g, _, _ = _gpu(w, **opts)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+
+
+def test_nearest_site_kernel_against_brute_force():
+    for idx in (2, 3, 5):
+        w = inputs.config(idx, "small")
+        rng = np.random.default_rng(100 + idx)
+        q = np.concatenate([rng.random((2000, 3)), rng.random((500, 3)) * 4.0 - 1.5,
+                            w.sites[rng.integers(0, w.n, 200)] + 1e-7])
+        with binding.Context(w.sites) as ctx:
+            got = ctx.nearest(q)
+        d = ((q[:, None, :] - w.sites[None, :, :]) ** 2).sum(-1) if w.n <= 5000 else None
+        if d is None:
+            ref = np.array([np.argmin(((w.sites - x) ** 2).sum(1)) for x in q])
+        else:
+            ref = d.argmin(1)
+        assert np.array_equal(got, ref)
+
+
+def test_regular_grid_terminates_with_equal_cells():
+    # degenerate input (cospherical sites): only measure and centroid are unique
+    for dim, k in ((2, 4), (3, 3)):
+        s = inputs.grid_sites(k, dim)
+        if dim == 2:
+            v, t = inputs.unit_square_mesh()
+            kind = 0
+        else:
+            v, t = inputs.cube_kuhn_mesh(2)
+            kind = 2
+        g = binding.compute(s, v, t, kind)
+        assert np.allclose(g.measure, 1.0 / k ** dim, rtol=0, atol=1e-12)
+        assert np.allclose(g.centroid, s, rtol=0, atol=1e-11)
+
+
+def test_edge_cases():
+    v, t = inputs.unit_square_mesh()
+    g = binding.compute(np.array([[0.3, 0.4]]), v, t, 0)       # n = 1: the cell is the domain
+    assert abs(g.measure[0] - 1.0) < 1e-15 and g.neighbours(0).size == 0
+    v3, t3 = inputs.cube_kuhn_mesh(1)
+    g = binding.compute(np.array([[0.25, 0.5, 0.5], [0.75, 0.5, 0.5], [5.0, 5.0, 5.0]]), v3, t3, 2)
+    assert np.allclose(g.measure, [0.5, 0.5, 0.0], atol=1e-15)   # a far site has an empty cell
+    assert np.allclose(g.centroid[2], [5.0, 5.0, 5.0]) and g.n_nonempty == 2
+    with pytest.raises(binding.VdError):                          # non-manifold: three triangles on one edge
+        binding.compute(np.random.default_rng(0).random((5, 3)),
+                        np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1.0]]),
+                        np.array([[0, 1, 2], [0, 1, 3], [0, 1, 4]], dtype=np.int32), 1)
+    with pytest.raises(binding.VdError):                          # zero-measure simplex
+        binding.compute(np.random.default_rng(0).random((5, 2)), np.array([[0, 0], [1, 0], [2, 0.0]]),
+                        np.array([[0, 1, 2]], dtype=np.int32), 0)
+    with pytest.raises(binding.VdError):                          # NaN site
+        binding.compute(np.array([[0.1, np.nan]]), v, t, 0)
+
+
+def test_results_are_bitwise_reproducible():
+    w = inputs.config(2, "small")
+    a, _, _ = _gpu(w)
+    b, _, _ = _gpu(w)
+    for f in ("measure", "centroid", "nbr", "piece_simplex", "piece_measure", "vert_xyz", "vert_flags"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
