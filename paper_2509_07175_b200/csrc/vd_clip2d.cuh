@@ -22,6 +22,16 @@ struct Poly2 {
   int nc;
 };
 
+// fallback position of a new corner (ill-conditioned planes): where the edge from the removed corner c to
+// the surviving corner b meets the line, by interpolation
+__device__ __forceinline__ void lerp_to_plane(double cx, double cy, double cz, double bx, double by, double bz, double nx, double ny,
+                                              double nz, double d, double& x, double& y, double& z) {
+  const double sc = nx * cx + ny * cy + nz * cz - d, sn = nx * bx + ny * by + nz * bz - d;
+  double t = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
+  t = fmin(fmax(t, 0.0), 1.0);
+  x = cx + t * (bx - cx); y = cy + t * (by - cy); z = cz + t * (bz - cz);
+}
+
 template <int K>
 __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
@@ -161,12 +171,14 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
           if (c == pv) break;
         }
         // X = edge(pv) ∩ B_ij : start of the new edge, which takes flag j
-        solve3(S.enx[pv], S.eny[pv], S.enz[pv], S.ed[pv], nx, ny, nz, d, pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]);
+        if (!solve3(S.enx[pv], S.eny[pv], S.enz[pv], S.ed[pv], nx, ny, nz, d, pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
+          lerp_to_plane(S.cx[r0], S.cy[r0], S.cz[r0], S.cx[pv], S.cy[pv], S.cz[pv], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
         S.tnx[k] = nx; S.tny[k] = ny; S.tnz[k] = nz; S.td[k] = d; S.tflag[k] = j; S.tnn[k] = -1;
         S.tstate[k] = (s == pv && p == r0) ? ST_IN : ST_UNKNOWN;   // on the searched real edge
         ++k;
         // E = B_ij ∩ edge(r1) : the rest of edge r1 keeps its plane and flag
-        solve3(nx, ny, nz, d, S.enx[r1], S.eny[r1], S.enz[r1], S.ed[r1], pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]);
+        if (!solve3(nx, ny, nz, d, S.enx[r1], S.eny[r1], S.enz[r1], S.ed[r1], pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
+          lerp_to_plane(S.cx[r1], S.cy[r1], S.cz[r1], S.cx[nxt], S.cy[nxt], S.cz[nxt], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
         S.tnx[k] = S.enx[r1]; S.tny[k] = S.eny[r1]; S.tnz[k] = S.enz[r1]; S.td[k] = S.ed[r1];
         S.tflag[k] = S.eflag[r1]; S.tnn[k] = -1;
         S.tstate[k] = (s == nxt && p == r1) ? ST_IN : ST_UNKNOWN;

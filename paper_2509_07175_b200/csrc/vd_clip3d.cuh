@@ -12,7 +12,7 @@ struct Poly3 {
   int pflag[P];                           // flag of plane f
   double cx[C], cy[C], cz[C];             // corner coordinates (local)
   int cnn[C];                             // nearest site of an outside corner
-  int key[C][3];                          // scratch: ascending flag triple of a corner (output order)
+  int key[C][3];                          // scratch: flag triple of a corner (output order); rim points during a clip (P*3 doubles)
   unsigned short cp[C][3];                // the corner's three planes, cyclically ordered
   unsigned short cadj[C][3];              // corner across the polytope edge (cp[t], cp[t+1])
   unsigned short remap[C];                // scratch: index of a surviving corner after the clip
@@ -21,7 +21,8 @@ struct Poly3 {
   unsigned char cstate[C], cmark[C];
 };
 
-__device__ __forceinline__ void solve3(double ax, double ay, double az, double ad, double bx, double by, double bz, double bd,
+// returns false when the three planes are (numerically) parallel to a common line
+__device__ __forceinline__ bool solve3(double ax, double ay, double az, double ad, double bx, double by, double bz, double bd,
                                        double cx, double cy, double cz, double cd, double& x, double& y, double& z) {
   // Cramer: x = (ad (b x c) + bd (c x a) + cd (a x b)) / det[a, b, c]
   const double bcx = by * cz - bz * cy, bcy = bz * cx - bx * cz, bcz = bx * cy - by * cx;
@@ -32,6 +33,8 @@ __device__ __forceinline__ void solve3(double ax, double ay, double az, double a
   x = (ad * bcx + bd * cax + cd * abx) * inv;
   y = (ad * bcy + bd * cay + cd * aby) * inv;
   z = (ad * bcz + bd * caz + cd * abz) * inv;
+  const double na = ax * ax + ay * ay + az * az, nb = bx * bx + by * by + bz * bz, nc = cx * cx + cy * cy + cz * cz;
+  return det * det > 1e-24 * na * nb * nc;
 }
 
 // P <- P clipped by the half-space n.x <= d with flag j (Alg. 3 line 4), steps of P:L389: (1) the
@@ -89,6 +92,19 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     for (int k = 0; k < cnt; ++k) {
       S.be[base + k][0] = ea[k]; S.be[base + k][1] = eb[k]; S.be[base + k][2] = en[k];
       S.be[base + k][3] = (unsigned short)((c == p && (int)en[k] == s) ? 1 : 0);
+      {
+        // where the polytope edge (c, neighbour) meets the plane, by interpolation: the fallback position of
+        // the new corner when its three planes are ill-conditioned (degenerate inputs, e.g. regular grids)
+        const int nb = en[k];
+        const double sc = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+        const double sn = nx * S.cx[nb] + ny * S.cy[nb] + nz * S.cz[nb] - d;
+        double t = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
+        t = fmin(fmax(t, 0.0), 1.0);
+        double* rim = reinterpret_cast<double*>(&S.key[0][0]) + 3 * (base + k);
+        rim[0] = S.cx[c] + t * (S.cx[nb] - S.cx[c]);
+        rim[1] = S.cy[c] + t * (S.cy[nb] - S.cy[c]);
+        rim[2] = S.cz[c] + t * (S.cz[nb] - S.cz[c]);
+      }
       // the surviving neighbour's slot that pointed at c will point at the new corner
 #pragma unroll
       for (int t = 0; t < 3; ++t)
@@ -156,7 +172,11 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     S.cadj[t][1] = (unsigned short)nxt;
     S.cadj[t][2] = (unsigned short)prv;
     double x, y, z;
-    solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
+    const bool ok = solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
+    if (!ok) {
+      const double* rim = reinterpret_cast<const double*>(&S.key[0][0]) + 3 * e;
+      x = rim[0]; y = rim[1]; z = rim[2];
+    }
     S.cx[t] = x; S.cy[t] = y; S.cz[t] = z;
     S.cnn[t] = -1;
     // the new corner on the searched real edge p_s p is in Omega_i ∩ Omega_j
@@ -179,6 +199,9 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   pc.measure = 0; pc.mx = pc.my = pc.mz = 0;
   lc.pairs += 1;
   if (failed || nc < 4) {
+#ifdef VD_TRACE
+    if (lane == 0) printf("pair(%d,%d) dropped: failed=%d nc=%d np=%d\n", a, i, (int)failed, nc, np);
+#endif
     if (lane == 0) A.pieces[pairIdx] = pc;
     return 0;
   }
@@ -237,6 +260,9 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   vol = warp_sum(vol); mx = warp_sum(mx); my = warp_sum(my); mz = warp_sum(mz);
   if (vol < 0) { vol = -vol; mx = -mx; my = -my; mz = -mz; }
   if (!(vol > 0)) {
+#ifdef VD_TRACE
+    if (lane == 0) printf("pair(%d,%d) dropped: vol=%g nc=%d\n", a, i, vol, nc);
+#endif
     if (lane == 0) A.pieces[pairIdx] = pc;
     return 0;
   }
@@ -403,6 +429,9 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
         continue;
       }
     }
+#ifdef VD_TRACE
+    if (lane == 0) printf("pair(%d,%d) clip p=%d(%g,%g,%g) s=%d j=%d nc=%d np=%d\n", a, i, p, S.cx[p]+ox, S.cy[p]+oy, S.cz[p]+oz, s, j, nc, np);
+#endif
     lc.clips += 1;
     const int rc = apply_clip_3d(S, np, nc, p, s, nx, ny, nz, d, j);
     if (rc == 1) return 1;
