@@ -1,0 +1,261 @@
+#!/usr/bin/env python
+"""bench.py -- clipped Voronoi cells/s on B200 (BASELINE.json metric), one JSON line.
+
+A "step" is one pass of the whole hot path (S1 index, S3 seeds, S4+S5 clip + propagate, S6 assemble =
+one vd_compute) over one seeded synthetic workload.  `value` is device-timed with the inputs already
+resident in HBM (the context holds copies of sites and domain); `e2e` is the same metric through the C
+ABI with HOST buffers: vd_create + vd_set_domain + vd_compute + vd_cells_to_host + vd_destroy.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+N > 1 (torchrun): the path does not shard in this round ("replicas only"): every rank runs
+the whole workload on its own GPU; value = N * n / max-over-ranks time.
+--impl reference: the CPU oracle, as it stands, timed on the host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "clipped Voronoi cells/sec at 1 B200 (device-timed); achieved % of roofline"
+UNIT = "cells/s"
+# plain FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64 FMA
+# lanes x 2 flop at the maximum SM clock; no FP64 figure exists in MEASURED_PEAKS.json.
+FP64_LANES_PER_SM, SMS = 64, 148
+WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
+             2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
+             3: "C3: unit cube 48^3 x 6 tets (663,552), 1,000,000 clustered sites, seed 2",
+             4: "C4: torus 512x256 (262,144 triangles), 200,000 shell sites, seed 3",
+             5: "C5: unit cube 32^3 x 6 tets (196,608), 2,000,000 far-slab sites, seed 4"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 6 for k in range(4) if r[2 + k].startswith("Active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def algorithmic_flops(cnt, kind):
+    """8 flop per candidate distance (5 in 2D), 15 per search iteration,
+    per clip 2d flop x ~corners tested + 60 per new 3D corner (15 in 2D), 30 per fan tet of a piece."""
+    d3 = kind == 2
+    per_dist = 8 if kind != 0 else 5
+    per_clip = (6 * 12 + 60 * 4) if d3 else (4 * 6 + 15 * 2)
+    per_piece = 30 * (20 if d3 else 4)
+    return per_dist * cnt["dist_evals"] + 15 * cnt["search_iters"] + per_clip * cnt["clips"] + per_piece * cnt["pieces"]
+
+
+def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
+    """The oracle as it stands (tier B for volumes / 2D, tier A for the surface), timed on the host
+    cores on a bounded random sample of sites of the same workload."""
+    from oracle import oracle
+    rng = np.random.default_rng(seed)
+    tier = "A" if w.kind == 1 else "B"
+    k = min(w.n, 32)
+    t0 = time.perf_counter()
+    r = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, k, replace=False)), tier=tier)
+    dt = time.perf_counter() - t0
+    per_site = dt / k
+    k2 = int(min(w.n, max(k, seconds_target / max(per_site, 1e-9))))
+    if k2 > 2 * k:
+        k = k2
+        t0 = time.perf_counter()
+        r = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, k, replace=False)), tier=tier)
+        dt = time.perf_counter() - t0
+    return {"value": k / dt, "unit": UNIT, "cores": int(r.threads_used), "kind": "oracle",
+            "sample": f"{k} seeded-random sites of the workload, tier {tier}, {dt:.1f} s wall"}
+
+
+def run_reference(args, w):
+    """--impl reference: each step = the oracle on a bounded sample of sites."""
+    from oracle import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    tier = "A" if w.kind == 1 else "B"
+    rng = np.random.default_rng(777)
+    probe = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, min(w.n, 16), replace=False)), tier=tier)
+    t0 = time.perf_counter()
+    oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, min(w.n, 16), replace=False)), tier=tier)
+    per_site = (time.perf_counter() - t0) / min(w.n, 16)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    k = int(min(w.n, max(8, budget / max(per_site, 1e-9))))
+    times = []
+    for s in range(args.warmup + args.steps):
+        sub = np.sort(rng.choice(w.n, k, replace=False))
+        t0 = time.perf_counter()
+        oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=sub, tier=tier)
+        if s >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = sum(times)
+    val = k * len(times) / total
+    sample = f"{k} seeded-random sites per step, tier {tier}"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": int(probe.threads_used), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index, 1-based (default 2 = configs[1])")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    from paper_2509_07175_b200 import inputs
+    w = inputs.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2509_07175_b200 import binding
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the library has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream()
+    # inputs resident in HBM before the timed region
+    d_sites = torch.from_numpy(w.sites).to(dev)
+    d_verts = torch.from_numpy(w.verts).to(dev)
+    d_simp = torch.from_numpy(w.simplices).to(dev)
+    ctx = binding.Context(d_sites)
+    ctx.set_stream(stream.cuda_stream)
+    ctx.set_domain(d_verts, d_simp, w.kind)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        ctx.compute()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    clip_ms, launches = 0.0, 0
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)            # L2 flush between timed iterations (not timed)
+        ev[k][0].record(stream)
+        ctx.compute()
+        ev[k][1].record(stream)
+        clip_ms += ctx.stage_ms()["clip"]
+        launches += ctx.counters()["launches"]
+    barrier()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    cnt = ctx.counters()
+    stage = ctx.stage_ms()
+    cells = ctx.cells
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * w.n * args.steps / (ms * 1e-3)
+
+    # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(2, min(args.steps, 5))
+    d2h = 0
+    for _ in range(e2e_steps):
+        c2 = binding.Context(w.sites)
+        c2.set_stream(stream.cuda_stream)
+        c2.set_domain(w.verts, w.simplices, w.kind)
+        c2.compute()
+        h = c2.to_host()
+        c2.destroy()
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
+                                            "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
+    h2d = w.sites.nbytes + w.verts.nbytes + w.simplices.nbytes
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_val = world * w.n / float(t.item())
+
+    flops = algorithmic_flops(cnt, w.kind)
+    clip_s = clip_ms / args.steps * 1e-3
+    sm_max = clocks["sm_max_mhz"] or 1965.0
+    peak = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    achieved = flops / clip_s / 1e12
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "nonempty_cells": int(cells.n_nonempty), "pieces": int(cells.n_pieces), "corners": int(cells.n_verts)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(launches),
+        "stage_ms": stage, "counters": cnt,
+        "roofline": {"bound": "alu", "kernel": "k_clip (S4+S5)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": None,
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
+                     "algorithmic_flop_per_step": flops, "kernel_ms_per_step": clip_ms / args.steps,
+                     "share_of_step": clip_ms / ms},
+    }
+    ctx.destroy()
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"] = cpu_oracle_sample(w)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -9,6 +9,8 @@
 
 namespace vd {
 
+unsigned long long g_launches = 0;
+
 vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what) {
   if (e == cudaSuccess) return VD_OK;
   if (c) c->lastError = std::string(what) + ": " + cudaGetErrorString(e);
@@ -172,6 +174,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     c->nbrCap = 8 * c->pairCap;
   }
   memset(&c->counters, 0, sizeof(c->counters));
+  const unsigned long long launches0 = g_launches;
   cudaStream_t st = c->stream;
   vd_status s;
   for (int attempt = 0;; ++attempt) {
@@ -220,6 +223,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   c->counters.search_iters = (int64_t)h.cnt.search_iters; c->counters.clips = (int64_t)h.cnt.clips;
   c->counters.overflow_pairs = (int64_t)h.ovfTail;
   c->counters.reruns = reruns; c->counters.waves = waves;
+  c->counters.launches = (int64_t)(g_launches - launches0);
   vd_cells& r = c->cells;
   r.n = c->n; r.dim = c->dim; r.nfl = c->nfl;
   r.n_nonempty = (int64_t)h.nNonEmpty; r.n_pieces = (int64_t)h.nPieces; r.n_verts = (int64_t)h.nVerts; r.n_nbrs = (int64_t)h.nNbrs;

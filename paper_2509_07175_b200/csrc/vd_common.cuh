@@ -7,8 +7,9 @@
 #ifndef VD_LANES
 #define VD_LANES 32
 #endif
+namespace vd { extern unsigned long long g_launches; }   // kernels launched by this library (host counter)
 #ifndef VD_LAUNCH
-#define VD_LAUNCH(kernel, grid, block, smem, stream) kernel<<<(grid), (block), (smem), (stream)>>>
+#define VD_LAUNCH(kernel, grid, block, smem, stream) ++vd::g_launches, kernel<<<(grid), (block), (smem), (stream)>>>
 #endif
 
 namespace vd {
