@@ -24,43 +24,24 @@ __device__ __forceinline__ double slab_d2(const GridIndex& g, int ax, double q, 
   return d * d;
 }
 
-// Scan one contiguous site range [s, s+cnt) for sites closer than (best, bestId).  Uniform result.
-__device__ __forceinline__ void scan_range(const GridIndex& g, double qx, double qy, double qz, int s, int cnt,
-                                           double& best, int& bestId, QueryStats& st) {
-  st.dist_evals += (unsigned)cnt;
-  for (int k0 = 0; k0 < cnt; k0 += kLanes) {
-    const int k = k0 + lane_id();
-    double d2 = best;
-    int id = 0x7fffffff;
-    if (k < cnt) {
-      const double4 p = g.sites[s + k];
-      const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
-      d2 = dx * dx + dy * dy + dz * dz;
-      id = __double_as_longlong(p.w) & 0x7fffffff;
-    }
-    const bool better = (k < cnt) && closer(d2, id, best, bestId);
-    if (__any_sync(kFull, better)) {
-      if (!better) { d2 = best; id = bestId; }
-      warp_argmin(d2, id);
-      best = d2;
-      bestId = id;
-    }
-  }
-}
-
 // Scan every cell of the box [x0..x1]x[y0..y1]x[z0..z1] whose row can hold a site closer than best.
-// One lane per row (y,z): box-distance pruning, x-extent tightened to the ball, one contiguous range.
-__device__ __forceinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0,
-                                         int y1, int z0, int z1, double& best, int& bestId, QueryStats& st) {
+// One lane per row (y,z): box-distance pruning, x-extent tightened to the ball, one contiguous site
+// range per row.  The candidates of all rows are then packed 32 at a time over the lanes (prefix sum of
+// the row counts; the row that owns candidate t is found from a bit mask of row starts), so a typical
+// query of ~30 candidates in 4-9 rows costs one round of distance evaluations instead of one per row.
+static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0, int y1,
+                                      int z0, int z1, double& best, int& bestId, QueryStats& st) {
+  __shared__ int sBase[kWarpsPerBlock][kLanes];
+  const int lane = lane_id();
+  int* base = sBase[(threadIdx.x / kLanes) % kWarpsPerBlock];
   const int ny = y1 - y0 + 1;
   const int nrows = ny * (z1 - z0 + 1);
   for (int r0 = 0; r0 < nrows; r0 += kLanes) {
-    const int r = r0 + lane_id();
+    const int r = r0 + lane;
     int s = 0, cnt = 0;
-    double rd2 = 0.0;
     if (r < nrows) {
       const int y = y0 + r % ny, z = z0 + r / ny;
-      rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
+      const double rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
       if (!(rd2 > best)) {
         int xa = x0, xb = x1;
         if (best < 1e300) {
@@ -69,21 +50,51 @@ __device__ __forceinline__ void scan_box(const GridIndex& g, double qx, double q
           xb = min(x1, (int)floor((qx + w - g.lo[0]) * g.inv_h[0] + 1e-6));
         }
         if (xa <= xb) {
-          const int base = (z * g.G[1] + y) * g.G[0];
-          s = __ldg(&g.cellStart[base + xa]);
-          cnt = __ldg(&g.cellStart[base + xb + 1]) - s;
-          rd2 += slab_d2(g, 0, qx, xa, xb);
+          const int rowBase = (z * g.G[1] + y) * g.G[0];
+          s = __ldg(&g.cellStart[rowBase + xa]);
+          cnt = __ldg(&g.cellStart[rowBase + xb + 1]) - s;
         }
       }
     }
-    unsigned m = __ballot_sync(kFull, cnt > 0);
-    while (m) {
-      const int src = __ffs(m) - 1;
-      m &= m - 1;
-      const int ss = shfl(s, src), cc = shfl(cnt, src);
-      const double dd = shfl(rd2, src);
-      if (dd > best) continue;
-      scan_range(g, qx, qy, qz, ss, cc, best, bestId, st);
+    int incl = cnt;
+#pragma unroll
+    for (int off = 1; off < kLanes; off <<= 1) {
+      const int o = __shfl_up_sync(kFull, incl, off);
+      if (lane >= off) incl += o;
+    }
+    const int excl = incl - cnt;
+    const int total = shfl(incl, kLanes - 1);
+    st.dist_evals += (unsigned)total;
+    for (int t0 = 0; t0 < total; t0 += kLanes) {
+      // rows that start inside this chunk, plus the row that straddles its beginning
+      unsigned bit = 0;
+      if (cnt > 0) {
+        if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
+        else if (excl < t0 && incl > t0) bit = 1u;
+      }
+      const unsigned starts = __reduce_or_sync(kFull, bit);
+      const unsigned owners = __ballot_sync(kFull, bit != 0);
+      if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
+      __syncwarp();
+      const int t = t0 + lane;
+      double d2 = best;
+      int id = 0x7fffffff;
+      const bool valid = t < total;
+      if (valid) {
+        const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
+        const double4 p = g.sites[base[owner] + t];
+        const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
+        d2 = dx * dx + dy * dy + dz * dz;
+        id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
+      }
+      const bool better = valid && closer(d2, id, best, bestId);
+      if (__any_sync(kFull, better)) {
+        if (!better) { d2 = best; id = bestId; }
+        warp_argmin(d2, id);
+        best = d2;
+        bestId = id;
+      }
+      __syncwarp();
     }
   }
 }
@@ -91,7 +102,7 @@ __device__ __forceinline__ void scan_box(const GridIndex& g, double qx, double q
 // N_q: the site nearest to q among those closer than the incoming (best, bestId); ties to
 // the lowest id (reading U5).  Call with best = +inf, bestId = INT_MAX for an unbounded query, or
 // with best = |q - v_i|^2, bestId = i for a point-in-cell test (Eq. 2).
-__device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
+static __device__ __noinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                         QueryStats& st) {
   st.queries += 1;
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);

@@ -1,0 +1,45 @@
+"""Full-size BASELINE.json configs on the GPU, in the launch configuration bench.py times: global
+invariants over all cells plus element-by-element parity on sampled sites the oracle computes one by
+one (seeded-random half, extremes of the GPU report half -- choosing WHICH sites to check from the GPU
+output is harmless, the check itself is independent)."""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2509_07175_b200 import binding, inputs
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _sample(g, n, k, seed):
+    rng = np.random.default_rng(seed)
+    rnd = rng.choice(n, size=min(n, k // 2), replace=False)
+    npieces = np.diff(g.piece_off)
+    nnbr = np.diff(g.nbr_off)
+    pos = np.where(g.measure > 0)[0]
+    q = k // 8
+    ext = np.concatenate([np.argsort(-g.measure)[:q], np.argsort(-npieces)[:q], np.argsort(-nnbr)[:q],
+                          pos[np.argsort(g.measure[pos])[:q]]])
+    return np.unique(np.concatenate([rnd, ext])).astype(np.int64)
+
+
+@pytest.mark.parametrize("idx,k", [(2, 256), (4, 192), (5, 96), (3, 96)])
+def test_full_config_invariants_and_sampled_parity(idx, k):
+    w = inputs.config(idx)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        ctx.compute()
+        g = ctx.to_host()
+        cnt = ctx.counters()
+    chk = parity.global_checks(g, w)
+    assert chk["sum_measure_rel"] <= 1e-11, chk
+    assert chk["per_simplex_rel"] <= 1e-10, chk
+    assert chk["nbr_symmetric"], chk
+    assert cnt["pieces"] == len(g.piece_simplex)
+    ids = _sample(g, w.n, k, 1000 + idx)
+    tier = "A" if w.kind == inputs.KIND_TRI_SURFACE else "B"
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=ids, tier=tier)
+    bad = parity.assert_parity(g, o, w.diameter, allow_excused=1)
+    assert bad["_max_rel_measure"] <= 1e-9
