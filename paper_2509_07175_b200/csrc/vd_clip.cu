@@ -24,7 +24,7 @@ constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
 
 // items: pairs[begin .. end) when list == nullptr, else pairs[list[begin .. end)]
-template <int KIND, bool BIG>
+template <int KIND, bool BIG, bool HV>
 __global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end) {
   constexpr int W = BIG ? 1 : kWarpsPerBlock;
   __shared__ GridIndex g;
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, cons
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
     for (int64_t k = begin + warp; k < end; k += nwarps) {
       const int64_t idx = list ? (int64_t)list[k] : k;
-      const int rc = clip_pair_3d(S[w], g, A, idx, st, lc);
+      const int rc = clip_pair_3d<BIG ? P3B : P3, BIG ? C3B : C3, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
         if (BIG) {
           if (lane_id() == 0) {
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, cons
     __shared__ Poly2<BIG ? K2B : K2> S[W];
     for (int64_t k = begin + warp; k < end; k += nwarps) {
       const int64_t idx = list ? (int64_t)list[k] : k;
-      const int rc = clip_pair_2d(S[w], g, A, idx, st, lc);
+      const int rc = clip_pair_2d<BIG ? K2B : K2, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
         if (BIG) {
           if (lane_id() == 0) {
@@ -125,10 +125,10 @@ vd_status stage_seed(vd_ctx* c) {
   return cuda_check(c, cudaGetLastError(), "seed");
 }
 
-template <int KIND>
+template <int KIND, bool HV>
 static void launch_wave(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, int64_t ob, int64_t oe) {
-  if (e > b) VD_LAUNCH((k_clip<KIND, false>), blocks_for(e - b, kWarpsPerBlock, 148 * 6), kBlock, 0, c->stream)(A, nullptr, b, e);
-  if (oe > ob) VD_LAUNCH((k_clip<KIND, true>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe);
+  if (e > b) VD_LAUNCH((k_clip<KIND, false, HV>), blocks_for(e - b, kWarpsPerBlock, 148 * 6), kBlock, 0, c->stream)(A, nullptr, b, e);
+  if (oe > ob) VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe);
 }
 
 vd_status stage_clip(vd_ctx* c) {
@@ -146,8 +146,14 @@ vd_status stage_clip(vd_ctx* c) {
     if (end > c->pairCap) end = c->pairCap;
     if (oend > c->ovfCap) oend = c->ovfCap;
     if (end == begin && oend == obegin) break;   // "while L1 is not empty"
-    if (c->kind == KIND_TET_3D) launch_wave<KIND_TET_3D>(c, A, begin, end, obegin, oend);
-    else launch_wave<KIND_TRI_2D>(c, A, begin, end, obegin, oend);
+    const bool hv = h.nHeavy > 0;   // refined cells exist: the kernels that know the second index level
+    if (c->kind == KIND_TET_3D) {
+      if (hv) launch_wave<KIND_TET_3D, true>(c, A, begin, end, obegin, oend);
+      else launch_wave<KIND_TET_3D, false>(c, A, begin, end, obegin, oend);
+    } else {
+      if (hv) launch_wave<KIND_TRI_2D, true>(c, A, begin, end, obegin, oend);
+      else launch_wave<KIND_TRI_2D, false>(c, A, begin, end, obegin, oend);
+    }
     begin = end;
     obegin = oend;
     ++waves;

@@ -32,7 +32,7 @@ __device__ __forceinline__ void lerp_to_plane(double cx, double cy, double cz, d
   x = cx + t * (bx - cx); y = cy + t * (by - cy); z = cz + t * (bz - cz);
 }
 
-template <int K>
+template <int K, bool HV>
 __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = A.pairs[pairIdx];
@@ -80,7 +80,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
 #ifdef VD_TRACE
   {
     double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0u, 0u};
-    nearest(g, pr.wx, pr.wy, pr.wz, b, bi, s2);
+    nearest<HV>(g, pr.wx, pr.wy, pr.wz, b, bi, s2);
     const double dx = pr.wx - six, dy = pr.wy - siy, dz = pr.wz - siz;
     const double di = dx * dx + dy * dy + dz * dz;
     if (lane == 0 && bi != i && di - b > 1e-13) printf("BAD WITNESS pair(%d,%d) w=(%g,%g) nearest=%d di2=%g best=%g\n", a, i, pr.wx, pr.wy, bi, di, b);
@@ -95,7 +95,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
       const double dx = qx - six, dy = qy - siy, dz = qz - siz;
       double best = dx * dx + dy * dy + dz * dz;
       int bestId = i;
-      nearest(g, qx, qy, qz, best, bestId, st);
+      nearest<HV>(g, qx, qy, qz, best, bestId, st);
       bool inside = bestId == i;
       if (!inside) {
         bool own = false;
@@ -124,7 +124,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     double psx = wx, psy = wy, psz = wz;
     if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
     double nx, ny, nz, d;
-    const int j = find_bisector(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
+    const int j = find_bisector<HV>(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
                                 nx, ny, nz, d, st, lc);
     if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
     bool own = false;

@@ -318,7 +318,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
 }
 
 // returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
-template <int P, int C>
+template <int P, int C, bool HV>
 __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = A.pairs[pairIdx];
@@ -380,7 +380,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
         const double dx = qx - six, dy = qy - siy, dz = qz - siz;
         double best = dx * dx + dy * dy + dz * dz;
         int bestId = i;
-        nearest(g, qx, qy, qz, best, bestId, st);
+        nearest<HV>(g, qx, qy, qz, best, bestId, st);
         bool inside = bestId == i;
         if (!inside) {
           // flag rule in the form of reading U6: N_q already owns a plane of P
@@ -417,7 +417,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
     double psx = wx, psy = wy, psz = wz;
     if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
     double nx, ny, nz, d;
-    const int j = find_bisector(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
+    const int j = find_bisector<HV>(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
                                 nx, ny, nz, d, st, lc);
     if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
     {

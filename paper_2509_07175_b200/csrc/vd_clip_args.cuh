@@ -64,6 +64,7 @@ __device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, doubl
 // the segment lies in P, and P is inside H_ik for every site k that owns one of them, so N_q = v_k can
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
+template <bool HV>
 static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, double ox, double oy, double oz,
                                              double vix, double viy, double viz,   // v_i local
                                              double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
@@ -88,7 +89,7 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
-    nearest(g, ax, ay, az, best, bestId, st);
+    nearest<HV>(g, ax, ay, az, best, bestId, st);
 #ifdef VD_TRACE
     if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
 #endif

@@ -43,7 +43,14 @@ struct GridIndex {
   int n;
   const int* __restrict__ cellStart;      // [G0*G1*G2 + 1]
   const double4* __restrict__ sites;      // sorted; w = original id (as int bits)
+  // second level (clustered sites): a cell holding more than kHeavy sites carries its own K^3 sub-grid;
+  // its sites are sorted by sub-cell, subStart holds absolute first-site indices (K^3 + 1 entries)
+  const int* __restrict__ heavyPrefix;    // [G0*G1*G2 + 1] number of refined cells below a cell index (null: no second level)
+  const int* __restrict__ subOff;         // [G0*G1*G2] (K << 26) | offset into subStart, or -1
+  const int* __restrict__ subStart;
 };
+
+constexpr int kHeavy = 32;                // sites per cell above which the cell is refined (one warp round)
 
 // One unit of work: simplex a, site i, and a witness point w in T_a ∩ Ω_i
 // (DESIGN.md "witness"): the start p_s of virtual edges instead of v_i (Alg. 3 line 3).

@@ -87,6 +87,9 @@ __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64
   out.n = (int)n;
   out.cellStart = cellStart;
   out.sites = sorted;
+  out.heavyPrefix = nullptr;
+  out.subOff = nullptr;
+  out.subStart = nullptr;
   *g = out;
 }
 
@@ -116,6 +119,123 @@ __global__ void __launch_bounds__(kBlock) k_cell_scatter(const double* __restric
   }
 }
 
+// ---- second level: cells with more than kHeavy sites get a K^3 sub-grid (clustered site sets: a uniform
+// grid at the paper's density leaves thousands of sites in one cell).  K is chosen so that a sub-cell holds
+// `density` sites on average; the cell's sites are re-sorted by sub-cell key.
+__device__ __forceinline__ int sub_k(int cnt, double density, int nd) {
+  const double t = (double)cnt / density;
+  int K = (int)ceil(nd == 3 ? cbrt(t) : (nd == 2 ? sqrt(t) : t));
+  return min(max(K, 2), 31);
+}
+
+__global__ void __launch_bounds__(kBlock) k_sub_plan(const GridIndex* __restrict__ gp, double density, int64_t gridCap,
+                                                      int* __restrict__ heavyFlag, int* __restrict__ need) {
+  const GridIndex g = *gp;
+  const int64_t G = (int64_t)g.G[0] * g.G[1] * g.G[2];
+  const int nd = (g.h[0] > 0) + (g.h[1] > 0) + (g.h[2] > 0);
+  for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c <= gridCap; c += (int64_t)gridDim.x * blockDim.x) {
+    int hv = 0, nd3 = 0;
+    if (c < G) {
+      const int cnt = g.cellStart[c + 1] - g.cellStart[c];
+      if (cnt > kHeavy && nd > 0) {
+        const int K = sub_k(cnt, density, nd);
+        hv = 1;
+        nd3 = (g.h[0] > 0 ? K : 1) * (g.h[1] > 0 ? K : 1) * (g.h[2] > 0 ? K : 1) + 1;
+      }
+    }
+    heavyFlag[c] = hv;
+    need[c] = nd3;
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_sub_pack(const GridIndex* __restrict__ gp, double density, const int* __restrict__ offRaw,
+                                                      int64_t subCap, int* __restrict__ subOff) {
+  const GridIndex g = *gp;
+  const int64_t G = (int64_t)g.G[0] * g.G[1] * g.G[2];
+  const int nd = (g.h[0] > 0) + (g.h[1] > 0) + (g.h[2] > 0);
+  for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < G; c += (int64_t)gridDim.x * blockDim.x) {
+    const int cnt = g.cellStart[c + 1] - g.cellStart[c];
+    int v = -1;
+    if (cnt > kHeavy && nd > 0 && (int64_t)offRaw[c + 1] <= subCap) v = (sub_k(cnt, density, nd) << 26) | offRaw[c];
+    subOff[c] = v;
+  }
+}
+
+__device__ __forceinline__ int sub_key(const GridIndex& g, int c, int K, double x, double y, double z) {
+  const int cx = c % g.G[0], cy = (c / g.G[0]) % g.G[1], cz = c / (g.G[0] * g.G[1]);
+  const int Kx = g.h[0] > 0 ? K : 1, Ky = g.h[1] > 0 ? K : 1, Kz = g.h[2] > 0 ? K : 1;
+  const int kx = min(max((int)floor((x - (g.lo[0] + cx * g.h[0])) * (Kx * g.inv_h[0])), 0), Kx - 1);
+  const int ky = min(max((int)floor((y - (g.lo[1] + cy * g.h[1])) * (Ky * g.inv_h[1])), 0), Ky - 1);
+  const int kz = min(max((int)floor((z - (g.lo[2] + cz * g.h[2])) * (Kz * g.inv_h[2])), 0), Kz - 1);
+  return (kz * Ky + ky) * Kx + kx;
+}
+
+// sites are in top-cell order in `sorted`; p = position there
+__global__ void __launch_bounds__(kBlock) k_sub_count(const GridIndex* __restrict__ gp, const double4* __restrict__ sorted, int64_t n,
+                                                       const int* __restrict__ cellOf, const int* __restrict__ subOff,
+                                                       int* __restrict__ subKey, int* __restrict__ subCount) {
+  const GridIndex g = *gp;
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+    const double4 s = sorted[p];
+    const int id = (int)(__double_as_longlong(s.w) & 0x7fffffff);
+    const int c = cellOf[id];
+    const int so = subOff[c];
+    int key = -1;
+    if (so >= 0) {
+      key = sub_key(g, c, so >> 26, s.x, s.y, s.z);
+      atomicAdd(&subCount[(so & 0x3ffffff) + key], 1);
+    }
+    subKey[p] = key;
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_sub_scatter(const double4* __restrict__ sorted, int64_t n, const int* __restrict__ cellOf,
+                                                         const int* __restrict__ cellStart, const int* __restrict__ subOff,
+                                                         const int* __restrict__ subKey, const int* __restrict__ subScan,
+                                                         int* __restrict__ subCount, double4* __restrict__ sorted2) {
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+    const double4 s = sorted[p];
+    const int key = subKey[p];
+    int64_t dst = p;
+    if (key >= 0) {
+      const int id = (int)(__double_as_longlong(s.w) & 0x7fffffff);
+      const int c = cellOf[id];
+      const int off = subOff[c] & 0x3ffffff;
+      dst = cellStart[c] + (subScan[off + key] - subScan[off]) + (atomicSub(&subCount[off + key], 1) - 1);
+    }
+    sorted2[dst] = s;
+  }
+}
+
+// subScan (exclusive scan of the sub-cell counts, all refined cells concatenated) -> absolute start indices
+__global__ void __launch_bounds__(kBlock) k_sub_finalize(const GridIndex* __restrict__ gp, const int* __restrict__ subOff,
+                                                          const int* __restrict__ subScan, int* __restrict__ subStart) {
+  const GridIndex g = *gp;
+  const int64_t G = (int64_t)g.G[0] * g.G[1] * g.G[2];
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
+  for (int64_t c = warp; c < G; c += nwarps) {
+    const int so = subOff[c];
+    if (so < 0) continue;
+    const int K = so >> 26, off = so & 0x3ffffff;
+    const int cells = (g.h[0] > 0 ? K : 1) * (g.h[1] > 0 ? K : 1) * (g.h[2] > 0 ? K : 1);
+    const int base = subScan[off], start = g.cellStart[c];
+    __syncwarp();   // every lane holds the base before entry 0 is rewritten in place
+    for (int k = lane_id(); k <= cells; k += kLanes) subStart[off + k] = start + subScan[off + k] - base;
+  }
+}
+
+__global__ void k_grid_finish(GridIndex* g, const double4* sorted2, const int* heavyPrefix, const int* subOff, const int* subStart,
+                              unsigned int* nHeavy) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    *nHeavy = (unsigned int)heavyPrefix[(int64_t)g->G[0] * g->G[1] * g->G[2]];
+    g->sites = sorted2;
+    g->heavyPrefix = heavyPrefix;
+    g->subOff = subOff;
+    g->subStart = subStart;
+  }
+}
+
 // S2 as a kernel: one warp per query point.
 __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __restrict__ gp, const double* __restrict__ q3, int64_t nq,
                                                             int* __restrict__ out, Counters* cnt) {
@@ -126,7 +246,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
   for (int64_t q = warp; q < nq; q += nwarps) {
     double best = 2e300;
     int bestId = 0x7fffffff;
-    nearest(g, q3[q * 3 + 0], q3[q * 3 + 1], q3[q * 3 + 2], best, bestId, st);
+    nearest<true>(g, q3[q * 3 + 0], q3[q * 3 + 1], q3[q * 3 + 2], best, bestId, st);
     if (lane_id() == 0) out[q] = bestId;
   }
   if (lane_id() == 0 && cnt) {
@@ -168,6 +288,37 @@ vd_status stage_index(vd_ctx* c) {
   exclusive_scan<int, int>(c->cellFill.as<int>(), gridCap + 1, c->cellStart.as<int>(), c->scanTmp.as<int>(), st);
   VD_LAUNCH(k_cell_scatter, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->cellOf.as<int>(), c->cellStart.as<int>(),
                                                                 c->cellFill.as<int>(), c->sorted.as<double4>());
+  // second level
+  const int64_t subCap = (int64_t)(4.0 * (double)n / density) + gridCap + 64;
+  c->subCap = subCap;
+  if ((s = ensure(c, c->heavyFlag, sizeof(int) * (gridCap + 2)))) return s;
+  if ((s = ensure(c, c->heavyPrefix, sizeof(int) * (gridCap + 3)))) return s;
+  if ((s = ensure(c, c->subNeed, sizeof(int) * (gridCap + 2)))) return s;
+  if ((s = ensure(c, c->subOffRaw, sizeof(int) * (gridCap + 3)))) return s;
+  if ((s = ensure(c, c->subOff, sizeof(int) * (gridCap + 2)))) return s;
+  if ((s = ensure(c, c->subCount, sizeof(int) * (subCap + 2)))) return s;
+  if ((s = ensure(c, c->subStart, sizeof(int) * (subCap + 3)))) return s;
+  if ((s = ensure(c, c->subKey, sizeof(int) * n))) return s;
+  if ((s = ensure(c, c->sorted2, sizeof(double4) * n))) return s;
+  if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(subCap > n ? subCap : n) * 2))) return s;
+  GridIndex* gp = c->grid.as<GridIndex>();
+  const int gb = grid_for(gridCap + 1, kBlock);
+  VD_LAUNCH(k_sub_plan, gb, kBlock, 0, st)(gp, density, gridCap, c->heavyFlag.as<int>(), c->subNeed.as<int>());
+  exclusive_scan<int, int>(c->heavyFlag.as<int>(), gridCap + 1, c->heavyPrefix.as<int>(), c->scanTmp.as<int>(), st);
+  exclusive_scan<int, int>(c->subNeed.as<int>(), gridCap + 1, c->subOffRaw.as<int>(), c->scanTmp.as<int>(), st);
+  VD_LAUNCH(k_sub_pack, gb, kBlock, 0, st)(gp, density, c->subOffRaw.as<int>(), subCap, c->subOff.as<int>());
+  cudaMemsetAsync(c->subCount.p, 0, sizeof(int) * (subCap + 2), st);
+  VD_LAUNCH(k_sub_count, grid_for(n, kBlock), kBlock, 0, st)(gp, c->sorted.as<double4>(), n, c->cellOf.as<int>(), c->subOff.as<int>(),
+                                                             c->subKey.as<int>(), c->subCount.as<int>());
+  exclusive_scan<int, int>(c->subCount.as<int>(), subCap + 1, c->subStart.as<int>(), c->scanTmp.as<int>(), st);
+  // subStart holds the scan for now; the scatter consumes subCount as a cursor, then the scan is rebased in place
+  VD_LAUNCH(k_sub_scatter, grid_for(n, kBlock), kBlock, 0, st)(c->sorted.as<double4>(), n, c->cellOf.as<int>(), c->cellStart.as<int>(),
+                                                               c->subOff.as<int>(), c->subKey.as<int>(), c->subStart.as<int>(),
+                                                               c->subCount.as<int>(), c->sorted2.as<double4>());
+  VD_LAUNCH(k_sub_finalize, grid_for(gridCap, kWarpsPerBlock), kBlock, 0, st)(gp, c->subOff.as<int>(), c->subStart.as<int>(),
+                                                                               c->subStart.as<int>());
+  VD_LAUNCH(k_grid_finish, 1, 1, 0, st)(gp, c->sorted2.as<double4>(), c->heavyPrefix.as<int>(), c->subOff.as<int>(),
+                                         c->subStart.as<int>(), &c->control.as<Control>()->nHeavy);
   c->indexValid = true;
   return cuda_check(c, cudaGetLastError(), "site index");
 }

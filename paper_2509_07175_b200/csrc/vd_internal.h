@@ -14,7 +14,7 @@ struct Control {
   unsigned long long vertTail;   // corners allocated in the pool
   unsigned long long nbrTail;    // face flags allocated in the pool
   unsigned int err;              // ERR_* bits
-  unsigned int pad;
+  unsigned int nHeavy;           // refined cells of the site index (second level)
   Counters cnt;
   unsigned long long nPieces, nNonEmpty, nVerts, nNbrs;   // totals written by S6
 };
@@ -56,6 +56,8 @@ struct vd_ctx {
   vd::DevBuf cellFill;    // int [gridCap+1]
   vd::DevBuf sorted;      // double4 [n]
   vd::DevBuf scanTmp;     // scan scratch
+  vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart, subKey, sorted2;   // second level
+  int64_t subCap = 0;
   // S3-S5
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
   vd::DevBuf control;     // Control

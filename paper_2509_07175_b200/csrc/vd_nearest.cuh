@@ -29,6 +29,13 @@ __device__ __forceinline__ double slab_d2(const GridIndex& g, int ax, double q, 
 // range per row.  The candidates of all rows are then packed 32 at a time over the lanes (prefix sum of
 // the row counts; the row that owns candidate t is found from a bit mask of row starts), so a typical
 // query of ~30 candidates in 4-9 rows costs one round of distance evaluations instead of one per row.
+static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
+                                              int& bestId, QueryStats& st);
+
+// TOP = true: g is the site index itself and may hold refined cells (second level); a row that contains
+// one is walked cell by cell afterwards: plain cells are scanned as they are, a refined cell through its
+// own sub-grid (the same routine with TOP = false on a view of that cell).
+template <bool TOP>
 static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0, int y1,
                                       int z0, int z1, double& best, int& bestId, QueryStats& st) {
   __shared__ int sBase[kWarpsPerBlock][kLanes];
@@ -39,6 +46,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
   for (int r0 = 0; r0 < nrows; r0 += kLanes) {
     const int r = r0 + lane;
     int s = 0, cnt = 0;
+    int hxa = 0, hxb = -1;   // x extent of a row that holds refined cells
     if (r < nrows) {
       const int y = y0 + r % ny, z = z0 + r / ny;
       const double rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
@@ -53,6 +61,10 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
           const int rowBase = (z * g.G[1] + y) * g.G[0];
           s = __ldg(&g.cellStart[rowBase + xa]);
           cnt = __ldg(&g.cellStart[rowBase + xb + 1]) - s;
+          if (TOP && g.heavyPrefix && cnt > kHeavy &&
+              __ldg(&g.heavyPrefix[rowBase + xb + 1]) != __ldg(&g.heavyPrefix[rowBase + xa])) {
+            cnt = 0; hxa = xa; hxb = xb;
+          }
         }
       }
     }
@@ -96,16 +108,86 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
       }
       __syncwarp();
     }
+    if (TOP) {
+      unsigned hm = __ballot_sync(kFull, hxa <= hxb);
+      while (hm) {
+        const int src = __ffs(hm) - 1;
+        hm &= hm - 1;
+        const int rr = r0 + src;
+        const int y = y0 + rr % ny, z = z0 + rr / ny;
+        const int xa = shfl(hxa, src), xb = shfl(hxb, src);
+        for (int x = xa; x <= xb; ++x) scan_cell(g, x, y, z, qx, qy, qz, best, bestId, st);
+      }
+    }
   }
+}
+
+// View of a refined cell's sub-grid as a grid of its own.
+__device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z, int so, GridIndex& v) {
+  const int K = so >> 26;
+  const int cc[3] = {x, y, z};
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const int Ka = g.h[a] > 0 ? K : 1;
+    v.lo[a] = g.lo[a] + cc[a] * g.h[a];
+    v.h[a] = g.h[a] / Ka;
+    v.inv_h[a] = Ka * g.inv_h[a];
+    v.hi[a] = v.lo[a] + g.h[a];
+    v.G[a] = Ka;
+  }
+  v.n = 0;
+  v.cellStart = g.subStart + (so & 0x3ffffff);
+  v.sites = g.sites;
+  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr;
+}
+
+// One cell of the top grid: a plain cell is scanned directly, a refined cell through its sub-grid,
+// restricted to the ball (q, sqrt(best)).
+static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
+                                              int& bestId, QueryStats& st) {
+  const int c = (z * g.G[1] + y) * g.G[0] + x;
+  if (slab_d2(g, 0, qx, x, x) + slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z) > best) return;
+  const int so = __ldg(&g.subOff[c]);
+  if (so < 0) {
+    scan_box<false>(g, qx, qy, qz, x, x, y, y, z, z, best, bestId, st);   // plain cell: a 1 x 1 x 1 box of the top grid
+    return;
+  }
+  GridIndex v;
+  sub_view(g, x, y, z, so, v);
+  int vx0 = 0, vx1 = v.G[0] - 1, vy0 = 0, vy1 = v.G[1] - 1, vz0 = 0, vz1 = v.G[2] - 1;
+  if (best < 1e300) {
+    const double r = sqrt(best);
+    vx0 = cell_of(v, 0, qx - r - 1e-6 * v.h[0]); vx1 = cell_of(v, 0, qx + r + 1e-6 * v.h[0]);
+    vy0 = cell_of(v, 1, qy - r - 1e-6 * v.h[1]); vy1 = cell_of(v, 1, qy + r + 1e-6 * v.h[1]);
+    vz0 = cell_of(v, 2, qz - r - 1e-6 * v.h[2]); vz1 = cell_of(v, 2, qz + r + 1e-6 * v.h[2]);
+  }
+  scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
+}
+
+// The 3 x 3 x 3 sub-cells around q inside its (refined) home cell: tightens a loose bound cheaply.
+static __device__ __noinline__ void probe_cell(const GridIndex& g, int x, int y, int z, int so, double qx, double qy, double qz,
+                                               double& best, int& bestId, QueryStats& st) {
+  GridIndex v;
+  sub_view(g, x, y, z, so, v);
+  const int hx = cell_of(v, 0, qx), hy = cell_of(v, 1, qy), hz = cell_of(v, 2, qz);
+  scan_box<false>(v, qx, qy, qz, max(hx - 1, 0), min(hx + 1, v.G[0] - 1), max(hy - 1, 0), min(hy + 1, v.G[1] - 1), max(hz - 1, 0),
+                  min(hz + 1, v.G[2] - 1), best, bestId, st);
 }
 
 // N_q: the site nearest to q among those closer than the incoming (best, bestId); ties to
 // the lowest id (reading U5).  Call with best = +inf, bestId = INT_MAX for an unbounded query, or
 // with best = |q - v_i|^2, bestId = i for a point-in-cell test (Eq. 2).
+template <bool HV>
 static __device__ __noinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                         QueryStats& st) {
   st.queries += 1;
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);
+  if (HV) {
+    // refined home cell: look at the sub-cells around q first, so that a loose bound does not make the
+    // ball span thousands of sub-grid rows
+    const int so = __ldg(&g.subOff[(cz * g.G[1] + cy) * g.G[0] + cx]);
+    if (so >= 0) probe_cell(g, cx, cy, cz, so, qx, qy, qz, best, bestId, st);
+  }
   // how far q lies outside the grid box on each axis
   const double ox = fmax(fmax(g.lo[0] - qx, qx - g.hi[0]), 0.0);
   const double oy = fmax(fmax(g.lo[1] - qy, qy - g.hi[1]), 0.0);
@@ -145,18 +227,18 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
       const int xl = cx - s, xr = cx + s;
       const int xa = max(xl, 0), xb = min(xr, g.G[0] - 1);
       if (s == 0) {
-        scan_box(g, qx, qy, qz, xa, xb, y0, y1, z0, z1, sb, si, st);
+        scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, z0, z1, sb, si, st);
       } else {
-        if (cz - s >= 0) scan_box(g, qx, qy, qz, xa, xb, y0, y1, cz - s, cz - s, sb, si, st);
-        if (cz + s < g.G[2]) scan_box(g, qx, qy, qz, xa, xb, y0, y1, cz + s, cz + s, sb, si, st);
+        if (cz - s >= 0) scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, cz - s, cz - s, sb, si, st);
+        if (cz + s < g.G[2]) scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, cz + s, cz + s, sb, si, st);
         const int zi0 = max(cz - s + 1, 0), zi1 = min(cz + s - 1, g.G[2] - 1);
         if (zi0 <= zi1) {
-          if (cy - s >= 0) scan_box(g, qx, qy, qz, xa, xb, cy - s, cy - s, zi0, zi1, sb, si, st);
-          if (cy + s < g.G[1]) scan_box(g, qx, qy, qz, xa, xb, cy + s, cy + s, zi0, zi1, sb, si, st);
+          if (cy - s >= 0) scan_box<HV>(g, qx, qy, qz, xa, xb, cy - s, cy - s, zi0, zi1, sb, si, st);
+          if (cy + s < g.G[1]) scan_box<HV>(g, qx, qy, qz, xa, xb, cy + s, cy + s, zi0, zi1, sb, si, st);
           const int yi0 = max(cy - s + 1, 0), yi1 = min(cy + s - 1, g.G[1] - 1);
           if (yi0 <= yi1) {
-            if (xl >= 0) scan_box(g, qx, qy, qz, xl, xl, yi0, yi1, zi0, zi1, sb, si, st);
-            if (xr < g.G[0]) scan_box(g, qx, qy, qz, xr, xr, yi0, yi1, zi0, zi1, sb, si, st);
+            if (xl >= 0) scan_box<HV>(g, qx, qy, qz, xl, xl, yi0, yi1, zi0, zi1, sb, si, st);
+            if (xr < g.G[0]) scan_box<HV>(g, qx, qy, qz, xr, xr, yi0, yi1, zi0, zi1, sb, si, st);
           }
         }
       }
@@ -169,7 +251,7 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
   const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
   const int y0 = cell_of(g, 1, qy - r - 1e-6 * g.h[1]), y1 = cell_of(g, 1, qy + r + 1e-6 * g.h[1]);
   const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
-  scan_box(g, qx, qy, qz, x0, x1, y0, y1, z0, z1, best, bestId, st);
+  scan_box<HV>(g, qx, qy, qz, x0, x1, y0, y1, z0, z1, best, bestId, st);
 }
 
 }  // namespace vd
