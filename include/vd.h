@@ -99,7 +99,8 @@ typedef struct vd_counters {
   int64_t overflow_pairs; /* pairs that needed the large-capacity path                             */
   int64_t reruns;         /* times the whole compute was repeated after growing a pool            */
   int64_t launches;       /* kernels this library launched inside the last vd_compute               */
-  int64_t reserved[6];
+  int64_t row_evals;      /* grid rows examined by those queries (index efficiency)                    */
+  int64_t reserved[5];
 } vd_counters;
 
 /* vd_create: copy n sites of dimension dim (row-major [n][dim], fp64).  Builds nothing heavy: the

@@ -49,7 +49,7 @@ class vd_options(ctypes.Structure):
 
 class vd_counters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips",
-                                               "waves", "overflow_pairs", "reruns", "launches")] + [("reserved", ctypes.c_int64 * 6)]
+                                               "waves", "overflow_pairs", "reruns", "launches", "row_evals")] + [("reserved", ctypes.c_int64 * 5)]
 
 
 def load():

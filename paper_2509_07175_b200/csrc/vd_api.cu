@@ -220,6 +220,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   const int64_t reruns = c->counters.reruns, waves = c->counters.waves;
   c->counters.pairs = (int64_t)h.cnt.pairs; c->counters.pieces = (int64_t)h.cnt.pieces;
   c->counters.queries = (int64_t)h.cnt.queries; c->counters.dist_evals = (int64_t)h.cnt.dist_evals;
+  c->counters.row_evals = (int64_t)h.cnt.rows;
   c->counters.search_iters = (int64_t)h.cnt.search_iters; c->counters.clips = (int64_t)h.cnt.clips;
   c->counters.overflow_pairs = (int64_t)h.ovfTail;
   c->counters.reruns = reruns; c->counters.waves = waves;

@@ -25,19 +25,22 @@ constexpr int K2 = 32, K2B = 256;
 
 // items: pairs[begin .. end) when list == nullptr, else pairs[list[begin .. end)]
 template <int KIND, bool BIG, bool HV>
-__global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end) {
+__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end) {
   constexpr int W = BIG ? 1 : kWarpsPerBlock;
   __shared__ GridIndex g;
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes;
-  const int64_t warp = (int64_t)blockIdx.x * W + w;
-  const int64_t nwarps = (int64_t)gridDim.x * W;
-  QueryStats st = {0u, 0u};
+  QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u};
   if constexpr (KIND == KIND_TET_3D) {
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
-    for (int64_t k = begin + warp; k < end; k += nwarps) {
+    for (;;) {
+      // dynamic work distribution: pieces range from 4 to hundreds of corners
+      unsigned long long t = 0;
+      if (lane_id() == 0) t = atomicAdd(&A.ctl->fetch[BIG ? 1 : 0], 1ull);
+      const int64_t k = begin + (int64_t)shfl(t, 0);
+      if (k >= end) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
       const int rc = clip_pair_3d<BIG ? P3B : P3, BIG ? C3B : C3, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
@@ -57,7 +60,11 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock) k_clip(ClipArgs A, cons
     }
   } else {
     __shared__ Poly2<BIG ? K2B : K2> S[W];
-    for (int64_t k = begin + warp; k < end; k += nwarps) {
+    for (;;) {
+      unsigned long long t = 0;
+      if (lane_id() == 0) t = atomicAdd(&A.ctl->fetch[BIG ? 1 : 0], 1ull);
+      const int64_t k = begin + (int64_t)shfl(t, 0);
+      if (k >= end) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
       const int rc = clip_pair_2d<BIG ? K2B : K2, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
@@ -127,6 +134,7 @@ vd_status stage_seed(vd_ctx* c) {
 
 template <int KIND, bool HV>
 static void launch_wave(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, int64_t ob, int64_t oe) {
+  cudaMemsetAsync(&c->control.as<Control>()->fetch[0], 0, 2 * sizeof(unsigned long long), c->stream);
   if (e > b) VD_LAUNCH((k_clip<KIND, false, HV>), blocks_for(e - b, kWarpsPerBlock, 148 * 6), kBlock, 0, c->stream)(A, nullptr, b, e);
   if (oe > ob) VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe);
 }

@@ -79,7 +79,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
   bool failed = false;
 #ifdef VD_TRACE
   {
-    double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0u, 0u};
+    double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0u, 0u, 0u};
     nearest<HV>(g, pr.wx, pr.wy, pr.wz, b, bi, s2);
     const double dx = pr.wx - six, dy = pr.wy - siy, dz = pr.wz - siz;
     const double di = dx * dx + dy * dy + dz * dz;
@@ -95,7 +95,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
       const double dx = qx - six, dy = qy - siy, dz = qz - siz;
       double best = dx * dx + dy * dy + dz * dz;
       int bestId = i;
-      nearest<HV>(g, qx, qy, qz, best, bestId, st);
+      nearest<HV>(g, qx, qy, qz, best, bestId, st, true);
       bool inside = bestId == i;
       if (!inside) {
         bool own = false;

@@ -380,7 +380,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
         const double dx = qx - six, dy = qy - siy, dz = qz - siz;
         double best = dx * dx + dy * dy + dz * dz;
         int bestId = i;
-        nearest<HV>(g, qx, qy, qz, best, bestId, st);
+        nearest<HV>(g, qx, qy, qz, best, bestId, st, true);
         bool inside = bestId == i;
         if (!inside) {
           // flag rule in the form of reading U6: N_q already owns a plane of P

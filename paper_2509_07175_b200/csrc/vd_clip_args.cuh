@@ -42,6 +42,7 @@ __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& s
     atomicAdd(&ctl->cnt.clips, (unsigned long long)lc.clips);
     atomicAdd(&ctl->cnt.queries, (unsigned long long)st.queries);
     atomicAdd(&ctl->cnt.dist_evals, (unsigned long long)st.dist_evals);
+    atomicAdd(&ctl->cnt.rows, (unsigned long long)st.rows);
   }
 }
 
@@ -89,7 +90,7 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
-    nearest<HV>(g, ax, ay, az, best, bestId, st);
+    nearest<HV>(g, ax, ay, az, best, bestId, st, true);
 #ifdef VD_TRACE
     if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
 #endif

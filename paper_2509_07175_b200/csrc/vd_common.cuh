@@ -50,7 +50,7 @@ struct GridIndex {
   const int* __restrict__ subStart;
 };
 
-constexpr int kHeavy = 32;                // sites per cell above which the cell is refined (one warp round)
+constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
 
 // One unit of work: simplex a, site i, and a witness point w in T_a ∩ Ω_i
 // (DESIGN.md "witness"): the start p_s of virtual edges instead of v_i (Alg. 3 line 3).
@@ -70,7 +70,7 @@ struct Piece {
 };
 
 struct Counters {
-  unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs;
+  unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs, rows;
 };
 
 __device__ __forceinline__ int lane_id() { return (int)(threadIdx.x % kLanes); }

@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
   const GridIndex g = *gp;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
-  QueryStats st = {0u, 0u};
+  QueryStats st = {0u, 0u, 0u};
   for (int64_t q = warp; q < nq; q += nwarps) {
     double best = 2e300;
     int bestId = 0x7fffffff;

@@ -13,6 +13,7 @@ struct Control {
   unsigned long long ovfTail;    // pairs deferred to the large-capacity path
   unsigned long long vertTail;   // corners allocated in the pool
   unsigned long long nbrTail;    // face flags allocated in the pool
+  unsigned long long fetch[2];   // work cursors of the running wave: fast tier, large tier
   unsigned int err;              // ERR_* bits
   unsigned int nHeavy;           // refined cells of the site index (second level)
   Counters cnt;

@@ -7,7 +7,7 @@
 namespace vd {
 
 struct QueryStats {
-  unsigned queries, dist_evals;
+  unsigned queries, dist_evals, rows;
 };
 
 __device__ __forceinline__ int cell_of(const GridIndex& g, int ax, double q) {
@@ -43,12 +43,14 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
   int* base = sBase[(threadIdx.x / kLanes) % kWarpsPerBlock];
   const int ny = y1 - y0 + 1;
   const int nrows = ny * (z1 - z0 + 1);
+  st.rows += (unsigned)nrows;
   for (int r0 = 0; r0 < nrows; r0 += kLanes) {
     const int r = r0 + lane;
     int s = 0, cnt = 0;
     int hxa = 0, hxb = -1;   // x extent of a row that holds refined cells
     if (r < nrows) {
-      const int y = y0 + r % ny, z = z0 + r / ny;
+      const int rz = __float2int_rz(__fdividef((float)r + 0.5f, (float)ny));   // r / ny without the integer-division sequence
+      const int y = y0 + (r - rz * ny), z = z0 + rz;
       const double rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
       if (!(rd2 > best)) {
         int xa = x0, xb = x1;
@@ -130,7 +132,7 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
   for (int a = 0; a < 3; ++a) {
     const int Ka = g.h[a] > 0 ? K : 1;
     v.lo[a] = g.lo[a] + cc[a] * g.h[a];
-    v.h[a] = g.h[a] / Ka;
+    v.h[a] = g.h[a] * (1.0 / Ka);
     v.inv_h[a] = Ka * g.inv_h[a];
     v.hi[a] = v.lo[a] + g.h[a];
     v.G[a] = Ka;
@@ -164,29 +166,52 @@ static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, 
   scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
 }
 
-// The 3 x 3 x 3 sub-cells around q inside its (refined) home cell: tightens a loose bound cheaply.
-static __device__ __noinline__ void probe_cell(const GridIndex& g, int x, int y, int z, int so, double qx, double qy, double qz,
-                                               double& best, int& bestId, QueryStats& st) {
-  GridIndex v;
-  sub_view(g, x, y, z, so, v);
-  const int hx = cell_of(v, 0, qx), hy = cell_of(v, 1, qy), hz = cell_of(v, 2, qz);
-  scan_box<false>(v, qx, qy, qz, max(hx - 1, 0), min(hx + 1, v.G[0] - 1), max(hy - 1, 0), min(hy + 1, v.G[1] - 1), max(hz - 1, 0),
-                  min(hz + 1, v.G[2] - 1), best, bestId, st);
-}
-
 // N_q: the site nearest to q among those closer than the incoming (best, bestId); ties to
 // the lowest id (reading U5).  Call with best = +inf, bestId = INT_MAX for an unbounded query, or
 // with best = |q - v_i|^2, bestId = i for a point-in-cell test (Eq. 2).
+// nearer_ok: the caller only needs SOME site clearly nearer than the incoming bound when one exists (a
+// corner that is outside Omega_i, an intermediate step of the bisector search): the routine then returns as
+// soon as the cells around q have produced one, without proving it the nearest (reading U17).  When no
+// site is clearly nearer, the full scan runs and the answer is exact, so acceptance is always exact.
 template <bool HV>
 static __device__ __noinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
-                                        QueryStats& st) {
+                                        QueryStats& st, bool nearer_ok = false) {
+  const double bound0 = best;
   st.queries += 1;
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);
   if (HV) {
-    // refined home cell: look at the sub-cells around q first, so that a loose bound does not make the
-    // ball span thousands of sub-grid rows
+    // Refined home cell (dense cluster): work in its sub-grid.  If the ball lies inside the home cell,
+    // the sub-grid alone decides; a loose bound is first tightened on the 3 x 3 x 3 sub-cells around q.
     const int so = __ldg(&g.subOff[(cz * g.G[1] + cy) * g.G[0] + cx]);
-    if (so >= 0) probe_cell(g, cx, cy, cz, so, qx, qy, qz, best, bestId, st);
+    if (so >= 0) {
+      GridIndex v;
+      sub_view(g, cx, cy, cz, so, v);
+      for (int pass = 0; pass < 2; ++pass) {
+        if (best < 1e300) {
+          const double r = sqrt(best);
+          bool in = true;
+#pragma unroll
+          for (int a = 0; a < 3; ++a) {
+            const double qa = a == 0 ? qx : (a == 1 ? qy : qz);
+            if (g.h[a] > 0) in = in && (qa - r > v.lo[a] + 1e-6 * g.h[a]) && (qa + r < v.hi[a] - 1e-6 * g.h[a]);
+            else in = in && (r < 1e300);
+          }
+          const int vx0 = cell_of(v, 0, qx - r - 1e-6 * v.h[0]), vx1 = cell_of(v, 0, qx + r + 1e-6 * v.h[0]);
+          const int vy0 = cell_of(v, 1, qy - r - 1e-6 * v.h[1]), vy1 = cell_of(v, 1, qy + r + 1e-6 * v.h[1]);
+          const int vz0 = cell_of(v, 2, qz - r - 1e-6 * v.h[2]), vz1 = cell_of(v, 2, qz + r + 1e-6 * v.h[2]);
+          if (in && (vy1 - vy0 + 1) * (vz1 - vz0 + 1) <= kLanes) {
+            scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
+            return;
+          }
+        }
+        if (pass == 0) {
+          const int hx = cell_of(v, 0, qx), hy = cell_of(v, 1, qy), hz = cell_of(v, 2, qz);
+          scan_box<false>(v, qx, qy, qz, max(hx - 1, 0), min(hx + 1, v.G[0] - 1), max(hy - 1, 0), min(hy + 1, v.G[1] - 1),
+                          max(hz - 1, 0), min(hz + 1, v.G[2] - 1), best, bestId, st);
+          if (nearer_ok && best < bound0 * (1.0 - 1e-9)) return;
+        }
+      }
+    }
   }
   // how far q lies outside the grid box on each axis
   const double ox = fmax(fmax(g.lo[0] - qx, qx - g.hi[0]), 0.0);
@@ -246,6 +271,7 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
     if (closer(sb, si, best, bestId)) { best = sb; bestId = si; }
     if (done || !(best < 1e300)) return;
   }
+  if (nearer_ok && best < bound0 * (1.0 - 1e-9)) return;
   // the ball (q, sqrt(best)) decides: scan its bounding box of cells, rows pruned as best shrinks
   const double r = sqrt(best);
   const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
