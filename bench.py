@@ -153,7 +153,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2509_07175_b200 import binding
+    from paper_2509_07175_b200 import binding, ranks
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -198,11 +198,7 @@ def main():
     cnt = ctx.counters()
     stage = ctx.stage_ms()
     cells = ctx.cells
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * w.n * args.steps / (ms * 1e-3)
+    value, ms = ranks.whole_job_rate(float(w.n * args.steps), ms, dev)
 
     # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
     barrier()
@@ -221,10 +217,7 @@ def main():
     d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
                                             "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
     h2d = w.sites.nbytes + w.verts.nbytes + w.simplices.nbytes
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_val = world * w.n / float(t.item())
+    e2e_val, _ = ranks.whole_job_rate(float(w.n), e2e_s * 1e3, dev)
 
     flops = algorithmic_flops(cnt, w.kind)
     clip_s = clip_ms / args.steps * 1e-3

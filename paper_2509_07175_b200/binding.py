@@ -158,6 +158,7 @@ class Context:
     def set_options(self, **kw):
         o = vd_options()
         o.real_edges = 1
+        o.persistent = 1
         for k, v in kw.items():
             setattr(o, k, v)
         self._check(self._lib.vd_set_options(self._h, ctypes.byref(o)))

@@ -82,7 +82,7 @@ static void set_default_options(vd_options& o) {
   o.grid_density = 4.0;
   o.step_out = 0;
   o.real_edges = 1;
-  o.persistent = 0;
+  o.persistent = 1;
 }
 
 static int64_t next_pow2(int64_t v) {
@@ -273,6 +273,7 @@ vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
   c->opt = *o;
   if (!(c->opt.grid_density > 0)) c->opt.grid_density = d.grid_density;
   if (c->opt.real_edges < 0) c->opt.real_edges = d.real_edges;
+  if (c->opt.persistent < 0) c->opt.persistent = d.persistent;
   return VD_OK;
 }
 

@@ -25,7 +25,7 @@ constexpr int K2 = 32, K2B = 256;
 
 // items: pairs[begin .. end) when list == nullptr, else pairs[list[begin .. end)]
 template <int KIND, bool BIG, bool HV>
-__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end) {
+__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end, bool persist) {
   constexpr int W = BIG ? 1 : kWarpsPerBlock;
   __shared__ GridIndex g;
   if (threadIdx.x == 0) g = *A.grid;
@@ -37,10 +37,8 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
     for (;;) {
       // dynamic work distribution: pieces range from 4 to hundreds of corners
-      unsigned long long t = 0;
-      if (lane_id() == 0) t = atomicAdd(&A.ctl->fetch[BIG ? 1 : 0], 1ull);
-      const int64_t k = begin + (int64_t)shfl(t, 0);
-      if (k >= end) break;
+      const int64_t k = next_ticket<BIG>(A, begin, end, persist);
+      if (k < 0) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
       const int rc = clip_pair_3d<BIG ? P3B : P3, BIG ? C3B : C3, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
@@ -56,15 +54,14 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
           if ((int64_t)slot < A.ovfCap) A.ovf[slot] = (int)idx; else atomicOr(&A.ctl->err, ERR_PAIR_CAP);
         }
       }
+      if (!BIG) pair_done(A);
       __syncwarp();
     }
   } else {
     __shared__ Poly2<BIG ? K2B : K2> S[W];
     for (;;) {
-      unsigned long long t = 0;
-      if (lane_id() == 0) t = atomicAdd(&A.ctl->fetch[BIG ? 1 : 0], 1ull);
-      const int64_t k = begin + (int64_t)shfl(t, 0);
-      if (k >= end) break;
+      const int64_t k = next_ticket<BIG>(A, begin, end, persist);
+      if (k < 0) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
       const int rc = clip_pair_2d<BIG ? K2B : K2, HV>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
@@ -80,6 +77,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
           if ((int64_t)slot < A.ovfCap) A.ovf[slot] = (int)idx; else atomicOr(&A.ctl->err, ERR_PAIR_CAP);
         }
       }
+      if (!BIG) pair_done(A);
       __syncwarp();
     }
   }
@@ -125,6 +123,7 @@ vd_status stage_seed(vd_ctx* c) {
   // nearest site of every mesh vertex: classifies the corners of every T_a and seeds the pair list
   if ((s = stage_nearest_points(c, c->verts.as<double>(), c->nv, c->vnn.as<int>()))) return s;
   cudaMemsetAsync(c->visited.p, 0, sizeof(unsigned long long) * c->hashCap, st);
+  cudaMemsetAsync(c->pairs.p, 0xff, sizeof(Pair) * c->pairCap, st);   // simplex id < 0: slot not yet pushed
   cudaMemsetAsync(c->sitePieces.p, 0, sizeof(int) * c->n, st);
   cudaMemsetAsync(c->siteNbrRaw.p, 0, sizeof(int) * c->n, st);
   const ClipArgs A = make_args(c);
@@ -133,38 +132,64 @@ vd_status stage_seed(vd_ctx* c) {
 }
 
 template <int KIND, bool HV>
-static void launch_wave(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, int64_t ob, int64_t oe) {
-  cudaMemsetAsync(&c->control.as<Control>()->fetch[0], 0, 2 * sizeof(unsigned long long), c->stream);
-  if (e > b) VD_LAUNCH((k_clip<KIND, false, HV>), blocks_for(e - b, kWarpsPerBlock, 148 * 6), kBlock, 0, c->stream)(A, nullptr, b, e);
-  if (oe > ob) VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe);
+static void launch_fast(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, bool persist) {
+  const int blocks = persist ? 148 * 3 : blocks_for(e - b, kWarpsPerBlock, 148 * 6);
+  VD_LAUNCH((k_clip<KIND, false, HV>), blocks, kBlock, 0, c->stream)(A, nullptr, b, e, persist);
+}
+
+template <int KIND, bool HV>
+static void launch_big(vd_ctx* c, const ClipArgs& A, int64_t ob, int64_t oe) {
+  VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe, false);
+}
+
+static void launch(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, int64_t e, bool persist) {
+  const bool tet = c->kind == KIND_TET_3D;
+  if (!big) {
+    if (tet) { if (hv) launch_fast<KIND_TET_3D, true>(c, A, b, e, persist); else launch_fast<KIND_TET_3D, false>(c, A, b, e, persist); }
+    else     { if (hv) launch_fast<KIND_TRI_2D, true>(c, A, b, e, persist); else launch_fast<KIND_TRI_2D, false>(c, A, b, e, persist); }
+  } else {
+    if (tet) { if (hv) launch_big<KIND_TET_3D, true>(c, A, b, e); else launch_big<KIND_TET_3D, false>(c, A, b, e); }
+    else     { if (hv) launch_big<KIND_TRI_2D, true>(c, A, b, e); else launch_big<KIND_TRI_2D, false>(c, A, b, e); }
+  }
+}
+
+static cudaError_t read_control(vd_ctx* c, Control& h) {
+  cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  return e;
+}
+
+static void set_cursor(vd_ctx* c, int which, unsigned long long v) {
+  cudaMemcpyAsync(&c->control.as<Control>()->fetch[which], &v, sizeof(v), cudaMemcpyHostToDevice, c->stream);
+  cudaStreamSynchronize(c->stream);   // v lives on the host stack
 }
 
 vd_status stage_clip(vd_ctx* c) {
   const ClipArgs A = make_args(c);
-  cudaStream_t st = c->stream;
-  int64_t begin = 0, obegin = 0;
-  int64_t waves = 0;
+  const bool persist = c->opt.persistent != 0;
+  int64_t begin = 0, obegin = 0, waves = 0;
   Control h;
+  cudaError_t e = read_control(c, h);   // seeds pushed so far, refined cells of the index
+  if (e != cudaSuccess) return cuda_check(c, e, "clip");
+  const bool hv = h.nHeavy > 0;         // refined cells exist: the kernels that know the second index level
   for (;;) {
-    cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_check(c, e, "clip wave");
     if (h.err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) break;   // caller grows the pools and reruns
     int64_t end = (int64_t)h.pairTail, oend = (int64_t)h.ovfTail;
     if (end > c->pairCap) end = c->pairCap;
     if (oend > c->ovfCap) oend = c->ovfCap;
     if (end == begin && oend == obegin) break;   // "while L1 is not empty"
-    const bool hv = h.nHeavy > 0;   // refined cells exist: the kernels that know the second index level
-    if (c->kind == KIND_TET_3D) {
-      if (hv) launch_wave<KIND_TET_3D, true>(c, A, begin, end, obegin, oend);
-      else launch_wave<KIND_TET_3D, false>(c, A, begin, end, obegin, oend);
-    } else {
-      if (hv) launch_wave<KIND_TRI_2D, true>(c, A, begin, end, obegin, oend);
-      else launch_wave<KIND_TRI_2D, false>(c, A, begin, end, obegin, oend);
+    if (end > begin) {
+      // wave mode: one launch per wavefront.  persistent mode: the kernel drains the queue as it grows
+      set_cursor(c, 0, persist ? (unsigned long long)begin : 0ull);
+      launch(c, A, hv, false, persist ? 0 : begin, end, persist);
+      ++waves;
+    } else if (oend > obegin) {
+      set_cursor(c, 1, 0ull);
+      launch(c, A, hv, true, obegin, oend, false);
+      obegin = oend;
     }
-    begin = end;
-    obegin = oend;
-    ++waves;
+    if ((e = read_control(c, h)) != cudaSuccess) return cuda_check(c, e, "clip wave");
+    if (end > begin) begin = persist ? (int64_t)h.finished : end;
   }
   c->hostControl = h;
   c->counters.waves = waves;

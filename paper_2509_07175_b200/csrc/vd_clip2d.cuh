@@ -35,7 +35,7 @@ __device__ __forceinline__ void lerp_to_plane(double cx, double cy, double cz, d
 template <int K, bool HV>
 __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
-  const Pair pr = A.pairs[pairIdx];
+  const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
   int tv[3];
   double tx[3], ty[3], tz[3];

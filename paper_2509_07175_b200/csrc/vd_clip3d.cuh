@@ -321,7 +321,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
 template <int P, int C, bool HV>
 __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
-  const Pair pr = A.pairs[pairIdx];
+  const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
   int tv[4];
   double tx[4], ty[4], tz[4];

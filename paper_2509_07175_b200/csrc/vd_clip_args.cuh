@@ -52,9 +52,57 @@ __device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, doubl
   if (!visit(A.visited, A.hashMask, a, j)) return;
   const unsigned long long slot = atomicAdd(&A.ctl->pairTail, 1ull);
   if ((int64_t)slot >= A.pairCap) { atomicOr(&A.ctl->err, ERR_PAIR_CAP); return; }
-  Pair p;
-  p.a = a; p.i = j; p.wx = wx; p.wy = wy; p.wz = wz;
-  A.pairs[slot] = p;
+  // the simplex id doubles as the slot's ready flag for the device-side queue: written last, after a fence
+  Pair* p = &A.pairs[slot];
+  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz;
+  __threadfence();
+  *reinterpret_cast<volatile int*>(&p->a) = a;
+}
+
+// A pair may have been written by another SM a moment ago: read it past the (incoherent) L1.
+__device__ __forceinline__ Pair load_pair(const ClipArgs& A, int64_t idx) {
+  const Pair* p = &A.pairs[idx];
+  Pair r;
+  r.a = __ldcg(&p->a); r.i = __ldcg(&p->i);
+  r.wx = __ldcg(&p->wx); r.wy = __ldcg(&p->wy); r.wz = __ldcg(&p->wz);
+  return r;
+}
+
+// Next unit of work for this warp, or -1.  Wave mode: tickets begin .. end-1 of the current wave (Alg. 4's
+// "for each pair in L1 in parallel").  Persistent mode: the pair list is a device-side queue; a
+// ticket beyond the tail waits until the pair is pushed, and the kernel ends when every dispatched pair
+// has finished (then nobody can push any more): no host round trip per wave.
+template <bool BIG>
+__device__ __forceinline__ int64_t next_ticket(const ClipArgs& A, int64_t begin, int64_t end, bool persist) {
+  long long t = 0;
+  if (lane_id() == 0) {
+    t = (long long)atomicAdd(&A.ctl->fetch[BIG ? 1 : 0], 1ull) + begin;
+    if (!persist) {
+      if (t >= end) t = -1;
+    } else {
+      for (;;) {
+        const unsigned long long fin = *reinterpret_cast<volatile unsigned long long*>(&A.ctl->finished);
+        unsigned long long tail = *reinterpret_cast<volatile unsigned long long*>(&A.ctl->pairTail);
+        if (tail > (unsigned long long)A.pairCap) tail = (unsigned long long)A.pairCap;
+        if ((unsigned long long)t < tail) break;
+        if (fin >= tail) { t = -1; break; }
+        __nanosleep(256);
+      }
+      if (t >= 0) {
+        while (*reinterpret_cast<volatile int*>(&A.pairs[t].a) < 0) __nanosleep(64);
+        __threadfence();
+      }
+    }
+  }
+  return (int64_t)shfl(t, 0);
+}
+
+__device__ __forceinline__ void pair_done(const ClipArgs& A) {
+  __syncwarp();
+  if (lane_id() == 0) {
+    __threadfence();
+    atomicAdd(&A.ctl->finished, 1ull);
+  }
 }
 
 // Edge-based bisector search (section IV-B) on the segment p_s -> p_t, all in coordinates

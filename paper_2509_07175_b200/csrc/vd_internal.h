@@ -13,7 +13,8 @@ struct Control {
   unsigned long long ovfTail;    // pairs deferred to the large-capacity path
   unsigned long long vertTail;   // corners allocated in the pool
   unsigned long long nbrTail;    // face flags allocated in the pool
-  unsigned long long fetch[2];   // work cursors of the running wave: fast tier, large tier
+  unsigned long long fetch[2];   // work cursors: fast tier, large tier
+  unsigned long long finished;   // pairs the fast tier has completed (persistent mode: termination)
   unsigned int err;              // ERR_* bits
   unsigned int nHeavy;           // refined cells of the site index (second level)
   Counters cnt;

@@ -57,7 +57,7 @@ def test_replica_parity(idx):
     assert g.n_nonempty == int((o.measure > 0).sum())
 
 
-@pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0)])
+@pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -127,3 +127,37 @@ def test_results_are_reproducible():
     assert np.allclose(a.measure, b.measure, rtol=1e-12, atol=0)
     assert np.allclose(a.centroid, b.centroid, rtol=0, atol=1e-12)
     assert np.allclose(a.piece_measure, b.piece_measure, rtol=1e-11, atol=0)
+
+
+def test_wave_mode_and_device_queue_agree():
+    """persistent=0 (one launch per wavefront) and persistent=1 (device-side queue) produce the
+    same cells; the clustered replica exercises the refined (two-level) site index in both."""
+    for idx in (3, 4):
+        w = inputs.config(idx, "small")
+        a, ca, _ = _gpu(w, persistent=0)
+        b, cb, _ = _gpu(w, persistent=1)
+        assert ca["waves"] > 1 and cb["waves"] >= 1
+        for f in ("nbr_off", "nbr", "piece_off", "piece_simplex", "vert_off", "vert_flags"):
+            assert np.array_equal(getattr(a, f), getattr(b, f)), f
+        assert np.allclose(a.measure, b.measure, rtol=1e-12, atol=0)
+
+
+def test_refined_index_on_heavily_clustered_sites():
+    """A cluster of 3,000 sites inside one grid cell next to 500 spread sites: the refined cells of the
+    site index must give the same nearest sites as brute force, and the cells must tile the cube."""
+    rng = np.random.default_rng(42)
+    s = np.concatenate([0.5 + 0.004 * rng.standard_normal((3000, 3)), rng.random((500, 3))])
+    s = np.clip(s, 0.0, 1.0)
+    v, t = inputs.cube_kuhn_mesh(3)
+    q = np.concatenate([rng.random((1500, 3)), 0.5 + 0.01 * rng.standard_normal((1500, 3))])
+    with binding.Context(s) as ctx:
+        got = ctx.nearest(q)
+        ctx.set_domain(v, t, 2)
+        ctx.compute()
+        g = ctx.to_host()
+    ref = ((q[:, None, :] - s[None, :, :]) ** 2).sum(-1).argmin(1)
+    assert np.array_equal(got, ref)
+    assert abs(g.measure.sum() - 1.0) < 1e-12
+    sub = np.sort(rng.choice(len(s), 150, replace=False))
+    o = oracle.compute(s, v, t, 2, subset=sub, tier="B")
+    parity.assert_parity(g, o, np.sqrt(3.0), abs_measure=1e-14)
