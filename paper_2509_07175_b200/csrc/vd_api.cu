@@ -169,9 +169,12 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   if (!c->haveDomain) { c->lastError = "vd_compute before vd_set_domain"; return VD_E_STATE; }
   c->haveResult = false;
   if (c->pairCap == 0) {
-    c->pairCap = c->opt.pair_capacity > 0 ? c->opt.pair_capacity : (8 * c->m + 4 * c->n + (1 << 16));
-    c->vertCap = c->opt.vert_capacity > 0 ? c->opt.vert_capacity : 12 * c->pairCap;
-    c->nbrCap = 8 * c->pairCap;
+    // pairs = pieces: a simplex meets ~2-20 cells in the paper-like workloads; corners ~11 per 3D piece.
+    // Underestimates are repaired by doubling and rerunning (counters.reruns)
+    const int64_t est = 16 * c->m + 2 * c->n;
+    c->pairCap = c->opt.pair_capacity > 0 ? c->opt.pair_capacity : (est + 6 * c->n + (1 << 16));
+    c->vertCap = c->opt.vert_capacity > 0 ? c->opt.vert_capacity : (14 * est + (1 << 16));
+    c->nbrCap = 8 * est + (1 << 16);
   }
   memset(&c->counters, 0, sizeof(c->counters));
   const unsigned long long launches0 = g_launches;

@@ -19,6 +19,7 @@ struct Poly2 {
   double tx[K], ty[K], tz[K], tnx[K], tny[K], tnz[K], td[K];
   int tflag[K], tnn[K];
   unsigned char tstate[K];
+  double u[12];   // per-pair constants: origin, v_i absolute, v_i local, witness local
   int nc;
 };
 
@@ -74,7 +75,11 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     S.cnn[k] = nn;
     S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
   }
-  if (lane == 0) S.nc = 3;
+  if (lane == 0) {
+    S.nc = 3;
+    S.u[0] = ox; S.u[1] = oy; S.u[2] = oz; S.u[3] = six; S.u[4] = siy; S.u[5] = siz;
+    S.u[6] = vix; S.u[7] = viy; S.u[8] = viz; S.u[9] = wx; S.u[10] = wy; S.u[11] = wz;
+  }
   __syncwarp();
   bool failed = false;
 #ifdef VD_TRACE
@@ -124,7 +129,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     double psx = wx, psy = wy, psz = wz;
     if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
     double nx, ny, nz, d;
-    const int j = find_bisector<HV>(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
+    const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
                                 nx, ny, nz, d, st, lc);
     if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
     bool own = false;

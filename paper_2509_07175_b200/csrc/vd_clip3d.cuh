@@ -8,6 +8,7 @@ namespace vd {
 
 template <int P, int C>
 struct Poly3 {
+  double u[12];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local)
   double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   int pflag[P];                           // flag of plane f
   double cx[C], cy[C], cz[C];             // corner coordinates (local)
@@ -323,43 +324,51 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   const int lane = lane_id();
   const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
-  int tv[4];
-  double tx[4], ty[4], tz[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    tv[k] = __ldg(&A.simp[(int64_t)a * 4 + k]);
-    tx[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 0]);
-    ty[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 1]);
-    tz[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 2]);
+  // ---- P <- T (Alg. 3 line 1): 4 planes (flags from the simplex adjacency), 4 corners.  Lane k < 4
+  // loads tet vertex k; coordinates are local to vertex 0.  The per-pair constants live in shared memory
+  // (S.u), not in registers: they would be spilled around every call of the query routines.
+  double vx = 0, vy = 0, vz = 0;
+  int vk = 0;
+  if (lane < 4) {
+    vk = __ldg(&A.simp[(int64_t)a * 4 + lane]);
+    vx = __ldg(&A.verts[(int64_t)vk * 3 + 0]); vy = __ldg(&A.verts[(int64_t)vk * 3 + 1]); vz = __ldg(&A.verts[(int64_t)vk * 3 + 2]);
   }
-  const double ox = tx[0], oy = ty[0], oz = tz[0];
-  const double six = __ldg(&A.sites[(int64_t)i * 3 + 0]), siy = __ldg(&A.sites[(int64_t)i * 3 + 1]),
-               siz = __ldg(&A.sites[(int64_t)i * 3 + 2]);
-  const double vix = six - ox, viy = siy - oy, viz = siz - oz;
-  const double wx = pr.wx - ox, wy = pr.wy - oy, wz = pr.wz - oz;
-
-  // ---- P <- T (Alg. 3 line 1): 4 planes (flags from the simplex adjacency), 4 corners
+  {
+    const double o0 = shfl(vx, 0), o1 = shfl(vy, 0), o2 = shfl(vz, 0);
+    if (lane < 4) { S.cx[lane] = vx - o0; S.cy[lane] = vy - o1; S.cz[lane] = vz - o2; }
+    if (lane == 0) {
+      const double s0 = __ldg(&A.sites[(int64_t)i * 3 + 0]), s1 = __ldg(&A.sites[(int64_t)i * 3 + 1]), s2 = __ldg(&A.sites[(int64_t)i * 3 + 2]);
+      S.u[0] = o0; S.u[1] = o1; S.u[2] = o2;
+      S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
+      S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
+      S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
+    }
+  }
+  __syncwarp();
+  const double &ox = S.u[0], &oy = S.u[1], &oz = S.u[2], &six = S.u[3], &siy = S.u[4], &siz = S.u[5];
+  const double &vix = S.u[6], &viy = S.u[7], &viz = S.u[8], &wx = S.u[9], &wy = S.u[10], &wz = S.u[11];
   if (lane < 4) {
     const int k = lane;
     const int q0 = (k + 1) & 3, q1 = (k + 2) & 3, q2 = (k + 3) & 3;
-    const double ax = tx[q1] - tx[q0], ay = ty[q1] - ty[q0], az = tz[q1] - tz[q0];
-    const double bx = tx[q2] - tx[q0], by = ty[q2] - ty[q0], bz = tz[q2] - tz[q0];
+    const double ax = S.cx[q1] - S.cx[q0], ay = S.cy[q1] - S.cy[q0], az = S.cz[q1] - S.cz[q0];
+    const double bx = S.cx[q2] - S.cx[q0], by = S.cy[q2] - S.cy[q0], bz = S.cz[q2] - S.cz[q0];
     double nx = ay * bz - az * by, ny = az * bx - ax * bz, nz = ax * by - ay * bx;
-    const double side = nx * (tx[k] - tx[q0]) + ny * (ty[k] - ty[q0]) + nz * (tz[k] - tz[q0]);
+    const double side = nx * (S.cx[k] - S.cx[q0]) + ny * (S.cy[k] - S.cy[q0]) + nz * (S.cz[k] - S.cz[q0]);
     if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
     S.pnx[k] = nx; S.pny[k] = ny; S.pnz[k] = nz;
-    S.pd[k] = nx * (tx[q0] - ox) + ny * (ty[q0] - oy) + nz * (tz[q0] - oz);
+    S.pd[k] = nx * S.cx[q0] + ny * S.cy[q0] + nz * S.cz[q0];
     S.pflag[k] = ~__ldg(&A.adj[(int64_t)a * 4 + k]);
-    // corner k = tet vertex k = the three faces other than k, in the cyclic order of DESIGN.md
-    const int tri[4][3] = {{1, 3, 2}, {0, 2, 3}, {0, 3, 1}, {0, 1, 2}};
-    S.cx[k] = tx[k] - ox; S.cy[k] = ty[k] - oy; S.cz[k] = tz[k] - oz;
-#pragma unroll
-    for (int t = 0; t < 3; ++t) {
-      S.cp[k][t] = (unsigned short)tri[k][t];
-      S.cadj[k][t] = (unsigned short)(6 - k - tri[k][t] - tri[k][(t + 1) % 3]);
-    }
+    // corner k = tet vertex k = the three faces other than k, cyclically ordered so that neighbouring
+    // corners traverse their shared edge in opposite directions: (1,3,2) (0,2,3) (0,3,1) (0,1,2)
+    const int t0 = (k == 0) ? 1 : 0;
+    const int t1 = (k == 0) ? 3 : ((k == 1) ? 2 : ((k == 2) ? 3 : 1));
+    const int t2 = (k == 0) ? 2 : ((k == 1) ? 3 : ((k == 2) ? 1 : 2));
+    S.cp[k][0] = (unsigned short)t0; S.cp[k][1] = (unsigned short)t1; S.cp[k][2] = (unsigned short)t2;
+    S.cadj[k][0] = (unsigned short)(6 - k - t0 - t1);
+    S.cadj[k][1] = (unsigned short)(6 - k - t1 - t2);
+    S.cadj[k][2] = (unsigned short)(6 - k - t2 - t0);
     // corners of T are classified from the per-vertex nearest site (S3): in Omega_i iff N_p = v_i
-    const int nn = __ldg(&A.vnn[tv[k]]);
+    const int nn = __ldg(&A.vnn[vk]);
     S.cnn[k] = nn;
     S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
   }
@@ -417,7 +426,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
     double psx = wx, psy = wy, psz = wz;
     if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
     double nx, ny, nz, d;
-    const int j = find_bisector<HV>(A, g, i, S.cnn[p], ox, oy, oz, vix, viy, viz, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
+    const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
                                 nx, ny, nz, d, st, lc);
     if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
     {

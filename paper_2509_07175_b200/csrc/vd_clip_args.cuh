@@ -114,10 +114,11 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
 template <bool HV>
-static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, double ox, double oy, double oz,
-                                             double vix, double viy, double viz,   // v_i local
+static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j,
+                                             const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
                                              double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
                                              double& nx, double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
+  const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
   for (int it = 0; it < 96; ++it) {
     lc.search_iters += 1;
     const double vjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
@@ -132,7 +133,7 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
     const double qx = psx + t * (ptx - psx), qy = psy + t * (pty - psy), qz = psz + t * (ptz - psz);
     // point-in-cell test of the intersecting point: N_q in {i, j} means q is in Omega_i
     const double ax = qx + ox, ay = qy + oy, az = qz + oz;
-    const double dix = ax - (vix + ox), diy = ay - (viy + oy), diz = az - (viz + oz);
+    const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
     double best = di2;
