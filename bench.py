@@ -30,6 +30,9 @@ UNIT = "cells/s"
 # plain FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64 FMA
 # lanes x 2 flop at the maximum SM clock; no FP64 figure exists in MEASURED_PEAKS.json.
 FP64_LANES_PER_SM, SMS = 64, 148
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_clip launch, from the committed ncu --set full capture
+# (profiles/r01_k_clip_c2_full.md); null for configs without a capture
+NCU_TRAFFIC_BYTES = {2: 0.48e9 + 7.03e9}
 WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
              2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
              3: "C3: unit cube 48^3 x 6 tets (663,552), 1,000,000 clustered sites, seed 2",
@@ -236,7 +239,7 @@ def main():
         "gpu_launches": int(launches),
         "stage_ms": stage, "counters": cnt,
         "roofline": {"bound": "alu", "kernel": "k_clip (S4+S5)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": None,
+                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
                      "algorithmic_flop_per_step": flops, "kernel_ms_per_step": clip_ms / args.steps,
                      "share_of_step": clip_ms / ms},
