@@ -112,6 +112,12 @@ vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out);
  * (P:L483-492).  Same errors as vd_create. */
 vd_status vd_update_sites(vd_ctx* ctx, const double* sites);
 
+/* vd_lloyd: `iterations` steps of Lloyd's method with density 1 (section VII-D, Eq. 3): compute
+ * the clipped / restricted cells, move every site with a non-empty cell to its cell's centroid, repeat; then
+ * one more vd_compute so that *out_cells describes the final sites.  Everything stays on the device.
+ * sites_out (host or device, [n][dim], may be NULL) receives the final sites.  Errors as vd_compute. */
+vd_status vd_lloyd(vd_ctx* ctx, int iterations, vd_cells* out_cells, double* sites_out);
+
 /* vd_set_domain: copy the domain M = {T_a}: verts [nv][dim] fp64, simplices [m][3]
  * (both triangle kinds) or [m][4] (tets), int32, 0-based, any orientation.  Derives the simplex
  * adjacency that initialises the edge/face flags (Fig. 2a).  May be called again.

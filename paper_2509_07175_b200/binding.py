@@ -17,7 +17,7 @@ from . import build as _build
 VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D = 0, 1, 2
 STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_INPUT", 5: "VD_E_CUDA",
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
-EXPORTS = ["vd_create", "vd_update_sites", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
+EXPORTS = ["vd_create", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
            "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_cells_to_host",
            "vd_nearest", "vd_get_adjacency", "vd_last_error", "vd_version"]
 
@@ -63,6 +63,7 @@ def load():
     vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
     lib.vd_create.argtypes = [vp, i64, ci, ctypes.POINTER(vp)]
     lib.vd_update_sites.argtypes = [vp, vp]
+    lib.vd_lloyd.argtypes = [vp, ci, ctypes.POINTER(vd_cells), vp]
     lib.vd_set_domain.argtypes = [vp, vp, i64, vp, i64, ci]
     lib.vd_compute.argtypes = [vp, ctypes.POINTER(vd_cells)]
     lib.vd_destroy.argtypes = [vp]
@@ -176,6 +177,12 @@ class Context:
     def compute(self) -> vd_cells:
         self._check(self._lib.vd_compute(self._h, ctypes.byref(self.cells)))
         return self.cells
+
+    def lloyd(self, iterations: int) -> np.ndarray:
+        """vd_lloyd: returns the final sites [n][dim]; self.cells describes them."""
+        out = np.empty((self.n, self.dim), np.float64)
+        self._check(self._lib.vd_lloyd(self._h, int(iterations), ctypes.byref(self.cells), out.ctypes.data))
+        return out
 
     def counters(self) -> dict:
         c = vd_counters()

@@ -77,6 +77,20 @@ static vd_status upload_points(vd_ctx* c, const double* src, int64_t n, int dim,
   return VD_OK;
 }
 
+// Lloyd step ("we compute centroids of Voronoi cells as the new sites"): empty cells keep their site
+__global__ void __launch_bounds__(kBlock) k_move_sites(const double* __restrict__ measure, const double* __restrict__ centroid,
+                                                        int64_t n, int dim, double* __restrict__ sites3) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    if (measure[i] > 0.0)
+      for (int a = 0; a < dim; ++a) sites3[i * 3 + a] = centroid[i * dim + a];
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_unpad3(const double* __restrict__ in3, int64_t n, int dim, double* __restrict__ out) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    for (int a = 0; a < dim; ++a) out[i * dim + a] = in3[i * 3 + a];
+}
+
 static void set_default_options(vd_options& o) {
   memset(&o, 0, sizeof(o));
   o.grid_density = 4.0;
@@ -239,6 +253,30 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   *out = r;
   c->haveResult = true;
   return VD_OK;
+}
+
+vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) {
+  if (!c || !out || iterations < 0) return VD_E_ARG;
+  vd_status s;
+  int blocks = (int)((c->n + kBlock - 1) / kBlock);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  for (int it = 0; it < iterations; ++it) {
+    if ((s = vd_compute(c, out))) return s;
+    VD_LAUNCH(k_move_sites, blocks, kBlock, 0, c->stream)(c->oMeasure.as<double>(), c->oCentroid.as<double>(), c->n, c->dim,
+                                                         c->sites.as<double>());
+    c->indexValid = false;
+  }
+  if ((s = vd_compute(c, out))) return s;
+  if (sites_out) {
+    DevBuf tmp;
+    if ((s = ensure(c, tmp, sizeof(double) * c->n * c->dim))) return s;
+    VD_LAUNCH(k_unpad3, blocks, kBlock, 0, c->stream)(c->sites.as<double>(), c->n, c->dim, tmp.as<double>());
+    cudaError_t e = cudaMemcpyAsync(sites_out, tmp.p, sizeof(double) * c->n * c->dim, cudaMemcpyDefault, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    release(c, tmp);
+    if (e != cudaSuccess) return cuda_check(c, e, "vd_lloyd");
+  }
+  return cuda_check(c, cudaGetLastError(), "vd_lloyd");
 }
 
 void vd_destroy(vd_ctx* c) {

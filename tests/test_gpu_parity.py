@@ -161,3 +161,28 @@ def test_refined_index_on_heavily_clustered_sites():
     sub = np.sort(rng.choice(len(s), 150, replace=False))
     o = oracle.compute(s, v, t, 2, subset=sub, tier="B")
     parity.assert_parity(g, o, np.sqrt(3.0), abs_measure=1e-14)
+
+
+def test_lloyd_iterations_follow_the_oracle():
+    """vd_lloyd (section VII-D, density 1): sites <- centroids, three times, against the same loop driven by
+    the oracle's centroids (2D and 3D)."""
+    for kind, dim in ((0, 2), (2, 3)):
+        rng = np.random.default_rng(77 + dim)
+        s0 = rng.random((300, dim))
+        if dim == 2:
+            v, t = inputs.unit_square_mesh()
+        else:
+            v, t = inputs.cube_kuhn_mesh(2)
+        with binding.Context(s0) as ctx:
+            ctx.set_domain(v, t, kind)
+            got = ctx.lloyd(3)
+            g = ctx.to_host()
+        s = s0.copy()
+        for _ in range(3):
+            o = oracle.compute(s, v, t, kind)
+            s = np.where(o.measure[:, None] > 0, o.centroid, s)
+        assert np.abs(got - s).max() <= 1e-9
+        o = oracle.compute(s, v, t, kind)
+        assert np.allclose(g.measure, o.measure, rtol=1e-7, atol=1e-12)
+        # Lloyd's method lowers the CVT energy: cells get more equal in size
+        assert g.measure.std() < oracle.compute(s0, v, t, kind).measure.std()
