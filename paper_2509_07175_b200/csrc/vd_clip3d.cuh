@@ -2,6 +2,7 @@
 // / Alg. 1 on the cell structure of section VI-C: an array of planes and an
 // array of corners, each corner the intersection of three planes = a triangle of the dual mesh.
 #pragma once
+#include "vd_batch.cuh"
 #include "vd_clip_args.cuh"
 
 namespace vd {
@@ -378,32 +379,40 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
 
   // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
   for (int guard = 0; guard < 4 * P + 16; ++guard) {
-    // point-in-cell tests of the unclassified corners (section IV-A)
-    for (int c0 = 0; c0 < nc; c0 += kLanes) {
-      const int c = c0 + lane;
-      unsigned um = __ballot_sync(kFull, c < nc && S.cstate[c] == ST_UNKNOWN);
-      while (um) {
-        const int cc = c0 + __ffs(um) - 1;
-        um &= um - 1;
-        const double qx = S.cx[cc] + ox, qy = S.cy[cc] + oy, qz = S.cz[cc] + oz;
-        const double dx = qx - six, dy = qy - siy, dz = qz - siz;
-        double best = dx * dx + dy * dy + dz * dz;
-        int bestId = i;
-        nearest<HV>(g, qx, qy, qz, best, bestId, st, true);
-        bool inside = bestId == i;
-        if (!inside) {
-          // flag rule in the form of reading U6: N_q already owns a plane of P
-          bool own = false;
-          for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == bestId);
-          inside = __any_sync(kFull, own);
+    // point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one
+    // batched pass (vd_batch.cuh); the batch state lives in the scratch area S.key
+    static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
+    QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
+    for (;;) {
+      int nq = 0;
+      for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
+        const int c = c0 + lane;
+        const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
+        const unsigned m = __ballot_sync(kFull, unk);
+        const int slot = nq + __popc(m & ((1u << lane) - 1u));
+        if (unk && slot < kQB) {
+          const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
+          const double dx = qx - six, dy = qy - siy, dz = qz - siz;
+          Q.item[slot] = c;
+          Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
+          Q.best[slot] = dx * dx + dy * dy + dz * dz;
+          Q.bestId[slot] = i;
         }
-        if (lane == 0) {
-          S.cstate[cc] = inside ? ST_IN : ST_OUT;
-          S.cnn[cc] = bestId;
-        }
+        nq = min(kQB, nq + __popc(m));
       }
+      if (nq == 0) break;
+      __syncwarp();
+      batch_nearest<HV>(g, Q, nq, st);
+      if (lane < nq) {
+        const int c = Q.item[lane], id = Q.bestId[lane];
+        bool inside = id == i;
+        // flag rule in the form of reading U6: N_q already owns a plane of P
+        for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
+        S.cstate[c] = inside ? ST_IN : ST_OUT;
+        S.cnn[c] = id;
+      }
+      __syncwarp();
     }
-    __syncwarp();
     // select an outside corner p; prefer one with a neighbour p_s in Omega_i (a real edge, Alg. 1 line 3)
     int p = -1, s = -1;
     for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
