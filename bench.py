@@ -32,7 +32,7 @@ UNIT = "cells/s"
 FP64_LANES_PER_SM, SMS = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_clip launch, from the committed ncu --set full capture
 # (profiles/r01_k_clip_c2_full.md); null for configs without a capture
-NCU_TRAFFIC_BYTES = {2: 0.48e9 + 7.03e9}
+NCU_TRAFFIC_BYTES = {2: 0.185e9 + 0.959e9}
 WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
              2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
              3: "C3: unit cube 48^3 x 6 tets (663,552), 1,000,000 clustered sites, seed 2",
