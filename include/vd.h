@@ -40,8 +40,15 @@ typedef enum {
   VD_E_NOCONVERGE = 8  /* an iteration cap was hit (degenerate input: duplicate sites, ...)      */
 } vd_status;
 
-/* Domain kinds.  dim == 2 <=> VD_TRI_2D;  dim == 3 <=> VD_TRI_SURFACE or VD_TET_3D. */
-typedef enum { VD_TRI_2D = 0, VD_TRI_SURFACE = 1, VD_TET_3D = 2 } vd_domain_kind;
+/* Domain kinds.  dim == 2 <=> VD_TRI_2D, VD_BOX_2D;  dim == 3 <=> VD_TRI_SURFACE, VD_TET_3D, VD_BOX_3D. */
+typedef enum {
+  VD_TRI_2D = 0, VD_TRI_SURFACE = 1, VD_TET_3D = 2,
+  /* "simple domains" of section V-B ("e.g. a cube"): an axis-aligned rectangle (dim 2) or box
+   * (dim 3) given by its two opposite corners, verts = [lo, hi], nv = 2, simplices ignored (may be NULL), m = 1.
+   * The whole domain is ONE piece per cell (piece_simplex = 0): the dissolved clipped cell, every domain face
+   * flagged ~m = ~1. */
+  VD_BOX_2D = 3, VD_BOX_3D = 4
+} vd_domain_kind;
 
 /* Result of vd_compute: CSR arrays, 0-based, DEVICE pointers.
  *

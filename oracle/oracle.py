@@ -110,9 +110,11 @@ def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0) -> 
     lib = _load()
     sites = np.ascontiguousarray(sites, dtype=np.float64)
     verts = np.ascontiguousarray(verts, dtype=np.float64)
-    simplices = np.ascontiguousarray(simplices, dtype=np.int32)
     n, dim = sites.shape
     nv = verts.shape[0]
+    if int(kind) in (3, 4):   # simple domain: verts = (lo, hi), one piece
+        simplices = np.zeros((1, 0), dtype=np.int32)
+    simplices = np.ascontiguousarray(simplices, dtype=np.int32)
     m, nc = simplices.shape
     if subset is not None:
         subset = np.ascontiguousarray(subset, dtype=np.int64)
@@ -122,7 +124,7 @@ def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0) -> 
         sp, ns = None, 0
         ids = np.arange(n, dtype=np.int64)
     res = ctypes.POINTER(_Result)()
-    rc = lib.vdo_compute(sites.ctypes.data, n, dim, verts.ctypes.data, nv, simplices.ctypes.data, m,
+    rc = lib.vdo_compute(sites.ctypes.data, n, dim, verts.ctypes.data, nv, simplices.ctypes.data if simplices.size else None, m,
                          int(kind), sp, ns, 1 if tier == "B" else 0, int(threads), ctypes.byref(res))
     if rc != 0:
         raise RuntimeError(f"vdo_compute failed with status {rc}")

@@ -18,6 +18,8 @@
 // carrying one label per edge / face (the flag of an edge/face is the adjacent
 // simplex or the neighbouring cell):
 //     label >= 0      : site id j   (the edge/face lies on the bisector B_ij)
+// Kinds 3 / 4 are the paper's "simple domains" (section V-B): an axis-aligned rectangle / box given
+// by its two opposite corners, treated as ONE convex piece (simplex id 0, m = 1, every face labelled ~m).
 //     label <  0      : ~label = id of the simplex adjacent across that edge/face,
 //                       ~label == m means a face on the domain boundary
 // (0-based restatement of the paper's +j / -b convention; reading U3 in DESIGN.md).
@@ -69,7 +71,7 @@ static inline V3 cross(const V3& a, const V3& b) {
   return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
 }
 
-enum { KIND_TRI_2D = 0, KIND_TRI_SURFACE = 1, KIND_TET_3D = 2 };
+enum { KIND_TRI_2D = 0, KIND_TRI_SURFACE = 1, KIND_TET_3D = 2, KIND_BOX_2D = 3, KIND_BOX_3D = 4 };
 static const int LABEL_PAD = INT32_MIN;        // padding when a corner has fewer labels than expected
 static const int LABEL_BOX = INT32_MIN + 1;    // faces of the phase-1 box (tier B), never output
 
@@ -329,14 +331,14 @@ static Polyhedron simplex_polyhedron(const Domain& D, int64_t a) {
   return G;
 }
 
-static Polyhedron box_polyhedron(const V3& lo, const V3& hi) {
+static Polyhedron box_polyhedron(const V3& lo, const V3& hi, int label = LABEL_BOX) {
   Polyhedron G;
   for (int c = 0; c < 8; ++c)
     G.V.push_back({(c & 1) ? hi.x : lo.x, (c & 2) ? hi.y : lo.y, (c & 4) ? hi.z : lo.z});
   static const int loops[6][4] = {{0, 4, 6, 2}, {1, 3, 7, 5}, {0, 1, 5, 4}, {2, 6, 7, 3}, {0, 2, 3, 1}, {4, 5, 7, 6}};
   for (int f = 0; f < 6; ++f) {
     G.F.push_back(std::vector<int>(loops[f], loops[f] + 4));
-    G.L.push_back(LABEL_BOX);
+    G.L.push_back(label);
   }
   return G;
 }
@@ -436,8 +438,9 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
   for (int64_t a = 0; a < D.m; ++a) {
     PieceOut po;
     bool ok = false;
-    if (D.kind == KIND_TET_3D) {
-      Polyhedron G = simplex_polyhedron(D, a);
+    if (D.kind == KIND_TET_3D || D.kind == KIND_BOX_3D) {
+      // a simple domain (section V-B: "e.g. a cube") is one convex piece; its faces are domain boundary (~m)
+      Polyhedron G = D.kind == KIND_BOX_3D ? box_polyhedron(D.verts[0], D.verts[1], ~(int)D.m) : simplex_polyhedron(D, a);
       if (planes) {
         for (size_t k = 0; k < HS.size() && !G.empty(); ++k) clip_polyhedron(G, HS[k]);
       } else {
@@ -446,7 +449,14 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
       }
       ok = !G.empty() && finish_polyhedron(G, (int32_t)a, po);
     } else {
-      Polygon G = simplex_polygon(D, a);
+      Polygon G;
+      if (D.kind == KIND_BOX_2D) {
+        const V3 lo = D.verts[0], hi = D.verts[1];
+        G.P = {{lo.x, lo.y, 0}, {hi.x, lo.y, 0}, {hi.x, hi.y, 0}, {lo.x, hi.y, 0}};
+        G.L = {~(int)D.m, ~(int)D.m, ~(int)D.m, ~(int)D.m};
+      } else {
+        G = simplex_polygon(D, a);
+      }
       if (planes) {
         for (size_t k = 0; k < HS.size() && !G.empty(); ++k) clip_polygon(G, HS[k]);
       } else {
@@ -532,21 +542,23 @@ void vdo_free(vdo_result* r) {
 int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, int64_t nv,
                 const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
                 int tier, int nthreads, vdo_result** out) {
-  if (!sites || !verts || !simplices || !out || n < 1 || m < 1 || nv < 1) return 1;
-  if (!((kind == KIND_TRI_2D && dim == 2) || (kind != KIND_TRI_2D && dim == 3))) return 1;
+  const bool box = kind == KIND_BOX_2D || kind == KIND_BOX_3D;
+  if (!sites || !verts || (!simplices && !box) || !out || n < 1 || m < 1 || nv < 1) return 1;
+  if (!(((kind == KIND_TRI_2D || kind == KIND_BOX_2D) && dim == 2) || ((kind == KIND_TRI_SURFACE || kind == KIND_TET_3D || kind == KIND_BOX_3D) && dim == 3))) return 1;
+  if (box && (nv != 2 || m != 1)) return 1;   // verts = the two opposite corners (lo, hi)
   if (kind == KIND_TRI_SURFACE && tier == 1) return 1;  // a surface has no enclosing-box shortcut here: use tier A
   Problem Pb;
   Pb.n = n;
   Pb.sites.resize(n);
   for (int64_t i = 0; i < n; ++i) Pb.sites[i] = load_point(sites + i * dim, dim);
   Domain& D = Pb.D;
-  D.kind = kind; D.dim = dim; D.nc = (kind == KIND_TET_3D) ? 4 : 3; D.nv = nv; D.m = m;
+  D.kind = kind; D.dim = dim; D.nc = box ? 0 : ((kind == KIND_TET_3D) ? 4 : 3); D.nv = nv; D.m = m;
   D.verts.resize(nv);
   for (int64_t v = 0; v < nv; ++v) D.verts[v] = load_point(verts + v * dim, dim);
-  D.simp.assign(simplices, simplices + m * D.nc);
+  if (!box) D.simp.assign(simplices, simplices + m * D.nc);
   for (int64_t k = 0; k < m * D.nc; ++k)
     if (D.simp[k] < 0 || D.simp[k] >= nv) return 4;
-  if (build_adjacency(D)) return 4;
+  if (!box && build_adjacency(D)) return 4;
 
   const int64_t ns = subset ? n_subset : n;
   std::vector<CellOut> cells(ns);
@@ -584,7 +596,7 @@ int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, in
   for (size_t t = 0; t < pool.size(); ++t) pool[t].join();
 
   vdo_result* R = (vdo_result*)calloc(1, sizeof(vdo_result));
-  R->ns = ns; R->dim = dim; R->nfl = (kind == KIND_TET_3D) ? 3 : 2; R->threads_used = nthreads;
+  R->ns = ns; R->dim = dim; R->nfl = (kind == KIND_TET_3D || kind == KIND_BOX_3D) ? 3 : 2; R->threads_used = nthreads;
   for (int64_t s = 0; s < ns; ++s) {
     R->n_pieces += (int64_t)cells[s].pieces.size();
     R->n_nbrs += (int64_t)cells[s].nbr.size();
@@ -600,8 +612,8 @@ int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, in
   R->vert_off = (int64_t*)malloc(sizeof(int64_t) * (R->n_pieces + 1));
   R->vert_xyz = (double*)malloc(sizeof(double) * (R->n_verts * dim + 1));
   R->vert_flags = (int32_t*)malloc(sizeof(int32_t) * (R->n_verts * R->nfl + 1));
-  R->simplex_adj = (int32_t*)malloc(sizeof(int32_t) * (m * D.nc));
-  memcpy(R->simplex_adj, D.adj.data(), sizeof(int32_t) * m * D.nc);
+  R->simplex_adj = (int32_t*)malloc(sizeof(int32_t) * (m * D.nc + 1));
+  if (!box) memcpy(R->simplex_adj, D.adj.data(), sizeof(int32_t) * m * D.nc);
   int64_t ip = 0, iv = 0, in = 0;
   for (int64_t s = 0; s < ns; ++s) {
     const CellOut& c = cells[s];

@@ -14,7 +14,7 @@ import numpy as np
 
 from . import build as _build
 
-VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D = 0, 1, 2
+VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D, VD_BOX_2D, VD_BOX_3D = 0, 1, 2, 3, 4
 STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_INPUT", 5: "VD_E_CUDA",
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
 EXPORTS = ["vd_create", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
@@ -169,9 +169,14 @@ class Context:
         self._check(self._lib.vd_update_sites(self._h, p))
 
     def set_domain(self, verts, simplices, kind):
+        """verts [nv][dim], simplices [m][3|4]; for VD_BOX_2D / VD_BOX_3D verts = (lo, hi) and simplices is None."""
         pv, k1 = _ptr(verts, np.float64)
-        ps, k2 = _ptr(simplices, np.int32)
-        self.kind, self.m, self.nc = int(kind), int(simplices.shape[0]), int(simplices.shape[1])
+        if int(kind) in (VD_BOX_2D, VD_BOX_3D):
+            ps, self.m, self.nc = None, 1, 4 if int(kind) == VD_BOX_2D else 8
+        else:
+            ps, k2 = _ptr(simplices, np.int32)
+            self.m, self.nc = int(simplices.shape[0]), int(simplices.shape[1])
+        self.kind = int(kind)
         self._check(self._lib.vd_set_domain(self._h, pv, int(verts.shape[0]), ps, self.m, int(kind)))
 
     def compute(self) -> vd_cells:

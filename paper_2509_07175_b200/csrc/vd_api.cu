@@ -157,18 +157,52 @@ vd_status vd_update_sites(vd_ctx* c, const double* sites) {
 }
 
 vd_status vd_set_domain(vd_ctx* c, const double* verts, int64_t nv, const int32_t* simplices, int64_t m, vd_domain_kind kind) {
-  if (!c || !verts || !simplices || nv < 1 || m < 1) return VD_E_ARG;
-  if (kind != VD_TRI_2D && kind != VD_TRI_SURFACE && kind != VD_TET_3D) return VD_E_ARG;
-  if ((kind == VD_TRI_2D) != (c->dim == 2)) return VD_E_DIM;
+  const bool box = kind == VD_BOX_2D || kind == VD_BOX_3D;
+  if (!c || !verts || (!simplices && !box) || nv < 1 || m < 1) return VD_E_ARG;
+  if (kind < VD_TRI_2D || kind > VD_BOX_3D) return VD_E_ARG;
+  if ((kind == VD_TRI_2D || kind == VD_BOX_2D) != (c->dim == 2)) return VD_E_DIM;
   if (m > 0x3fffffff || nv > 0x7fffffff) return VD_E_ARG;
+  if (box && (nv != 2 || m != 1)) return VD_E_ARG;
   c->haveDomain = false;
   c->haveResult = false;
   c->kind = (int)kind;
-  c->nc = kind == VD_TET_3D ? 4 : 3;
-  c->nfl = kind == VD_TET_3D ? 3 : 2;
-  c->nv = nv;
+  const bool solid = kind == VD_TET_3D || kind == VD_BOX_3D;
+  c->nc = kind == VD_BOX_3D ? 8 : ((kind == VD_TET_3D || kind == VD_BOX_2D) ? 4 : 3);
+  c->nfl = solid ? 3 : 2;
   c->m = m;
-  vd_status s = upload_points(c, verts, nv, c->dim, c->verts, "vd_set_domain");
+  vd_status s;
+  if (box) {
+    // simple domain (section V-B): expand (lo, hi) into the 4 / 8 corners; they are the "mesh vertices" whose
+    // nearest sites seed the pair list and classify the corners; corner c = bits (x, y, z)
+    double lh[6] = {0, 0, 0, 0, 0, 0};
+    cudaError_t e = cudaMemcpyAsync(lh, verts, sizeof(double) * 2 * c->dim, cudaMemcpyDefault, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "vd_set_domain");
+    const int dim = c->dim, ncorner = c->nc;
+    double cv[8 * 3];
+    int32_t ids[8], adj[8];
+    for (int k = 0; k < ncorner; ++k) {
+      for (int a = 0; a < dim; ++a) {
+        const double lo = lh[a], hi = lh[dim + a];
+        if (!(hi > lo)) { c->lastError = "vd_set_domain: empty box"; return VD_E_INPUT; }
+        cv[k * dim + a] = ((k >> a) & 1) ? hi : lo;
+      }
+      ids[k] = k;
+      adj[k] = (int32_t)m;
+    }
+    c->nv = ncorner;
+    if ((s = upload_points(c, cv, ncorner, dim, c->verts, "vd_set_domain"))) return s;
+    if ((s = ensure(c, c->simp, sizeof(int) * ncorner))) return s;
+    if ((s = ensure(c, c->adj, sizeof(int) * ncorner))) return s;
+    e = cudaMemcpyAsync(c->simp.p, ids, sizeof(int) * ncorner, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->adj.p, adj, sizeof(int) * ncorner, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "vd_set_domain");
+    c->haveDomain = true;
+    return VD_OK;
+  }
+  c->nv = nv;
+  s = upload_points(c, verts, nv, c->dim, c->verts, "vd_set_domain");
   if (s != VD_OK) return s;
   if ((s = ensure(c, c->simp, sizeof(int) * m * c->nc))) return s;
   cudaError_t e = cudaMemcpyAsync(c->simp.p, simplices, sizeof(int) * m * c->nc, cudaMemcpyDefault, c->stream);
@@ -189,6 +223,14 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     c->pairCap = c->opt.pair_capacity > 0 ? c->opt.pair_capacity : (est + 6 * c->n + (1 << 16));
     c->vertCap = c->opt.vert_capacity > 0 ? c->opt.vert_capacity : (14 * est + (1 << 16));
     c->nbrCap = 8 * est + (1 << 16);
+    if (c->kind == VD_BOX_2D || c->kind == VD_BOX_3D) {
+      // whole cells: one pair per site; a Poisson-Voronoi cell has 6 corners / edges in 2D, ~27.1 corners and
+      // ~15.5 faces in 3D on average
+      const bool solid = c->kind == VD_BOX_3D;
+      c->pairCap = c->opt.pair_capacity > 0 ? c->opt.pair_capacity : (2 * c->n + (1 << 16));
+      c->vertCap = c->opt.vert_capacity > 0 ? c->opt.vert_capacity : ((solid ? 32 : 8) * c->n + (1 << 16));
+      c->nbrCap = (solid ? 20 : 8) * c->n + (1 << 16);
+    }
   }
   memset(&c->counters, 0, sizeof(c->counters));
   const unsigned long long launches0 = g_launches;

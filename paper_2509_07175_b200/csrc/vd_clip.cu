@@ -19,6 +19,15 @@ __global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc) {
   }
 }
 
+// Simple domains (section V-B): a site inside the box owns its own position, so (box, v_i) is a non-empty pair
+// with witness v_i ("each site must be in its own Voronoi cell").
+__global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, double lx, double ly, double lz, double hx, double hy, double hz) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double x = A.sites[i * 3 + 0], y = A.sites[i * 3 + 1], z = A.sites[i * 3 + 2];
+    if (x >= lx && x <= hx && y >= ly && y <= hy && z >= lz && z <= hz) push_pair(A, 0, (int)i, x, y, z);
+  }
+}
+
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
@@ -33,14 +42,15 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u};
-  if constexpr (KIND == KIND_TET_3D) {
+  constexpr bool BOX = KIND == KIND_BOX_2D || KIND == KIND_BOX_3D;
+  if constexpr (KIND == KIND_TET_3D || KIND == KIND_BOX_3D) {
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
     for (;;) {
       // dynamic work distribution: pieces range from 4 to hundreds of corners
       const int64_t k = next_ticket<BIG>(A, begin, end, persist);
       if (k < 0) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
-      const int rc = clip_pair_3d<BIG ? P3B : P3, BIG ? C3B : C3, HV>(S[w], g, A, idx, st, lc);
+      const int rc = clip_pair_3d<BIG ? P3B : P3, BIG ? C3B : C3, HV, BOX>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
         if (BIG) {
           if (lane_id() == 0) {
@@ -63,7 +73,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
       const int64_t k = next_ticket<BIG>(A, begin, end, persist);
       if (k < 0) break;
       const int64_t idx = list ? (int64_t)list[k] : k;
-      const int rc = clip_pair_2d<BIG ? K2B : K2, HV>(S[w], g, A, idx, st, lc);
+      const int rc = clip_pair_2d<BIG ? K2B : K2, HV, BOX>(S[w], g, A, idx, st, lc);
       if (rc == 1) {
         if (BIG) {
           if (lane_id() == 0) {
@@ -128,6 +138,14 @@ vd_status stage_seed(vd_ctx* c) {
   cudaMemsetAsync(c->siteNbrRaw.p, 0, sizeof(int) * c->n, st);
   const ClipArgs A = make_args(c);
   VD_LAUNCH(k_seed, blocks_for(c->m, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
+  if (c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D) {
+    double cv[8 * 3];
+    cudaMemcpyAsync(cv, c->verts.p, sizeof(double) * 3 * c->nc, cudaMemcpyDeviceToHost, st);
+    cudaStreamSynchronize(st);
+    const double* lo = cv;
+    const double* hi = cv + 3 * (c->nc - 1);
+    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, 148 * 8), kBlock, 0, st)(A, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2]);
+  }
   return cuda_check(c, cudaGetLastError(), "seed");
 }
 
@@ -142,14 +160,19 @@ static void launch_big(vd_ctx* c, const ClipArgs& A, int64_t ob, int64_t oe) {
   VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe, false);
 }
 
+template <int KIND>
+static void launch_kind(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, int64_t e, bool persist) {
+  if (!big) { if (hv) launch_fast<KIND, true>(c, A, b, e, persist); else launch_fast<KIND, false>(c, A, b, e, persist); }
+  else      { if (hv) launch_big<KIND, true>(c, A, b, e); else launch_big<KIND, false>(c, A, b, e); }
+}
+
+// one kernel per piece structure: triangles (both triangle kinds share the loop code), tets, rectangle, box
 static void launch(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, int64_t e, bool persist) {
-  const bool tet = c->kind == KIND_TET_3D;
-  if (!big) {
-    if (tet) { if (hv) launch_fast<KIND_TET_3D, true>(c, A, b, e, persist); else launch_fast<KIND_TET_3D, false>(c, A, b, e, persist); }
-    else     { if (hv) launch_fast<KIND_TRI_2D, true>(c, A, b, e, persist); else launch_fast<KIND_TRI_2D, false>(c, A, b, e, persist); }
-  } else {
-    if (tet) { if (hv) launch_big<KIND_TET_3D, true>(c, A, b, e); else launch_big<KIND_TET_3D, false>(c, A, b, e); }
-    else     { if (hv) launch_big<KIND_TRI_2D, true>(c, A, b, e); else launch_big<KIND_TRI_2D, false>(c, A, b, e); }
+  switch (c->kind) {
+    case KIND_TET_3D: launch_kind<KIND_TET_3D>(c, A, hv, big, b, e, persist); break;
+    case KIND_BOX_3D: launch_kind<KIND_BOX_3D>(c, A, hv, big, b, e, persist); break;
+    case KIND_BOX_2D: launch_kind<KIND_BOX_2D>(c, A, hv, big, b, e, persist); break;
+    default:          launch_kind<KIND_TRI_2D>(c, A, hv, big, b, e, persist); break;
   }
 }
 

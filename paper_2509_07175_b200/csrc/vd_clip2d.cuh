@@ -33,50 +33,71 @@ __device__ __forceinline__ void lerp_to_plane(double cx, double cy, double cz, d
   x = cx + t * (bx - cx); y = cy + t * (by - cy); z = cz + t * (bz - cz);
 }
 
-template <int K, bool HV>
+template <int K, bool HV, bool BOX>
 __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
-  int tv[3];
-  double tx[3], ty[3], tz[3];
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    tv[k] = __ldg(&A.simp[(int64_t)a * 3 + k]);
-    tx[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 0]);
-    ty[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 1]);
-    tz[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 2]);
-  }
-  const double ox = tx[0], oy = ty[0], oz = tz[0];
   const double six = __ldg(&A.sites[(int64_t)i * 3 + 0]), siy = __ldg(&A.sites[(int64_t)i * 3 + 1]),
                siz = __ldg(&A.sites[(int64_t)i * 3 + 2]);
+  double ox, oy, oz, pnx, pny, pnz;
+  if constexpr (BOX) {
+    // simple domain (section V-B): P <- the rectangle; verts holds its 4 corners (bits x, y), the loop
+    // runs 0 -> 1 -> 3 -> 2, edge k from corner k to k+1: bottom, right, top, left
+    ox = __ldg(&A.verts[0]); oy = __ldg(&A.verts[1]); oz = __ldg(&A.verts[2]);
+    const double e0 = __ldg(&A.verts[9]) - ox, e1 = __ldg(&A.verts[10]) - oy;
+    pnx = 0.0; pny = 0.0; pnz = 1.0;
+    if (lane < 4) {
+      const int k = lane, vid = k ^ (k >> 1);
+      S.cx[k] = (vid & 1) ? e0 : 0.0; S.cy[k] = (vid & 2) ? e1 : 0.0; S.cz[k] = 0.0;
+      S.enx[k] = k == 1 ? 1.0 : (k == 3 ? -1.0 : 0.0);
+      S.eny[k] = k == 2 ? 1.0 : (k == 0 ? -1.0 : 0.0);
+      S.enz[k] = 0.0;
+      S.ed[k] = k == 1 ? e0 : (k == 2 ? e1 : 0.0);
+      S.eflag[k] = ~A.m;
+      const int nn = __ldg(&A.vnn[vid]);
+      S.cnn[k] = nn;
+      S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
+    }
+    if (lane == 0) S.nc = 4;
+  } else {
+    int tv[3];
+    double tx[3], ty[3], tz[3];
+  #pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      tv[k] = __ldg(&A.simp[(int64_t)a * 3 + k]);
+      tx[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 0]);
+      ty[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 1]);
+      tz[k] = __ldg(&A.verts[(int64_t)tv[k] * 3 + 2]);
+    }
+    ox = tx[0]; oy = ty[0]; oz = tz[0];
+    // triangle plane (local): unit normal, offset 0 (corner 0 is the origin)
+    {
+      const double ax = tx[1] - ox, ay = ty[1] - oy, az = tz[1] - oz, bx = tx[2] - ox, by = ty[2] - oy, bz = tz[2] - oz;
+      pnx = ay * bz - az * by; pny = az * bx - ax * bz; pnz = ax * by - ay * bx;
+      const double inv = 1.0 / sqrt(pnx * pnx + pny * pny + pnz * pnz);
+      pnx *= inv; pny *= inv; pnz *= inv;
+    }
+    // ---- P <- T: corner k = vertex k, edge k = (k -> k+1) lies opposite vertex k+2
+    if (lane < 3) {
+      const int k = lane, k1 = (k + 1) % 3, k2 = (k + 2) % 3;
+      S.cx[k] = tx[k] - ox; S.cy[k] = ty[k] - oy; S.cz[k] = tz[k] - oz;
+      const double ex = tx[k1] - tx[k], ey = ty[k1] - ty[k], ez = tz[k1] - tz[k];
+      double nx = ey * pnz - ez * pny, ny = ez * pnx - ex * pnz, nz = ex * pny - ey * pnx;   // e x n
+      const double side = nx * (tx[k2] - tx[k]) + ny * (ty[k2] - ty[k]) + nz * (tz[k2] - tz[k]);
+      if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
+      S.enx[k] = nx; S.eny[k] = ny; S.enz[k] = nz;
+      S.ed[k] = nx * (tx[k] - ox) + ny * (ty[k] - oy) + nz * (tz[k] - oz);
+      S.eflag[k] = ~__ldg(&A.adj[(int64_t)a * 3 + k2]);
+      const int nn = __ldg(&A.vnn[tv[k]]);
+      S.cnn[k] = nn;
+      S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
+    }
+    if (lane == 0) S.nc = 3;
+  }
   const double vix = six - ox, viy = siy - oy, viz = siz - oz;
   const double wx = pr.wx - ox, wy = pr.wy - oy, wz = pr.wz - oz;
-  // triangle plane (local): unit normal, offset 0 (corner 0 is the origin)
-  double pnx, pny, pnz;
-  {
-    const double ax = tx[1] - ox, ay = ty[1] - oy, az = tz[1] - oz, bx = tx[2] - ox, by = ty[2] - oy, bz = tz[2] - oz;
-    pnx = ay * bz - az * by; pny = az * bx - ax * bz; pnz = ax * by - ay * bx;
-    const double inv = 1.0 / sqrt(pnx * pnx + pny * pny + pnz * pnz);
-    pnx *= inv; pny *= inv; pnz *= inv;
-  }
-  // ---- P <- T: corner k = vertex k, edge k = (k -> k+1) lies opposite vertex k+2
-  if (lane < 3) {
-    const int k = lane, k1 = (k + 1) % 3, k2 = (k + 2) % 3;
-    S.cx[k] = tx[k] - ox; S.cy[k] = ty[k] - oy; S.cz[k] = tz[k] - oz;
-    const double ex = tx[k1] - tx[k], ey = ty[k1] - ty[k], ez = tz[k1] - tz[k];
-    double nx = ey * pnz - ez * pny, ny = ez * pnx - ex * pnz, nz = ex * pny - ey * pnx;   // e x n
-    const double side = nx * (tx[k2] - tx[k]) + ny * (ty[k2] - ty[k]) + nz * (tz[k2] - tz[k]);
-    if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
-    S.enx[k] = nx; S.eny[k] = ny; S.enz[k] = nz;
-    S.ed[k] = nx * (tx[k] - ox) + ny * (ty[k] - oy) + nz * (tz[k] - oz);
-    S.eflag[k] = ~__ldg(&A.adj[(int64_t)a * 3 + k2]);
-    const int nn = __ldg(&A.vnn[tv[k]]);
-    S.cnn[k] = nn;
-    S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
-  }
   if (lane == 0) {
-    S.nc = 3;
     S.u[0] = ox; S.u[1] = oy; S.u[2] = oz; S.u[3] = six; S.u[4] = siy; S.u[5] = siz;
     S.u[6] = vix; S.u[7] = viy; S.u[8] = viz; S.u[9] = wx; S.u[10] = wy; S.u[11] = wz;
   }
@@ -98,11 +119,13 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
       if (S.cstate[c] != ST_UNKNOWN) continue;
       const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
       const double dx = qx - six, dy = qy - siy, dz = qz - siz;
-      double best = dx * dx + dy * dy + dz * dz;
+      const double di2 = dx * dx + dy * dy + dz * dz;
+      double best = di2;
       int bestId = i;
       nearest<HV>(g, qx, qy, qz, best, bestId, st, true);
-      bool inside = bestId == i;
-      if (!inside) {
+      // closed cell: a tie up to rounding is inside; a near tie is when the other site owns an edge of P (U6, U17)
+      bool inside = bestId == i || best >= di2 * (1.0 - 1e-13);
+      if (!inside && best >= di2 * (1.0 - 1e-9)) {
         bool own = false;
         for (int f = lane; f < nc; f += kLanes) own |= (S.eflag[f] == bestId);
         inside = __any_sync(kFull, own);   // flag rule (reading U6)

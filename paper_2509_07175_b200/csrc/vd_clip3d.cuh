@@ -320,7 +320,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
 }
 
 // returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
-template <int P, int C, bool HV>
+template <int P, int C, bool HV, bool BOX>
 __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = load_pair(A, pairIdx);
@@ -328,15 +328,14 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   // ---- P <- T (Alg. 3 line 1): 4 planes (flags from the simplex adjacency), 4 corners.  Lane k < 4
   // loads tet vertex k; coordinates are local to vertex 0.  The per-pair constants live in shared memory
   // (S.u), not in registers: they would be spilled around every call of the query routines.
-  double vx = 0, vy = 0, vz = 0;
-  int vk = 0;
-  if (lane < 4) {
-    vk = __ldg(&A.simp[(int64_t)a * 4 + lane]);
-    vx = __ldg(&A.verts[(int64_t)vk * 3 + 0]); vy = __ldg(&A.verts[(int64_t)vk * 3 + 1]); vz = __ldg(&A.verts[(int64_t)vk * 3 + 2]);
-  }
-  {
+  int np = 4, nc = 4;
+  if constexpr (BOX) {
+    // simple domain (section V-B): P <- the box; verts holds its 8 corners, corner c = bits (x, y, z),
+    // planes 0..5 = -x +x -y +y -z +z, local origin = lo
+    double vx = 0, vy = 0, vz = 0;
+    if (lane < 8) { vx = __ldg(&A.verts[lane * 3 + 0]); vy = __ldg(&A.verts[lane * 3 + 1]); vz = __ldg(&A.verts[lane * 3 + 2]); }
     const double o0 = shfl(vx, 0), o1 = shfl(vy, 0), o2 = shfl(vz, 0);
-    if (lane < 4) { S.cx[lane] = vx - o0; S.cy[lane] = vy - o1; S.cz[lane] = vz - o2; }
+    const double e0 = shfl(vx, 7) - o0, e1 = shfl(vy, 7) - o1, e2 = shfl(vz, 7) - o2;
     if (lane == 0) {
       const double s0 = __ldg(&A.sites[(int64_t)i * 3 + 0]), s1 = __ldg(&A.sites[(int64_t)i * 3 + 1]), s2 = __ldg(&A.sites[(int64_t)i * 3 + 2]);
       S.u[0] = o0; S.u[1] = o1; S.u[2] = o2;
@@ -344,37 +343,77 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
       S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
       S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
     }
+    if (lane < 6) {
+      const int axis = lane >> 1, hiSide = lane & 1;
+      const double sg = hiSide ? 1.0 : -1.0;
+      S.pnx[lane] = axis == 0 ? sg : 0.0; S.pny[lane] = axis == 1 ? sg : 0.0; S.pnz[lane] = axis == 2 ? sg : 0.0;
+      S.pd[lane] = hiSide ? (axis == 0 ? e0 : (axis == 1 ? e1 : e2)) : 0.0;
+      S.pflag[lane] = ~A.m;
+    }
+    if (lane < 8) {
+      const int c = lane;
+      S.cx[c] = (c & 1) ? e0 : 0.0; S.cy[c] = (c & 2) ? e1 : 0.0; S.cz[c] = (c & 4) ? e2 : 0.0;
+      const int px = (c & 1) ? 1 : 0, py = (c & 2) ? 3 : 2, pz = (c & 4) ? 5 : 4;
+      // cyclic plane order mirrored at odd corners, so that neighbours traverse the shared edge in opposite directions
+      const bool odd = __popc(c) & 1;
+      S.cp[c][0] = (unsigned short)px; S.cp[c][1] = (unsigned short)(odd ? pz : py); S.cp[c][2] = (unsigned short)(odd ? py : pz);
+      S.cadj[c][0] = (unsigned short)(odd ? (c ^ 2) : (c ^ 4));
+      S.cadj[c][1] = (unsigned short)(c ^ 1);
+      S.cadj[c][2] = (unsigned short)(odd ? (c ^ 4) : (c ^ 2));
+      const int nn = __ldg(&A.vnn[c]);
+      S.cnn[c] = nn;
+      S.cstate[c] = (nn == i) ? ST_IN : ST_OUT;
+    }
+    np = 6; nc = 8;
+  } else {
+    double vx = 0, vy = 0, vz = 0;
+    int vk = 0;
+    if (lane < 4) {
+      vk = __ldg(&A.simp[(int64_t)a * 4 + lane]);
+      vx = __ldg(&A.verts[(int64_t)vk * 3 + 0]); vy = __ldg(&A.verts[(int64_t)vk * 3 + 1]); vz = __ldg(&A.verts[(int64_t)vk * 3 + 2]);
+    }
+    {
+      const double o0 = shfl(vx, 0), o1 = shfl(vy, 0), o2 = shfl(vz, 0);
+      if (lane < 4) { S.cx[lane] = vx - o0; S.cy[lane] = vy - o1; S.cz[lane] = vz - o2; }
+      if (lane == 0) {
+        const double s0 = __ldg(&A.sites[(int64_t)i * 3 + 0]), s1 = __ldg(&A.sites[(int64_t)i * 3 + 1]), s2 = __ldg(&A.sites[(int64_t)i * 3 + 2]);
+        S.u[0] = o0; S.u[1] = o1; S.u[2] = o2;
+        S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
+        S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
+        S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
+      }
+    }
+    __syncwarp();
+    if (lane < 4) {
+      const int k = lane;
+      const int q0 = (k + 1) & 3, q1 = (k + 2) & 3, q2 = (k + 3) & 3;
+      const double ax = S.cx[q1] - S.cx[q0], ay = S.cy[q1] - S.cy[q0], az = S.cz[q1] - S.cz[q0];
+      const double bx = S.cx[q2] - S.cx[q0], by = S.cy[q2] - S.cy[q0], bz = S.cz[q2] - S.cz[q0];
+      double nx = ay * bz - az * by, ny = az * bx - ax * bz, nz = ax * by - ay * bx;
+      const double side = nx * (S.cx[k] - S.cx[q0]) + ny * (S.cy[k] - S.cy[q0]) + nz * (S.cz[k] - S.cz[q0]);
+      if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
+      S.pnx[k] = nx; S.pny[k] = ny; S.pnz[k] = nz;
+      S.pd[k] = nx * S.cx[q0] + ny * S.cy[q0] + nz * S.cz[q0];
+      S.pflag[k] = ~__ldg(&A.adj[(int64_t)a * 4 + k]);
+      // corner k = tet vertex k = the three faces other than k, cyclically ordered so that neighbouring
+      // corners traverse their shared edge in opposite directions: (1,3,2) (0,2,3) (0,3,1) (0,1,2)
+      const int t0 = (k == 0) ? 1 : 0;
+      const int t1 = (k == 0) ? 3 : ((k == 1) ? 2 : ((k == 2) ? 3 : 1));
+      const int t2 = (k == 0) ? 2 : ((k == 1) ? 3 : ((k == 2) ? 1 : 2));
+      S.cp[k][0] = (unsigned short)t0; S.cp[k][1] = (unsigned short)t1; S.cp[k][2] = (unsigned short)t2;
+      S.cadj[k][0] = (unsigned short)(6 - k - t0 - t1);
+      S.cadj[k][1] = (unsigned short)(6 - k - t1 - t2);
+      S.cadj[k][2] = (unsigned short)(6 - k - t2 - t0);
+      // corners of T are classified from the per-vertex nearest site (S3): in Omega_i iff N_p = v_i
+      const int nn = __ldg(&A.vnn[vk]);
+      S.cnn[k] = nn;
+      S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
+    }
+    __syncwarp();
   }
   __syncwarp();
   const double &ox = S.u[0], &oy = S.u[1], &oz = S.u[2], &six = S.u[3], &siy = S.u[4], &siz = S.u[5];
   const double &vix = S.u[6], &viy = S.u[7], &viz = S.u[8], &wx = S.u[9], &wy = S.u[10], &wz = S.u[11];
-  if (lane < 4) {
-    const int k = lane;
-    const int q0 = (k + 1) & 3, q1 = (k + 2) & 3, q2 = (k + 3) & 3;
-    const double ax = S.cx[q1] - S.cx[q0], ay = S.cy[q1] - S.cy[q0], az = S.cz[q1] - S.cz[q0];
-    const double bx = S.cx[q2] - S.cx[q0], by = S.cy[q2] - S.cy[q0], bz = S.cz[q2] - S.cz[q0];
-    double nx = ay * bz - az * by, ny = az * bx - ax * bz, nz = ax * by - ay * bx;
-    const double side = nx * (S.cx[k] - S.cx[q0]) + ny * (S.cy[k] - S.cy[q0]) + nz * (S.cz[k] - S.cz[q0]);
-    if (side > 0) { nx = -nx; ny = -ny; nz = -nz; }
-    S.pnx[k] = nx; S.pny[k] = ny; S.pnz[k] = nz;
-    S.pd[k] = nx * S.cx[q0] + ny * S.cy[q0] + nz * S.cz[q0];
-    S.pflag[k] = ~__ldg(&A.adj[(int64_t)a * 4 + k]);
-    // corner k = tet vertex k = the three faces other than k, cyclically ordered so that neighbouring
-    // corners traverse their shared edge in opposite directions: (1,3,2) (0,2,3) (0,3,1) (0,1,2)
-    const int t0 = (k == 0) ? 1 : 0;
-    const int t1 = (k == 0) ? 3 : ((k == 1) ? 2 : ((k == 2) ? 3 : 1));
-    const int t2 = (k == 0) ? 2 : ((k == 1) ? 3 : ((k == 2) ? 1 : 2));
-    S.cp[k][0] = (unsigned short)t0; S.cp[k][1] = (unsigned short)t1; S.cp[k][2] = (unsigned short)t2;
-    S.cadj[k][0] = (unsigned short)(6 - k - t0 - t1);
-    S.cadj[k][1] = (unsigned short)(6 - k - t1 - t2);
-    S.cadj[k][2] = (unsigned short)(6 - k - t2 - t0);
-    // corners of T are classified from the per-vertex nearest site (S3): in Omega_i iff N_p = v_i
-    const int nn = __ldg(&A.vnn[vk]);
-    S.cnn[k] = nn;
-    S.cstate[k] = (nn == i) ? ST_IN : ST_OUT;
-  }
-  __syncwarp();
-  int np = 4, nc = 4;
   bool failed = false;
 
   // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
@@ -405,11 +444,20 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
       batch_nearest<HV>(g, Q, nq, st);
       if (lane < nq) {
         const int c = Q.item[lane], id = Q.bestId[lane];
-        bool inside = id == i;
-        // flag rule in the form of reading U6: N_q already owns a plane of P
-        for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
+        // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
+        // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
+        // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
+        // such site ends the query, U17) means outside.
+        const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
+        const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
+        bool inside = id == i || best >= di2 * (1.0 - 1e-13);
+        if (!inside && best >= di2 * (1.0 - 1e-9))
+          for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
         S.cstate[c] = inside ? ST_IN : ST_OUT;
         S.cnn[c] = id;
+#ifdef VD_TRACE
+        printf("pair(%d,%d) classify c=%d q=(%g,%g,%g) best=%g di2=%g id=%d inside=%d\n", a, i, c, Q.qx[lane], Q.qy[lane], Q.qz[lane], best, di2, id, (int)inside);
+#endif
       }
       __syncwarp();
     }

@@ -143,10 +143,13 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
 #ifdef VD_TRACE
     if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
 #endif
-    if (bestId == i || bestId == j) return j;
-    bool own = false;
-    for (int f = lane_id(); f < nflags; f += kLanes) own |= (flags[f] == bestId);
-    if (__any_sync(kFull, own)) return j;
+    const double bound = fmin(di2, dj2);
+    if (bestId == i || bestId == j || best >= bound * (1.0 - 1e-13)) return j;   // nothing nearer, up to rounding
+    if (best >= bound * (1.0 - 1e-9)) {   // a (near) tie with a site that owns a plane of P: flag rule
+      bool own = false;
+      for (int f = lane_id(); f < nflags; f += kLanes) own |= (flags[f] == bestId);
+      if (__any_sync(kFull, own)) return j;
+    }
     j = bestId;
     ptx = qx; pty = qy; ptz = qz;
   }

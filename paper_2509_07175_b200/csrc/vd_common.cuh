@@ -19,7 +19,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kWarpsPerBlock = 8;
 constexpr int kBlock = kWarpsPerBlock * kLanes;
 
-enum { KIND_TRI_2D = 0, KIND_TRI_SURFACE = 1, KIND_TET_3D = 2 };
+enum { KIND_TRI_2D = 0, KIND_TRI_SURFACE = 1, KIND_TET_3D = 2, KIND_BOX_2D = 3, KIND_BOX_3D = 4 };
 
 // device-side sticky error bits (read once at the end of vd_compute)
 enum {

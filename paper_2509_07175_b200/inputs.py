@@ -9,7 +9,8 @@ density L399, sites far from the domain L481, surface meshes L290), whose own me
 and site sets are not available.
 
 Domain kinds follow ``include/vd.h``: 0 = 2D triangles, 1 = surface triangles (in
-R^3), 2 = 3D tetrahedra.
+R^3), 2 = 3D tetrahedra, 3 / 4 = axis-aligned rectangle / box given by (lo, hi)
+(the "simple domains" of PAPER.md L241-243: no mesh, one piece per cell).
 """
 from __future__ import annotations
 
@@ -21,6 +22,8 @@ import numpy as np
 KIND_TRI_2D = 0
 KIND_TRI_SURFACE = 1
 KIND_TET_3D = 2
+KIND_BOX_2D = 3
+KIND_BOX_3D = 4
 
 
 @dataclass
@@ -30,7 +33,7 @@ class Workload:
     dim: int
     sites: np.ndarray      # [n, dim] float64
     verts: np.ndarray      # [nv, dim] float64
-    simplices: np.ndarray  # [m, 3 or 4] int32
+    simplices: np.ndarray  # [m, 3 or 4] int32; None for the box kinds
     measure: float         # |M| (area / surface area / volume), from the mesh recipe
     diameter: float        # diameter of the domain's bounding box
 
@@ -40,7 +43,7 @@ class Workload:
 
     @property
     def m(self) -> int:
-        return int(self.simplices.shape[0])
+        return 1 if self.simplices is None else int(self.simplices.shape[0])
 
 
 # --------------------------------------------------------------------------- domains
@@ -209,6 +212,17 @@ def config(idx: int, scale: str = "full") -> Workload:
 
 def custom(kind: int, sites, verts, simplices, name="custom") -> Workload:
     return _wl(name, kind, np.asarray(sites, dtype=np.float64), verts, simplices)
+
+
+def box(dim: int, n: int, seed: int = 7, lo=None, hi=None, name=None) -> Workload:
+    """n white-noise sites in an axis-aligned box, the box itself as the (simple) domain: the paper's
+    "Voronoi diagram of sites in a cube" setting (Fig. 1 caption L5, Table VI)."""
+    lo = np.zeros(dim) if lo is None else np.asarray(lo, dtype=np.float64)
+    hi = np.ones(dim) if hi is None else np.asarray(hi, dtype=np.float64)
+    rng = np.random.default_rng(seed)
+    sites = lo + (hi - lo) * rng.random((n, dim))
+    return Workload(name or f"box{dim}d_{n}", KIND_BOX_2D if dim == 2 else KIND_BOX_3D, dim, sites,
+                    np.stack([lo, hi]), None, float(np.prod(hi - lo)), float(np.linalg.norm(hi - lo)))
 
 
 def grid_sites(k: int, dim: int) -> np.ndarray:

@@ -42,3 +42,25 @@ def test_full_config_invariants_and_sampled_parity(idx, k):
     tier = "A" if w.kind == inputs.KIND_TRI_SURFACE else "B"
     o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=ids, tier=tier)
     bad = parity.assert_parity(g, o, w.diameter, allow_excused=1, abs_measure=1e-12 * w.measure / w.m)
+
+
+@pytest.mark.parametrize("dim,n,k", [(3, 1000000, 256), (2, 2000000, 256)])
+def test_box_domain_at_scale(dim, n, k):
+    """Whole-cell mode at the paper's scale of sites in a cube / square: cells partition
+    the box, neighbour relation symmetric, sampled cells equal the oracle's."""
+    w = inputs.box(dim, n, seed=9)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, None, w.kind)
+        ctx.compute()
+        g = ctx.to_host()
+        cnt = ctx.counters()
+    assert abs(g.measure.sum() - 1.0) <= 1e-11
+    assert np.abs((g.measure[:, None] * g.centroid).sum(0) - 0.5).max() <= 1e-11
+    assert cnt["pieces"] == n and (np.diff(g.piece_off) == 1).all()
+    src = np.repeat(np.arange(n, dtype=np.int64), np.diff(g.nbr_off))
+    fwd = np.sort(src * n + g.nbr)
+    rev = np.sort(g.nbr.astype(np.int64) * n + src)
+    assert np.array_equal(fwd, rev)
+    ids = _sample(g, n, k, 77 + dim)
+    o = oracle.compute(w.sites, w.verts, None, w.kind, subset=ids, tier="B")
+    parity.assert_parity(g, o, w.diameter, ids=ids, allow_excused=1)

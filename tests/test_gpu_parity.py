@@ -186,3 +186,90 @@ def test_lloyd_iterations_follow_the_oracle():
         assert np.allclose(g.measure, o.measure, rtol=1e-7, atol=1e-12)
         # Lloyd's method lowers the CVT energy: cells get more equal in size
         assert g.measure.std() < oracle.compute(s0, v, t, kind).measure.std()
+
+
+# ---------------------------------------------------------------------- simple domains
+def _box_parity(w, subset=None, **opts):
+    g, cnt, _ = _gpu(w, **opts)
+    o = oracle.compute(w.sites, w.verts, None, w.kind, subset=subset, tier="A" if w.n <= 6000 else "B")
+    parity.assert_parity(g, o, w.diameter, ids=subset)
+    assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
+    return g, o, cnt
+
+
+@pytest.mark.parametrize("dim,n", [(2, 20000), (3, 6000)])
+def test_box_domain_parity(dim, n):
+    w = inputs.box(dim, n, seed=31)
+    g, o, cnt = _box_parity(w)
+    assert cnt["pieces"] == n and (g.piece_simplex == 0).all()
+    assert np.array_equal(g.piece_off, np.arange(n + 1))
+
+
+def test_box_domain_golden_hand_cases():
+    import json, os
+    here = os.path.dirname(os.path.abspath(__file__))
+    cases = json.load(open(os.path.join(here, "golden", "unit_square_cases.json")))["cases"]
+    box = np.array([[0.0, 0.0], [1.0, 1.0]])
+    for case in cases:
+        s = np.array(case["sites"], dtype=np.float64)
+        g = binding.compute(s, box, None, binding.VD_BOX_2D)
+        assert np.allclose(g.measure, case["area"], rtol=0, atol=1e-12)
+        for i, nb in enumerate(case["nbr"]):
+            assert g.neighbours(i).tolist() == nb
+
+
+def test_box_domain_sites_outside_clustered_and_shifted():
+    rng = np.random.default_rng(8)
+    lo, hi = np.array([0.1, -0.2, 0.3]), np.array([1.3, 0.9, 1.1])
+    inside = lo + (hi - lo) * rng.random((1500, 3))
+    around = lo + (hi - lo) * (rng.random((1500, 3)) * 1.6 - 0.3)
+    blob = lo + (hi - lo) * (0.5 + 0.01 * rng.standard_normal((1500, 3)))
+    sites = np.concatenate([inside, around, blob])
+    w = inputs.Workload("box_mixed", inputs.KIND_BOX_3D, 3, sites, np.stack([lo, hi]), None,
+                        float(np.prod(hi - lo)), float(np.linalg.norm(hi - lo)))
+    g, o, cnt = _box_parity(w)
+    assert (g.measure == 0).any()       # far outside sites own nothing of the box
+    # a box that contains no site at all: every cell is cut by box faces only from outside
+    w2 = inputs.Workload("box_empty", inputs.KIND_BOX_3D, 3, sites, np.stack([hi + 0.05, hi + 0.2]), None,
+                         0.15 ** 3, float(np.linalg.norm([0.15] * 3)))
+    _box_parity(w2)
+
+
+def test_box_domain_edge_cases():
+    one = inputs.box(3, 1)
+    g, _, _ = _gpu(one)
+    assert abs(g.measure[0] - 1.0) <= 1e-15 and g.neighbours(0).size == 0
+    assert int(g.vert_off[1]) == 8 and (g.vert_flags == ~1).all()
+    two = inputs.box(2, 2, seed=3)
+    _box_parity(two)
+    # regular grid: every Voronoi corner is degenerate (4 / 8 equidistant sites)
+    for dim, k in [(2, 16), (3, 6)]:
+        s = inputs.grid_sites(k, dim)
+        w = inputs.Workload("box_grid", inputs.KIND_BOX_2D if dim == 2 else inputs.KIND_BOX_3D, dim, s,
+                            np.stack([np.zeros(dim), np.ones(dim)]), None, 1.0, float(np.sqrt(dim)))
+        g, _, _ = _gpu(w)
+        assert np.allclose(g.measure, 1.0 / k ** dim, rtol=1e-9, atol=0)
+        assert np.abs(g.centroid - s).max() <= 1e-9
+    # bad boxes
+    with binding.Context(one.sites) as ctx:
+        with pytest.raises(binding.VdError) as e:
+            ctx.set_domain(np.array([[0.0, 0, 0], [1.0, 1.0, 0.0]]), None, binding.VD_BOX_3D)
+        assert e.value.status == 4
+        with pytest.raises(binding.VdError) as e:
+            ctx.set_domain(np.array([[0.0, 0], [1.0, 1.0]]), None, binding.VD_BOX_2D)
+        assert e.value.status == 2
+
+
+def test_box_domain_wave_mode_and_lloyd():
+    w = inputs.box(3, 3000, seed=5)
+    _box_parity(w, persistent=0)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, None, w.kind)
+        s = w.sites
+        for _ in range(2):
+            o = oracle.compute(s, w.verts, None, w.kind, tier="B")
+            s = np.where((o.measure > 0)[:, None], o.centroid, s)
+        got = ctx.lloyd(2)
+        assert np.abs(got - s).max() <= 1e-9
+        g = ctx.to_host()
+        parity.assert_parity(g, oracle.compute(got, w.verts, None, w.kind, tier="B"), w.diameter)

@@ -240,3 +240,58 @@ def test_surface_pieces_lie_in_their_triangle():
     empty = c.measure == 0
     assert empty.any()
     assert np.array_equal(c.centroid[empty], w.sites[empty])
+
+
+# ---------------------------------------------------------------------- simple domains (box kinds)
+@pytest.mark.parametrize("dim", [2, 3])
+def test_box_cells_are_the_dissolved_mesh_cells(dim):
+    """The box kinds must give, per site, exactly the union of the pieces the meshed kinds give on a
+    mesh of the same box (Eq. 1 does not depend on how the domain is cut up): same measure, centroid
+    and neighbour sets; every corner with a box-face flag lies on the box boundary."""
+    n = 300
+    wb = inputs.box(dim, n, seed=21)
+    if dim == 2:
+        v, t = inputs.square_grid_mesh(3)
+        kind = inputs.KIND_TRI_2D
+    else:
+        v, t = inputs.cube_kuhn_mesh(2)
+        kind = inputs.KIND_TET_3D
+    cm = oracle.compute(wb.sites, v, t, kind)
+    cb = oracle.compute(wb.sites, wb.verts, None, wb.kind)
+    assert abs(cb.measure.sum() - 1.0) <= 1e-12
+    assert np.allclose(cb.measure, cm.measure, rtol=1e-11, atol=0)
+    assert np.abs(cb.centroid - cm.centroid).max() <= 1e-12
+    assert np.array_equal(cb.nbr_off, cm.nbr_off) and np.array_equal(cb.nbr, cm.nbr)
+    assert np.array_equal(cb.piece_off, np.arange(n + 1)) and (cb.piece_simplex == 0).all()
+    on_face = (cb.vert_flags == ~1).any(axis=1)
+    x = cb.vert_xyz[on_face]
+    assert (np.minimum(np.abs(x), np.abs(x - 1.0)).min(axis=1) <= 1e-14).all()
+    assert on_face.any() and (~on_face).any()
+
+
+def test_box_cells_qhull_and_tiers():
+    """Interior cells of a shifted, non-cubic box against Qhull; tier A == tier B; sites outside the box."""
+    from scipy.spatial import ConvexHull, Voronoi
+    lo, hi = np.array([0.1, -0.2, 0.3]), np.array([1.3, 0.9, 1.1])
+    rng = np.random.default_rng(4)
+    sites = lo + (hi - lo) * (rng.random((400, 3)) * 1.2 - 0.1)
+    box = np.stack([lo, hi])
+    a = oracle.compute(sites, box, None, inputs.KIND_BOX_3D)
+    b = oracle.compute(sites, box, None, inputs.KIND_BOX_3D, tier="B")
+    assert abs(a.measure.sum() - np.prod(hi - lo)) <= 1e-12
+    assert np.array_equal(a.vert_flags, b.vert_flags) and np.array_equal(a.nbr, b.nbr)
+    assert np.allclose(a.measure, b.measure, rtol=1e-11, atol=0)
+    vor = Voronoi(sites)
+    checked = 0
+    for i in range(len(sites)):
+        if a.measure[i] == 0:
+            continue
+        _, fl = a.piece_verts(int(a.piece_off[i]))
+        if (fl < 0).any():
+            continue
+        region = vor.regions[vor.point_region[i]]
+        assert -1 not in region
+        vol = ConvexHull(vor.vertices[region]).volume
+        assert abs(vol - a.measure[i]) <= 1e-9 * vol
+        checked += 1
+    assert checked > 40
