@@ -84,14 +84,20 @@ typedef struct vd_cells {
 /* Tunables (P:L383 grid density; P:L369 step-out).  Zero / negative fields mean "default". */
 typedef struct vd_options {
   double grid_density;    /* average sites per grid cell of the site index (default 4.0; paper 2~4) */
-  int32_t step_out;       /* 1: use the improved search of section VI-A; default 0     */
+  int32_t ball_cells;     /* one-shot bisector search (reading U18): most grid cells its ball
+                             scan may cover; 0 = default (64); < 0: only the stepwise search of P:L137.
+                             (The step-out of section VI-A, is not needed: U7.)            */
   int32_t real_edges;     /* 1 (default): search on a real edge p_s p_t when the outside corner has
                              a known-inside neighbour (Alg. 1); 0: always the virtual
                              edge from the pair's witness point (Alg. 3)               */
   int32_t persistent;     /* 1 (default): device-side work queue; 0: one launch per wave  */
   int64_t pair_capacity;  /* initial capacity of the (simplex, site) pair list; grows on demand     */
   int64_t vert_capacity;  /* initial capacity of the corner pool; grows on demand                   */
-  int32_t reserved[8];
+  int32_t near_clips;     /* every piece of cell i is first clipped by the bisectors of this many of the
+                             sites nearest to v_i (reading U19), so that the point-in-cell loop
+                             starts from a small polytope; 0 = default (20 for VD_BOX_3D, none for the
+                             other kinds); < 0: none; at most 32.  3D kinds only.                        */
+  int32_t reserved[7];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */

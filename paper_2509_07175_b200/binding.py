@@ -42,9 +42,9 @@ class vd_cells(ctypes.Structure):
 
 
 class vd_options(ctypes.Structure):
-    _fields_ = [("grid_density", ctypes.c_double), ("step_out", ctypes.c_int32), ("real_edges", ctypes.c_int32),
+    _fields_ = [("grid_density", ctypes.c_double), ("ball_cells", ctypes.c_int32), ("real_edges", ctypes.c_int32),
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
-                ("reserved", ctypes.c_int32 * 8)]
+                ("near_clips", ctypes.c_int32), ("reserved", ctypes.c_int32 * 7)]
 
 
 class vd_counters(ctypes.Structure):

@@ -94,7 +94,6 @@ __global__ void __launch_bounds__(kBlock) k_unpad3(const double* __restrict__ in
 static void set_default_options(vd_options& o) {
   memset(&o, 0, sizeof(o));
   o.grid_density = 4.0;
-  o.step_out = 0;
   o.real_edges = 1;
   o.persistent = 1;
 }
@@ -325,7 +324,7 @@ void vd_destroy(vd_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->vnn, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
+                   &c->scanTmp, &c->vnn, &c->nearList, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
                    &c->oPieceMeasure, &c->oVertOff, &c->oVertXYZ, &c->oVertFlags};

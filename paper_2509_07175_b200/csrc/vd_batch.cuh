@@ -46,12 +46,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& g, QBatch& B,
       if (myRows > kQBMaxRows) { loose = true; myRows = 0; }
     }
   }
-  int incl = myRows;
-#pragma unroll
-  for (int off = 1; off < kQB; off <<= 1) {
-    const int o = __shfl_up_sync(kFull, incl, off);
-    if (lane >= off) incl += o;
-  }
+  const int incl = warp_incl_scan(myRows);
   if (lane < nq) B.rowStart[lane] = incl - myRows;
   if (lane == nq - 1) B.rowStart[nq] = incl;
   unsigned looseMask = __ballot_sync(kFull, loose);
@@ -75,12 +70,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& g, QBatch& B,
         cnt = __ldg(&g.cellStart[rowBase + B.x1[u] + 1]) - s;
       }
     }
-    int pin = cnt;
-#pragma unroll
-    for (int off = 1; off < kLanes; off <<= 1) {
-      const int o = __shfl_up_sync(kFull, pin, off);
-      if (lane >= off) pin += o;
-    }
+    const int pin = warp_incl_scan(cnt);
     const int excl = pin - cnt;
     const int total = shfl(pin, kLanes - 1);
     st.dist_evals += (unsigned)total;

@@ -28,6 +28,22 @@ __global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, double lx, do
   }
 }
 
+// Reading U19: the sites nearest to every site (approximately, from the 3 x 3 x 3 grid cells around it), nearest
+// first; one warp per site.  Their bisectors are the first clips of every piece of that site's cell.
+__global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ list, int K) {
+  __shared__ GridIndex g;
+  __shared__ int ids[kWarpsPerBlock][kLanes];
+  if (threadIdx.x == 0) g = *A.grid;
+  __syncthreads();
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  QueryStats st = {0u, 0u, 0u};
+  for (int64_t i = (int64_t)blockIdx.x * kWarpsPerBlock + w; i < A.n; i += (int64_t)gridDim.x * kWarpsPerBlock) {
+    const int k = near_sites(g, A.sites[i * 3 + 0], A.sites[i * 3 + 1], A.sites[i * 3 + 2], (int)i, K, ids[w], st);
+    if (lane < K) list[i * K + lane] = lane < k ? ids[w][lane] : -1;
+    __syncwarp();
+  }
+}
+
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
@@ -94,6 +110,14 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
   flush_counters(A.ctl, st, lc);
 }
 
+// reading U19: by default only the whole-cell kinds start from the bisectors of the nearest sites (measured: on
+// tet meshes the extra plane tests and redundant clips cost more than the searches they save)
+static int near_clips_of(const vd_ctx* c) {
+  const int k = c->opt.near_clips;
+  if (k == 0) return (c->kind == KIND_BOX_3D) ? 20 : 0;
+  return k > kLanes ? kLanes : k;
+}
+
 static ClipArgs make_args(vd_ctx* c) {
   ClipArgs A;
   A.grid = c->grid.as<GridIndex>();
@@ -102,8 +126,12 @@ static ClipArgs make_args(vd_ctx* c) {
   A.simp = c->simp.as<int>();
   A.adj = c->adj.as<int>();
   A.vnn = c->vnn.as<int>();
+  A.nearList = nullptr;
   A.n = (int)c->n; A.m = (int)c->m; A.kind = c->kind;
-  A.realEdges = c->opt.real_edges; A.stepOut = c->opt.step_out;
+  A.realEdges = c->opt.real_edges;
+  A.ballCells = c->opt.ball_cells == 0 ? 64 : c->opt.ball_cells;
+  A.nearClips = near_clips_of(c);
+  if (A.nearClips > 0 && c->nearList.p) A.nearList = c->nearList.as<int>();
   A.ctl = c->control.as<Control>();
   A.pairs = c->pairs.as<Pair>();
   A.pieces = c->pieces.as<Piece>();
@@ -136,7 +164,14 @@ vd_status stage_seed(vd_ctx* c) {
   cudaMemsetAsync(c->pairs.p, 0xff, sizeof(Pair) * c->pairCap, st);   // simplex id < 0: slot not yet pushed
   cudaMemsetAsync(c->sitePieces.p, 0, sizeof(int) * c->n, st);
   cudaMemsetAsync(c->siteNbrRaw.p, 0, sizeof(int) * c->n, st);
+  const int K = near_clips_of(c);
+  if (K > 0) {
+    if ((s = ensure(c, c->nearList, sizeof(int) * c->n * K))) return s;
+  } else {
+    release(c, c->nearList);
+  }
   const ClipArgs A = make_args(c);
+  if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, 148 * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
   VD_LAUNCH(k_seed, blocks_for(c->m, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
   if (c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D) {
     double cv[8 * 3];

@@ -82,12 +82,7 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
         if (S.cmark[nb] != 2) { ea[cnt] = S.cp[c][t]; eb[cnt] = S.cp[c][(t + 1) % 3]; en[cnt] = (unsigned short)nb; ++cnt; }
       }
     }
-    int incl = cnt;
-#pragma unroll
-    for (int off = 1; off < kLanes; off <<= 1) {
-      const int o = __shfl_up_sync(kFull, incl, off);
-      if (lane >= off) incl += o;
-    }
+    const int incl = warp_incl_scan(cnt);
     const int base = L + incl - cnt;
     const int tot = shfl(incl, kLanes - 1);
     if (L + tot > P) return 1;
@@ -416,51 +411,40 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   const double &vix = S.u[6], &viy = S.u[7], &viz = S.u[8], &wx = S.u[9], &wy = S.u[10], &wz = S.u[11];
   bool failed = false;
 
-  // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
-  for (int guard = 0; guard < 4 * P + 16; ++guard) {
-    // point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one
-    // batched pass (vd_batch.cuh); the batch state lives in the scratch area S.key
-    static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
-    QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
-    for (;;) {
-      int nq = 0;
-      for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
-        const int c = c0 + lane;
-        const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
-        const unsigned m = __ballot_sync(kFull, unk);
-        const int slot = nq + __popc(m & ((1u << lane) - 1u));
-        if (unk && slot < kQB) {
-          const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
-          const double dx = qx - six, dy = qy - siy, dz = qz - siz;
-          Q.item[slot] = c;
-          Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
-          Q.best[slot] = dx * dx + dy * dy + dz * dz;
-          Q.bestId[slot] = i;
-        }
-        nq = min(kQB, nq + __popc(m));
+  // ---- reading U19: clip by the bisectors of the sites nearest to v_i first.  Any B_ij is a valid clip of
+  // Omega_i (Eq. 1); these need no search, most of them bound the cell, and what is left for the point-in-cell
+  // loop is a small polytope around the cell.  A plane that does not cut P is skipped.
+  if (A.nearList) {
+    const int K = A.nearClips;
+    const int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
+    for (int t = 0; t < K; ++t) {
+      const int j = shfl(mine, t);
+      if (j < 0) break;
+      const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
+                   wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+      const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
+      const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+      // the corner farthest beyond the plane starts R_p
+      double far = 0.0;
+      int p = 0x7fffffff;
+      const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
+      for (int c = lane; c < nc; c += kLanes) {
+        const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+        if (sd > tol && S.cstate[c] != ST_IN && closer(-sd, c, far, p)) { far = -sd; p = c; }
       }
-      if (nq == 0) break;
-      __syncwarp();
-      batch_nearest<HV>(g, Q, nq, st);
-      if (lane < nq) {
-        const int c = Q.item[lane], id = Q.bestId[lane];
-        // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
-        // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
-        // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
-        // such site ends the query, U17) means outside.
-        const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
-        const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
-        bool inside = id == i || best >= di2 * (1.0 - 1e-13);
-        if (!inside && best >= di2 * (1.0 - 1e-9))
-          for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
-        S.cstate[c] = inside ? ST_IN : ST_OUT;
-        S.cnn[c] = id;
-#ifdef VD_TRACE
-        printf("pair(%d,%d) classify c=%d q=(%g,%g,%g) best=%g di2=%g id=%d inside=%d\n", a, i, c, Q.qx[lane], Q.qy[lane], Q.qz[lane], best, di2, id, (int)inside);
-#endif
-      }
-      __syncwarp();
+      warp_argmin(far, p);
+      if (p == 0x7fffffff) continue;   // the plane does not cut P
+      if (np >= P) return 1;
+      lc.clips += 1;
+      const int rc = apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
+      if (rc == 1) return 1;
+      if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); break; }
+      if (nc == 0) break;
     }
+  }
+
+  // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
+  for (int guard = 0; guard < 8 * P + 32 && !failed; ++guard) {
     // select an outside corner p; prefer one with a neighbour p_s in Omega_i (a real edge, Alg. 1 line 3)
     int p = -1, s = -1;
     for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
@@ -477,7 +461,57 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
       if (mr) { const int src = __ffs(mr) - 1; p = c0 + src; s = shfl(sn, src); }
       else if (mo) { p = c0 + __ffs(mo) - 1; }
     }
-    if (p < 0) break;            // every corner is in Omega_i: P = T ∩ Omega_i
+    if (p < 0) {
+      // no corner is known to be outside: only now test the unclassified ones -- a clip from a known outside
+      // corner removes unclassified corners beyond its plane for free (they are candidates of R_p)
+      // point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one
+      // batched pass (vd_batch.cuh); the batch state lives in the scratch area S.key
+      static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
+      QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
+      bool any = false;
+      for (;;) {
+        int nq = 0;
+        for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
+          const int c = c0 + lane;
+          const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
+          const unsigned m = __ballot_sync(kFull, unk);
+          const int slot = nq + __popc(m & ((1u << lane) - 1u));
+          if (unk && slot < kQB) {
+            const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
+            const double dx = qx - six, dy = qy - siy, dz = qz - siz;
+            Q.item[slot] = c;
+            Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
+            Q.best[slot] = dx * dx + dy * dy + dz * dz;
+            Q.bestId[slot] = i;
+          }
+          nq = min(kQB, nq + __popc(m));
+        }
+        if (nq == 0) break;
+        any = true;
+        __syncwarp();
+        batch_nearest<HV>(g, Q, nq, st);
+        if (lane < nq) {
+          const int c = Q.item[lane], id = Q.bestId[lane];
+          // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
+          // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
+          // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
+          // such site ends the query, U17) means outside.
+          const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
+          const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
+          bool inside = id == i || best >= di2 * (1.0 - 1e-13);
+          if (!inside && best >= di2 * (1.0 - 1e-9))
+            for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
+          S.cstate[c] = inside ? ST_IN : ST_OUT;
+          S.cnn[c] = id;
+  #ifdef VD_TRACE
+          printf("pair(%d,%d) classify c=%d q=(%g,%g,%g) best=%g di2=%g id=%d inside=%d\n", a, i, c, Q.qx[lane], Q.qy[lane], Q.qz[lane], best, di2, id, (int)inside);
+  #endif
+        }
+        __syncwarp();
+      }
+      if (!any) break;           // every corner is in Omega_i: P = T ∩ Omega_i
+      continue;
+    }
     if (np >= P) return 1;
     // find a bisector B_ij on the real edge p_s p or on the virtual edge w p (Alg. 1 line 4 / Alg. 3 line 3)
     double psx = wx, psy = wy, psz = wz;

@@ -12,8 +12,9 @@ struct ClipArgs {
   const int* simp;         // [m][nc]
   const int* adj;          // [m][nc]
   const int* vnn;          // [nv] nearest site of every mesh vertex
+  const int* nearList;     // [n][nearClips] or nullptr
   int n, m, kind;
-  int realEdges, stepOut;
+  int realEdges, ballCells, nearClips;
   Control* ctl;
   Pair* pairs;
   Piece* pieces;
@@ -105,6 +106,146 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
   }
 }
 
+// Whole-cell kinds (reading U19): up to k of the sites nearest to v_i among the 3 x 3 x 3 grid cells around it,
+// nearest first, into out[]; returns how many.  Any bisector B_ij is a valid clip of Omega_i (Eq. 1), and the
+// nearest few sites are almost always Voronoi neighbours, so clipping the box by them first costs no search and
+// leaves a small polytope whose corners are all close to the cell.  Selection is approximate on purpose: each
+// lane keeps the nearest of the candidates it saw, the k best lanes win.
+static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, double vy, double vz, int i, int k, int* out, QueryStats& st) {
+  __shared__ int sBaseN[kWarpsPerBlock][kLanes];
+  const int lane = lane_id();
+  int* base = sBaseN[(threadIdx.x / kLanes) % kWarpsPerBlock];
+  const int cx = cell_of(g, 0, vx), cy = cell_of(g, 1, vy), cz = cell_of(g, 2, vz);
+  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.G[0] - 1);
+  const int y0 = max(cy - 1, 0), y1 = min(cy + 1, g.G[1] - 1);
+  const int z0 = max(cz - 1, 0), z1 = min(cz + 1, g.G[2] - 1);
+  const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
+  int s = 0, cnt = 0;
+  if (lane < nrows) {
+    const int rz = lane / ny;
+    const int rowBase = ((z0 + rz) * g.G[1] + y0 + (lane - rz * ny)) * g.G[0];
+    s = __ldg(&g.cellStart[rowBase + x0]);
+    cnt = __ldg(&g.cellStart[rowBase + x1 + 1]) - s;
+  }
+  const int incl = warp_incl_scan(cnt);
+  const int excl = incl - cnt;
+  const int total = min(shfl(incl, kLanes - 1), 16 * kLanes);   // a dense cluster: the first 512 will do
+  st.dist_evals += (unsigned)total;
+  double md = 2e300;
+  int mi = 0x7fffffff;
+  for (int t0 = 0; t0 < total; t0 += kLanes) {
+    unsigned bit = 0;
+    if (cnt > 0) {
+      if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
+      else if (excl < t0 && incl > t0) bit = 1u;
+    }
+    const unsigned starts = __reduce_or_sync(kFull, bit);
+    const unsigned owners = __ballot_sync(kFull, bit != 0);
+    if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
+    __syncwarp();
+    const int t = t0 + lane;
+    if (t < total) {
+      const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
+      const double4 p = g.sites[base[owner] + t];
+      const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
+      const double dx = vx - p.x, dy = vy - p.y, dz = vz - p.z;
+      const double d2 = dx * dx + dy * dy + dz * dz;
+      if (id != i && d2 > 0.0 && closer(d2, id, md, mi)) { md = d2; mi = id; }
+    }
+    __syncwarp();
+  }
+  int found = 0;
+  for (; found < k; ++found) {
+    double bd = md;
+    int bi = mi;
+    warp_argmin(bd, bi);
+    if (bi == 0x7fffffff) break;
+    if (lane == 0) out[found] = bi;
+    if (mi == bi) { md = 2e300; mi = 0x7fffffff; }
+  }
+  __syncwarp();
+  return found;
+}
+
+// One-shot form of the edge-based bisector search (reading U18).  Along p_s -> p_t every g_k(t) = |x-v_k|^2 -
+// |x-v_i|^2 is linear and >= 0 at p_s, so the target bisector is the one with the smallest crossing parameter
+// t_k.  With q = B_ij ∩ segment (parameter tq), every site whose bisector crosses before q is nearer to q than
+// v_i, i.e. lies in the ball (q, |q - v_i|): one complete scan of that ball, keeping the smallest t_k, ends the
+// search -- P:L137's iteration would visit a chain of such sites one nearest-site query at a time.  Sites nearer
+// only within rounding do not compete (1e-13 relative; 1e-9 when the site owns a flag of P: the flag rule of
+// P:L109-111, readings U6/U17).  Returns false, doing nothing, when the ball covers too many grid cells (q still
+// far from Omega_i): the caller then takes an ordinary step.  Coordinates are absolute.  Warp-uniform result.
+static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double qx, double qy, double qz, double r2, double psx,
+                                                    double psy, double psz, double dis2, double tq, int i, int j, const int* flags,
+                                                    int nflags, int maxCells, double& tbest, int& jbest, QueryStats& st) {
+  __shared__ int sBaseT[kWarpsPerBlock][kLanes];
+  const int lane = lane_id();
+  int* base = sBaseT[(threadIdx.x / kLanes) % kWarpsPerBlock];
+  const double r = sqrt(r2);
+  const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
+  const int y0 = cell_of(g, 1, qy - r - 1e-6 * g.h[1]), y1 = cell_of(g, 1, qy + r + 1e-6 * g.h[1]);
+  const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
+  const int ny = y1 - y0 + 1;
+  const int nrows = ny * (z1 - z0 + 1);
+  if (nrows > kLanes || nrows * (x1 - x0 + 1) > maxCells) return false;
+  st.queries += 1;
+  st.rows += (unsigned)nrows;
+  int s = 0, cnt = 0;
+  if (lane < nrows) {
+    const int rz = lane / ny;
+    const int y = y0 + (lane - rz * ny), z = z0 + rz;
+    const double rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
+    if (!(rd2 > r2)) {
+      const double w = sqrt(r2 - rd2);
+      const int xa = max(x0, (int)floor((qx - w - g.lo[0]) * g.inv_h[0] - 1e-6));
+      const int xb = min(x1, (int)floor((qx + w - g.lo[0]) * g.inv_h[0] + 1e-6));
+      if (xa <= xb) {
+        const int rowBase = (z * g.G[1] + y) * g.G[0];
+        s = __ldg(&g.cellStart[rowBase + xa]);
+        cnt = __ldg(&g.cellStart[rowBase + xb + 1]) - s;
+      }
+    }
+  }
+  const int incl = warp_incl_scan(cnt);
+  const int excl = incl - cnt;
+  const int total = shfl(incl, kLanes - 1);
+  st.dist_evals += (unsigned)total;
+  double tb = 2.0;
+  int jb = 0x7fffffff;
+  for (int t0 = 0; t0 < total; t0 += kLanes) {
+    unsigned bit = 0;
+    if (cnt > 0) {
+      if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
+      else if (excl < t0 && incl > t0) bit = 1u;
+    }
+    const unsigned starts = __reduce_or_sync(kFull, bit);
+    const unsigned owners = __ballot_sync(kFull, bit != 0);
+    if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
+    __syncwarp();
+    const int t = t0 + lane;
+    if (t < total) {
+      const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
+      const double4 p = g.sites[base[owner] + t];
+      const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
+      const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
+      const double dq2 = dx * dx + dy * dy + dz * dz;
+      bool cand = id != i && id != j && dq2 < r2 * (1.0 - 1e-13);
+      if (cand && !(dq2 < r2 * (1.0 - 1e-9)))
+        for (int f = 0; f < nflags; ++f) cand = cand && (flags[f] != id);
+      if (cand) {
+        const double ex = psx - p.x, ey = psy - p.y, ez = psz - p.z;
+        const double gs = ex * ex + ey * ey + ez * ez - dis2, gq = dq2 - r2;
+        const double tk = gs > 0.0 ? tq * gs / (gs - gq) : 0.0;
+        if (closer(tk, id, tb, jb)) { tb = tk; jb = id; }
+      }
+    }
+    __syncwarp();
+  }
+  warp_argmin(tb, jb);
+  if (closer(tb, jb, tbest, jbest)) { tbest = tb; jbest = jb; }
+  return true;
+}
+
 // Edge-based bisector search (section IV-B) on the segment p_s -> p_t, all in coordinates
 // local to the origin o.  p_s is in Omega_i, the nearest site of p_t is j != i.  Iterates
 // q = B_ij ∩ segment, k = N_q, until k is i or j; then B_ij is the target bisector.  Along the segment
@@ -136,6 +277,23 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
+    if (!HV && A.ballCells > 0) {
+      // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
+      double tb = 2.0;
+      int jb = 0x7fffffff;
+      const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
+      if (scan_ball_min_t(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz, t, i, j, flags, nflags,
+                          A.ballCells, tb, jb, st)) {
+        if (jb != 0x7fffffff) {
+          j = jb;
+          const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
+                       wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+          nx = wjx - vix; ny = wjy - viy; nz = wjz - viz;
+          d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+        }
+        return j;
+      }
+    }
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }

@@ -84,6 +84,7 @@ __device__ __forceinline__ bool closer(double d2, int id, double best, int bestI
 
 // Warp argmin of (d2, id) with the tie rule "lowest id" (reading U5); result uniform.
 __device__ __forceinline__ void warp_argmin(double& d2, int& id) {
+  // (three __reduce_min_sync over the words of the bit pattern were measured slower than this butterfly)
 #pragma unroll
   for (int off = kLanes / 2; off > 0; off >>= 1) {
     const double od = __shfl_xor_sync(kFull, d2, off);
@@ -101,6 +102,17 @@ __device__ __forceinline__ int warp_sum(int v) {
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int off = kLanes / 2; off > 0; off >>= 1) v += __shfl_xor_sync(kFull, v, off);
+  return v;
+}
+
+// inclusive prefix sum over the lanes
+__device__ __forceinline__ int warp_incl_scan(int v) {
+  const int lane = lane_id();
+#pragma unroll
+  for (int off = 1; off < kLanes; off <<= 1) {
+    const int o = __shfl_up_sync(kFull, v, off);
+    if (lane >= off) v += o;
+  }
   return v;
 }
 

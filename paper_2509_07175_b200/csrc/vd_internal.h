@@ -62,6 +62,7 @@ struct vd_ctx {
   int64_t subCap = 0;
   // S3-S5
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
+  vd::DevBuf nearList;    // int [n][nearClips]  sites nearest to every site, nearest first, -1 padded (reading U19)
   vd::DevBuf control;     // Control
   vd::DevBuf pairs;       // Pair [pairCap]
   vd::DevBuf pieces;      // Piece [pairCap]

@@ -70,12 +70,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         }
       }
     }
-    int incl = cnt;
-#pragma unroll
-    for (int off = 1; off < kLanes; off <<= 1) {
-      const int o = __shfl_up_sync(kFull, incl, off);
-      if (lane >= off) incl += o;
-    }
+    const int incl = warp_incl_scan(cnt);
     const int excl = incl - cnt;
     const int total = shfl(incl, kLanes - 1);
     st.dist_evals += (unsigned)total;

@@ -57,7 +57,8 @@ def test_replica_parity(idx):
     assert g.n_nonempty == int((o.measure > 0).sum())
 
 
-@pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0)])
+@pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
+                                  dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -263,6 +264,8 @@ def test_box_domain_edge_cases():
 def test_box_domain_wave_mode_and_lloyd():
     w = inputs.box(3, 3000, seed=5)
     _box_parity(w, persistent=0)
+    _box_parity(w, near_clips=-1)              # the paper's loop alone, from the whole box
+    _box_parity(w, near_clips=32, ball_cells=-1)
     with binding.Context(w.sites) as ctx:
         ctx.set_domain(w.verts, None, w.kind)
         s = w.sites
