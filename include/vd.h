@@ -90,7 +90,12 @@ typedef struct vd_options {
   int32_t real_edges;     /* 1 (default): search on a real edge p_s p_t when the outside corner has
                              a known-inside neighbour (Alg. 1); 0: always the virtual
                              edge from the pair's witness point (Alg. 3)               */
-  int32_t persistent;     /* 1 (default): device-side work queue; 0: one launch per wave  */
+  int32_t persistent;     /* how S4 is scheduled (P:L257's wavefronts):
+                             1 (default): 3D kinds "phased" -- every step of Alg. 3 is its own small kernel
+                                over a whole wave, polytopes parked in HBM between steps (the one-kernel
+                                form is bound by instruction fetch); 2D / surface kinds: device-side queue;
+                             2: phased (3D kinds only);  3: device-side work queue, one persistent kernel;
+                             0: one launch of the one-kernel form per wave                               */
   int64_t pair_capacity;  /* initial capacity of the (simplex, site) pair list; grows on demand     */
   int64_t vert_capacity;  /* initial capacity of the corner pool; grows on demand                   */
   int32_t near_clips;     /* every piece of cell i is first clipped by the bisectors of this many of the

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvd.so")
-SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_assemble.cu"]
+SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_phase.cu", "vd_assemble.cu"]
 
 
 def lib_path() -> str:

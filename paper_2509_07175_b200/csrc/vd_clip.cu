@@ -44,6 +44,8 @@ __global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ l
   }
 }
 
+vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end);   // vd_phase.cu
+
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
@@ -224,7 +226,10 @@ static void set_cursor(vd_ctx* c, int which, unsigned long long v) {
 
 vd_status stage_clip(vd_ctx* c) {
   const ClipArgs A = make_args(c);
-  const bool persist = c->opt.persistent != 0;
+  const int mode = c->opt.persistent;
+  const bool solid = c->kind == KIND_TET_3D || c->kind == KIND_BOX_3D;
+  const bool phased = solid && (mode == 1 || mode == 2);   // 3D kinds: one small kernel per step (vd_phase.cu)
+  const bool persist = mode != 0 && !phased;               // otherwise the device-side queue, or one launch per wave
   int64_t begin = 0, obegin = 0, waves = 0;
   Control h;
   cudaError_t e = read_control(c, h);   // seeds pushed so far, refined cells of the index
@@ -236,7 +241,12 @@ vd_status stage_clip(vd_ctx* c) {
     if (end > c->pairCap) end = c->pairCap;
     if (oend > c->ovfCap) oend = c->ovfCap;
     if (end == begin && oend == obegin) break;   // "while L1 is not empty"
-    if (end > begin) {
+    if (end > begin && phased) {
+      // phased mode: one small kernel per step of Alg. 3 over the whole wave (vd_phase.cu)
+      const vd_status s = run_phases(c, A, hv, begin, end);
+      if (s != VD_OK) return s;
+      ++waves;
+    } else if (end > begin) {
       // wave mode: one launch per wavefront.  persistent mode: the kernel drains the queue as it grows
       set_cursor(c, 0, persist ? (unsigned long long)begin : 0ull);
       launch(c, A, hv, false, persist ? 0 : begin, end, persist);

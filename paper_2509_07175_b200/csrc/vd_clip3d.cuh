@@ -314,16 +314,23 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   return 0;
 }
 
-// returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
-template <int P, int C, bool HV, bool BOX>
-__device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+// ---- the steps of Alg. 3 on one (simplex, site) pair, as separate functions: the one-kernel path (clip_pair_3d)
+// and the phased path (vd_phase.cu: one small kernel per step, the polytope parked in HBM between them) share them.
+
+#define VD_POLY_REFS                                                                                               \
+  const double &ox = S.u[0], &oy = S.u[1], &oz = S.u[2], &six = S.u[3], &siy = S.u[4], &siz = S.u[5];            \
+  const double &vix = S.u[6], &viy = S.u[7], &viz = S.u[8], &wx = S.u[9], &wy = S.u[10], &wz = S.u[11];          \
+  (void)ox; (void)oy; (void)oz; (void)six; (void)siy; (void)siz; (void)vix; (void)viy; (void)viz; (void)wx; (void)wy; (void)wz
+
+// P <- T_a or the box (Alg. 3 line 1) and the per-pair constants S.u
+template <int P, int C, bool BOX>
+__device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, const Pair& pr, int& np, int& nc) {
   const int lane = lane_id();
-  const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
   // ---- P <- T (Alg. 3 line 1): 4 planes (flags from the simplex adjacency), 4 corners.  Lane k < 4
   // loads tet vertex k; coordinates are local to vertex 0.  The per-pair constants live in shared memory
   // (S.u), not in registers: they would be spilled around every call of the query routines.
-  int np = 4, nc = 4;
+  np = 4; nc = 4;
   if constexpr (BOX) {
     // simple domain (section V-B): P <- the box; verts holds its 8 corners, corner c = bits (x, y, z),
     // planes 0..5 = -x +x -y +y -z +z, local origin = lo
@@ -407,13 +414,15 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
     __syncwarp();
   }
   __syncwarp();
-  const double &ox = S.u[0], &oy = S.u[1], &oz = S.u[2], &six = S.u[3], &siy = S.u[4], &siz = S.u[5];
-  const double &vix = S.u[6], &viy = S.u[7], &viz = S.u[8], &wx = S.u[9], &wy = S.u[10], &wz = S.u[11];
-  bool failed = false;
+}
 
-  // ---- reading U19: clip by the bisectors of the sites nearest to v_i first.  Any B_ij is a valid clip of
-  // Omega_i (Eq. 1); these need no search, most of them bound the cell, and what is left for the point-in-cell
-  // loop is a small polytope around the cell.  A plane that does not cut P is skipped.
+// Reading U19: clip by the bisectors of the sites nearest to v_i first.  Any B_ij is a valid clip of Omega_i
+// (Eq. 1); these need no search, most of them bound the cell, and what is left for the point-in-cell loop is a
+// small polytope around the cell.  A plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology).
+template <int P, int C>
+__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int& np, int& nc, LocalCnt& lc) {
+  const int lane = lane_id();
+  VD_POLY_REFS;
   if (A.nearList) {
     const int K = A.nearClips;
     const int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
@@ -437,107 +446,146 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
       if (np >= P) return 1;
       lc.clips += 1;
       const int rc = apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
-      if (rc == 1) return 1;
-      if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); break; }
+      if (rc) return rc;
       if (nc == 0) break;
     }
   }
 
-  // ---- while P has a corner outside Omega_i (Alg. 3 line 2)
-  for (int guard = 0; guard < 8 * P + 32 && !failed; ++guard) {
-    // select an outside corner p; prefer one with a neighbour p_s in Omega_i (a real edge, Alg. 1 line 3)
-    int p = -1, s = -1;
-    for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
-      const int c = c0 + lane;
-      const bool out = c < nc && S.cstate[c] == ST_OUT;
-      int sn = -1;
-      if (out && A.realEdges) {
+  return 0;
+}
+
+// An outside corner p, preferring one with a neighbour p_s in Omega_i (a real edge, Alg. 1 line 3); -1 if no
+// corner is known to be outside.
+template <int P, int C>
+__device__ __forceinline__ int select_out_3d(const Poly3<P, C>& S, const ClipArgs& A, int nc, int& sOut) {
+  const int lane = lane_id();
+  int p = -1, s = -1;
+  for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
+    const int c = c0 + lane;
+    const bool out = c < nc && S.cstate[c] == ST_OUT;
+    int sn = -1;
+    if (out && A.realEdges) {
 #pragma unroll
-        for (int t = 0; t < 3; ++t)
-          if (S.cstate[S.cadj[c][t]] == ST_IN) sn = S.cadj[c][t];
-      }
-      const unsigned mr = __ballot_sync(kFull, sn >= 0);
-      const unsigned mo = __ballot_sync(kFull, out);
-      if (mr) { const int src = __ffs(mr) - 1; p = c0 + src; s = shfl(sn, src); }
-      else if (mo) { p = c0 + __ffs(mo) - 1; }
+      for (int t = 0; t < 3; ++t)
+        if (S.cstate[S.cadj[c][t]] == ST_IN) sn = S.cadj[c][t];
     }
-    if (p < 0) {
-      // no corner is known to be outside: only now test the unclassified ones -- a clip from a known outside
-      // corner removes unclassified corners beyond its plane for free (they are candidates of R_p)
-      // point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one
-      // batched pass (vd_batch.cuh); the batch state lives in the scratch area S.key
-      static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
-      QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
-      bool any = false;
-      for (;;) {
-        int nq = 0;
-        for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
-          const int c = c0 + lane;
-          const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
-          const unsigned m = __ballot_sync(kFull, unk);
-          const int slot = nq + __popc(m & ((1u << lane) - 1u));
-          if (unk && slot < kQB) {
-            const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
-            const double dx = qx - six, dy = qy - siy, dz = qz - siz;
-            Q.item[slot] = c;
-            Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
-            Q.best[slot] = dx * dx + dy * dy + dz * dz;
-            Q.bestId[slot] = i;
-          }
-          nq = min(kQB, nq + __popc(m));
-        }
-        if (nq == 0) break;
-        any = true;
-        __syncwarp();
-        batch_nearest<HV>(g, Q, nq, st);
-        if (lane < nq) {
-          const int c = Q.item[lane], id = Q.bestId[lane];
-          // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
-          // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
-          // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
-          // such site ends the query, U17) means outside.
-          const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
-          const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
-          bool inside = id == i || best >= di2 * (1.0 - 1e-13);
-          if (!inside && best >= di2 * (1.0 - 1e-9))
-            for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
-          S.cstate[c] = inside ? ST_IN : ST_OUT;
-          S.cnn[c] = id;
-  #ifdef VD_TRACE
-          printf("pair(%d,%d) classify c=%d q=(%g,%g,%g) best=%g di2=%g id=%d inside=%d\n", a, i, c, Q.qx[lane], Q.qy[lane], Q.qz[lane], best, di2, id, (int)inside);
-  #endif
-        }
-        __syncwarp();
+    const unsigned mr = __ballot_sync(kFull, sn >= 0);
+    const unsigned mo = __ballot_sync(kFull, out);
+    if (mr) { const int src = __ffs(mr) - 1; p = c0 + src; s = shfl(sn, src); }
+    else if (mo) { p = c0 + __ffs(mo) - 1; }
+  }
+  sOut = s;
+  return p;
+}
+
+// Point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one batched
+// pass (vd_batch.cuh); the batch state lives in the scratch area S.key.  Returns whether there were any.
+template <int P, int C, bool HV>
+__device__ __forceinline__ bool classify_unknown_3d(Poly3<P, C>& S, const GridIndex& g, int i, int np, int nc, QueryStats& st) {
+  const int lane = lane_id();
+  VD_POLY_REFS;
+  static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
+  QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
+  bool any = false;
+  for (;;) {
+    int nq = 0;
+    for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
+      const int c = c0 + lane;
+      const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
+      const unsigned m = __ballot_sync(kFull, unk);
+      const int slot = nq + __popc(m & ((1u << lane) - 1u));
+      if (unk && slot < kQB) {
+        const double qx = S.cx[c] + ox, qy = S.cy[c] + oy, qz = S.cz[c] + oz;
+        const double dx = qx - six, dy = qy - siy, dz = qz - siz;
+        Q.item[slot] = c;
+        Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
+        Q.best[slot] = dx * dx + dy * dy + dz * dz;
+        Q.bestId[slot] = i;
       }
-      if (!any) break;           // every corner is in Omega_i: P = T ∩ Omega_i
+      nq = min(kQB, nq + __popc(m));
+    }
+    if (nq == 0) break;
+    any = true;
+    __syncwarp();
+    batch_nearest<HV>(g, Q, nq, st);
+    if (lane < nq) {
+      const int c = Q.item[lane], id = Q.bestId[lane];
+      // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
+      // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
+      // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
+      // such site ends the query, U17) means outside.
+      const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
+      const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
+      bool inside = id == i || best >= di2 * (1.0 - 1e-13);
+      if (!inside && best >= di2 * (1.0 - 1e-9))
+        for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);
+      S.cstate[c] = inside ? ST_IN : ST_OUT;
+      S.cnn[c] = id;
+#ifdef VD_TRACE
+      printf("pair(?,%d) classify c=%d q=(%g,%g,%g) best=%g di2=%g id=%d inside=%d\n", i, c, Q.qx[lane], Q.qy[lane], Q.qz[lane], best, di2, id, (int)inside);
+#endif
+    }
+    __syncwarp();
+  }
+  return any;
+}
+
+// One clipping from the known-outside corner p (Alg. 3 lines 3-4): bisector search on the real edge p_s p or on the
+// virtual edge w p, then the clip.  Returns 0 ok, 1 capacity, 2 topology, 3 search cap.
+template <int P, int C, bool HV>
+__device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int i, int p, int s, int& np,
+                                            int& nc, QueryStats& st, LocalCnt& lc) {
+  const int lane = lane_id();
+  VD_POLY_REFS;
+  if (np >= P) return 1;
+  double psx = wx, psy = wy, psz = wz;
+  if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
+  double nx, ny, nz, d;
+  const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
+                                  nx, ny, nz, d, st, lc);
+  if (j < 0) return 3;
+  bool own = false;
+  for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == j);
+  if (__any_sync(kFull, own)) {   // B_ij already bounds P: p lies on it up to rounding
+    if (lane == 0) S.cstate[p] = ST_IN;
+    __syncwarp();
+    return 0;
+  }
+#ifdef VD_TRACE
+  if (lane == 0) printf("pair(?,%d) clip p=%d(%g,%g,%g) s=%d j=%d nc=%d np=%d\n", i, p, S.cx[p]+ox, S.cy[p]+oy, S.cz[p]+oz, s, j, nc, np);
+#endif
+  lc.clips += 1;
+  return apply_clip_3d(S, np, nc, p, s, nx, ny, nz, d, j);
+}
+
+// returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
+template <int P, int C, bool HV, bool BOX>
+__device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+  const Pair pr = load_pair(A, pairIdx);
+  const int a = pr.a, i = pr.i;
+  int np, nc;
+  init_poly_3d<P, C, BOX>(S, A, pr, np, nc);
+  bool failed = false;
+  {
+    const int rc = preclip_3d(S, A, i, np, nc, lc);
+    if (rc == 1) return 1;
+    if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
+  }
+  // ---- while P has a corner outside Omega_i (Alg. 3 line 2).  A corner known to be outside is clipped away
+  // first; only when none is left are the unclassified corners tested: a clip removes unclassified corners
+  // beyond its plane for free (they are candidates of R_p)
+  for (int guard = 0; guard < 8 * P + 32 && !failed; ++guard) {
+    int s;
+    const int p = select_out_3d(S, A, nc, s);
+    if (p < 0) {
+      if (!classify_unknown_3d<P, C, HV>(S, g, i, np, nc, st)) break;   // every corner is in Omega_i
       continue;
     }
-    if (np >= P) return 1;
-    // find a bisector B_ij on the real edge p_s p or on the virtual edge w p (Alg. 1 line 4 / Alg. 3 line 3)
-    double psx = wx, psy = wy, psz = wz;
-    if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
-    double nx, ny, nz, d;
-    const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
-                                nx, ny, nz, d, st, lc);
-    if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
-    {
-      bool own = false;
-      for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == j);
-      if (__any_sync(kFull, own)) {   // B_ij already bounds P: p lies on it up to rounding
-        if (lane == 0) S.cstate[p] = ST_IN;
-        __syncwarp();
-        continue;
-      }
-    }
-#ifdef VD_TRACE
-    if (lane == 0) printf("pair(%d,%d) clip p=%d(%g,%g,%g) s=%d j=%d nc=%d np=%d\n", a, i, p, S.cx[p]+ox, S.cy[p]+oy, S.cz[p]+oz, s, j, nc, np);
-#endif
-    lc.clips += 1;
-    const int rc = apply_clip_3d(S, np, nc, p, s, nx, ny, nz, d, j);
+    const int rc = clip_from_3d<P, C, HV>(S, g, A, i, p, s, np, nc, st, lc);
     if (rc == 1) return 1;
-    if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); break; }
+    if (rc) { failed = true; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); }
   }
-  return finish_piece_3d(S, A, pairIdx, a, i, np, nc, ox, oy, oz, failed, lc);
+  return finish_piece_3d(S, A, pairIdx, a, i, np, nc, S.u[0], S.u[1], S.u[2], failed, lc);
 }
 
 }  // namespace vd

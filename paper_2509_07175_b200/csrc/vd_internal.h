@@ -64,6 +64,8 @@ struct vd_ctx {
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
   vd::DevBuf nearList;    // int [n][nearClips]  sites nearest to every site, nearest first, -1 padded (reading U19)
   vd::DevBuf control;     // Control
+  vd::DevBuf phaseCells;  // phased mode: polytopes of one wave parked between the step kernels (vd_phase.cu)
+  vd::DevBuf phaseLists;  // phased mode: work lists + counters
   vd::DevBuf pairs;       // Pair [pairCap]
   vd::DevBuf pieces;      // Piece [pairCap]
   vd::DevBuf visited;     // u64 [hashCap]

@@ -1,0 +1,234 @@
+// vd_phase.cu -- S4 as a sequence of small kernels ("phased" mode, vd_options.persistent = 2) for the 3D kinds.
+//
+// The one-kernel clip path (vd_clip.cu) is bound by instruction fetch: ~100 KB of code whose 24 warps per SM sit
+// in different steps of Alg. 3, against a 32 KB L1.5 instruction cache.  Here every step of Alg. 3 is its own
+// kernel over all pairs of a wave, and the polytope of each pair is parked in HBM between the steps (5.2 KB per
+// pair; a round over 1 M pairs moves ~10 GB, ~1.5 ms of HBM time -- bandwidth is what a B200 has to spare):
+//
+//   k_ph_init    P <- T_a or the box (Alg. 3 line 1), then the clips by the nearest sites (reading U19)
+//   k_ph_verify  point-in-cell tests of all unclassified corners (section IV-A)          --+  rounds, until no
+//   k_ph_fix     per pair with a corner outside: bisector search + clip (Alg. 3 l. 3-4)  --+  corner is outside
+//   k_ph_finish  measure, moments, corners, flags, propagation
+//
+// Pairs pushed by k_ph_finish form the next wave (Alg. 4's L1/L2 swap).  Pairs that outgrow the fast tier
+// go to the large-capacity kernel of vd_clip.cu, as in the other modes.
+#include "vd_clip3d.cuh"
+
+namespace vd {
+
+constexpr int P3 = 32, C3 = 64;
+using PolyF = Poly3<P3, C3>;
+
+struct CellState {
+  PolyF S;
+  int np, nc;      // np < 0: the pair left the phased path (capacity: large tier)
+  int a, i;
+  int failed, pad;
+};
+static_assert(sizeof(CellState) % 8 == 0, "copied in 8-byte words");
+
+struct PhaseCtl {
+  unsigned ticket, nClip, nDone, pad;
+};
+
+__device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes) {
+  const unsigned long long* s = reinterpret_cast<const unsigned long long*>(src);
+  unsigned long long* d = reinterpret_cast<unsigned long long*>(dst);
+  for (int k = lane_id(); k < bytes / 8; k += kLanes) d[k] = s[k];
+}
+
+__device__ __forceinline__ int next_item(PhaseCtl* pc, int count) {
+  unsigned t = 0;
+  if (lane_id() == 0) t = atomicAdd(&pc->ticket, 1u);
+  t = shfl(t, 0);
+  return t < (unsigned)count ? (int)t : -1;
+}
+
+__device__ __forceinline__ void defer_pair(const ClipArgs& A, int64_t idx) {
+  if (lane_id() == 0) {
+    const unsigned long long slot = atomicAdd(&A.ctl->ovfTail, 1ull);
+    if ((int64_t)slot < A.ovfCap) A.ovf[slot] = (int)idx; else atomicOr(&A.ctl->err, ERR_PAIR_CAP);
+  }
+}
+
+template <bool BOX>
+__global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __restrict__ cells, int64_t begin, int count, PhaseCtl* pc) {
+  __shared__ PolyF S[kWarpsPerBlock];
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  QueryStats st = {0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u};
+  for (;;) {
+    const int t = next_item(pc, count);
+    if (t < 0) break;
+    const Pair pr = load_pair(A, begin + t);
+    int np, nc;
+    init_poly_3d<P3, C3, BOX>(S[w], A, pr, np, nc);
+    const int rc = preclip_3d(S[w], A, pr.i, np, nc, lc);
+    int failed = 0;
+    if (rc == 1) { defer_pair(A, begin + t); np = -1; }
+    if (rc == 2) { failed = 1; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
+    __syncwarp();
+    CellState* c = &cells[t];
+    if (np >= 0) copy_words(&c->S, &S[w], (int)sizeof(PolyF));
+    if (lane == 0) { c->np = np; c->nc = nc; c->a = pr.a; c->i = pr.i; c->failed = failed; }
+    __syncwarp();
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
+// list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
+template <bool HV>
+__global__ void __launch_bounds__(kBlock, 3) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+                                                     int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
+  __shared__ GridIndex g;
+  __shared__ PolyF S[kWarpsPerBlock];
+  if (threadIdx.x == 0) g = *A.grid;
+  __syncthreads();
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  QueryStats st = {0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u};
+  for (;;) {
+    const int t = next_item(pc, count);
+    if (t < 0) break;
+    const int slot = list ? list[t] : t;
+    if (slot < 0) continue;
+    CellState* c = &cells[slot];
+    const int np = c->np, nc = c->nc;
+    if (np < 0) continue;
+    bool out = false;
+    if (!c->failed && nc > 0) {
+      copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+      __syncwarp();
+      const bool any = classify_unknown_3d<P3, C3, HV>(S[w], g, c->i, np, nc, st);
+      for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
+      out = __any_sync(kFull, out);
+      if (any) {
+        copy_words(c->S.cnn, S[w].cnn, (int)sizeof(S[w].cnn));
+        copy_words(c->S.cstate, S[w].cstate, (int)sizeof(S[w].cstate));
+      }
+    }
+    if (lane == 0) {
+      if (out) clipList[atomicAdd(&pc->nClip, 1u)] = slot;
+      else doneList[atomicAdd(&pc->nDone, 1u)] = slot;
+    }
+    __syncwarp();
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
+// every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
+// round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
+template <bool HV>
+__global__ void __launch_bounds__(kBlock, 3) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
+                                                     int64_t begin, PhaseCtl* pc) {
+  __shared__ GridIndex g;
+  __shared__ PolyF S[kWarpsPerBlock];
+  if (threadIdx.x == 0) g = *A.grid;
+  __syncthreads();
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  QueryStats st = {0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u};
+  for (;;) {
+    const int t = next_item(pc, count);
+    if (t < 0) break;
+    const int slot = list[t];
+    CellState* c = &cells[slot];
+    int np = c->np, nc = c->nc;
+    const int i = c->i;
+    copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+    __syncwarp();
+    int failed = 0;
+    for (int guard = 0; guard < 4 * P3 && nc > 0; ++guard) {
+      int s;
+      const int p = select_out_3d(S[w], A, nc, s);
+      if (p < 0) break;
+      const int rc = clip_from_3d<P3, C3, HV>(S[w], g, A, i, p, s, np, nc, st, lc);
+      if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
+      if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
+    }
+    __syncwarp();
+    if (np >= 0) copy_words(&c->S, &S[w], (int)sizeof(PolyF));
+    if (lane == 0) {
+      c->np = np; c->nc = nc; c->failed = failed;
+      list[t] = np >= 0 ? slot : -1;
+    }
+    __syncwarp();
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
+__global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+                                                     int64_t begin, PhaseCtl* pc) {
+  __shared__ PolyF S[kWarpsPerBlock];
+  const int w = (int)threadIdx.x / kLanes;
+  QueryStats st = {0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u};
+  for (;;) {
+    const int t = next_item(pc, count);
+    if (t < 0) break;
+    const int slot = list[t];
+    const CellState* c = &cells[slot];
+    copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+    __syncwarp();
+    finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc);
+    __syncwarp();
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
+static vd_status reset_ctl(vd_ctx* c, PhaseCtl* pc, bool all) {
+  return cuda_check(c, cudaMemsetAsync(pc, 0, all ? sizeof(PhaseCtl) : sizeof(unsigned) * 2, c->stream), "phase ctl");
+}
+
+// One wave: pairs [begin, end) of the pair list, all of one 3D kind.
+vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end) {
+  const int64_t chunk = (int64_t)1 << 20;
+  const int64_t cap = end - begin < chunk ? end - begin : chunk;
+  vd_status s;
+  if ((s = ensure(c, c->phaseCells, sizeof(CellState) * (size_t)cap))) return s;
+  if ((s = ensure(c, c->phaseLists, sizeof(int) * 3 * (size_t)cap + sizeof(PhaseCtl)))) return s;
+  CellState* cells = c->phaseCells.as<CellState>();
+  int* listA = c->phaseLists.as<int>();
+  int* listB = listA + cap;
+  int* done = listB + cap;
+  PhaseCtl* pc = reinterpret_cast<PhaseCtl*>(done + cap);
+  cudaStream_t st = c->stream;
+  const int grid = 148 * 4;
+  for (int64_t b = begin; b < end; b += chunk) {
+    const int count = (int)((end - b) < chunk ? (end - b) : chunk);
+    if ((s = reset_ctl(c, pc, true))) return s;
+    if (c->kind == KIND_BOX_3D) VD_LAUNCH(k_ph_init<true>, grid, kBlock, 0, st)(A, cells, b, count, pc);
+    else VD_LAUNCH(k_ph_init<false>, grid, kBlock, 0, st)(A, cells, b, count, pc);
+    const int* cur = nullptr;
+    int curCount = count;
+    int* clip = listA;
+    int* other = listB;
+    for (int round = 0; round < 4 * P3; ++round) {
+      if ((s = reset_ctl(c, pc, false))) return s;   // ticket and nClip; nDone keeps growing
+      if (hv) VD_LAUNCH(k_ph_verify<true>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
+      else VD_LAUNCH(k_ph_verify<false>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
+      PhaseCtl h;
+      cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      if (e != cudaSuccess) return cuda_check(c, e, "phase round");
+      if (h.nClip == 0) break;
+      if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
+      if (hv) VD_LAUNCH(k_ph_fix<true>, 148 * 3, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
+      else VD_LAUNCH(k_ph_fix<false>, 148 * 3, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
+      cur = clip;
+      curCount = (int)h.nClip;
+      int* tmp = clip; clip = other; other = tmp;
+    }
+    PhaseCtl h;
+    cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
+    if (h.nDone > 0) {
+      if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
+      VD_LAUNCH(k_ph_finish, grid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, pc);
+    }
+  }
+  return cuda_check(c, cudaGetLastError(), "phases");
+}
+
+}  // namespace vd

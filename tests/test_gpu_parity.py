@@ -58,7 +58,7 @@ def test_replica_parity(idx):
 
 
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
-                                  dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12)])
+                                  dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -130,17 +130,20 @@ def test_results_are_reproducible():
     assert np.allclose(a.piece_measure, b.piece_measure, rtol=1e-11, atol=0)
 
 
-def test_wave_mode_and_device_queue_agree():
-    """persistent=0 (one launch per wavefront) and persistent=1 (device-side queue) produce the
-    same cells; the clustered replica exercises the refined (two-level) site index in both."""
+def test_schedules_agree():
+    """persistent=0 (one launch per wavefront), 3 (device-side queue) and the default (3D kinds: one
+    kernel per step of Alg. 3) produce the same cells; the clustered replica exercises the refined (two-level)
+    site index in all of them."""
     for idx in (3, 4):
         w = inputs.config(idx, "small")
         a, ca, _ = _gpu(w, persistent=0)
-        b, cb, _ = _gpu(w, persistent=1)
-        assert ca["waves"] > 1 and cb["waves"] >= 1
-        for f in ("nbr_off", "nbr", "piece_off", "piece_simplex", "vert_off", "vert_flags"):
-            assert np.array_equal(getattr(a, f), getattr(b, f)), f
-        assert np.allclose(a.measure, b.measure, rtol=1e-12, atol=0)
+        assert ca["waves"] > 1
+        for mode in (1, 3):
+            b, cb, _ = _gpu(w, persistent=mode)
+            assert cb["waves"] >= 1
+            for f in ("nbr_off", "nbr", "piece_off", "piece_simplex", "vert_off", "vert_flags"):
+                assert np.array_equal(getattr(a, f), getattr(b, f)), f
+            assert np.allclose(a.measure, b.measure, rtol=1e-12, atol=0)
 
 
 def test_refined_index_on_heavily_clustered_sites():
@@ -264,6 +267,7 @@ def test_box_domain_edge_cases():
 def test_box_domain_wave_mode_and_lloyd():
     w = inputs.box(3, 3000, seed=5)
     _box_parity(w, persistent=0)
+    _box_parity(w, persistent=3)
     _box_parity(w, near_clips=-1)              # the paper's loop alone, from the whole box
     _box_parity(w, near_clips=32, ball_cells=-1)
     with binding.Context(w.sites) as ctx:
