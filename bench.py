@@ -76,12 +76,18 @@ class ClockSampler:
 
 def algorithmic_flops(cnt, kind):
     """8 flop per candidate distance (5 in 2D), 15 per search iteration,
-    per clip 2d flop x ~corners tested + 60 per new 3D corner (15 in 2D), 30 per fan tet of a piece."""
-    d3 = kind == 2
-    per_dist = 8 if kind != 0 else 5
+    per clip 2d flop x ~corners tested + 60 per new 3D corner (15 in 2D), 30 per fan tet of a piece.
+    Returned per step kernel of S4 (phased schedule) and in total."""
+    d3 = kind in (2, 4)
+    per_dist = 8 if kind not in (0, 3) else 5
     per_clip = (6 * 12 + 60 * 4) if d3 else (4 * 6 + 15 * 2)
     per_piece = 30 * (20 if d3 else 4)
-    return per_dist * cnt["dist_evals"] + 15 * cnt["search_iters"] + per_clip * cnt["clips"] + per_piece * cnt["pieces"]
+    pre, se = cnt.get("pre_clips", 0), cnt.get("search_evals", 0)
+    parts = {"init": per_clip * pre,
+             "verify": per_dist * (cnt["dist_evals"] - se),
+             "fix": per_dist * se + 15 * cnt["search_iters"] + per_clip * (cnt["clips"] - pre),
+             "finish": per_piece * cnt["pieces"]}
+    return parts, sum(parts.values())
 
 
 def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
@@ -105,7 +111,7 @@ def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
             "sample": f"{k} seeded-random sites of the workload, tier {tier}, {dt:.1f} s wall"}
 
 
-def run_reference(args, w):
+def run_reference(args, w, workload):
     """--impl reference: each step = the oracle on a bounded sample of sites."""
     from oracle import oracle
     rank = int(os.environ.get("RANK", "0"))
@@ -133,7 +139,7 @@ def run_reference(args, w):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "sample": sample},
+        "config": {"workload": workload, "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": int(probe.threads_used), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
@@ -144,14 +150,17 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index, 1-based (default 2 = configs[1])")
+    ap.add_argument("--box", type=int, default=0, help="instead of a BASELINE config: N white-noise sites in the unit cube, the cube itself "
+                    "as a simple domain (VD_BOX_3D; the setting of the paper's Fig. 1 / Table VI)")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
     from paper_2509_07175_b200 import inputs
-    w = inputs.config(args.config)
+    w = inputs.box(3, args.box, seed=9) if args.box else inputs.config(args.config)
+    workload = f"whole cells of {args.box} uniform sites in the unit cube (VD_BOX_3D, paper Fig. 1 setting)" if args.box else WORKLOADS[args.config]
     if args.impl == "reference":
-        run_reference(args, w)
+        run_reference(args, w, workload)
         return
 
     import torch
@@ -170,7 +179,7 @@ def main():
     # inputs resident in HBM before the timed region
     d_sites = torch.from_numpy(w.sites).to(dev)
     d_verts = torch.from_numpy(w.verts).to(dev)
-    d_simp = torch.from_numpy(w.simplices).to(dev)
+    d_simp = torch.from_numpy(w.simplices).to(dev) if w.simplices is not None else None
     ctx = binding.Context(d_sites)
     ctx.set_stream(stream.cuda_stream)
     ctx.set_domain(d_verts, d_simp, w.kind)
@@ -188,12 +197,15 @@ def main():
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     clip_ms, launches = 0.0, 0
+    phase_ms = {"init": 0.0, "verify": 0.0, "fix": 0.0, "finish": 0.0}
     for k in range(args.steps):
         flush.fill_(k & 0xff)            # L2 flush between timed iterations (not timed)
         ev[k][0].record(stream)
         ctx.compute()
         ev[k][1].record(stream)
         clip_ms += ctx.stage_ms()["clip"]
+        for name, v in ctx.phase_ms().items():
+            phase_ms[name] += v
         launches += ctx.counters()["launches"]
     barrier()
     clocks = sampler.stop()
@@ -219,30 +231,38 @@ def main():
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
                                             "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
-    h2d = w.sites.nbytes + w.verts.nbytes + w.simplices.nbytes
+    h2d = w.sites.nbytes + w.verts.nbytes + (w.simplices.nbytes if w.simplices is not None else 0)
     e2e_val, _ = ranks.whole_job_rate(float(w.n), e2e_s * 1e3, dev)
 
-    flops = algorithmic_flops(cnt, w.kind)
-    clip_s = clip_ms / args.steps * 1e-3
+    parts, flops = algorithmic_flops(cnt, w.kind)
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    achieved = flops / clip_s / 1e12
+    if sum(phase_ms.values()) > 0:
+        # phased schedule: the dominant kernel is the step kernel with the largest device time (CUDA events
+        # around every launch, inside the library, on the stream the kernels run on)
+        top = max(phase_ms, key=phase_ms.get)
+        kernel, kernel_ms, kernel_flops = "k_ph_" + top, phase_ms[top] / args.steps, parts[top]
+    else:
+        kernel, kernel_ms, kernel_flops = "k_clip (S4+S5, one-kernel schedule)", clip_ms / args.steps, flops
+    achieved = kernel_flops / (kernel_ms * 1e-3) / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
+        "config": {"workload": workload, "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "nonempty_cells": int(cells.n_nonempty), "pieces": int(cells.n_pieces), "corners": int(cells.n_verts)},
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": int(launches),
         "stage_ms": stage, "counters": cnt,
-        "roofline": {"bound": "alu", "kernel": "k_clip (S4+S5)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
+        "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
-                     "algorithmic_flop_per_step": flops, "kernel_ms_per_step": clip_ms / args.steps,
-                     "share_of_step": clip_ms / ms},
+                     "algorithmic_flop_per_step": kernel_flops, "kernel_ms_per_step": kernel_ms,
+                     "share_of_step": kernel_ms * args.steps / ms,
+                     "s4_ms_per_step": clip_ms / args.steps, "s4_algorithmic_flop_per_step": flops},
     }
     ctx.destroy()
     if rank == 0:

@@ -118,7 +118,9 @@ typedef struct vd_counters {
   int64_t reruns;         /* times the whole compute was repeated after growing a pool            */
   int64_t launches;       /* kernels this library launched inside the last vd_compute               */
   int64_t row_evals;      /* grid rows examined by those queries (index efficiency)                    */
-  int64_t reserved[5];
+  int64_t search_evals;   /* the part of dist_evals spent inside bisector searches                     */
+  int64_t pre_clips;      /* the part of clips done by nearest-site bisectors (vd_options.near_clips)  */
+  int64_t reserved[3];
 } vd_counters;
 
 /* vd_create: copy n sites of dimension dim (row-major [n][dim], fp64).  Builds nothing heavy: the
@@ -167,6 +169,11 @@ vd_status vd_get_counters(const vd_ctx* ctx, vd_counters* out);
 /* Per-stage device times (ms, CUDA events) of the last vd_compute:
  * [0] site index (S1)  [1] seeds (S3)  [2] clip + propagate (S4+S5)  [3] assemble (S6)  [4] total. */
 vd_status vd_get_stage_ms(const vd_ctx* ctx, double out_ms[5]);
+
+/* Phased schedule (vd_options.persistent): device time (ms, CUDA events, summed over all launches) of the step
+ * kernels of S4 in the last vd_compute: [0] k_ph_init  [1] k_ph_verify  [2] k_ph_fix  [3] k_ph_finish;
+ * all 0 when another schedule ran. */
+vd_status vd_get_phase_ms(const vd_ctx* ctx, double out_ms[4]);
 
 /* Copy the last result into caller HOST buffers (any may be NULL to skip).  Sizes are those of
  * vd_cells.  Synchronises the context's stream. */

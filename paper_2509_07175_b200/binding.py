@@ -18,7 +18,7 @@ VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D, VD_BOX_2D, VD_BOX_3D = 0, 1, 2, 3, 4
 STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_INPUT", 5: "VD_E_CUDA",
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
 EXPORTS = ["vd_create", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
-           "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_cells_to_host",
+           "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_get_phase_ms", "vd_cells_to_host",
            "vd_nearest", "vd_get_adjacency", "vd_last_error", "vd_version"]
 
 _LIB_PATH = _build.lib_path()
@@ -49,7 +49,7 @@ class vd_options(ctypes.Structure):
 
 class vd_counters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips",
-                                               "waves", "overflow_pairs", "reruns", "launches", "row_evals")] + [("reserved", ctypes.c_int64 * 5)]
+                                               "waves", "overflow_pairs", "reruns", "launches", "row_evals", "search_evals", "pre_clips")] + [("reserved", ctypes.c_int64 * 3)]
 
 
 def load():
@@ -73,6 +73,7 @@ def load():
     lib.vd_set_options.argtypes = [vp, ctypes.POINTER(vd_options)]
     lib.vd_get_counters.argtypes = [vp, ctypes.POINTER(vd_counters)]
     lib.vd_get_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    lib.vd_get_phase_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     lib.vd_cells_to_host.argtypes = [vp] + [vp] * 10
     lib.vd_nearest.argtypes = [vp, vp, i64, vp]
     lib.vd_get_adjacency.argtypes = [vp, vp]
@@ -198,6 +199,11 @@ class Context:
         a = (ctypes.c_double * 5)()
         self._check(self._lib.vd_get_stage_ms(self._h, a))
         return dict(zip(("index", "seed", "clip", "assemble", "total"), [float(x) for x in a]))
+
+    def phase_ms(self):
+        a = (ctypes.c_double * 4)()
+        self._check(self._lib.vd_get_phase_ms(self._h, a))
+        return dict(zip(("init", "verify", "fix", "finish"), [float(x) for x in a]))
 
     def to_host(self, full=True) -> HostCells:
         r = self.cells

@@ -232,6 +232,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     }
   }
   memset(&c->counters, 0, sizeof(c->counters));
+  for (double& v : c->phaseMs) v = 0.0;
   const unsigned long long launches0 = g_launches;
   cudaStream_t st = c->stream;
   vd_status s;
@@ -280,6 +281,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   c->counters.queries = (int64_t)h.cnt.queries; c->counters.dist_evals = (int64_t)h.cnt.dist_evals;
   c->counters.row_evals = (int64_t)h.cnt.rows;
   c->counters.search_iters = (int64_t)h.cnt.search_iters; c->counters.clips = (int64_t)h.cnt.clips;
+  c->counters.search_evals = (int64_t)h.cnt.search_evals; c->counters.pre_clips = (int64_t)h.cnt.pre_clips;
   c->counters.overflow_pairs = (int64_t)h.ovfTail;
   c->counters.reruns = reruns; c->counters.waves = waves;
   c->counters.launches = (int64_t)(g_launches - launches0);
@@ -331,6 +333,8 @@ void vd_destroy(vd_ctx* c) {
   for (DevBuf* b : all) release(c, *b);
   for (int k = 0; k < 6; ++k)
     if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+  for (int k = 0; k < 4; ++k)
+    if (c->phaseEv[k]) cudaEventDestroy(c->phaseEv[k]);
   delete c;
 }
 
@@ -362,6 +366,12 @@ vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
 vd_status vd_get_counters(const vd_ctx* c, vd_counters* out) {
   if (!c || !out) return VD_E_ARG;
   *out = c->counters;
+  return VD_OK;
+}
+
+vd_status vd_get_phase_ms(const vd_ctx* c, double out_ms[4]) {
+  if (!c || !out_ms) return VD_E_ARG;
+  for (int k = 0; k < 4; ++k) out_ms[k] = c->phaseMs[k];
   return VD_OK;
 }
 

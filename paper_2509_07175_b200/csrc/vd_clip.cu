@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
-  LocalCnt lc = {0u, 0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   constexpr bool BOX = KIND == KIND_BOX_2D || KIND == KIND_BOX_3D;
   if constexpr (KIND == KIND_TET_3D || KIND == KIND_BOX_3D) {
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];

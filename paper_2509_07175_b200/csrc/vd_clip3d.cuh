@@ -8,7 +8,7 @@
 namespace vd {
 
 template <int P, int C>
-struct Poly3 {
+struct alignas(16) Poly3 {
   double u[12];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local)
   double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   int pflag[P];                           // flag of plane f
@@ -445,6 +445,7 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
       if (p == 0x7fffffff) continue;   // the plane does not cut P
       if (np >= P) return 1;
       lc.clips += 1;
+      lc.pre_clips += 1;
       const int rc = apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
       if (rc) return rc;
       if (nc == 0) break;

@@ -32,7 +32,7 @@ struct ClipArgs {
 enum { ST_UNKNOWN = 0, ST_IN = 1, ST_OUT = 2 };
 
 struct LocalCnt {
-  unsigned pairs, pieces, search_iters, clips;
+  unsigned pairs, pieces, search_iters, clips, search_evals, pre_clips;
 };
 
 __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& st, const LocalCnt& lc) {
@@ -41,6 +41,8 @@ __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& s
     atomicAdd(&ctl->cnt.pieces, (unsigned long long)lc.pieces);
     atomicAdd(&ctl->cnt.search_iters, (unsigned long long)lc.search_iters);
     atomicAdd(&ctl->cnt.clips, (unsigned long long)lc.clips);
+    if (lc.search_evals) atomicAdd(&ctl->cnt.search_evals, (unsigned long long)lc.search_evals);
+    if (lc.pre_clips) atomicAdd(&ctl->cnt.pre_clips, (unsigned long long)lc.pre_clips);
     atomicAdd(&ctl->cnt.queries, (unsigned long long)st.queries);
     atomicAdd(&ctl->cnt.dist_evals, (unsigned long long)st.dist_evals);
     atomicAdd(&ctl->cnt.rows, (unsigned long long)st.rows);
@@ -255,7 +257,7 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double q
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
 template <bool HV>
-static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j,
+static __device__ __noinline__ int find_bisector_impl(const ClipArgs& A, const GridIndex& g, int i, int j,
                                              const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
                                              double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
                                              double& nx, double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
@@ -312,6 +314,16 @@ static __device__ __noinline__ int find_bisector(const ClipArgs& A, const GridIn
     ptx = qx; pty = qy; ptz = qz;
   }
   return -1;
+}
+
+template <bool HV>
+__device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
+                                             double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
+                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
+  const unsigned e0 = st.dist_evals;
+  const int r = find_bisector_impl<HV>(A, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, nx, ny, nz, d, st, lc);
+  lc.search_evals += st.dist_evals - e0;
+  return r;
 }
 
 }  // namespace vd

@@ -71,6 +71,7 @@ struct Piece {
 
 struct Counters {
   unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs, rows;
+  unsigned long long search_evals, pre_clips;   // distance evaluations inside bisector searches; clips by nearest-site bisectors (U19)
 };
 
 __device__ __forceinline__ int lane_id() { return (int)(threadIdx.x % kLanes); }

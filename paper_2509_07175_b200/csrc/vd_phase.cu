@@ -23,18 +23,25 @@ struct CellState {
   PolyF S;
   int np, nc;      // np < 0: the pair left the phased path (capacity: large tier)
   int a, i;
-  int failed, pad;
+  int failed, pad[3];
 };
-static_assert(sizeof(CellState) % 8 == 0, "copied in 8-byte words");
+static_assert(sizeof(CellState) % 16 == 0 && sizeof(PolyF) % 16 == 0, "copied in 16-byte words");
 
 struct PhaseCtl {
   unsigned ticket, nClip, nDone, pad;
 };
 
+// warp copy in 16-byte words, four loads in flight per lane
 __device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes) {
-  const unsigned long long* s = reinterpret_cast<const unsigned long long*>(src);
-  unsigned long long* d = reinterpret_cast<unsigned long long*>(dst);
-  for (int k = lane_id(); k < bytes / 8; k += kLanes) d[k] = s[k];
+  const uint4* s = reinterpret_cast<const uint4*>(src);
+  uint4* d = reinterpret_cast<uint4*>(dst);
+  const int n = bytes / 16, lane = lane_id();
+  int k = lane;
+  for (; k + 3 * kLanes < n; k += 4 * kLanes) {
+    const uint4 a = s[k], b = s[k + kLanes], c = s[k + 2 * kLanes], e = s[k + 3 * kLanes];
+    d[k] = a; d[k + kLanes] = b; d[k + 2 * kLanes] = c; d[k + 3 * kLanes] = e;
+  }
+  for (; k < n; k += kLanes) d[k] = s[k];
 }
 
 __device__ __forceinline__ int next_item(PhaseCtl* pc, int count) {
@@ -56,7 +63,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
-  LocalCnt lc = {0u, 0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -78,7 +85,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 
 // list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 3) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, 4) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
                                                      int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
@@ -86,7 +93,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_verify(ClipArgs A, CellState* 
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
-  LocalCnt lc = {0u, 0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -119,7 +126,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_verify(ClipArgs A, CellState* 
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 3) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, 4) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
                                                      int64_t begin, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
@@ -127,7 +134,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_fix(ClipArgs A, CellState* __r
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
-  LocalCnt lc = {0u, 0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -162,7 +169,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
-  LocalCnt lc = {0u, 0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -180,52 +187,75 @@ static vd_status reset_ctl(vd_ctx* c, PhaseCtl* pc, bool all) {
   return cuda_check(c, cudaMemsetAsync(pc, 0, all ? sizeof(PhaseCtl) : sizeof(unsigned) * 2, c->stream), "phase ctl");
 }
 
-// One wave: pairs [begin, end) of the pair list, all of one 3D kind.
+// One wave: pairs [begin, end) of the pair list, all of one 3D kind.  Every launch is bracketed by two events;
+// the elapsed times are read after the round's synchronisation (vd_get_phase_ms).
 vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end) {
   const int64_t chunk = (int64_t)1 << 20;
   const int64_t cap = end - begin < chunk ? end - begin : chunk;
   vd_status s;
   if ((s = ensure(c, c->phaseCells, sizeof(CellState) * (size_t)cap))) return s;
   if ((s = ensure(c, c->phaseLists, sizeof(int) * 3 * (size_t)cap + sizeof(PhaseCtl)))) return s;
+  for (cudaEvent_t& e : c->phaseEv)
+    if (!e && cudaEventCreate(&e) != cudaSuccess) return cuda_check(c, cudaGetLastError(), "phase events");
   CellState* cells = c->phaseCells.as<CellState>();
   int* listA = c->phaseLists.as<int>();
   int* listB = listA + cap;
   int* done = listB + cap;
   PhaseCtl* pc = reinterpret_cast<PhaseCtl*>(done + cap);
   cudaStream_t st = c->stream;
+  cudaEvent_t* ev = c->phaseEv;
   const int grid = 148 * 4;
+  auto elapsed = [&](int which, cudaEvent_t a, cudaEvent_t b) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) c->phaseMs[which] += ms;
+  };
+  auto read_ctl = [&](PhaseCtl& h) -> cudaError_t {
+    cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e;
+  };
   for (int64_t b = begin; b < end; b += chunk) {
     const int count = (int)((end - b) < chunk ? (end - b) : chunk);
     if ((s = reset_ctl(c, pc, true))) return s;
+    cudaEventRecord(ev[0], st);
     if (c->kind == KIND_BOX_3D) VD_LAUNCH(k_ph_init<true>, grid, kBlock, 0, st)(A, cells, b, count, pc);
     else VD_LAUNCH(k_ph_init<false>, grid, kBlock, 0, st)(A, cells, b, count, pc);
+    cudaEventRecord(ev[1], st);
     const int* cur = nullptr;
     int curCount = count;
     int* clip = listA;
     int* other = listB;
+    bool initTimed = false, fixPending = false;
+    PhaseCtl h;
     for (int round = 0; round < 4 * P3; ++round) {
       if ((s = reset_ctl(c, pc, false))) return s;   // ticket and nClip; nDone keeps growing
+      cudaEventRecord(ev[2], st);
       if (hv) VD_LAUNCH(k_ph_verify<true>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
       else VD_LAUNCH(k_ph_verify<false>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
-      PhaseCtl h;
-      cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
-      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      cudaEventRecord(ev[3], st);
+      const cudaError_t e = read_ctl(h);
       if (e != cudaSuccess) return cuda_check(c, e, "phase round");
+      if (!initTimed) { elapsed(0, ev[0], ev[1]); initTimed = true; }
+      if (fixPending) { elapsed(2, ev[1], ev[2]); fixPending = false; }   // previous fix: between its start mark and this verify
+      elapsed(1, ev[2], ev[3]);
       if (h.nClip == 0) break;
       if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
-      if (hv) VD_LAUNCH(k_ph_fix<true>, 148 * 3, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
-      else VD_LAUNCH(k_ph_fix<false>, 148 * 3, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
+      cudaEventRecord(ev[1], st);
+      if (hv) VD_LAUNCH(k_ph_fix<true>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
+      else VD_LAUNCH(k_ph_fix<false>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
+      fixPending = true;
       cur = clip;
       curCount = (int)h.nClip;
       int* tmp = clip; clip = other; other = tmp;
     }
-    PhaseCtl h;
-    cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
     if (h.nDone > 0) {
       if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
+      cudaEventRecord(ev[0], st);
       VD_LAUNCH(k_ph_finish, grid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, pc);
+      cudaEventRecord(ev[1], st);
+      const cudaError_t e = cudaStreamSynchronize(st);
+      if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
+      elapsed(3, ev[0], ev[1]);
     }
   }
   return cuda_check(c, cudaGetLastError(), "phases");
