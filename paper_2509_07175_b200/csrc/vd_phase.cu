@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 
 // list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 4) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
                                                      int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
@@ -110,8 +110,8 @@ __global__ void __launch_bounds__(kBlock, 4) k_ph_verify(ClipArgs A, CellState* 
       for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
       out = __any_sync(kFull, out);
       if (any) {
-        copy_words(c->S.cnn, S[w].cnn, (int)sizeof(S[w].cnn));
-        copy_words(c->S.cstate, S[w].cstate, (int)sizeof(S[w].cstate));
+        copy_words(c->S.cnn, S[w].cnn, (nc * 4 + 15) & ~15);
+        copy_words(c->S.cstate, S[w].cstate, (nc + 15) & ~15);
       }
     }
     if (lane == 0) {
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_ph_verify(ClipArgs A, CellState* 
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 4) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
                                                      int64_t begin, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
