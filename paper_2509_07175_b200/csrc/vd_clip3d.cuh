@@ -7,20 +7,24 @@
 
 namespace vd {
 
+// Member order matters to the phased schedule (vd_phase.cu), which parks polytopes in HBM between kernels: first
+// what the point-in-cell tests read, then the rest of the polytope, scratch last (never copied).  Every array
+// starts on a 16-byte boundary.
 template <int P, int C>
 struct alignas(16) Poly3 {
   double u[12];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local)
-  double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   int pflag[P];                           // flag of plane f
   double cx[C], cy[C], cz[C];             // corner coordinates (local)
-  int cnn[C];                             // nearest site of an outside corner
-  int key[C][3];                          // scratch: flag triple of a corner (output order); rim points during a clip (P*3 doubles)
+  unsigned char cstate[C];
+  int cnn[C];                             // nearest site of an outside corner            <- end of what the tests touch
+  double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   unsigned short cp[C][3];                // the corner's three planes, cyclically ordered
   unsigned short cadj[C][3];              // corner across the polytope edge (cp[t], cp[t+1])
-  unsigned short remap[C];                // scratch: index of a surviving corner after the clip
-  unsigned short pa[P], pb[P];            // scratch: new corner whose rim edge starts / ends at a plane
+  int key[C][3];                          // scratch from here on: flag triple of a corner (output order); rim points during a clip
+  unsigned short remap[C];                // index of a surviving corner after the clip
+  unsigned short pa[P], pb[P];            // new corner whose rim edge starts / ends at a plane
   unsigned short be[P][4];                // rim edges of R_p: (a, b, inside neighbour, flags)
-  unsigned char cstate[C], cmark[C];
+  unsigned char cmark[C];
 };
 
 // returns false when the three planes are (numerically) parallel to a common line
@@ -183,6 +187,36 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
   nc = nSurv + L;
   np = N + 1;
   return __any_sync(kFull, bad) ? 2 : 0;
+}
+
+// Drop the planes that no corner lies on any more (box faces and early bisectors cut away by later ones): P's
+// plane list is a capacity (P planes in the fast tier) and the flag rules loop over it.
+template <int P, int C>
+__device__ void compact_planes_3d(Poly3<P, C>& S, int& np, int nc) {
+  const int lane = lane_id();
+  for (int f = lane; f < np; f += kLanes) S.pa[f] = 0;
+  __syncwarp();
+  for (int c = lane; c < nc; c += kLanes) { S.pa[S.cp[c][0]] = 1; S.pa[S.cp[c][1]] = 1; S.pa[S.cp[c][2]] = 1; }
+  __syncwarp();
+  int run = 0;
+  for (int f0 = 0; f0 < np; f0 += kLanes) {
+    const int f = f0 + lane;
+    const bool live = f < np && S.pa[f] != 0;
+    const unsigned m = __ballot_sync(kFull, live);
+    const int t = run + __popc(m & ((1u << lane) - 1u));
+    double a = 0, b = 0, c = 0, d = 0;
+    int fl = 0;
+    if (live) { a = S.pnx[f]; b = S.pny[f]; c = S.pnz[f]; d = S.pd[f]; fl = S.pflag[f]; }
+    __syncwarp();   // targets t <= f lie in this chunk or in earlier ones, already read
+    if (live) { S.pnx[t] = a; S.pny[t] = b; S.pnz[t] = c; S.pd[t] = d; S.pflag[t] = fl; S.pb[f] = (unsigned short)t; }
+    run += __popc(m);
+    __syncwarp();
+  }
+  for (int c = lane; c < nc; c += kLanes) {
+    S.cp[c][0] = S.pb[S.cp[c][0]]; S.cp[c][1] = S.pb[S.cp[c][1]]; S.cp[c][2] = S.pb[S.cp[c][2]];
+  }
+  __syncwarp();
+  np = run;
 }
 
 // Record the finished piece: measure and first moment (fan tetrahedra over every face, S6 input),
@@ -443,7 +477,10 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
       }
       warp_argmin(far, p);
       if (p == 0x7fffffff) continue;   // the plane does not cut P
-      if (np >= P) return 1;
+      if (np >= P) {
+        compact_planes_3d(S, np, nc);
+        if (np >= P) return 1;
+      }
       lc.clips += 1;
       lc.pre_clips += 1;
       const int rc = apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
@@ -538,7 +575,10 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
                                             int& nc, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
   VD_POLY_REFS;
-  if (np >= P) return 1;
+  if (np >= P) {
+    compact_planes_3d(S, np, nc);
+    if (np >= P) return 1;
+  }
   double psx = wx, psy = wy, psz = wz;
   if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
   double nx, ny, nz, d;

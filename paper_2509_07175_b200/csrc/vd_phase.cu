@@ -27,6 +27,10 @@ struct CellState {
 };
 static_assert(sizeof(CellState) % 16 == 0 && sizeof(PolyF) % 16 == 0, "copied in 16-byte words");
 
+constexpr int kTestBytes = (int)offsetof(PolyF, pnx);    // what k_ph_verify reads (and, for cstate and cnn, writes back)
+constexpr int kPolyBytes = (int)offsetof(PolyF, key);    // the polytope without its scratch arrays
+static_assert(kTestBytes % 16 == 0 && kPolyBytes % 16 == 0, "copied in 16-byte words");
+
 struct PhaseCtl {
   unsigned ticket, nClip, nDone, pad;
 };
@@ -76,7 +80,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
     if (rc == 2) { failed = 1; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
     __syncwarp();
     CellState* c = &cells[t];
-    if (np >= 0) copy_words(&c->S, &S[w], (int)sizeof(PolyF));
+    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
     if (lane == 0) { c->np = np; c->nc = nc; c->a = pr.a; c->i = pr.i; c->failed = failed; }
     __syncwarp();
   }
@@ -104,7 +108,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_verify(ClipArgs A, Ce
     if (np < 0) continue;
     bool out = false;
     if (!c->failed && nc > 0) {
-      copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+      copy_words(&S[w], &c->S, kTestBytes);
       __syncwarp();
       const bool any = classify_unknown_3d<P3, C3, HV>(S[w], g, c->i, np, nc, st);
       for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_fix(ClipArgs A, CellS
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
     const int i = c->i;
-    copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+    copy_words(&S[w], &c->S, kPolyBytes);
     __syncwarp();
     int failed = 0;
     for (int guard = 0; guard < 4 * P3 && nc > 0; ++guard) {
@@ -154,7 +158,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_fix(ClipArgs A, CellS
       if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
     }
     __syncwarp();
-    if (np >= 0) copy_words(&c->S, &S[w], (int)sizeof(PolyF));
+    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
     if (lane == 0) {
       c->np = np; c->nc = nc; c->failed = failed;
       list[t] = np >= 0 ? slot : -1;
@@ -175,7 +179,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
     if (t < 0) break;
     const int slot = list[t];
     const CellState* c = &cells[slot];
-    copy_words(&S[w], &c->S, (int)sizeof(PolyF));
+    copy_words(&S[w], &c->S, kPolyBytes);
     __syncwarp();
     finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc);
     __syncwarp();
