@@ -192,7 +192,7 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
 // Drop the planes that no corner lies on any more (box faces and early bisectors cut away by later ones): P's
 // plane list is a capacity (P planes in the fast tier) and the flag rules loop over it.
 template <int P, int C>
-__device__ void compact_planes_3d(Poly3<P, C>& S, int& np, int nc) {
+static __device__ __noinline__ void compact_planes_3d(Poly3<P, C>& S, int& np, int nc) {
   const int lane = lane_id();
   for (int f = lane; f < np; f += kLanes) S.pa[f] = 0;
   __syncwarp();
