@@ -129,6 +129,7 @@ static ClipArgs make_args(vd_ctx* c) {
   A.adj = c->adj.as<int>();
   A.vnn = c->vnn.as<int>();
   A.nearList = nullptr;
+  A.queue = 0;
   A.n = (int)c->n; A.m = (int)c->m; A.kind = c->kind;
   A.realEdges = c->opt.real_edges;
   A.ballCells = c->opt.ball_cells == 0 ? 64 : c->opt.ball_cells;
@@ -225,11 +226,12 @@ static void set_cursor(vd_ctx* c, int which, unsigned long long v) {
 }
 
 vd_status stage_clip(vd_ctx* c) {
-  const ClipArgs A = make_args(c);
+  ClipArgs A = make_args(c);
   const int mode = c->opt.persistent;
   const bool solid = c->kind == KIND_TET_3D || c->kind == KIND_BOX_3D;
   const bool phased = solid && (mode == 1 || mode == 2);   // 3D kinds: one small kernel per step (vd_phase.cu)
   const bool persist = mode != 0 && !phased;               // otherwise the device-side queue, or one launch per wave
+  A.queue = persist ? 1 : 0;
   int64_t begin = 0, obegin = 0, waves = 0;
   Control h;
   cudaError_t e = read_control(c, h);   // seeds pushed so far, refined cells of the index

@@ -10,6 +10,12 @@ namespace vd {
 // Member order matters to the phased schedule (vd_phase.cu), which parks polytopes in HBM between kernels: first
 // what the point-in-cell tests read, then the rest of the polytope, scratch last (never copied).  Every array
 // starts on a 16-byte boundary.
+// A warp's private chunks of the corner pool and the face-flag pool (phased finish kernel).
+struct WarpPool {
+  unsigned long long vbase, nbase;
+  int vleft, nleft, vchunk, nchunk;
+};
+
 template <int P, int C>
 struct alignas(16) Poly3 {
   double u[12];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local)
@@ -223,7 +229,7 @@ static __device__ __noinline__ void compact_planes_3d(Poly3<P, C>& S, int& np, i
 // corners with their flag triples in canonical order, face flags, and the propagation of P:L266-273.
 template <int P, int C>
 __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairIdx, int a, int i, int np, int nc, double ox,
-                               double oy, double oz, bool failed, LocalCnt& lc) {
+                               double oy, double oz, bool failed, LocalCnt& lc, WarpPool* wp = nullptr) {
   const int lane = lane_id();
   Piece pc;
   pc.site = i; pc.simplex = a; pc.nverts = 0; pc.nnbr = 0; pc.vbase = 0; pc.nbase = 0;
@@ -299,12 +305,28 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   }
   if (nnbr > C) nnbr = C;
   // face flags -> pool
-  unsigned long long nb0 = 0;
-  if (lane == 0) nb0 = atomicAdd(&A.ctl->nbrTail, (unsigned long long)nnbr);
-  nb0 = shfl(nb0, 0);
-  unsigned long long vb0 = 0;
-  if (lane == 0) vb0 = atomicAdd(&A.ctl->vertTail, (unsigned long long)nc);
-  vb0 = shfl(vb0, 0);
+  unsigned long long nb0 = 0, vb0 = 0;
+  if (wp) {
+    // the two pool cursors are single addresses that every piece of the step would hit: a warp takes a chunk
+    // at a time and hands out of it (the pools get holes; S6 gathers by (base, count) per piece)
+    if (wp->nleft < nnbr) {
+      const int take = max(wp->nchunk, nnbr);
+      if (lane == 0) nb0 = atomicAdd(&A.ctl->nbrTail, (unsigned long long)take);
+      wp->nbase = shfl(nb0, 0); wp->nleft = take;
+    }
+    if (wp->vleft < nc) {
+      const int take = max(wp->vchunk, nc);
+      if (lane == 0) vb0 = atomicAdd(&A.ctl->vertTail, (unsigned long long)take);
+      wp->vbase = shfl(vb0, 0); wp->vleft = take;
+    }
+    nb0 = wp->nbase; wp->nbase += nnbr; wp->nleft -= nnbr;
+    vb0 = wp->vbase; wp->vbase += nc; wp->vleft -= nc;
+  } else {
+    if (lane == 0) nb0 = atomicAdd(&A.ctl->nbrTail, (unsigned long long)nnbr);
+    nb0 = shfl(nb0, 0);
+    if (lane == 0) vb0 = atomicAdd(&A.ctl->vertTail, (unsigned long long)nc);
+    vb0 = shfl(vb0, 0);
+  }
   if ((int64_t)(nb0 + nnbr) > A.nbrCap || (int64_t)(vb0 + nc) > A.vertCap) {
     if (lane == 0) {
       atomicOr(&A.ctl->err, (int64_t)(vb0 + nc) > A.vertCap ? ERR_VERT_CAP : ERR_NBR_CAP);

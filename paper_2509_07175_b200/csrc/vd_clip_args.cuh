@@ -15,6 +15,7 @@ struct ClipArgs {
   const int* nearList;     // [n][nearClips] or nullptr
   int n, m, kind;
   int realEdges, ballCells, nearClips;
+  int queue;               // 1: the pair list is read by a running kernel (device-side queue): publish slots with a fence
   Control* ctl;
   Pair* pairs;
   Piece* pieces;
@@ -58,7 +59,7 @@ __device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, doubl
   // the simplex id doubles as the slot's ready flag for the device-side queue: written last, after a fence
   Pair* p = &A.pairs[slot];
   p->i = j; p->wx = wx; p->wy = wy; p->wz = wz;
-  __threadfence();
+  if (A.queue) __threadfence();   // other schedules read the list in a later launch
   *reinterpret_cast<volatile int*>(&p->a) = a;
 }
 

@@ -169,19 +169,20 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_fix(ClipArgs A, CellS
 }
 
 __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
-                                                     int64_t begin, PhaseCtl* pc) {
+                                                     int64_t begin, int vchunk, int nchunk) {
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
-  for (;;) {
-    const int t = next_item(pc, count);
-    if (t < 0) break;
+  WarpPool wp = {0ull, 0ull, 0, 0, vchunk, nchunk};
+  // uniform work per piece: a static stride instead of a ticket (one same-address atomic less per piece)
+  const int stride = (int)gridDim.x * kWarpsPerBlock;
+  for (int t = (int)blockIdx.x * kWarpsPerBlock + w; t < count; t += stride) {
     const int slot = list[t];
     const CellState* c = &cells[slot];
     copy_words(&S[w], &c->S, kPolyBytes);
     __syncwarp();
-    finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc);
+    finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc, &wp);
     __syncwarp();
   }
   flush_counters(A.ctl, st, lc);
@@ -253,9 +254,11 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
       int* tmp = clip; clip = other; other = tmp;
     }
     if (h.nDone > 0) {
-      if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
+      // pool chunk per warp: ~1/32 of an even share of the pool, so that the slack (one open chunk per warp) stays small
+      const int64_t warps = (int64_t)grid * kWarpsPerBlock;
+      auto chunk_of = [&](int64_t cap) { const int64_t v = cap / (warps * 32); return (int)(v < 64 ? 64 : (v > 1024 ? 1024 : v)); };
       cudaEventRecord(ev[0], st);
-      VD_LAUNCH(k_ph_finish, grid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, pc);
+      VD_LAUNCH(k_ph_finish, grid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, chunk_of(c->vertCap), chunk_of(c->nbrCap));
       cudaEventRecord(ev[1], st);
       const cudaError_t e = cudaStreamSynchronize(st);
       if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
