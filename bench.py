@@ -217,15 +217,17 @@ def main():
 
     # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
     barrier()
-    t0 = time.perf_counter()
     e2e_steps = max(2, min(args.steps, 5))
     d2h = 0
-    for _ in range(e2e_steps):
+    for k in range(e2e_steps + 1):
+        if k == 1:      # the first pass is warm-up: it page-locks the staging buffers and fills the memory pool
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
         c2 = binding.Context(w.sites)
         c2.set_stream(stream.cuda_stream)
         c2.set_domain(w.verts, w.simplices, w.kind)
         c2.compute()
-        h = c2.to_host()
+        h = c2.to_host(pinned=True)
         c2.destroy()
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps

@@ -103,6 +103,24 @@ def _ptr(x, dtype):
     return a.ctypes.data, a
 
 
+_pinned = {}
+
+
+def _staging(name, shape, dtype, pinned):
+    """Host array for a result; pinned=True: a view of a cached page-locked buffer (grown on demand, reused by
+    later calls: the arrays of the previous pinned result are overwritten), so that the copy runs at PCIe speed."""
+    if not pinned:
+        return np.empty(shape, dtype)
+    import torch
+    count = int(np.prod(shape))
+    nbytes = max(1, count * np.dtype(dtype).itemsize)
+    buf = _pinned.get(name)
+    if buf is None or buf.numel() < nbytes:
+        buf = torch.empty(int(nbytes * 1.25) + 4096, dtype=torch.uint8, pin_memory=True)
+        _pinned[name] = buf
+    return buf.numpy()[:count * np.dtype(dtype).itemsize].view(dtype).reshape(shape)
+
+
 @dataclass
 class HostCells:
     """Result of vd_compute copied to the host (same CSR arrays as include/vd.h's vd_cells)."""
@@ -205,18 +223,20 @@ class Context:
         self._check(self._lib.vd_get_phase_ms(self._h, a))
         return dict(zip(("init", "verify", "fix", "finish"), [float(x) for x in a]))
 
-    def to_host(self, full=True) -> HostCells:
+    def to_host(self, full=True, pinned=False) -> HostCells:
+        """vd_cells_to_host into fresh numpy arrays, or (pinned=True) into cached page-locked staging buffers."""
         r = self.cells
         n, dim, nfl = int(r.n), int(r.dim), int(r.nfl)
         npc, nvt, nnb = int(r.n_pieces), int(r.n_verts), int(r.n_nbrs)
+        E = lambda name, shape, dt: _staging(name, shape, dt, pinned)
         out = HostCells(
             n=n, dim=dim, nfl=nfl, n_nonempty=int(r.n_nonempty),
-            measure=np.empty(n, np.float64), centroid=np.empty((n, dim), np.float64),
-            nbr_off=np.empty(n + 1, np.int64), nbr=np.empty(nnb, np.int32),
-            piece_off=np.empty(n + 1, np.int64), piece_simplex=np.empty(npc, np.int32),
-            piece_measure=np.empty(npc, np.float64), vert_off=np.empty(npc + 1, np.int64),
-            vert_xyz=np.empty((nvt, dim), np.float64) if full else np.empty((0, dim), np.float64),
-            vert_flags=np.empty((nvt, nfl), np.int32) if full else np.empty((0, nfl), np.int32))
+            measure=E("measure", (n,), np.float64), centroid=E("centroid", (n, dim), np.float64),
+            nbr_off=E("nbr_off", (n + 1,), np.int64), nbr=E("nbr", (nnb,), np.int32),
+            piece_off=E("piece_off", (n + 1,), np.int64), piece_simplex=E("piece_simplex", (npc,), np.int32),
+            piece_measure=E("piece_measure", (npc,), np.float64), vert_off=E("vert_off", (npc + 1,), np.int64),
+            vert_xyz=E("vert_xyz", (nvt, dim), np.float64) if full else np.empty((0, dim), np.float64),
+            vert_flags=E("vert_flags", (nvt, nfl), np.int32) if full else np.empty((0, nfl), np.int32))
         d = lambda a: a.ctypes.data if a.size else None
         self._check(self._lib.vd_cells_to_host(
             self._h, d(out.measure), d(out.centroid), d(out.nbr_off), d(out.nbr), d(out.piece_off),

@@ -17,9 +17,26 @@ vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what) {
   return e == cudaErrorMemoryAllocation ? VD_E_NOMEM : VD_E_CUDA;
 }
 
+// Device memory comes from the stream-ordered allocator (cudaMallocAsync) with the default pool told to keep what is
+// freed: creating and destroying contexts in a loop (bench.py's end-to-end leg, a Lloyd driver that rebuilds its
+// context) then costs no cudaMalloc / cudaFree of multi-GB pools after the first round.  vd_set_allocator overrides it.
+static void keep_freed_memory_in_pool() {
+  static bool done[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || done[dev]) return;
+  cudaMemPool_t pool;
+  if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+    unsigned long long keep = ~0ull;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+  }
+  cudaGetLastError();
+  done[dev] = true;
+}
+
 void release(vd_ctx* c, DevBuf& b) {
   if (!b.p) return;
-  if (c->freeFn) c->freeFn(b.p, c->allocUser); else cudaFree(b.p);
+  if (c->freeFn) c->freeFn(b.p, c->allocUser);
+  else if (cudaFreeAsync(b.p, c->stream) != cudaSuccess) { cudaGetLastError(); cudaFree(b.p); }
   b.p = nullptr;
   b.cap = 0;
 }
@@ -35,8 +52,9 @@ vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
     p = c->allocFn(bytes, c->allocUser, (void*)c->stream);
     if (!p) { c->lastError = "allocator hook returned NULL"; return VD_E_NOMEM; }
   } else {
-    const cudaError_t e = cudaMalloc(&p, bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); c->lastError = "cudaMalloc failed"; return VD_E_NOMEM; }
+    cudaError_t e = cudaMallocAsync(&p, bytes, c->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); e = cudaMalloc(&p, bytes); }
+    if (e != cudaSuccess) { cudaGetLastError(); c->lastError = "device memory allocation failed"; return VD_E_NOMEM; }
   }
   b.p = p;
   b.cap = bytes;
@@ -136,6 +154,7 @@ vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out) {
   if (n > 0x7fffffff) return VD_E_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return VD_E_CUDA; }
+  keep_freed_memory_in_pool();
   vd_ctx* c = new (std::nothrow) vd_ctx();
   if (!c) return VD_E_NOMEM;
   c->n = n;
@@ -232,11 +251,11 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     }
   }
   memset(&c->counters, 0, sizeof(c->counters));
-  for (double& v : c->phaseMs) v = 0.0;
   const unsigned long long launches0 = g_launches;
   cudaStream_t st = c->stream;
   vd_status s;
   for (int attempt = 0;; ++attempt) {
+    for (double& v : c->phaseMs) v = 0.0;
     if ((s = alloc_pools(c))) return s;
     if ((s = ensure(c, c->control, sizeof(Control)))) return s;
     cudaMemsetAsync(c->control.p, 0, sizeof(Control), st);
@@ -326,7 +345,8 @@ void vd_destroy(vd_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
+                   &c->scanTmp, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
                    &c->oPieceMeasure, &c->oVertOff, &c->oVertXYZ, &c->oVertFlags};

@@ -280,3 +280,28 @@ def test_box_domain_wave_mode_and_lloyd():
         assert np.abs(got - s).max() <= 1e-9
         g = ctx.to_host()
         parity.assert_parity(g, oracle.compute(got, w.verts, None, w.kind, tier="B"), w.diameter)
+
+
+def test_support_calls_phase_times_counters_and_pinned_copy():
+    w = inputs.config(2, "small")
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        ctx.compute()
+        ph, cnt, st = ctx.phase_ms(), ctx.counters(), ctx.stage_ms()
+        a = ctx.to_host()
+        b = ctx.to_host(pinned=True)
+    assert all(v > 0 for v in ph.values()) and sum(ph.values()) <= st["clip"] * 1.05
+    assert 0 < cnt["search_evals"] < cnt["dist_evals"] and cnt["pre_clips"] == 0
+    for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex", "piece_measure", "vert_off", "vert_xyz", "vert_flags"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    wb = inputs.box(3, 2000, seed=1)
+    with binding.Context(wb.sites) as ctx:
+        ctx.set_domain(wb.verts, None, wb.kind)
+        ctx.compute()
+        cnt = ctx.counters()
+        assert 0 < cnt["pre_clips"] < cnt["clips"]
+    w1 = inputs.config(1, "small")
+    with binding.Context(w1.sites) as ctx:     # 2D kinds run the one-kernel schedule: no step kernels
+        ctx.set_domain(w1.verts, w1.simplices, w1.kind)
+        ctx.compute()
+        assert sum(ctx.phase_ms().values()) == 0.0
