@@ -8,8 +8,8 @@ ABI with HOST buffers: vd_create + vd_set_domain + vd_compute + vd_cells_to_host
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
 
-N > 1 (torchrun): the path does not shard in this round ("replicas only"): every rank runs
-the whole workload on its own GPU; value = N * n / max-over-ranks time.
+N > 1 (torchrun): the path shards by simplex: rank r clips its contiguous block of M against the
+replicated sites, one NCCL all-reduce of per-cell (measure, moment) per step; value = n / max-over-ranks time.
 --impl reference: the CPU oracle, as it stands, timed on the host cores on a bounded sample.
 """
 import argparse
@@ -41,37 +41,81 @@ WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    """SM clock and clock-event (throttle) reasons sampled DURING the timed region, through NVML -- the library
+    nvidia-smi itself reads -- from a thread of this process, every 50 ms.  (A `nvidia-smi -lms 20` child process was
+    measured to slow the phased schedule, which synchronises with the host once per round, from 35 to 47 ms per C2
+    step: every one of its polls holds the driver for milliseconds.  Two NVML reads per sample do not.)  Falls back
+    to `nvidia-smi -lms 200` when NVML cannot be opened."""
 
-    def __init__(self, index):
-        self.index = index
-        self.rows = []
+    def __init__(self, index, uuid=None):
+        self.index, self.uuid = index, uuid
+        self.sm, self.mx, self.reasons = [], [], set()
+        self.stop_flag = threading.Event()
+        self.thread = None
         self.proc = None
+        self.source = None
+
+    def _nvml_loop(self, nv, h):
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                self.reasons.update(n for bit, n in names.items() if r & bit)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.05)
 
     def start(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = None
+            if self.uuid:
+                for u in (self.uuid, "GPU-" + self.uuid):
+                    try:
+                        h = nv.nvmlDeviceGetHandleByUUID(u)
+                        break
+                    except Exception:
+                        h = None
+            if h is None:
+                h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.mx.append(float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)))
+            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
+            self.thread.start()
+            self.source = "nvml, 50 ms"
+            return
+        except Exception:
+            self.thread = None
         q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}",
-                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
+            self.source = "nvidia-smi -lms 200"
         except OSError:
             self.proc = None
 
     def _read(self):
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            r = [x.strip() for x in line.split(",")]
+            if len(r) >= 6 and r[0].replace(".", "").isdigit():
+                self.sm.append(float(r[0]))
+                self.mx.append(float(r[1]))
+                self.reasons.update(names[k] for k in range(4) if r[2 + k].startswith("Active"))
 
     def stop(self):
+        self.stop_flag.set()
+        if self.thread:
+            self.thread.join(timeout=1.0)
         if self.proc:
             self.proc.terminate()
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[k] for r in self.rows if len(r) >= 6 for k in range(4) if r[2 + k].startswith("Active")})
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": max(self.mx) if self.mx else None,
+                "reasons": sorted(self.reasons), "samples": len(self.sm), "source": self.source}
 
 
 def algorithmic_flops(cnt, kind):
@@ -182,6 +226,13 @@ def main():
     d_simp = torch.from_numpy(w.simplices).to(dev) if w.simplices is not None else None
     ctx = binding.Context(d_sites)
     ctx.set_stream(stream.cuda_stream)
+    # N > 1: the path shards by simplex: rank r clips its block of M against the replicated sites, one
+    # all-reduce of per-cell (measure, first moment) combines the partial cells -- inside the timed region.  Simple
+    # domains (one piece per cell) have nothing to partition: every rank runs its own replica.
+    sharded = world > 1 and w.simplices is not None
+    if sharded:
+        blk = ranks.simplex_block(w.m, rank, world)
+        ctx.set_options(simplex_begin=blk[0], simplex_end=blk[1])
     ctx.set_domain(d_verts, d_simp, w.kind)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
@@ -190,9 +241,16 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    fp64_meas, _ = binding.fp64_peak(stream.cuda_stream)   # dependent-FMA-chain kernel (vd_dfma_peak), outside the timed region
     for _ in range(args.warmup):
         ctx.compute()
-    sampler = ClockSampler(local)
+        if sharded:
+            ranks.combine_partial_cells(*ctx.device_tensors(), d_sites)
+    try:
+        uuid = str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid)
     sampler.start()
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -202,6 +260,8 @@ def main():
         flush.fill_(k & 0xff)            # L2 flush between timed iterations (not timed)
         ev[k][0].record(stream)
         ctx.compute()
+        if sharded:
+            ranks.combine_partial_cells(*ctx.device_tensors(), d_sites)
         ev[k][1].record(stream)
         clip_ms += ctx.stage_ms()["clip"]
         for name, v in ctx.phase_ms().items():
@@ -213,7 +273,8 @@ def main():
     cnt = ctx.counters()
     stage = ctx.stage_ms()
     cells = ctx.cells
-    value, ms = ranks.whole_job_rate(float(w.n * args.steps), ms, dev)
+    # sharded: the ranks together made ONE diagram of n cells per step; replicas: one each
+    value, ms = ranks.whole_job_rate(float(w.n * args.steps) / (world if sharded else 1), ms, dev)
 
     # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
     barrier()
@@ -225,6 +286,8 @@ def main():
             t0 = time.perf_counter()
         c2 = binding.Context(w.sites)
         c2.set_stream(stream.cuda_stream)
+        if sharded:
+            c2.set_options(simplex_begin=blk[0], simplex_end=blk[1])
         c2.set_domain(w.verts, w.simplices, w.kind)
         c2.compute()
         h = c2.to_host(pinned=True)
@@ -234,7 +297,7 @@ def main():
     d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
                                             "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
     h2d = w.sites.nbytes + w.verts.nbytes + (w.simplices.nbytes if w.simplices is not None else 0)
-    e2e_val, _ = ranks.whole_job_rate(float(w.n), e2e_s * 1e3, dev)
+    e2e_val, _ = ranks.whole_job_rate(float(w.n) / (world if sharded else 1), e2e_s * 1e3, dev)
 
     parts, flops = algorithmic_flops(cnt, w.kind)
     sm_max = clocks["sm_max_mhz"] or 1965.0
@@ -249,10 +312,11 @@ def main():
     achieved = kernel_flops / (kernel_ms * 1e-3) / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "parallelism": ("1 GPU" if world == 1 else (f"simplices in {world} contiguous blocks, sites replicated, one all-reduce of cell moments"
+                                                              if sharded else "replicas only")),
                    "nonempty_cells": int(cells.n_nonempty), "pieces": int(cells.n_pieces), "corners": int(cells.n_verts)},
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
@@ -262,6 +326,8 @@ def main():
         "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
+                     "peak_measured": fp64_meas, "frac_of_measured": achieved / fp64_meas,
+                     "peak_measured_source": "vd_dfma_peak: 8 dependent DFMA chains per thread, 148 x 8 blocks x 256 threads, best of 3, this run",
                      "algorithmic_flop_per_step": kernel_flops, "kernel_ms_per_step": kernel_ms,
                      "share_of_step": kernel_ms * args.steps / ms,
                      "s4_ms_per_step": clip_ms / args.steps, "s4_algorithmic_flop_per_step": flops},

@@ -102,7 +102,12 @@ typedef struct vd_options {
                              sites nearest to v_i (reading U19), so that the point-in-cell loop
                              starts from a small polytope; 0 = default (20 for VD_BOX_3D, none for the
                              other kinds); < 0: none; at most 32.  3D kinds only.                        */
-  int32_t reserved[7];
+  int32_t simplex_begin;  /* multi-GPU sharding: only simplices a in [simplex_begin, simplex_end) are   */
+  int32_t simplex_end;    /* processed -- every piece P_{a,i} of such a simplex, and no other (pairs never leave their
+                             simplex: propagation is by positive flags).  measure / centroid / neighbours /
+                             pieces of a cell are then its PARTIAL sums over that block of M; ranks combine measure and
+                             measure x centroid by one sum.  0, 0 (default) = all of M.  Meshed kinds only.            */
+  int32_t reserved[5];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */
@@ -188,6 +193,12 @@ vd_status vd_nearest(vd_ctx* ctx, const double* queries, int64_t nq, int32_t* ou
 /* Simplex adjacency derived by vd_set_domain, [m][3 or 4] int32: adj[a][k] = simplex across the
  * edge/face opposite local corner k, or m on the domain boundary.  out: host or device. */
 vd_status vd_get_adjacency(vd_ctx* ctx, int32_t* out);
+
+/* Measurement support, not part of the path: the plain FP64 FMA rate of the current device (TFLOP/s, best of three
+ * launches of a dependent-FMA-chain kernel on `cuda_stream`, 2 flop per FMA) -- the denominator of the "alu" roofline
+ * that bench.py reports (the path's inner work is fp64 subtract / multiply-add / compare).
+ * ms_out (may be NULL): duration of that launch.  Errors: VD_E_ARG, VD_E_CUDA, VD_E_NOMEM. */
+vd_status vd_dfma_peak(void* cuda_stream, double* tflops_out, double* ms_out);
 
 const char* vd_last_error(const vd_ctx* ctx);
 const char* vd_version(void);

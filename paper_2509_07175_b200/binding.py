@@ -19,7 +19,7 @@ STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_IN
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
 EXPORTS = ["vd_create", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
            "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_get_phase_ms", "vd_cells_to_host",
-           "vd_nearest", "vd_get_adjacency", "vd_last_error", "vd_version"]
+           "vd_nearest", "vd_get_adjacency", "vd_dfma_peak", "vd_last_error", "vd_version"]
 
 _LIB_PATH = _build.lib_path()
 _lib = None
@@ -44,7 +44,8 @@ class vd_cells(ctypes.Structure):
 class vd_options(ctypes.Structure):
     _fields_ = [("grid_density", ctypes.c_double), ("ball_cells", ctypes.c_int32), ("real_edges", ctypes.c_int32),
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
-                ("near_clips", ctypes.c_int32), ("reserved", ctypes.c_int32 * 7)]
+                ("near_clips", ctypes.c_int32), ("simplex_begin", ctypes.c_int32), ("simplex_end", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 5)]
 
 
 class vd_counters(ctypes.Structure):
@@ -77,6 +78,7 @@ def load():
     lib.vd_cells_to_host.argtypes = [vp] + [vp] * 10
     lib.vd_nearest.argtypes = [vp, vp, i64, vp]
     lib.vd_get_adjacency.argtypes = [vp, vp]
+    lib.vd_dfma_peak.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.vd_last_error.argtypes = [vp]
     lib.vd_last_error.restype = ctypes.c_char_p
     lib.vd_version.restype = ctypes.c_char_p
@@ -202,6 +204,20 @@ class Context:
         self._check(self._lib.vd_compute(self._h, ctypes.byref(self.cells)))
         return self.cells
 
+    def device_tensors(self):
+        """(measure [n], centroid [n][dim]) as torch tensors that VIEW the context's device buffers (no copy; valid
+        until the next compute): what the ranks hand to the all-reduce of the sharded path (ranks.combine_partial_cells)."""
+        import torch
+
+        class _View:
+            def __init__(self, ptr, shape):
+                self.__cuda_array_interface__ = {"shape": shape, "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+        r = self.cells
+        n, dim = int(r.n), int(r.dim)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        return (torch.as_tensor(_View(r.measure, (n,)), device=dev), torch.as_tensor(_View(r.centroid, (n, dim)), device=dev))
+
     def lloyd(self, iterations: int) -> np.ndarray:
         """vd_lloyd: returns the final sites [n][dim]; self.cells describes them."""
         out = np.empty((self.n, self.dim), np.float64)
@@ -271,6 +287,15 @@ class Context:
             self.destroy()
         except Exception:
             pass
+
+
+def fp64_peak(stream=None) -> tuple[float, float]:
+    """vd_dfma_peak: (TFLOP/s, ms) of the dependent-FMA-chain kernel on the current device."""
+    t, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    st = load().vd_dfma_peak(ctypes.c_void_p(stream or 0), ctypes.byref(t), ctypes.byref(ms))
+    if st != 0:
+        raise VdError(st, "vd_dfma_peak")
+    return float(t.value), float(ms.value)
 
 
 def compute(sites, verts, simplices, kind, **options) -> HostCells:

@@ -3,11 +3,12 @@ from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvd.so")
-SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_phase.cu", "vd_assemble.cu"]
+SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_phase.cu", "vd_assemble.cu", "vd_peak.cu"]
 
 
 def lib_path() -> str:
@@ -19,15 +20,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "vd.h")]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
-    objs = []
-    for s in srcs:
+    extra = os.environ.get("VD_NVCC_FLAGS", "").split()   # experiments: -DVD_... switches of the kernels
+
+    def compile_one(s):
         o = s[:-3] + ".o"
         cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-               "-Xcompiler", "-fPIC", "-c", s, "-o", o]
+               "-Xcompiler", "-fPIC"] + extra + ["-c", s, "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)
-        objs.append(o)
+        return o
+
+    with ThreadPoolExecutor(max_workers=len(srcs)) as pool:   # one nvcc per translation unit, side by side
+        objs = list(pool.map(compile_one, srcs))
     subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs)
     for o in objs:
         os.remove(o)

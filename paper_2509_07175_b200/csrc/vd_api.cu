@@ -380,6 +380,11 @@ vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
   if (!(c->opt.grid_density > 0)) c->opt.grid_density = d.grid_density;
   if (c->opt.real_edges < 0) c->opt.real_edges = d.real_edges;
   if (c->opt.persistent < 0) c->opt.persistent = d.persistent;
+  if (c->opt.simplex_begin < 0 || c->opt.simplex_end < 0 || (c->opt.simplex_end > 0 && c->opt.simplex_begin > c->opt.simplex_end)) {
+    c->opt.simplex_begin = c->opt.simplex_end = 0;
+    c->lastError = "vd_set_options: bad simplex range";
+    return VD_E_ARG;
+  }
   return VD_OK;
 }
 

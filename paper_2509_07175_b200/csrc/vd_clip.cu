@@ -9,7 +9,7 @@ namespace vd {
 // S3 (Alg. 2 line 4, for every corner instead of the first; Alg. 4 lines 3-6): the nearest site
 // of a corner of T_a owns that corner, so (T_a, N_p) is a non-empty pair and p is its witness.
 __global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc) {
-  for (int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; a < A.m; a += (int64_t)gridDim.x * blockDim.x) {
+  for (int64_t a = A.aBegin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; a < A.aEnd; a += (int64_t)gridDim.x * blockDim.x) {
     for (int k = 0; k < nc; ++k) {
       const int v = A.simp[a * nc + k];
       const int j = A.vnn[v];
@@ -134,6 +134,12 @@ static ClipArgs make_args(vd_ctx* c) {
   A.realEdges = c->opt.real_edges;
   A.ballCells = c->opt.ball_cells == 0 ? 64 : c->opt.ball_cells;
   A.nearClips = near_clips_of(c);
+  A.aBegin = 0; A.aEnd = (int)c->m;
+  if (c->opt.simplex_end > 0 && c->kind != KIND_BOX_2D && c->kind != KIND_BOX_3D) {
+    A.aBegin = c->opt.simplex_begin < 0 ? 0 : c->opt.simplex_begin;
+    A.aEnd = c->opt.simplex_end > (int)c->m ? (int)c->m : c->opt.simplex_end;
+    if (A.aBegin > A.aEnd) A.aBegin = A.aEnd;
+  }
   if (A.nearClips > 0 && c->nearList.p) A.nearList = c->nearList.as<int>();
   A.ctl = c->control.as<Control>();
   A.pairs = c->pairs.as<Pair>();
@@ -175,7 +181,7 @@ vd_status stage_seed(vd_ctx* c) {
   }
   const ClipArgs A = make_args(c);
   if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, 148 * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
-  VD_LAUNCH(k_seed, blocks_for(c->m, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
+  VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
   if (c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D) {
     double cv[8 * 3];
     cudaMemcpyAsync(cv, c->verts.p, sizeof(double) * 3 * c->nc, cudaMemcpyDeviceToHost, st);

@@ -83,39 +83,43 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
   for (int c0 = 0; c0 < nc; c0 += kLanes) {
     const int c = c0 + lane;
     const bool rem = c < nc && S.cmark[c] == 2;
-    int cnt = 0;
-    unsigned short ea[3], eb[3], en[3];
+    // rim edge t of c: the neighbour across (cp[t], cp[t+1]) stays.  No arrays indexed at run time here: they
+    // would live in local memory
+    int nb0 = 0, nb1 = 0, nb2 = 0;
+    bool r0 = false, r1 = false, r2 = false;
     if (rem) {
-#pragma unroll
-      for (int t = 0; t < 3; ++t) {
-        const int nb = S.cadj[c][t];
-        if (S.cmark[nb] != 2) { ea[cnt] = S.cp[c][t]; eb[cnt] = S.cp[c][(t + 1) % 3]; en[cnt] = (unsigned short)nb; ++cnt; }
-      }
+      nb0 = S.cadj[c][0]; nb1 = S.cadj[c][1]; nb2 = S.cadj[c][2];
+      r0 = S.cmark[nb0] != 2; r1 = S.cmark[nb1] != 2; r2 = S.cmark[nb2] != 2;
     }
+    const int cnt = (int)r0 + (int)r1 + (int)r2;
     const int incl = warp_incl_scan(cnt);
     const int base = L + incl - cnt;
     const int tot = shfl(incl, kLanes - 1);
     if (L + tot > P) return 1;
-    for (int k = 0; k < cnt; ++k) {
-      S.be[base + k][0] = ea[k]; S.be[base + k][1] = eb[k]; S.be[base + k][2] = en[k];
-      S.be[base + k][3] = (unsigned short)((c == p && (int)en[k] == s) ? 1 : 0);
-      {
+    if (rem) {
+      const double sc = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+#pragma unroll
+      for (int t = 0; t < 3; ++t) {
+        const bool rt = t == 0 ? r0 : (t == 1 ? r1 : r2);
+        if (!rt) continue;
+        const int nb = t == 0 ? nb0 : (t == 1 ? nb1 : nb2);
+        const int e = base + (t == 0 ? 0 : (t == 1 ? (int)r0 : (int)r0 + (int)r1));
+        S.be[e][0] = S.cp[c][t]; S.be[e][1] = S.cp[c][(t + 1) % 3]; S.be[e][2] = (unsigned short)nb;
+        S.be[e][3] = (unsigned short)((c == p && nb == s) ? 1 : 0);
         // where the polytope edge (c, neighbour) meets the plane, by interpolation: the fallback position of
         // the new corner when its three planes are ill-conditioned (degenerate inputs, e.g. regular grids)
-        const int nb = en[k];
-        const double sc = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
         const double sn = nx * S.cx[nb] + ny * S.cy[nb] + nz * S.cz[nb] - d;
-        double t = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
-        t = fmin(fmax(t, 0.0), 1.0);
-        double* rim = reinterpret_cast<double*>(&S.key[0][0]) + 3 * (base + k);
-        rim[0] = S.cx[c] + t * (S.cx[nb] - S.cx[c]);
-        rim[1] = S.cy[c] + t * (S.cy[nb] - S.cy[c]);
-        rim[2] = S.cz[c] + t * (S.cz[nb] - S.cz[c]);
-      }
-      // the surviving neighbour's slot that pointed at c will point at the new corner
+        double tt = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
+        tt = fmin(fmax(tt, 0.0), 1.0);
+        double* rim = reinterpret_cast<double*>(&S.key[0][0]) + 3 * e;
+        rim[0] = S.cx[c] + tt * (S.cx[nb] - S.cx[c]);
+        rim[1] = S.cy[c] + tt * (S.cy[nb] - S.cy[c]);
+        rim[2] = S.cz[c] + tt * (S.cz[nb] - S.cz[c]);
+        // the surviving neighbour's slot that pointed at c will point at the new corner
 #pragma unroll
-      for (int t = 0; t < 3; ++t)
-        if (S.cadj[en[k]][t] == c) S.cadj[en[k]][t] = (unsigned short)(0x8000 | (base + k));
+        for (int q = 0; q < 3; ++q)
+          if (S.cadj[nb][q] == c) S.cadj[nb][q] = (unsigned short)(0x8000 | e);
+      }
     }
     L += tot;
     nRemoved += __popc(__ballot_sync(kFull, rem));
@@ -605,7 +609,7 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
   if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
   double nx, ny, nz, d;
   const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
-                                  nx, ny, nz, d, st, lc);
+                                  nx, ny, nz, d, st, lc, reinterpret_cast<double*>(&S.key[0][0]));
   if (j < 0) return 3;
   bool own = false;
   for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == j);

@@ -15,6 +15,7 @@ struct ClipArgs {
   const int* nearList;     // [n][nearClips] or nullptr
   int n, m, kind;
   int realEdges, ballCells, nearClips;
+  int aBegin, aEnd;        // simplices seeded by this context (vd_options.simplex_begin / simplex_end; a rank's block of M)
   int queue;               // 1: the pair list is read by a running kernel (device-side queue): publish slots with a fence
   Control* ctl;
   Pair* pairs;
@@ -258,15 +259,19 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double q
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
 template <bool HV>
-static __device__ __noinline__ int find_bisector_impl(const ClipArgs& A, const GridIndex& g, int i, int j,
+// The arguments are scalars and pointers on purpose: a struct passed by reference to this (not inlined) function
+// would be copied into every thread's local memory, and so would by-reference results -- the plane comes back
+// through out4 (the caller's shared-memory scratch, or a local array), the iteration count as the return's pair.
+static __device__ __noinline__ int find_bisector_impl(const double* __restrict__ sites, int ballCells, const GridIndex& g, int i, int j,
                                              const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
                                              double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
-                                             double& nx, double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
+                                             double* out4, QueryStats& st, unsigned& iters) {
   const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
+  double nx, ny, nz, d;
   for (int it = 0; it < 96; ++it) {
-    lc.search_iters += 1;
-    const double vjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
-                 vjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+    iters += 1;
+    const double vjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
+                 vjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
     nx = vjx - vix; ny = vjy - viy; nz = vjz - viz;
     d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz));
     const double gs = d - (nx * psx + ny * psy + nz * psz);
@@ -280,23 +285,24 @@ static __device__ __noinline__ int find_bisector_impl(const ClipArgs& A, const G
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
-    if (!HV && A.ballCells > 0) {
+    if (!HV && ballCells > 0) {
       // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
       double tb = 2.0;
       int jb = 0x7fffffff;
       const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
       if (scan_ball_min_t(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz, t, i, j, flags, nflags,
-                          A.ballCells, tb, jb, st)) {
+                          ballCells, tb, jb, st)) {
         if (jb != 0x7fffffff) {
           j = jb;
-          const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
-                       wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+          const double wjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
+                       wjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
           nx = wjx - vix; ny = wjy - viy; nz = wjz - viz;
           d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
         }
-        return j;
+        goto found;
       }
     }
+    {
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
@@ -305,24 +311,41 @@ static __device__ __noinline__ int find_bisector_impl(const ClipArgs& A, const G
     if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
 #endif
     const double bound = fmin(di2, dj2);
-    if (bestId == i || bestId == j || best >= bound * (1.0 - 1e-13)) return j;   // nothing nearer, up to rounding
+    if (bestId == i || bestId == j || best >= bound * (1.0 - 1e-13)) goto found;   // nothing nearer, up to rounding
     if (best >= bound * (1.0 - 1e-9)) {   // a (near) tie with a site that owns a plane of P: flag rule
       bool own = false;
       for (int f = lane_id(); f < nflags; f += kLanes) own |= (flags[f] == bestId);
-      if (__any_sync(kFull, own)) return j;
+      if (__any_sync(kFull, own)) goto found;
     }
     j = bestId;
     ptx = qx; pty = qy; ptz = qz;
+    }
   }
   return -1;
+found:
+  if (lane_id() == 0) { out4[0] = nx; out4[1] = ny; out4[2] = nz; out4[3] = d; }
+  __syncwarp();
+  return j;
 }
 
+// scratch4: four doubles of the warp's shared-memory scratch (3D kinds); nullptr: a local array
 template <bool HV>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
-                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc) {
+                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch4 = nullptr) {
   const unsigned e0 = st.dist_evals;
-  const int r = find_bisector_impl<HV>(A, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, nx, ny, nz, d, st, lc);
+  unsigned iters = 0;
+  int r;
+  if (scratch4) {
+    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, scratch4, st, iters);
+    nx = scratch4[0]; ny = scratch4[1]; nz = scratch4[2]; d = scratch4[3];
+  } else {
+    // every lane writes its own copy
+    double out[4] = {0, 0, 0, 0};
+    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out, st, iters);
+    nx = __shfl_sync(kFull, out[0], 0); ny = __shfl_sync(kFull, out[1], 0); nz = __shfl_sync(kFull, out[2], 0); d = __shfl_sync(kFull, out[3], 0);
+  }
+  lc.search_iters += iters;
   lc.search_evals += st.dist_evals - e0;
   return r;
 }

@@ -16,6 +16,9 @@
 
 namespace vd {
 
+#ifndef VD_PH_BLOCKS
+#define VD_PH_BLOCKS 4   // resident blocks per SM of the verify / fix kernels (plain index)
+#endif
 constexpr int P3 = 32, C3 = 64;
 using PolyF = Poly3<P3, C3>;
 
@@ -89,7 +92,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 
 // list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
                                                      int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
@@ -130,7 +133,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_verify(ClipArgs A, Ce
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : 4) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
                                                      int64_t begin, PhaseCtl* pc) {
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];

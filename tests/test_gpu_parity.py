@@ -290,6 +290,10 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
         ph, cnt, st = ctx.phase_ms(), ctx.counters(), ctx.stage_ms()
         a = ctx.to_host()
         b = ctx.to_host(pinned=True)
+        dm, dc = ctx.device_tensors()          # views of the device results (what the ranks all-reduce)
+        assert np.array_equal(dm.cpu().numpy(), a.measure) and np.array_equal(dc.cpu().numpy(), a.centroid)
+    tf, ms = binding.fp64_peak()               # the measured denominator of the "alu" roofline
+    assert 5.0 < tf < 80.0 and ms > 0
     assert all(v > 0 for v in ph.values()) and sum(ph.values()) <= st["clip"] * 1.05
     assert 0 < cnt["search_evals"] < cnt["dist_evals"] and cnt["pre_clips"] == 0
     for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex", "piece_measure", "vert_off", "vert_xyz", "vert_flags"):
@@ -305,3 +309,44 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
         ctx.set_domain(w1.verts, w1.simplices, w1.kind)
         ctx.compute()
         assert sum(ctx.phase_ms().values()) == 0.0
+
+
+@pytest.mark.parametrize("idx,world", [(2, 2), (4, 3), (1, 2)])
+def test_simplex_blocks_partition_the_diagram(idx, world):
+    """Multi-GPU sharding on one device: every rank's block of M computed on its own, then combined
+    as the ranks would.  Each block must hold exactly the whole run's pieces on its simplices (the oracle-checked
+    ones of test_replica_parity), and the partial measures / moments must add up to the whole cells."""
+    import torch
+    from paper_2509_07175_b200 import ranks
+    w = inputs.config(idx, "small")
+    whole, _, _ = _gpu(w)
+    measure = np.zeros(w.n)
+    moment = np.zeros((w.n, w.sites.shape[1]))
+    pieces = [[] for _ in range(w.n)]
+    for r in range(world):
+        b, e = ranks.simplex_block(w.m, r, world)
+        part, cnt, _ = _gpu(w, simplex_begin=b, simplex_end=e)
+        assert ((part.piece_simplex >= b) & (part.piece_simplex < e)).all()
+        m2, c2 = ranks.combine_partial_cells(torch.from_numpy(part.measure.copy()), torch.from_numpy(part.centroid.copy()),
+                                             torch.from_numpy(w.sites.copy()))
+        assert np.array_equal(m2.numpy(), part.measure)          # no group: a rank's own combination
+        measure += part.measure
+        moment += part.measure[:, None] * part.centroid
+        for i in range(w.n):
+            for p in range(part.piece_off[i], part.piece_off[i + 1]):
+                v0, v1 = part.vert_off[p], part.vert_off[p + 1]
+                pieces[i].append((int(part.piece_simplex[p]), part.vert_flags[v0:v1].tobytes(), float(part.piece_measure[p]), part.vert_xyz[v0:v1]))
+    for i in range(w.n):
+        ref = []
+        for p in range(whole.piece_off[i], whole.piece_off[i + 1]):
+            v0, v1 = whole.vert_off[p], whole.vert_off[p + 1]
+            ref.append((int(whole.piece_simplex[p]), whole.vert_flags[v0:v1].tobytes(), float(whole.piece_measure[p]), whole.vert_xyz[v0:v1]))
+        got = sorted(pieces[i], key=lambda t: t[0])
+        assert [t[:2] for t in got] == [t[:2] for t in ref], i     # the same pieces, corner for corner, whichever rank made them
+        for g, o in zip(got, ref):                                  # floating point: to rounding (test_results_are_reproducible)
+            assert abs(g[2] - o[2]) <= 1e-11 * o[2] + 1e-300
+            assert np.abs(g[3] - o[3]).max() <= 1e-12 * w.diameter
+    assert np.abs(measure - whole.measure).max() <= 1e-12 * whole.measure.max()
+    pos = whole.measure > 0
+    cen = moment[pos] / measure[pos][:, None]
+    assert np.abs(cen - whole.centroid[pos]).max() <= 1e-12 * w.diameter

@@ -42,3 +42,60 @@ def test_whole_job_rate_single_process():
     from paper_2509_07175_b200 import ranks
     rate, ms = ranks.whole_job_rate(500.0, 20.0)
     assert ms == 20.0 and abs(rate - 25000.0) < 1e-9
+
+
+def _shard_worker(rank, world, port, out):
+    """Each rank runs the ORACLE on its block of simplices (the CUDA path needs a GPU; the exchange step does
+    not), then the ranks combine partial cells exactly as bench.py --gpus N does."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from oracle import oracle
+    from paper_2509_07175_b200 import inputs, ranks
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = inputs.config(2, "small")
+    b, e = ranks.simplex_block(w.m, rank, world)
+    part = oracle.compute(w.sites, w.verts, w.simplices[b:e], w.kind)
+    m, c = ranks.combine_partial_cells(torch.from_numpy(part.measure.copy()), torch.from_numpy(part.centroid.copy()),
+                                       torch.from_numpy(w.sites.copy()))
+    out.put((rank, b, e, m.numpy(), c.numpy()))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_simplex_blocks_cover_and_balance():
+    from paper_2509_07175_b200 import ranks
+    for m, world in [(48000, 8), (7, 3), (2, 4), (1, 1)]:
+        blocks = [ranks.simplex_block(m, r, world) for r in range(world)]
+        assert blocks[0][0] == 0 and blocks[-1][1] == m
+        assert all(blocks[k][1] == blocks[k + 1][0] for k in range(world - 1))
+        sizes = [e - b for b, e in blocks]
+        assert max(sizes) - min(sizes) <= 1
+
+
+def test_sharded_cells_combine_to_the_whole_two_ranks_gloo():
+    import numpy as np
+    from oracle import oracle
+    from paper_2509_07175_b200 import inputs
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=300) for _ in range(2)), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    w = inputs.config(2, "small")
+    whole = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    assert res[0][1] == 0 and res[0][2] == res[1][1] and res[1][2] == w.m
+    for _, _, _, m, c in res:      # every rank ends with the whole diagram's measures and centroids
+        assert np.abs(m - whole.measure).max() <= 1e-12 * whole.measure.max()
+        assert np.abs(c - whole.centroid).max() <= 1e-9
+        assert abs(m.sum() - w.measure) <= 1e-12 * w.measure
