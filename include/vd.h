@@ -107,7 +107,10 @@ typedef struct vd_options {
                              simplex: propagation is by positive flags).  measure / centroid / neighbours /
                              pieces of a cell are then its PARTIAL sums over that block of M; ranks combine measure and
                              measure x centroid by one sum.  0, 0 (default) = all of M.  Meshed kinds only.            */
-  int32_t reserved[5];
+  int32_t tail_pairs;     /* phased schedule: a round that leaves at most this many pairs with a corner outside hands
+                             them to one kernel that tests and clips them to completion (no further rounds for the
+                             wave); 0 = default (32768); < 0: never                                                */
+  int32_t reserved[4];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */
@@ -176,9 +179,10 @@ vd_status vd_get_counters(const vd_ctx* ctx, vd_counters* out);
 vd_status vd_get_stage_ms(const vd_ctx* ctx, double out_ms[5]);
 
 /* Phased schedule (vd_options.persistent): device time (ms, CUDA events, summed over all launches) of the step
- * kernels of S4 in the last vd_compute: [0] k_ph_init  [1] k_ph_verify  [2] k_ph_fix  [3] k_ph_finish;
- * all 0 when another schedule ran. */
-vd_status vd_get_phase_ms(const vd_ctx* ctx, double out_ms[4]);
+ * kernels of S4 in the last vd_compute: [0] k_ph_init  [1] k_ph_verify  [2] k_ph_fix  [3] k_ph_finish
+ * [4] k_ph_tail (the last few pairs of a wave: tests and clips to completion in one launch); all 0 when another
+ * schedule ran. */
+vd_status vd_get_phase_ms(const vd_ctx* ctx, double out_ms[5]);
 
 /* Copy the last result into caller HOST buffers (any may be NULL to skip).  Sizes are those of
  * vd_cells.  Synchronises the context's stream. */

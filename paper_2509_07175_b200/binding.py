@@ -45,7 +45,7 @@ class vd_options(ctypes.Structure):
     _fields_ = [("grid_density", ctypes.c_double), ("ball_cells", ctypes.c_int32), ("real_edges", ctypes.c_int32),
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
                 ("near_clips", ctypes.c_int32), ("simplex_begin", ctypes.c_int32), ("simplex_end", ctypes.c_int32),
-                ("reserved", ctypes.c_int32 * 5)]
+                ("tail_pairs", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4)]
 
 
 class vd_counters(ctypes.Structure):
@@ -235,9 +235,9 @@ class Context:
         return dict(zip(("index", "seed", "clip", "assemble", "total"), [float(x) for x in a]))
 
     def phase_ms(self):
-        a = (ctypes.c_double * 4)()
+        a = (ctypes.c_double * 5)()
         self._check(self._lib.vd_get_phase_ms(self._h, a))
-        return dict(zip(("init", "verify", "fix", "finish"), [float(x) for x in a]))
+        return dict(zip(("init", "verify", "fix", "finish", "tail"), [float(x) for x in a]))
 
     def to_host(self, full=True, pinned=False) -> HostCells:
         """vd_cells_to_host into fresh numpy arrays, or (pinned=True) into cached page-locked staging buffers."""

@@ -394,9 +394,9 @@ vd_status vd_get_counters(const vd_ctx* c, vd_counters* out) {
   return VD_OK;
 }
 
-vd_status vd_get_phase_ms(const vd_ctx* c, double out_ms[4]) {
+vd_status vd_get_phase_ms(const vd_ctx* c, double out_ms[5]) {
   if (!c || !out_ms) return VD_E_ARG;
-  for (int k = 0; k < 4; ++k) out_ms[k] = c->phaseMs[k];
+  for (int k = 0; k < 5; ++k) out_ms[k] = c->phaseMs[k];
   return VD_OK;
 }
 

@@ -97,7 +97,6 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     const int tot = shfl(incl, kLanes - 1);
     if (L + tot > P) return 1;
     if (rem) {
-      const double sc = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
 #pragma unroll
       for (int t = 0; t < 3; ++t) {
         const bool rt = t == 0 ? r0 : (t == 1 ? r1 : r2);
@@ -105,16 +104,8 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
         const int nb = t == 0 ? nb0 : (t == 1 ? nb1 : nb2);
         const int e = base + (t == 0 ? 0 : (t == 1 ? (int)r0 : (int)r0 + (int)r1));
         S.be[e][0] = S.cp[c][t]; S.be[e][1] = S.cp[c][(t + 1) % 3]; S.be[e][2] = (unsigned short)nb;
-        S.be[e][3] = (unsigned short)((c == p && nb == s) ? 1 : 0);
-        // where the polytope edge (c, neighbour) meets the plane, by interpolation: the fallback position of
-        // the new corner when its three planes are ill-conditioned (degenerate inputs, e.g. regular grids)
-        const double sn = nx * S.cx[nb] + ny * S.cy[nb] + nz * S.cz[nb] - d;
-        double tt = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
-        tt = fmin(fmax(tt, 0.0), 1.0);
-        double* rim = reinterpret_cast<double*>(&S.key[0][0]) + 3 * e;
-        rim[0] = S.cx[c] + tt * (S.cx[nb] - S.cx[c]);
-        rim[1] = S.cy[c] + tt * (S.cy[nb] - S.cy[c]);
-        rim[2] = S.cz[c] + tt * (S.cz[nb] - S.cz[c]);
+        // the removed corner, and whether (c, nb) is the searched real edge p_s p
+        S.be[e][3] = (unsigned short)(c | ((c == p && nb == s) ? 0x8000 : 0));
         // the surviving neighbour's slot that pointed at c will point at the new corner
 #pragma unroll
         for (int q = 0; q < 3; ++q)
@@ -128,6 +119,28 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
   const int nSurv = nc - nRemoved;
   if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
   if (nSurv + L > C) return 1;
+  // (2b) where the new corners are: rim edge (a -> b) gives the corner (a, b, N), the solution of its three planes;
+  // one lane per rim edge, while the removed corners are still in place for the fallback
+  for (int e = lane; e < L; e += kLanes) {
+    const int ea = S.be[e][0], eb = S.be[e][1];
+    double x, y, z;
+    const bool ok = solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
+    if (!ok) {
+      // ill-conditioned planes (degenerate inputs, e.g. regular grids): where the polytope edge (c, neighbour)
+      // meets the new plane, by interpolation
+      const int c = S.be[e][3] & 0x7fff, nb = S.be[e][2];
+      const double sc = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+      const double sn = nx * S.cx[nb] + ny * S.cy[nb] + nz * S.cz[nb] - d;
+      double tt = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
+      tt = fmin(fmax(tt, 0.0), 1.0);
+      x = S.cx[c] + tt * (S.cx[nb] - S.cx[c]);
+      y = S.cy[c] + tt * (S.cy[nb] - S.cy[c]);
+      z = S.cz[c] + tt * (S.cz[nb] - S.cz[c]);
+    }
+    double* rim = reinterpret_cast<double*>(&S.key[0][0]) + 3 * e;
+    rim[0] = x; rim[1] = y; rim[2] = z;
+  }
+  __syncwarp();
   // (3a) compact the surviving corners to the front
   int run = 0;
   for (int c0 = 0; c0 < nc; c0 += kLanes) {
@@ -182,16 +195,11 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     if (nxt == 0xffff || prv == 0xffff || S.pa[ea] != t || S.pb[eb] != t) bad = true;
     S.cadj[t][1] = (unsigned short)nxt;
     S.cadj[t][2] = (unsigned short)prv;
-    double x, y, z;
-    const bool ok = solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
-    if (!ok) {
-      const double* rim = reinterpret_cast<const double*>(&S.key[0][0]) + 3 * e;
-      x = rim[0]; y = rim[1]; z = rim[2];
-    }
-    S.cx[t] = x; S.cy[t] = y; S.cz[t] = z;
+    const double* rim = reinterpret_cast<const double*>(&S.key[0][0]) + 3 * e;
+    S.cx[t] = rim[0]; S.cy[t] = rim[1]; S.cz[t] = rim[2];
     S.cnn[t] = -1;
     // the new corner on the searched real edge p_s p is in Omega_i ∩ Omega_j
-    S.cstate[t] = S.be[e][3] ? ST_IN : ST_UNKNOWN;
+    S.cstate[t] = (S.be[e][3] & 0x8000) ? ST_IN : ST_UNKNOWN;
   }
   __syncwarp();
   nc = nSurv + L;

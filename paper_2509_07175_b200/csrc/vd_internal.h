@@ -40,7 +40,7 @@ struct vd_ctx {
   vd_options opt{};
   vd_counters counters{};
   double stageMs[5] = {0, 0, 0, 0, 0};
-  double phaseMs[4] = {0, 0, 0, 0};
+  double phaseMs[5] = {0, 0, 0, 0, 0};
   cudaEvent_t phaseEv[4] = {nullptr, nullptr, nullptr, nullptr};
   std::string lastError;
   cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};

@@ -20,6 +20,7 @@ namespace vd {
 #define VD_PH_BLOCKS 4   // resident blocks per SM of the verify / fix kernels (plain index)
 #endif
 constexpr int P3 = 32, C3 = 64;
+constexpr int kTailPairs = 32768;   // a round with at most this many pairs left is finished by k_ph_tail
 using PolyF = Poly3<P3, C3>;
 
 struct CellState {
@@ -171,6 +172,53 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
   flush_counters(A.ctl, st, lc);
 }
 
+// The last few pairs of a wave (a verify round left fewer than kTailPairs with a corner outside): tests and clips
+// alternate inside one launch until every corner is in Omega_i -- Alg. 3's loop as it stands --
+// instead of one round trip to the host and two nearly empty launches per remaining round.  Finished pairs join the
+// done list.  The whole loop in one kernel is the instruction-fetch-bound form (header of this file); on a few
+// thousand pairs that does not matter.
+template <bool HV>
+__global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+                                                       int64_t begin, int* __restrict__ doneList, PhaseCtl* pc) {
+  __shared__ GridIndex g;
+  __shared__ PolyF S[kWarpsPerBlock];
+  if (threadIdx.x == 0) g = *A.grid;
+  __syncthreads();
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  QueryStats st = {0u, 0u, 0u};
+  LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  for (;;) {
+    const int t = next_item(pc, count);
+    if (t < 0) break;
+    const int slot = list[t];
+    CellState* c = &cells[slot];
+    int np = c->np, nc = c->nc;
+    const int i = c->i;
+    copy_words(&S[w], &c->S, kPolyBytes);
+    __syncwarp();
+    int failed = 0;
+    for (int guard = 0; guard < 8 * P3 + 32 && nc > 0; ++guard) {
+      int s;
+      const int p = select_out_3d(S[w], A, nc, s);
+      if (p < 0) {
+        if (!classify_unknown_3d<P3, C3, HV>(S[w], g, i, np, nc, st)) break;   // every corner is in Omega_i
+        continue;
+      }
+      const int rc = clip_from_3d<P3, C3, HV>(S[w], g, A, i, p, s, np, nc, st, lc);
+      if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
+      if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
+    }
+    __syncwarp();
+    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
+    if (lane == 0) {
+      c->np = np; c->nc = nc; c->failed = failed;
+      if (np >= 0) doneList[atomicAdd(&pc->nDone, 1u)] = slot;
+    }
+    __syncwarp();
+  }
+  flush_counters(A.ctl, st, lc);
+}
+
 __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
                                                      int64_t begin, int vchunk, int nchunk) {
   __shared__ PolyF S[kWarpsPerBlock];
@@ -213,6 +261,7 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
   cudaStream_t st = c->stream;
   cudaEvent_t* ev = c->phaseEv;
   const int grid = 148 * 4;
+  const int tailPairs = c->opt.tail_pairs == 0 ? kTailPairs : c->opt.tail_pairs;   // < 0: never
   auto elapsed = [&](int which, cudaEvent_t a, cudaEvent_t b) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) c->phaseMs[which] += ms;
@@ -248,6 +297,16 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
       elapsed(1, ev[2], ev[3]);
       if (h.nClip == 0) break;
       if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
+      if ((int)h.nClip <= tailPairs) {
+        cudaEventRecord(ev[1], st);
+        if (hv) VD_LAUNCH(k_ph_tail<true>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, done, pc);
+        else VD_LAUNCH(k_ph_tail<false>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, done, pc);
+        cudaEventRecord(ev[2], st);
+        const cudaError_t e2 = read_ctl(h);
+        if (e2 != cudaSuccess) return cuda_check(c, e2, "phase tail");
+        elapsed(4, ev[1], ev[2]);
+        break;
+      }
       cudaEventRecord(ev[1], st);
       if (hv) VD_LAUNCH(k_ph_fix<true>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
       else VD_LAUNCH(k_ph_fix<false>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);

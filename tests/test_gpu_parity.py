@@ -47,10 +47,11 @@ def test_c1_full_parity():
     assert cnt["pieces"] == len(o.piece_simplex)
 
 
-@pytest.mark.parametrize("idx", [2, 3, 4, 5])
-def test_replica_parity(idx):
+@pytest.mark.parametrize("idx,opts", [(2, {}), (3, {}), (4, {}), (5, {}),
+                                      (3, dict(tail_pairs=-1)), (5, dict(tail_pairs=-1))])   # rounds of k_ph_verify / k_ph_fix only
+def test_replica_parity(idx, opts):
     w = inputs.config(idx, "small")
-    g, cnt, adj = _gpu(w)
+    g, cnt, adj = _gpu(w, **opts)
     o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
     parity.assert_parity(g, o, w.diameter)
     assert np.array_equal(adj, o.simplex_adj)
@@ -58,7 +59,8 @@ def test_replica_parity(idx):
 
 
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
-                                  dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3)])
+                                  dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
+                                  dict(tail_pairs=-1), dict(tail_pairs=64)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -294,7 +296,7 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
         assert np.array_equal(dm.cpu().numpy(), a.measure) and np.array_equal(dc.cpu().numpy(), a.centroid)
     tf, ms = binding.fp64_peak()               # the measured denominator of the "alu" roofline
     assert 5.0 < tf < 80.0 and ms > 0
-    assert all(v > 0 for v in ph.values()) and sum(ph.values()) <= st["clip"] * 1.05
+    assert all(ph[k] > 0 for k in ("init", "verify", "finish")) and ph["fix"] + ph["tail"] > 0 and sum(ph.values()) <= st["clip"] * 1.05
     assert 0 < cnt["search_evals"] < cnt["dist_evals"] and cnt["pre_clips"] == 0
     for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex", "piece_measure", "vert_off", "vert_xyz", "vert_flags"):
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
