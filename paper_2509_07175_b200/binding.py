@@ -45,7 +45,8 @@ class vd_options(ctypes.Structure):
     _fields_ = [("grid_density", ctypes.c_double), ("ball_cells", ctypes.c_int32), ("real_edges", ctypes.c_int32),
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
                 ("near_clips", ctypes.c_int32), ("simplex_begin", ctypes.c_int32), ("simplex_end", ctypes.c_int32),
-                ("tail_pairs", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4)]
+                ("tail_pairs", ctypes.c_int32), ("first_clip", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 3)]
 
 
 class vd_counters(ctypes.Structure):

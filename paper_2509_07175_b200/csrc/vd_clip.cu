@@ -134,6 +134,7 @@ static ClipArgs make_args(vd_ctx* c) {
   A.realEdges = c->opt.real_edges;
   A.ballCells = c->opt.ball_cells == 0 ? 64 : c->opt.ball_cells;
   A.nearClips = near_clips_of(c);
+  A.firstClip = c->opt.first_clip >= 0 ? 1 : 0;
   A.aBegin = 0; A.aEnd = (int)c->m;
   if (c->opt.simplex_end > 0 && c->kind != KIND_BOX_2D && c->kind != KIND_BOX_3D) {
     A.aBegin = c->opt.simplex_begin < 0 ? 0 : c->opt.simplex_begin;

@@ -301,7 +301,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         S.key[slot][0] = S.pflag[f];
         const double inv = 1.0 / fk;
         // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
-        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz);
+        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i);
       }
     }
     nnbr += __popc(pm);
@@ -484,45 +484,59 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
   __syncwarp();
 }
 
-// Reading U19: clip by the bisectors of the sites nearest to v_i first.  Any B_ij is a valid clip of Omega_i
-// (Eq. 1); these need no search, most of them bound the cell, and what is left for the point-in-cell loop is a
-// small polytope around the cell.  A plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology).
+// P <- P clipped by the bisector B_ij of a GIVEN site j, no search: any B_ij is a valid clip of Omega_i (Eq. 1).  A
+// plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology).
 template <int P, int C>
-__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int& np, int& nc, LocalCnt& lc) {
+__device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A, int j, int& np, int& nc, LocalCnt& lc) {
   const int lane = lane_id();
   VD_POLY_REFS;
-  if (A.nearList) {
+  const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
+               wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+  const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
+  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+  // the corner farthest beyond the plane starts R_p
+  double far = 0.0;
+  int p = 0x7fffffff;
+  const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
+  for (int c = lane; c < nc; c += kLanes) {
+    const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+    if (sd > tol && S.cstate[c] != ST_IN && closer(-sd, c, far, p)) { far = -sd; p = c; }
+  }
+  warp_argmin(far, p);
+  if (p == 0x7fffffff) return 0;   // the plane does not cut P
+  if (np >= P) {
+    compact_planes_3d(S, np, nc);
+    if (np >= P) return 1;
+  }
+  lc.clips += 1;
+  lc.pre_clips += 1;
+  return apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
+}
+
+// Clips that need no search, before the point-in-cell loop of Alg. 3 starts:
+// (a) a pair (a, i) discovered through the face of P_{a,u} on B_ui: that face lies in T_a, so B_iu bounds P_{a,i} --
+//     the first clip of G_{a,j} (Fig. 6), taken from the tuple (u, f) the pair carries;
+// (b) reading U19: the bisectors of the sites nearest to v_i.  Most of them bound the cell, and what is left for the
+//     point-in-cell loop is a small polytope around the cell.
+// Returns 0, 1 (capacity), 2 (topology).
+template <int P, int C>
+__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int u, int& np, int& nc, LocalCnt& lc) {
+  const int lane = lane_id();
+  if (A.firstClip && u >= 0 && u != i) {
+    const int rc = clip_by_site_3d(S, A, u, np, nc, lc);
+    if (rc) return rc;
+  }
+  if (A.nearList && nc > 0) {
     const int K = A.nearClips;
     const int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
     for (int t = 0; t < K; ++t) {
       const int j = shfl(mine, t);
       if (j < 0) break;
-      const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
-                   wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
-      const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
-      const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
-      // the corner farthest beyond the plane starts R_p
-      double far = 0.0;
-      int p = 0x7fffffff;
-      const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
-      for (int c = lane; c < nc; c += kLanes) {
-        const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
-        if (sd > tol && S.cstate[c] != ST_IN && closer(-sd, c, far, p)) { far = -sd; p = c; }
-      }
-      warp_argmin(far, p);
-      if (p == 0x7fffffff) continue;   // the plane does not cut P
-      if (np >= P) {
-        compact_planes_3d(S, np, nc);
-        if (np >= P) return 1;
-      }
-      lc.clips += 1;
-      lc.pre_clips += 1;
-      const int rc = apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
+      const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
       if (rc) return rc;
       if (nc == 0) break;
     }
   }
-
   return 0;
 }
 
@@ -642,7 +656,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   init_poly_3d<P, C, BOX>(S, A, pr, np, nc);
   bool failed = false;
   {
-    const int rc = preclip_3d(S, A, i, np, nc, lc);
+    const int rc = preclip_3d(S, A, i, pr.u, np, nc, lc);
     if (rc == 1) return 1;
     if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
   }

@@ -15,6 +15,7 @@ struct ClipArgs {
   const int* nearList;     // [n][nearClips] or nullptr
   int n, m, kind;
   int realEdges, ballCells, nearClips;
+  int firstClip;           // 1: a discovered pair (a, i) is first clipped by B_iu, u the discovering site
   int aBegin, aEnd;        // simplices seeded by this context (vd_options.simplex_begin / simplex_end; a rank's block of M)
   int queue;               // 1: the pair list is read by a running kernel (device-side queue): publish slots with a fence
   Control* ctl;
@@ -53,13 +54,13 @@ __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& s
 
 // Propagation (Alg. 4 lines 11-15): a positive flag j on an edge/face of P_{a,i} means
 // Omega_j meets T_a; push (a, j) once, with a witness point on that edge/face.
-__device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, double wx, double wy, double wz) {
+__device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, double wx, double wy, double wz, int u = -1) {
   if (!visit(A.visited, A.hashMask, a, j)) return;
   const unsigned long long slot = atomicAdd(&A.ctl->pairTail, 1ull);
   if ((int64_t)slot >= A.pairCap) { atomicOr(&A.ctl->err, ERR_PAIR_CAP); return; }
   // the simplex id doubles as the slot's ready flag for the device-side queue: written last, after a fence
   Pair* p = &A.pairs[slot];
-  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz;
+  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz; p->u = u;
   if (A.queue) __threadfence();   // other schedules read the list in a later launch
   *reinterpret_cast<volatile int*>(&p->a) = a;
 }
@@ -70,6 +71,7 @@ __device__ __forceinline__ Pair load_pair(const ClipArgs& A, int64_t idx) {
   Pair r;
   r.a = __ldcg(&p->a); r.i = __ldcg(&p->i);
   r.wx = __ldcg(&p->wx); r.wy = __ldcg(&p->wy); r.wz = __ldcg(&p->wz);
+  r.u = __ldcg(&p->u); r.pad = 0;
   return r;
 }
 

@@ -57,6 +57,7 @@ constexpr int kHeavy = 64;                // sites per cell above which the cell
 struct Pair {
   int a, i;
   double wx, wy, wz;
+  int u, pad;   // the site whose piece P_{a,u} discovered this pair through its face on B_ui (the tuple (u, f) of P:L211); -1: a seed
 };
 
 // Per-pair output record.

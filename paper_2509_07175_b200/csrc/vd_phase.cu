@@ -39,12 +39,19 @@ struct PhaseCtl {
   unsigned ticket, nClip, nDone, pad;
 };
 
-// warp copy in 16-byte words, four loads in flight per lane
+// warp copy in 16-byte words, eight (then four) loads in flight per lane
 __device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes) {
   const uint4* s = reinterpret_cast<const uint4*>(src);
   uint4* d = reinterpret_cast<uint4*>(dst);
   const int n = bytes / 16, lane = lane_id();
   int k = lane;
+  for (; k + 7 * kLanes < n; k += 8 * kLanes) {
+    uint4 v[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = s[k + q * kLanes];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) d[k + q * kLanes] = v[q];
+  }
   for (; k + 3 * kLanes < n; k += 4 * kLanes) {
     const uint4 a = s[k], b = s[k + kLanes], c = s[k + 2 * kLanes], e = s[k + 3 * kLanes];
     d[k] = a; d[k + kLanes] = b; d[k + 2 * kLanes] = c; d[k + 3 * kLanes] = e;
@@ -78,7 +85,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
     const Pair pr = load_pair(A, begin + t);
     int np, nc;
     init_poly_3d<P3, C3, BOX>(S[w], A, pr, np, nc);
-    const int rc = preclip_3d(S[w], A, pr.i, np, nc, lc);
+    const int rc = preclip_3d(S[w], A, pr.i, pr.u, np, nc, lc);
     int failed = 0;
     if (rc == 1) { defer_pair(A, begin + t); np = -1; }
     if (rc == 2) { failed = 1; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }

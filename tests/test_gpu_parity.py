@@ -60,7 +60,7 @@ def test_replica_parity(idx, opts):
 
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
                                   dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
-                                  dict(tail_pairs=-1), dict(tail_pairs=64)])
+                                  dict(tail_pairs=-1), dict(tail_pairs=64), dict(first_clip=-1)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -129,7 +129,9 @@ def test_results_are_reproducible():
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
     assert np.allclose(a.measure, b.measure, rtol=1e-12, atol=0)
     assert np.allclose(a.centroid, b.centroid, rtol=0, atol=1e-12)
-    assert np.allclose(a.piece_measure, b.piece_measure, rtol=1e-11, atol=0)
+    # sliver pieces (1e-14 of their simplex) carry an absolute rounding error ~ eps x |simplex|: the floor of the
+    # full-size parity test
+    assert np.allclose(a.piece_measure, b.piece_measure, rtol=1e-11, atol=1e-12 * w.measure / w.m)
 
 
 def test_schedules_agree():
@@ -297,7 +299,8 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
     tf, ms = binding.fp64_peak()               # the measured denominator of the "alu" roofline
     assert 5.0 < tf < 80.0 and ms > 0
     assert all(ph[k] > 0 for k in ("init", "verify", "finish")) and ph["fix"] + ph["tail"] > 0 and sum(ph.values()) <= st["clip"] * 1.05
-    assert 0 < cnt["search_evals"] < cnt["dist_evals"] and cnt["pre_clips"] == 0
+    assert 0 < cnt["search_evals"] < cnt["dist_evals"]
+    assert 0 < cnt["pre_clips"] <= cnt["pairs"]      # discovered pairs start with the bisector that discovered them
     for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex", "piece_measure", "vert_off", "vert_xyz", "vert_flags"):
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
     wb = inputs.box(3, 2000, seed=1)
