@@ -269,6 +269,8 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
     const bool live = f < np && S.pa[f] != 0xffff;
     double fx = 0, fy = 0, fz = 0;
     int fk = 0;
+    // positive flags of the faces adjacent to f: scalars, not an array indexed at run time
+    int aw0 = -1, aw1 = -1, aw2 = -1, aw3 = -1, aw4 = -1, aw5 = -1, aw6 = -1, naw = 0;
     if (live) {
       // walk the face loop: from a corner, the edge that starts at plane f leads to the next corner
       const int c0 = S.pa[f];
@@ -278,6 +280,15 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
       double vx = 0, vy = 0, vz = 0;
       for (int step = 0; step < nc; ++step) {
         const int t = (S.cp[c][0] == f) ? 0 : ((S.cp[c][1] == f) ? 1 : 2);
+        {
+          // the edge about to be walked separates f from the next plane of c's cyclic triple
+          const int gf = S.pflag[S.cp[c][t == 2 ? 0 : t + 1]];
+          if (gf >= 0) {
+            if (naw == 0) aw0 = gf; else if (naw == 1) aw1 = gf; else if (naw == 2) aw2 = gf; else if (naw == 3) aw3 = gf;
+            else if (naw == 4) aw4 = gf; else if (naw == 5) aw5 = gf; else if (naw == 6) aw6 = gf;
+            ++naw;
+          }
+        }
         c = S.cadj[c][t];
         if (c == c0) break;
         const double wx = S.cx[c] - rx, wy = S.cy[c] - ry, wz = S.cz[c] - rz;
@@ -301,7 +312,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         S.key[slot][0] = S.pflag[f];
         const double inv = 1.0 / fk;
         // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
-        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i);
+        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, aw0, aw1, aw2, aw3, aw4, aw5, aw6);
       }
     }
     nnbr += __popc(pm);
@@ -515,16 +526,27 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
 
 // Clips that need no search, before the point-in-cell loop of Alg. 3 starts:
 // (a) a pair (a, i) discovered through the face of P_{a,u} on B_ui: that face lies in T_a, so B_iu bounds P_{a,i} --
-//     the first clip of G_{a,j} (Fig. 6), taken from the tuple (u, f) the pair carries;
+//     the first clip of G_{a,j} (Fig. 6), taken from the tuple (u, f) the pair carries; then B_iw for
+//     every face of P_{a,u} adjacent to f with a positive flag w ("clip by B_{j,w} for each adjacent face of f",
+//     P:L211): cells u, i, w meet along that edge of f, which lies in T_a, so B_iw bounds P_{a,i} too;
 // (b) reading U19: the bisectors of the sites nearest to v_i.  Most of them bound the cell, and what is left for the
 //     point-in-cell loop is a small polytope around the cell.
 // Returns 0, 1 (capacity), 2 (topology).
 template <int P, int C>
-__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int u, int& np, int& nc, LocalCnt& lc) {
+__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int u, const Pair* pp, int& np, int& nc, LocalCnt& lc) {
   const int lane = lane_id();
   if (A.firstClip && u >= 0 && u != i) {
-    const int rc = clip_by_site_3d(S, A, u, np, nc, lc);
-    if (rc) return rc;
+    // lane 0: u; lanes 1 .. kPairW: the adjacent faces' sites (each bounds Omega_i along an edge of f that lies in T_a)
+    int mine = -1;
+    if (lane == 0) mine = u;
+    else if (lane <= kPairW) mine = __ldcg(&pp->w[lane - 1]);
+    for (int t = 0; t <= kPairW && nc > 0; ++t) {
+      const int j = shfl(mine, t);
+      if (j < 0) break;
+      if (j == i) continue;
+      const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
+      if (rc) return rc;
+    }
   }
   if (A.nearList && nc > 0) {
     const int K = A.nearClips;
@@ -656,7 +678,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   init_poly_3d<P, C, BOX>(S, A, pr, np, nc);
   bool failed = false;
   {
-    const int rc = preclip_3d(S, A, i, pr.u, np, nc, lc);
+    const int rc = preclip_3d(S, A, i, pr.u, &A.pairs[pairIdx], np, nc, lc);
     if (rc == 1) return 1;
     if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
   }

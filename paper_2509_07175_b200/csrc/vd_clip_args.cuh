@@ -54,13 +54,18 @@ __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& s
 
 // Propagation (Alg. 4 lines 11-15): a positive flag j on an edge/face of P_{a,i} means
 // Omega_j meets T_a; push (a, j) once, with a witness point on that edge/face.
-__device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, double wx, double wy, double wz, int u = -1) {
+__device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, double wx, double wy, double wz, int u = -1,
+                                          int w0 = -1, int w1 = -1, int w2 = -1, int w3 = -1, int w4 = -1, int w5 = -1, int w6 = -1) {
   if (!visit(A.visited, A.hashMask, a, j)) return;
   const unsigned long long slot = atomicAdd(&A.ctl->pairTail, 1ull);
   if ((int64_t)slot >= A.pairCap) { atomicOr(&A.ctl->err, ERR_PAIR_CAP); return; }
   // the simplex id doubles as the slot's ready flag for the device-side queue: written last, after a fence
   Pair* p = &A.pairs[slot];
-  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz; p->u = u;
+  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz;
+  if (u >= 0) {   // the list was filled with -1 (S3)
+    p->u = u;
+    p->w[0] = w0; p->w[1] = w1; p->w[2] = w2; p->w[3] = w3; p->w[4] = w4; p->w[5] = w5; p->w[6] = w6;
+  }
   if (A.queue) __threadfence();   // other schedules read the list in a later launch
   *reinterpret_cast<volatile int*>(&p->a) = a;
 }
@@ -71,7 +76,7 @@ __device__ __forceinline__ Pair load_pair(const ClipArgs& A, int64_t idx) {
   Pair r;
   r.a = __ldcg(&p->a); r.i = __ldcg(&p->i);
   r.wx = __ldcg(&p->wx); r.wy = __ldcg(&p->wy); r.wz = __ldcg(&p->wz);
-  r.u = __ldcg(&p->u); r.pad = 0;
+  r.u = __ldcg(&p->u);   // w[] is read lane by lane where it is used (preclip_3d)
   return r;
 }
 

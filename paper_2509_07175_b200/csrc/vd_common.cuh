@@ -54,11 +54,17 @@ constexpr int kHeavy = 64;                // sites per cell above which the cell
 
 // One unit of work: simplex a, site i, and a witness point w in T_a ∩ Ω_i
 // (DESIGN.md "witness"): the start p_s of virtual edges instead of v_i (Alg. 3 line 3).
+constexpr int kPairW = 7;
+
 struct Pair {
   int a, i;
   double wx, wy, wz;
-  int u, pad;   // the site whose piece P_{a,u} discovered this pair through its face on B_ui (the tuple (u, f) of P:L211); -1: a seed
+  // The tuple (u, f) of P:L211 in the form the clip needs: u = the site whose piece P_{a,u} discovered this pair
+  // through its face f on B_ui, w[] = the positive flags of the faces of P_{a,u} adjacent to f.  -1: none (a seed).
+  int u;
+  int w[kPairW];
 };
+static_assert(sizeof(Pair) == 64, "one pair per 64 bytes");
 
 // Per-pair output record.
 struct Piece {

@@ -300,7 +300,7 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
     assert 5.0 < tf < 80.0 and ms > 0
     assert all(ph[k] > 0 for k in ("init", "verify", "finish")) and ph["fix"] + ph["tail"] > 0 and sum(ph.values()) <= st["clip"] * 1.05
     assert 0 < cnt["search_evals"] < cnt["dist_evals"]
-    assert 0 < cnt["pre_clips"] <= cnt["pairs"]      # discovered pairs start with the bisector that discovered them
+    assert 0 < cnt["pre_clips"] < cnt["clips"]       # discovered pairs start with the bisectors their discovery names
     for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex", "piece_measure", "vert_off", "vert_xyz", "vert_flags"):
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
     wb = inputs.box(3, 2000, seed=1)
@@ -349,7 +349,7 @@ def test_simplex_blocks_partition_the_diagram(idx, world):
         got = sorted(pieces[i], key=lambda t: t[0])
         assert [t[:2] for t in got] == [t[:2] for t in ref], i     # the same pieces, corner for corner, whichever rank made them
         for g, o in zip(got, ref):                                  # floating point: to rounding (test_results_are_reproducible)
-            assert abs(g[2] - o[2]) <= 1e-11 * o[2] + 1e-300
+            assert abs(g[2] - o[2]) <= 1e-11 * o[2] + 1e-12 * w.measure / w.m
             assert np.abs(g[3] - o[3]).max() <= 1e-12 * w.diameter
     assert np.abs(measure - whole.measure).max() <= 1e-12 * whole.measure.max()
     pos = whole.measure > 0
