@@ -312,7 +312,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         S.key[slot][0] = S.pflag[f];
         const double inv = 1.0 / fk;
         // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
-        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, aw0, aw1, aw2, aw3, aw4, aw5, aw6);
+        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, aw0, aw1, aw2, aw3, aw4, aw5, naw > kPairW ? -2 : aw6);
       }
     }
     nnbr += __popc(pm);
@@ -496,7 +496,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
 }
 
 // P <- P clipped by the bisector B_ij of a GIVEN site j, no search: any B_ij is a valid clip of Omega_i (Eq. 1).  A
-// plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology).
+// plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology), -1 (skipped).
 template <int P, int C>
 __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A, int j, int& np, int& nc, LocalCnt& lc) {
   const int lane = lane_id();
@@ -514,7 +514,7 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
     if (sd > tol && S.cstate[c] != ST_IN && closer(-sd, c, far, p)) { far = -sd; p = c; }
   }
   warp_argmin(far, p);
-  if (p == 0x7fffffff) return 0;   // the plane does not cut P
+  if (p == 0x7fffffff) return -1;   // the plane does not cut P
   if (np >= P) {
     compact_planes_3d(S, np, nc);
     if (np >= P) return 1;
@@ -540,12 +540,25 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
     int mine = -1;
     if (lane == 0) mine = u;
     else if (lane <= kPairW) mine = __ldcg(&pp->w[lane - 1]);
+    // When every one of them cut P, the face of P on B_iu IS f: a convex polygon is the intersection of the
+    // half-planes of its edges, f's edges come from exactly these faces (and faces of T_a, which P has), and on
+    // B_iu the half-spaces H_iw and H_uw agree.  f is a face of the finished P_{a,u}, so its corners are in Omega_i:
+    // they need no point-in-cell test.
+    bool complete = true;
+    const int pu = np;   // B_iu's plane index, if it cuts
     for (int t = 0; t <= kPairW && nc > 0; ++t) {
       const int j = shfl(mine, t);
+      if (j == -2) complete = false;   // f had more adjacent faces than a pair carries
       if (j < 0) break;
-      if (j == i) continue;
+      if (j == i) { complete = false; continue; }
       const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
-      if (rc) return rc;
+      if (rc > 0) return rc;
+      if (rc < 0) complete = false;
+    }
+    if (complete && nc > 0 && np < P) {   // (np == P: the plane list may have been compacted, pu renumbered)
+      for (int c = lane; c < nc; c += kLanes)
+        if (S.cp[c][0] == pu || S.cp[c][1] == pu || S.cp[c][2] == pu) S.cstate[c] = ST_IN;
+      __syncwarp();
     }
   }
   if (A.nearList && nc > 0) {
@@ -555,7 +568,7 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
       const int j = shfl(mine, t);
       if (j < 0) break;
       const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
-      if (rc) return rc;
+      if (rc > 0) return rc;
       if (nc == 0) break;
     }
   }
