@@ -33,6 +33,71 @@ __device__ __forceinline__ void lerp_to_plane(double cx, double cy, double cz, d
   x = cx + t * (bx - cx); y = cy + t * (by - cy); z = cz + t * (bz - cz);
 }
 
+// P <- P clipped by the line (n, d) with flag j, starting from the outside corner p; s = the known-inside neighbour
+// of p when the clip comes from a search on the real edge p_s p (else -1).  The few-corner loop surgery is done by
+// lane 0.  Returns 0, or 1 when the loop outgrows K.
+template <int K>
+__device__ __forceinline__ int apply_clip_2d(Poly2<K>& S, int p, int s, double nx, double ny, double nz, double d, int j,
+                                             double pnx, double pny, double pnz) {
+  const int lane = lane_id();
+  const int nc = S.nc;
+  __syncwarp();
+  int rc = 0;
+  if (lane == 0) {
+    // outside run around p (P:L391's R_p for a loop): corners beyond the line, not known inside
+    int r0 = p, r1 = p, len = 1;
+    while (len < nc) {
+      const int q = (r0 + nc - 1) % nc;
+      const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
+      if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
+      r0 = q; ++len;
+    }
+    while (len < nc) {
+      const int q = (r1 + 1) % nc;
+      const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
+      if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
+      r1 = q; ++len;
+    }
+    if (len >= nc) {
+      S.nc = 0;
+    } else if (nc - len + 2 > K) {
+      rc = 1;
+    } else {
+      const int pv = (r0 + nc - 1) % nc, nxt = (r1 + 1) % nc;
+      int k = 0;
+      for (int c = nxt;; c = (c + 1) % nc) {   // survivors nxt .. pv keep corner and edge
+        S.tx[k] = S.cx[c]; S.ty[k] = S.cy[c]; S.tz[k] = S.cz[c];
+        S.tnx[k] = S.enx[c]; S.tny[k] = S.eny[c]; S.tnz[k] = S.enz[c]; S.td[k] = S.ed[c];
+        S.tflag[k] = S.eflag[c]; S.tnn[k] = S.cnn[c]; S.tstate[k] = S.cstate[c];
+        ++k;
+        if (c == pv) break;
+      }
+      // X = edge(pv) ∩ B_ij : start of the new edge, which takes flag j
+      if (!solve3(S.enx[pv], S.eny[pv], S.enz[pv], S.ed[pv], nx, ny, nz, d, pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
+        lerp_to_plane(S.cx[r0], S.cy[r0], S.cz[r0], S.cx[pv], S.cy[pv], S.cz[pv], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
+      S.tnx[k] = nx; S.tny[k] = ny; S.tnz[k] = nz; S.td[k] = d; S.tflag[k] = j; S.tnn[k] = -1;
+      S.tstate[k] = (s == pv && p == r0) ? ST_IN : ST_UNKNOWN;   // on the searched real edge
+      ++k;
+      // E = B_ij ∩ edge(r1) : the rest of edge r1 keeps its plane and flag
+      if (!solve3(nx, ny, nz, d, S.enx[r1], S.eny[r1], S.enz[r1], S.ed[r1], pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
+        lerp_to_plane(S.cx[r1], S.cy[r1], S.cz[r1], S.cx[nxt], S.cy[nxt], S.cz[nxt], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
+      S.tnx[k] = S.enx[r1]; S.tny[k] = S.eny[r1]; S.tnz[k] = S.enz[r1]; S.td[k] = S.ed[r1];
+      S.tflag[k] = S.eflag[r1]; S.tnn[k] = -1;
+      S.tstate[k] = (s == nxt && p == r1) ? ST_IN : ST_UNKNOWN;
+      ++k;
+      for (int c = 0; c < k; ++c) {
+        S.cx[c] = S.tx[c]; S.cy[c] = S.ty[c]; S.cz[c] = S.tz[c];
+        S.enx[c] = S.tnx[c]; S.eny[c] = S.tny[c]; S.enz[c] = S.tnz[c]; S.ed[c] = S.td[c];
+        S.eflag[c] = S.tflag[c]; S.cnn[c] = S.tnn[c]; S.cstate[c] = S.tstate[c];
+      }
+      S.nc = k;
+    }
+  }
+  rc = shfl(rc, 0);
+  __syncwarp();
+  return rc;
+}
+
 template <int K, bool HV, bool BOX>
 __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
@@ -112,6 +177,44 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     if (lane == 0 && bi != i && di - b > 1e-13) printf("BAD WITNESS pair(%d,%d) w=(%g,%g) nearest=%d di2=%g best=%g\n", a, i, pr.wx, pr.wy, bi, di, b);
   }
 #endif
+  // ---- clips that need no search (as for tets: vd_clip3d.cuh preclip_3d): a pair discovered through the
+  // edge e of P_{a,u} on B_ui starts with B_iu, then B_iw for the (at most two) edges of P_{a,u} adjacent to e with a
+  // positive flag w.  When all of them cut, P's edge on B_iu is e itself, and its two end points are in Omega_i.
+  if (A.firstClip && pr.u >= 0 && pr.u != i) {
+    const Pair* pp = &A.pairs[pairIdx];
+    const int w0 = __ldcg(&pp->w[0]), w1 = __ldcg(&pp->w[1]);
+    bool complete = true;
+    for (int t = 0; t < 3 && S.nc > 0; ++t) {
+      const int j = t == 0 ? pr.u : (t == 1 ? w0 : w1);
+      if (j < 0) continue;
+      if (j == i) { complete = false; continue; }
+      const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
+                   wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+      const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
+      const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+      const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
+      const int nc = S.nc;
+      double far = tol;
+      int p = -1;
+      bool owned = false;
+      for (int c = 0; c < nc; ++c) {   // the corner farthest beyond the line starts the outside run
+        const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+        if (sd > far && S.cstate[c] != ST_IN) { far = sd; p = c; }
+        owned |= (S.eflag[c] == j);
+      }
+      if (p < 0 || owned) { complete = false; continue; }   // the line does not cut P
+      lc.clips += 1;
+      lc.pre_clips += 1;
+      if (apply_clip_2d(S, p, -1, nx, ny, nz, d, j, pnx, pny, pnz)) return 1;
+    }
+    __syncwarp();
+    if (complete && lane == 0) {
+      const int nc = S.nc;
+      for (int c = 0; c < nc; ++c)
+        if (S.eflag[c] == pr.u) { S.cstate[c] = ST_IN; S.cstate[(c + 1) % nc] = ST_IN; }
+    }
+    __syncwarp();
+  }
   for (int guard = 0; guard < 4 * K; ++guard) {
     const int nc = S.nc;
     // point-in-cell tests of unclassified corners (section IV-A)
@@ -168,62 +271,10 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
 #endif
     lc.clips += 1;
     __syncwarp();
-    int rc = 0;
-    if (lane == 0) {
-      // outside run around p (P:L391's R_p for a loop): corners beyond the line, not known inside
-      int r0 = p, r1 = p, len = 1;
-      while (len < nc) {
-        const int q = (r0 + nc - 1) % nc;
-        const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
-        if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
-        r0 = q; ++len;
-      }
-      while (len < nc) {
-        const int q = (r1 + 1) % nc;
-        const double sd = nx * S.cx[q] + ny * S.cy[q] + nz * S.cz[q] - d;
-        if (!(sd > 0.0 && S.cstate[q] != ST_IN)) break;
-        r1 = q; ++len;
-      }
-      if (len >= nc) {
-        S.nc = 0;
-      } else if (nc - len + 2 > K) {
-        rc = 1;
-      } else {
-        const int pv = (r0 + nc - 1) % nc, nxt = (r1 + 1) % nc;
-        int k = 0;
-        for (int c = nxt;; c = (c + 1) % nc) {   // survivors nxt .. pv keep corner and edge
-          S.tx[k] = S.cx[c]; S.ty[k] = S.cy[c]; S.tz[k] = S.cz[c];
-          S.tnx[k] = S.enx[c]; S.tny[k] = S.eny[c]; S.tnz[k] = S.enz[c]; S.td[k] = S.ed[c];
-          S.tflag[k] = S.eflag[c]; S.tnn[k] = S.cnn[c]; S.tstate[k] = S.cstate[c];
-          ++k;
-          if (c == pv) break;
-        }
-        // X = edge(pv) ∩ B_ij : start of the new edge, which takes flag j
-        if (!solve3(S.enx[pv], S.eny[pv], S.enz[pv], S.ed[pv], nx, ny, nz, d, pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
-          lerp_to_plane(S.cx[r0], S.cy[r0], S.cz[r0], S.cx[pv], S.cy[pv], S.cz[pv], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
-        S.tnx[k] = nx; S.tny[k] = ny; S.tnz[k] = nz; S.td[k] = d; S.tflag[k] = j; S.tnn[k] = -1;
-        S.tstate[k] = (s == pv && p == r0) ? ST_IN : ST_UNKNOWN;   // on the searched real edge
-        ++k;
-        // E = B_ij ∩ edge(r1) : the rest of edge r1 keeps its plane and flag
-        if (!solve3(nx, ny, nz, d, S.enx[r1], S.eny[r1], S.enz[r1], S.ed[r1], pnx, pny, pnz, 0.0, S.tx[k], S.ty[k], S.tz[k]))
-          lerp_to_plane(S.cx[r1], S.cy[r1], S.cz[r1], S.cx[nxt], S.cy[nxt], S.cz[nxt], nx, ny, nz, d, S.tx[k], S.ty[k], S.tz[k]);
-        S.tnx[k] = S.enx[r1]; S.tny[k] = S.eny[r1]; S.tnz[k] = S.enz[r1]; S.td[k] = S.ed[r1];
-        S.tflag[k] = S.eflag[r1]; S.tnn[k] = -1;
-        S.tstate[k] = (s == nxt && p == r1) ? ST_IN : ST_UNKNOWN;
-        ++k;
-        for (int c = 0; c < k; ++c) {
-          S.cx[c] = S.tx[c]; S.cy[c] = S.ty[c]; S.cz[c] = S.tz[c];
-          S.enx[c] = S.tnx[c]; S.eny[c] = S.tny[c]; S.enz[c] = S.tnz[c]; S.ed[c] = S.td[c];
-          S.eflag[c] = S.tflag[c]; S.cnn[c] = S.tnn[c]; S.cstate[c] = S.tstate[c];
-        }
-        S.nc = k;
-      }
-    }
+    int rc = apply_clip_2d(S, p, s, nx, ny, nz, d, j, pnx, pny, pnz);
 #ifdef VD_TRACE
     if (lane == 0) { printf("   loop:"); for (int c = 0; c < S.nc; ++c) printf(" (%.4f,%.4f|f%d|s%d)", S.cx[c]+ox, S.cy[c]+oy, S.eflag[c], (int)S.cstate[c]); printf("\n"); }
 #endif
-    rc = shfl(rc, 0);
-    __syncwarp();
     if (rc) return 1;
     if (S.nc == 0) break;
   }
@@ -276,8 +327,10 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
       A.poolNbr[nb0 + k++] = S.eflag[c];
       const int c1 = (c + 1) % nc;
       // witness: the edge midpoint lies in T_a ∩ Omega_i ∩ Omega_j
+      // with the tuple (u, f) of P:L211: this cell, and the positive flags of the two edges adjacent to edge c
+      const int fp = S.eflag[(c + nc - 1) % nc], fn = S.eflag[c1];
       push_pair(A, a, S.eflag[c], 0.5 * (S.cx[c] + S.cx[c1]) + ox, 0.5 * (S.cy[c] + S.cy[c1]) + oy,
-                0.5 * (S.cz[c] + S.cz[c1]) + oz);
+                0.5 * (S.cz[c] + S.cz[c1]) + oz, i, fp >= 0 ? fp : -1, fn >= 0 ? fn : -1);
     }
   }
   // corners with their two edge flags, ascending; ranked lexicographically
