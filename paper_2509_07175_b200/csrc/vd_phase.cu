@@ -324,10 +324,12 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
     }
     if (h.nDone > 0) {
       // pool chunk per warp: ~1/32 of an even share of the pool, so that the slack (one open chunk per warp) stays small
-      const int64_t warps = (int64_t)grid * kWarpsPerBlock;
+      // static stride over the grid: exactly the resident blocks (3 per SM), or the last third would run alone
+      const int fgrid = 148 * 3;
+      const int64_t warps = (int64_t)fgrid * kWarpsPerBlock;
       auto chunk_of = [&](int64_t cap) { const int64_t v = cap / (warps * 32); return (int)(v > 1024 ? 1024 : v); };   // small pools: piece by piece
       cudaEventRecord(ev[0], st);
-      VD_LAUNCH(k_ph_finish, grid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, chunk_of(c->vertCap), chunk_of(c->nbrCap));
+      VD_LAUNCH(k_ph_finish, fgrid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, chunk_of(c->vertCap), chunk_of(c->nbrCap));
       cudaEventRecord(ev[1], st);
       const cudaError_t e = cudaStreamSynchronize(st);
       if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
