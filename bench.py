@@ -32,7 +32,7 @@ UNIT = "cells/s"
 FP64_LANES_PER_SM, SMS = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ph_fix, mean of the two launches in the committed
 # ncu --set full capture (profiles/r01_k_ph_fix_c2.md: 0.908 + 1.599 GB and 0.685 + 1.203 GB; the launches of a step
-# differ in size -- these two are rounds 1 and 2 of the third wavefront); null for configs without a capture
+# differ in size -- these two are the first two rounds of a step's first wavefront); null for configs without a capture
 NCU_TRAFFIC_BYTES = {2: 0.5 * (0.908e9 + 1.599e9 + 0.685e9 + 1.203e9)}
 WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
              2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
