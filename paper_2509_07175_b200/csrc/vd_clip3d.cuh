@@ -57,6 +57,105 @@ template <int P, int C>
 __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, double nx, double ny, double nz, double d, int j) {
   const int lane = lane_id();
   const int N = np;   // index of the new plane
+  if (nc <= kLanes) {
+    // ---- Pieces of at most 32 corners (every tet piece; most whole cells): one corner per lane, the corner sets
+    // are bit masks in registers, and when the clip adds at least as many corners as it removes (always, unless
+    // R_p swallows a whole face) the new corners take the slots of the removed ones: nothing else moves.
+    const int c = lane;
+    const bool live = c < nc;
+    const unsigned lt = (1u << lane) - 1u;
+    int a0 = 0, a1 = 0, a2 = 0;
+    bool cand = false;
+    if (live) {
+      const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
+      cand = (c == p) || (sd > 0.0 && S.cstate[c] != ST_IN);
+      a0 = S.cadj[c][0]; a1 = S.cadj[c][1]; a2 = S.cadj[c][2];
+    }
+    // (1) R_p: flood from p over polytope edges among the candidates
+    const unsigned nbm = live ? ((1u << a0) | (1u << a1) | (1u << a2)) : 0u;
+    unsigned R = 1u << p;
+    for (;;) {
+      const unsigned grow = __ballot_sync(kFull, cand && !((R >> c) & 1u) && (nbm & R) != 0u);
+      if (!grow) break;
+      R |= grow;
+    }
+    // (2) rim edges of the removed corners
+    const bool rem = live && ((R >> c) & 1u);
+    const bool r0 = rem && !((R >> a0) & 1u), r1 = rem && !((R >> a1) & 1u), r2 = rem && !((R >> a2) & 1u);
+    const int cnt = (int)r0 + (int)r1 + (int)r2;
+    const unsigned b0 = __ballot_sync(kFull, cnt & 1), b1 = __ballot_sync(kFull, cnt & 2);
+    const int L = __popc(b0) + 2 * __popc(b1), k = __popc(R);
+    if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
+    if (L > P || nc - k + L > C) return 1;
+    if (L >= k) {
+      const int base = __popc(b0 & lt) + 2 * __popc(b1 & lt);
+      if (lane == 0) { S.pnx[N] = nx; S.pny[N] = ny; S.pnz[N] = nz; S.pd[N] = d; S.pflag[N] = j; }
+      if (rem) S.remap[__popc(R & lt)] = (unsigned short)c;   // slot list: the e-th new corner takes the e-th removed slot
+      // which of the surviving neighbour's three slots points back at c (read before anybody rewrites them)
+      int q0 = 0, q1 = 0, q2 = 0;
+      if (r0) q0 = (S.cadj[a0][0] == c) ? 0 : ((S.cadj[a0][1] == c) ? 1 : 2);
+      if (r1) q1 = (S.cadj[a1][0] == c) ? 0 : ((S.cadj[a1][1] == c) ? 1 : 2);
+      if (r2) q2 = (S.cadj[a2][0] == c) ? 0 : ((S.cadj[a2][1] == c) ? 1 : 2);
+      for (int f = lane; f <= N; f += kLanes) { S.pa[f] = 0xffff; S.pb[f] = 0xffff; }
+      __syncwarp();
+      if (rem) {
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+          const bool rt = t == 0 ? r0 : (t == 1 ? r1 : r2);
+          if (!rt) continue;
+          const int nb = t == 0 ? a0 : (t == 1 ? a1 : a2);
+          const int q = t == 0 ? q0 : (t == 1 ? q1 : q2);
+          const int e = base + (t == 0 ? 0 : (t == 1 ? (int)r0 : (int)r0 + (int)r1));
+          const int slot = e < k ? (int)S.remap[e] : nc + (e - k);
+          S.be[e][0] = S.cp[c][t]; S.be[e][1] = S.cp[c][(t + 1) % 3]; S.be[e][2] = (unsigned short)nb;
+          S.be[e][3] = (unsigned short)(c | ((c == p && nb == s) ? 0x8000 : 0));
+          S.cadj[nb][q] = (unsigned short)slot;   // the surviving neighbour now points at the new corner
+        }
+      }
+      __syncwarp();
+      // (2b) + (3) one lane per rim edge (a -> b): the new corner (a, b, N), its position, its neighbours along N
+      bool bad = false;
+      int t = 0, ea = 0, eb = 0, nb = 0, fl = 0;
+      double x = 0, y = 0, z = 0;
+      const int e = lane;
+      if (e < L) {
+        t = e < k ? (int)S.remap[e] : nc + (e - k);
+        ea = S.be[e][0]; eb = S.be[e][1]; nb = S.be[e][2]; fl = S.be[e][3];
+        const bool ok = solve3(S.pnx[ea], S.pny[ea], S.pnz[ea], S.pd[ea], S.pnx[eb], S.pny[eb], S.pnz[eb], S.pd[eb], nx, ny, nz, d, x, y, z);
+        if (!ok) {   // ill-conditioned planes: where the polytope edge (removed corner, neighbour) meets the new plane
+          const int rc = fl & 0x7fff;
+          const double sc = nx * S.cx[rc] + ny * S.cy[rc] + nz * S.cz[rc] - d;
+          const double sn = nx * S.cx[nb] + ny * S.cy[nb] + nz * S.cz[nb] - d;
+          double tt = (sc - sn) > 0.0 ? sc / (sc - sn) : 0.0;
+          tt = fmin(fmax(tt, 0.0), 1.0);
+          x = S.cx[rc] + tt * (S.cx[nb] - S.cx[rc]);
+          y = S.cy[rc] + tt * (S.cy[nb] - S.cy[rc]);
+          z = S.cz[rc] + tt * (S.cz[nb] - S.cz[rc]);
+        }
+        if (S.pa[ea] != 0xffff || S.pb[eb] != 0xffff) bad = true;   // (racy duplicates are caught below)
+        S.pa[ea] = (unsigned short)t;
+        S.pb[eb] = (unsigned short)t;
+      }
+      __syncwarp();   // every read of a removed corner is done: its slot may be rewritten
+      if (e < L) {
+        S.cp[t][0] = (unsigned short)ea; S.cp[t][1] = (unsigned short)eb; S.cp[t][2] = (unsigned short)N;
+        S.cadj[t][0] = (unsigned short)nb;
+        const int nxt = S.pa[eb];   // edge (b -> N) is shared with the corner whose rim edge starts at b
+        const int prv = S.pb[ea];   // edge (N -> a) with the corner whose rim edge ends at a
+        if (nxt == 0xffff || prv == 0xffff || S.pa[ea] != t || S.pb[eb] != t) bad = true;
+        S.cadj[t][1] = (unsigned short)nxt;
+        S.cadj[t][2] = (unsigned short)prv;
+        S.cx[t] = x; S.cy[t] = y; S.cz[t] = z;
+        S.cnn[t] = -1;
+        S.cstate[t] = (fl & 0x8000) ? ST_IN : ST_UNKNOWN;   // on the searched real edge p_s p: in Omega_i
+      }
+      __syncwarp();
+      nc = nc - k + L;
+      np = N + 1;
+      return __any_sync(kFull, bad) ? 2 : 0;
+    }
+  }
+  // ---- general form: any number of corners, survivors compacted to the front
   // (1) candidates: strictly outside the plane and not known to be in Omega_i; p itself always
   for (int c = lane; c < nc; c += kLanes) {
     const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
