@@ -33,6 +33,19 @@ struct alignas(16) Poly3 {
   unsigned char cmark[C];
 };
 
+// What the point-in-cell tests of a piece touch: the leading members of Poly3, at the same offsets, and room for the
+// batch state.  k_ph_verify holds this (2.8 KB per warp) instead of the whole polytope (5.2 KB): the shared memory
+// it does not take is L1 for the site records the tests stream through.
+template <int P, int C>
+struct alignas(16) PolyTest3 {
+  double u[12];
+  int pflag[P];
+  double cx[C], cy[C], cz[C];
+  unsigned char cstate[C];
+  int cnn[C];
+  int key[(sizeof(QBatch) + 11) / 12 + 1][3];   // scratch: the batch of queries
+};
+
 // returns false when the three planes are (numerically) parallel to a common line
 __device__ __forceinline__ bool solve3(double ax, double ay, double az, double ad, double bx, double by, double bz, double bd,
                                        double cx, double cy, double cz, double cd, double& x, double& y, double& z) {
@@ -700,8 +713,9 @@ __device__ __forceinline__ int select_out_3d(const Poly3<P, C>& S, const ClipArg
 
 // Point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one batched
 // pass (vd_batch.cuh); the batch state lives in the scratch area S.key.  Returns whether there were any.
-template <int P, int C, bool HV>
-__device__ __forceinline__ bool classify_unknown_3d(Poly3<P, C>& S, const GridIndex& g, int i, int np, int nc, QueryStats& st) {
+// PolyT: Poly3<P, C>, or PolyTest3<P, C> (the members the tests touch, nothing else: k_ph_verify)
+template <class PolyT, bool HV>
+__device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st) {
   const int lane = lane_id();
   VD_POLY_REFS;
   static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
@@ -801,7 +815,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
     int s;
     const int p = select_out_3d(S, A, nc, s);
     if (p < 0) {
-      if (!classify_unknown_3d<P, C, HV>(S, g, i, np, nc, st)) break;   // every corner is in Omega_i
+      if (!classify_unknown_3d<Poly3<P, C>, HV>(S, g, i, np, nc, st)) break;   // every corner is in Omega_i
       continue;
     }
     const int rc = clip_from_3d<P, C, HV>(S, g, A, i, p, s, np, nc, st, lc);

@@ -19,9 +19,13 @@ namespace vd {
 #ifndef VD_PH_BLOCKS
 #define VD_PH_BLOCKS 4   // resident blocks per SM of the verify / fix kernels (plain index)
 #endif
+#ifndef VD_PHV_BLOCKS
+#define VD_PHV_BLOCKS VD_PH_BLOCKS   // the verify kernel's own (its shared memory would allow more than fix's)
+#endif
 constexpr int P3 = 32, C3 = 64;
 constexpr int kTailPairs = 32768;   // a round with at most this many pairs left is finished by k_ph_tail
 using PolyF = Poly3<P3, C3>;
+using PolyT = PolyTest3<P3, C3>;   // k_ph_verify's view of a parked polytope
 
 struct CellState {
   PolyF S;
@@ -34,6 +38,8 @@ static_assert(sizeof(CellState) % 16 == 0 && sizeof(PolyF) % 16 == 0, "copied in
 constexpr int kTestBytes = (int)offsetof(PolyF, pnx);    // what k_ph_verify reads (and, for cstate and cnn, writes back)
 constexpr int kPolyBytes = (int)offsetof(PolyF, key);    // the polytope without its scratch arrays
 static_assert(kTestBytes % 16 == 0 && kPolyBytes % 16 == 0, "copied in 16-byte words");
+static_assert(offsetof(PolyT, key) == kTestBytes && offsetof(PolyT, cnn) == offsetof(PolyF, cnn) && offsetof(PolyT, cstate) == offsetof(PolyF, cstate),
+              "PolyTest3 mirrors the head of Poly3");
 
 struct PhaseCtl {
   unsigned ticket, nClip, nDone, pad;
@@ -100,10 +106,10 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 
 // list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
+__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
                                                      int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
   __shared__ GridIndex g;
-  __shared__ PolyF S[kWarpsPerBlock];
+  __shared__ PolyT S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
@@ -121,7 +127,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_verify(Cli
     if (!c->failed && nc > 0) {
       copy_words(&S[w], &c->S, kTestBytes);
       __syncwarp();
-      const bool any = classify_unknown_3d<P3, C3, HV>(S[w], g, c->i, np, nc, st);
+      const bool any = classify_unknown_3d<PolyT, HV>(S[w], g, c->i, np, nc, st);
       for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
       out = __any_sync(kFull, out);
       if (any) {
@@ -208,7 +214,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
       int s;
       const int p = select_out_3d(S[w], A, nc, s);
       if (p < 0) {
-        if (!classify_unknown_3d<P3, C3, HV>(S[w], g, i, np, nc, st)) break;   // every corner is in Omega_i
+        if (!classify_unknown_3d<PolyF, HV>(S[w], g, i, np, nc, st)) break;   // every corner is in Omega_i
         continue;
       }
       const int rc = clip_from_3d<P3, C3, HV>(S[w], g, A, i, p, s, np, nc, st, lc);
