@@ -233,7 +233,7 @@ def main():
     # domains (one piece per cell) have nothing to partition: every rank runs its own replica.
     sharded = world > 1 and w.simplices is not None
     if sharded:
-        blk = ranks.simplex_block(w.m, rank, world)
+        blk = ranks.simplex_blocks_balanced(w.sites, w.verts, w.simplices, world)[rank]   # about equal pairs per rank
         ctx.set_options(simplex_begin=blk[0], simplex_end=blk[1])
     ctx.set_domain(d_verts, d_simp, w.kind)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2

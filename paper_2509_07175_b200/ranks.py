@@ -53,3 +53,49 @@ def combine_partial_cells(measure, centroid, sites):
     safe = torch.where(total > 0, total, torch.ones_like(total))
     cen = torch.where((total > 0)[:, None], moment / safe[:, None], sites)
     return total, cen
+
+
+def simplex_blocks_balanced(sites, verts, simplices, world: int, grid: int = 0):
+    """Contiguous blocks of M with about equal WORK instead of equal simplex count ("balanced by an
+    estimate of pairs (sites per simplex + 1)").  The number of pieces of T_a is about 1 + the number of sites
+    near it; that is estimated from a coarse histogram of the sites (grid^d bins of ~64 sites over the joint bounding box):
+    density at the simplex's centroid times the simplex's measure, plus a fringe term.  Returns [(begin, end)] * world, the
+    same on every rank (numpy only, deterministic).  Clustered sites (BASELINE config 3) make equal-count blocks
+    differ several-fold in pairs."""
+    import numpy as np
+    s = np.asarray(sites, np.float64)
+    v = np.asarray(verts, np.float64)
+    t = np.asarray(simplices)
+    m, d = t.shape[0], s.shape[1]
+    if grid <= 0:   # ~64 sites per bin: a density estimate, not noise
+        grid = int(min(64, max(2, round((s.shape[0] / 64.0) ** (1.0 / d)))))
+    lo = np.minimum(s.min(0), v.min(0))
+    hi = np.maximum(s.max(0), v.max(0))
+    ext = np.where(hi > lo, hi - lo, 1.0)
+    bins = np.minimum((np.clip((s - lo) / ext, 0.0, 1.0) * grid).astype(np.int64), grid - 1)
+    flat = np.ravel_multi_index(tuple(bins.T), (grid,) * d)
+    hist = np.bincount(flat, minlength=grid ** d).astype(np.float64)
+    cell_vol = float(np.prod(ext / grid))
+    corners = v[t]                                            # [m][k][d]
+    cen = corners.mean(1)
+    cb = np.minimum((np.clip((cen - lo) / ext, 0.0, 1.0) * grid).astype(np.int64), grid - 1)
+    dens = hist[np.ravel_multi_index(tuple(cb.T), (grid,) * d)] / cell_vol
+    k = t.shape[1]
+    if k == d + 1:      # a d-simplex in R^d: its measure
+        e = corners[:, 1:, :] - corners[:, :1, :]
+        meas = np.abs(np.linalg.det(e)) / float(np.prod(np.arange(1, d + 1)))
+    else:               # a triangle in R^3 (surface): its area times one bin's thickness -- the slab of sites it meets
+        e1, e2 = corners[:, 1] - corners[:, 0], corners[:, 2] - corners[:, 0]
+        meas = 0.5 * np.linalg.norm(np.cross(e1, e2), axis=1) * float(np.mean(ext / grid))
+    inside = dens * meas                                      # expected sites inside T_a
+    # cells meeting T_a: the sites inside, a fringe of cells cut by its boundary (~ inside^((d-1)/d)), at least one
+    work = 1.0 + inside + 3.0 * inside ** ((d - 1.0) / d)
+    cum = np.cumsum(work)
+    cuts = [0]
+    for r in range(1, world):
+        cuts.append(int(np.searchsorted(cum, cum[-1] * r / world)))
+    cuts.append(m)
+    cuts = [min(max(c, 0), m) for c in cuts]
+    for k in range(1, len(cuts)):
+        cuts[k] = max(cuts[k], cuts[k - 1])
+    return [(cuts[r], cuts[r + 1]) for r in range(world)]

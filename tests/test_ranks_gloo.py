@@ -99,3 +99,23 @@ def test_sharded_cells_combine_to_the_whole_two_ranks_gloo():
         assert np.abs(m - whole.measure).max() <= 1e-12 * whole.measure.max()
         assert np.abs(c - whole.centroid).max() <= 1e-9
         assert abs(m.sum() - w.measure) <= 1e-12 * w.measure
+
+
+def test_balanced_blocks_follow_the_pairs():
+    """Work-balanced blocks on the clustered replica: contiguous, covering, and closer to equal PAIRS
+    (counted by the oracle: pieces per simplex) than equal-count blocks are."""
+    import numpy as np
+    from oracle import oracle
+    from paper_2509_07175_b200 import inputs, ranks
+    w = inputs.config(3, "small")
+    world = 4
+    blocks = ranks.simplex_blocks_balanced(w.sites, w.verts, w.simplices, world)
+    assert blocks[0][0] == 0 and blocks[-1][1] == w.m and all(blocks[k][1] == blocks[k + 1][0] for k in range(world - 1))
+    assert blocks == ranks.simplex_blocks_balanced(w.sites, w.verts, w.simplices, world)      # deterministic
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    per_simplex = np.bincount(o.piece_simplex, minlength=w.m)
+    bal = [per_simplex[b:e].sum() for b, e in blocks]
+    eq = [per_simplex[slice(*ranks.simplex_block(w.m, r, world))].sum() for r in range(world)]
+    assert sum(bal) == sum(eq) == len(o.piece_simplex)
+    assert max(bal) < max(eq), (bal, eq)
+    assert max(bal) <= 1.5 * sum(bal) / world, bal
