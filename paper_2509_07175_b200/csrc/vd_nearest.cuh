@@ -181,6 +181,7 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
     if (so >= 0) {
       GridIndex v;
       sub_view(g, cx, cy, cz, so, v);
+#pragma unroll 1   // (code size: the refined-index kernels are instruction-fetch bound)
       for (int pass = 0; pass < 2; ++pass) {
         if (best < 1e300) {
           const double r = sqrt(best);
@@ -232,12 +233,22 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
         // beyond the grid hold no cells)
         double lb = 2e300;
         const int k = s - 1;
-        if (cx - k > 0) lb = fmin(lb, slab_d2(g, 0, qx, 0, cx - k - 1) + oy * oy + oz * oz);
-        if (cx + k < g.G[0] - 1) lb = fmin(lb, slab_d2(g, 0, qx, cx + k + 1, g.G[0] - 1) + oy * oy + oz * oz);
-        if (cy - k > 0) lb = fmin(lb, slab_d2(g, 1, qy, 0, cy - k - 1) + ox * ox + oz * oz);
-        if (cy + k < g.G[1] - 1) lb = fmin(lb, slab_d2(g, 1, qy, cy + k + 1, g.G[1] - 1) + ox * ox + oz * oz);
-        if (cz - k > 0) lb = fmin(lb, slab_d2(g, 2, qz, 0, cz - k - 1) + ox * ox + oy * oy);
-        if (cz + k < g.G[2] - 1) lb = fmin(lb, slab_d2(g, 2, qz, cz + k + 1, g.G[2] - 1) + ox * ox + oy * oy);
+        const double o2 = ox * ox + oy * oy + oz * oz;
+        auto axis_bound = [&](int a) {
+          const int ca = a == 0 ? cx : (a == 1 ? cy : cz);
+          const double qa = a == 0 ? qx : (a == 1 ? qy : qz), oa = a == 0 ? ox : (a == 1 ? oy : oz);
+          const double rest = o2 - oa * oa;   // how far q lies outside the grid box on the other two axes
+          if (ca - k > 0) lb = fmin(lb, slab_d2(g, a, qa, 0, ca - k - 1) + rest);
+          if (ca + k < g.G[a] - 1) lb = fmin(lb, slab_d2(g, a, qa, ca + k + 1, g.G[a] - 1) + rest);
+        };
+        // rolled in the refined-index kernels only: they are bound by instruction fetch (75 KB of code), the
+        // plain-index kernels by the instructions they execute
+        if constexpr (HV) {
+#pragma unroll 1
+          for (int a = 0; a < 3; ++a) axis_bound(a);
+        } else {
+          axis_bound(0); axis_bound(1); axis_bound(2);
+        }
         if (lb > fmin(best, sb)) { done = true; break; }
         if (sb < 1e300) break;
       }
@@ -246,21 +257,37 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
       const int z0 = max(cz - s, 0), z1 = min(cz + s, g.G[2] - 1);
       const int xl = cx - s, xr = cx + s;
       const int xa = max(xl, 0), xb = min(xr, g.G[0] - 1);
-      if (s == 0) {
-        scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, z0, z1, sb, si, st);
-      } else {
-        if (cz - s >= 0) scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, cz - s, cz - s, sb, si, st);
-        if (cz + s < g.G[2]) scan_box<HV>(g, qx, qy, qz, xa, xb, y0, y1, cz + s, cz + s, sb, si, st);
-        const int zi0 = max(cz - s + 1, 0), zi1 = min(cz + s - 1, g.G[2] - 1);
-        if (zi0 <= zi1) {
-          if (cy - s >= 0) scan_box<HV>(g, qx, qy, qz, xa, xb, cy - s, cy - s, zi0, zi1, sb, si, st);
-          if (cy + s < g.G[1]) scan_box<HV>(g, qx, qy, qz, xa, xb, cy + s, cy + s, zi0, zi1, sb, si, st);
-          const int yi0 = max(cy - s + 1, 0), yi1 = min(cy + s - 1, g.G[1] - 1);
-          if (yi0 <= yi1) {
-            if (xl >= 0) scan_box<HV>(g, qx, qy, qz, xl, xl, yi0, yi1, zi0, zi1, sb, si, st);
-            if (xr < g.G[0]) scan_box<HV>(g, qx, qy, qz, xr, xr, yi0, yi1, zi0, zi1, sb, si, st);
+      // the shell's faces: z = cz -+ s, then y = cy -+ s between them, then x = cx -+ s inside both (through ONE call
+      // site in the refined-index kernels: six inlined call sequences are 3 KB of code)
+      const int zi0 = max(cz - s + 1, 0), zi1 = min(cz + s - 1, g.G[2] - 1);
+      const int yi0 = max(cy - s + 1, 0), yi1 = min(cy + s - 1, g.G[1] - 1);
+      auto face = [&](int f) {
+        int bx0 = xa, bx1 = xb, by0 = y0, by1 = y1, bz0 = z0, bz1 = z1;
+        bool ok = true;
+        if (s > 0) {
+          if (f < 2) {
+            const int z = f == 0 ? cz - s : cz + s;
+            ok = z >= 0 && z < g.G[2];
+            bz0 = z; bz1 = z;
+          } else if (f < 4) {
+            const int y = f == 2 ? cy - s : cy + s;
+            ok = y >= 0 && y < g.G[1] && zi0 <= zi1;
+            by0 = y; by1 = y; bz0 = zi0; bz1 = zi1;
+          } else {
+            const int x = f == 4 ? xl : xr;
+            ok = x >= 0 && x < g.G[0] && zi0 <= zi1 && yi0 <= yi1;
+            bx0 = x; bx1 = x; by0 = yi0; by1 = yi1; bz0 = zi0; bz1 = zi1;
           }
         }
+        if (ok) scan_box<HV>(g, qx, qy, qz, bx0, bx1, by0, by1, bz0, bz1, sb, si, st);
+      };
+      if constexpr (HV) {
+        const int nf = s == 0 ? 1 : 6;
+#pragma unroll 1
+        for (int f = 0; f < nf; ++f) face(f);
+      } else {
+        face(0);
+        if (s > 0) { face(1); face(2); face(3); face(4); face(5); }
       }
     }
     if (closer(sb, si, best, bestId)) { best = sb; bestId = si; }
