@@ -161,6 +161,7 @@ vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out) {
   c->dim = dim;
   set_default_options(c->opt);
   for (int k = 0; k < 6; ++k) cudaEventCreate(&c->ev[k]);
+  if (cudaMallocHost(&c->pinned, 1024) != cudaSuccess) { cudaGetLastError(); c->pinned = nullptr; }
   const vd_status s = upload_points(c, sites, n, dim, c->sites, "vd_create");
   if (s != VD_OK) { vd_destroy(c); return s; }
   *out = c;
@@ -355,6 +356,7 @@ void vd_destroy(vd_ctx* c) {
     if (c->ev[k]) cudaEventDestroy(c->ev[k]);
   for (int k = 0; k < 4; ++k)
     if (c->phaseEv[k]) cudaEventDestroy(c->phaseEv[k]);
+  if (c->pinned) cudaFreeHost(c->pinned);
   delete c;
 }
 

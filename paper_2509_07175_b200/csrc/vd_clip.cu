@@ -222,8 +222,11 @@ static void launch(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, i
 }
 
 static cudaError_t read_control(vd_ctx* c, Control& h) {
-  cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
+  static_assert(sizeof(Control) <= 1024, "fits the page-locked staging block");
+  Control* dst = c->pinned ? reinterpret_cast<Control*>(c->pinned) : &h;
+  cudaError_t e = cudaMemcpyAsync(dst, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess && dst != &h) h = *dst;
   return e;
 }
 

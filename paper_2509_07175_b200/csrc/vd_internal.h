@@ -88,6 +88,7 @@ struct vd_ctx {
   vd::DevBuf oMeasure, oCentroid, oNbrOff, oNbr, oPieceOff, oPieceSimplex, oPieceMeasure, oVertOff, oVertXYZ, oVertFlags;
   vd_cells cells{};
   vd::Control hostControl{};
+  void* pinned = nullptr;   // page-locked staging for the small device -> host reads of a compute (round / wave counters)
 };
 
 namespace vd {

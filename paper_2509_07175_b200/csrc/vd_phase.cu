@@ -280,8 +280,11 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
     if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) c->phaseMs[which] += ms;
   };
   auto read_ctl = [&](PhaseCtl& h) -> cudaError_t {
-    cudaError_t e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
+    // through page-locked memory: a copy into pageable memory is staged by the driver (tens of microseconds, once per round)
+    PhaseCtl* dst = c->pinned ? reinterpret_cast<PhaseCtl*>(c->pinned) : &h;
+    cudaError_t e = cudaMemcpyAsync(dst, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess && dst != &h) h = *dst;
     return e;
   };
   for (int64_t b = begin; b < end; b += chunk) {
