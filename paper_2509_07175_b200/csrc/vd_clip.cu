@@ -19,6 +19,42 @@ __global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc) {
   }
 }
 
+// More seeds when a simplex holds very many cells (n >= 64 m: a square of two triangles, "rectangle m = 1"):
+// the pairs of T_a are found by propagation from its seeds over positive flags, one generation of
+// neighbours per wavefront, so with only the corners as seeds a simplex of k cells takes ~k^(1/d) dependent
+// wavefronts.  S interior points per simplex (a fixed low-discrepancy lattice in barycentric coordinates), each with
+// its nearest site, seed (a, N_p) with witness p just as the centroid does in Alg. 4.
+__global__ void __launch_bounds__(kBlock) k_sample_points(ClipArgs A, int nc, int S, double* __restrict__ pts) {
+  const int64_t total = (int64_t)(A.aEnd - A.aBegin) * S;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t a = A.aBegin + idx / S;
+    const int j = (int)(idx % S) + 1;
+    const double alpha[4] = {0.7548776662466927, 0.5698402909980532, 0.8191725133961645, 0.6710436067037893};
+    double w[4], sum = 0.0;
+    for (int k = 0; k < nc; ++k) {
+      const double r = j * alpha[k];
+      w[k] = (r - floor(r)) + 0.02;   // strictly inside
+      sum += w[k];
+    }
+    double x = 0, y = 0, z = 0;
+    for (int k = 0; k < nc; ++k) {
+      const int v = A.simp[a * nc + k];
+      const double t = w[k] / sum;
+      x += t * A.verts[(int64_t)v * 3 + 0]; y += t * A.verts[(int64_t)v * 3 + 1]; z += t * A.verts[(int64_t)v * 3 + 2];
+    }
+    pts[idx * 3 + 0] = x; pts[idx * 3 + 1] = y; pts[idx * 3 + 2] = z;
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_seed_points(ClipArgs A, int S, const double* __restrict__ pts, const int* __restrict__ nn) {
+  const int64_t total = (int64_t)(A.aEnd - A.aBegin) * S;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+    const int j = nn[idx];
+    if (j < 0 || j >= A.n) continue;
+    push_pair(A, (int)(A.aBegin + idx / S), j, pts[idx * 3 + 0], pts[idx * 3 + 1], pts[idx * 3 + 2]);
+  }
+}
+
 // Simple domains (section V-B): a site inside the box owns its own position, so (box, v_i) is a non-empty pair
 // with witness v_i ("each site must be in its own Voronoi cell").
 __global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, double lx, double ly, double lz, double hx, double hy, double hz) {
@@ -183,7 +219,19 @@ vd_status stage_seed(vd_ctx* c) {
   const ClipArgs A = make_args(c);
   if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, 148 * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
   VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
-  if (c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D) {
+  const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
+  const int64_t mLocal = A.aEnd - A.aBegin;
+  if (!boxKind && mLocal > 0 && c->n >= 64 * mLocal) {
+    const int64_t want = c->n / (4 * mLocal);
+    const int S = (int)(want > 256 ? 256 : want);
+    const int64_t total = mLocal * S;
+    if ((s = ensure(c, c->seedPts, sizeof(double) * 3 * total))) return s;
+    if ((s = ensure(c, c->seedNN, sizeof(int) * total))) return s;
+    VD_LAUNCH(k_sample_points, blocks_for(total, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc, S, c->seedPts.as<double>());
+    if ((s = stage_nearest_points(c, c->seedPts.as<double>(), total, c->seedNN.as<int>()))) return s;
+    VD_LAUNCH(k_seed_points, blocks_for(total, kBlock, 148 * 8), kBlock, 0, st)(A, S, c->seedPts.as<double>(), c->seedNN.as<int>());
+  }
+  if (boxKind) {
     double cv[8 * 3];
     cudaMemcpyAsync(cv, c->verts.p, sizeof(double) * 3 * c->nc, cudaMemcpyDeviceToHost, st);
     cudaStreamSynchronize(st);

@@ -64,6 +64,7 @@ struct vd_ctx {
   int64_t subCap = 0;
   // S3-S5
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
+  vd::DevBuf seedPts, seedNN;   // extra seed points inside the simplices and their nearest sites (few simplices, many sites)
   vd::DevBuf nearList;    // int [n][nearClips]  sites nearest to every site, nearest first, -1 padded (reading U19)
   vd::DevBuf control;     // Control
   vd::DevBuf phaseCells;  // phased mode: polytopes of one wave parked between the step kernels (vd_phase.cu)
