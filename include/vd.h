@@ -113,7 +113,10 @@ typedef struct vd_options {
   int32_t first_clip;     /* 0 / 1 (default): a pair (T_a, v_i) discovered through the face of P_{a,u} on B_ui is first
                              clipped by that bisector, without a search -- the first clip of G_{a,j};
                              < 0: every clip is found by a search (Alg. 3 as printed).  3D kinds.                   */
-  int32_t reserved[3];
+  int32_t seed_corners;   /* corners of every simplex whose nearest site seeds a pair (Alg. 2 line 4): 0 = default
+                             (1: the first corner, as in Alg. 2); >= 3 / 4: all of them.  The result does not depend
+                             on it; discovered pairs are cheaper than seeds (first_clip).  Meshed kinds.             */
+  int32_t reserved[2];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */

@@ -6,11 +6,14 @@
 
 namespace vd {
 
-// S3 (Alg. 2 line 4, for every corner instead of the first; Alg. 4 lines 3-6): the nearest site
-// of a corner of T_a owns that corner, so (T_a, N_p) is a non-empty pair and p is its witness.
-__global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc) {
+// S3 (Alg. 2 line 4: the first corner; Alg. 4 lines 3-6: the centroid): the nearest site of a corner of
+// T_a owns that corner, so (T_a, N_p) is a non-empty pair and p is its witness.  One corner per simplex by default
+// (vd_options.seed_corners): a seed pair starts from the bare simplex, a pair discovered from it brings the tuple
+// (u, f) of P:L211 -- first clips without a search, corners known inside (U21, U22) -- so fewer seeds mean
+// cheaper pairs; the closure of any one seed under positive flags is still every cell meeting T_a.
+__global__ void __launch_bounds__(kBlock) k_seed(ClipArgs A, int nc, int nseed) {
   for (int64_t a = A.aBegin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; a < A.aEnd; a += (int64_t)gridDim.x * blockDim.x) {
-    for (int k = 0; k < nc; ++k) {
+    for (int k = 0; k < nseed; ++k) {
       const int v = A.simp[a * nc + k];
       const int j = A.vnn[v];
       if (j < 0 || j >= A.n) continue;
@@ -217,8 +220,9 @@ vd_status stage_seed(vd_ctx* c) {
     release(c, c->nearList);
   }
   const ClipArgs A = make_args(c);
+  const bool boxKind0 = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
   if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, 148 * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
-  VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc);
+  VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
   const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
   const int64_t mLocal = A.aEnd - A.aBegin;
   if (!boxKind && mLocal > 0 && c->n >= 64 * mLocal) {
