@@ -69,23 +69,32 @@ struct AsmArgs {
   int dim;
 };
 
-// one warp per site
-__global__ void __launch_bounds__(kBlock) k_site_assemble(AsmArgs A) {
+// one THREAD per site: an empty cell gets measure 0, centroid = the site (include/vd.h); the others are listed for the
+// warp-per-site kernels (when nearly every cell is empty -- far sites, BASELINE config 5: 0.07 % own a part of the
+// domain -- a warp per site would spend the stage on two million empty visits)
+__global__ void __launch_bounds__(kBlock) k_site_empty(AsmArgs A, int* __restrict__ list) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) {
+    if (A.pieceOff[i + 1] == A.pieceOff[i]) {
+      A.oMeasure[i] = 0.0;
+      for (int a = 0; a < A.dim; ++a) A.oCentroid[i * A.dim + a] = A.sites[i * 3 + a];
+      A.nbrCnt[i] = 0;
+    } else {
+      list[atomicAdd(&A.ctl->nListed, 1u)] = (int)i;
+    }
+  }
+}
+
+// one warp per listed (non-empty) site
+__global__ void __launch_bounds__(kBlock) k_site_assemble(AsmArgs A, const int* __restrict__ list) {
   const int lane = lane_id();
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
   int nonEmpty = 0;
-  for (int64_t i = warp; i < A.n; i += nwarps) {
+  const int64_t listed = A.ctl->nListed;
+  for (int64_t li = warp; li < listed; li += nwarps) {
+    const int64_t i = list[li];
     const int64_t b = A.pieceOff[i], e = A.pieceOff[i + 1];
     const int k = (int)(e - b);
-    if (k == 0) {
-      if (lane == 0) {
-        A.oMeasure[i] = 0.0;   // empty cell: measure 0, centroid = the site (include/vd.h)
-        for (int a = 0; a < A.dim; ++a) A.oCentroid[i * A.dim + a] = A.sites[i * 3 + a];
-        A.nbrCnt[i] = 0;
-      }
-      continue;
-    }
     ++nonEmpty;
     for (int t = lane; t < k; t += kLanes) A.vcount[b + t] = A.pieces[A.order[b + t]].simplex;
     __syncwarp();
@@ -136,11 +145,14 @@ __global__ void __launch_bounds__(kBlock) k_site_assemble(AsmArgs A) {
 }
 
 __global__ void __launch_bounds__(kBlock) k_compact_nbr(const int* __restrict__ nbrRaw, const int64_t* __restrict__ nbrRawOff,
-                                                         const int64_t* __restrict__ nbrOff, int64_t n, int* __restrict__ oNbr) {
+                                                         const int64_t* __restrict__ nbrOff, const Control* __restrict__ ctl,
+                                                         const int* __restrict__ list, int* __restrict__ oNbr) {
   const int lane = lane_id();
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
-  for (int64_t i = warp; i < n; i += nwarps) {
+  const int64_t listed = ctl->nListed;
+  for (int64_t li = warp; li < listed; li += nwarps) {
+    const int64_t i = list[li];
     const int64_t r0 = nbrRawOff[i];
     const int rk = (int)(nbrRawOff[i + 1] - r0);
     int64_t out = nbrOff[i];
@@ -230,14 +242,16 @@ vd_status stage_assemble(vd_ctx* c) {
   A.oMeasure = c->oMeasure.as<double>(); A.oCentroid = c->oCentroid.as<double>();
   A.oPieceSimplex = c->oPieceSimplex.as<int>(); A.oPieceMeasure = c->oPieceMeasure.as<double>();
   A.ctl = c->control.as<Control>(); A.n = n; A.dim = dim;
-  VD_LAUNCH(k_site_assemble, blocks_for(n, kWarpsPerBlock), kBlock, 0, st)(A);
+  if ((s = ensure(c, c->siteList, sizeof(int) * n))) return s;
+  VD_LAUNCH(k_site_empty, blocks_for(n, kBlock), kBlock, 0, st)(A, c->siteList.as<int>());
+  VD_LAUNCH(k_site_assemble, blocks_for(n, kWarpsPerBlock), kBlock, 0, st)(A, c->siteList.as<int>());
   exclusive_scan<int, int64_t>(c->vcount.as<int>(), nPieces, c->oVertOff.as<int64_t>(), tmp, st);
   exclusive_scan<int, int64_t>(c->nbrCnt.as<int>(), n, c->oNbrOff.as<int64_t>(), tmp, st);
   VD_LAUNCH(k_gather_verts, blocks_for(nPieces, kWarpsPerBlock), kBlock, 0, st)(
       c->pieces.as<Piece>(), c->order.as<int>(), c->oVertOff.as<int64_t>(), nPieces, c->poolXYZ.as<double>(), c->poolFlags.as<int>(),
       dim, nfl, c->oVertXYZ.as<double>(), c->oVertFlags.as<int>());
   VD_LAUNCH(k_compact_nbr, blocks_for(n, kWarpsPerBlock), kBlock, 0, st)(c->nbrRaw.as<int>(), c->nbrRawOff.as<int64_t>(),
-                                                                          c->oNbrOff.as<int64_t>(), n, c->oNbr.as<int>());
+                                                                          c->oNbrOff.as<int64_t>(), c->control.as<Control>(), c->siteList.as<int>(), c->oNbr.as<int>());
   VD_LAUNCH(k_totals, 1, 1, 0, st)(c->control.as<Control>(), c->oPieceOff.as<int64_t>(), c->oVertOff.as<int64_t>(),
                                    c->oNbrOff.as<int64_t>(), n, nPieces);
   return cuda_check(c, cudaGetLastError(), "assemble");

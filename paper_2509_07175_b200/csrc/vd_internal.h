@@ -19,6 +19,7 @@ struct Control {
   unsigned int nHeavy;           // refined cells of the site index (second level)
   Counters cnt;
   unsigned long long nPieces, nNonEmpty, nVerts, nNbrs;   // totals written by S6
+  unsigned int nListed, padListed;                        // S6: non-empty sites listed for the warp-per-site kernels
 };
 
 struct DevBuf {
@@ -84,6 +85,7 @@ struct vd_ctx {
   vd::DevBuf nbrRawOff;   // int64 [n+1]
   vd::DevBuf nbrRaw;      // int [sum raw]
   vd::DevBuf nbrCnt;      // int [n]
+  vd::DevBuf siteList;    // int [n]  the non-empty sites
   vd::DevBuf vcount;      // int [pieces]
   // outputs (vd_cells)
   vd::DevBuf oMeasure, oCentroid, oNbrOff, oNbr, oPieceOff, oPieceSimplex, oPieceMeasure, oVertOff, oVertXYZ, oVertFlags;
