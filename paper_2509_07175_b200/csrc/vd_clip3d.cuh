@@ -381,8 +381,9 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
     const bool live = f < np && S.pa[f] != 0xffff;
     double fx = 0, fy = 0, fz = 0;
     int fk = 0;
-    // positive flags of the faces adjacent to f: scalars, not an array indexed at run time
-    int aw0 = -1, aw1 = -1, aw2 = -1, aw3 = -1, aw4 = -1, aw5 = -1, aw6 = -1, naw = 0;
+    // the planes of the faces adjacent to f, eight bits each: decoded only for a pair that is really pushed
+    unsigned long long awp = 0ull;
+    int naw = 0;
     if (live) {
       // walk the face loop: from a corner, the edge that starts at plane f leads to the next corner
       const int c0 = S.pa[f];
@@ -394,12 +395,8 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         const int t = (S.cp[c][0] == f) ? 0 : ((S.cp[c][1] == f) ? 1 : 2);
         {
           // the edge about to be walked separates f from the next plane of c's cyclic triple
-          const int gf = S.pflag[S.cp[c][t == 2 ? 0 : t + 1]];
-          if (gf >= 0) {
-            if (naw == 0) aw0 = gf; else if (naw == 1) aw1 = gf; else if (naw == 2) aw2 = gf; else if (naw == 3) aw3 = gf;
-            else if (naw == 4) aw4 = gf; else if (naw == 5) aw5 = gf; else if (naw == 6) aw6 = gf;
-            ++naw;
-          }
+          if (naw < 8) awp |= (unsigned long long)S.cp[c][t == 2 ? 0 : t + 1] << (8 * naw);
+          ++naw;
         }
         c = S.cadj[c][t];
         if (c == c0) break;
@@ -424,7 +421,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         S.key[slot][0] = S.pflag[f];
         const double inv = 1.0 / fk;
         // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
-        push_pair(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, aw0, aw1, aw2, aw3, aw4, aw5, naw > kPairW ? -2 : aw6);
+        push_pair_faces(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, awp, naw, S.pflag);
       }
     }
     nnbr += __popc(pm);
@@ -471,24 +468,33 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   }
   for (int k = lane; k < nnbr; k += kLanes) A.poolNbr[nb0 + k] = S.key[k][0];
   __syncwarp();
-  // corners: ascending flag triple, corners ranked lexicographically by it
+  // corners: ascending flag triple, corners ranked lexicographically by it.  Two 64-bit keys per corner (flags biased
+  // to unsigned; the corner index breaks ties) in the scratch arrays key / remap / pa / pb, all free by now
+  using PolyPC = Poly3<P, C>;
+  static_assert(offsetof(PolyPC, be) - offsetof(PolyPC, key) >= 16 * (size_t)C, "room for two 64-bit keys per corner");
+  ulonglong2* K = reinterpret_cast<ulonglong2*>(&S.key[0][0]);
+  __syncwarp();
   for (int c = lane; c < nc; c += kLanes) {
     int f0 = S.pflag[S.cp[c][0]], f1 = S.pflag[S.cp[c][1]], f2 = S.pflag[S.cp[c][2]];
     int t;
     if (f0 > f1) { t = f0; f0 = f1; f1 = t; }
     if (f1 > f2) { t = f1; f1 = f2; f2 = t; }
     if (f0 > f1) { t = f0; f0 = f1; f1 = t; }
-    S.key[c][0] = f0; S.key[c][1] = f1; S.key[c][2] = f2;
+    ulonglong2 k;
+    k.x = ((unsigned long long)((unsigned)f0 ^ 0x80000000u) << 32) | (unsigned long long)((unsigned)f1 ^ 0x80000000u);
+    k.y = ((unsigned long long)((unsigned)f2 ^ 0x80000000u) << 32) | (unsigned long long)(unsigned)c;
+    K[c] = k;
   }
   __syncwarp();
   for (int c = lane; c < nc; c += kLanes) {
-    const int k0 = S.key[c][0], k1 = S.key[c][1], k2 = S.key[c][2];
+    const ulonglong2 k = K[c];
     int rank = 0;
     for (int o = 0; o < nc; ++o) {
-      const int o0 = S.key[o][0], o1 = S.key[o][1], o2 = S.key[o][2];
-      const bool less = o0 < k0 || (o0 == k0 && (o1 < k1 || (o1 == k1 && (o2 < k2 || (o2 == k2 && o < c)))));
-      rank += less ? 1 : 0;
+      const ulonglong2 q = K[o];
+      rank += (q.x < k.x || (q.x == k.x && q.y < k.y)) ? 1 : 0;
     }
+    const int k0 = (int)((unsigned)(k.x >> 32) ^ 0x80000000u), k1 = (int)((unsigned)k.x ^ 0x80000000u),
+              k2 = (int)((unsigned)(k.y >> 32) ^ 0x80000000u);
     const int64_t v = (int64_t)vb0 + rank;
     A.poolXYZ[v * 3 + 0] = S.cx[c] + ox; A.poolXYZ[v * 3 + 1] = S.cy[c] + oy; A.poolXYZ[v * 3 + 2] = S.cz[c] + oz;
     A.poolFlags[v * 3 + 0] = k0; A.poolFlags[v * 3 + 1] = k1; A.poolFlags[v * 3 + 2] = k2;

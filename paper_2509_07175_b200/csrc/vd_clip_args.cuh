@@ -70,6 +70,33 @@ __device__ __forceinline__ void push_pair(const ClipArgs& A, int a, int j, doubl
   *reinterpret_cast<volatile int*>(&p->a) = a;
 }
 
+// The same for a pair discovered through a face f of a finished 3D piece: the adjacent faces arrive as plane indices
+// (eight bits each in `planes`, `nplanes` of them, at most eight kept) and are turned into sites here, after the
+// visited test -- four out of five pushes end there.
+__device__ __forceinline__ void push_pair_faces(const ClipArgs& A, int a, int j, double wx, double wy, double wz, int u,
+                                                unsigned long long planes, int nplanes, const int* pflag) {
+  if (!visit(A.visited, A.hashMask, a, j)) return;
+  const unsigned long long slot = atomicAdd(&A.ctl->pairTail, 1ull);
+  if ((int64_t)slot >= A.pairCap) { atomicOr(&A.ctl->err, ERR_PAIR_CAP); return; }
+  Pair* p = &A.pairs[slot];
+  p->i = j; p->wx = wx; p->wy = wy; p->wz = wz;
+  p->u = u;
+  int cnt = 0;
+  const int kept = nplanes < 8 ? nplanes : 8;
+  for (int k = 0; k < kept; ++k) {
+    const int fl = pflag[(int)((planes >> (8 * k)) & 0xffull)];
+    if (fl >= 0) {
+      if (cnt < kPairW) p->w[cnt] = fl;   // (the list was filled with -1: S3)
+      ++cnt;
+    }
+  }
+  // more adjacent faces than a pair carries: the mark sits right behind the last site (the reader stops at the first
+  // negative entry)
+  if (nplanes > 8 || cnt > kPairW) p->w[cnt < kPairW ? cnt : kPairW - 1] = -2;
+  if (A.queue) __threadfence();
+  *reinterpret_cast<volatile int*>(&p->a) = a;
+}
+
 // A pair may have been written by another SM a moment ago: read it past the (incoherent) L1.
 __device__ __forceinline__ Pair load_pair(const ClipArgs& A, int64_t idx) {
   const Pair* p = &A.pairs[idx];
