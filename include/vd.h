@@ -109,7 +109,7 @@ typedef struct vd_options {
                              measure x centroid by one sum.  0, 0 (default) = all of M.  Meshed kinds only.            */
   int32_t tail_pairs;     /* phased schedule: a round that leaves at most this many pairs with a corner outside hands
                              them to one kernel that tests and clips them to completion (no further rounds for the
-                             wave); 0 = default (32768); < 0: never                                                */
+                             wave); 0 = default (65536); < 0: never                                                */
   int32_t first_clip;     /* 0 / 1 (default): a pair (T_a, v_i) discovered through the face of P_{a,u} on B_ui is first
                              clipped by that bisector, without a search -- the first clip of G_{a,j};
                              < 0: every clip is found by a search (Alg. 3 as printed).  3D kinds.                   */

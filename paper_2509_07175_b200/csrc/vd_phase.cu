@@ -23,7 +23,7 @@ namespace vd {
 #define VD_PHV_BLOCKS VD_PH_BLOCKS   // the verify kernel's own (its shared memory would allow more than fix's)
 #endif
 constexpr int P3 = 32, C3 = 64;
-constexpr int kTailPairs = 32768;   // a round with at most this many pairs left is finished by k_ph_tail
+constexpr int kTailPairs = 65536;   // a round with at most this many pairs left is finished by k_ph_tail
 using PolyF = Poly3<P3, C3>;
 using PolyT = PolyTest3<P3, C3>;   // k_ph_verify's view of a parked polytope
 
