@@ -359,3 +359,34 @@ def test_simplex_blocks_partition_the_diagram(idx, world):
     pos = whole.measure > 0
     cen = moment[pos] / measure[pos][:, None]
     assert np.abs(cen - whole.centroid[pos]).max() <= 1e-12 * w.diameter
+
+
+@pytest.mark.parametrize("kind", ["tet", "tri"])
+def test_one_simplex_many_cells(kind):
+    """A single simplex holding thousands of cells: the interior seed points (n >= 64 m) and, through them, long
+    chains of discovered pairs -- Voronoi faces of nine and more edges among them, whose adjacent-face list does
+    not fit a pair (U21, U22).  (The misplaced "list truncated" mark of an earlier build shows on the C2
+    replica, test_replica_parity[2]: it needs such a face next to faces of the simplex.)"""
+    rng = np.random.default_rng(77)
+    if kind == "tet":
+        verts = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1]], np.float64)
+        simp = np.array([[0, 1, 2, 3]], np.int32)
+        sites = rng.random((3000, 3)) * 1.2 - 0.1
+        w = inputs.custom(inputs.KIND_TET_3D, sites, verts, simp, "one_tet")
+    else:
+        verts = np.array([[0, 0], [1, 0], [0, 1]], np.float64)
+        simp = np.array([[0, 1, 2]], np.int32)
+        sites = rng.random((4000, 2)) * 1.2 - 0.1
+        w = inputs.custom(inputs.KIND_TRI_2D, sites, verts, simp, "one_tri")
+    g, cnt, _ = _gpu(w)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+    assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
+    assert cnt["waves"] >= 1 and cnt["pre_clips"] > 0
+    if kind == "tet":      # the case this test is for does occur: some finished piece has a face of more than 8 edges
+        nedges = []
+        for p in range(len(g.piece_simplex)):
+            fl = g.vert_flags[g.vert_off[p]:g.vert_off[p + 1]]
+            ids, counts = np.unique(fl[fl >= 0], return_counts=True)
+            nedges.append(counts.max() if len(counts) else 0)
+        assert max(nedges) > 8
