@@ -292,7 +292,9 @@ vd_status stage_clip(vd_ctx* c) {
   const int mode = c->opt.persistent;
   const bool solid = c->kind == KIND_TET_3D || c->kind == KIND_BOX_3D;
   const bool phased = solid && (mode == 1 || mode == 2);   // 3D kinds: one small kernel per step (vd_phase.cu)
-  const bool persist = mode != 0 && !phased;               // otherwise the device-side queue, or one launch per wave
+  // otherwise the one-kernel form: a device-side queue (3), or one launch per wave (0; and the default of the triangle
+  // kinds: with the discovery tuples and interior seeds their wavefronts are few, and the queue's polling costs more)
+  const bool persist = !phased && (mode == 3 || (mode == 2 && !solid));
   A.queue = persist ? 1 : 0;
   int64_t begin = 0, obegin = 0, waves = 0;
   Control h;
