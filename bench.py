@@ -43,7 +43,7 @@ WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
 
 class ClockSampler:
     """SM clock and clock-event (throttle) reasons sampled DURING the timed region, through NVML -- the library
-    nvidia-smi itself reads -- from a thread of this process, every 50 ms.  (A `nvidia-smi -lms 20` child process was
+    nvidia-smi itself reads -- from a thread of this process (every 250 ms) and from the timed loop between two steps.  (A `nvidia-smi -lms 20` child process was
     measured to slow the phased schedule, which synchronises with the host once per round, from 35 to 47 ms per C2
     step: every one of its polls holds the driver for milliseconds.  Two NVML reads per sample do not.)  Falls back
     to `nvidia-smi -lms 200` when NVML cannot be opened."""
@@ -55,18 +55,28 @@ class ClockSampler:
         self.thread = None
         self.proc = None
         self.source = None
+        self.nv = None
+        self.handle = None
 
-    def _nvml_loop(self, nv, h):
+    def sample(self):
+        """One NVML sample (SM clock, clock-event reasons).  Also called by the timed loop itself between two steps,
+        outside the event-bracketed part: an NVML read can hold the driver while the phased schedule waits on it."""
+        if self.nv is None:
+            return
+        nv, h = self.nv, self.handle
         names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
                  nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"}
+        try:
+            self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+            r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+            self.reasons.update(n for bit, n in names.items() if r & bit)
+        except Exception:
+            pass
+
+    def _nvml_loop(self, nv, h):
         while not self.stop_flag.is_set():
-            try:
-                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
-                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
-                self.reasons.update(n for bit, n in names.items() if r & bit)
-            except Exception:
-                pass
-            self.stop_flag.wait(0.05)
+            self.sample()
+            self.stop_flag.wait(0.25)
 
     def start(self):
         try:
@@ -83,9 +93,10 @@ class ClockSampler:
             if h is None:
                 h = nv.nvmlDeviceGetHandleByIndex(self.index)
             self.mx.append(float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)))
+            self.nv, self.handle = nv, h
             self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
             self.thread.start()
-            self.source = "nvml, 50 ms"
+            self.source = "nvml: thread every 250 ms + once between timed steps"
             return
         except Exception:
             self.thread = None
@@ -265,13 +276,15 @@ def main():
         if sharded:
             ranks.combine_partial_cells(*ctx.device_tensors(), d_sites)
         ev[k][1].record(stream)
+        sampler.sample()
         clip_ms += ctx.stage_ms()["clip"]
         for name, v in ctx.phase_ms().items():
             phase_ms[name] += v
         launches += ctx.counters()["launches"]
     barrier()
     clocks = sampler.stop()
-    ms = sum(a.elapsed_time(b) for a, b in ev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = sum(step_ms)
     cnt = ctx.counters()
     stage = ctx.stage_ms()
     cells = ctx.cells
@@ -314,7 +327,7 @@ def main():
     achieved = kernel_flops / (kernel_ms * 1e-3) / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "ms_steps": [round(x, 3) for x in step_ms], "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
                    "parallelism": ("1 GPU" if world == 1 else (f"simplices in {world} contiguous blocks, sites replicated, one all-reduce of cell moments"
