@@ -43,10 +43,11 @@ WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
 
 class ClockSampler:
     """SM clock and clock-event (throttle) reasons sampled DURING the timed region, through NVML -- the library
-    nvidia-smi itself reads -- from a thread of this process (every 250 ms) and from the timed loop between two steps.  (A `nvidia-smi -lms 20` child process was
-    measured to slow the phased schedule, which synchronises with the host once per round, from 35 to 47 ms per C2
-    step: every one of its polls holds the driver for milliseconds.  Two NVML reads per sample do not.)  Falls back
-    to `nvidia-smi -lms 200` when NVML cannot be opened."""
+    nvidia-smi itself reads --, by the timed loop itself right after every step, outside the event brackets.  (A
+    `nvidia-smi -lms 20` child process was measured to slow the phased schedule, which synchronises with the host
+    once per round, from 35 to 47 ms per C2 step: every one of its polls holds the driver for milliseconds.)  Falls back to `nvidia-smi -lms 200` when NVML
+    cannot be opened.  (About one step in thirty still takes 10-40 ms longer on these shared hosts, with or without
+    any sampling: the schedule waits on the host some 25 times per step; `ms_steps` lists every step.)"""
 
     def __init__(self, index, uuid=None):
         self.index, self.uuid = index, uuid
@@ -73,11 +74,6 @@ class ClockSampler:
         except Exception:
             pass
 
-    def _nvml_loop(self, nv, h):
-        while not self.stop_flag.is_set():
-            self.sample()
-            self.stop_flag.wait(0.25)
-
     def start(self):
         try:
             import pynvml as nv
@@ -94,9 +90,8 @@ class ClockSampler:
                 h = nv.nvmlDeviceGetHandleByIndex(self.index)
             self.mx.append(float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)))
             self.nv, self.handle = nv, h
-            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
-            self.thread.start()
-            self.source = "nvml: thread every 250 ms + once between timed steps"
+            self.source = "nvml, read by the timed loop after every step (outside the event brackets)"
+            self.sample()
             return
         except Exception:
             self.thread = None
