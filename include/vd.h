@@ -117,7 +117,10 @@ typedef struct vd_options {
   int32_t seed_corners;   /* corners of every simplex whose nearest site seeds a pair (Alg. 2 line 4): 0 = default
                              (1: the first corner, as in Alg. 2); >= 3 / 4: all of them.  The result does not depend
                              on it; discovered pairs are cheaper than seeds (first_clip).  Meshed kinds.             */
-  int32_t reserved[2];
+  int32_t small_wave;     /* phased schedule: a wavefront of fewer pairs than this runs as ONE launch of the one-kernel
+                             form (the last wavefronts of a step hold a few hundred pairs: a dozen launches and three
+                             counter reads each otherwise); 0 = default (8192); < 0: never                          */
+  int32_t reserved[1];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */

@@ -46,7 +46,7 @@ class vd_options(ctypes.Structure):
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
                 ("near_clips", ctypes.c_int32), ("simplex_begin", ctypes.c_int32), ("simplex_end", ctypes.c_int32),
                 ("tail_pairs", ctypes.c_int32), ("first_clip", ctypes.c_int32),
-                ("seed_corners", ctypes.c_int32), ("reserved", ctypes.c_int32 * 2)]
+                ("seed_corners", ctypes.c_int32), ("small_wave", ctypes.c_int32), ("reserved", ctypes.c_int32 * 1)]
 
 
 class vd_counters(ctypes.Structure):

@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ l
 
 vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end);   // vd_phase.cu
 
+constexpr int kSmallWave = 8192;       // phased schedule: a wavefront smaller than this runs as one launch of the one-kernel form
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
@@ -307,8 +308,9 @@ vd_status stage_clip(vd_ctx* c) {
     if (end > c->pairCap) end = c->pairCap;
     if (oend > c->ovfCap) oend = c->ovfCap;
     if (end == begin && oend == obegin) break;   // "while L1 is not empty"
-    if (end > begin && phased) {
-      // phased mode: one small kernel per step of Alg. 3 over the whole wave (vd_phase.cu)
+    if (end > begin && phased && end - begin >= (c->opt.small_wave == 0 ? kSmallWave : c->opt.small_wave)) {
+      // phased mode: one small kernel per step of Alg. 3 over the whole wave (vd_phase.cu); a wave of a few thousand
+      // pairs (the last wavefronts) takes the branch below instead: one launch and one counter read, not a dozen
       const vd_status s = run_phases(c, A, hv, begin, end);
       if (s != VD_OK) return s;
       ++waves;

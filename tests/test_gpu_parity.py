@@ -47,8 +47,12 @@ def test_c1_full_parity():
     assert cnt["pieces"] == len(o.piece_simplex)
 
 
+# small_wave=-1: the step kernels of the phased schedule on every wavefront, however small (the replicas' wavefronts
+# are below the default threshold and would run the one-kernel form); tail_pairs=-1: rounds of k_ph_verify / k_ph_fix only
 @pytest.mark.parametrize("idx,opts", [(2, {}), (3, {}), (4, {}), (5, {}),
-                                      (3, dict(tail_pairs=-1)), (5, dict(tail_pairs=-1))])   # rounds of k_ph_verify / k_ph_fix only
+                                      (2, dict(small_wave=-1)), (3, dict(small_wave=-1)), (5, dict(small_wave=-1)),
+                                      (2, dict(small_wave=-1, tail_pairs=-1)), (3, dict(small_wave=-1, tail_pairs=-1)),
+                                      (5, dict(small_wave=-1, tail_pairs=-1))])
 def test_replica_parity(idx, opts):
     w = inputs.config(idx, "small")
     g, cnt, adj = _gpu(w, **opts)
@@ -60,7 +64,8 @@ def test_replica_parity(idx, opts):
 
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
                                   dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
-                                  dict(tail_pairs=-1), dict(tail_pairs=64), dict(first_clip=-1), dict(seed_corners=4), dict(seed_corners=2)])
+                                  dict(tail_pairs=-1, small_wave=-1), dict(tail_pairs=64, small_wave=-1), dict(first_clip=-1), dict(first_clip=-1, small_wave=-1),
+                                  dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -143,7 +148,7 @@ def test_schedules_agree():
         a, ca, _ = _gpu(w, persistent=0)
         assert ca["waves"] > 1
         for mode in (1, 3):
-            b, cb, _ = _gpu(w, persistent=mode)
+            b, cb, _ = _gpu(w, persistent=mode, small_wave=-1)
             assert cb["waves"] >= 1
             for f in ("nbr_off", "nbr", "piece_off", "piece_simplex", "vert_off", "vert_flags"):
                 assert np.array_equal(getattr(a, f), getattr(b, f)), f
@@ -205,10 +210,10 @@ def _box_parity(w, subset=None, **opts):
     return g, o, cnt
 
 
-@pytest.mark.parametrize("dim,n", [(2, 20000), (3, 6000)])
-def test_box_domain_parity(dim, n):
+@pytest.mark.parametrize("dim,n,opts", [(2, 20000, {}), (3, 6000, {}), (3, 6000, dict(small_wave=-1))])   # the last: the step kernels
+def test_box_domain_parity(dim, n, opts):
     w = inputs.box(dim, n, seed=31)
-    g, o, cnt = _box_parity(w)
+    g, o, cnt = _box_parity(w, **opts)
     assert cnt["pieces"] == n and (g.piece_simplex == 0).all()
     assert np.array_equal(g.piece_off, np.arange(n + 1))
 
@@ -289,6 +294,7 @@ def test_box_domain_wave_mode_and_lloyd():
 def test_support_calls_phase_times_counters_and_pinned_copy():
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
+        ctx.set_options(small_wave=-1)     # the step kernels also on this replica's small wavefronts
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         ph, cnt, st = ctx.phase_ms(), ctx.counters(), ctx.stage_ms()
