@@ -31,9 +31,9 @@ UNIT = "cells/s"
 # lanes x 2 flop at the maximum SM clock; no FP64 figure exists in MEASURED_PEAKS.json.
 FP64_LANES_PER_SM, SMS = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ph_fix, mean of the two launches in the committed
-# ncu --set full capture (profiles/r01_k_ph_fix_c2.md: 0.934 + 1.648 GB and 0.636 + 1.105 GB; the launches of a step
+# ncu --set full capture (profiles/r01_k_ph_fix_c2.md: 0.933 + 1.648 GB and 0.636 + 1.105 GB; the launches of a step
 # differ in size -- these two are the first two rounds of a step's largest wavefront); null for configs without a capture
-NCU_TRAFFIC_BYTES = {2: 0.5 * (0.934e9 + 1.648e9 + 0.636e9 + 1.105e9)}
+NCU_TRAFFIC_BYTES = {2: 0.5 * (0.933e9 + 1.648e9 + 0.636e9 + 1.105e9)}
 WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
              2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
              3: "C3: unit cube 48^3 x 6 tets (663,552), 1,000,000 clustered sites, seed 2",
