@@ -42,7 +42,9 @@
 // Pins (tests/test_oracle_pins.py): hand-worked closed forms in the unit square, regular grids,
 // sum of measures = |M|, first-moment identity, per-simplex conservation, neighbour symmetry,
 // corner equidistance + no nearer site by brute force, scipy/Qhull Voronoi volumes and Delaunay
-// neighbours for interior cells, tier A == tier B.
+// neighbours for interior cells, tier A == tier B; negative flags: every corner flagged ~b lies on the face T_a
+// really shares with T_b, every corner flagged ~m on a face no other simplex owns, and conversely every corner on a
+// face of T_a carries that face's flag (mesh topology recomputed in numpy) -- so no function here is "parity unpinned".
 
 #include <algorithm>
 #include <atomic>

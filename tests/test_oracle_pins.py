@@ -74,6 +74,81 @@ def _check_invariants(w, c, corner_sample=4000, seed=0):
                 continue  # two boundary faces of one tet share the label ~m: F is not countable from labels
             F = len(np.unique(fl))
             assert xyz.shape[0] == 2 * F - 4
+    # (7) negative flags name the face T_a really shares with that simplex / the domain boundary
+    assert _check_negative_flags(w, c) > 0
+
+
+def _check_negative_flags(w, c):
+    """Negative flags (Fig. 2a; 0-based restatement U3): a corner flagged ~b, b < m, lies on the face / edge
+    that T_a really SHARES with T_b (the two simplices have exactly d vertices in common, and the corner lies in
+    their affine hull); a corner flagged ~m lies on a face of T_a that no other simplex owns, i.e. on the domain
+    boundary.  The mesh topology used here is recomputed from `simplices` with numpy (sorted face rows, np.unique),
+    not taken from the oracle.  Returns how many (corner, flag) incidences were checked."""
+    simp = np.asarray(w.simplices)
+    m, nc = simp.shape
+    d = nc - 1                                   # vertices of a face (tets: 3) or an edge (triangles: 2)
+    tol = 1e-12 * w.diameter
+    V = w.verts
+    # owners of every face: face k of simplex a = its vertices without local corner k
+    faces = np.stack([np.sort(np.delete(simp, k, axis=1), axis=1) for k in range(nc)], axis=1)   # [m, nc, d]
+    _, inv, counts = np.unique(faces.reshape(-1, d), axis=0, return_inverse=True, return_counts=True)
+    owners = counts[inv].reshape(m, nc)          # 1 = boundary face, 2 = interior face
+    assert owners.max() <= 2
+
+    def dist_to_hull(x, P):
+        """distance from points x [k, dim] to the affine hull of P [k, d, dim] (a plane through 3 points in R^3, a
+        line through 2 points in R^2 or R^3)"""
+        e = P[:, 1:] - P[:, :1]
+        r = x - P[:, 0]
+        if d == 3:
+            n = np.cross(e[:, 0], e[:, 1])
+            return np.abs((r * n).sum(1)) / np.linalg.norm(n, axis=1)
+        t = (r * e[:, 0]).sum(1) / (e[:, 0] ** 2).sum(1)
+        return np.linalg.norm(r - t[:, None] * e[:, 0], axis=1)
+
+    a_of_corner = np.repeat(c.piece_simplex, np.diff(c.vert_off))
+    checked = 0
+    for col in range(c.vert_flags.shape[1]):
+        fl = c.vert_flags[:, col]
+        neg = np.nonzero(fl < 0)[0]
+        b = ~fl[neg]
+        a = a_of_corner[neg]
+        x = c.vert_xyz[neg]
+        inner = b < m
+        # ---- ~b, b < m: the face is shared, and the corner lies on it
+        ai, bi, xi = a[inner], b[inner], x[inner]
+        common = (simp[ai][:, :, None] == simp[bi][:, None, :]).any(2)          # [k, nc] vertex of a also in b
+        assert (common.sum(1) == d).all(), "flag ~b names a simplex that does not share a face with T_a"
+        P = V[simp[ai]][common].reshape(len(ai), d, V.shape[1])
+        assert dist_to_hull(xi, P).max(initial=0.0) <= tol, "corner flagged ~b is not on the face T_a shares with T_b"
+        checked += len(ai)
+        # ---- ~m: on a boundary face of T_a
+        ab, xb = a[~inner], x[~inner]
+        assert (b[~inner] == m).all()
+        best = np.full(len(ab), np.inf)
+        for k in range(nc):
+            on_bd = owners[ab, k] == 1
+            if on_bd.any():
+                P = V[np.delete(simp[ab[on_bd]], k, axis=1)]
+                best[on_bd] = np.minimum(best[on_bd], dist_to_hull(xb[on_bd], P))
+        assert best.max(initial=0.0) <= tol, "corner flagged ~m is not on the domain boundary"
+        checked += len(ab)
+    # ---- converse: a corner that lies on face k of T_a carries that face's flag (~other owner, or ~m)
+    order = np.argsort(inv, kind="stable")
+    flat_owner = np.repeat(np.arange(m), nc)[order]
+    other = np.full(m * nc, m, dtype=np.int64)
+    first = np.nonzero(np.diff(np.concatenate([[-1], inv[order]])) != 0)[0]
+    for s, cnt in zip(first, counts):
+        if cnt == 2:
+            other[order[s]], other[order[s + 1]] = flat_owner[s + 1], flat_owner[s]
+    other = other.reshape(m, nc)
+    for k in range(nc):
+        P = V[np.delete(simp[a_of_corner], k, axis=1)]
+        on = dist_to_hull(c.vert_xyz, P) <= tol
+        want = ~other[a_of_corner[on], k]
+        assert (c.vert_flags[on] == want[:, None]).any(1).all(), "corner on a face of T_a lacks that face's flag"
+        checked += int(on.sum())
+    return checked
 
 
 # ---------------------------------------------------------------------- golden hand cases
