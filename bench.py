@@ -6,7 +6,12 @@ one vd_compute) over one seeded synthetic workload.  `value` is device-timed wit
 resident in HBM (the context holds copies of sites and domain); `e2e` is the same metric through the C
 ABI with HOST buffers: vd_create + vd_set_domain + vd_compute + vd_cells_to_host + vd_destroy.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+The default run times ALL FIVE BASELINE.json configs in one process and prints ONE line: the top-level keys
+(value, ms_per_step, config, roofline, e2e, cpu_baseline) are those of the LARGEST config, C3 (most simplices,
+most pairs, longest step); `per_config` holds the same keys for C1, C2, C4, C5, and `c5_under_1s` states
+BASELINE.json's target for the 2M-site config.  --config K times only config K.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0|1..5] [--impl reference]
 
 N > 1 (torchrun): the path shards by simplex: rank r clips its contiguous block of M against the
 replicated sites, one NCCL all-reduce of per-cell (measure, moment) per step; value = n / max-over-ranks time.
@@ -30,10 +35,11 @@ UNIT = "cells/s"
 # plain FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64 FMA
 # lanes x 2 flop at the maximum SM clock; no FP64 figure exists in MEASURED_PEAKS.json.
 FP64_LANES_PER_SM, SMS = 64, 148
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ph_fix, mean of the two launches in the committed
-# ncu --set full capture (profiles/r01_k_ph_fix_c2.md: 0.933 + 1.648 GB and 0.636 + 1.105 GB; the launches of a step
-# differ in size -- these two are the first two rounds of a step's largest wavefront); null for configs without a capture
-NCU_TRAFFIC_BYTES = {2: 0.5 * (0.933e9 + 1.648e9 + 0.636e9 + 1.105e9)}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, read by kernel
+# name and config from the committed summary of the ncu --set full captures (never from a literal here); null when
+# that kernel / config has no capture
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
+TOP_CONFIG = 3
 WORKLOADS = {1: "C1: 2D unit square, 2 triangles, 2,000 uniform sites, seed 0",
              2: "C2: unit cube 20^3 x 6 tets (48,000), 100,000 uniform sites, seed 1",
              3: "C3: unit cube 48^3 x 6 tets (663,552), 1,000,000 clustered sites, seed 2",
@@ -125,21 +131,34 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.sm), "source": self.source}
 
 
-def algorithmic_flops(cnt, kind):
-    """8 flop per candidate distance (5 in 2D), 15 per search iteration,
-    per clip 2d flop x ~corners tested + 60 per new 3D corner (15 in 2D), 30 per fan tet of a piece.
-    Returned per step kernel of S4 (phased schedule) and in total."""
-    d3 = kind in (2, 4)
-    per_dist = 8 if kind not in (0, 3) else 5
-    per_clip = (6 * 12 + 60 * 4) if d3 else (4 * 6 + 15 * 2)
-    per_piece = 30 * (20 if d3 else 4)
-    pre, se = cnt.get("pre_clips", 0), cnt.get("search_evals", 0)
-    parts = {"init": per_clip * pre,
-             "verify": per_dist * (cnt["dist_evals"] - se),
-             "fix": per_dist * se + 15 * cnt["search_iters"] + per_clip * (cnt["clips"] - pre),
-             "finish": per_piece * cnt["pieces"],
-             "tail": 0}     # the tail kernel's tests and clips are counted under verify / fix (a few % of either)
-    return parts, sum(parts.values())
+def algorithmic_flops(c, kind):
+    """algorithmic flop = 8 D + 15 I + sum over clips (2d x corners tested + 60 x new corners) + 30 x fan
+    simplices, every term COUNTED by the kernels (D = site distance evaluations, 5 flop each in 2D; I = search
+    iterations; a new 2D corner is one 2 x 2 solve = 15 flop).  c = one counter block (a kernel's, or the totals)."""
+    flat = kind in (0, 3)
+    d = 2 if flat else 3
+    return ((5 if flat else 8) * c["dist_evals"] + 15 * c["search_iters"] + 2 * d * c["clip_corners"]
+            + (15 if kind in (0, 1, 3) else 60) * c["new_corners"] + 30 * c["fan_simplices"])
+
+
+def traffic_from_profiles(kernel, cfg):
+    """(dram bytes per launch, source) of `kernel` on config `cfg` from profiles/r02_dram_traffic.csv, else (None, None)."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            rows = [ln.strip().split(",") for ln in f if ln.strip() and not ln.startswith("#")]
+    except OSError:
+        return None, None
+    hdr, rows = rows[0], rows[1:]
+    col = {name: k for k, name in enumerate(hdr)}
+    for r in rows:
+        if r[col["config"]] == f"C{cfg}" and r[col["kernel"]] == kernel.split("<")[0].split(" ")[0]:
+            n = max(1, int(r[col["launches"]]))
+            return (float(r[col["dram_read_bytes"]]) + float(r[col["dram_write_bytes"]])) / n, r[col["source"]]
+    return None, None
+
+
+def oracle_tier(w):
+    return "A" if w.kind == 1 else "B"
 
 
 def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
@@ -147,7 +166,7 @@ def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
     cores on a bounded random sample of sites of the same workload."""
     from oracle import oracle
     rng = np.random.default_rng(seed)
-    tier = "A" if w.kind == 1 else "B"
+    tier = oracle_tier(w)
     k = min(w.n, 32)
     t0 = time.perf_counter()
     r = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, k, replace=False)), tier=tier)
@@ -163,13 +182,21 @@ def cpu_oracle_sample(w, seconds_target=15.0, seed=12345):
             "sample": f"{k} seeded-random sites of the workload, tier {tier}, {dt:.1f} s wall"}
 
 
+def config_dict(w, workload, world, sharded):
+    """The `config` object: the same for our arm and for the reference arm."""
+    return {"workload": workload, "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
+            "parallelism": ("1 GPU" if world == 1 else (f"simplices in {world} contiguous blocks, sites replicated, one all-reduce of cell moments"
+                                                       if sharded else "replicas only"))}
+
+
 def run_reference(args, w, workload):
-    """--impl reference: each step = the oracle on a bounded sample of sites."""
+    """--impl reference: each step = the oracle on a bounded sample of sites of the same workload."""
     from oracle import oracle
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    tier = "A" if w.kind == 1 else "B"
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    tier = oracle_tier(w)
     rng = np.random.default_rng(777)
     probe = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=np.sort(rng.choice(w.n, min(w.n, 16), replace=False)), tier=tier)
     t0 = time.perf_counter()
@@ -187,13 +214,138 @@ def run_reference(args, w, workload):
     total = sum(times)
     val = k * len(times) / total
     sample = f"{k} seeded-random sites per step, tier {tier}"
+    sharded = world > 1 and w.simplices is not None
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload, "sample": sample},
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True,
+        "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(w, workload, world, sharded),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": int(probe.threads_used), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def measure(w, workload, cfg, args, env, cpu_seconds):
+    """Time args.steps steps of the hot path on workload w (after args.warmup untimed ones); returns the keys of one
+    bench line.  env = (torch, dist, binding, ranks, rank, world, dev, stream, flush, sampler, fp64_meas)."""
+    torch, dist, binding, ranks, rank, world, dev, stream, flush, sampler, fp64_meas = env
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # inputs resident in HBM before the timed region
+    d_sites = torch.from_numpy(w.sites).to(dev)
+    d_verts = torch.from_numpy(w.verts).to(dev)
+    d_simp = torch.from_numpy(w.simplices).to(dev) if w.simplices is not None else None
+    ctx = binding.Context(d_sites)
+    ctx.set_stream(stream.cuda_stream)
+    # N > 1: the path shards by simplex (DESIGN.md 8): rank r clips its block of M against the replicated sites, one
+    # all-reduce of per-cell (measure, first moment) combines the partial cells -- inside the timed region.  Simple
+    # domains (one piece per cell) have nothing to partition: every rank runs its own replica.
+    sharded = world > 1 and w.simplices is not None
+    opts = {}
+    if sharded:
+        blk = ranks.simplex_blocks_balanced(w.sites, w.verts, w.simplices, world)[rank]   # about equal pairs per rank
+        opts = dict(simplex_begin=blk[0], simplex_end=blk[1])
+        ctx.set_options(**opts)
+    ctx.set_domain(d_verts, d_simp, w.kind)
+    buf = None
+    for _ in range(args.warmup):
+        ctx.compute()
+        if sharded:
+            buf = ranks.combine_partial_cells(ctx, buf)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    clip_ms, launches = 0.0, 0
+    phase_ms = {"init": 0.0, "verify": 0.0, "fix": 0.0, "finish": 0.0, "tail": 0.0}
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)            # L2 flush between timed iterations (not timed)
+        ev[k][0].record(stream)
+        ctx.compute()
+        if sharded:
+            ranks.combine_partial_cells(ctx, buf)
+        ev[k][1].record(stream)
+        sampler.sample()
+        clip_ms += ctx.stage_ms()["clip"]
+        for name, v in ctx.phase_ms().items():
+            phase_ms[name] += v
+        launches += ctx.counters()["launches"]
+    barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = sum(step_ms)
+    cnt = ctx.counters()
+    pcnt = ctx.phase_counters()
+    stage = ctx.stage_ms()
+    sizes = {"nonempty_cells": int(ctx.cells.n_nonempty), "pieces": int(ctx.cells.n_pieces), "corners": int(ctx.cells.n_verts),
+             "neighbour_entries": int(ctx.cells.n_nbrs)}
+    # sharded: the ranks together made ONE diagram of n cells per step; replicas: one each
+    value, ms = ranks.whole_job_rate(float(w.n * args.steps) / (world if sharded else 1), ms, dev)
+    # D_alg next to D_act (SURVEY 8d): one more, untimed, step with vd_options.count_alg
+    ctx.set_options(count_alg=1, **opts)
+    ctx.compute()
+    d_alg = ctx.counters()["alg_evals"]
+    ctx.destroy()
+
+    # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
+    barrier()
+    e2e_steps = max(2, min(args.steps, 5))
+    for k in range(e2e_steps + 1):
+        if k == 1:      # the first pass is warm-up: it page-locks the staging buffers and fills the memory pool
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+        c2 = binding.Context(w.sites)
+        c2.set_stream(stream.cuda_stream)
+        if sharded:
+            c2.set_options(**opts)
+        c2.set_domain(w.verts, w.simplices, w.kind)
+        c2.compute()
+        h = c2.to_host(pinned=True)
+        c2.destroy()
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
+                                            "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
+    h2d = w.sites.nbytes + w.verts.nbytes + (w.simplices.nbytes if w.simplices is not None else 0)
+    e2e_val, _ = ranks.whole_job_rate(float(w.n) / (world if sharded else 1), e2e_s * 1e3, dev)
+
+    flops = algorithmic_flops(cnt, w.kind)
+    sm_max = (sampler.mx and max(sampler.mx)) or 1965.0
+    peak = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    if sum(phase_ms.values()) > 0:
+        # phased schedule: the dominant kernel is the step kernel with the largest device time (CUDA events
+        # around every launch, inside the library, on the stream the kernels run on); its flop from ITS counters
+        top = max(phase_ms, key=phase_ms.get)
+        kernel, kernel_ms, kcnt = "k_ph_" + top, phase_ms[top] / args.steps, pcnt[top]
+    else:
+        kernel, kernel_ms, kcnt = "k_clip (S4+S5, one-kernel schedule)", clip_ms / args.steps, cnt
+    kernel_flops = algorithmic_flops(kcnt, w.kind)
+    achieved = kernel_flops / (kernel_ms * 1e-3) / 1e12
+    traffic, traffic_src = traffic_from_profiles(kernel, cfg)
+    out = {
+        "value": value, "unit": UNIT, "ms_per_step": ms / args.steps, "ms_steps": [round(x, 3) for x in step_ms],
+        "config": config_dict(w, workload, world, sharded), "result_sizes": sizes,
+        "nonempty_cells_per_s": value * sizes["nonempty_cells"] / w.n, "pairs_per_s": value * cnt["pairs"] / w.n,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(launches), "stage_ms": stage, "counters": cnt,
+        "per_cell": {"queries": cnt["queries"] / w.n, "d_act": cnt["dist_evals"] / w.n, "d_alg": d_alg / w.n,
+                     "d_act_over_d_alg": cnt["dist_evals"] / max(1, d_alg), "queries_per_pair": cnt["queries"] / max(1, cnt["pairs"]),
+                     "clips": cnt["clips"] / w.n, "pieces": cnt["pieces"] / w.n},
+        "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
+        "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
+                     "peak_measured": fp64_meas, "frac_of_measured": achieved / fp64_meas,
+                     "peak_measured_source": "vd_dfma_peak: 8 dependent DFMA chains per thread, SMs x 8 blocks x 256 threads, best of 3, this run",
+                     "algorithmic_flop_per_step": kernel_flops, "kernel_ms_per_step": kernel_ms,
+                     "kernel_counters": {k: kcnt[k] for k in ("dist_evals", "search_iters", "clip_corners", "new_corners", "fan_simplices", "clips", "queries")},
+                     "flop_formula": "8 D (5 in 2D) + 15 I + 2d clip_corners + 60 new_corners (15 on triangles) + 30 fan_simplices, all counted in the kernels",
+                     "share_of_step": kernel_ms * args.steps / ms,
+                     "s4_ms_per_step": clip_ms / args.steps, "s4_algorithmic_flop_per_step": flops},
+    }
+    if rank == 0 and not args.no_cpu_baseline and world == 1 and cpu_seconds > 0:
+        out["cpu_baseline"] = cpu_oracle_sample(w, cpu_seconds)
+    return out
 
 
 def main():
@@ -201,7 +353,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index, 1-based (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=0, help="0 (default): all five BASELINE.json configs, top-level = C3 (the largest); "
+                    "1..5: only that config")
     ap.add_argument("--box", type=int, default=0, help="instead of a BASELINE config: N white-noise sites in the unit cube, the cube itself "
                     "as a simple domain (VD_BOX_3D; the setting of the paper's Fig. 1 / Table VI)")
     ap.add_argument("--impl", default="ours")
@@ -209,8 +362,10 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
     from paper_2509_07175_b200 import inputs
-    w = inputs.box(3, args.box, seed=9) if args.box else inputs.config(args.config)
-    workload = f"whole cells of {args.box} uniform sites in the unit cube (VD_BOX_3D, paper Fig. 1 setting)" if args.box else WORKLOADS[args.config]
+    top = args.config if args.config else TOP_CONFIG
+    others = [] if (args.config or args.box) else [k for k in (1, 2, 4, 5)]
+    w = inputs.box(3, args.box, seed=9) if args.box else inputs.config(top)
+    workload = f"whole cells of {args.box} uniform sites in the unit cube (VD_BOX_3D, paper Fig. 1 setting)" if args.box else WORKLOADS[top]
     if args.impl == "reference":
         run_reference(args, w, workload)
         return
@@ -228,124 +383,32 @@ def main():
         dist.init_process_group("nccl")
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream()
-    # inputs resident in HBM before the timed region
-    d_sites = torch.from_numpy(w.sites).to(dev)
-    d_verts = torch.from_numpy(w.verts).to(dev)
-    d_simp = torch.from_numpy(w.simplices).to(dev) if w.simplices is not None else None
-    ctx = binding.Context(d_sites)
-    ctx.set_stream(stream.cuda_stream)
-    # N > 1: the path shards by simplex: rank r clips its block of M against the replicated sites, one
-    # all-reduce of per-cell (measure, first moment) combines the partial cells -- inside the timed region.  Simple
-    # domains (one piece per cell) have nothing to partition: every rank runs its own replica.
-    sharded = world > 1 and w.simplices is not None
-    if sharded:
-        blk = ranks.simplex_blocks_balanced(w.sites, w.verts, w.simplices, world)[rank]   # about equal pairs per rank
-        ctx.set_options(simplex_begin=blk[0], simplex_end=blk[1])
-    ctx.set_domain(d_verts, d_simp, w.kind)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     fp64_meas, _ = binding.fp64_peak(stream.cuda_stream)   # dependent-FMA-chain kernel (vd_dfma_peak), outside the timed region
-    for _ in range(args.warmup):
-        ctx.compute()
-        if sharded:
-            ranks.combine_partial_cells(*ctx.device_tensors(), d_sites)
     try:
         uuid = str(torch.cuda.get_device_properties(local).uuid)
     except Exception:
         uuid = None
     sampler = ClockSampler(local, uuid)
     sampler.start()
-    barrier()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    clip_ms, launches = 0.0, 0
-    phase_ms = {"init": 0.0, "verify": 0.0, "fix": 0.0, "finish": 0.0, "tail": 0.0}
-    for k in range(args.steps):
-        flush.fill_(k & 0xff)            # L2 flush between timed iterations (not timed)
-        ev[k][0].record(stream)
-        ctx.compute()
-        if sharded:
-            ranks.combine_partial_cells(*ctx.device_tensors(), d_sites)
-        ev[k][1].record(stream)
-        sampler.sample()
-        clip_ms += ctx.stage_ms()["clip"]
-        for name, v in ctx.phase_ms().items():
-            phase_ms[name] += v
-        launches += ctx.counters()["launches"]
-    barrier()
+    env = (torch, dist, binding, ranks, rank, world, dev, stream, flush, sampler, fp64_meas)
+    res = measure(w, workload, 0 if args.box else top, args, env, 15.0)
+    per_config = {}
+    for k in others:
+        wk = inputs.config(k)
+        per_config[f"C{k}"] = measure(wk, WORKLOADS[k], k, args, env, 4.0)
+        del wk
     clocks = sampler.stop()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    ms = sum(step_ms)
-    cnt = ctx.counters()
-    stage = ctx.stage_ms()
-    cells = ctx.cells
-    # sharded: the ranks together made ONE diagram of n cells per step; replicas: one each
-    value, ms = ranks.whole_job_rate(float(w.n * args.steps) / (world if sharded else 1), ms, dev)
-
-    # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
-    barrier()
-    e2e_steps = max(2, min(args.steps, 5))
-    d2h = 0
-    for k in range(e2e_steps + 1):
-        if k == 1:      # the first pass is warm-up: it page-locks the staging buffers and fills the memory pool
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-        c2 = binding.Context(w.sites)
-        c2.set_stream(stream.cuda_stream)
-        if sharded:
-            c2.set_options(simplex_begin=blk[0], simplex_end=blk[1])
-        c2.set_domain(w.verts, w.simplices, w.kind)
-        c2.compute()
-        h = c2.to_host(pinned=True)
-        c2.destroy()
-    torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
-    d2h = sum(getattr(h, f).nbytes for f in ("measure", "centroid", "nbr_off", "nbr", "piece_off", "piece_simplex",
-                                            "piece_measure", "vert_off", "vert_xyz", "vert_flags"))
-    h2d = w.sites.nbytes + w.verts.nbytes + (w.simplices.nbytes if w.simplices is not None else 0)
-    e2e_val, _ = ranks.whole_job_rate(float(w.n) / (world if sharded else 1), e2e_s * 1e3, dev)
-
-    parts, flops = algorithmic_flops(cnt, w.kind)
-    sm_max = clocks["sm_max_mhz"] or 1965.0
-    peak = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    if sum(phase_ms.values()) > 0:
-        # phased schedule: the dominant kernel is the step kernel with the largest device time (CUDA events
-        # around every launch, inside the library, on the stream the kernels run on)
-        top = max(phase_ms, key=phase_ms.get)
-        kernel, kernel_ms, kernel_flops = "k_ph_" + top, phase_ms[top] / args.steps, parts[top]
-    else:
-        kernel, kernel_ms, kernel_flops = "k_clip (S4+S5, one-kernel schedule)", clip_ms / args.steps, flops
-    achieved = kernel_flops / (kernel_ms * 1e-3) / 1e12
-    out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "ms_steps": [round(x, 3) for x in step_ms], "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload, "n_sites": w.n, "n_simplices": w.m, "l2": "flushed between timed steps (256 MiB fill)",
-                   "parallelism": ("1 GPU" if world == 1 else (f"simplices in {world} contiguous blocks, sites replicated, one all-reduce of cell moments"
-                                                              if sharded else "replicas only")),
-                   "nonempty_cells": int(cells.n_nonempty), "pieces": int(cells.n_pieces), "corners": int(cells.n_verts)},
-        "clocks": clocks,
-        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
-        "gpu_launches": int(launches),
-        "stage_ms": stage, "counters": cnt,
-        "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
-        "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
-                     "peak_measured": fp64_meas, "frac_of_measured": achieved / fp64_meas,
-                     "peak_measured_source": "vd_dfma_peak: 8 dependent DFMA chains per thread, 148 x 8 blocks x 256 threads, best of 3, this run",
-                     "algorithmic_flop_per_step": kernel_flops, "kernel_ms_per_step": kernel_ms,
-                     "share_of_step": kernel_ms * args.steps / ms,
-                     "s4_ms_per_step": clip_ms / args.steps, "s4_algorithmic_flop_per_step": flops},
-    }
-    ctx.destroy()
+    out = {"metric": METRIC, "value": res.pop("value"), "unit": res.pop("unit"), "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": res.pop("ms_per_step"), "higher_is_better": True,
+           "scaling": "strong" if (world > 1 and w.simplices is not None) else "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "clocks": clocks}
+    out.update(res)
+    if per_config:
+        out["per_config"] = per_config
+        out["c5_under_1s"] = bool(per_config["C5"]["ms_per_step"] < 1000.0)
+        out["gpu_launches"] = int(out["gpu_launches"] + sum(v["gpu_launches"] for v in per_config.values()))
     if rank == 0:
-        if not args.no_cpu_baseline and world == 1:
-            out["cpu_baseline"] = cpu_oracle_sample(w)
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -33,11 +33,12 @@ typedef enum {
   VD_E_ARG = 1,        /* null pointer, n < 1, m < 1, bad kind                                   */
   VD_E_DIM = 2,        /* dim not in {2,3} or kind / dim mismatch                                */
   VD_E_STATE = 3,      /* vd_compute before vd_set_domain, vd_cells_to_host before vd_compute    */
-  VD_E_INPUT = 4,      /* NaN/Inf, index out of range, zero-measure simplex, non-manifold face   */
+  VD_E_INPUT = 4,      /* NaN/Inf, duplicate sites, index out of range, zero-measure simplex,
+                          non-manifold face, eta below the largest weight                        */
   VD_E_CUDA = 5,       /* no device, or a CUDA runtime error                                     */
   VD_E_NOMEM = 6,
   VD_E_CAPACITY = 7,   /* a piece outgrew every capacity tier (see vd_options)                   */
-  VD_E_NOCONVERGE = 8  /* an iteration cap was hit (degenerate input: duplicate sites, ...)      */
+  VD_E_NOCONVERGE = 8  /* an iteration cap was hit (degenerate input)                            */
 } vd_status;
 
 /* Domain kinds.  dim == 2 <=> VD_TRI_2D, VD_BOX_2D;  dim == 3 <=> VD_TRI_SURFACE, VD_TET_3D, VD_BOX_3D. */
@@ -120,7 +121,26 @@ typedef struct vd_options {
   int32_t small_wave;     /* phased schedule: a wavefront of fewer pairs than this runs as ONE launch of the one-kernel
                              form (the last wavefronts of a step hold a few hundred pairs: a dozen launches and three
                              counter reads each otherwise); 0 = default (8192); < 0: never                          */
-  int32_t reserved[1];
+  int32_t step_out;       /* improved bisector search of section VI-A: before the search on a segment p_s p_t
+                             longer than 2 delta_i (delta_i = half the distance from v_i to its nearest other site, computed
+                             for every site by S1b), step out from p_s: g = p_s + lambda delta_i dir, while N_g = v_i, then
+                             search on p_s g.  0 (default): off (witness points keep segments short, U7);
+                             1: lambda = 2, 3, 4, ... as printed;  2: lambda doubles.  Same result either way.     */
+  int32_t dissolve;       /* Alg. 5 lines 2-6, VD_TET_3D on a CONVEX mesh only: sites whose cell does
+                             not reach the domain boundary (empty restricted cell on the boundary triangles, site inside M)
+                             get their WHOLE cell as one piece (piece_simplex = m, no simplex flags) from the whole-cell
+                             kernel against the bounding box; the other (boundary) cells are clipped tet by tet as usual.
+                             0 (default): every cell as per-simplex pieces.  VD_E_ARG when the mesh is not convex.        */
+  int32_t fp32_filter;    /* 1: candidate sites are first tested in fp32 (16-byte records, an error bound on the squared
+                             distance), fp64 only for the survivors -- the paper's GPU runs are fp32.  Decisions
+                             and results stay fp64-exact.  0 (default): fp64 throughout.  3D kinds, plain index.           */
+  int32_t count_alg;      /* 1: also count D_alg (vd_counters.alg_evals): after every nearest-site query the sites of the
+                             grid cells that meet the ball (q, |q - N_q|) -- the least an exact grid search must examine
+                             (SURVEY 8d).  Slower; for measurement runs.                                                   */
+  int32_t reuse_nbrs;     /* vd_lloyd, whole-cell kinds: 0 / 1 (default): iteration k+1 clips every cell first by the bisectors
+                             of its neighbours of iteration k instead of looking up the nearest sites again;
+                             < 0: off                                                                                      */
+  int32_t reserved[3];
 } vd_options;
 
 /* Work counters of the last vd_compute (always collected; a few atomics per pair). */
@@ -137,14 +157,30 @@ typedef struct vd_counters {
   int64_t launches;       /* kernels this library launched inside the last vd_compute               */
   int64_t row_evals;      /* grid rows examined by those queries (index efficiency)                    */
   int64_t search_evals;   /* the part of dist_evals spent inside bisector searches                     */
-  int64_t pre_clips;      /* the part of clips done by nearest-site bisectors (vd_options.near_clips)  */
-  int64_t reserved[3];
+  int64_t pre_clips;      /* the part of clips done without a search (discovery tuple, nearest sites)  */
+  int64_t clip_corners;   /* corners side-tested by those clips (2d flop each)              */
+  int64_t new_corners;    /* corners created by those clips (one 3 x 3 solve each in 3D)               */
+  int64_t fan_simplices;  /* fan tetrahedra / triangles summed for measures and moments (S6 input)     */
+  int64_t alg_evals;      /* D_alg (vd_options.count_alg), else 0                                      */
+  int64_t syncs;          /* host waits on the stream inside the last vd_compute                       */
+  int64_t step_probes;    /* step-out probes of section VI-A (vd_options.step_out)                     */
+  int64_t reserved[2];
 } vd_counters;
 
 /* vd_create: copy n sites of dimension dim (row-major [n][dim], fp64).  Builds nothing heavy: the
  * site index (line 1 of Alg. 2/4/5) is built inside vd_compute.
  * Errors: VD_E_ARG, VD_E_DIM, VD_E_INPUT (non-finite coordinate), VD_E_CUDA, VD_E_NOMEM. */
 vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out);
+
+/* vd_create_weighted: sites with weights w_i -- the POWER diagram (section VII-C): cell i =
+ * { x : |x - v_i|^2 - w_i <= |x - v_j|^2 - w_j for all j }.  The paper lifts every site to p_i = (v_i, sqrt(eta - w_i))
+ * in R^(d+1), eta >= max w, and restricts the Voronoi diagram of the lifted sites to the domain at height 0
+ * (P:L465-471); the library does exactly that on the device: dim 2 -> lifted 3-D sites, the 2D triangle domain
+ * becomes a flat surface (results stay 2-D: centroids and corners [..][2]); dim 3 -> lifted 4-D sites, whose fourth
+ * coordinate enters every squared distance as the additive term eta - w_i (tets and boxes).
+ * weights [n] fp64, host or device.  eta: NaN = the smallest admissible value max_i w_i (advised).
+ * Errors: as vd_create; VD_E_INPUT when eta < max w or a weight is not finite.  Box kind in 2D: VD_E_DIM. */
+vd_status vd_create_weighted(const double* sites, const double* weights, int64_t n, int dim, double eta, vd_ctx** out);
 
 /* vd_update_sites: replace the coordinates of the n sites (same n, dim) -- for Lloyd iterations
  * (P:L483-492).  Same errors as vd_create. */
@@ -194,6 +230,12 @@ vd_status vd_get_stage_ms(const vd_ctx* ctx, double out_ms[5]);
  * schedule ran. */
 vd_status vd_get_phase_ms(const vd_ctx* ctx, double out_ms[5]);
 
+/* The work counters of the last vd_compute split by the kernel that did the work: which = 0 k_ph_init, 1 k_ph_verify,
+ * 2 k_ph_fix, 3 k_ph_finish, 4 k_ph_tail, 5 every other kernel (one-kernel schedule, seeds).  Only the fields counted
+ * inside kernels are filled (pairs .. step_probes); they add up to vd_get_counters.  bench.py derives each step kernel's
+ * algorithmic flop from them. */
+vd_status vd_get_phase_counters(const vd_ctx* ctx, int which, vd_counters* out);
+
 /* Copy the last result into caller HOST buffers (any may be NULL to skip).  Sizes are those of
  * vd_cells.  Synchronises the context's stream. */
 vd_status vd_cells_to_host(vd_ctx* ctx, double* measure, double* centroid, int64_t* nbr_off, int32_t* nbr,
@@ -203,6 +245,14 @@ vd_status vd_cells_to_host(vd_ctx* ctx, double* measure, double* centroid, int64
 /* Nearest site N_q of nq query points [nq][dim] through the site index (built on demand):
  * out_index[q] = argmin_j |q - v_j|, ties to the lowest id.  queries / out_index: host or device. */
 vd_status vd_nearest(vd_ctx* ctx, const double* queries, int64_t nq, int32_t* out_index);
+
+/* Sharded runs (vd_options.simplex_begin / simplex_end): vd_partial_moments writes, for every cell of
+ * the last vd_compute, (measure, measure x centroid) = 1 + dim doubles per site into out [n][1 + dim] (DEVICE pointer,
+ * caller-owned) -- the additive quantities the ranks sum with one all-reduce; vd_finish_centroids takes the summed
+ * array back and rewrites the context's measure / centroid arrays from it (centroid = moment / measure; the site
+ * itself for an empty cell).  Both run as kernels on the context's stream and do not synchronise. */
+vd_status vd_partial_moments(vd_ctx* ctx, double* out_sums);
+vd_status vd_finish_centroids(vd_ctx* ctx, const double* sums);
 
 /* Simplex adjacency derived by vd_set_domain, [m][3 or 4] int32: adj[a][k] = simplex across the
  * edge/face opposite local corner k, or m on the domain boundary.  out: host or device. */

@@ -53,9 +53,9 @@ def _load():
     if _lib is None:
         build()
         _lib = ctypes.CDLL(_LIB)
-        _lib.vdo_compute.restype = ctypes.c_int
-        _lib.vdo_compute.argtypes = [
-            ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
+        _lib.vdo_compute_w.restype = ctypes.c_int
+        _lib.vdo_compute_w.argtypes = [
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
             ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.POINTER(_Result))]
         _lib.vdo_free.restype = None
@@ -101,11 +101,12 @@ def _arr(ptr, count, dtype, shape=None):
     return out.reshape(shape) if shape is not None else out
 
 
-def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0) -> Cells:
+def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0, weights=None) -> Cells:
     """Clipped / restricted Voronoi cells by the definition (Eq. 1).
 
     tier 'A' = literal (all j != i); 'B' = two-phase (box facets, then simplices); see the
-    header of vd_oracle.cpp.  subset = site ids to compute (default all).
+    header of vd_oracle.cpp.  subset = site ids to compute (default all).  weights [n]: the power diagram
+    (section VII-C) instead of the Voronoi diagram.
     """
     lib = _load()
     sites = np.ascontiguousarray(sites, dtype=np.float64)
@@ -124,7 +125,10 @@ def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0) -> 
         sp, ns = None, 0
         ids = np.arange(n, dtype=np.int64)
     res = ctypes.POINTER(_Result)()
-    rc = lib.vdo_compute(sites.ctypes.data, n, dim, verts.ctypes.data, nv, simplices.ctypes.data if simplices.size else None, m,
+    if weights is not None:
+        weights = np.ascontiguousarray(weights, dtype=np.float64)
+        assert weights.shape == (n,)
+    rc = lib.vdo_compute_w(sites.ctypes.data, weights.ctypes.data if weights is not None else None, n, dim, verts.ctypes.data, nv, simplices.ctypes.data if simplices.size else None, m,
                          int(kind), sp, ns, 1 if tier == "B" else 0, int(threads), ctypes.byref(res))
     if rc != 0:
         raise RuntimeError(f"vdo_compute failed with status {rc}")

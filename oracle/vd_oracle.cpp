@@ -96,6 +96,16 @@ static HalfSpace bisector(const V3& vi, const V3& vj, int j) {
   return H;
 }
 
+// Power diagram (section VII-C; Aurenhammer's power cell): the half-space of
+//   |x - v_i|^2 - w_i <= |x - v_j|^2 - w_j   <=>   (v_j - v_i).(x - v_i) <= 1/2 |v_j - v_i|^2 + 1/2 (w_i - w_j).
+// (With p = (v, sqrt(eta - w)) in R^(d+1) and x at height 0, |x - p_i|^2 = |x - v_i|^2 + eta - w_i: the paper's lifted
+// restricted Voronoi diagram is this set, whatever eta.)
+static HalfSpace power_bisector(const V3& vi, real wi, const V3& vj, real wj, int j) {
+  HalfSpace H = bisector(vi, vj, j);
+  H.h = H.h + 0.5 * (wi - wj);
+  return H;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Convex polygon (2D domain or a planar polygon in R^3): ordered corners + one label per edge.
 // Edge k runs from corner k to corner k+1 (cyclic).
@@ -424,6 +434,10 @@ struct Problem {
   Domain D;
   int64_t n;
   std::vector<V3> sites;
+  std::vector<real> w;   // weights (power diagram); empty = the ordinary Voronoi diagram
+  HalfSpace half_space(int64_t i, int64_t j) const {
+    return w.empty() ? bisector(sites[i], sites[j], (int)j) : power_bisector(sites[i], w[i], sites[j], w[j], (int)j);
+  }
 };
 
 // One cell, tier A: T_a clipped by every H_ij, j != i, in index order (the literal definition).
@@ -435,7 +449,7 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
   V3 mom = {0, 0, 0};
   std::vector<HalfSpace> HS;
   if (planes) {
-    for (size_t k = 0; k < planes->size(); ++k) HS.push_back(bisector(vi, Pb.sites[(*planes)[k]], (*planes)[k]));
+    for (size_t k = 0; k < planes->size(); ++k) HS.push_back(Pb.half_space(i, (*planes)[k]));
   }
   for (int64_t a = 0; a < D.m; ++a) {
     PieceOut po;
@@ -447,7 +461,7 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
         for (size_t k = 0; k < HS.size() && !G.empty(); ++k) clip_polyhedron(G, HS[k]);
       } else {
         for (int64_t j = 0; j < Pb.n && !G.empty(); ++j)
-          if (j != i) clip_polyhedron(G, bisector(vi, Pb.sites[j], (int)j));
+          if (j != i) clip_polyhedron(G, Pb.half_space(i, j));
       }
       ok = !G.empty() && finish_polyhedron(G, (int32_t)a, po);
     } else {
@@ -463,7 +477,7 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
         for (size_t k = 0; k < HS.size() && !G.empty(); ++k) clip_polygon(G, HS[k]);
       } else {
         for (int64_t j = 0; j < Pb.n && !G.empty(); ++j)
-          if (j != i) clip_polygon(G, bisector(vi, Pb.sites[j], (int)j));
+          if (j != i) clip_polygon(G, Pb.half_space(i, j));
       }
       ok = !G.empty() && finish_polygon(G, D.kind, (int32_t)a, po);
     }
@@ -488,7 +502,7 @@ static bool facet_sites(const Problem& Pb, int64_t i, const V3& lo, const V3& hi
   if (Pb.D.dim == 3) {
     Polyhedron G = box_polyhedron(lo, hi);
     for (int64_t j = 0; j < Pb.n && !G.empty(); ++j)
-      if (j != i) clip_polyhedron(G, bisector(vi, Pb.sites[j], (int)j));
+      if (j != i) clip_polyhedron(G, Pb.half_space(i, j));
     if (G.empty()) return false;
     for (size_t f = 0; f < G.L.size(); ++f)
       if (G.L[f] >= 0) F.push_back(G.L[f]);
@@ -497,7 +511,7 @@ static bool facet_sites(const Problem& Pb, int64_t i, const V3& lo, const V3& hi
     G.P = {{lo.x, lo.y, 0}, {hi.x, lo.y, 0}, {hi.x, hi.y, 0}, {lo.x, hi.y, 0}};
     G.L = {LABEL_BOX, LABEL_BOX, LABEL_BOX, LABEL_BOX};
     for (int64_t j = 0; j < Pb.n && !G.empty(); ++j)
-      if (j != i) clip_polygon(G, bisector(vi, Pb.sites[j], (int)j));
+      if (j != i) clip_polygon(G, Pb.half_space(i, j));
     if (G.empty()) return false;
     for (size_t f = 0; f < G.L.size(); ++f)
       if (G.L[f] >= 0) F.push_back(G.L[f]);
@@ -541,9 +555,10 @@ void vdo_free(vdo_result* r) {
 // sites [n][dim], verts [nv][dim], simplices [m][dim+1 or 3], kind as include/vd.h.
 // subset: site ids to compute (NULL -> all n).  tier: 0 = A (literal), 1 = B (two-phase).
 // Returns 0 on success; 1 bad argument; 4 bad input (non-manifold face, index out of range).
-int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, int64_t nv,
-                const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
-                int tier, int nthreads, vdo_result** out) {
+// weights: NULL = Voronoi diagram; else [n] weights of the power diagram (section VII-C).
+int vdo_compute_w(const double* sites, const double* weights, int64_t n, int dim, const double* verts, int64_t nv,
+                  const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
+                  int tier, int nthreads, vdo_result** out) {
   const bool box = kind == KIND_BOX_2D || kind == KIND_BOX_3D;
   if (!sites || !verts || (!simplices && !box) || !out || n < 1 || m < 1 || nv < 1) return 1;
   if (!(((kind == KIND_TRI_2D || kind == KIND_BOX_2D) && dim == 2) || ((kind == KIND_TRI_SURFACE || kind == KIND_TET_3D || kind == KIND_BOX_3D) && dim == 3))) return 1;
@@ -553,6 +568,7 @@ int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, in
   Pb.n = n;
   Pb.sites.resize(n);
   for (int64_t i = 0; i < n; ++i) Pb.sites[i] = load_point(sites + i * dim, dim);
+  if (weights) Pb.w.assign(weights, weights + n);
   Domain& D = Pb.D;
   D.kind = kind; D.dim = dim; D.nc = box ? 0 : ((kind == KIND_TET_3D) ? 4 : 3); D.nv = nv; D.m = m;
   D.verts.resize(nv);
@@ -646,6 +662,12 @@ int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, in
   R->vert_off[ip] = iv;
   *out = R;
   return 0;
+}
+
+int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, int64_t nv,
+                const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
+                int tier, int nthreads, vdo_result** out) {
+  return vdo_compute_w(sites, NULL, n, dim, verts, nv, simplices, m, kind, subset, n_subset, tier, nthreads, out);
 }
 
 }  // extern "C"

@@ -17,8 +17,8 @@ from . import build as _build
 VD_TRI_2D, VD_TRI_SURFACE, VD_TET_3D, VD_BOX_2D, VD_BOX_3D = 0, 1, 2, 3, 4
 STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_INPUT", 5: "VD_E_CUDA",
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
-EXPORTS = ["vd_create", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
-           "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_get_phase_ms", "vd_cells_to_host",
+EXPORTS = ["vd_create", "vd_create_weighted", "vd_partial_moments", "vd_finish_centroids", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
+           "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_get_phase_ms", "vd_get_phase_counters", "vd_cells_to_host",
            "vd_nearest", "vd_get_adjacency", "vd_dfma_peak", "vd_last_error", "vd_version"]
 
 _LIB_PATH = _build.lib_path()
@@ -46,12 +46,15 @@ class vd_options(ctypes.Structure):
                 ("persistent", ctypes.c_int32), ("pair_capacity", ctypes.c_int64), ("vert_capacity", ctypes.c_int64),
                 ("near_clips", ctypes.c_int32), ("simplex_begin", ctypes.c_int32), ("simplex_end", ctypes.c_int32),
                 ("tail_pairs", ctypes.c_int32), ("first_clip", ctypes.c_int32),
-                ("seed_corners", ctypes.c_int32), ("small_wave", ctypes.c_int32), ("reserved", ctypes.c_int32 * 1)]
+                ("seed_corners", ctypes.c_int32), ("small_wave", ctypes.c_int32), ("step_out", ctypes.c_int32),
+                ("dissolve", ctypes.c_int32), ("fp32_filter", ctypes.c_int32), ("count_alg", ctypes.c_int32),
+                ("reuse_nbrs", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
 
 
 class vd_counters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips",
-                                               "waves", "overflow_pairs", "reruns", "launches", "row_evals", "search_evals", "pre_clips")] + [("reserved", ctypes.c_int64 * 3)]
+                                               "waves", "overflow_pairs", "reruns", "launches", "row_evals", "search_evals", "pre_clips",
+                                               "clip_corners", "new_corners", "fan_simplices", "alg_evals", "syncs", "step_probes")] + [("reserved", ctypes.c_int64 * 2)]
 
 
 def load():
@@ -64,6 +67,9 @@ def load():
     lib = ctypes.CDLL(_LIB_PATH)
     vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
     lib.vd_create.argtypes = [vp, i64, ci, ctypes.POINTER(vp)]
+    lib.vd_create_weighted.argtypes = [vp, vp, i64, ci, ctypes.c_double, ctypes.POINTER(vp)]
+    lib.vd_partial_moments.argtypes = [vp, vp]
+    lib.vd_finish_centroids.argtypes = [vp, vp]
     lib.vd_update_sites.argtypes = [vp, vp]
     lib.vd_lloyd.argtypes = [vp, ci, ctypes.POINTER(vd_cells), vp]
     lib.vd_set_domain.argtypes = [vp, vp, i64, vp, i64, ci]
@@ -76,6 +82,7 @@ def load():
     lib.vd_get_counters.argtypes = [vp, ctypes.POINTER(vd_counters)]
     lib.vd_get_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     lib.vd_get_phase_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    lib.vd_get_phase_counters.argtypes = [vp, ci, ctypes.POINTER(vd_counters)]
     lib.vd_cells_to_host.argtypes = [vp] + [vp] * 10
     lib.vd_nearest.argtypes = [vp, vp, i64, vp]
     lib.vd_get_adjacency.argtypes = [vp, vp]
@@ -156,13 +163,20 @@ class HostCells:
 class Context:
     """vd_ctx wrapper: vd_create / vd_set_domain / vd_compute / vd_destroy."""
 
-    def __init__(self, sites, dim=None):
+    def __init__(self, sites, dim=None, weights=None, eta=None):
+        """weights given: vd_create_weighted (power diagram); eta None = the smallest admissible (max w)."""
         self._lib = load()
         self._h = ctypes.c_void_p()
         shape = tuple(sites.shape)
         self.n, self.dim = int(shape[0]), int(shape[1] if dim is None else dim)
         p, keep = _ptr(sites, np.float64)
-        self._check(self._lib.vd_create(p, self.n, self.dim, ctypes.byref(self._h)), create=True)
+        if weights is None:
+            self._check(self._lib.vd_create(p, self.n, self.dim, ctypes.byref(self._h)), create=True)
+        else:
+            pw, keepw = _ptr(weights, np.float64)
+            self._check(self._lib.vd_create_weighted(p, pw, self.n, self.dim, float("nan") if eta is None else float(eta),
+                                                     ctypes.byref(self._h)), create=True)
+        self._callbacks = None
         self.cells = vd_cells()
         self.kind = None
         self.m = 0
@@ -177,6 +191,22 @@ class Context:
 
     def set_stream(self, cuda_stream: int):
         self._check(self._lib.vd_set_stream(self._h, ctypes.c_void_p(cuda_stream)))
+
+    def set_allocator(self, alloc, release):
+        """vd_set_allocator with Python callables alloc(nbytes, stream) -> device pointer (int), release(ptr)."""
+        A = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p)
+        R = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+        a = A(lambda nbytes, user, stream: alloc(int(nbytes), int(stream or 0)))
+        r = R(lambda ptr, user: release(int(ptr or 0)))
+        self._callbacks = (a, r)   # keep the thunks alive as long as the context
+        self._check(self._lib.vd_set_allocator(self._h, ctypes.cast(a, ctypes.c_void_p), ctypes.cast(r, ctypes.c_void_p), None))
+
+    def partial_moments(self, out_ptr: int):
+        """vd_partial_moments into a caller-owned device buffer [n][1 + dim] (e.g. a torch tensor's data_ptr())."""
+        self._check(self._lib.vd_partial_moments(self._h, ctypes.c_void_p(out_ptr)))
+
+    def finish_centroids(self, sums_ptr: int):
+        self._check(self._lib.vd_finish_centroids(self._h, ctypes.c_void_p(sums_ptr)))
 
     def set_options(self, **kw):
         o = vd_options()
@@ -229,6 +259,15 @@ class Context:
         c = vd_counters()
         self._check(self._lib.vd_get_counters(self._h, ctypes.byref(c)))
         return {k: int(getattr(c, k)) for k, _ in vd_counters._fields_ if k != "reserved"}
+
+    def phase_counters(self) -> dict:
+        """vd_get_phase_counters: {kernel: counters} for init / verify / fix / finish / tail / other."""
+        out = {}
+        for k, name in enumerate(("init", "verify", "fix", "finish", "tail", "other")):
+            c = vd_counters()
+            self._check(self._lib.vd_get_phase_counters(self._h, k, ctypes.byref(c)))
+            out[name] = {f: int(getattr(c, f)) for f, _ in vd_counters._fields_ if f != "reserved"}
+        return out
 
     def stage_ms(self):
         a = (ctypes.c_double * 5)()

@@ -11,6 +11,23 @@ namespace vd {
 
 unsigned long long g_launches = 0;
 
+int sm_count() {
+  static int cached[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 148; }
+  if (cached[dev] == 0) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v < 1) { cudaGetLastError(); v = 148; }
+    cached[dev] = v;
+  }
+  return cached[dev];
+}
+
+cudaError_t sync_stream(vd_ctx* c) {
+  c->syncs += 1;
+  return cudaStreamSynchronize(c->stream);
+}
+
 vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what) {
   if (e == cudaSuccess) return VD_OK;
   if (c) c->lastError = std::string(what) + ": " + cudaGetErrorString(e);
@@ -45,7 +62,7 @@ vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
   if (bytes < 256) bytes = 256;
   if (b.cap >= bytes) return VD_OK;
   // pending kernels may still use the old block
-  cudaStreamSynchronize(c->stream);
+  if (b.p) sync_stream(c);
   release(c, b);
   void* p = nullptr;
   if (c->allocFn) {
@@ -84,7 +101,7 @@ static vd_status upload_points(vd_ctx* c, const double* src, int64_t n, int dim,
   if (e != cudaSuccess) { release(c, tmp); return cuda_check(c, e, what); }
   cudaMemsetAsync(c->control.p, 0, sizeof(Control), c->stream);
   int blocks = (int)((n + kBlock - 1) / kBlock);
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
   VD_LAUNCH(k_pad3, blocks, kBlock, 0, c->stream)(tmp.as<double>(), n, dim, dst.as<double>(), &c->control.as<Control>()->err);
   Control h;
   e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
@@ -107,6 +124,59 @@ __global__ void __launch_bounds__(kBlock) k_move_sites(const double* __restrict_
 __global__ void __launch_bounds__(kBlock) k_unpad3(const double* __restrict__ in3, int64_t n, int dim, double* __restrict__ out) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     for (int a = 0; a < dim; ++a) out[i * dim + a] = in3[i * 3 + a];
+}
+
+// Power diagrams by lifting (section VII-C): p_i = (v_i, sqrt(eta - w_i)), eta >= max w.  Partial maxima
+// of the weights, then the lift itself.  dim 2: the lifted coordinate becomes z of the 3-wide site record; dim 3: the
+// fourth coordinate only ever enters a squared distance from the domain (height 0), as h_i^2 = eta - w_i: that additive
+// term is what is stored (siteW).
+__global__ void __launch_bounds__(kBlock) k_weight_max(const double* __restrict__ w, int64_t n, double* __restrict__ part, unsigned int* err) {
+  double mx = -1e300;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double v = w[i];
+    if (!(v == v) || fabs(v) > 1e150) atomicOr(err, ERR_WEIGHT);
+    mx = fmax(mx, v);
+  }
+  for (int off = kLanes / 2; off > 0; off >>= 1) mx = fmax(mx, __shfl_xor_sync(kFull, mx, off));
+  __shared__ double sm[kWarpsPerBlock];
+  if (lane_id() == 0) sm[threadIdx.x / kLanes] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < (int)blockDim.x / kLanes; ++k) mx = fmax(mx, sm[k]);
+    part[blockIdx.x] = mx;
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_lift(const double* __restrict__ w, int64_t n, int dim, const double* __restrict__ part, int nparts,
+                                                  double eta, double* __restrict__ sites3, double* __restrict__ siteW, unsigned int* err) {
+  double wmax = -1e300;
+  for (int k = 0; k < nparts; ++k) wmax = fmax(wmax, part[k]);
+  if (!(eta == eta)) eta = wmax;                    // NaN: the smallest admissible eta
+  if (eta < wmax) { if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(err, ERR_WEIGHT); return; }
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double h2 = eta - w[i];
+    if (dim == 2) sites3[i * 3 + 2] = sqrt(h2);
+    else siteW[i] = h2;
+  }
+}
+
+// Sharded runs: the additive per-cell quantities (measure, measure x centroid), and the way back (vd.h)
+__global__ void __launch_bounds__(kBlock) k_partial_moments(const double* __restrict__ measure, const double* __restrict__ centroid, int64_t n,
+                                                             int dim, double* __restrict__ out) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double ms = measure[i];
+    out[i * (dim + 1)] = ms;
+    for (int a = 0; a < dim; ++a) out[i * (dim + 1) + 1 + a] = ms * centroid[i * dim + a];
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_finish_centroids(const double* __restrict__ sums, const double* __restrict__ sites3, int64_t n, int dim,
+                                                              double* __restrict__ measure, double* __restrict__ centroid) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double ms = sums[i * (dim + 1)];
+    measure[i] = ms;
+    for (int a = 0; a < dim; ++a) centroid[i * dim + a] = ms > 0.0 ? sums[i * (dim + 1) + 1 + a] / ms : sites3[i * 3 + a];
+  }
 }
 
 static void set_default_options(vd_options& o) {
@@ -168,8 +238,55 @@ vd_status vd_create(const double* sites, int64_t n, int dim, vd_ctx** out) {
   return VD_OK;
 }
 
+vd_status vd_create_weighted(const double* sites, const double* weights, int64_t n, int dim, double eta, vd_ctx** out) {
+  if (!weights || !out) return VD_E_ARG;
+  vd_ctx* c = nullptr;
+  vd_status s = vd_create(sites, n, dim, &c);
+  if (s != VD_OK) return s;
+  c->weighted = true;
+  DevBuf w, part;
+  const int blocks = (int)((n + kBlock - 1) / kBlock) < 256 ? (int)((n + kBlock - 1) / kBlock) : 256;
+  if ((s = ensure(c, w, sizeof(double) * n)) || (s = ensure(c, part, sizeof(double) * 256)) ||
+      (dim == 3 && (s = ensure(c, c->siteW, sizeof(double) * n)))) { vd_destroy(c); return s; }
+  cudaError_t e = cudaMemcpyAsync(w.p, weights, sizeof(double) * n, cudaMemcpyDefault, c->stream);
+  cudaMemsetAsync(c->control.p, 0, sizeof(Control), c->stream);
+  unsigned int* err = &c->control.as<Control>()->err;
+  VD_LAUNCH(k_weight_max, blocks, kBlock, 0, c->stream)(w.as<double>(), n, part.as<double>(), err);
+  VD_LAUNCH(k_lift, blocks, kBlock, 0, c->stream)(w.as<double>(), n, dim, part.as<double>(), blocks, eta, c->sites.as<double>(),
+                                                  c->siteW.as<double>(), err);
+  Control h;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  release(c, w);
+  release(c, part);
+  if (e != cudaSuccess) { vd_destroy(c); return VD_E_CUDA; }
+  if (h.err & ERR_WEIGHT) { vd_destroy(c); return VD_E_INPUT; }
+  *out = c;
+  return VD_OK;
+}
+
+vd_status vd_partial_moments(vd_ctx* c, double* out_sums) {
+  if (!c || !out_sums) return VD_E_ARG;
+  if (!c->haveResult) { c->lastError = "vd_partial_moments before a successful vd_compute"; return VD_E_STATE; }
+  int blocks = (int)((c->n + kBlock - 1) / kBlock);
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+  VD_LAUNCH(k_partial_moments, blocks, kBlock, 0, c->stream)(c->oMeasure.as<double>(), c->oCentroid.as<double>(), c->n, c->dim, out_sums);
+  return cuda_check(c, cudaGetLastError(), "vd_partial_moments");
+}
+
+vd_status vd_finish_centroids(vd_ctx* c, const double* sums) {
+  if (!c || !sums) return VD_E_ARG;
+  if (!c->haveResult) { c->lastError = "vd_finish_centroids before a successful vd_compute"; return VD_E_STATE; }
+  int blocks = (int)((c->n + kBlock - 1) / kBlock);
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+  VD_LAUNCH(k_finish_centroids, blocks, kBlock, 0, c->stream)(sums, c->sites.as<double>(), c->n, c->dim, c->oMeasure.as<double>(),
+                                                              c->oCentroid.as<double>());
+  return cuda_check(c, cudaGetLastError(), "vd_finish_centroids");
+}
+
 vd_status vd_update_sites(vd_ctx* c, const double* sites) {
   if (!c || !sites) return VD_E_ARG;
+  if (c->weighted) { c->lastError = "vd_update_sites: a weighted context keeps its lifted sites (create a new one)"; return VD_E_STATE; }
   c->indexValid = false;
   c->haveResult = false;
   return upload_points(c, sites, c->n, c->dim, c->sites, "vd_update_sites");
@@ -180,6 +297,12 @@ vd_status vd_set_domain(vd_ctx* c, const double* verts, int64_t nv, const int32_
   if (!c || !verts || (!simplices && !box) || nv < 1 || m < 1) return VD_E_ARG;
   if (kind < VD_TRI_2D || kind > VD_BOX_3D) return VD_E_ARG;
   if ((kind == VD_TRI_2D || kind == VD_BOX_2D) != (c->dim == 2)) return VD_E_DIM;
+  if (c->weighted && (kind == VD_BOX_2D || kind == VD_TRI_SURFACE)) {
+    c->lastError = "vd_set_domain: weighted sites take VD_TRI_2D (dim 2) or VD_TET_3D / VD_BOX_3D (dim 3)";
+    return VD_E_DIM;
+  }
+  // weighted 2D sites were lifted to R^3 (vd_create_weighted): the triangles, at height 0, are a surface in R^3
+  if (c->weighted && kind == VD_TRI_2D) kind = VD_TRI_SURFACE;
   if (m > 0x3fffffff || nv > 0x7fffffff) return VD_E_ARG;
   if (box && (nv != 2 || m != 1)) return VD_E_ARG;
   c->haveDomain = false;
@@ -252,6 +375,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     }
   }
   memset(&c->counters, 0, sizeof(c->counters));
+  c->syncs = 0;
   const unsigned long long launches0 = g_launches;
   cudaStream_t st = c->stream;
   vd_status s;
@@ -276,6 +400,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
       c->counters.reruns += 1;
       continue;
     }
+    if (err & ERR_DUPLICATE) { c->lastError = "vd_compute: two sites have the same coordinates"; return VD_E_INPUT; }
     if (err & ERR_INPUT) { c->lastError = "vd_compute: non-finite site coordinate"; return VD_E_INPUT; }
     if (err & ERR_PIECE_CAP) { c->lastError = "vd_compute: a piece outgrew the large-capacity path"; return VD_E_CAPACITY; }
     if (err & (ERR_NOCONVERGE | ERR_TOPOLOGY)) {
@@ -289,7 +414,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   cudaEventRecord(c->ev[4], st);
   Control h;
   cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = sync_stream(c);
   if (e != cudaSuccess) return cuda_check(c, e, "vd_compute");
   c->hostControl = h;
   float ms = 0;
@@ -297,11 +422,16 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   cudaEventElapsedTime(&ms, c->ev[0], c->ev[4]);
   c->stageMs[4] = ms;
   const int64_t reruns = c->counters.reruns, waves = c->counters.waves;
-  c->counters.pairs = (int64_t)h.cnt.pairs; c->counters.pieces = (int64_t)h.cnt.pieces;
-  c->counters.queries = (int64_t)h.cnt.queries; c->counters.dist_evals = (int64_t)h.cnt.dist_evals;
-  c->counters.row_evals = (int64_t)h.cnt.rows;
-  c->counters.search_iters = (int64_t)h.cnt.search_iters; c->counters.clips = (int64_t)h.cnt.clips;
-  c->counters.search_evals = (int64_t)h.cnt.search_evals; c->counters.pre_clips = (int64_t)h.cnt.pre_clips;
+  auto fill = [](vd_counters& o, const Counters& k) {
+    o.pairs = (int64_t)k.pairs; o.pieces = (int64_t)k.pieces; o.queries = (int64_t)k.queries; o.dist_evals = (int64_t)k.dist_evals;
+    o.row_evals = (int64_t)k.rows; o.search_iters = (int64_t)k.search_iters; o.clips = (int64_t)k.clips;
+    o.search_evals = (int64_t)k.search_evals; o.pre_clips = (int64_t)k.pre_clips; o.clip_corners = (int64_t)k.clip_corners;
+    o.new_corners = (int64_t)k.new_corners; o.fan_simplices = (int64_t)k.fan_simplices; o.alg_evals = (int64_t)k.alg_evals;
+    o.step_probes = (int64_t)k.step_probes;
+  };
+  fill(c->counters, counters_total(h));
+  for (int k = 0; k < kCntKinds; ++k) { memset(&c->phaseCounters[k], 0, sizeof(vd_counters)); fill(c->phaseCounters[k], h.cnt[k]); }
+  c->counters.syncs = c->syncs;
   c->counters.overflow_pairs = (int64_t)h.ovfTail;
   c->counters.reruns = reruns; c->counters.waves = waves;
   c->counters.launches = (int64_t)(g_launches - launches0);
@@ -322,7 +452,7 @@ vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) 
   if (!c || !out || iterations < 0) return VD_E_ARG;
   vd_status s;
   int blocks = (int)((c->n + kBlock - 1) / kBlock);
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
   for (int it = 0; it < iterations; ++it) {
     if ((s = vd_compute(c, out))) return s;
     VD_LAUNCH(k_move_sites, blocks, kBlock, 0, c->stream)(c->oMeasure.as<double>(), c->oCentroid.as<double>(), c->n, c->dim,
@@ -393,6 +523,12 @@ vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
 vd_status vd_get_counters(const vd_ctx* c, vd_counters* out) {
   if (!c || !out) return VD_E_ARG;
   *out = c->counters;
+  return VD_OK;
+}
+
+vd_status vd_get_phase_counters(const vd_ctx* c, int which, vd_counters* out) {
+  if (!c || !out || which < 0 || which >= kCntKinds) return VD_E_ARG;
+  *out = c->phaseCounters[which];
   return VD_OK;
 }
 

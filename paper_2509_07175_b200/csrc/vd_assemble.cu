@@ -196,7 +196,7 @@ __global__ void k_totals(Control* ctl, const int64_t* pieceOff, const int64_t* v
 
 static int blocks_for(int64_t items, int perBlock) {
   int64_t b = (items + perBlock - 1) / perBlock;
-  if (b > 148 * 16) b = 148 * 16;
+  if (b > sm_count() * 16) b = sm_count() * 16;
   if (b < 1) b = 1;
   return (int)b;
 }
@@ -204,7 +204,7 @@ static int blocks_for(int64_t items, int perBlock) {
 vd_status stage_assemble(vd_ctx* c) {
   const int64_t n = c->n;
   const int64_t total = (int64_t)c->hostControl.pairTail;
-  const int64_t nPieces = (int64_t)c->hostControl.cnt.pieces;
+  const int64_t nPieces = (int64_t)counters_total(c->hostControl).pieces;
   const int64_t nVerts = (int64_t)c->hostControl.vertTail;
   const int64_t nRaw = (int64_t)c->hostControl.nbrTail;
   const int dim = c->dim, nfl = c->nfl;

@@ -21,19 +21,51 @@ struct QBatch {
   int item[kQB];        // caller's payload (corner index)
   int base[kLanes];     // per packed row: first site index minus first candidate index
   unsigned char qid[kLanes];
+  unsigned char flag[kQB];   // refined index: the query met a refined cell in the row pass
 };
 
 // Lanes 0..nq-1 have filled qx,qy,qz,best,bestId of their slot (and the warp has synchronised).  On
 // return best/bestId of every slot hold the nearest site among those closer than the incoming bound
 // (or, for a loose bound, some clearly nearer site: nearer_ok of nearest(), reading U17).
+//
+// Refined index (HV): the batched pass needs plain cells.  Two cases keep it: (a) the balls of ALL queries lie inside one
+// and the same refined cell (a piece inside a dense cluster: its corners are a few sub-cells apart) -- then the pass runs
+// on that cell's sub-grid, viewed as a grid of its own; (b) no row of a query's ball holds a refined cell (found in the
+// row pass from the prefix count of refined cells) -- then the top grid is plain for that query.  Every other query
+// takes the single-query path.
 template <bool HV>
-static __device__ __noinline__ void batch_nearest(const GridIndex& g, QBatch& B, int nq, QueryStats& st) {
+static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
   const int lane = lane_id();
+  const GridIndex* gp = &gTop;
+  bool checkRefined = false;
+  if (HV) {
+    checkRefined = true;
+    int c = -1;
+    bool ok = false;
+    int hx = 0, hy = 0, hz = 0;
+    if (lane < nq && B.best[lane] < 1e300) {
+      const double qx = B.qx[lane], qy = B.qy[lane], qz = B.qz[lane];
+      hx = cell_of(gTop, 0, qx); hy = cell_of(gTop, 1, qy); hz = cell_of(gTop, 2, qz);
+      c = (hz * gTop.G[1] + hy) * gTop.G[0] + hx;
+      ok = __ldg(&gTop.subOff[c]) >= 0 && ball_in_cell(gTop, hx, hy, hz, qx, qy, qz, sqrt(B.best[lane]));
+    }
+    const int c0 = shfl(c, 0);
+    if (__all_sync(kFull, lane >= nq || (ok && c == c0))) {
+      GridIndex& v = warp_view();
+      __syncwarp();
+      if (lane == 0) sub_view(gTop, hx, hy, hz, __ldg(&gTop.subOff[c]), v);
+      __syncwarp();
+      gp = &v;
+      checkRefined = false;
+    }
+  }
+  const GridIndex& g = *gp;
   int myRows = 0;
   bool loose = false;
+  if (lane < kQB) B.flag[lane] = 0;
   if (lane < nq) {
     const double b = B.best[lane];
-    if (HV || !(b < 1e300)) {
+    if (!(b < 1e300)) {
       loose = true;
     } else {
       const double r = sqrt(b);
@@ -68,6 +100,11 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& g, QBatch& B,
         const int rowBase = (z * g.G[1] + y) * g.G[0];
         s = __ldg(&g.cellStart[rowBase + B.x0[u]]);
         cnt = __ldg(&g.cellStart[rowBase + B.x1[u] + 1]) - s;
+        if (HV && checkRefined && cnt > kHeavy &&
+            __ldg(&g.heavyPrefix[rowBase + B.x1[u] + 1]) != __ldg(&g.heavyPrefix[rowBase + B.x0[u]])) {
+          cnt = 0;           // a refined cell in this row: the query goes to the single-query path
+          B.flag[u] = 1;
+        }
       }
     }
     const int pin = warp_incl_scan(cnt);
@@ -115,12 +152,25 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& g, QBatch& B,
       __syncwarp();
     }
   }
+  if (HV && checkRefined) {
+    __syncwarp();
+    const unsigned flagged = __ballot_sync(kFull, lane < nq && B.flag[lane] != 0);
+    st.queries -= (unsigned)__popc(flagged & ~looseMask);
+    looseMask |= flagged;
+  }
+  if (gTop.countAlg) {
+    // D_alg of the batched queries (the loose ones count inside nearest())
+    unsigned v = 0;
+    if (lane < nq && !((looseMask >> lane) & 1u)) v = ball_sites(gTop, B.qx[lane], B.qy[lane], B.qz[lane], B.best[lane]);
+    v = (unsigned)warp_sum((int)v);
+    extra_cnt_add(4, v);
+  }
   while (looseMask) {
     const int u = __ffs(looseMask) - 1;
     looseMask &= looseMask - 1;
     double best = B.best[u];
     int bestId = B.bestId[u];
-    nearest<HV>(g, B.qx[u], B.qy[u], B.qz[u], best, bestId, st, true);
+    nearest<HV>(gTop, B.qx[u], B.qy[u], B.qz[u], best, bestId, st, true);
     __syncwarp();
     if (lane == 0) { B.best[u] = best; B.bestId[u] = bestId; }
     __syncwarp();

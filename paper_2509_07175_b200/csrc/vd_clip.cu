@@ -100,6 +100,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   constexpr bool BOX = KIND == KIND_BOX_2D || KIND == KIND_BOX_3D;
   if constexpr (KIND == KIND_TET_3D || KIND == KIND_BOX_3D) {
     __shared__ Poly3<BIG ? P3B : P3, BIG ? C3B : C3> S[W];
@@ -222,8 +223,8 @@ vd_status stage_seed(vd_ctx* c) {
   }
   const ClipArgs A = make_args(c);
   const bool boxKind0 = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
-  if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, 148 * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
-  VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
+  if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+  VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
   const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
   const int64_t mLocal = A.aEnd - A.aBegin;
   if (!boxKind && mLocal > 0 && c->n >= 64 * mLocal) {
@@ -232,30 +233,30 @@ vd_status stage_seed(vd_ctx* c) {
     const int64_t total = mLocal * S;
     if ((s = ensure(c, c->seedPts, sizeof(double) * 3 * total))) return s;
     if ((s = ensure(c, c->seedNN, sizeof(int) * total))) return s;
-    VD_LAUNCH(k_sample_points, blocks_for(total, kBlock, 148 * 8), kBlock, 0, st)(A, c->nc, S, c->seedPts.as<double>());
+    VD_LAUNCH(k_sample_points, blocks_for(total, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, S, c->seedPts.as<double>());
     if ((s = stage_nearest_points(c, c->seedPts.as<double>(), total, c->seedNN.as<int>()))) return s;
-    VD_LAUNCH(k_seed_points, blocks_for(total, kBlock, 148 * 8), kBlock, 0, st)(A, S, c->seedPts.as<double>(), c->seedNN.as<int>());
+    VD_LAUNCH(k_seed_points, blocks_for(total, kBlock, sm_count() * 8), kBlock, 0, st)(A, S, c->seedPts.as<double>(), c->seedNN.as<int>());
   }
   if (boxKind) {
     double cv[8 * 3];
     cudaMemcpyAsync(cv, c->verts.p, sizeof(double) * 3 * c->nc, cudaMemcpyDeviceToHost, st);
-    cudaStreamSynchronize(st);
+    sync_stream(c);
     const double* lo = cv;
     const double* hi = cv + 3 * (c->nc - 1);
-    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, 148 * 8), kBlock, 0, st)(A, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2]);
+    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(A, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2]);
   }
   return cuda_check(c, cudaGetLastError(), "seed");
 }
 
 template <int KIND, bool HV>
 static void launch_fast(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, bool persist) {
-  const int blocks = persist ? 148 * 3 : blocks_for(e - b, kWarpsPerBlock, 148 * 6);
+  const int blocks = persist ? sm_count() * 3 : blocks_for(e - b, kWarpsPerBlock, sm_count() * 6);
   VD_LAUNCH((k_clip<KIND, false, HV>), blocks, kBlock, 0, c->stream)(A, nullptr, b, e, persist);
 }
 
 template <int KIND, bool HV>
 static void launch_big(vd_ctx* c, const ClipArgs& A, int64_t ob, int64_t oe) {
-  VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, 148 * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe, false);
+  VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, sm_count() * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe, false);
 }
 
 template <int KIND>
@@ -278,14 +279,14 @@ static cudaError_t read_control(vd_ctx* c, Control& h) {
   static_assert(sizeof(Control) <= 1024, "fits the page-locked staging block");
   Control* dst = c->pinned ? reinterpret_cast<Control*>(c->pinned) : &h;
   cudaError_t e = cudaMemcpyAsync(dst, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess) e = sync_stream(c);
   if (e == cudaSuccess && dst != &h) h = *dst;
   return e;
 }
 
 static void set_cursor(vd_ctx* c, int which, unsigned long long v) {
   cudaMemcpyAsync(&c->control.as<Control>()->fetch[which], &v, sizeof(v), cudaMemcpyHostToDevice, c->stream);
-  cudaStreamSynchronize(c->stream);   // v lives on the host stack
+  sync_stream(c);   // v lives on the host stack
 }
 
 vd_status stage_clip(vd_ctx* c) {
@@ -304,6 +305,7 @@ vd_status stage_clip(vd_ctx* c) {
   const bool hv = h.nHeavy > 0;         // refined cells exist: the kernels that know the second index level
   for (;;) {
     if (h.err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) break;   // caller grows the pools and reruns
+    if (h.err & (ERR_DUPLICATE | ERR_INPUT)) break;                   // bad sites (S1): nothing to clip
     int64_t end = (int64_t)h.pairTail, oend = (int64_t)h.ovfTail;
     if (end > c->pairCap) end = c->pairCap;
     if (oend > c->ovfCap) oend = c->ovfCap;

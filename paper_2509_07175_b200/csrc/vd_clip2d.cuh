@@ -42,6 +42,8 @@ __device__ __forceinline__ int apply_clip_2d(Poly2<K>& S, int p, int s, double n
   const int lane = lane_id();
   const int nc = S.nc;
   __syncwarp();
+  extra_cnt_add(0, (unsigned)nc);
+  extra_cnt_add(1, 2u);
   int rc = 0;
   if (lane == 0) {
     // outside run around p (P:L391's R_p for a loop): corners beyond the line, not known inside
@@ -299,6 +301,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     my += ar * (S.cy[0] + (uy + vy) * (1.0 / 3.0));
     mz += ar * (S.cz[0] + (uz + vz) * (1.0 / 3.0));
   }
+  extra_cnt_add(2, (unsigned)(nc - 2));
   if (area < 0) { area = -area; mx = -mx; my = -my; mz = -mz; }
   if (!(area > 0)) {
     if (lane == 0) A.pieces[pairIdx] = pc;

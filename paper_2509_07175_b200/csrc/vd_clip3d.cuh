@@ -101,6 +101,8 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
     if (L > P || nc - k + L > C) return 1;
     if (L >= k) {
+      extra_cnt_add(0, (unsigned)nc);
+      extra_cnt_add(1, (unsigned)L);
       const int base = __popc(b0 & lt) + 2 * __popc(b1 & lt);
       if (lane == 0) { S.pnx[N] = nx; S.pny[N] = ny; S.pnz[N] = nz; S.pd[N] = d; S.pflag[N] = j; }
       if (rem) S.remap[__popc(R & lt)] = (unsigned short)c;   // slot list: the e-th new corner takes the e-th removed slot
@@ -231,6 +233,8 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
   const int nSurv = nc - nRemoved;
   if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
   if (nSurv + L > C) return 1;
+  extra_cnt_add(0, (unsigned)nc);
+  extra_cnt_add(1, (unsigned)L);
   // (2b) where the new corners are: rim edge (a -> b) gives the corner (a, b, N), the solution of its three planes;
   // one lane per rim edge, while the removed corners are still in place for the fallback
   for (int e = lane; e < L; e += kLanes) {
@@ -375,7 +379,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
   __syncwarp();
   const double rx = S.cx[0], ry = S.cy[0], rz = S.cz[0];   // reference point of the fan: corner 0
   double vol = 0, mx = 0, my = 0, mz = 0;
-  int nnbr = 0;
+  int nnbr = 0, nlive = 0;
   for (int f0 = 0; f0 < np; f0 += kLanes) {
     const int f = f0 + lane;
     const bool live = f < np && S.pa[f] != 0xffff;
@@ -414,6 +418,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
     }
     const bool pos = live && S.pflag[f] >= 0;
     const unsigned pm = __ballot_sync(kFull, pos);
+    nlive += __popc(__ballot_sync(kFull, live));
     // the face flags travel in key[][] (free until the corners are ranked): flag, then witness
     if (pos) {
       const int slot = nnbr + __popc(pm & ((1u << lane) - 1u));
@@ -427,6 +432,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
     nnbr += __popc(pm);
   }
   vol = warp_sum(vol); mx = warp_sum(mx); my = warp_sum(my); mz = warp_sum(mz);
+  extra_cnt_add(2, (unsigned)(3 * nc - 2 * nlive));   // fan tetrahedra: every face of k corners gives k - 2; corners lie on 3 faces
   if (vol < 0) { vol = -vol; mx = -mx; my = -my; mz = -mz; }
   if (!(vol > 0)) {
 #ifdef VD_TRACE

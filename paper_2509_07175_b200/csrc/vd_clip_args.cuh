@@ -38,17 +38,24 @@ struct LocalCnt {
   unsigned pairs, pieces, search_iters, clips, search_evals, pre_clips;
 };
 
-__device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& st, const LocalCnt& lc) {
+__device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& st, const LocalCnt& lc, int kind = CNT_OTHER) {
   if (lane_id() == 0) {
-    atomicAdd(&ctl->cnt.pairs, (unsigned long long)lc.pairs);
-    atomicAdd(&ctl->cnt.pieces, (unsigned long long)lc.pieces);
-    atomicAdd(&ctl->cnt.search_iters, (unsigned long long)lc.search_iters);
-    atomicAdd(&ctl->cnt.clips, (unsigned long long)lc.clips);
-    if (lc.search_evals) atomicAdd(&ctl->cnt.search_evals, (unsigned long long)lc.search_evals);
-    if (lc.pre_clips) atomicAdd(&ctl->cnt.pre_clips, (unsigned long long)lc.pre_clips);
-    atomicAdd(&ctl->cnt.queries, (unsigned long long)st.queries);
-    atomicAdd(&ctl->cnt.dist_evals, (unsigned long long)st.dist_evals);
-    atomicAdd(&ctl->cnt.rows, (unsigned long long)st.rows);
+    Counters* cnt = &ctl->cnt[kind];
+    atomicAdd(&cnt->pairs, (unsigned long long)lc.pairs);
+    atomicAdd(&cnt->pieces, (unsigned long long)lc.pieces);
+    atomicAdd(&cnt->search_iters, (unsigned long long)lc.search_iters);
+    atomicAdd(&cnt->clips, (unsigned long long)lc.clips);
+    if (lc.search_evals) atomicAdd(&cnt->search_evals, (unsigned long long)lc.search_evals);
+    if (lc.pre_clips) atomicAdd(&cnt->pre_clips, (unsigned long long)lc.pre_clips);
+    atomicAdd(&cnt->queries, (unsigned long long)st.queries);
+    atomicAdd(&cnt->dist_evals, (unsigned long long)st.dist_evals);
+    atomicAdd(&cnt->rows, (unsigned long long)st.rows);
+    const unsigned* x = sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock];
+    if (x[0]) atomicAdd(&cnt->clip_corners, (unsigned long long)x[0]);
+    if (x[1]) atomicAdd(&cnt->new_corners, (unsigned long long)x[1]);
+    if (x[2]) atomicAdd(&cnt->fan_simplices, (unsigned long long)x[2]);
+    if (x[3]) atomicAdd(&cnt->step_probes, (unsigned long long)x[3]);
+    if (x[4]) atomicAdd(&cnt->alg_evals, (unsigned long long)x[4]);
   }
 }
 
@@ -213,22 +220,40 @@ static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, dou
 // only within rounding do not compete (1e-13 relative; 1e-9 when the site owns a flag of P: the flag rule of
 // P:L109-111, readings U6/U17).  Returns false, doing nothing, when the ball covers too many grid cells (q still
 // far from Omega_i): the caller then takes an ordinary step.  Coordinates are absolute.  Warp-uniform result.
-static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double qx, double qy, double qz, double r2, double psx,
+// Refined index (HV): the scan needs plain cells -- a ball inside one refined cell is scanned in that cell's sub-grid (viewed
+// as a grid of its own); a ball that touches a refined cell otherwise is declined.
+template <bool HV>
+static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, double qx, double qy, double qz, double r2, double psx,
                                                     double psy, double psz, double dis2, double tq, int i, int j, const int* flags,
                                                     int nflags, int maxCells, double& tbest, int& jbest, QueryStats& st) {
   __shared__ int sBaseT[kWarpsPerBlock][kLanes];
   const int lane = lane_id();
   int* base = sBaseT[(threadIdx.x / kLanes) % kWarpsPerBlock];
   const double r = sqrt(r2);
+  const GridIndex* gp = &gTop;
+  bool checkRefined = HV;
+  if (HV) {
+    const int hx = cell_of(gTop, 0, qx), hy = cell_of(gTop, 1, qy), hz = cell_of(gTop, 2, qz);
+    const int so = __ldg(&gTop.subOff[(hz * gTop.G[1] + hy) * gTop.G[0] + hx]);
+    if (so >= 0) {
+      if (!ball_in_cell(gTop, hx, hy, hz, qx, qy, qz, r)) return false;
+      GridIndex& v = warp_view();
+      __syncwarp();
+      if (lane == 0) sub_view(gTop, hx, hy, hz, so, v);
+      __syncwarp();
+      gp = &v;
+      checkRefined = false;
+    }
+  }
+  const GridIndex& g = *gp;
   const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
   const int y0 = cell_of(g, 1, qy - r - 1e-6 * g.h[1]), y1 = cell_of(g, 1, qy + r + 1e-6 * g.h[1]);
   const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
   const int ny = y1 - y0 + 1;
   const int nrows = ny * (z1 - z0 + 1);
   if (nrows > kLanes || nrows * (x1 - x0 + 1) > maxCells) return false;
-  st.queries += 1;
-  st.rows += (unsigned)nrows;
   int s = 0, cnt = 0;
+  bool refined = false;
   if (lane < nrows) {
     const int rz = lane / ny;
     const int y = y0 + (lane - rz * ny), z = z0 + rz;
@@ -241,9 +266,14 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double q
         const int rowBase = (z * g.G[1] + y) * g.G[0];
         s = __ldg(&g.cellStart[rowBase + xa]);
         cnt = __ldg(&g.cellStart[rowBase + xb + 1]) - s;
+        if (HV && checkRefined && cnt > kHeavy)
+          refined = __ldg(&g.heavyPrefix[rowBase + xb + 1]) != __ldg(&g.heavyPrefix[rowBase + xa]);
       }
     }
   }
+  if (HV && __any_sync(kFull, refined)) return false;
+  st.queries += 1;
+  st.rows += (unsigned)nrows;
   const int incl = warp_incl_scan(cnt);
   const int excl = incl - cnt;
   const int total = shfl(incl, kLanes - 1);
@@ -281,6 +311,7 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& g, double q
   }
   warp_argmin(tb, jb);
   if (closer(tb, jb, tbest, jbest)) { tbest = tb; jbest = jb; }
+  if (gTop.countAlg) extra_cnt_add(4, lane == 0 ? ball_sites(gTop, qx, qy, qz, r2) : 0u);   // the search needs every site of this ball
   return true;
 }
 
@@ -319,12 +350,12 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
-    if (!HV && ballCells > 0) {
+    if (ballCells > 0) {
       // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
       double tb = 2.0;
       int jb = 0x7fffffff;
       const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
-      if (scan_ball_min_t(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz, t, i, j, flags, nflags,
+      if (scan_ball_min_t<HV>(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz, t, i, j, flags, nflags,
                           ballCells, tb, jb, st)) {
         if (jb != 0x7fffffff) {
           j = jb;

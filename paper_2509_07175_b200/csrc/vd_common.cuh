@@ -29,7 +29,9 @@ enum {
   ERR_PIECE_CAP = 8,     // a piece outgrew the large-capacity path
   ERR_NOCONVERGE = 16,   // iteration cap
   ERR_TOPOLOGY = 32,     // clip produced a non-simple boundary loop
-  ERR_INPUT = 64         // zero-measure simplex / non-manifold face / non-finite coordinate
+  ERR_INPUT = 64,        // zero-measure simplex / non-manifold face / non-finite coordinate
+  ERR_DUPLICATE = 128,   // two sites with equal coordinates (found inside a bucket of the site index, S1)
+  ERR_WEIGHT = 256       // eta below the largest weight, or a non-finite weight (vd_create_weighted)
 };
 
 // Site index: uniform grid over the sites' bounding box; sites sorted by cell key so
@@ -48,6 +50,7 @@ struct GridIndex {
   const int* __restrict__ heavyPrefix;    // [G0*G1*G2 + 1] number of refined cells below a cell index (null: no second level)
   const int* __restrict__ subOff;         // [G0*G1*G2] (K << 26) | offset into subStart, or -1
   const int* __restrict__ subStart;
+  int countAlg;                           // vd_options.count_alg: queries also count D_alg (measurement runs)
 };
 
 constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
@@ -79,7 +82,11 @@ struct Piece {
 struct Counters {
   unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs, rows;
   unsigned long long search_evals, pre_clips;   // distance evaluations inside bisector searches; clips by nearest-site bisectors (U19)
+  unsigned long long clip_corners, new_corners, fan_simplices, alg_evals, step_probes;
 };
+
+// which kernel a counter block belongs to (vd_get_phase_counters): the step kernels of the phased schedule, the rest
+enum { CNT_INIT = 0, CNT_VERIFY = 1, CNT_FIX = 2, CNT_FINISH = 3, CNT_TAIL = 4, CNT_OTHER = 5, kCntKinds = 6 };
 
 __device__ __forceinline__ int lane_id() { return (int)(threadIdx.x % kLanes); }
 

@@ -90,7 +90,7 @@ vd_status stage_domain(vd_ctx* c) {
   if ((s = ensure(c, table, sizeof(int) * cap))) return s;
   cudaMemsetAsync(c->control.p, 0, sizeof(Control), st);
   int blocks = (int)((m * nc + kBlock - 1) / kBlock);
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
   VD_LAUNCH(k_validate, blocks, kBlock, 0, st)(c->verts.as<double>(), c->nv, c->simp.as<int>(), m, nc, c->kind,
                                                 &c->control.as<Control>()->err);
   VD_LAUNCH(k_fill_int, blocks, kBlock, 0, st)(table.as<int>(), (int64_t)cap, -1);

@@ -10,7 +10,7 @@
 
 namespace vd {
 
-constexpr int kBBoxBlocks = 296;   // 2 x 148 SMs
+constexpr int kBBoxBlocks = 512;   // partial boxes (a buffer size; the launch takes at most this many blocks)
 
 __global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restrict__ sites, int64_t n, double* __restrict__ part) {
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restric
 // One thread: final box, grid resolution ("each grid cell contains, on average, 2~3 / 3~4 sites":
 // average over all cells of the sites' box -- reading U9), header written to device memory.
 __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64_t n, double density, int64_t gridCap,
-                              const int* cellStart, const double4* sorted, GridIndex* g, unsigned int* err) {
+                              const int* cellStart, const double4* sorted, int countAlg, GridIndex* g, unsigned int* err) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
   for (int k = 0; k < nparts; ++k)
@@ -90,6 +90,7 @@ __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64
   out.heavyPrefix = nullptr;
   out.subOff = nullptr;
   out.subStart = nullptr;
+  out.countAlg = countAlg;
   *g = out;
 }
 
@@ -236,6 +237,24 @@ __global__ void k_grid_finish(GridIndex* g, const double4* sorted2, const int* h
   }
 }
 
+// Duplicate sites (reading U14: VD_E_INPUT): equal coordinates mean equal cell and sub-cell keys, so the two sites sit
+// in the same finest bucket of the finished index.  One thread per sorted position compares with the rest of its bucket.
+__global__ void __launch_bounds__(kBlock) k_find_duplicates(const GridIndex* __restrict__ gp, int64_t n, unsigned int* err) {
+  const GridIndex g = *gp;
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+    const double4 s = g.sites[p];
+    const int cx = cell_of(g, 0, s.x), cy = cell_of(g, 1, s.y), cz = cell_of(g, 2, s.z);
+    const int c = (cz * g.G[1] + cy) * g.G[0] + cx;
+    int end = g.cellStart[c + 1];
+    const int so = g.subOff ? g.subOff[c] : -1;
+    if (so >= 0) end = g.subStart[(so & 0x3ffffff) + sub_key(g, c, so >> 26, s.x, s.y, s.z) + 1];
+    for (int64_t q = p + 1; q < end; ++q) {
+      const double4 t = g.sites[q];
+      if (t.x == s.x && t.y == s.y && t.z == s.z) { atomicOr(err, ERR_DUPLICATE); break; }
+    }
+  }
+}
+
 // S2 as a kernel: one warp per query point.
 __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __restrict__ gp, const double* __restrict__ q3, int64_t nq,
                                                             int* __restrict__ out, Counters* cnt) {
@@ -257,7 +276,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
 
 static int grid_for(int64_t items, int perBlock) {
   int64_t b = (items + perBlock - 1) / perBlock;
-  const int64_t cap = 148 * 16;
+  const int64_t cap = sm_count() * 16;
   if (b > cap) b = cap;
   if (b < 1) b = 1;
   return (int)b;
@@ -281,7 +300,8 @@ vd_status stage_index(vd_ctx* c) {
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
-                                         c->sorted.as<double4>(), c->grid.as<GridIndex>(), &c->control.as<Control>()->err);
+                                         c->sorted.as<double4>(), c->opt.count_alg > 0 ? 1 : 0, c->grid.as<GridIndex>(),
+                                         &c->control.as<Control>()->err);
   cudaMemsetAsync(c->cellFill.p, 0, sizeof(int) * (gridCap + 2), st);
   VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
                                                               c->cellFill.as<int>());
@@ -319,6 +339,7 @@ vd_status stage_index(vd_ctx* c) {
                                                                                c->subStart.as<int>());
   VD_LAUNCH(k_grid_finish, 1, 1, 0, st)(gp, c->sorted2.as<double4>(), c->heavyPrefix.as<int>(), c->subOff.as<int>(),
                                          c->subStart.as<int>(), &c->control.as<Control>()->nHeavy);
+  VD_LAUNCH(k_find_duplicates, grid_for(n, kBlock), kBlock, 0, st)(gp, n, &c->control.as<Control>()->err);
   c->indexValid = true;
   return cuda_check(c, cudaGetLastError(), "site index");
 }
@@ -326,7 +347,7 @@ vd_status stage_index(vd_ctx* c) {
 vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out) {
   if (nq <= 0) return VD_OK;
   const int blocks = grid_for(nq, kWarpsPerBlock);
-  VD_LAUNCH(k_nearest_points, blocks, kBlock, 0, c->stream)(c->grid.as<GridIndex>(), q3, nq, out, &c->control.as<Control>()->cnt);
+  VD_LAUNCH(k_nearest_points, blocks, kBlock, 0, c->stream)(c->grid.as<GridIndex>(), q3, nq, out, &c->control.as<Control>()->cnt[CNT_OTHER]);
   return cuda_check(c, cudaGetLastError(), "nearest");
 }
 

@@ -17,10 +17,19 @@ struct Control {
   unsigned long long finished;   // pairs the fast tier has completed (persistent mode: termination)
   unsigned int err;              // ERR_* bits
   unsigned int nHeavy;           // refined cells of the site index (second level)
-  Counters cnt;
+  Counters cnt[kCntKinds];       // per kernel kind (CNT_*): k_ph_init, verify, fix, finish, tail, everything else
   unsigned long long nPieces, nNonEmpty, nVerts, nNbrs;   // totals written by S6
   unsigned int nListed, padListed;                        // S6: non-empty sites listed for the warp-per-site kernels
 };
+
+inline Counters counters_total(const Control& h) {
+  Counters t = {};
+  const int nf = (int)(sizeof(Counters) / sizeof(unsigned long long));
+  for (int k = 0; k < kCntKinds; ++k)
+    for (int f = 0; f < nf; ++f)
+      reinterpret_cast<unsigned long long*>(&t)[f] += reinterpret_cast<const unsigned long long*>(&h.cnt[k])[f];
+  return t;
+}
 
 struct DevBuf {
   void* p = nullptr;
@@ -32,7 +41,10 @@ struct DevBuf {
 
 struct vd_ctx {
   int64_t n = 0, nv = 0, m = 0;
-  int dim = 0, kind = -1, nc = 0, nfl = 0;
+  int dim = 0, kind = -1, nc = 0, nfl = 0;   // dim = the caller's dimension (inputs and outputs); kind = the kind the kernels run
+  bool weighted = false;   // vd_create_weighted: dim 2 -> sites lifted to R^3, VD_TRI_2D runs as a flat surface;
+                           //                     dim 3 -> siteW holds the additive term eta - w_i of every site
+  int64_t syncs = 0;       // host waits on the stream inside the current vd_compute
   bool haveDomain = false, haveResult = false, indexValid = false;
   cudaStream_t stream = nullptr;
   void* (*allocFn)(size_t, void*, void*) = nullptr;
@@ -40,6 +52,7 @@ struct vd_ctx {
   void* allocUser = nullptr;
   vd_options opt{};
   vd_counters counters{};
+  vd_counters phaseCounters[6] = {};   // per kernel kind (vd_get_phase_counters)
   double stageMs[5] = {0, 0, 0, 0, 0};
   double phaseMs[5] = {0, 0, 0, 0, 0};
   cudaEvent_t phaseEv[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -49,7 +62,8 @@ struct vd_ctx {
   int64_t pairCap = 0, vertCap = 0, nbrCap = 0, hashCap = 0, ovfCap = 0, gridCap = 0;
 
   // inputs
-  vd::DevBuf sites;       // double [n][3] (z = 0 for dim 2)
+  vd::DevBuf sites;       // double [n][3] (z = 0 for dim 2; z = sqrt(eta - w_i) for weighted 2D sites)
+  vd::DevBuf siteW;       // double [n]  eta - w_i (weighted 3D sites), else empty
   vd::DevBuf verts;       // double [nv][3]
   vd::DevBuf simp;        // int [m][nc]
   vd::DevBuf adj;         // int [m][nc]
@@ -95,6 +109,9 @@ struct vd_ctx {
 };
 
 namespace vd {
+
+int sm_count();   // multiprocessors of the current device (cudaDevAttrMultiProcessorCount, cached): launch grids are multiples of it
+cudaError_t sync_stream(vd_ctx* c);   // cudaStreamSynchronize on the context's stream, counted (vd_counters.syncs)
 
 // memory
 vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes);

@@ -10,6 +10,20 @@ struct QueryStats {
   unsigned queries, dist_evals, rows;
 };
 
+// Work counters that are bumped rarely (per clip, per piece, per measurement-mode query) live in shared memory, one row
+// per warp, instead of in registers of kernels that run at their register cap: [0] corners side-tested by clips,
+// [1] corners created by clips, [2] fan simplices of finished pieces, [3] step-out probes, [4] D_alg.
+constexpr int kExtraCnt = 5;
+static __shared__ unsigned sExtraCnt[kWarpsPerBlock][kExtraCnt + 3];
+
+__device__ __forceinline__ void extra_cnt_reset() {
+  if (lane_id() < kExtraCnt) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][lane_id()] = 0u;
+  __syncwarp();
+}
+__device__ __forceinline__ void extra_cnt_add(int which, unsigned v) {
+  if (lane_id() == 0) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][which] += v;
+}
+
 __device__ __forceinline__ int cell_of(const GridIndex& g, int ax, double q) {
   int c = (int)floor((q - g.lo[ax]) * g.inv_h[ax]);
   return min(max(c, 0), g.G[ax] - 1);
@@ -119,6 +133,28 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
   }
 }
 
+// One GridIndex per warp in shared memory: the view of a refined cell's sub-grid that a query (or a batch of queries,
+// or a one-shot search) works in.  (As a local variable it lived in local memory: the struct is passed by reference
+// to functions that are not inlined.)
+static __shared__ GridIndex sView[kWarpsPerBlock];
+
+__device__ __forceinline__ GridIndex& warp_view() { return sView[(threadIdx.x / kLanes) % kWarpsPerBlock]; }
+
+// Is the ball (q, r) strictly inside cell (cx, cy, cz) of g (with a margin against the rounding of cell assignment)?
+__device__ __forceinline__ bool ball_in_cell(const GridIndex& g, int cx, int cy, int cz, double qx, double qy, double qz, double r) {
+  const int cc[3] = {cx, cy, cz};
+  const double q[3] = {qx, qy, qz};
+  bool in = r < 1e150;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (g.h[a] > 0) {
+      const double lo = g.lo[a] + cc[a] * g.h[a], m = 1e-6 * g.h[a];
+      in = in && (q[a] - r > lo + m) && (q[a] + r < lo + g.h[a] - m);
+    }
+  }
+  return in;
+}
+
 // View of a refined cell's sub-grid as a grid of its own.
 __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z, int so, GridIndex& v) {
   const int K = so >> 26;
@@ -135,7 +171,7 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
   v.n = 0;
   v.cellStart = g.subStart + (so & 0x3ffffff);
   v.sites = g.sites;
-  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr;
+  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0;
 }
 
 // One cell of the top grid: a plain cell is scanned directly, a refined cell through its sub-grid,
@@ -149,8 +185,10 @@ static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, 
     scan_box<false>(g, qx, qy, qz, x, x, y, y, z, z, best, bestId, st);   // plain cell: a 1 x 1 x 1 box of the top grid
     return;
   }
-  GridIndex v;
-  sub_view(g, x, y, z, so, v);
+  GridIndex& v = warp_view();
+  __syncwarp();
+  if (lane_id() == 0) sub_view(g, x, y, z, so, v);
+  __syncwarp();
   int vx0 = 0, vx1 = v.G[0] - 1, vy0 = 0, vy1 = v.G[1] - 1, vz0 = 0, vz1 = v.G[2] - 1;
   if (best < 1e300) {
     const double r = sqrt(best);
@@ -161,6 +199,47 @@ static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, 
   scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
 }
 
+// D_alg: the sites stored in the grid cells (sub-cells of refined cells) that meet the ball (q, sqrt(r2)) --
+// the least any exact search over this index examines.  One THREAD per query; measurement runs only (vd_options.count_alg).
+static __device__ __noinline__ unsigned ball_sites(const GridIndex& g, double qx, double qy, double qz, double r2) {
+  if (!(r2 < 1e300)) return (unsigned)g.n;
+  const double r = sqrt(r2);
+  const int y0 = cell_of(g, 1, qy - r), y1 = cell_of(g, 1, qy + r), z0 = cell_of(g, 2, qz - r), z1 = cell_of(g, 2, qz + r);
+  const int x0 = cell_of(g, 0, qx - r), x1 = cell_of(g, 0, qx + r);
+  unsigned total = 0;
+  for (int z = z0; z <= z1; ++z)
+    for (int y = y0; y <= y1; ++y) {
+      const double rd2 = slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z);
+      if (rd2 > r2) continue;
+      const double w = sqrt(r2 - rd2);
+      const int xa = max(x0, cell_of(g, 0, qx - w)), xb = min(x1, cell_of(g, 0, qx + w));
+      if (xa > xb) continue;
+      const int rowBase = (z * g.G[1] + y) * g.G[0];
+      if (!g.subOff) { total += (unsigned)(g.cellStart[rowBase + xb + 1] - g.cellStart[rowBase + xa]); continue; }
+      for (int x = xa; x <= xb; ++x) {
+        const int so = g.subOff[rowBase + x];
+        const unsigned cnt = (unsigned)(g.cellStart[rowBase + x + 1] - g.cellStart[rowBase + x]);
+        if (so < 0) { total += cnt; continue; }
+        GridIndex v;
+        sub_view(g, x, y, z, so, v);
+        const int sx0 = cell_of(v, 0, qx - r), sx1 = cell_of(v, 0, qx + r), sy0 = cell_of(v, 1, qy - r), sy1 = cell_of(v, 1, qy + r);
+        const int sz0 = cell_of(v, 2, qz - r), sz1 = cell_of(v, 2, qz + r);
+        if (sx0 == 0 && sy0 == 0 && sz0 == 0 && sx1 == v.G[0] - 1 && sy1 == v.G[1] - 1 && sz1 == v.G[2] - 1) { total += cnt; continue; }
+        for (int sz = sz0; sz <= sz1; ++sz)
+          for (int sy = sy0; sy <= sy1; ++sy) {
+            const double sd2 = slab_d2(v, 1, qy, sy, sy) + slab_d2(v, 2, qz, sz, sz);
+            if (sd2 > r2) continue;
+            const double sw = sqrt(r2 - sd2);
+            const int sa = max(sx0, cell_of(v, 0, qx - sw)), sb = min(sx1, cell_of(v, 0, qx + sw));
+            if (sa > sb) continue;
+            const int sb0 = (sz * v.G[1] + sy) * v.G[0];
+            total += (unsigned)(v.cellStart[sb0 + sb + 1] - v.cellStart[sb0 + sa]);
+          }
+      }
+    }
+  return total;
+}
+
 // N_q: the site nearest to q among those closer than the incoming (best, bestId); ties to
 // the lowest id (reading U5).  Call with best = +inf, bestId = INT_MAX for an unbounded query, or
 // with best = |q - v_i|^2, bestId = i for a point-in-cell test (Eq. 2).
@@ -169,8 +248,22 @@ static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, 
 // soon as the cells around q have produced one, without proving it the nearest (reading U17).  When no
 // site is clearly nearer, the full scan runs and the answer is exact, so acceptance is always exact.
 template <bool HV>
-static __device__ __noinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
+static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
+                                             QueryStats& st, bool nearer_ok);
+
+template <bool HV>
+__device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                         QueryStats& st, bool nearer_ok = false) {
+  nearest_impl<HV>(g, qx, qy, qz, best, bestId, st, nearer_ok);
+  if (g.countAlg) {
+    if (lane_id() == 0) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][4] += ball_sites(g, qx, qy, qz, best);
+    __syncwarp();
+  }
+}
+
+template <bool HV>
+static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
+                                             QueryStats& st, bool nearer_ok) {
   const double bound0 = best;
   st.queries += 1;
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);
@@ -179,8 +272,10 @@ static __device__ __noinline__ void nearest(const GridIndex& g, double qx, doubl
     // the sub-grid alone decides; a loose bound is first tightened on the 3 x 3 x 3 sub-cells around q.
     const int so = __ldg(&g.subOff[(cz * g.G[1] + cy) * g.G[0] + cx]);
     if (so >= 0) {
-      GridIndex v;
-      sub_view(g, cx, cy, cz, so, v);
+      GridIndex& v = warp_view();
+      __syncwarp();
+      if (lane_id() == 0) sub_view(g, cx, cy, cz, so, v);
+      __syncwarp();
 #pragma unroll 1   // (code size: the refined-index kernels are instruction-fetch bound)
       for (int pass = 0; pass < 2; ++pass) {
         if (best < 1e300) {

@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
     if (lane == 0) { c->np = np; c->nc = nc; c->a = pr.a; c->i = pr.i; c->failed = failed; }
     __syncwarp();
   }
-  flush_counters(A.ctl, st, lc);
+  flush_counters(A.ctl, st, lc, CNT_INIT);
 }
 
 // list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
@@ -115,6 +116,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -141,7 +143,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
     }
     __syncwarp();
   }
-  flush_counters(A.ctl, st, lc);
+  flush_counters(A.ctl, st, lc, CNT_VERIFY);
 }
 
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
@@ -156,6 +158,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -182,7 +185,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
     }
     __syncwarp();
   }
-  flush_counters(A.ctl, st, lc);
+  flush_counters(A.ctl, st, lc, CNT_FIX);
 }
 
 // The last few pairs of a wave (a verify round left fewer than kTailPairs with a corner outside): tests and clips
@@ -200,6 +203,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   for (;;) {
     const int t = next_item(pc, count);
     if (t < 0) break;
@@ -229,7 +233,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
     }
     __syncwarp();
   }
-  flush_counters(A.ctl, st, lc);
+  flush_counters(A.ctl, st, lc, CNT_TAIL);
 }
 
 __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
@@ -238,6 +242,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
+  extra_cnt_reset();
   WarpPool wp = {0ull, 0ull, 0, 0, vchunk, nchunk};
   // uniform work per piece: a static stride instead of a ticket (one same-address atomic less per piece)
   const int stride = (int)gridDim.x * kWarpsPerBlock;
@@ -249,7 +254,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
     finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc, &wp);
     __syncwarp();
   }
-  flush_counters(A.ctl, st, lc);
+  flush_counters(A.ctl, st, lc, CNT_FINISH);
 }
 
 static vd_status reset_ctl(vd_ctx* c, PhaseCtl* pc, bool all) {
@@ -273,7 +278,7 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
   PhaseCtl* pc = reinterpret_cast<PhaseCtl*>(done + cap);
   cudaStream_t st = c->stream;
   cudaEvent_t* ev = c->phaseEv;
-  const int grid = 148 * 4;
+  const int grid = sm_count() * 4;
   const int tailPairs = c->opt.tail_pairs == 0 ? kTailPairs : c->opt.tail_pairs;   // < 0: never
   auto elapsed = [&](int which, cudaEvent_t a, cudaEvent_t b) {
     float ms = 0.f;
@@ -283,7 +288,7 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
     // through page-locked memory: a copy into pageable memory is staged by the driver (tens of microseconds, once per round)
     PhaseCtl* dst = c->pinned ? reinterpret_cast<PhaseCtl*>(c->pinned) : &h;
     cudaError_t e = cudaMemcpyAsync(dst, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = sync_stream(c);
     if (e == cudaSuccess && dst != &h) h = *dst;
     return e;
   };
@@ -334,13 +339,13 @@ vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64
     if (h.nDone > 0) {
       // pool chunk per warp: ~1/32 of an even share of the pool, so that the slack (one open chunk per warp) stays small
       // static stride over the grid: exactly the resident blocks (3 per SM), or the last third would run alone
-      const int fgrid = 148 * 3;
+      const int fgrid = sm_count() * 3;
       const int64_t warps = (int64_t)fgrid * kWarpsPerBlock;
       auto chunk_of = [&](int64_t cap) { const int64_t v = cap / (warps * 32); return (int)(v > 1024 ? 1024 : v); };   // small pools: piece by piece
       cudaEventRecord(ev[0], st);
       VD_LAUNCH(k_ph_finish, fgrid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, chunk_of(c->vertCap), chunk_of(c->nbrCap));
       cudaEventRecord(ev[1], st);
-      const cudaError_t e = cudaStreamSynchronize(st);
+      const cudaError_t e = sync_stream(c);
       if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
       elapsed(3, ev[0], ev[1]);
     }

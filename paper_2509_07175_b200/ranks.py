@@ -2,7 +2,8 @@
 
 The hot path shards by simplex: rank r owns a contiguous block of M (simplex_block), the sites
 and their index are replicated, and one all-reduce of per-cell (measure, first moment) combines the partial
-cells (combine_partial_cells).  Measurement: the slowest rank's device time (max) and the units each rank
+cells (combine_partial_cells: the packing and the division run in the library's kernels -- vd_partial_moments /
+vd_finish_centroids --, this module only calls all_reduce).  Measurement: the slowest rank's device time (max) and the units each rank
 processed (sum); rank 0 reports units / max time.
 """
 from __future__ import annotations
@@ -22,12 +23,6 @@ def whole_job_rate(units_local: float, ms_local: float, device=None) -> tuple[fl
     return float(u.item()) / (float(t.item()) * 1e-3), float(t.item())
 
 
-def shard_of_replicas(n_units: int, rank: int, world: int) -> range:
-    """Simple domains (one piece per cell, nothing to partition): every rank owns all units of its own copy."""
-    del rank, world
-    return range(n_units)
-
-
 def simplex_block(m: int, rank: int, world: int) -> tuple[int, int]:
     """Rank's contiguous block [begin, end) of the m simplices (vd_options.simplex_begin / simplex_end).
 
@@ -39,20 +34,25 @@ def simplex_block(m: int, rank: int, world: int) -> tuple[int, int]:
     return begin, begin + base + (1 if rank < extra else 0)
 
 
-def combine_partial_cells(measure, centroid, sites):
-    """The one exchange step of the sharded path: per-cell partial measure and first moment (measure x centroid)
-    summed over ranks (all_reduce: NCCL over NVLink on GPUs, gloo in the CPU tests); centroid = moment / measure,
-    the site itself for an empty cell (vd.h).  Tensors [n], [n][dim], [n][dim] on the rank's device; returns the
-    combined (measure, centroid).  Without an initialised group it returns its inputs' own combination."""
-    moment = centroid * measure[:, None]
-    total = measure.clone()
+def all_reduce_sums(packed):
+    """The one exchange step of the sharded path: per-cell (measure, first moment) rows [n][1 + dim], summed over
+    the ranks in place (all_reduce: NCCL over NVLink on GPUs, gloo in the CPU tests).  No group: unchanged."""
     if dist.is_available() and dist.is_initialized():
-        packed = torch.cat([total[:, None], moment], dim=1).contiguous()
         dist.all_reduce(packed, op=dist.ReduceOp.SUM)
-        total, moment = packed[:, 0].contiguous(), packed[:, 1:]
-    safe = torch.where(total > 0, total, torch.ones_like(total))
-    cen = torch.where((total > 0)[:, None], moment / safe[:, None], sites)
-    return total, cen
+    return packed
+
+
+def combine_partial_cells(ctx, buf=None):
+    """After ctx.compute() on this rank's block of M: vd_partial_moments packs (measure, measure x centroid) per cell
+    into a device buffer, one all-reduce sums it over the ranks, vd_finish_centroids rewrites the context's measure /
+    centroid arrays from the sums (centroid = moment / measure, the site itself for an empty cell) -- every rank then
+    holds the whole diagram's measures and centroids.  Returns the buffer (pass it back in to reuse it)."""
+    if buf is None:
+        buf = torch.empty((ctx.n, 1 + ctx.dim), dtype=torch.float64, device=torch.device("cuda", torch.cuda.current_device()))
+    ctx.partial_moments(buf.data_ptr())
+    all_reduce_sums(buf)
+    ctx.finish_centroids(buf.data_ptr())
+    return buf
 
 
 def simplex_blocks_balanced(sites, verts, simplices, world: int, grid: int = 0):

@@ -4,9 +4,10 @@ Both sides deliver the same CSR shape with pieces ordered by simplex id and the 
 ordered by their ascending flag tuple, so equal structure means equal arrays.
 Tolerances (BASELINE.json north_star): neighbour sets, piece simplices, corner counts and corner
 flags bit-exact; |Δmeasure| <= 1e-9 * measure; |Δcentroid| <= 1e-9 * max(|centroid|, diam);
-|Δvertex| <= 1e-9 * diam.  `abs_measure` is the rounding floor for sliver cells: a cell whose
-measure is 1e-9 of a simplex is a difference of nearly equal corner coordinates, so its measure carries an
-absolute error of about eps * |simplex|; callers at full scale pass 1e-12 * |M| / m.
+|Δvertex| <= 1e-9 * diam.  `simplex_measure` ([m] array, or a scalar) switches on the rounding floor for sliver
+cells: a cell whose measure is 1e-9 of a simplex is a difference of nearly equal corner coordinates, so
+its measure carries an absolute error of about eps * |T_a| on either side; the floor is 64 * eps * the largest simplex
+the cell touches -- nothing looser.
 """
 from __future__ import annotations
 
@@ -35,7 +36,10 @@ def _match_ties(gx, ox, fl):
     return worst
 
 
-def compare(gpu, ora, diam, ids=None, tiny_measure=1e-12, abs_measure=0.0):
+EPS = 2.220446049250313e-16
+
+
+def compare(gpu, ora, diam, ids=None, tiny_measure=1e-12, abs_measure=0.0, simplex_measure=None):
     """gpu: binding.HostCells over all n sites; ora: oracle.Cells over `ora.ids`.
     Returns a dict of mismatch lists (empty lists = parity)."""
     ids = np.asarray(ora.ids if ids is None else ids, dtype=np.int64)
@@ -84,7 +88,11 @@ def compare(gpu, ora, diam, ids=None, tiny_measure=1e-12, abs_measure=0.0):
         m_o, m_g = float(ora.measure[s]), float(gpu.measure[i])
         if m_o > 0:
             max_meas = max(max_meas, abs(m_g - m_o) / m_o)
-        if abs(m_g - m_o) > REL * m_o + abs_measure:
+        floor = abs_measure
+        if simplex_measure is not None and op1 > op0:
+            sm = np.asarray(simplex_measure, dtype=np.float64)
+            floor += 64.0 * EPS * float(sm[os_].max() if sm.ndim else sm)
+        if abs(m_g - m_o) > REL * m_o + floor:
             bad["measure"].append((int(i), m_g, m_o))
         dc = float(np.linalg.norm(gpu.centroid[i] - ora.centroid[s]))
         if dc > REL * max(float(np.linalg.norm(ora.centroid[s])), diam):
@@ -94,12 +102,25 @@ def compare(gpu, ora, diam, ids=None, tiny_measure=1e-12, abs_measure=0.0):
     return bad
 
 
-def assert_parity(gpu, ora, diam, ids=None, allow_excused=0, abs_measure=0.0):
-    bad = compare(gpu, ora, diam, ids, abs_measure=abs_measure)
+def assert_parity(gpu, ora, diam, ids=None, allow_excused=0, abs_measure=0.0, simplex_measure=None):
+    bad = compare(gpu, ora, diam, ids, abs_measure=abs_measure, simplex_measure=simplex_measure)
     problems = {k: v for k, v in bad.items() if not k.startswith("_") and k != "excused" and v}
     assert not problems, {k: v[:5] for k, v in problems.items()}
     assert len(bad["excused"]) <= allow_excused, bad["excused"][:5]
     return bad
+
+
+def simplex_measures(w):
+    """|T_a| of every simplex of a meshed workload (plain determinant / cross-product formulas); |box| for box kinds."""
+    if w.simplices is None:
+        return np.float64(w.measure)
+    p = w.verts[w.simplices]
+    if w.kind == 0:
+        e1, e2 = p[:, 1] - p[:, 0], p[:, 2] - p[:, 0]
+        return np.abs(e1[:, 0] * e2[:, 1] - e1[:, 1] * e2[:, 0]) * 0.5
+    if w.kind == 1:
+        return np.linalg.norm(np.cross(p[:, 1] - p[:, 0], p[:, 2] - p[:, 0]), axis=1) * 0.5
+    return np.abs(np.linalg.det(p[:, 1:] - p[:, :1])) / 6.0
 
 
 def global_checks(gpu, w):

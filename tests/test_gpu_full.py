@@ -14,18 +14,26 @@ pytestmark = pytest.mark.gpu
 
 
 def _sample(g, n, k, seed):
+    """K sites: half seeded-random, half the extremes of the GPU report.  Where most cells are empty
+    (C4: 70 %, C5: 99.93 %) three quarters of the random half are drawn from the non-empty cells and the rest over all
+    sites, which checks emptiness."""
     rng = np.random.default_rng(seed)
-    rnd = rng.choice(n, size=min(n, k // 2), replace=False)
+    pos = np.where(g.measure > 0)[0]
+    half = min(n, k // 2)
+    if len(pos) < 0.9 * n:
+        rnd = np.concatenate([rng.choice(pos, size=min(len(pos), (3 * half) // 4), replace=False),
+                              rng.choice(n, size=half - (3 * half) // 4, replace=False)])
+    else:
+        rnd = rng.choice(n, size=half, replace=False)
     npieces = np.diff(g.piece_off)
     nnbr = np.diff(g.nbr_off)
-    pos = np.where(g.measure > 0)[0]
     q = k // 8
     ext = np.concatenate([np.argsort(-g.measure)[:q], np.argsort(-npieces)[:q], np.argsort(-nnbr)[:q],
                           pos[np.argsort(g.measure[pos])[:q]]])
     return np.unique(np.concatenate([rnd, ext])).astype(np.int64)
 
 
-@pytest.mark.parametrize("idx,k", [(2, 256), (4, 192), (5, 96), (3, 96)])
+@pytest.mark.parametrize("idx,k", [(2, 512), (4, 512), (5, 512), (3, 512)])
 def test_full_config_invariants_and_sampled_parity(idx, k):
     w = inputs.config(idx)
     with binding.Context(w.sites) as ctx:
@@ -41,7 +49,9 @@ def test_full_config_invariants_and_sampled_parity(idx, k):
     ids = _sample(g, w.n, k, 1000 + idx)
     tier = "A" if w.kind == inputs.KIND_TRI_SURFACE else "B"
     o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=ids, tier=tier)
-    bad = parity.assert_parity(g, o, w.diameter, allow_excused=1, abs_measure=1e-12 * w.measure / w.m)
+    bad = parity.assert_parity(g, o, w.diameter, simplex_measure=parity.simplex_measures(w))
+    print(f"C{idx}: {len(ids)} sampled cells ({int((o.measure == 0).sum())} empty), max rel measure error "
+          f"{bad['_max_rel_measure']:.3e}, max corner error {bad['_max_xyz']:.3e}")
 
 
 @pytest.mark.parametrize("dim,n,k", [(3, 1000000, 256), (2, 2000000, 256)])
@@ -63,4 +73,4 @@ def test_box_domain_at_scale(dim, n, k):
     assert np.array_equal(fwd, rev)
     ids = _sample(g, n, k, 77 + dim)
     o = oracle.compute(w.sites, w.verts, None, w.kind, subset=ids, tier="B")
-    parity.assert_parity(g, o, w.diameter, ids=ids, allow_excused=1)
+    parity.assert_parity(g, o, w.diameter, ids=ids, simplex_measure=parity.simplex_measures(w))

@@ -1,6 +1,9 @@
-"""Power diagrams by lifting: the oracle's surface kind on lifted sites is pinned against the power
-cell's own definition (half-plane clipping with power bisectors, written out here in numpy), and the CUDA path is
-compared with the oracle on the same lifted inputs."""
+"""Power diagrams.  The oracle's weighted kinds clip with the power cell's own half-spaces; they are
+pinned against (a) that definition written out here in numpy (2D), (b) the paper's construction -- the oracle's
+restricted Voronoi diagram of the LIFTED sites on the flat surface --, (c) equal weights = the Voronoi diagram, and
+(d) in 3D, brute force: every output corner has equal power distance to its cell's site and the sites of its flags,
+and no site has a smaller one.  The CUDA path (vd_create_weighted: the lifting runs in its kernels) is compared with
+the oracle on the same weighted inputs."""
 import numpy as np
 import pytest
 
@@ -65,31 +68,74 @@ def test_oracle_surface_kind_on_lifted_sites_is_the_power_diagram():
     assert np.array_equal(o0.nbr_off, o2.nbr_off) and np.array_equal(o0.nbr, o2.nbr)
 
 
-def test_lift_helper():
-    from paper_2509_07175_b200 import power
-    s, w = _weighted(50, 3, 0.1)
-    p = power.lift_sites(s, w)
-    assert p.shape == (50, 3) and np.allclose(p, _lift(s, w)) and p[:, 2].min() == 0.0       # eta = max w
-    q = power.lift_sites(s, w, eta=1.0)
-    # |x - p_i|^2 - |x - p_j|^2 at height 0 equals the power-distance difference, whatever eta
-    x = np.array([0.3, 0.7, 0.0])
-    for lifted in (p, q):
-        dd = ((x - lifted) ** 2).sum(1)
-        pw = ((x[:2] - s) ** 2).sum(1) - w
-        assert np.allclose(dd - dd[0], pw - pw[0], atol=1e-12)
-    with pytest.raises(ValueError):
-        power.lift_sites(s, w, eta=float(w.max()) - 1e-3)
+def test_oracle_weighted_kind_2d():
+    """The weighted 2D kind against the numpy definition and against the paper's lifted construction."""
+    s, w = _weighted(300, 11, 0.004)
+    verts, tris = inputs.square_grid_mesh(3)
+    ow = oracle.compute(s, verts, tris, inputs.KIND_TRI_2D, weights=w)
+    ref = np.array([_power_cell_area(i, s, w) for i in range(len(s))])
+    assert np.abs(ow.measure - ref).max() <= 1e-12 and (ref == 0).sum() > 0
+    v3 = np.concatenate([verts, np.zeros((len(verts), 1))], axis=1)
+    ol = oracle.compute(_lift(s, w), v3, tris, inputs.KIND_TRI_SURFACE, tier="A")
+    for f in ("nbr_off", "nbr", "piece_off", "piece_simplex", "vert_off", "vert_flags"):
+        assert np.array_equal(getattr(ow, f), getattr(ol, f)), f
+    assert np.abs(ow.vert_xyz - ol.vert_xyz[:, :2]).max() <= 1e-12 and np.abs(ol.vert_xyz[:, 2]).max() == 0.0
+    assert np.abs(ow.measure - ol.measure).max() <= 1e-13
+    # tier B (facets in the bounding box first) gives the same cells
+    ob = oracle.compute(s, verts, tris, inputs.KIND_TRI_2D, weights=w, tier="B")
+    assert np.array_equal(ob.vert_flags, ow.vert_flags) and np.abs(ob.measure - ow.measure).max() <= 1e-13
+
+
+def _weighted3(n, seed, scale=1.0):
+    rng = np.random.default_rng(seed)
+    s = rng.random((n, 3))
+    return s, scale * rng.uniform(-1.0, 1.0, n) / n ** (2.0 / 3.0)     # comparable to the squared site spacing
+
+
+def test_oracle_weighted_kind_3d():
+    s, w = _weighted3(400, 21, 0.6)
+    verts, tets = inputs.cube_kuhn_mesh(2)
+    o = oracle.compute(s, verts, tets, inputs.KIND_TET_3D, weights=w)
+    assert abs(o.measure.sum() - 1.0) <= 1e-12
+    assert (o.measure == 0).sum() > 0                                  # some sites are hidden
+    # every corner: equal power distance to its own site and to the sites of its flags, none smaller (brute force)
+    owner = np.repeat(np.repeat(np.arange(len(s)), np.diff(o.piece_off)), np.diff(o.vert_off))
+    rng = np.random.default_rng(0)
+    for v in rng.choice(len(o.vert_xyz), 3000, replace=False):
+        pd = ((s - o.vert_xyz[v]) ** 2).sum(1) - w
+        assert pd[owner[v]] <= pd.min() + 1e-12
+        for fl in o.vert_flags[v]:
+            if fl >= 0:
+                assert abs(pd[fl] - pd[owner[v]]) <= 1e-12
+    # neighbour symmetry, and a constant added to every weight changes nothing
+    pairs = {(i, int(j)) for i in range(len(s)) for j in o.neighbours(i)}
+    assert all((j, i) in pairs for i, j in pairs)
+    o2 = oracle.compute(s, verts, tets, inputs.KIND_TET_3D, weights=w + 0.37)
+    assert np.array_equal(o.vert_flags, o2.vert_flags) and np.abs(o.measure - o2.measure).max() <= 1e-13
+    # equal weights: the Voronoi diagram (P:L459), in the box kind too
+    o0 = oracle.compute(s, verts, tets, inputs.KIND_TET_3D, weights=np.full(len(s), 0.2))
+    o1 = oracle.compute(s, verts, tets, inputs.KIND_TET_3D)
+    assert np.array_equal(o0.vert_flags, o1.vert_flags) and np.abs(o0.measure - o1.measure).max() <= 1e-13
+    box = np.array([[0.0, 0, 0], [1.0, 1, 1]])
+    ob = oracle.compute(s, box, None, inputs.KIND_BOX_3D, weights=w)
+    assert np.abs(ob.measure - o.measure).max() <= 1e-12 and np.array_equal(ob.nbr, o.nbr)
 
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("n,spread,k", [(2000, 0.0005, 8), (500, 0.01, 4)])
 def test_power_diagram_parity_on_the_gpu(n, spread, k):
     import parity
-    from paper_2509_07175_b200 import power
+    from paper_2509_07175_b200 import binding, power
     s, w = _weighted(n, 5, spread)
     verts, tris = inputs.square_grid_mesh(k)
     g = power.power_cells(s, w, verts, tris)
-    o = oracle.compute(power.lift_sites(s, w), power.embed_domain(verts), tris, inputs.KIND_TRI_SURFACE, tier="A")
+    assert g.dim == 2 and g.vert_xyz.shape[1] == 2
+    o = oracle.compute(s, verts, tris, inputs.KIND_TRI_2D, weights=w)
     parity.assert_parity(g, o, np.sqrt(2.0))
     assert abs(g.measure.sum() - 1.0) <= 1e-11
-    assert (g.measure == 0).sum() == (o.measure == 0).sum()
+    assert (g.measure == 0).sum() == (o.measure == 0).sum() > 0 or spread < 0.001
+    g2 = power.power_cells(s, w, verts, tris, eta=float(w.max()) + 0.05)     # any admissible eta gives the same cells
+    parity.assert_parity(g2, o, np.sqrt(2.0))
+    with pytest.raises(binding.VdError) as e:                                # eta below the largest weight
+        power.power_cells(s, w, verts, tris, eta=float(w.max()) - 1e-3)
+    assert e.value.status == 4

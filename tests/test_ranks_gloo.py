@@ -13,7 +13,7 @@ def _worker(rank, world, port, out):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     # rank r processed 1000 units in (10 + 5 r) ms: whole job = 2000 units / 15 ms
     rate, ms = ranks.whole_job_rate(1000.0, 10.0 + 5.0 * rank)
-    out.put((rank, rate, ms, len(ranks.shard_of_replicas(7, rank, world))))
+    out.put((rank, rate, ms, 7))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -58,9 +58,13 @@ def _shard_worker(rank, world, port, out):
     w = inputs.config(2, "small")
     b, e = ranks.simplex_block(w.m, rank, world)
     part = oracle.compute(w.sites, w.verts, w.simplices[b:e], w.kind)
-    m, c = ranks.combine_partial_cells(torch.from_numpy(part.measure.copy()), torch.from_numpy(part.centroid.copy()),
-                                       torch.from_numpy(w.sites.copy()))
-    out.put((rank, b, e, m.numpy(), c.numpy()))
+    # what vd_partial_moments / vd_finish_centroids do on the device, written out for the oracle's partial cells
+    packed = torch.from_numpy(np.concatenate([part.measure[:, None], part.measure[:, None] * part.centroid], axis=1))
+    ranks.all_reduce_sums(packed)
+    s = packed.numpy()
+    m = s[:, 0].copy()
+    c = np.where(m[:, None] > 0, s[:, 1:] / np.where(m > 0, m, 1.0)[:, None], w.sites)
+    out.put((rank, b, e, m, c))
     dist.barrier()
     dist.destroy_process_group()
 
