@@ -12,7 +12,7 @@ SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_phase.c
 
 
 def lib_path() -> str:
-    return LIB
+    return os.environ.get("VD_LIB", LIB)   # experiments: another build of the same library
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

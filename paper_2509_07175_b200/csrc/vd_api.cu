@@ -1,6 +1,7 @@
 // vd_api.cu -- the C ABI of include/vd.h: argument marshalling, memory, the stage sequence of
 // vd_compute and the pool-growth / rerun policy.  No geometry happens on the host.
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -23,9 +24,33 @@ int sm_count() {
   return cached[dev];
 }
 
-cudaError_t sync_stream(vd_ctx* c) {
+cudaError_t sync_stream(vd_ctx* c, const char* why) {
   c->syncs += 1;
+  static const bool trace = getenv("VD_TRACE_SYNC") != nullptr;
+  if (trace) fprintf(stderr, "vd sync %lld: %s\n", (long long)c->syncs, why ? why : "?");
   return cudaStreamSynchronize(c->stream);
+}
+
+void phase_mark(vd_ctx* c, int kind) {
+  if (c->evUsed == (int)c->evPool.size()) {
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return; }
+    c->evPool.push_back(e);
+    c->evKind.push_back(-1);
+  }
+  c->evKind[c->evUsed] = kind;
+  cudaEventRecord(c->evPool[c->evUsed], c->stream);
+  c->evUsed += 1;
+}
+
+void phase_marks_collect(vd_ctx* c) {
+  for (int k = 0; k + 1 < c->evUsed; ++k) {
+    if (c->evKind[k] < 0) continue;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->evPool[k], c->evPool[k + 1]) == cudaSuccess) c->phaseMs[c->evKind[k]] += ms;
+    else cudaGetLastError();
+  }
+  c->evUsed = 0;
 }
 
 vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what) {
@@ -62,7 +87,7 @@ vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
   if (bytes < 256) bytes = 256;
   if (b.cap >= bytes) return VD_OK;
   // pending kernels may still use the old block
-  if (b.p) sync_stream(c);
+  if (b.p) sync_stream(c, "buffer grows");
   release(c, b);
   void* p = nullptr;
   if (c->allocFn) {
@@ -288,6 +313,7 @@ vd_status vd_update_sites(vd_ctx* c, const double* sites) {
   if (!c || !sites) return VD_E_ARG;
   if (c->weighted) { c->lastError = "vd_update_sites: a weighted context keeps its lifted sites (create a new one)"; return VD_E_STATE; }
   c->indexValid = false;
+  c->heavyKnown = -1;
   c->haveResult = false;
   return upload_points(c, sites, c->n, c->dim, c->sites, "vd_update_sites");
 }
@@ -414,7 +440,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   cudaEventRecord(c->ev[4], st);
   Control h;
   cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = sync_stream(c);
+  if (e == cudaSuccess) e = sync_stream(c, "totals");
   if (e != cudaSuccess) return cuda_check(c, e, "vd_compute");
   c->hostControl = h;
   float ms = 0;
@@ -458,6 +484,7 @@ vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) 
     VD_LAUNCH(k_move_sites, blocks, kBlock, 0, c->stream)(c->oMeasure.as<double>(), c->oCentroid.as<double>(), c->n, c->dim,
                                                          c->sites.as<double>());
     c->indexValid = false;
+  c->heavyKnown = -1;
   }
   if ((s = vd_compute(c, out))) return s;
   if (sites_out) {
@@ -476,7 +503,7 @@ void vd_destroy(vd_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->scanTmp, &c->delta, &c->siteW, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
                    &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
@@ -484,8 +511,7 @@ void vd_destroy(vd_ctx* c) {
   for (DevBuf* b : all) release(c, *b);
   for (int k = 0; k < 6; ++k)
     if (c->ev[k]) cudaEventDestroy(c->ev[k]);
-  for (int k = 0; k < 4; ++k)
-    if (c->phaseEv[k]) cudaEventDestroy(c->phaseEv[k]);
+  for (cudaEvent_t e : c->evPool) cudaEventDestroy(e);
   if (c->pinned) cudaFreeHost(c->pinned);
   delete c;
 }
@@ -509,6 +535,7 @@ vd_status vd_set_options(vd_ctx* c, const vd_options* o) {
   vd_options d;
   set_default_options(d);
   c->opt = *o;
+  c->heavyKnown = -1;
   if (!(c->opt.grid_density > 0)) c->opt.grid_density = d.grid_density;
   if (c->opt.real_edges < 0) c->opt.real_edges = d.real_edges;
   if (c->opt.persistent < 0) c->opt.persistent = d.persistent;

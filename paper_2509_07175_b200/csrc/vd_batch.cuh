@@ -24,46 +24,17 @@ struct QBatch {
   unsigned char flag[kQB];   // refined index: the query met a refined cell in the row pass
 };
 
-// Lanes 0..nq-1 have filled qx,qy,qz,best,bestId of their slot (and the warp has synchronised).  On
-// return best/bestId of every slot hold the nearest site among those closer than the incoming bound
-// (or, for a loose bound, some clearly nearer site: nearer_ok of nearest(), reading U17).
-//
-// Refined index (HV): the batched pass needs plain cells.  Two cases keep it: (a) the balls of ALL queries lie inside one
-// and the same refined cell (a piece inside a dense cluster: its corners are a few sub-cells apart) -- then the pass runs
-// on that cell's sub-grid, viewed as a grid of its own; (b) no row of a query's ball holds a refined cell (found in the
-// row pass from the prefix count of refined cells) -- then the top grid is plain for that query.  Every other query
-// takes the single-query path.
-template <bool HV>
-static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
+// One pass of the batch over ONE grid view g (the top grid, the sub-grid of a refined cell, or a single plain cell seen as a
+// 1 x 1 x 1 grid): the queries named in `active` enumerate the rows of g that their balls meet, the candidates of all rows
+// are packed 32 per round.  SKIP_REFINED (top grid of a refined index): a row that holds a refined cell is not scanned; the
+// query is flagged (B.flag) and that row is visited cell by cell afterwards.  A query whose ball spans more than
+// kQBMaxRows rows of g does not take part: it is returned in the mask of loose queries.
+template <bool SKIP_REFINED>
+static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B, int nq, unsigned active, QueryStats& st) {
   const int lane = lane_id();
-  const GridIndex* gp = &gTop;
-  bool checkRefined = false;
-  if (HV) {
-    checkRefined = true;
-    int c = -1;
-    bool ok = false;
-    int hx = 0, hy = 0, hz = 0;
-    if (lane < nq && B.best[lane] < 1e300) {
-      const double qx = B.qx[lane], qy = B.qy[lane], qz = B.qz[lane];
-      hx = cell_of(gTop, 0, qx); hy = cell_of(gTop, 1, qy); hz = cell_of(gTop, 2, qz);
-      c = (hz * gTop.G[1] + hy) * gTop.G[0] + hx;
-      ok = __ldg(&gTop.subOff[c]) >= 0 && ball_in_cell(gTop, hx, hy, hz, qx, qy, qz, sqrt(B.best[lane]));
-    }
-    const int c0 = shfl(c, 0);
-    if (__all_sync(kFull, lane >= nq || (ok && c == c0))) {
-      GridIndex& v = warp_view();
-      __syncwarp();
-      if (lane == 0) sub_view(gTop, hx, hy, hz, __ldg(&gTop.subOff[c]), v);
-      __syncwarp();
-      gp = &v;
-      checkRefined = false;
-    }
-  }
-  const GridIndex& g = *gp;
   int myRows = 0;
   bool loose = false;
-  if (lane < kQB) B.flag[lane] = 0;
-  if (lane < nq) {
+  if (lane < nq && ((active >> lane) & 1u)) {
     const double b = B.best[lane];
     if (!(b < 1e300)) {
       loose = true;
@@ -81,8 +52,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
   const int incl = warp_incl_scan(myRows);
   if (lane < nq) B.rowStart[lane] = incl - myRows;
   if (lane == nq - 1) B.rowStart[nq] = incl;
-  unsigned looseMask = __ballot_sync(kFull, loose);
-  st.queries += (unsigned)(nq - __popc(looseMask));
+  const unsigned looseMask = __ballot_sync(kFull, loose);
   __syncwarp();
   const int R = B.rowStart[nq];
   st.rows += (unsigned)R;
@@ -100,9 +70,9 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
         const int rowBase = (z * g.G[1] + y) * g.G[0];
         s = __ldg(&g.cellStart[rowBase + B.x0[u]]);
         cnt = __ldg(&g.cellStart[rowBase + B.x1[u] + 1]) - s;
-        if (HV && checkRefined && cnt > kHeavy &&
+        if (SKIP_REFINED && cnt > kHeavy &&
             __ldg(&g.heavyPrefix[rowBase + B.x1[u] + 1]) != __ldg(&g.heavyPrefix[rowBase + B.x0[u]])) {
-          cnt = 0;           // a refined cell in this row: the query goes to the single-query path
+          cnt = 0;           // a refined cell in this row
           B.flag[u] = 1;
         }
       }
@@ -152,12 +122,81 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
       __syncwarp();
     }
   }
-  if (HV && checkRefined) {
+  return looseMask;
+}
+
+// Lanes 0..nq-1 have filled qx,qy,qz,best,bestId of their slot (and the warp has synchronised).  On
+// return best/bestId of every slot hold the nearest site among those closer than the incoming bound
+// (or, for a loose bound, some clearly nearer site: nearer_ok of nearest(), reading U17).
+//
+// Refined index (HV): the corners of a piece inside a dense cluster sit in refined cells, and their balls usually reach
+// into a neighbouring cell -- refined as well, or plain.  Pass A runs on the top grid and scans the rows made of plain
+// cells only; pass B then visits, one after the other, the top cells of the rows pass A left out: a refined cell through
+// its sub-grid, a plain one as a 1 x 1 x 1 grid, each as a view that the same batched pass runs on, for the queries
+// whose ball meets that cell.  Only a query whose ball spans many rows (a corner in the void between clusters) takes the
+// single-query path.
+template <bool HV>
+static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
+  const int lane = lane_id();
+  if (lane < kQB) B.flag[lane] = 0;
+  __syncwarp();
+  unsigned looseMask = batch_pass<HV>(gTop, B, nq, (1u << nq) - 1u, st);
+  if (HV) {
     __syncwarp();
-    const unsigned flagged = __ballot_sync(kFull, lane < nq && B.flag[lane] != 0);
-    st.queries -= (unsigned)__popc(flagged & ~looseMask);
-    looseMask |= flagged;
+    const bool mine = lane < nq && B.flag[lane] != 0 && !((looseMask >> lane) & 1u);
+    const unsigned flagged = __ballot_sync(kFull, mine);
+    if (flagged) {
+      // my ball's box in the top grid (pass A left it in B), and the union over the flagged queries
+      int tx0 = 0x7fffffff, tx1 = -1, ty0 = 0x7fffffff, ty1 = -1, tz0 = 0x7fffffff, tz1 = -1;
+      if (mine) {
+        tx0 = B.x0[lane]; tx1 = B.x1[lane]; ty0 = B.y0[lane]; ty1 = ty0 + B.ny[lane] - 1;
+        const double r = sqrt(B.best[lane]);
+        tz0 = B.z0[lane]; tz1 = cell_of(gTop, 2, B.qz[lane] + r + 1e-6 * gTop.h[2]);
+      }
+      const int ux0 = __reduce_min_sync(kFull, tx0), ux1 = __reduce_max_sync(kFull, tx1);
+      const int uy0 = __reduce_min_sync(kFull, ty0), uy1 = __reduce_max_sync(kFull, ty1);
+      const int uz0 = __reduce_min_sync(kFull, tz0), uz1 = __reduce_max_sync(kFull, tz1);
+      if ((ux1 - ux0 + 1) * (uy1 - uy0 + 1) * (uz1 - uz0 + 1) > 64) {
+        looseMask |= flagged;   // (the flagged queries are far apart: not worth a cell-by-cell visit)
+      } else {
+        GridIndex& v = warp_view();
+        for (int z = uz0; z <= uz1; ++z)
+          for (int y = uy0; y <= uy1; ++y) {
+            const int rowBase = (z * gTop.G[1] + y) * gTop.G[0];
+            // was this row left out for me in pass A?  (it holds a refined cell within my x range)
+            bool rowMine = mine && y >= ty0 && y <= ty1 && z >= tz0 && z <= tz1;
+            if (rowMine) rowMine = __ldg(&gTop.heavyPrefix[rowBase + tx1 + 1]) != __ldg(&gTop.heavyPrefix[rowBase + tx0]);
+            if (!__any_sync(kFull, rowMine)) continue;
+            for (int x = ux0; x <= ux1; ++x) {
+              bool p = rowMine && x >= tx0 && x <= tx1;
+              if (p) p = !(slab_d2(gTop, 0, B.qx[lane], x, x) + slab_d2(gTop, 1, B.qy[lane], y, y) + slab_d2(gTop, 2, B.qz[lane], z, z) > B.best[lane]);
+              const unsigned pm = __ballot_sync(kFull, p);
+              if (!pm) continue;
+              const int c = rowBase + x;
+              if (__ldg(&gTop.cellStart[c + 1]) == __ldg(&gTop.cellStart[c])) continue;   // an empty cell
+              __syncwarp();
+              if (lane == 0) {
+                const int so = __ldg(&gTop.subOff[c]);
+                if (so >= 0) {
+                  sub_view(gTop, x, y, z, so, v);
+                } else {   // a plain cell as a grid of one cell
+                  const int cc[3] = {x, y, z};
+                  for (int a = 0; a < 3; ++a) {
+                    v.lo[a] = gTop.lo[a] + cc[a] * gTop.h[a]; v.h[a] = gTop.h[a]; v.inv_h[a] = gTop.inv_h[a];
+                    v.hi[a] = v.lo[a] + gTop.h[a]; v.G[a] = 1;
+                  }
+                  v.n = 0; v.cellStart = gTop.cellStart + c; v.sites = gTop.sites;
+                  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
+                }
+              }
+              __syncwarp();
+              looseMask |= batch_pass<false>(v, B, nq, pm, st);   // (a ball of many sub-rows: the single-query path finishes it)
+            }
+          }
+      }
+    }
   }
+  st.queries += (unsigned)(nq - __popc(looseMask));
   if (gTop.countAlg) {
     // D_alg of the batched queries (the loose ones count inside nearest())
     unsigned v = 0;
@@ -165,6 +204,9 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
     v = (unsigned)warp_sum((int)v);
     extra_cnt_add(4, v);
   }
+#ifdef VD_COUNT_LOOSE
+  extra_cnt_add(3, (unsigned)__popc(looseMask));   // (experiment: reported as step_probes)
+#endif
   while (looseMask) {
     const int u = __ffs(looseMask) - 1;
     looseMask &= looseMask - 1;

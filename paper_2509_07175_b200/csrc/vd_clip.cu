@@ -1,6 +1,8 @@
 // vd_clip.cu -- S3 seeds, S4 clip kernels (one warp per (simplex, site) pair), S5 propagation through
 // the pair list.  Alg. 4 / Alg. 5 lines 15-27 as a wavefront over one growing
 // list: wave k processes the pairs pushed by wave k-1.
+#include <string.h>
+
 #include "vd_clip2d.cuh"
 #include "vd_clip3d.cuh"
 
@@ -60,7 +62,10 @@ __global__ void __launch_bounds__(kBlock) k_seed_points(ClipArgs A, int S, const
 
 // Simple domains (section V-B): a site inside the box owns its own position, so (box, v_i) is a non-empty pair
 // with witness v_i ("each site must be in its own Voronoi cell").
-__global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, double lx, double ly, double lz, double hx, double hy, double hz) {
+__global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, int ncorner) {
+  // the box's corners are the "mesh vertices": corner 0 = lo, the last = hi
+  const double lx = A.verts[0], ly = A.verts[1], lz = A.verts[2];
+  const double hx = A.verts[3 * (ncorner - 1) + 0], hy = A.verts[3 * (ncorner - 1) + 1], hz = A.verts[3 * (ncorner - 1) + 2];
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) {
     const double x = A.sites[i * 3 + 0], y = A.sites[i * 3 + 1], z = A.sites[i * 3 + 2];
     if (x >= lx && x <= hx && y >= ly && y <= hy && z >= lz && z <= hz) push_pair(A, 0, (int)i, x, y, z);
@@ -83,17 +88,34 @@ __global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ l
   }
 }
 
-vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end);   // vd_phase.cu
+// vd_phase.cu
+vd_status phase_buffers(vd_ctx* c, int64_t cap);
+void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int rounds, int tailPairs);
+PhaseCtl* phase_ctl(vd_ctx* c, int64_t cap);
 
 constexpr int kSmallWave = 8192;       // phased schedule: a wavefront smaller than this runs as one launch of the one-kernel form
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
 constexpr int K2 = 32, K2B = 256;
 
-// items: pairs[begin .. end) when list == nullptr, else pairs[list[begin .. end)]
+// The one-kernel form: a warp takes a pair through all of Alg. 3.  What it works on comes from the wave program's state
+// (k_wave_begin): fast tier -- the wave [pc->begin, + pc->count) (WAVE_SINGLE), or the whole list from the wave's first pair
+// on as a device-side queue (WAVE_QUEUE); large tier (BIG) -- the deferred pairs ovf[ovfBegin .. ovfEnd).
 template <int KIND, bool BIG, bool HV>
-__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, int64_t begin, int64_t end, bool persist) {
+__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, const PhaseCtl* __restrict__ pc) {
   constexpr int W = BIG ? 1 : kWarpsPerBlock;
+  int64_t begin, end;
+  bool persist = false;
+  if (BIG) {
+    begin = (int64_t)A.ctl->ovfBegin; end = (int64_t)A.ctl->ovfEnd;
+    if (begin >= end) return;
+  } else {
+    const unsigned mode = pc->mode;
+    if (mode != WAVE_QUEUE && mode != WAVE_SINGLE) return;
+    persist = mode == WAVE_QUEUE;
+    begin = persist ? 0 : (int64_t)pc->begin;     // queue: tickets are absolute list positions (the cursor starts at the wave)
+    end = (int64_t)pc->begin + (int64_t)pc->count;
+  }
   __shared__ GridIndex g;
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
@@ -238,40 +260,88 @@ vd_status stage_seed(vd_ctx* c) {
     VD_LAUNCH(k_seed_points, blocks_for(total, kBlock, sm_count() * 8), kBlock, 0, st)(A, S, c->seedPts.as<double>(), c->seedNN.as<int>());
   }
   if (boxKind) {
-    double cv[8 * 3];
-    cudaMemcpyAsync(cv, c->verts.p, sizeof(double) * 3 * c->nc, cudaMemcpyDeviceToHost, st);
-    sync_stream(c);
-    const double* lo = cv;
-    const double* hi = cv + 3 * (c->nc - 1);
-    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(A, lo[0], lo[1], lo[2], hi[0], hi[1], hi[2]);
+    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc);
   }
   return cuda_check(c, cudaGetLastError(), "seed");
 }
 
-template <int KIND, bool HV>
-static void launch_fast(vd_ctx* c, const ClipArgs& A, int64_t b, int64_t e, bool persist) {
-  const int blocks = persist ? sm_count() * 3 : blocks_for(e - b, kWarpsPerBlock, sm_count() * 6);
-  VD_LAUNCH((k_clip<KIND, false, HV>), blocks, kBlock, 0, c->stream)(A, nullptr, b, e, persist);
+// ---- wave programs: the wavefront loop of Alg. 4 / 5 ("while L1 is not empty") without the host -----------
+//
+// A wave program is a fixed sequence of launches: k_wave_begin looks at the pair list and decides what this wave is (nothing
+// / phased / queue drain / one launch of the one-kernel form), the kernels that follow read that decision and their counts
+// from device memory (PhaseCtl) and return at once when they have no work, k_wave_end closes the wave and hands the deferred
+// pairs to the large tier.  The host enqueues programs a batch at a time and looks at the device once per batch.
+
+// allowPhased: 3D kinds under the phased schedule; smallMode: what a wave below smallWave pairs (or any wave when
+// !allowPhased) runs as -- WAVE_QUEUE or WAVE_SINGLE.
+__global__ void k_wave_begin(ClipArgs A, PhaseCtl* pc, int allowPhased, int smallWave, int smallMode, long long chunkCap) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  Control* ctl = A.ctl;
+  pc->mode = WAVE_NONE; pc->count = 0; pc->nDone = 0;
+  for (int k = 0; k < kMaxRounds + 2; ++k) pc->nClip[k] = 0;
+  for (int k = 0; k < 2 * kMaxRounds + 4; ++k) pc->ticket[k] = 0;
+  if (ctl->err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP | ERR_DUPLICATE | ERR_INPUT)) return;   // the host reruns / reports
+  const unsigned long long begin = ctl->waveEnd;
+  unsigned long long tail = ctl->pairTail;
+  if (tail > (unsigned long long)A.pairCap) tail = (unsigned long long)A.pairCap;
+  if (tail <= begin) return;
+  unsigned long long n = tail - begin;
+  ctl->nWaves += 1;
+  pc->begin = begin;
+  if (allowPhased && n >= (unsigned long long)smallWave) {
+    if (n > (unsigned long long)chunkCap) n = (unsigned long long)chunkCap;   // a wave larger than the parking area runs in chunks
+    pc->mode = WAVE_PHASED;
+    ctl->waveEnd = begin + n;
+  } else if (smallMode == WAVE_QUEUE) {
+    pc->mode = WAVE_QUEUE;
+    ctl->fetch[0] = begin;       // next ticket = next list position
+    ctl->finished = begin;       // the queue is drained when every dispatched pair has finished and none is left
+    ctl->waveEnd = tail;         // (k_wave_end moves it to the final tail)
+  } else {
+    pc->mode = WAVE_SINGLE;
+    ctl->fetch[0] = 0;
+    ctl->waveEnd = tail;
+  }
+  pc->count = (unsigned)n;
 }
 
-template <int KIND, bool HV>
-static void launch_big(vd_ctx* c, const ClipArgs& A, int64_t ob, int64_t oe) {
-  VD_LAUNCH((k_clip<KIND, true, HV>), blocks_for(oe - ob, 1, sm_count() * 8), kLanes, 0, c->stream)(A, A.ovf, ob, oe, false);
+__global__ void k_wave_end(ClipArgs A, PhaseCtl* pc) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  Control* ctl = A.ctl;
+  if (pc->mode == WAVE_QUEUE) {
+    unsigned long long tail = ctl->pairTail;
+    if (tail > (unsigned long long)A.pairCap) tail = (unsigned long long)A.pairCap;
+    ctl->waveEnd = tail;         // the queue kernel ended: every pair pushed so far has been processed
+  }
+  unsigned long long ot = ctl->ovfTail;
+  if (ot > (unsigned long long)A.ovfCap) ot = (unsigned long long)A.ovfCap;
+  ctl->ovfBegin = ctl->ovfDone;
+  ctl->ovfEnd = ot;
+  ctl->ovfDone = ot;
+  ctl->fetch[1] = 0;
 }
 
 template <int KIND>
-static void launch_kind(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, int64_t e, bool persist) {
-  if (!big) { if (hv) launch_fast<KIND, true>(c, A, b, e, persist); else launch_fast<KIND, false>(c, A, b, e, persist); }
-  else      { if (hv) launch_big<KIND, true>(c, A, b, e); else launch_big<KIND, false>(c, A, b, e); }
+static void launch_kind(vd_ctx* c, const ClipArgs& A, bool hv, bool big, const PhaseCtl* pc) {
+  cudaStream_t st = c->stream;
+  if (!big) {
+    const int blocks = sm_count() * 3;
+    if (hv) VD_LAUNCH((k_clip<KIND, false, true>), blocks, kBlock, 0, st)(A, nullptr, pc);
+    else VD_LAUNCH((k_clip<KIND, false, false>), blocks, kBlock, 0, st)(A, nullptr, pc);
+  } else {
+    const int blocks = sm_count() * 8;
+    if (hv) VD_LAUNCH((k_clip<KIND, true, true>), blocks, kLanes, 0, st)(A, A.ovf, pc);
+    else VD_LAUNCH((k_clip<KIND, true, false>), blocks, kLanes, 0, st)(A, A.ovf, pc);
+  }
 }
 
 // one kernel per piece structure: triangles (both triangle kinds share the loop code), tets, rectangle, box
-static void launch(vd_ctx* c, const ClipArgs& A, bool hv, bool big, int64_t b, int64_t e, bool persist) {
+static void launch(vd_ctx* c, const ClipArgs& A, bool hv, bool big, const PhaseCtl* pc) {
   switch (c->kind) {
-    case KIND_TET_3D: launch_kind<KIND_TET_3D>(c, A, hv, big, b, e, persist); break;
-    case KIND_BOX_3D: launch_kind<KIND_BOX_3D>(c, A, hv, big, b, e, persist); break;
-    case KIND_BOX_2D: launch_kind<KIND_BOX_2D>(c, A, hv, big, b, e, persist); break;
-    default:          launch_kind<KIND_TRI_2D>(c, A, hv, big, b, e, persist); break;
+    case KIND_TET_3D: launch_kind<KIND_TET_3D>(c, A, hv, big, pc); break;
+    case KIND_BOX_3D: launch_kind<KIND_BOX_3D>(c, A, hv, big, pc); break;
+    case KIND_BOX_2D: launch_kind<KIND_BOX_2D>(c, A, hv, big, pc); break;
+    default:          launch_kind<KIND_TRI_2D>(c, A, hv, big, pc); break;
   }
 }
 
@@ -279,58 +349,66 @@ static cudaError_t read_control(vd_ctx* c, Control& h) {
   static_assert(sizeof(Control) <= 1024, "fits the page-locked staging block");
   Control* dst = c->pinned ? reinterpret_cast<Control*>(c->pinned) : &h;
   cudaError_t e = cudaMemcpyAsync(dst, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, c->stream);
-  if (e == cudaSuccess) e = sync_stream(c);
+  if (e == cudaSuccess) e = sync_stream(c, "wave batch");
   if (e == cudaSuccess && dst != &h) h = *dst;
   return e;
 }
 
-static void set_cursor(vd_ctx* c, int which, unsigned long long v) {
-  cudaMemcpyAsync(&c->control.as<Control>()->fetch[which], &v, sizeof(v), cudaMemcpyHostToDevice, c->stream);
-  sync_stream(c);   // v lives on the host stack
-}
-
 vd_status stage_clip(vd_ctx* c) {
   ClipArgs A = make_args(c);
+  A.queue = 1;   // a program may run the device-side queue: pushed pairs are published with a fence
   const int mode = c->opt.persistent;
   const bool solid = c->kind == KIND_TET_3D || c->kind == KIND_BOX_3D;
   const bool phased = solid && (mode == 1 || mode == 2);   // 3D kinds: one small kernel per step (vd_phase.cu)
-  // otherwise the one-kernel form: a device-side queue (3), or one launch per wave (0; and the default of the triangle
-  // kinds: with the discovery tuples and interior seeds their wavefronts are few, and the queue's polling costs more)
-  const bool persist = !phased && (mode == 3 || (mode == 2 && !solid));
-  A.queue = persist ? 1 : 0;
-  int64_t begin = 0, obegin = 0, waves = 0;
+  // waves that do not run phased: a device-side queue that drains everything (3; the short last wavefronts of the 3D
+  // kinds; 2 for the triangle kinds), or one launch of the one-kernel form per wavefront (0; the triangle kinds' default:
+  // with the discovery tuples and interior seeds their wavefronts are few, and the queue's polling costs more)
+  const int smallMode = (mode == 3 || (mode == 2 && !solid) || (phased && mode == 1 && c->opt.small_wave >= 0)) ? WAVE_QUEUE : WAVE_SINGLE;
+  const int smallWave = !phased ? 0 : (c->opt.small_wave == 0 ? kSmallWave : (c->opt.small_wave < 0 ? 1 : c->opt.small_wave));
+  const int tailPairs = c->opt.tail_pairs == 0 ? 65536 : (c->opt.tail_pairs < 0 ? 0 : c->opt.tail_pairs);
+  const int rounds = 5;
+  const int64_t chunk = (int64_t)1 << 20;
+  const int64_t cap = phased ? (c->pairCap < chunk ? c->pairCap : chunk) : 1;
+  vd_status s;
+  if ((s = phase_buffers(c, cap))) return s;
+  PhaseCtl* pc = phase_ctl(c, cap);
+  // refined cells of the index decide which kernels run (those that know the second level), and bad sites end the step
+  // here: one look at the device -- unless this context already built the index of these very sites
   Control h;
-  cudaError_t e = read_control(c, h);   // seeds pushed so far, refined cells of the index
-  if (e != cudaSuccess) return cuda_check(c, e, "clip");
-  const bool hv = h.nHeavy > 0;         // refined cells exist: the kernels that know the second index level
-  for (;;) {
+  cudaError_t e = cudaSuccess;
+  if (c->heavyKnown >= 0) {
+    memset(&h, 0, sizeof(h));
+    h.nHeavy = (unsigned)c->heavyKnown;
+    h.pairTail = 1;   // (unknown yet: the seeds)
+  } else {
+    if ((e = read_control(c, h)) != cudaSuccess) return cuda_check(c, e, "clip");
+    if (!(h.err & (ERR_DUPLICATE | ERR_INPUT))) c->heavyKnown = (int)h.nHeavy;
+  }
+  const bool hv = h.nHeavy > 0;
+  int batch = (!phased && smallMode == WAVE_SINGLE) ? 8 : 6;   // the seeds' wave and the large ones it sets off
+  for (int guard = 0; guard < 4096; ++guard) {
     if (h.err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) break;   // caller grows the pools and reruns
     if (h.err & (ERR_DUPLICATE | ERR_INPUT)) break;                   // bad sites (S1): nothing to clip
-    int64_t end = (int64_t)h.pairTail, oend = (int64_t)h.ovfTail;
-    if (end > c->pairCap) end = c->pairCap;
-    if (oend > c->ovfCap) oend = c->ovfCap;
-    if (end == begin && oend == obegin) break;   // "while L1 is not empty"
-    if (end > begin && phased && end - begin >= (c->opt.small_wave == 0 ? kSmallWave : c->opt.small_wave)) {
-      // phased mode: one small kernel per step of Alg. 3 over the whole wave (vd_phase.cu); a wave of a few thousand
-      // pairs (the last wavefronts) takes the branch below instead: one launch and one counter read, not a dozen
-      const vd_status s = run_phases(c, A, hv, begin, end);
-      if (s != VD_OK) return s;
-      ++waves;
-    } else if (end > begin) {
-      // wave mode: one launch per wavefront.  persistent mode: the kernel drains the queue as it grows
-      set_cursor(c, 0, persist ? (unsigned long long)begin : 0ull);
-      launch(c, A, hv, false, persist ? 0 : begin, end, persist);
-      ++waves;
-    } else if (oend > obegin) {
-      set_cursor(c, 1, 0ull);
-      launch(c, A, hv, true, obegin, oend, false);
-      obegin = oend;
+    unsigned long long tail = h.pairTail, otail = h.ovfTail;
+    if (tail > (unsigned long long)c->pairCap) tail = (unsigned long long)c->pairCap;
+    if (otail > (unsigned long long)c->ovfCap) otail = (unsigned long long)c->ovfCap;
+    if (h.waveEnd >= tail && h.ovfDone >= otail) break;               // "while L1 is not empty"
+    for (int k = 0; k < batch; ++k) {
+      VD_LAUNCH(k_wave_begin, 1, 32, 0, c->stream)(A, pc, phased ? 1 : 0, smallWave, smallMode, (long long)cap);
+      if (phased) enqueue_phased(c, A, hv, cap, rounds, tailPairs);
+      launch(c, A, hv, false, pc);
+      VD_LAUNCH(k_wave_end, 1, 32, 0, c->stream)(A, pc);
+      launch(c, A, hv, true, pc);
     }
     if ((e = read_control(c, h)) != cudaSuccess) return cuda_check(c, e, "clip wave");
-    if (end > begin) begin = persist ? (int64_t)h.finished : end;
+    phase_marks_collect(c);
+    // what is waiting now is the next wave, exactly: a large one will set off another, a short one is drained -- with all
+    // that follows from it -- by the queue kernel of a single program
+    const unsigned long long waiting = (h.pairTail < (unsigned long long)c->pairCap ? h.pairTail : (unsigned long long)c->pairCap) - h.waveEnd;
+    batch = (!phased && smallMode == WAVE_SINGLE) ? 8 : ((phased && waiting >= (unsigned long long)smallWave) ? 2 : 1);   // (a program of the triangle kinds is four launches)
   }
   c->hostControl = h;
-  c->counters.waves = waves;
+  c->counters.waves = (int64_t)h.nWaves;
   return cuda_check(c, cudaGetLastError(), "clip");
 }
 

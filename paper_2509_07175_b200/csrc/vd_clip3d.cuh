@@ -43,7 +43,7 @@ struct alignas(16) PolyTest3 {
   double cx[C], cy[C], cz[C];
   unsigned char cstate[C];
   int cnn[C];
-  int key[(sizeof(QBatch) + 11) / 12 + 1][3];   // scratch: the batch of queries
+  int key[(sizeof(QBatch) + 40 + 11) / 12 + 1][3];   // scratch: the batch of queries
 };
 
 // returns false when the three planes are (numerically) parallel to a common line
@@ -730,7 +730,7 @@ template <class PolyT, bool HV>
 __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st) {
   const int lane = lane_id();
   VD_POLY_REFS;
-  static_assert(sizeof(QBatch) <= sizeof(S.key), "the batch state must fit the scratch area");
+  static_assert(sizeof(QBatch) + 40 <= sizeof(S.key), "the batch state (and a plane behind it) must fit the scratch area");
   QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
   bool any = false;
   for (;;) {

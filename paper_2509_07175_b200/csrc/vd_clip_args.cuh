@@ -2,6 +2,7 @@
 #pragma once
 #include "vd_internal.h"
 #include "vd_nearest.cuh"
+#include "vd_batch.cuh"
 
 namespace vd {
 
@@ -33,6 +34,22 @@ struct ClipArgs {
 };
 
 enum { ST_UNKNOWN = 0, ST_IN = 1, ST_OUT = 2 };
+
+// State of one WAVE PROGRAM (vd_clip.cu): the fixed sequence of launches that processes one wavefront of pairs with no
+// host in between.  Its first kernel (k_wave_begin) looks at the pair list and decides what the wave is; every other
+// kernel of the program reads that decision, and the counts it needs, from here.
+constexpr int kMaxRounds = 6;
+enum { WAVE_NONE = 0,     // nothing to do (the list is exhausted, or an error is pending)
+       WAVE_PHASED = 1,   // 3D kinds: one kernel per step of Alg. 3, polytopes parked in HBM (vd_phase.cu)
+       WAVE_QUEUE = 2,    // the one-kernel form as a device-side queue: drains this wave and everything it discovers
+       WAVE_SINGLE = 3 }; // the one-kernel form over exactly this wave
+struct PhaseCtl {
+  unsigned mode, count;             // WAVE_*, pairs of this wave (phased: at most the parking capacity)
+  unsigned long long begin;         // first pair of the wave in the pair list
+  unsigned nDone, pad;
+  unsigned nClip[kMaxRounds + 2];   // pairs with a corner outside after the tests of round r
+  unsigned ticket[2 * kMaxRounds + 4];   // one work cursor per launch of the program
+};
 
 struct LocalCnt {
   unsigned pairs, pieces, search_iters, clips, search_evals, pre_clips;
@@ -315,6 +332,40 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
   return true;
 }
 
+// Improved search of section VI-A (Fig. 8): before the search on a long segment p_s p_t, step out from p_s in
+// multiples of delta_i (S1b): g = p_s + lambda delta_i dir, lambda = 2, 3, ... (stepMode 2: lambda doubles), while
+// g is still in Omega_i; the first g outside, with its nearest site, replaces p_t -- the search then runs on the short
+// segment p_s g.  g never passes p_t (reading U7); a probe that meets the end of the segment leaves p_t as it is.  Coordinates
+// local to o = u[0..2]; the new end point and its site come back through pt[3] / j.  Returns the number of probes.
+template <bool HV>
+static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, const double* u, double psx, double psy, double psz, double* pt,
+                                            const int* flags, int nflags, QueryStats& st) {
+  const double delta = __ldg(&g.delta[i]);
+  const double sx = pt[0] - psx, sy = pt[1] - psy, sz = pt[2] - psz;
+  const double len = sqrt(sx * sx + sy * sy + sz * sz);
+  int probes = 0;
+  if (!(delta > 0.0) || !(len > 2.0 * delta)) return 0;
+  const double inv = 1.0 / len;
+  double lambda = 2.0;
+  for (int k = 0; k < 64; ++k) {
+    const double s = lambda * delta;
+    if (!(s < len)) break;
+    const double gx = psx + sx * inv * s, gy = psy + sy * inv * s, gz = psz + sz * inv * s;
+    const double ax = gx + u[0], ay = gy + u[1], az = gz + u[2];
+    const double dx = ax - u[3], dy = ay - u[4], dz = az - u[5];
+    const double di2 = dx * dx + dy * dy + dz * dz;
+    double best = di2;
+    int bestId = i;
+    nearest<HV>(g, ax, ay, az, best, bestId, st, true);
+    probes += 1;
+    bool outside = bestId != i && best < di2 * (1.0 - 1e-9);   // clearly nearer to another site (U8): g has left Omega_i
+    if (outside) { pt[0] = gx; pt[1] = gy; pt[2] = gz; j = bestId; break; }
+    lambda = g.stepMode == 1 ? lambda + 1.0 : lambda * 2.0;
+  }
+  (void)flags; (void)nflags;
+  return probes;
+}
+
 // Edge-based bisector search (section IV-B) on the segment p_s -> p_t, all in coordinates
 // local to the origin o.  p_s is in Omega_i, the nearest site of p_t is j != i.  Iterates
 // q = B_ij ∩ segment, k = N_q, until k is i or j; then B_ij is the target bisector.  Along the segment
@@ -330,9 +381,14 @@ template <bool HV>
 static __device__ __noinline__ int find_bisector_impl(const double* __restrict__ sites, int ballCells, const GridIndex& g, int i, int j,
                                              const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
                                              double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
-                                             double* out4, QueryStats& st, unsigned& iters) {
+                                             double* out4, QBatch* qb, QueryStats& st, unsigned& iters) {
   const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
   double nx, ny, nz, d;
+  if (g.stepMode) {   // section VI-A (vd_options.step_out): shorten the segment first
+    double pt[3] = {ptx, pty, ptz};
+    const int probes = step_out<HV>(g, i, j, u, psx, psy, psz, pt, flags, nflags, st);
+    if (probes) { ptx = pt[0]; pty = pt[1]; ptz = pt[2]; extra_cnt_add(3, (unsigned)probes); }
+  }
   for (int it = 0; it < 96; ++it) {
     iters += 1;
     const double vjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
@@ -350,7 +406,7 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
-    if (ballCells > 0) {
+    if (!HV && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
       // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
       double tb = 2.0;
       int jb = 0x7fffffff;
@@ -371,7 +427,18 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
-    nearest<HV>(g, ax, ay, az, best, bestId, st, true);
+    if (HV && qb) {
+      // refined index: the query as a batch of one -- the cell-by-cell pass over sub-grids (vd_batch.cuh) instead of the
+      // general single-query search
+      if (lane_id() == 0) { qb->qx[0] = ax; qb->qy[0] = ay; qb->qz[0] = az; qb->best[0] = best; qb->bestId[0] = bestId; }
+      __syncwarp();
+      batch_nearest<HV>(g, *qb, 1, st);
+      __syncwarp();
+      best = qb->best[0]; bestId = qb->bestId[0];
+      __syncwarp();
+    } else {
+      nearest<HV>(g, ax, ay, az, best, bestId, st, true);
+    }
 #ifdef VD_TRACE
     if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
 #endif
@@ -402,12 +469,16 @@ __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex&
   unsigned iters = 0;
   int r;
   if (scratch4) {
-    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, scratch4, st, iters);
+    // the scratch area holds the batch state of the point-in-cell tests; the plane comes back through its last 32 bytes
+    QBatch* qb = reinterpret_cast<QBatch*>(scratch4);
+    double* out4 = scratch4 + (sizeof(QBatch) + 7) / 8;
+    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out4, qb, st, iters);
+    scratch4 = out4;
     nx = scratch4[0]; ny = scratch4[1]; nz = scratch4[2]; d = scratch4[3];
   } else {
     // every lane writes its own copy
     double out[4] = {0, 0, 0, 0};
-    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out, st, iters);
+    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out, nullptr, st, iters);
     nx = __shfl_sync(kFull, out[0], 0); ny = __shfl_sync(kFull, out[1], 0); nz = __shfl_sync(kFull, out[2], 0); d = __shfl_sync(kFull, out[3], 0);
   }
   lc.search_iters += iters;

@@ -51,6 +51,9 @@ struct GridIndex {
   const int* __restrict__ subOff;         // [G0*G1*G2] (K << 26) | offset into subStart, or -1
   const int* __restrict__ subStart;
   int countAlg;                           // vd_options.count_alg: queries also count D_alg (measurement runs)
+  // S1b: delta_i = half the distance from v_i to its nearest other site, for the step-out of section VI-A
+  const double* __restrict__ delta;       // [n] by original site id, or null (vd_options.step_out = 0)
+  int stepMode;                           // 1: lambda = 2, 3, 4, ...; 2: lambda doubles
 };
 
 constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)

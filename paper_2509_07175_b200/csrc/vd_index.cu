@@ -48,7 +48,8 @@ __global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restric
 // One thread: final box, grid resolution ("each grid cell contains, on average, 2~3 / 3~4 sites":
 // average over all cells of the sites' box -- reading U9), header written to device memory.
 __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64_t n, double density, int64_t gridCap,
-                              const int* cellStart, const double4* sorted, int countAlg, GridIndex* g, unsigned int* err) {
+                              const int* cellStart, const double4* sorted, int countAlg, const double* delta, int stepMode,
+                              GridIndex* g, unsigned int* err) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
   for (int k = 0; k < nparts; ++k)
@@ -91,6 +92,8 @@ __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64
   out.subOff = nullptr;
   out.subStart = nullptr;
   out.countAlg = countAlg;
+  out.delta = delta;
+  out.stepMode = stepMode;
   *g = out;
 }
 
@@ -274,6 +277,28 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
   }
 }
 
+// S1b: delta_i = || N_i - v_i || / 2, N_i the site nearest to v_i other than v_i itself -- one warp per site, the
+// nearest-site query of S2 with the site's own record skipped.  The ball (v_i, delta_i) lies inside Omega_i; the step-out of
+// section VI-A advances in multiples of it.
+__global__ void __launch_bounds__(kBlock) k_delta(const GridIndex* __restrict__ gp, const double* __restrict__ sites3, int64_t n,
+                                                   double* __restrict__ delta, Counters* cnt) {
+  const GridIndex g = *gp;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
+  QueryStats st = {0u, 0u, 0u, 0};
+  for (int64_t i = warp; i < n; i += nwarps) {
+    double best = 2e300;
+    int bestId = 0x7fffffff;
+    st.skip = (int)i;
+    nearest<true, true>(g, sites3[i * 3 + 0], sites3[i * 3 + 1], sites3[i * 3 + 2], best, bestId, st);
+    if (lane_id() == 0) delta[i] = best < 1e300 ? 0.5 * sqrt(best) : 1e300;   // n = 1: no other site
+  }
+  if (lane_id() == 0 && cnt) {
+    atomicAdd(&cnt->queries, (unsigned long long)st.queries);
+    atomicAdd(&cnt->dist_evals, (unsigned long long)st.dist_evals);
+  }
+}
+
 static int grid_for(int64_t items, int perBlock) {
   int64_t b = (items + perBlock - 1) / perBlock;
   const int64_t cap = sm_count() * 16;
@@ -296,11 +321,14 @@ vd_status stage_index(vd_ctx* c) {
   if ((s = ensure(c, c->sorted, sizeof(double4) * n))) return s;
   if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(n > gridCap ? n : gridCap) * 2))) return s;
   if ((s = ensure(c, c->control, sizeof(Control)))) return s;
+  const int stepMode = c->opt.step_out > 0 ? (c->opt.step_out > 2 ? 2 : c->opt.step_out) : 0;
+  if (stepMode && (s = ensure(c, c->delta, sizeof(double) * n))) return s;
   cudaStream_t st = c->stream;
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
-                                         c->sorted.as<double4>(), c->opt.count_alg > 0 ? 1 : 0, c->grid.as<GridIndex>(),
+                                         c->sorted.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
+                                         stepMode ? c->delta.as<double>() : nullptr, stepMode, c->grid.as<GridIndex>(),
                                          &c->control.as<Control>()->err);
   cudaMemsetAsync(c->cellFill.p, 0, sizeof(int) * (gridCap + 2), st);
   VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
@@ -340,6 +368,9 @@ vd_status stage_index(vd_ctx* c) {
   VD_LAUNCH(k_grid_finish, 1, 1, 0, st)(gp, c->sorted2.as<double4>(), c->heavyPrefix.as<int>(), c->subOff.as<int>(),
                                          c->subStart.as<int>(), &c->control.as<Control>()->nHeavy);
   VD_LAUNCH(k_find_duplicates, grid_for(n, kBlock), kBlock, 0, st)(gp, n, &c->control.as<Control>()->err);
+  if (stepMode)   // S1b
+    VD_LAUNCH(k_delta, grid_for(n, kWarpsPerBlock), kBlock, 0, st)(gp, c->sites.as<double>(), n, c->delta.as<double>(),
+                                                                   &c->control.as<Control>()->cnt[CNT_OTHER]);
   c->indexValid = true;
   return cuda_check(c, cudaGetLastError(), "site index");
 }

@@ -1,6 +1,7 @@
 // vd_internal.h -- the context behind the C ABI (include/vd.h) and the stage entry points.
 #pragma once
 #include <string>
+#include <vector>
 
 #include "../../include/vd.h"
 #include "vd_common.cuh"
@@ -19,6 +20,11 @@ struct Control {
   unsigned int nHeavy;           // refined cells of the site index (second level)
   Counters cnt[kCntKinds];       // per kernel kind (CNT_*): k_ph_init, verify, fix, finish, tail, everything else
   unsigned long long nPieces, nNonEmpty, nVerts, nNbrs;   // totals written by S6
+  // wave programs (vd_clip.cu): the wavefronts of Alg. 4 / 5 advance on the device
+  unsigned long long waveEnd;    // pairs [0, waveEnd) of the list have been dispatched to a wave
+  unsigned long long ovfDone;    // deferred pairs [0, ovfDone) have been dispatched to the large tier
+  unsigned long long ovfBegin, ovfEnd;   // the large tier's range in the current program
+  unsigned long long nWaves;     // non-empty wavefronts so far
   unsigned int nListed, padListed;                        // S6: non-empty sites listed for the warp-per-site kernels
 };
 
@@ -45,6 +51,7 @@ struct vd_ctx {
   bool weighted = false;   // vd_create_weighted: dim 2 -> sites lifted to R^3, VD_TRI_2D runs as a flat surface;
                            //                     dim 3 -> siteW holds the additive term eta - w_i of every site
   int64_t syncs = 0;       // host waits on the stream inside the current vd_compute
+  int heavyKnown = -1;     // refined cells of the site index as last built, while sites and grid options are unchanged; else -1
   bool haveDomain = false, haveResult = false, indexValid = false;
   cudaStream_t stream = nullptr;
   void* (*allocFn)(size_t, void*, void*) = nullptr;
@@ -55,7 +62,11 @@ struct vd_ctx {
   vd_counters phaseCounters[6] = {};   // per kernel kind (vd_get_phase_counters)
   double stageMs[5] = {0, 0, 0, 0, 0};
   double phaseMs[5] = {0, 0, 0, 0, 0};
-  cudaEvent_t phaseEv[4] = {nullptr, nullptr, nullptr, nullptr};
+  // device times of the step kernels: an event before every launch of a wave program, read after the batch's one
+  // synchronisation (the interval that starts at event k belongs to step kernel evKind[k]; -1: not a step kernel)
+  std::vector<cudaEvent_t> evPool;
+  std::vector<int> evKind;
+  int evUsed = 0;
   std::string lastError;
   cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
 
@@ -74,6 +85,7 @@ struct vd_ctx {
   vd::DevBuf cellStart;   // int [gridCap+1]
   vd::DevBuf cellFill;    // int [gridCap+1]
   vd::DevBuf sorted;      // double4 [n]
+  vd::DevBuf delta;       // double [n]  S1b: half the distance to the nearest other site (vd_options.step_out)
   vd::DevBuf scanTmp;     // scan scratch
   vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart, subKey, sorted2;   // second level
   int64_t subCap = 0;
@@ -111,12 +123,15 @@ struct vd_ctx {
 namespace vd {
 
 int sm_count();   // multiprocessors of the current device (cudaDevAttrMultiProcessorCount, cached): launch grids are multiples of it
-cudaError_t sync_stream(vd_ctx* c);   // cudaStreamSynchronize on the context's stream, counted (vd_counters.syncs)
+cudaError_t sync_stream(vd_ctx* c, const char* why = nullptr);   // cudaStreamSynchronize on the context's stream, counted (vd_counters.syncs)
 
 // memory
 vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes);
 void release(vd_ctx* c, DevBuf& b);
 vd_status cuda_check(vd_ctx* c, cudaError_t e, const char* what);
+
+void phase_mark(vd_ctx* c, int kind);      // record the next event of the pool; the launches up to the next mark are `kind`
+void phase_marks_collect(vd_ctx* c);       // after a synchronisation: add the intervals to c->phaseMs, reset the pool
 
 // stages (each enqueues kernels on c->stream)
 vd_status stage_domain(vd_ctx* c);                 // S0  vd_domain.cu

@@ -8,6 +8,7 @@ namespace vd {
 
 struct QueryStats {
   unsigned queries, dist_evals, rows;
+  int skip;   // SKIP instantiations only (S1b): the site id that does not count as a candidate
 };
 
 // Work counters that are bumped rarely (per clip, per piece, per measurement-mode query) live in shared memory, one row
@@ -43,13 +44,14 @@ __device__ __forceinline__ double slab_d2(const GridIndex& g, int ax, double q, 
 // range per row.  The candidates of all rows are then packed 32 at a time over the lanes (prefix sum of
 // the row counts; the row that owns candidate t is found from a bit mask of row starts), so a typical
 // query of ~30 candidates in 4-9 rows costs one round of distance evaluations instead of one per row.
+template <bool SKIP>
 static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
                                               int& bestId, QueryStats& st);
 
 // TOP = true: g is the site index itself and may hold refined cells (second level); a row that contains
 // one is walked cell by cell afterwards: plain cells are scanned as they are, a refined cell through its
 // own sub-grid (the same routine with TOP = false on a view of that cell).
-template <bool TOP>
+template <bool TOP, bool SKIP = false>
 static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0, int y1,
                                       int z0, int z1, double& best, int& bestId, QueryStats& st) {
   __shared__ int sBase[kWarpsPerBlock][kLanes];
@@ -110,7 +112,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         d2 = dx * dx + dy * dy + dz * dz;
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       }
-      const bool better = valid && closer(d2, id, best, bestId);
+      const bool better = valid && closer(d2, id, best, bestId) && !(SKIP && id == st.skip);
       if (__any_sync(kFull, better)) {
         if (!better) { d2 = best; id = bestId; }
         warp_argmin(d2, id);
@@ -127,7 +129,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         const int rr = r0 + src;
         const int y = y0 + rr % ny, z = z0 + rr / ny;
         const int xa = shfl(hxa, src), xb = shfl(hxb, src);
-        for (int x = xa; x <= xb; ++x) scan_cell(g, x, y, z, qx, qy, qz, best, bestId, st);
+        for (int x = xa; x <= xb; ++x) scan_cell<SKIP>(g, x, y, z, qx, qy, qz, best, bestId, st);
       }
     }
   }
@@ -171,18 +173,19 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
   v.n = 0;
   v.cellStart = g.subStart + (so & 0x3ffffff);
   v.sites = g.sites;
-  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0;
+  v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
 }
 
 // One cell of the top grid: a plain cell is scanned directly, a refined cell through its sub-grid,
 // restricted to the ball (q, sqrt(best)).
+template <bool SKIP>
 static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
                                               int& bestId, QueryStats& st) {
   const int c = (z * g.G[1] + y) * g.G[0] + x;
   if (slab_d2(g, 0, qx, x, x) + slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z) > best) return;
   const int so = __ldg(&g.subOff[c]);
   if (so < 0) {
-    scan_box<false>(g, qx, qy, qz, x, x, y, y, z, z, best, bestId, st);   // plain cell: a 1 x 1 x 1 box of the top grid
+    scan_box<false, SKIP>(g, qx, qy, qz, x, x, y, y, z, z, best, bestId, st);   // plain cell: a 1 x 1 x 1 box of the top grid
     return;
   }
   GridIndex& v = warp_view();
@@ -196,7 +199,7 @@ static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, 
     vy0 = cell_of(v, 1, qy - r - 1e-6 * v.h[1]); vy1 = cell_of(v, 1, qy + r + 1e-6 * v.h[1]);
     vz0 = cell_of(v, 2, qz - r - 1e-6 * v.h[2]); vz1 = cell_of(v, 2, qz + r + 1e-6 * v.h[2]);
   }
-  scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
+  scan_box<false, SKIP>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
 }
 
 // D_alg: the sites stored in the grid cells (sub-cells of refined cells) that meet the ball (q, sqrt(r2)) --
@@ -247,21 +250,21 @@ static __device__ __noinline__ unsigned ball_sites(const GridIndex& g, double qx
 // corner that is outside Omega_i, an intermediate step of the bisector search): the routine then returns as
 // soon as the cells around q have produced one, without proving it the nearest (reading U17).  When no
 // site is clearly nearer, the full scan runs and the answer is exact, so acceptance is always exact.
-template <bool HV>
+template <bool HV, bool SKIP>
 static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                              QueryStats& st, bool nearer_ok);
 
-template <bool HV>
+template <bool HV, bool SKIP = false>
 __device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                         QueryStats& st, bool nearer_ok = false) {
-  nearest_impl<HV>(g, qx, qy, qz, best, bestId, st, nearer_ok);
+  nearest_impl<HV, SKIP>(g, qx, qy, qz, best, bestId, st, nearer_ok);
   if (g.countAlg) {
     if (lane_id() == 0) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][4] += ball_sites(g, qx, qy, qz, best);
     __syncwarp();
   }
 }
 
-template <bool HV>
+template <bool HV, bool SKIP>
 static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                              QueryStats& st, bool nearer_ok) {
   const double bound0 = best;
@@ -291,13 +294,13 @@ static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, 
           const int vy0 = cell_of(v, 1, qy - r - 1e-6 * v.h[1]), vy1 = cell_of(v, 1, qy + r + 1e-6 * v.h[1]);
           const int vz0 = cell_of(v, 2, qz - r - 1e-6 * v.h[2]), vz1 = cell_of(v, 2, qz + r + 1e-6 * v.h[2]);
           if (in && (vy1 - vy0 + 1) * (vz1 - vz0 + 1) <= kLanes) {
-            scan_box<false>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
+            scan_box<false, SKIP>(v, qx, qy, qz, vx0, vx1, vy0, vy1, vz0, vz1, best, bestId, st);
             return;
           }
         }
         if (pass == 0) {
           const int hx = cell_of(v, 0, qx), hy = cell_of(v, 1, qy), hz = cell_of(v, 2, qz);
-          scan_box<false>(v, qx, qy, qz, max(hx - 1, 0), min(hx + 1, v.G[0] - 1), max(hy - 1, 0), min(hy + 1, v.G[1] - 1),
+          scan_box<false, SKIP>(v, qx, qy, qz, max(hx - 1, 0), min(hx + 1, v.G[0] - 1), max(hy - 1, 0), min(hy + 1, v.G[1] - 1),
                           max(hz - 1, 0), min(hz + 1, v.G[2] - 1), best, bestId, st);
           if (nearer_ok && best < bound0 * (1.0 - 1e-9)) return;
         }
@@ -374,7 +377,7 @@ static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, 
             bx0 = x; bx1 = x; by0 = yi0; by1 = yi1; bz0 = zi0; bz1 = zi1;
           }
         }
-        if (ok) scan_box<HV>(g, qx, qy, qz, bx0, bx1, by0, by1, bz0, bz1, sb, si, st);
+        if (ok) scan_box<HV, SKIP>(g, qx, qy, qz, bx0, bx1, by0, by1, bz0, bz1, sb, si, st);
       };
       if constexpr (HV) {
         const int nf = s == 0 ? 1 : 6;
@@ -394,7 +397,7 @@ static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, 
   const int x0 = cell_of(g, 0, qx - r - 1e-6 * g.h[0]), x1 = cell_of(g, 0, qx + r + 1e-6 * g.h[0]);
   const int y0 = cell_of(g, 1, qy - r - 1e-6 * g.h[1]), y1 = cell_of(g, 1, qy + r + 1e-6 * g.h[1]);
   const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
-  scan_box<HV>(g, qx, qy, qz, x0, x1, y0, y1, z0, z1, best, bestId, st);
+  scan_box<HV, SKIP>(g, qx, qy, qz, x0, x1, y0, y1, z0, z1, best, bestId, st);
 }
 
 }  // namespace vd

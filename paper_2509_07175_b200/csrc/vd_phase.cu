@@ -41,10 +41,6 @@ static_assert(kTestBytes % 16 == 0 && kPolyBytes % 16 == 0, "copied in 16-byte w
 static_assert(offsetof(PolyT, key) == kTestBytes && offsetof(PolyT, cnn) == offsetof(PolyF, cnn) && offsetof(PolyT, cstate) == offsetof(PolyF, cstate),
               "PolyTest3 mirrors the head of Poly3");
 
-struct PhaseCtl {
-  unsigned ticket, nClip, nDone, pad;
-};
-
 // warp copy in 16-byte words, eight (then four) loads in flight per lane
 __device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes) {
   const uint4* s = reinterpret_cast<const uint4*>(src);
@@ -65,9 +61,9 @@ __device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes
   for (; k < n; k += kLanes) d[k] = s[k];
 }
 
-__device__ __forceinline__ int next_item(PhaseCtl* pc, int count) {
+__device__ __forceinline__ int next_item(PhaseCtl* pc, int slot, int count) {
   unsigned t = 0;
-  if (lane_id() == 0) t = atomicAdd(&pc->ticket, 1u);
+  if (lane_id() == 0) t = atomicAdd(&pc->ticket[slot], 1u);
   t = shfl(t, 0);
   return t < (unsigned)count ? (int)t : -1;
 }
@@ -80,14 +76,17 @@ __device__ __forceinline__ void defer_pair(const ClipArgs& A, int64_t idx) {
 }
 
 template <bool BOX>
-__global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __restrict__ cells, int64_t begin, int count, PhaseCtl* pc) {
+__global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __restrict__ cells, PhaseCtl* pc) {
+  if (pc->mode != WAVE_PHASED) return;
+  const int64_t begin = (int64_t)pc->begin;
+  const int count = (int)pc->count;
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   for (;;) {
-    const int t = next_item(pc, count);
+    const int t = next_item(pc, 0, count);
     if (t < 0) break;
     const Pair pr = load_pair(A, begin + t);
     int np, nc;
@@ -105,10 +104,18 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
   flush_counters(A.ctl, st, lc, CNT_INIT);
 }
 
-// list == nullptr: items 0 .. count-1; a negative list entry is a pair that left the path
+// Round r of a phased wave (lists[r & 1] receives the pairs that still have a corner outside).  Round 0 tests every pair of
+// the wave; round r > 0 the pairs that round r-1's k_ph_fix clipped -- it runs only if that kernel ran.  A negative list
+// entry is a pair that left the path.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
-                                                     int* __restrict__ clipList, int* __restrict__ doneList, PhaseCtl* pc) {
+__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
+                                                     int* __restrict__ doneList, PhaseCtl* pc, int r, int tailPairs) {
+  if (pc->mode != WAVE_PHASED) return;
+  if (r > 0 && (int)pc->nClip[r - 1] <= tailPairs) return;
+  const int* list = r > 0 ? lists + ((r - 1) & 1) * (int64_t)cap : nullptr;
+  const int count = r > 0 ? (int)pc->nClip[r - 1] : (int)pc->count;
+  int* clipList = lists + (r & 1) * (int64_t)cap;
+  const int slot = 4 + 2 * r;
   __shared__ GridIndex g;
   __shared__ PolyT S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -118,11 +125,11 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   for (;;) {
-    const int t = next_item(pc, count);
+    const int t = next_item(pc, slot, count);
     if (t < 0) break;
-    const int slot = list ? list[t] : t;
-    if (slot < 0) continue;
-    CellState* c = &cells[slot];
+    const int item = list ? list[t] : t;
+    if (item < 0) continue;
+    CellState* c = &cells[item];
     const int np = c->np, nc = c->nc;
     if (np < 0) continue;
     bool out = false;
@@ -138,8 +145,8 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
       }
     }
     if (lane == 0) {
-      if (out) clipList[atomicAdd(&pc->nClip, 1u)] = slot;
-      else doneList[atomicAdd(&pc->nDone, 1u)] = slot;
+      if (out) clipList[atomicAdd(&pc->nClip[r], 1u)] = item;
+      else doneList[atomicAdd(&pc->nDone, 1u)] = item;
     }
     __syncwarp();
   }
@@ -148,9 +155,15 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
 
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
+// Runs when round r's tests left more than tailPairs pairs with a corner outside (fewer: k_ph_tail finishes them).
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ list, int count,
-                                                     int64_t begin, PhaseCtl* pc) {
+__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
+                                                     PhaseCtl* pc, int r, int tailPairs) {
+  if (pc->mode != WAVE_PHASED || (int)pc->nClip[r] <= tailPairs) return;
+  int* list = lists + (r & 1) * (int64_t)cap;
+  const int count = (int)pc->nClip[r];
+  const int64_t begin = (int64_t)pc->begin;
+  const int tslot = 5 + 2 * r;
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -160,7 +173,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   for (;;) {
-    const int t = next_item(pc, count);
+    const int t = next_item(pc, tslot, count);
     if (t < 0) break;
     const int slot = list[t];
     CellState* c = &cells[slot];
@@ -193,9 +206,20 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
 // instead of one round trip to the host and two nearly empty launches per remaining round.  Finished pairs join the
 // done list.  The whole loop in one kernel is the instruction-fetch-bound form (header of this file); on a few
 // thousand pairs that does not matter.
+// One launch after the program's rounds.  The rounds stop at the first round r whose tests leave at most tailPairs pairs with
+// a corner outside: those pairs (tested, not clipped) are taken to completion here.  If every round ran its clips, the last
+// round's pairs (clipped, not yet re-tested) are -- so a wave always ends, whatever the number of rounds in the program.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
-                                                       int64_t begin, int* __restrict__ doneList, PhaseCtl* pc) {
+__global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ lists, int cap,
+                                                       int* __restrict__ doneList, PhaseCtl* pc, int rounds, int tailPairs) {
+  if (pc->mode != WAVE_PHASED) return;
+  int r = 0;
+  while (r < rounds - 1 && (int)pc->nClip[r] > tailPairs) ++r;
+  const int count = (int)pc->nClip[r];
+  if (count == 0) return;
+  const int* list = lists + (r & 1) * (int64_t)cap;
+  const int64_t begin = (int64_t)pc->begin;
+  const int tslot = 3;
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -205,9 +229,10 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   for (;;) {
-    const int t = next_item(pc, count);
+    const int t = next_item(pc, tslot, count);
     if (t < 0) break;
     const int slot = list[t];
+    if (slot < 0) continue;   // (the fix kernel marked a pair that left the path)
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
     const int i = c->i;
@@ -236,8 +261,11 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
   flush_counters(A.ctl, st, lc, CNT_TAIL);
 }
 
-__global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, int count,
-                                                     int64_t begin, int vchunk, int nchunk) {
+__global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ list, const PhaseCtl* pc,
+                                                     int vchunk, int nchunk) {
+  if (pc->mode != WAVE_PHASED) return;
+  const int count = (int)pc->nDone;
+  const int64_t begin = (int64_t)pc->begin;
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes;
   QueryStats st = {0u, 0u, 0u};
@@ -257,100 +285,48 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
   flush_counters(A.ctl, st, lc, CNT_FINISH);
 }
 
-static vd_status reset_ctl(vd_ctx* c, PhaseCtl* pc, bool all) {
-  return cuda_check(c, cudaMemsetAsync(pc, 0, all ? sizeof(PhaseCtl) : sizeof(unsigned) * 2, c->stream), "phase ctl");
-}
-
-// One wave: pairs [begin, end) of the pair list, all of one 3D kind.  Every launch is bracketed by two events;
-// the elapsed times are read after the round's synchronisation (vd_get_phase_ms).
-vd_status run_phases(vd_ctx* c, const ClipArgs& A, bool hv, int64_t begin, int64_t end) {
-  const int64_t chunk = (int64_t)1 << 20;
-  const int64_t cap = end - begin < chunk ? end - begin : chunk;
+// The step kernels of ONE wave program, enqueued without looking at the device: `rounds` rounds of {tests, then clips
+// or -- for a short list -- the finishing kernel}, one more finishing launch for what the last round's clips left, and
+// the finish kernel.  Every kernel decides from PhaseCtl whether it has work (a launch without work costs ~3 us); the
+// wave's size, its lists and its counters never visit the host (the paper's host loop is P:L257, L325).
+vd_status phase_buffers(vd_ctx* c, int64_t cap) {
   vd_status s;
   if ((s = ensure(c, c->phaseCells, sizeof(CellState) * (size_t)cap))) return s;
-  if ((s = ensure(c, c->phaseLists, sizeof(int) * 3 * (size_t)cap + sizeof(PhaseCtl)))) return s;
-  for (cudaEvent_t& e : c->phaseEv)
-    if (!e && cudaEventCreate(&e) != cudaSuccess) return cuda_check(c, cudaGetLastError(), "phase events");
-  CellState* cells = c->phaseCells.as<CellState>();
-  int* listA = c->phaseLists.as<int>();
-  int* listB = listA + cap;
-  int* done = listB + cap;
-  PhaseCtl* pc = reinterpret_cast<PhaseCtl*>(done + cap);
-  cudaStream_t st = c->stream;
-  cudaEvent_t* ev = c->phaseEv;
-  const int grid = sm_count() * 4;
-  const int tailPairs = c->opt.tail_pairs == 0 ? kTailPairs : c->opt.tail_pairs;   // < 0: never
-  auto elapsed = [&](int which, cudaEvent_t a, cudaEvent_t b) {
-    float ms = 0.f;
-    if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) c->phaseMs[which] += ms;
-  };
-  auto read_ctl = [&](PhaseCtl& h) -> cudaError_t {
-    // through page-locked memory: a copy into pageable memory is staged by the driver (tens of microseconds, once per round)
-    PhaseCtl* dst = c->pinned ? reinterpret_cast<PhaseCtl*>(c->pinned) : &h;
-    cudaError_t e = cudaMemcpyAsync(dst, pc, sizeof(h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = sync_stream(c);
-    if (e == cudaSuccess && dst != &h) h = *dst;
-    return e;
-  };
-  for (int64_t b = begin; b < end; b += chunk) {
-    const int count = (int)((end - b) < chunk ? (end - b) : chunk);
-    if ((s = reset_ctl(c, pc, true))) return s;
-    cudaEventRecord(ev[0], st);
-    if (c->kind == KIND_BOX_3D) VD_LAUNCH(k_ph_init<true>, grid, kBlock, 0, st)(A, cells, b, count, pc);
-    else VD_LAUNCH(k_ph_init<false>, grid, kBlock, 0, st)(A, cells, b, count, pc);
-    cudaEventRecord(ev[1], st);
-    const int* cur = nullptr;
-    int curCount = count;
-    int* clip = listA;
-    int* other = listB;
-    bool initTimed = false, fixPending = false;
-    PhaseCtl h;
-    for (int round = 0; round < 4 * P3; ++round) {
-      if ((s = reset_ctl(c, pc, false))) return s;   // ticket and nClip; nDone keeps growing
-      cudaEventRecord(ev[2], st);
-      if (hv) VD_LAUNCH(k_ph_verify<true>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
-      else VD_LAUNCH(k_ph_verify<false>, grid, kBlock, 0, st)(A, cells, cur, curCount, clip, done, pc);
-      cudaEventRecord(ev[3], st);
-      const cudaError_t e = read_ctl(h);
-      if (e != cudaSuccess) return cuda_check(c, e, "phase round");
-      if (!initTimed) { elapsed(0, ev[0], ev[1]); initTimed = true; }
-      if (fixPending) { elapsed(2, ev[1], ev[2]); fixPending = false; }   // previous fix: between its start mark and this verify
-      elapsed(1, ev[2], ev[3]);
-      if (h.nClip == 0) break;
-      if ((s = cuda_check(c, cudaMemsetAsync(&pc->ticket, 0, sizeof(unsigned), st), "phase ctl"))) return s;
-      if ((int)h.nClip <= tailPairs) {
-        cudaEventRecord(ev[1], st);
-        if (hv) VD_LAUNCH(k_ph_tail<true>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, done, pc);
-        else VD_LAUNCH(k_ph_tail<false>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, done, pc);
-        cudaEventRecord(ev[2], st);
-        const cudaError_t e2 = read_ctl(h);
-        if (e2 != cudaSuccess) return cuda_check(c, e2, "phase tail");
-        elapsed(4, ev[1], ev[2]);
-        break;
-      }
-      cudaEventRecord(ev[1], st);
-      if (hv) VD_LAUNCH(k_ph_fix<true>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
-      else VD_LAUNCH(k_ph_fix<false>, grid, kBlock, 0, st)(A, cells, clip, (int)h.nClip, b, pc);
-      fixPending = true;
-      cur = clip;
-      curCount = (int)h.nClip;
-      int* tmp = clip; clip = other; other = tmp;
-    }
-    if (h.nDone > 0) {
-      // pool chunk per warp: ~1/32 of an even share of the pool, so that the slack (one open chunk per warp) stays small
-      // static stride over the grid: exactly the resident blocks (3 per SM), or the last third would run alone
-      const int fgrid = sm_count() * 3;
-      const int64_t warps = (int64_t)fgrid * kWarpsPerBlock;
-      auto chunk_of = [&](int64_t cap) { const int64_t v = cap / (warps * 32); return (int)(v > 1024 ? 1024 : v); };   // small pools: piece by piece
-      cudaEventRecord(ev[0], st);
-      VD_LAUNCH(k_ph_finish, fgrid, kBlock, 0, st)(A, cells, done, (int)h.nDone, b, chunk_of(c->vertCap), chunk_of(c->nbrCap));
-      cudaEventRecord(ev[1], st);
-      const cudaError_t e = sync_stream(c);
-      if (e != cudaSuccess) return cuda_check(c, e, "phase finish");
-      elapsed(3, ev[0], ev[1]);
-    }
-  }
-  return cuda_check(c, cudaGetLastError(), "phases");
+  return ensure(c, c->phaseLists, sizeof(PhaseCtl) + sizeof(int) * 3 * (size_t)cap);   // the control block first (8-byte members)
 }
+
+void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int rounds, int tailPairs) {
+  CellState* cells = c->phaseCells.as<CellState>();
+  PhaseCtl* pc = c->phaseLists.as<PhaseCtl>();
+  int* lists = reinterpret_cast<int*>(pc + 1);
+  int* done = lists + 2 * cap;
+  cudaStream_t st = c->stream;
+  const int grid = sm_count() * 4;
+  const int icap = (int)cap;
+  phase_mark(c, 0);
+  if (c->kind == KIND_BOX_3D) VD_LAUNCH(k_ph_init<true>, grid, kBlock, 0, st)(A, cells, pc);
+  else VD_LAUNCH(k_ph_init<false>, grid, kBlock, 0, st)(A, cells, pc);
+  for (int r = 0; r < rounds; ++r) {
+    phase_mark(c, 1);
+    if (hv) VD_LAUNCH(k_ph_verify<true>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    else VD_LAUNCH(k_ph_verify<false>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    phase_mark(c, 2);
+    if (hv) VD_LAUNCH(k_ph_fix<true>, grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+    else VD_LAUNCH(k_ph_fix<false>, grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+  }
+  phase_mark(c, 4);
+  if (hv) VD_LAUNCH(k_ph_tail<true>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, rounds, tailPairs);
+  else VD_LAUNCH(k_ph_tail<false>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, rounds, tailPairs);
+  // pool chunk per warp: ~1/32 of an even share of the pool, so that the slack (one open chunk per warp) stays small;
+  // static stride over the grid: exactly the resident blocks (3 per SM), or the last third would run alone
+  const int fgrid = sm_count() * 3;
+  const int64_t warps = (int64_t)fgrid * kWarpsPerBlock;
+  auto chunk_of = [&](int64_t poolCap) { const int64_t v = poolCap / (warps * 32); return (int)(v > 1024 ? 1024 : v); };   // small pools: piece by piece
+  phase_mark(c, 3);
+  VD_LAUNCH(k_ph_finish, fgrid, kBlock, 0, st)(A, cells, done, pc, chunk_of(c->vertCap), chunk_of(c->nbrCap));
+  phase_mark(c, -1);
+}
+
+PhaseCtl* phase_ctl(vd_ctx* c, int64_t) { return c->phaseLists.as<PhaseCtl>(); }
 
 }  // namespace vd
