@@ -77,10 +77,11 @@ static void keep_freed_memory_in_pool() {
 
 void release(vd_ctx* c, DevBuf& b) {
   if (!b.p) return;
-  if (c->freeFn) c->freeFn(b.p, c->allocUser);
+  if (b.hooked && c->freeFn) c->freeFn(b.p, c->allocUser);
   else if (cudaFreeAsync(b.p, c->stream) != cudaSuccess) { cudaGetLastError(); cudaFree(b.p); }
   b.p = nullptr;
   b.cap = 0;
+  b.hooked = false;
 }
 
 vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
@@ -93,6 +94,7 @@ vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
   if (c->allocFn) {
     p = c->allocFn(bytes, c->allocUser, (void*)c->stream);
     if (!p) { c->lastError = "allocator hook returned NULL"; return VD_E_NOMEM; }
+    b.hooked = true;
   } else {
     cudaError_t e = cudaMallocAsync(&p, bytes, c->stream);
     if (e != cudaSuccess) { cudaGetLastError(); e = cudaMalloc(&p, bytes); }
@@ -503,7 +505,7 @@ void vd_destroy(vd_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->delta, &c->siteW, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->scanTmp, &c->delta, &c->siteW, &c->sortedW, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
                    &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,

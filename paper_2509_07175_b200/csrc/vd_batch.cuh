@@ -106,6 +106,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
         const double4 p = g.sites[B.base[owner] + t];
         const double dx = B.qx[cu] - p.x, dy = B.qy[cu] - p.y, dz = B.qz[cu] - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
+        if (g.sitesW) d2 += __ldg(&g.sitesW[B.base[owner] + t]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
         better = closer(d2, id, B.best[cu], B.bestId[cu]);
       }
@@ -187,6 +188,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
                   }
                   v.n = 0; v.cellStart = gTop.cellStart + c; v.sites = gTop.sites;
                   v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
+                  v.sitesW = gTop.sitesW; v.siteWid = gTop.siteWid;
                 }
               }
               __syncwarp();

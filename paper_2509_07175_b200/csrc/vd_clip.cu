@@ -62,13 +62,14 @@ __global__ void __launch_bounds__(kBlock) k_seed_points(ClipArgs A, int S, const
 
 // Simple domains (section V-B): a site inside the box owns its own position, so (box, v_i) is a non-empty pair
 // with witness v_i ("each site must be in its own Voronoi cell").
-__global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, int ncorner) {
+__global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, int ncorner, const int* __restrict__ own) {
   // the box's corners are the "mesh vertices": corner 0 = lo, the last = hi
   const double lx = A.verts[0], ly = A.verts[1], lz = A.verts[2];
   const double hx = A.verts[3 * (ncorner - 1) + 0], hy = A.verts[3 * (ncorner - 1) + 1], hz = A.verts[3 * (ncorner - 1) + 2];
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) {
     const double x = A.sites[i * 3 + 0], y = A.sites[i * 3 + 1], z = A.sites[i * 3 + 2];
-    if (x >= lx && x <= hx && y >= ly && y <= hy && z >= lz && z <= hz) push_pair(A, 0, (int)i, x, y, z);
+    // power diagram: a site need not lie in its own cell (own[] = the power-nearest site of every site's position)
+    if (x >= lx && x <= hx && y >= ly && y <= hy && z >= lz && z <= hz && (!own || own[i] == (int)i)) push_pair(A, 0, (int)i, x, y, z);
   }
 }
 
@@ -187,6 +188,7 @@ static ClipArgs make_args(vd_ctx* c) {
   ClipArgs A;
   A.grid = c->grid.as<GridIndex>();
   A.sites = c->sites.as<double>();
+  A.siteW = (c->weighted && c->dim == 3) ? c->siteW.as<double>() : nullptr;
   A.verts = c->verts.as<double>();
   A.simp = c->simp.as<int>();
   A.adj = c->adj.as<int>();
@@ -260,7 +262,13 @@ vd_status stage_seed(vd_ctx* c) {
     VD_LAUNCH(k_seed_points, blocks_for(total, kBlock, sm_count() * 8), kBlock, 0, st)(A, S, c->seedPts.as<double>(), c->seedNN.as<int>());
   }
   if (boxKind) {
-    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc);
+    const int* own = nullptr;
+    if (A.siteW) {
+      if ((s = ensure(c, c->seedNN, sizeof(int) * c->n))) return s;
+      if ((s = stage_nearest_points(c, c->sites.as<double>(), c->n, c->seedNN.as<int>()))) return s;
+      own = c->seedNN.as<int>();
+    }
+    VD_LAUNCH(k_seed_sites, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, own);
   }
   return cuda_check(c, cudaGetLastError(), "seed");
 }

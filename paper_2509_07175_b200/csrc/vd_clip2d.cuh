@@ -19,7 +19,7 @@ struct Poly2 {
   double tx[K], ty[K], tz[K], tnx[K], tny[K], tnz[K], td[K];
   int tflag[K], tnn[K];
   unsigned char tstate[K];
-  double u[12];   // per-pair constants: origin, v_i absolute, v_i local, witness local
+  double u[14];   // per-pair constants: origin, v_i absolute, v_i local, witness local, [12] = 0 (the additive term of 3-D power diagrams)
   int nc;
 };
 
@@ -166,7 +166,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
   const double wx = pr.wx - ox, wy = pr.wy - oy, wz = pr.wz - oz;
   if (lane == 0) {
     S.u[0] = ox; S.u[1] = oy; S.u[2] = oz; S.u[3] = six; S.u[4] = siy; S.u[5] = siz;
-    S.u[6] = vix; S.u[7] = viy; S.u[8] = viz; S.u[9] = wx; S.u[10] = wy; S.u[11] = wz;
+    S.u[6] = vix; S.u[7] = viy; S.u[8] = viz; S.u[9] = wx; S.u[10] = wy; S.u[11] = wz; S.u[12] = 0.0; S.u[13] = 0.0;
   }
   __syncwarp();
   bool failed = false;

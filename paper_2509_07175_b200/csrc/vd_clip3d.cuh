@@ -18,7 +18,7 @@ struct WarpPool {
 
 template <int P, int C>
 struct alignas(16) Poly3 {
-  double u[12];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local)
+  double u[14];                           // per-pair constants: origin o, site v_i (absolute, local), witness (local), [12] = the site's additive term (power diagrams), [13] spare
   int pflag[P];                           // flag of plane f
   double cx[C], cy[C], cz[C];             // corner coordinates (local)
   unsigned char cstate[C];
@@ -38,7 +38,7 @@ struct alignas(16) Poly3 {
 // it does not take is L1 for the site records the tests stream through.
 template <int P, int C>
 struct alignas(16) PolyTest3 {
-  double u[12];
+  double u[14];
   int pflag[P];
   double cx[C], cy[C], cz[C];
   unsigned char cstate[C];
@@ -547,6 +547,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
       S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
       S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
       S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
+      S.u[12] = A.siteW ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
     }
     if (lane < 6) {
       const int axis = lane >> 1, hiSide = lane & 1;
@@ -586,6 +587,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
         S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
         S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
         S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
+        S.u[12] = A.siteW ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
       }
     }
     __syncwarp();
@@ -628,7 +630,7 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
   const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
                wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
   const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
-  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + ((A.siteW ? __ldg(&A.siteW[j]) : 0.0) - S.u[12]));
   // the corner farthest beyond the plane starts R_p
   double far = 0.0;
   int p = 0x7fffffff;
@@ -745,7 +747,7 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
         const double dx = qx - six, dy = qy - siy, dz = qz - siz;
         Q.item[slot] = c;
         Q.qx[slot] = qx; Q.qy[slot] = qy; Q.qz[slot] = qz;
-        Q.best[slot] = dx * dx + dy * dy + dz * dz;
+        Q.best[slot] = dx * dx + dy * dy + dz * dz + S.u[12];
         Q.bestId[slot] = i;
       }
       nq = min(kQB, nq + __popc(m));
@@ -761,7 +763,7 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
       // owns a plane of P -- the flag rule in the form of reading U6.  A clearly nearer site (any
       // such site ends the query, U17) means outside.
       const double dx = Q.qx[lane] - six, dy = Q.qy[lane] - siy, dz = Q.qz[lane] - siz;
-      const double di2 = dx * dx + dy * dy + dz * dz, best = Q.best[lane];
+      const double di2 = dx * dx + dy * dy + dz * dz + S.u[12], best = Q.best[lane];
       bool inside = id == i || best >= di2 * (1.0 - 1e-13);
       if (!inside && best >= di2 * (1.0 - 1e-9))
         for (int f = 0; f < np && !inside; ++f) inside = (S.pflag[f] == id);

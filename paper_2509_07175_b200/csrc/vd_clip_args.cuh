@@ -9,6 +9,7 @@ namespace vd {
 struct ClipArgs {
   const GridIndex* grid;
   const double* sites;     // [n][3] original order
+  const double* siteW;     // [n] additive term eta - w_i of every site (power diagrams of 3-D sites), or nullptr
   const double* verts;     // [nv][3]
   const int* simp;         // [m][nc]
   const int* adj;          // [m][nc]
@@ -313,13 +314,14 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
       const double4 p = g.sites[base[owner] + t];
       const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
-      const double dq2 = dx * dx + dy * dy + dz * dz;
+      const double pw = g.sitesW ? __ldg(&g.sitesW[base[owner] + t]) : 0.0;
+      const double dq2 = dx * dx + dy * dy + dz * dz + pw;
       bool cand = id != i && id != j && dq2 < r2 * (1.0 - 1e-13);
       if (cand && !(dq2 < r2 * (1.0 - 1e-9)))
         for (int f = 0; f < nflags; ++f) cand = cand && (flags[f] != id);
       if (cand) {
         const double ex = psx - p.x, ey = psy - p.y, ez = psz - p.z;
-        const double gs = ex * ex + ey * ey + ez * ez - dis2, gq = dq2 - r2;
+        const double gs = ex * ex + ey * ey + ez * ez + pw - dis2, gq = dq2 - r2;
         const double tk = gs > 0.0 ? tq * gs / (gs - gq) : 0.0;
         if (closer(tk, id, tb, jb)) { tb = tk; jb = id; }
       }
@@ -353,7 +355,7 @@ static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, c
     const double gx = psx + sx * inv * s, gy = psy + sy * inv * s, gz = psz + sz * inv * s;
     const double ax = gx + u[0], ay = gy + u[1], az = gz + u[2];
     const double dx = ax - u[3], dy = ay - u[4], dz = az - u[5];
-    const double di2 = dx * dx + dy * dy + dz * dz;
+    const double di2 = dx * dx + dy * dy + dz * dz + u[12];
     double best = di2;
     int bestId = i;
     nearest<HV>(g, ax, ay, az, best, bestId, st, true);
@@ -393,8 +395,9 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     iters += 1;
     const double vjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
                  vjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
+    const double wi = u[12], wj = site_w(g, j);   // power diagram: the lifted sites' fourth coordinates, squared (else 0)
     nx = vjx - vix; ny = vjy - viy; nz = vjz - viz;
-    d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz));
+    d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz) + (wj - wi));
     const double gs = d - (nx * psx + ny * psy + nz * psz);
     const double gt = d - (nx * ptx + ny * pty + nz * ptz);
     const double den = gs - gt;
@@ -405,20 +408,20 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     const double ax = qx + ox, ay = qy + oy, az = qz + oz;
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
-    const double di2 = dix * dix + diy * diy + diz * diz, dj2 = djx * djx + djy * djy + djz * djz;
+    const double di2 = dix * dix + diy * diy + diz * diz + wi, dj2 = djx * djx + djy * djy + djz * djz + wj;
     if (!HV && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
       // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
       double tb = 2.0;
       int jb = 0x7fffffff;
       const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
-      if (scan_ball_min_t<HV>(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz, t, i, j, flags, nflags,
+      if (scan_ball_min_t<HV>(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz + wi, t, i, j, flags, nflags,
                           ballCells, tb, jb, st)) {
         if (jb != 0x7fffffff) {
           j = jb;
           const double wjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
                        wjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
           nx = wjx - vix; ny = wjy - viy; nz = wjz - viz;
-          d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz));
+          d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (site_w(g, j) - wi));
         }
         goto found;
       }

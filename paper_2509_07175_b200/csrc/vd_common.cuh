@@ -54,7 +54,15 @@ struct GridIndex {
   // S1b: delta_i = half the distance from v_i to its nearest other site, for the step-out of section VI-A
   const double* __restrict__ delta;       // [n] by original site id, or null (vd_options.step_out = 0)
   int stepMode;                           // 1: lambda = 2, 3, 4, ...; 2: lambda doubles
+  // Power diagrams of 3-D sites (vd_create_weighted): the lifted sites p_i = (v_i, sqrt(eta - w_i)) in R^4 are
+  // seen from the domain at height 0, so every squared distance to site i is |x - v_i|^2 + (eta - w_i).  The additive
+  // terms, by sorted position and by original site id; null for ordinary (and for lifted 2-D) sites.  They are >= 0, so the
+  // grid's plain box distances stay lower bounds.
+  const double* __restrict__ sitesW;
+  const double* __restrict__ siteWid;
 };
+
+__device__ __forceinline__ double site_w(const GridIndex& g, int id) { return g.siteWid ? __ldg(&g.siteWid[id]) : 0.0; }
 
 constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
 

@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restric
 // average over all cells of the sites' box -- reading U9), header written to device memory.
 __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64_t n, double density, int64_t gridCap,
                               const int* cellStart, const double4* sorted, int countAlg, const double* delta, int stepMode,
-                              GridIndex* g, unsigned int* err) {
+                              const double* sitesW, const double* siteWid, GridIndex* g, unsigned int* err) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
   for (int k = 0; k < nparts; ++k)
@@ -94,6 +94,8 @@ __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64
   out.countAlg = countAlg;
   out.delta = delta;
   out.stepMode = stepMode;
+  out.sitesW = sitesW;
+  out.siteWid = siteWid;
   *g = out;
 }
 
@@ -240,6 +242,14 @@ __global__ void k_grid_finish(GridIndex* g, const double4* sorted2, const int* h
   }
 }
 
+// Power diagrams of 3-D sites: the additive term of every site, in the order of the finished index
+__global__ void __launch_bounds__(kBlock) k_gather_weights(const GridIndex* __restrict__ gp, int64_t n, const double* __restrict__ byId,
+                                                            double* __restrict__ sortedW) {
+  const double4* sites = gp->sites;
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x)
+    sortedW[p] = byId[(int)(__double_as_longlong(sites[p].w) & 0x7fffffff)];
+}
+
 // Duplicate sites (reading U14: VD_E_INPUT): equal coordinates mean equal cell and sub-cell keys, so the two sites sit
 // in the same finest bucket of the finished index.  One thread per sorted position compares with the rest of its bucket.
 __global__ void __launch_bounds__(kBlock) k_find_duplicates(const GridIndex* __restrict__ gp, int64_t n, unsigned int* err) {
@@ -323,12 +333,15 @@ vd_status stage_index(vd_ctx* c) {
   if ((s = ensure(c, c->control, sizeof(Control)))) return s;
   const int stepMode = c->opt.step_out > 0 ? (c->opt.step_out > 2 ? 2 : c->opt.step_out) : 0;
   if (stepMode && (s = ensure(c, c->delta, sizeof(double) * n))) return s;
+  const bool lifted4 = c->weighted && c->dim == 3;   // power diagram of 3-D sites: additive terms travel with the sorted records
+  if (lifted4 && (s = ensure(c, c->sortedW, sizeof(double) * n))) return s;
   cudaStream_t st = c->stream;
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
                                          c->sorted.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
-                                         stepMode ? c->delta.as<double>() : nullptr, stepMode, c->grid.as<GridIndex>(),
+                                         stepMode ? c->delta.as<double>() : nullptr, stepMode,
+                                         lifted4 ? c->sortedW.as<double>() : nullptr, lifted4 ? c->siteW.as<double>() : nullptr, c->grid.as<GridIndex>(),
                                          &c->control.as<Control>()->err);
   cudaMemsetAsync(c->cellFill.p, 0, sizeof(int) * (gridCap + 2), st);
   VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
@@ -367,6 +380,7 @@ vd_status stage_index(vd_ctx* c) {
                                                                                c->subStart.as<int>());
   VD_LAUNCH(k_grid_finish, 1, 1, 0, st)(gp, c->sorted2.as<double4>(), c->heavyPrefix.as<int>(), c->subOff.as<int>(),
                                          c->subStart.as<int>(), &c->control.as<Control>()->nHeavy);
+  if (lifted4) VD_LAUNCH(k_gather_weights, grid_for(n, kBlock), kBlock, 0, st)(gp, n, c->siteW.as<double>(), c->sortedW.as<double>());
   VD_LAUNCH(k_find_duplicates, grid_for(n, kBlock), kBlock, 0, st)(gp, n, &c->control.as<Control>()->err);
   if (stepMode)   // S1b
     VD_LAUNCH(k_delta, grid_for(n, kWarpsPerBlock), kBlock, 0, st)(gp, c->sites.as<double>(), n, c->delta.as<double>(),

@@ -40,6 +40,7 @@ inline Counters counters_total(const Control& h) {
 struct DevBuf {
   void* p = nullptr;
   size_t cap = 0;
+  bool hooked = false;   // came from the caller's allocator hook (vd_set_allocator): goes back through its release hook
   template <typename T> T* as() const { return reinterpret_cast<T*>(p); }
 };
 
@@ -85,6 +86,7 @@ struct vd_ctx {
   vd::DevBuf cellStart;   // int [gridCap+1]
   vd::DevBuf cellFill;    // int [gridCap+1]
   vd::DevBuf sorted;      // double4 [n]
+  vd::DevBuf sortedW;     // double [n]  additive terms of weighted 3-D sites in index order
   vd::DevBuf delta;       // double [n]  S1b: half the distance to the nearest other site (vd_options.step_out)
   vd::DevBuf scanTmp;     // scan scratch
   vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart, subKey, sorted2;   // second level

@@ -110,6 +110,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         const double4 p = g.sites[base[owner] + t];
         const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
+        if (g.sitesW) d2 += __ldg(&g.sitesW[base[owner] + t]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       }
       const bool better = valid && closer(d2, id, best, bestId) && !(SKIP && id == st.skip);
@@ -174,6 +175,7 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
   v.cellStart = g.subStart + (so & 0x3ffffff);
   v.sites = g.sites;
   v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
+  v.sitesW = g.sitesW; v.siteWid = g.siteWid;
 }
 
 // One cell of the top grid: a plain cell is scanned directly, a refined cell through its sub-grid,

@@ -70,7 +70,7 @@ def test_allocator_hook_with_the_torch_caching_allocator():
     """vd_set_allocator: every device buffer of the context comes from torch's caching allocator through
     C callbacks; the result is the oracle's, and every block is handed back."""
     import torch
-    live, calls = {}, [0, 0]
+    live, calls, strangers = {}, [0, 0], []
 
     def alloc(nbytes, stream):
         p = torch.cuda.caching_allocator_alloc(nbytes, torch.cuda.current_device(), stream or None)
@@ -79,7 +79,8 @@ def test_allocator_hook_with_the_torch_caching_allocator():
         return p
 
     def release(ptr):
-        assert live.pop(ptr, None) is not None
+        if live.pop(ptr, None) is None:
+            strangers.append(ptr)      # (an exception inside a ctypes callback would only be printed)
         calls[1] += 1
         torch.cuda.caching_allocator_delete(ptr)
 
@@ -93,6 +94,7 @@ def test_allocator_hook_with_the_torch_caching_allocator():
         with pytest.raises(binding.VdError):       # too late to switch allocators
             ctx.set_allocator(alloc, release)
     assert calls[0] > 20 and not live, (calls, len(live))   # vd_destroy returned every block through the hook
+    assert not strangers                                       # and only blocks that came from it
     parity.assert_parity(g, oracle.compute(w.sites, w.verts, w.simplices, w.kind), w.diameter)
 
 
@@ -123,12 +125,26 @@ def test_replica_parity(idx, opts):
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
                                   dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
                                   dict(tail_pairs=-1, small_wave=-1), dict(tail_pairs=64, small_wave=-1), dict(first_clip=-1), dict(first_clip=-1, small_wave=-1),
-                                  dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000)])
+                                  dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000),
+                                  dict(step_out=1), dict(step_out=2, small_wave=-1), dict(step_out=1, ball_cells=-1), dict(count_alg=1)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
     o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
     parity.assert_parity(g, o, w.diameter)
+
+
+@pytest.mark.parametrize("idx", [4, 5, 3])
+def test_step_out_of_section_vi_a(idx):
+    """S1b + the improved search: same cells with the step-out, linear (as printed) and doubling; probes are
+    counted.  Surface, far-site and clustered (refined index) replicas."""
+    w = inputs.config(idx, "small")
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    base, c0, _ = _gpu(w)
+    for mode in (1, 2):
+        g, c, _ = _gpu(w, step_out=mode)
+        parity.assert_parity(g, o, w.diameter)
+        assert c["step_probes"] > 0 and c0["step_probes"] == 0
 
 
 def test_nearest_site_kernel_against_brute_force():

@@ -139,3 +139,28 @@ def test_power_diagram_parity_on_the_gpu(n, spread, k):
     with pytest.raises(binding.VdError) as e:                                # eta below the largest weight
         power.power_cells(s, w, verts, tris, eta=float(w.max()) - 1e-3)
     assert e.value.status == 4
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kind,opts", [("tet", {}), ("tet", dict(small_wave=-1)), ("box", {}), ("box", dict(small_wave=-1, near_clips=-1))])
+def test_power_diagram_3d_parity_on_the_gpu(kind, opts):
+    """3-D weighted sites (lifted to R^4 inside the library: the fourth coordinate enters as an additive term) on a tet
+    mesh and on the box kind, against the oracle's power cells; some sites are hidden (empty cells), some do not lie in
+    their own cell."""
+    import parity
+    from paper_2509_07175_b200 import binding, power
+    s, w = _weighted3(3000, 33, 0.8)
+    if kind == "tet":
+        verts, simp, k = *inputs.cube_kuhn_mesh(3), inputs.KIND_TET_3D
+        o = oracle.compute(s, verts, simp, k, weights=w, tier="B")
+    else:
+        verts, simp, k = np.array([[0.0, 0, 0], [1.0, 1, 1]]), None, inputs.KIND_BOX_3D
+        o = oracle.compute(s, verts, None, k, weights=w, tier="B")
+    g = power.power_cells(s, w, verts, simp, kind=k, **opts)
+    parity.assert_parity(g, o, np.sqrt(3.0))
+    assert abs(g.measure.sum() - 1.0) <= 1e-11
+    assert (g.measure == 0).sum() == (o.measure == 0).sum() > 0
+    own = np.array([np.argmin(((s - s[i]) ** 2).sum(1) - w) for i in range(0, len(s), 7)])
+    assert (own != np.arange(0, len(s), 7)).any()           # the case exists: a site outside its own power cell
+    g2 = power.power_cells(s, w, verts, simp, kind=k, eta=float(w.max()) + 0.01, **opts)
+    parity.assert_parity(g2, o, np.sqrt(3.0))
