@@ -246,6 +246,16 @@ vd_status vd_cells_to_host(vd_ctx* ctx, double* measure, double* centroid, int64
  * out_index[q] = argmin_j |q - v_j|, ties to the lowest id.  queries / out_index: host or device. */
 vd_status vd_nearest(vd_ctx* ctx, const double* queries, int64_t nq, int32_t* out_index);
 
+/* vd_nearest_static: vd_nearest for callers that must not allocate device memory (code next to a CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same result as vd_nearest; the call makes NO cudaMalloc / cudaFree or
+ * other allocating call: queries and results are staged in one fixed device array inside the library (about 1.8 MB, held by
+ * every GPU that loads libvd.so until the process exits).  Limits: nq <= 65536 per call (more: VD_E_ARG, with a message --
+ * split the batch); the site index must already exist (VD_E_STATE otherwise: building it allocates -- run vd_compute or
+ * vd_nearest once); every call of every context shares the array, which keeps the previous call's contents (the call clears
+ * what must start at zero), so calls that overlap on the GPU race: one at a time.  queries / out_index: host or device.
+ * Synchronises the context's stream.  Errors: VD_E_ARG, VD_E_STATE, VD_E_INPUT (non-finite query), VD_E_CUDA. */
+vd_status vd_nearest_static(vd_ctx* ctx, const double* queries, int64_t nq, int32_t* out_index);
+
 /* Sharded runs (vd_options.simplex_begin / simplex_end): vd_partial_moments writes, for every cell of
  * the last vd_compute, (measure, measure x centroid) = 1 + dim doubles per site into out [n][1 + dim] (DEVICE pointer,
  * caller-owned) -- the additive quantities the ranks sum with one all-reduce; vd_finish_centroids takes the summed

@@ -19,7 +19,7 @@ STATUS = {0: "VD_OK", 1: "VD_E_ARG", 2: "VD_E_DIM", 3: "VD_E_STATE", 4: "VD_E_IN
           6: "VD_E_NOMEM", 7: "VD_E_CAPACITY", 8: "VD_E_NOCONVERGE"}
 EXPORTS = ["vd_create", "vd_create_weighted", "vd_partial_moments", "vd_finish_centroids", "vd_update_sites", "vd_lloyd", "vd_set_domain", "vd_compute", "vd_destroy", "vd_set_stream",
            "vd_set_allocator", "vd_set_options", "vd_get_counters", "vd_get_stage_ms", "vd_get_phase_ms", "vd_get_phase_counters", "vd_cells_to_host",
-           "vd_nearest", "vd_get_adjacency", "vd_dfma_peak", "vd_last_error", "vd_version"]
+           "vd_nearest", "vd_nearest_static", "vd_get_adjacency", "vd_dfma_peak", "vd_last_error", "vd_version"]
 
 _LIB_PATH = _build.lib_path()
 _lib = None
@@ -85,6 +85,7 @@ def load():
     lib.vd_get_phase_counters.argtypes = [vp, ci, ctypes.POINTER(vd_counters)]
     lib.vd_cells_to_host.argtypes = [vp] + [vp] * 10
     lib.vd_nearest.argtypes = [vp, vp, i64, vp]
+    lib.vd_nearest_static.argtypes = [vp, vp, i64, vp]
     lib.vd_get_adjacency.argtypes = [vp, vp]
     lib.vd_dfma_peak.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.vd_last_error.argtypes = [vp]
@@ -304,6 +305,17 @@ class Context:
         q = np.ascontiguousarray(queries, dtype=np.float64)
         out = np.empty(q.shape[0], np.int32)
         self._check(self._lib.vd_nearest(self._h, q.ctypes.data, q.shape[0], out.ctypes.data))
+        return out
+
+    def nearest_static(self, queries, out=None):
+        """vd_nearest_static: no device allocation (at most 65536 queries; the index must exist).  queries / out: numpy
+        arrays or torch tensors (host or CUDA); out (int32 [nq]) is created as a numpy array when not given."""
+        pq, keep = _ptr(queries, np.float64)
+        nq = int(queries.shape[0])
+        if out is None:
+            out = np.empty(nq, np.int32)
+        po = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        self._check(self._lib.vd_nearest_static(self._h, pq, nq, po))
         return out
 
     def adjacency(self) -> np.ndarray:

@@ -396,4 +396,84 @@ vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out
   return cuda_check(c, cudaGetLastError(), "nearest");
 }
 
+// ---- vd_nearest_static: the nearest-site query for callers that must not allocate (vd.h) ---------------------------------
+//
+// vd_nearest stages its queries and results in buffers it allocates per call.  This variant stages them in ONE file-scope
+// device array of fixed size instead, so the call makes no cudaMalloc / cudaFree (nor any allocating routine): usable where
+// allocation is forbidden (a stream under graph capture elsewhere in the process, a serving loop, a harness that traps
+// cudaMalloc).  Every GPU that loads libvd.so holds the array (about 1.8 MB) until the process exits.  All calls, from every
+// context, share it: it keeps the last call's contents, and calls that overlap on the GPU race -- one call at a time.
+constexpr int kStaticMaxQueries = 1 << 16;
+
+struct NearestScratch {
+  double q[(size_t)kStaticMaxQueries * 3];   // the queries as given, [nq][dim]
+  int res[kStaticMaxQueries];                // N_q of every query
+  unsigned bad;                              // set when a query coordinate is not finite; must start at zero: cleared by every call
+  unsigned pad[63];
+};
+
+static __device__ __align__(256) unsigned char g_nearest_scratch[sizeof(NearestScratch)];
+
+// k_nearest_points with its input and output in the scratch block: one warp per query point; a 2-D query is padded with z = 0
+// on the fly (the sites of a 2-D problem are stored that way).
+__global__ void __launch_bounds__(kBlock) k_nearest_points_static(const GridIndex* __restrict__ gp, NearestScratch* __restrict__ S, int64_t nq, int dim) {
+  const GridIndex g = *gp;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
+  QueryStats st = {0u, 0u, 0u, 0};
+  for (int64_t q = warp; q < nq; q += nwarps) {
+    const double x = S->q[q * dim + 0], y = S->q[q * dim + 1], z = dim == 3 ? S->q[q * dim + 2] : 0.0;
+    const bool finite = x == x && y == y && z == z && fabs(x) <= 1e150 && fabs(y) <= 1e150 && fabs(z) <= 1e150;
+    double best = 2e300;
+    int bestId = 0x7fffffff;
+    if (finite) nearest<true>(g, x, y, z, best, bestId, st);
+    if (lane_id() == 0) {
+      S->res[q] = finite ? bestId : -1;
+      if (!finite) atomicOr(&S->bad, 1u);
+    }
+  }
+}
+
+// The array's name is a host-side stand-in in host code, not a device address: the address is asked for once per device,
+// with that device current, and handed to the kernel.
+static NearestScratch* nearest_scratch(vd_ctx* c) {
+  static NearestScratch* ptr[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); c->lastError = "vd_nearest_static: no current device"; return nullptr; }
+  if (!ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_nearest_scratch);
+    if (e != cudaSuccess || !p) { cudaGetLastError(); c->lastError = std::string("vd_nearest_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e); return nullptr; }
+    ptr[dev] = reinterpret_cast<NearestScratch*>(p);
+  }
+  return ptr[dev];
+}
+
 }  // namespace vd
+
+extern "C" vd_status vd_nearest_static(vd_ctx* c, const double* queries, int64_t nq, int32_t* out_index) {
+  using namespace vd;
+  if (!c || !queries || !out_index || nq < 1) return VD_E_ARG;
+  if (nq > kStaticMaxQueries) {
+    c->lastError = "vd_nearest_static: at most " + std::to_string(kStaticMaxQueries) + " queries per call (the static scratch block); split the batch or use vd_nearest";
+    return VD_E_ARG;
+  }
+  if (!c->indexValid) {
+    c->lastError = "vd_nearest_static: the site index is not built (building it allocates: run vd_compute or vd_nearest once first)";
+    return VD_E_STATE;
+  }
+  NearestScratch* S = nearest_scratch(c);
+  if (!S) return VD_E_CUDA;
+  cudaStream_t st = c->stream;
+  cudaError_t e = cudaMemsetAsync(&S->bad, 0, sizeof(unsigned), st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(S->q, queries, sizeof(double) * c->dim * nq, cudaMemcpyDefault, st);
+  if (e != cudaSuccess) return cuda_check(c, e, "vd_nearest_static");
+  VD_LAUNCH(k_nearest_points_static, grid_for(nq, kWarpsPerBlock), kBlock, 0, st)(c->grid.as<GridIndex>(), S, nq, c->dim);
+  unsigned bad = 0;
+  e = cudaMemcpyAsync(out_index, S->res, sizeof(int) * nq, cudaMemcpyDefault, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, &S->bad, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_check(c, e, "vd_nearest_static");
+  if (bad) { c->lastError = "vd_nearest_static: non-finite query coordinate"; return VD_E_INPUT; }
+  return VD_OK;
+}
