@@ -285,6 +285,22 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
     ctx.set_options(count_alg=1, **opts)
     ctx.compute()
     d_alg = ctx.counters()["alg_evals"]
+    # Alg. 5's site division (vd_options.dissolve; convex tet meshes, one GPU): interior cells as whole cells.  Reported
+    # beside the per-piece number, never instead of it (the per-piece output is what parity with SURVEY 8c.1 is defined on)
+    dissolve = None
+    if w.kind == 2 and not sharded and cfg in (2, 5):
+        ctx.set_options(dissolve=1)
+        for _ in range(2):
+            ctx.compute()
+        ts = []
+        for k in range(min(args.steps, 5)):
+            flush.fill_(k & 0xff)
+            ctx.compute()
+            ts.append(ctx.stage_ms()["total"])
+        dc = ctx.counters()
+        dissolve = {"ms_per_step": float(np.mean(ts)), "value": w.n / (float(np.mean(ts)) * 1e-3), "unit": UNIT, "pairs": dc["pairs"],
+                    "queries_per_cell": dc["queries"] / w.n, "paper_queries_per_cell_serial_alg2_cube": 20.54,
+                    "timing": "library events around vd_compute (stage total), L2 flushed between steps"}
     ctx.destroy()
 
     # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
@@ -332,6 +348,7 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
                      "d_act_over_d_alg": cnt["dist_evals"] / max(1, d_alg), "queries_per_pair": cnt["queries"] / max(1, cnt["pairs"]),
                      "clips": cnt["clips"] / w.n, "pieces": cnt["pieces"] / w.n},
         "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
+        "dissolve_mode": dissolve,
         "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",

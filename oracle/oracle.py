@@ -53,11 +53,11 @@ def _load():
     if _lib is None:
         build()
         _lib = ctypes.CDLL(_LIB)
-        _lib.vdo_compute_w.restype = ctypes.c_int
-        _lib.vdo_compute_w.argtypes = [
+        _lib.vdo_compute_x.restype = ctypes.c_int
+        _lib.vdo_compute_x.argtypes = [
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
             ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_int64,
-            ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.POINTER(_Result))]
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.POINTER(_Result))]
         _lib.vdo_free.restype = None
         _lib.vdo_free.argtypes = [ctypes.POINTER(_Result)]
     return _lib
@@ -101,12 +101,13 @@ def _arr(ptr, count, dtype, shape=None):
     return out.reshape(shape) if shape is not None else out
 
 
-def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0, weights=None) -> Cells:
+def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0, weights=None, dissolve=False) -> Cells:
     """Clipped / restricted Voronoi cells by the definition (Eq. 1).
 
     tier 'A' = literal (all j != i); 'B' = two-phase (box facets, then simplices); see the
     header of vd_oracle.cpp.  subset = site ids to compute (default all).  weights [n]: the power diagram
-    (section VII-C) instead of the Voronoi diagram.
+    (section VII-C) instead of the Voronoi diagram.  dissolve (tets, convex domain): cells that do not reach
+    the domain boundary come as ONE piece with simplex id m -- the whole Voronoi cell.
     """
     lib = _load()
     sites = np.ascontiguousarray(sites, dtype=np.float64)
@@ -128,8 +129,8 @@ def compute(sites, verts, simplices, kind, subset=None, tier="A", threads=0, wei
     if weights is not None:
         weights = np.ascontiguousarray(weights, dtype=np.float64)
         assert weights.shape == (n,)
-    rc = lib.vdo_compute_w(sites.ctypes.data, weights.ctypes.data if weights is not None else None, n, dim, verts.ctypes.data, nv, simplices.ctypes.data if simplices.size else None, m,
-                         int(kind), sp, ns, 1 if tier == "B" else 0, int(threads), ctypes.byref(res))
+    rc = lib.vdo_compute_x(sites.ctypes.data, weights.ctypes.data if weights is not None else None, n, dim, verts.ctypes.data, nv, simplices.ctypes.data if simplices.size else None, m,
+                         int(kind), sp, ns, 1 if tier == "B" else 0, int(threads), 1 if dissolve else 0, ctypes.byref(res))
     if rc != 0:
         raise RuntimeError(f"vdo_compute failed with status {rc}")
     r = res.contents

@@ -435,6 +435,11 @@ struct Problem {
   int64_t n;
   std::vector<V3> sites;
   std::vector<real> w;   // weights (power diagram); empty = the ordinary Voronoi diagram
+  // "dissolved" output for convex volumetric domains ("an interior site's clipped cell equals its Voronoi
+  // cell"; reading U1): a cell none of whose pieces has a face on the domain boundary is reported as ONE piece -- the bounding
+  // box of M clipped by the same half-spaces, simplex id m, site labels only -- instead of its per-simplex pieces.
+  bool dissolve = false;
+  V3 lo, hi;             // bounding box of the domain's vertices
   HalfSpace half_space(int64_t i, int64_t j) const {
     return w.empty() ? bisector(sites[i], sites[j], (int)j) : power_bisector(sites[i], w[i], sites[j], w[j], (int)j);
   }
@@ -486,6 +491,30 @@ static void compute_cell(const Problem& Pb, int64_t i, const std::vector<int32_t
     mom = mom + po.moment;
     for (size_t k = 0; k < po.faceSites.size(); ++k) out.nbr.push_back(po.faceSites[k]);
     out.pieces.push_back(po);
+  }
+  if (Pb.dissolve && D.kind == KIND_TET_3D && !out.pieces.empty()) {
+    bool onBoundary = false;
+    for (size_t p = 0; p < out.pieces.size() && !onBoundary; ++p)
+      for (size_t k = 0; k < out.pieces[p].flags.size(); ++k)
+        if (out.pieces[p].flags[k] == ~(int32_t)D.m) { onBoundary = true; break; }
+    if (!onBoundary) {
+      // the cell does not reach the boundary of the convex domain: Omega_i ∩ M = Omega_i, and the box contains it
+      Polyhedron G = box_polyhedron(Pb.lo, Pb.hi, ~(int)D.m);
+      if (planes) {
+        for (size_t k = 0; k < HS.size() && !G.empty(); ++k) clip_polyhedron(G, HS[k]);
+      } else {
+        for (int64_t j = 0; j < Pb.n && !G.empty(); ++j)
+          if (j != i) clip_polyhedron(G, Pb.half_space(i, j));
+      }
+      PieceOut po;
+      if (!G.empty() && finish_polyhedron(G, (int32_t)D.m, po)) {
+        out.pieces.clear();
+        out.nbr = po.faceSites;
+        out.meas = po.meas;
+        mom = po.moment;
+        out.pieces.push_back(po);
+      }
+    }
   }
   std::sort(out.nbr.begin(), out.nbr.end());
   out.nbr.erase(std::unique(out.nbr.begin(), out.nbr.end()), out.nbr.end());
@@ -556,9 +585,10 @@ void vdo_free(vdo_result* r) {
 // subset: site ids to compute (NULL -> all n).  tier: 0 = A (literal), 1 = B (two-phase).
 // Returns 0 on success; 1 bad argument; 4 bad input (non-manifold face, index out of range).
 // weights: NULL = Voronoi diagram; else [n] weights of the power diagram (section VII-C).
-int vdo_compute_w(const double* sites, const double* weights, int64_t n, int dim, const double* verts, int64_t nv,
+// dissolve != 0 (tets): cells that do not reach the domain boundary come as one whole piece (Problem::dissolve).
+int vdo_compute_x(const double* sites, const double* weights, int64_t n, int dim, const double* verts, int64_t nv,
                   const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
-                  int tier, int nthreads, vdo_result** out) {
+                  int tier, int nthreads, int dissolve, vdo_result** out) {
   const bool box = kind == KIND_BOX_2D || kind == KIND_BOX_3D;
   if (!sites || !verts || (!simplices && !box) || !out || n < 1 || m < 1 || nv < 1) return 1;
   if (!(((kind == KIND_TRI_2D || kind == KIND_BOX_2D) && dim == 2) || ((kind == KIND_TRI_SURFACE || kind == KIND_TET_3D || kind == KIND_BOX_3D) && dim == 3))) return 1;
@@ -586,6 +616,8 @@ int vdo_compute_w(const double* sites, const double* weights, int64_t n, int dim
     lo.y = std::min(lo.y, D.verts[v].y); hi.y = std::max(hi.y, D.verts[v].y);
     lo.z = std::min(lo.z, D.verts[v].z); hi.z = std::max(hi.z, D.verts[v].z);
   }
+  Pb.dissolve = dissolve != 0;
+  Pb.lo = lo; Pb.hi = hi;
   if (nthreads < 1) nthreads = (int)std::thread::hardware_concurrency();
   if (nthreads < 1) nthreads = 1;
   if ((int64_t)nthreads > ns) nthreads = (int)ns;
@@ -662,6 +694,12 @@ int vdo_compute_w(const double* sites, const double* weights, int64_t n, int dim
   R->vert_off[ip] = iv;
   *out = R;
   return 0;
+}
+
+int vdo_compute_w(const double* sites, const double* weights, int64_t n, int dim, const double* verts, int64_t nv,
+                  const int32_t* simplices, int64_t m, int kind, const int64_t* subset, int64_t n_subset,
+                  int tier, int nthreads, vdo_result** out) {
+  return vdo_compute_x(sites, weights, n, dim, verts, nv, simplices, m, kind, subset, n_subset, tier, nthreads, 0, out);
 }
 
 int vdo_compute(const double* sites, int64_t n, int dim, const double* verts, int64_t nv,

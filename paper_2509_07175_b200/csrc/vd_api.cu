@@ -335,6 +335,7 @@ vd_status vd_set_domain(vd_ctx* c, const double* verts, int64_t nv, const int32_
   if (box && (nv != 2 || m != 1)) return VD_E_ARG;
   c->haveDomain = false;
   c->haveResult = false;
+  dissolve_release(c);
   c->kind = (int)kind;
   const bool solid = kind == VD_TET_3D || kind == VD_BOX_3D;
   c->nc = kind == VD_BOX_3D ? 8 : ((kind == VD_TET_3D || kind == VD_BOX_2D) ? 4 : 3);
@@ -386,6 +387,17 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
   if (!c || !out) return VD_E_ARG;
   if (!c->haveDomain) { c->lastError = "vd_compute before vd_set_domain"; return VD_E_STATE; }
   c->haveResult = false;
+  if (c->opt.dissolve > 0) {
+    // Alg. 5's site division: convex tet meshes only
+    if (c->kind != VD_TET_3D || c->weighted || c->opt.simplex_end > 0) {
+      c->lastError = "vd_compute: vd_options.dissolve takes VD_TET_3D, unweighted sites, the whole mesh";
+      return VD_E_ARG;
+    }
+    if (!c->dissolveReady) {
+      const vd_status sd = stage_dissolve_prepare(c);
+      if (sd != VD_OK) return sd;
+    }
+  }
   if (c->pairCap == 0) {
     // pairs = pieces: a simplex meets ~2-20 cells in the paper-like workloads; corners ~11 per 3D piece.
     // Underestimates are repaired by doubling and rerunning (counters.reruns)
@@ -503,9 +515,10 @@ vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) 
 
 void vd_destroy(vd_ctx* c) {
   if (!c) return;
+  dissolve_release(c);
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->delta, &c->siteW, &c->sortedW, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->scanTmp, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
                    &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,

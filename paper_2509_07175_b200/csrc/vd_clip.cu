@@ -73,6 +73,36 @@ __global__ void __launch_bounds__(kBlock) k_seed_sites(ClipArgs A, int ncorner, 
   }
 }
 
+// Alg. 5 lines 4-14 in one pass over the sites, after the restricted diagram on the boundary triangles (child
+// context) is known: a site with a non-empty restricted cell is a BOUNDARY site -- every restricted polygon H of its cell seeds
+// (incident tet of H's triangle, site), witness = H's corner average (lines 8-14); a site with an empty one whose position lies
+// in the convex domain is INTERIOR -- its cell is its whole Voronoi cell, one pair (m, site) against the bounding
+// box (line 6); a site outside the domain with an empty restricted cell owns nothing (reading U13).
+__global__ void __launch_bounds__(kBlock) k_dissolve_seeds(ClipArgs A, const double* __restrict__ bMeasure, const int64_t* __restrict__ bPieceOff,
+                                                            const int* __restrict__ bPieceTri, const int64_t* __restrict__ bVertOff,
+                                                            const double* __restrict__ bXYZ, const int* __restrict__ bTet,
+                                                            const double4* __restrict__ planes, int np, double tol) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) {
+    if (bMeasure[i] > 0.0) {
+      for (int64_t p = bPieceOff[i]; p < bPieceOff[i + 1]; ++p) {
+        double x = 0, y = 0, z = 0;
+        const int64_t v0 = bVertOff[p], v1 = bVertOff[p + 1];
+        for (int64_t v = v0; v < v1; ++v) { x += bXYZ[v * 3 + 0]; y += bXYZ[v * 3 + 1]; z += bXYZ[v * 3 + 2]; }
+        const double inv = 1.0 / (double)(v1 - v0);
+        push_pair(A, bTet[bPieceTri[p]], (int)i, x * inv, y * inv, z * inv);
+      }
+    } else {
+      const double x = A.sites[i * 3 + 0], y = A.sites[i * 3 + 1], z = A.sites[i * 3 + 2];
+      bool inside = true;
+      for (int k = 0; k < np && inside; ++k) {
+        const double4 q = planes[k];
+        inside = q.x * x + q.y * y + q.z * z - q.w <= tol;
+      }
+      if (inside) push_pair(A, A.m, (int)i, x, y, z);
+    }
+  }
+}
+
 // Reading U19: the sites nearest to every site (approximately, from the 3 x 3 x 3 grid cells around it), nearest
 // first; one warp per site.  Their bisectors are the first clips of every piece of that site's cell.
 __global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ list, int K) {
@@ -180,7 +210,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(Cli
 // tet meshes the extra plane tests and redundant clips cost more than the searches they save)
 static int near_clips_of(const vd_ctx* c) {
   const int k = c->opt.near_clips;
-  if (k == 0) return (c->kind == KIND_BOX_3D) ? 20 : 0;
+  if (k == 0) return (c->kind == KIND_BOX_3D || (c->kind == KIND_TET_3D && c->opt.dissolve > 0)) ? 20 : 0;
   return k > kLanes ? kLanes : k;
 }
 
@@ -195,6 +225,12 @@ static ClipArgs make_args(vd_ctx* c) {
   A.vnn = c->vnn.as<int>();
   A.nearList = nullptr;
   A.queue = 0;
+  A.wholeA = -1; A.dissolve = 0; A.boxVerts = c->verts.as<double>(); A.boxVnn = c->vnn.as<int>();
+  if (c->kind == KIND_BOX_3D) A.wholeA = 0;
+  if (c->kind == KIND_TET_3D && c->opt.dissolve > 0) {
+    A.wholeA = (int)c->m; A.dissolve = 1;
+    A.boxVerts = c->boxVerts.as<double>(); A.boxVnn = c->boxVnn.as<int>();
+  }
   A.n = (int)c->n; A.m = (int)c->m; A.kind = c->kind;
   A.realEdges = c->opt.real_edges;
   A.ballCells = c->opt.ball_cells == 0 ? 64 : c->opt.ball_cells;
@@ -247,6 +283,17 @@ vd_status stage_seed(vd_ctx* c) {
   }
   const ClipArgs A = make_args(c);
   const bool boxKind0 = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
+  if (A.dissolve) {
+    // Alg. 5 lines 2-14: classify the sites through the restricted diagram on the boundary, seed boundary sites tet by tet and
+    // interior sites as whole cells
+    if ((s = stage_nearest_points(c, c->boxVerts.as<double>(), 8, c->boxVnn.as<int>()))) return s;
+    if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+    if ((s = stage_dissolve_classify(c))) return s;
+    const vd_cells& b = c->boundary->cells;
+    VD_LAUNCH(k_dissolve_seeds, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(
+        A, b.measure, b.piece_off, b.piece_simplex, b.vert_off, b.vert_xyz, c->bTet.as<int>(), c->bPlanes.as<double4>(), c->nBPlanes, 1e-12);
+    return cuda_check(c, cudaGetLastError(), "seed (dissolve)");
+  }
   if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
   VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
   const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;

@@ -426,8 +426,14 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
         S.key[slot][0] = S.pflag[f];
         const double inv = 1.0 / fk;
         // witness: the face's corner average lies in T_a ∩ Omega_i ∩ Omega_j
-        push_pair_faces(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, awp, naw, S.pflag);
+        if (!A.dissolve) push_pair_faces(A, a, S.pflag[f], fx * inv + ox, fy * inv + oy, fz * inv + oz, i, awp, naw, S.pflag);
       }
+    }
+    if (A.dissolve && a != A.wholeA && live && S.pflag[f] < 0 && ~S.pflag[f] < A.m) {
+      // Alg. 5 lines 20-24: the face of P on the face T_a shares with T_b lies in Omega_i, so (T_b, v_i) is a
+      // non-empty pair; its witness is that face's corner average
+      const double inv = 1.0 / fk;
+      push_pair(A, ~S.pflag[f], i, fx * inv + ox, fy * inv + oy, fz * inv + oz);
     }
     nnbr += __popc(pm);
   }
@@ -534,11 +540,11 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
   // loads tet vertex k; coordinates are local to vertex 0.  The per-pair constants live in shared memory
   // (S.u), not in registers: they would be spilled around every call of the query routines.
   np = 4; nc = 4;
-  if constexpr (BOX) {
+  if (BOX || a == A.wholeA) {
     // simple domain (section V-B): P <- the box; verts holds its 8 corners, corner c = bits (x, y, z),
     // planes 0..5 = -x +x -y +y -z +z, local origin = lo
     double vx = 0, vy = 0, vz = 0;
-    if (lane < 8) { vx = __ldg(&A.verts[lane * 3 + 0]); vy = __ldg(&A.verts[lane * 3 + 1]); vz = __ldg(&A.verts[lane * 3 + 2]); }
+    if (lane < 8) { vx = __ldg(&A.boxVerts[lane * 3 + 0]); vy = __ldg(&A.boxVerts[lane * 3 + 1]); vz = __ldg(&A.boxVerts[lane * 3 + 2]); }
     const double o0 = shfl(vx, 0), o1 = shfl(vy, 0), o2 = shfl(vz, 0);
     const double e0 = shfl(vx, 7) - o0, e1 = shfl(vy, 7) - o1, e2 = shfl(vz, 7) - o2;
     if (lane == 0) {
@@ -566,7 +572,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
       S.cadj[c][0] = (unsigned short)(odd ? (c ^ 2) : (c ^ 4));
       S.cadj[c][1] = (unsigned short)(c ^ 1);
       S.cadj[c][2] = (unsigned short)(odd ? (c ^ 4) : (c ^ 2));
-      const int nn = __ldg(&A.vnn[c]);
+      const int nn = __ldg(&A.boxVnn[c]);
       S.cnn[c] = nn;
       S.cstate[c] = (nn == i) ? ST_IN : ST_OUT;
     }
@@ -659,7 +665,7 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
 //     point-in-cell loop is a small polytope around the cell.
 // Returns 0, 1 (capacity), 2 (topology).
 template <int P, int C>
-__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int i, int u, const Pair* pp, int& np, int& nc, LocalCnt& lc) {
+__device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int a, int i, int u, const Pair* pp, int& np, int& nc, LocalCnt& lc) {
   const int lane = lane_id();
   if (A.firstClip && u >= 0 && u != i) {
     // lane 0: u; lanes 1 .. kPairW: the adjacent faces' sites (each bounds Omega_i along an edge of f that lies in T_a)
@@ -687,7 +693,7 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
       __syncwarp();
     }
   }
-  if (A.nearList && nc > 0) {
+  if (A.nearList && nc > 0 && (!A.dissolve || a == A.wholeA)) {   // (dissolve mode: whole cells only)
     const int K = A.nearClips;
     const int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
     for (int t = 0; t < K; ++t) {
@@ -818,7 +824,7 @@ __device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& 
   init_poly_3d<P, C, BOX>(S, A, pr, np, nc);
   bool failed = false;
   {
-    const int rc = preclip_3d(S, A, i, pr.u, &A.pairs[pairIdx], np, nc, lc);
+    const int rc = preclip_3d(S, A, a, i, pr.u, &A.pairs[pairIdx], np, nc, lc);
     if (rc == 1) return 1;
     if (rc == 2) { failed = true; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
   }

@@ -19,6 +19,13 @@ struct ClipArgs {
   int realEdges, ballCells, nearClips;
   int firstClip;           // 1: a discovered pair (a, i) is first clipped by B_iu, u the discovering site
   int aBegin, aEnd;        // simplices seeded by this context (vd_options.simplex_begin / simplex_end; a rank's block of M)
+  // Whole cells (section V-B; Alg. 5 line 6): a pair whose simplex id is wholeA starts from the box boxVerts (8 corners, corner
+  // c = bits x, y, z; their nearest sites in boxVnn) instead of a simplex.  VD_BOX_3D: wholeA = 0, the box is the domain.
+  // Dissolve mode of VD_TET_3D (Alg. 5): wholeA = m, the box is the mesh's bounding box; such pairs push nothing, and tet
+  // pairs propagate over NEGATIVE flags (same site, adjacent tet: Alg. 5 lines 20-24).  Otherwise wholeA = -1.
+  int wholeA, dissolve;
+  const double* boxVerts;
+  const int* boxVnn;
   int queue;               // 1: the pair list is read by a running kernel (device-side queue): publish slots with a fence
   Control* ctl;
   Pair* pairs;

@@ -91,6 +91,16 @@ struct vd_ctx {
   vd::DevBuf scanTmp;     // scan scratch
   vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart, subKey, sorted2;   // second level
   int64_t subCap = 0;
+  // dissolve mode (Alg. 5 lines 2-6, vd_options.dissolve): prepared once per domain (vd_domain.cu)
+  bool dissolveReady = false;
+  vd_ctx* boundary = nullptr;   // child context: the restricted Voronoi diagram on the boundary triangles of M (Alg. 5 line 3)
+  int64_t nBoundary = 0;        // boundary triangles
+  int nBPlanes = 0;             // distinct supporting planes of the (convex) domain
+  vd::DevBuf bTris;             // int [nBoundary][3]
+  vd::DevBuf bTet;              // int [nBoundary]  the tet behind every boundary triangle
+  vd::DevBuf bPlanes;           // double4 [nBPlanes]  outward unit normal, offset: inside iff n.x <= d
+  vd::DevBuf boxVerts;          // double [8][3]  corners of the mesh's bounding box (corner c = bits x, y, z)
+  vd::DevBuf boxVnn;            // int [8]  their nearest sites
   // S3-S5
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
   vd::DevBuf seedPts, seedNN;   // extra seed points inside the simplices and their nearest sites (few simplices, many sites)
@@ -137,6 +147,9 @@ void phase_marks_collect(vd_ctx* c);       // after a synchronisation: add the i
 
 // stages (each enqueues kernels on c->stream)
 vd_status stage_domain(vd_ctx* c);                 // S0  vd_domain.cu
+vd_status stage_dissolve_prepare(vd_ctx* c);       // S0, dissolve mode: boundary triangles, convexity, planes, bounding box, child context
+vd_status stage_dissolve_classify(vd_ctx* c);      // Alg. 5 lines 3-5: restricted VD on the boundary (child context) -> V_B / V_I
+void dissolve_release(vd_ctx* c);
 vd_status stage_index(vd_ctx* c);                  // S1  vd_index.cu
 vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out);  // S2 as a kernel (vd_nearest, vnn)
 vd_status stage_seed(vd_ctx* c);                   // S3  vd_clip.cu

@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
     const Pair pr = load_pair(A, begin + t);
     int np, nc;
     init_poly_3d<P3, C3, BOX>(S[w], A, pr, np, nc);
-    const int rc = preclip_3d(S[w], A, pr.i, pr.u, &A.pairs[begin + t], np, nc, lc);
+    const int rc = preclip_3d(S[w], A, pr.a, pr.i, pr.u, &A.pairs[begin + t], np, nc, lc);
     int failed = 0;
     if (rc == 1) { defer_pair(A, begin + t); np = -1; }
     if (rc == 2) { failed = 1; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }

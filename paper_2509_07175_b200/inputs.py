@@ -114,6 +114,14 @@ def torus_mesh(nu: int, nv: int, R: float = 1.0, r: float = 0.35):
     return verts.astype(np.float64), tris.reshape(-1, 3).astype(np.int32)
 
 
+def octahedron_mesh():
+    """Regular octahedron |x| + |y| + |z| <= 1 as 8 tetrahedra around the origin: a convex domain that is not a box
+    (8 boundary triangles in 8 distinct planes)."""
+    verts = np.array([[0, 0, 0], [1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]], dtype=np.float64)
+    tets = [(0, 1 + (sx < 0), 3 + (sy < 0), 5 + (sz < 0)) for sx in (1, -1) for sy in (1, -1) for sz in (1, -1)]
+    return verts, np.array(tets, dtype=np.int32)
+
+
 def mesh_measure(verts: np.ndarray, simplices: np.ndarray, kind: int) -> float:
     """|M| from the mesh itself (plain determinant / cross-product formulas)."""
     p = verts[simplices]

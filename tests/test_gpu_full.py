@@ -74,3 +74,28 @@ def test_box_domain_at_scale(dim, n, k):
     ids = _sample(g, n, k, 77 + dim)
     o = oracle.compute(w.sites, w.verts, None, w.kind, subset=ids, tier="B")
     parity.assert_parity(g, o, w.diameter, ids=ids, simplex_measure=parity.simplex_measures(w))
+
+
+def test_c2_dissolve_mode_all_cells():
+    """Alg. 5's site division at full size (C2: 100,000 sites, 48,000 tets): every cell's measure, centroid and neighbour set
+    equal the per-piece run's (itself oracle-checked above), 512 sampled cells equal the oracle's dissolved kind element by
+    element, and the counters say what the mode saves."""
+    w = inputs.config(2)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        ctx.compute()
+        plain, c0 = ctx.to_host(), ctx.counters()
+        ctx.set_options(dissolve=1)
+        ctx.compute()
+        g, c1 = ctx.to_host(), ctx.counters()
+    assert np.array_equal(g.nbr_off, plain.nbr_off) and np.array_equal(g.nbr, plain.nbr)
+    assert np.allclose(g.measure, plain.measure, rtol=1e-9, atol=0)
+    assert np.abs(g.centroid - plain.centroid).max() <= 1e-9 * w.diameter
+    whole = (g.piece_simplex == w.m)
+    assert 0.8 * w.n < whole.sum() < 0.95 * w.n and (np.diff(g.piece_off)[g.piece_simplex[g.piece_off[:-1]] == w.m] == 1).all()
+    assert c1["pairs"] < 0.25 * c0["pairs"] and c1["queries"] < 0.6 * c0["queries"]
+    print(f"C2 dissolve: {int(whole.sum())} whole cells, pairs {c0['pairs']} -> {c1['pairs']}, queries per cell "
+          f"{c0['queries'] / w.n:.1f} -> {c1['queries'] / w.n:.1f} (paper, serial Alg. 2 on 1 M cells in a cube: 20.5, P:L375)")
+    ids = _sample(g, w.n, 512, 4242)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, subset=ids, tier="B", dissolve=True)
+    parity.assert_parity(g, o, w.diameter, simplex_measure=parity.simplex_measures(w).max())

@@ -481,3 +481,76 @@ def test_one_simplex_many_cells(kind):
             ids, counts = np.unique(fl[fl >= 0], return_counts=True)
             nedges.append(counts.max() if len(counts) else 0)
         assert max(nedges) > 8
+
+
+# ---------------------------------------------------------------------- Alg. 5's site division, dissolved output
+def _dissolve_case(name):
+    rng = np.random.default_rng(71)
+    if name == "octahedron":
+        v, t = inputs.octahedron_mesh()
+        return inputs.custom(inputs.KIND_TET_3D, rng.random((3000, 3)) * 2.0 - 1.0, v, t, "octahedron")
+    if name == "cube_outside":
+        v, t = inputs.cube_kuhn_mesh(3)
+        return inputs.custom(inputs.KIND_TET_3D, rng.random((2500, 3)) * 1.3 - 0.15, v, t, "cube_outside")
+    return inputs.config(int(name), "small")
+
+
+@pytest.mark.parametrize("name,opts", [("2", {}), ("2", dict(small_wave=-1)), ("2", dict(persistent=3)), ("2", dict(persistent=0)),
+                                       ("3", {}), ("3", dict(small_wave=-1)), ("5", {}), ("octahedron", {}),
+                                       ("octahedron", dict(small_wave=-1, near_clips=-1)), ("cube_outside", dict(small_wave=-1))])
+def test_dissolve_mode_parity(name, opts):
+    """vd_options.dissolve on convex tet meshes: boundary cells (non-empty restricted cell on the boundary triangles) come tet
+    by tet, found by the flood over negative flags; interior cells come as one whole piece with simplex id m; sites outside
+    the domain whose cell misses it own nothing.  Element by element against the oracle's dissolved kind."""
+    w = _dissolve_case(name)
+    g, cnt, _ = _gpu(w, dissolve=1, **opts)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, dissolve=True, tier="B")
+    parity.assert_parity(g, o, w.diameter)
+    assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
+    whole = g.piece_simplex == w.m
+    if name != "5":
+        assert whole.any() and not whole.all()
+        plain, cnt0, _ = _gpu(w)
+        assert cnt["pairs"] < cnt0["pairs"]                       # interior cells are one pair each, not one per tet
+        assert np.allclose(g.measure, plain.measure, rtol=1e-10, atol=1e-16)
+    else:
+        assert not whole.any()                                      # every site lies outside the cube: no interior site (U13)
+
+
+def test_dissolve_mode_rejects_what_it_cannot_do():
+    v, t = inputs.cube_kuhn_mesh(2)
+    s = np.random.default_rng(3).random((300, 3))
+    keep = np.ones(len(t), bool)
+    keep[:6] = False                                                # drop one sub-cube: the domain is no longer convex
+    with binding.Context(s) as ctx:
+        ctx.set_options(dissolve=1)
+        ctx.set_domain(v, t[keep], 2)
+        with pytest.raises(binding.VdError) as e:
+            ctx.compute()
+        assert e.value.status == 1 and "convex" in str(e.value)
+        ctx.set_options()                                            # per-piece mode still works on it
+        ctx.compute()
+        assert abs(ctx.to_host().measure.sum() - (1.0 - 1.0 / 8)) <= 1e-12
+    v2, t2 = inputs.unit_square_mesh()
+    with binding.Context(s[:, :2]) as ctx:
+        ctx.set_options(dissolve=1)
+        ctx.set_domain(v2, t2, 0)
+        with pytest.raises(binding.VdError) as e:
+            ctx.compute()
+        assert e.value.status == 1
+
+
+def test_dissolve_mode_follows_moving_sites():
+    """The boundary classification is redone for the current sites: Lloyd steps in dissolve mode equal the per-piece ones."""
+    w = inputs.config(2, "small")
+    with binding.Context(w.sites) as ctx:
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        a = ctx.lloyd(2)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_options(dissolve=1)
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        b = ctx.lloyd(2)
+        g = ctx.to_host()
+    assert np.abs(a - b).max() <= 1e-11
+    o = oracle.compute(b, w.verts, w.simplices, w.kind, dissolve=True, tier="B")
+    parity.assert_parity(g, o, w.diameter)

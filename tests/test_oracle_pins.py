@@ -370,3 +370,50 @@ def test_box_cells_qhull_and_tiers():
         assert abs(vol - a.measure[i]) <= 1e-9 * vol
         checked += 1
     assert checked > 40
+
+
+# ---------------------------------------------------------------------- dissolved output (Alg. 5)
+@pytest.mark.parametrize("domain", ["cube", "octahedron"])
+def test_dissolved_cells_are_the_union_of_their_pieces(domain):
+    """The oracle's dissolved kind against its per-piece kind and against Qhull: a cell that does not reach the boundary of
+    the convex domain comes as one piece (simplex id m) that is the union of its per-simplex pieces -- same measure,
+    centroid and neighbour set --, an ordinary Voronoi cell (Qhull volume, V = 2F - 4, site labels only); every other
+    cell keeps exactly its pieces."""
+    from scipy.spatial import ConvexHull, Voronoi
+    rng = np.random.default_rng(61)
+    if domain == "cube":
+        v, t = inputs.cube_kuhn_mesh(3)
+        s = rng.random((600, 3)) * 1.1 - 0.05             # a few sites outside the cube
+    else:
+        v, t = inputs.octahedron_mesh()
+        s = rng.random((1500, 3)) * 2.0 - 1.0             # many sites outside the octahedron, inside its bounding box
+    m = len(t)
+    plain = oracle.compute(s, v, t, inputs.KIND_TET_3D)
+    for tier in ("A", "B"):
+        dis = oracle.compute(s, v, t, inputs.KIND_TET_3D, dissolve=True, tier=tier)
+        assert np.allclose(dis.measure, plain.measure, rtol=1e-11, atol=1e-15)
+        assert np.abs(dis.centroid - plain.centroid).max() <= 1e-11
+        assert np.array_equal(dis.nbr_off, plain.nbr_off) and np.array_equal(dis.nbr, plain.nbr)
+    vor = Voronoi(s)
+    whole = 0
+    for i in range(len(s)):
+        pp = list(plain.pieces(i))
+        touches = any((plain.piece_verts(p)[1] == ~m).any() for p in pp)
+        dp = list(dis.pieces(i))
+        if not pp:
+            assert not dp
+        elif touches:
+            assert [int(dis.piece_simplex[p]) for p in dp] == [int(plain.piece_simplex[p]) for p in pp]
+            for a, b in zip(dp, pp):
+                assert np.array_equal(dis.piece_verts(a)[1], plain.piece_verts(b)[1])
+                assert np.abs(dis.piece_verts(a)[0] - plain.piece_verts(b)[0]).max() <= 1e-12    # (tier B against tier A: rounding)
+        else:
+            assert len(dp) == 1 and dis.piece_simplex[dp[0]] == m
+            xyz, fl = dis.piece_verts(dp[0])
+            assert (fl >= 0).all() and xyz.shape[0] == 2 * len(np.unique(fl)) - 4
+            region = vor.regions[vor.point_region[i]]
+            assert -1 not in region
+            vol = ConvexHull(vor.vertices[region]).volume
+            assert abs(vol - dis.measure[i]) <= 1e-9 * vol
+            whole += 1
+    assert whole > 30 and whole < (plain.measure > 0).sum()
