@@ -8,7 +8,12 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvd.so")
-SOURCES = ["vd_api.cu", "vd_domain.cu", "vd_index.cu", "vd_clip.cu", "vd_phase.cu", "vd_assemble.cu", "vd_peak.cu"]
+# (source, object suffix, extra flags): the clip / phase kernels are compiled twice -- lean (optional query features compiled
+# out) and full -- into namespaces of their own (header of csrc/vd_clip.cu)
+LEAN = ["-DVD_EXT=0", "-DVD_VARIANT=lean"]
+FULL = ["-DVD_EXT=1", "-DVD_VARIANT=full"]
+SOURCES = [("vd_clip.cu", "_lean", LEAN), ("vd_phase.cu", "_lean", LEAN), ("vd_clip.cu", "_full", FULL), ("vd_phase.cu", "_full", FULL),
+           ("vd_api.cu", "", []), ("vd_domain.cu", "", []), ("vd_index.cu", "", []), ("vd_assemble.cu", "", []), ("vd_peak.cu", "", [])]
 
 
 def lib_path() -> str:
@@ -16,16 +21,17 @@ def lib_path() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    srcs = [os.path.join(CSRC, s) for s in SOURCES]
+    srcs = [(os.path.join(CSRC, s), sfx, fl) for s, sfx, fl in SOURCES]
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "vd.h")]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     extra = os.environ.get("VD_NVCC_FLAGS", "").split()   # experiments: -DVD_... switches of the kernels
 
-    def compile_one(s):
-        o = s[:-3] + ".o"
+    def compile_one(item):
+        s, sfx, flags = item
+        o = s[:-3] + sfx + ".o"
         cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-               "-Xcompiler", "-fPIC"] + extra + ["-c", s, "-o", o]
+               "-Xcompiler", "-fPIC"] + flags + extra + ["-c", s, "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)

@@ -427,9 +427,11 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     cudaEventRecord(c->ev[0], st);
     if ((s = stage_index(c))) return s;
     cudaEventRecord(c->ev[1], st);
-    if ((s = stage_seed(c))) return s;
+    // the full kernels only where a feature they alone carry is in use (header of vd_clip.cu)
+    const bool ext = (c->weighted && c->dim == 3) || c->opt.step_out > 0 || c->opt.count_alg > 0;
+    if ((s = ext ? full::stage_seed(c) : lean::stage_seed(c))) return s;
     cudaEventRecord(c->ev[2], st);
-    if ((s = stage_clip(c))) return s;
+    if ((s = ext ? full::stage_clip(c) : lean::stage_clip(c))) return s;
     cudaEventRecord(c->ev[3], st);
     const unsigned err = c->hostControl.err;
     if (err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) {

@@ -106,7 +106,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
         const double4 p = g.sites[B.base[owner] + t];
         const double dx = B.qx[cu] - p.x, dy = B.qy[cu] - p.y, dz = B.qz[cu] - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
-        if (g.sitesW) d2 += __ldg(&g.sitesW[B.base[owner] + t]);
+        if (has_weights(g)) d2 += __ldg(&g.sitesW[B.base[owner] + t]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
         better = closer(d2, id, B.best[cu], B.bestId[cu]);
       }
@@ -199,7 +199,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
     }
   }
   st.queries += (unsigned)(nq - __popc(looseMask));
-  if (gTop.countAlg) {
+  if (counts_alg(gTop)) {
     // D_alg of the batched queries (the loose ones count inside nearest())
     unsigned v = 0;
     if (lane < nq && !((looseMask >> lane) & 1u)) v = ball_sites(gTop, B.qx[lane], B.qy[lane], B.qz[lane], B.best[lane]);

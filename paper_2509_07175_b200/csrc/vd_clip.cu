@@ -6,7 +6,11 @@
 #include "vd_clip2d.cuh"
 #include "vd_clip3d.cuh"
 
+// This file (and vd_phase.cu) is compiled TWICE (build.py): as namespace vd::lean with VD_EXT = 0 -- the kernels without the code
+// of the optional query features (weighted 3-D sites, step-out, D_alg counting) -- and as vd::full with VD_EXT = 1.  The kernels
+// are bound by instruction fetch: the lean ones are 4-7 % faster on the BASELINE configs.  vd_compute picks per call.
 namespace vd {
+namespace VD_VARIANT {
 
 // S3 (Alg. 2 line 4: the first corner; Alg. 4 lines 3-6: the centroid): the nearest site of a corner of
 // T_a owns that corner, so (T_a, N_p) is a non-empty pair and p is its witness.  One corner per simplex by default
@@ -467,4 +471,5 @@ vd_status stage_clip(vd_ctx* c) {
   return cuda_check(c, cudaGetLastError(), "clip");
 }
 
+}  // namespace VD_VARIANT
 }  // namespace vd

@@ -553,7 +553,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
       S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
       S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
       S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
-      S.u[12] = A.siteW ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
+      S.u[12] = (VD_EXT && A.siteW) ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
     }
     if (lane < 6) {
       const int axis = lane >> 1, hiSide = lane & 1;
@@ -593,7 +593,7 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
         S.u[3] = s0; S.u[4] = s1; S.u[5] = s2;
         S.u[6] = s0 - o0; S.u[7] = s1 - o1; S.u[8] = s2 - o2;
         S.u[9] = pr.wx - o0; S.u[10] = pr.wy - o1; S.u[11] = pr.wz - o2;
-        S.u[12] = A.siteW ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
+        S.u[12] = (VD_EXT && A.siteW) ? __ldg(&A.siteW[i]) : 0.0; S.u[13] = 0.0;
       }
     }
     __syncwarp();
@@ -636,7 +636,7 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
   const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
                wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
   const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
-  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + ((A.siteW ? __ldg(&A.siteW[j]) : 0.0) - S.u[12]));
+  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (((VD_EXT && A.siteW) ? __ldg(&A.siteW[j]) : 0.0) - S.u[12]));
   // the corner farthest beyond the plane starts R_p
   double far = 0.0;
   int p = 0x7fffffff;

@@ -321,7 +321,7 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
       const double4 p = g.sites[base[owner] + t];
       const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
-      const double pw = g.sitesW ? __ldg(&g.sitesW[base[owner] + t]) : 0.0;
+      const double pw = has_weights(g) ? __ldg(&g.sitesW[base[owner] + t]) : 0.0;
       const double dq2 = dx * dx + dy * dy + dz * dz + pw;
       bool cand = id != i && id != j && dq2 < r2 * (1.0 - 1e-13);
       if (cand && !(dq2 < r2 * (1.0 - 1e-9)))
@@ -337,7 +337,7 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
   }
   warp_argmin(tb, jb);
   if (closer(tb, jb, tbest, jbest)) { tbest = tb; jbest = jb; }
-  if (gTop.countAlg) extra_cnt_add(4, lane == 0 ? ball_sites(gTop, qx, qy, qz, r2) : 0u);   // the search needs every site of this ball
+  if (counts_alg(gTop)) extra_cnt_add(4, lane == 0 ? ball_sites(gTop, qx, qy, qz, r2) : 0u);   // the search needs every site of this ball
   return true;
 }
 
@@ -393,7 +393,7 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
                                              double* out4, QBatch* qb, QueryStats& st, unsigned& iters) {
   const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
   double nx, ny, nz, d;
-  if (g.stepMode) {   // section VI-A (vd_options.step_out): shorten the segment first
+  if (has_step_out(g)) {   // section VI-A (vd_options.step_out): shorten the segment first
     double pt[3] = {ptx, pty, ptz};
     const int probes = step_out<HV>(g, i, j, u, psx, psy, psz, pt, flags, nflags, st);
     if (probes) { ptx = pt[0]; pty = pt[1]; ptz = pt[2]; extra_cnt_add(3, (unsigned)probes); }

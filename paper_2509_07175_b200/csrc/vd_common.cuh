@@ -62,7 +62,16 @@ struct GridIndex {
   const double* __restrict__ siteWid;
 };
 
-__device__ __forceinline__ double site_w(const GridIndex& g, int id) { return g.siteWid ? __ldg(&g.siteWid[id]) : 0.0; }
+// The optional features of a query (weighted sites, step-out, D_alg counting) behind three predicates: the kernels exist in
+// a lean form (EXT = false: the predicates are compile-time false, the code behind them is gone) and a full form -- the
+// clip kernels are bound by instruction fetch, and every resident-but-unused code path costs them.
+#ifndef VD_EXT
+#define VD_EXT 1
+#endif
+__device__ __forceinline__ bool has_weights(const GridIndex& g) { return VD_EXT && g.sitesW != nullptr; }
+__device__ __forceinline__ bool has_step_out(const GridIndex& g) { return VD_EXT && g.stepMode != 0; }
+__device__ __forceinline__ bool counts_alg(const GridIndex& g) { return VD_EXT && g.countAlg != 0; }
+__device__ __forceinline__ double site_w(const GridIndex& g, int id) { return has_weights(g) ? __ldg(&g.siteWid[id]) : 0.0; }
 
 constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
 

@@ -4,6 +4,9 @@
 #include <vector>
 
 #include "../../include/vd.h"
+#ifndef VD_VARIANT
+#define VD_VARIANT full
+#endif
 #include "vd_common.cuh"
 
 namespace vd {
@@ -152,8 +155,9 @@ vd_status stage_dissolve_classify(vd_ctx* c);      // Alg. 5 lines 3-5: restrict
 void dissolve_release(vd_ctx* c);
 vd_status stage_index(vd_ctx* c);                  // S1  vd_index.cu
 vd_status stage_nearest_points(vd_ctx* c, const double* q3, int64_t nq, int* out);  // S2 as a kernel (vd_nearest, vnn)
-vd_status stage_seed(vd_ctx* c);                   // S3  vd_clip.cu
-vd_status stage_clip(vd_ctx* c);                   // S4+S5  vd_clip.cu
+// S3 and S4+S5 (vd_clip.cu, vd_phase.cu) exist twice: lean (no optional query features compiled in) and full
+namespace lean { vd_status stage_seed(vd_ctx* c); vd_status stage_clip(vd_ctx* c); }
+namespace full { vd_status stage_seed(vd_ctx* c); vd_status stage_clip(vd_ctx* c); }
 vd_status stage_assemble(vd_ctx* c);               // S6  vd_assemble.cu
 
 }  // namespace vd

@@ -110,7 +110,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         const double4 p = g.sites[base[owner] + t];
         const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
-        if (g.sitesW) d2 += __ldg(&g.sitesW[base[owner] + t]);
+        if (has_weights(g)) d2 += __ldg(&g.sitesW[base[owner] + t]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       }
       const bool better = valid && closer(d2, id, best, bestId) && !(SKIP && id == st.skip);
@@ -260,7 +260,7 @@ template <bool HV, bool SKIP = false>
 __device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                         QueryStats& st, bool nearer_ok = false) {
   nearest_impl<HV, SKIP>(g, qx, qy, qz, best, bestId, st, nearer_ok);
-  if (g.countAlg) {
+  if (counts_alg(g)) {
     if (lane_id() == 0) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][4] += ball_sites(g, qx, qy, qz, best);
     __syncwarp();
   }

@@ -15,6 +15,7 @@
 #include "vd_clip3d.cuh"
 
 namespace vd {
+namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
 
 #ifndef VD_PH_BLOCKS
 #define VD_PH_BLOCKS 4   // resident blocks per SM of the verify / fix kernels (plain index)
@@ -329,4 +330,5 @@ void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int roun
 
 PhaseCtl* phase_ctl(vd_ctx* c, int64_t) { return c->phaseLists.as<PhaseCtl>(); }
 
+}  // namespace VD_VARIANT
 }  // namespace vd
