@@ -13,6 +13,7 @@
 // Pairs pushed by k_ph_finish form the next wave (Alg. 4's L1/L2 swap).  Pairs that outgrow the fast tier
 // go to the large-capacity kernel of vd_clip.cu, as in the other modes.
 #include "vd_clip3d.cuh"
+#include "vd_tma.cuh"
 
 namespace vd {
 namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
@@ -62,6 +63,39 @@ __device__ __forceinline__ void copy_words(void* dst, const void* src, int bytes
   for (; k < n; k += kLanes) d[k] = s[k];
 }
 
+// Parked polytope -> shared memory through the TMA unit: lane 0 issues the bulk copy, every lane waits on the warp's mbarrier
+// (whose phase parity the caller keeps).  VD_NO_TMA: the per-lane load / store loops (for comparison).
+__device__ __forceinline__ void unpark(void* smem, const void* gmem, int bytes, unsigned long long* bar, unsigned& parity) {
+#ifdef VD_NO_TMA
+  copy_words(smem, gmem, bytes);
+  __syncwarp();
+#else
+  __syncwarp();   // every lane is done with what the buffer held
+  if (lane_id() == 0) tma_load(smem, gmem, (unsigned)bytes, bar);
+  tma_wait(bar, parity);
+  parity ^= 1u;
+#endif
+}
+
+// Shared memory -> parked polytope; returns when the shared-memory source may be overwritten.
+__device__ __forceinline__ void park(void* gmem, const void* smem, int bytes) {
+#ifdef VD_NO_TMA
+  copy_words(gmem, smem, bytes);
+  __syncwarp();
+#else
+  __syncwarp();   // the warp's stores to the buffer are done
+  if (lane_id() == 0) { tma_store(gmem, smem, (unsigned)bytes); tma_store_commit(); tma_store_wait_read(); }
+  __syncwarp();
+#endif
+}
+
+#define VD_WARP_BAR                                                        \
+  __shared__ unsigned long long sBar[kWarpsPerBlock];                      \
+  unsigned long long* bar = &sBar[(int)threadIdx.x / kLanes];              \
+  unsigned parity = 0u;                                                    \
+  if (lane_id() == 0) tma_bar_init(bar);                                   \
+  __syncwarp()
+
 __device__ __forceinline__ int next_item(PhaseCtl* pc, int slot, int count) {
   unsigned t = 0;
   if (lane_id() == 0) t = atomicAdd(&pc->ticket[slot], 1u);
@@ -98,7 +132,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
     if (rc == 2) { failed = 1; atomicOr(&A.ctl->err, ERR_TOPOLOGY); }
     __syncwarp();
     CellState* c = &cells[t];
-    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
+    if (np >= 0) park(&c->S, &S[w], kPolyBytes);
     if (lane == 0) { c->np = np; c->nc = nc; c->a = pr.a; c->i = pr.i; c->failed = failed; }
     __syncwarp();
   }
@@ -125,6 +159,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
+  VD_WARP_BAR;
   for (;;) {
     const int t = next_item(pc, slot, count);
     if (t < 0) break;
@@ -135,14 +170,24 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
     if (np < 0) continue;
     bool out = false;
     if (!c->failed && nc > 0) {
-      copy_words(&S[w], &c->S, kTestBytes);
-      __syncwarp();
+      unpark(&S[w], &c->S, kTestBytes, bar, parity);
       const bool any = classify_unknown_3d<PolyT, HV>(S[w], g, c->i, np, nc, st);
       for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
       out = __any_sync(kFull, out);
       if (any) {
+#ifdef VD_NO_TMA
         copy_words(c->S.cnn, S[w].cnn, (nc * 4 + 15) & ~15);
         copy_words(c->S.cstate, S[w].cstate, (nc + 15) & ~15);
+#else
+        __syncwarp();
+        if (lane == 0) {
+          tma_store(c->S.cnn, S[w].cnn, (unsigned)((nc * 4 + 15) & ~15));
+          tma_store(c->S.cstate, S[w].cstate, (unsigned)((nc + 15) & ~15));
+          tma_store_commit();
+          tma_store_wait_read();
+        }
+        __syncwarp();
+#endif
       }
     }
     if (lane == 0) {
@@ -173,6 +218,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
+  VD_WARP_BAR;
   for (;;) {
     const int t = next_item(pc, tslot, count);
     if (t < 0) break;
@@ -180,8 +226,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
     const int i = c->i;
-    copy_words(&S[w], &c->S, kPolyBytes);
-    __syncwarp();
+    unpark(&S[w], &c->S, kPolyBytes, bar, parity);
     int failed = 0;
     for (int guard = 0; guard < 4 * P3 && nc > 0; ++guard) {
       int s;
@@ -191,8 +236,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
       if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
       if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
     }
-    __syncwarp();
-    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
+    if (np >= 0) park(&c->S, &S[w], kPolyBytes);
     if (lane == 0) {
       c->np = np; c->nc = nc; c->failed = failed;
       list[t] = np >= 0 ? slot : -1;
@@ -229,6 +273,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
+  VD_WARP_BAR;
   for (;;) {
     const int t = next_item(pc, tslot, count);
     if (t < 0) break;
@@ -237,8 +282,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
     const int i = c->i;
-    copy_words(&S[w], &c->S, kPolyBytes);
-    __syncwarp();
+    unpark(&S[w], &c->S, kPolyBytes, bar, parity);
     int failed = 0;
     for (int guard = 0; guard < 8 * P3 + 32 && nc > 0; ++guard) {
       int s;
@@ -251,8 +295,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __
       if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
       if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
     }
-    __syncwarp();
-    if (np >= 0) copy_words(&c->S, &S[w], kPolyBytes);
+    if (np >= 0) park(&c->S, &S[w], kPolyBytes);
     if (lane == 0) {
       c->np = np; c->nc = nc; c->failed = failed;
       if (np >= 0) doneList[atomicAdd(&pc->nDone, 1u)] = slot;
@@ -272,14 +315,14 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
   QueryStats st = {0u, 0u, 0u};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
+  VD_WARP_BAR;
   WarpPool wp = {0ull, 0ull, 0, 0, vchunk, nchunk};
   // uniform work per piece: a static stride instead of a ticket (one same-address atomic less per piece)
   const int stride = (int)gridDim.x * kWarpsPerBlock;
   for (int t = (int)blockIdx.x * kWarpsPerBlock + w; t < count; t += stride) {
     const int slot = list[t];
     const CellState* c = &cells[slot];
-    copy_words(&S[w], &c->S, kPolyBytes);
-    __syncwarp();
+    unpark(&S[w], &c->S, kPolyBytes, bar, parity);
     finish_piece_3d(S[w], A, begin + slot, c->a, c->i, c->np, c->nc, S[w].u[0], S[w].u[1], S[w].u[2], c->failed != 0, lc, &wp);
     __syncwarp();
   }
