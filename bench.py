@@ -301,6 +301,20 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
         dissolve = {"ms_per_step": float(np.mean(ts)), "value": w.n / (float(np.mean(ts)) * 1e-3), "unit": UNIT, "pairs": dc["pairs"],
                     "queries_per_cell": dc["queries"] / w.n, "paper_queries_per_cell_serial_alg2_cube": 20.54,
                     "timing": "library events around vd_compute (stage total), L2 flushed between steps"}
+    # Lloyd iterations on the device (section VII-D, density 1; --lloyd IT): wall time of vd_lloyd, with and without the
+    # reuse of the previous iteration's neighbours as first clips (vd_options.reuse_nbrs)
+    lloyd = None
+    if args.lloyd > 0:
+        lloyd = {"iterations": args.lloyd, "paper": "5 M sites x 100 iterations in 31.07 s on an RTX 3080, fp32 (P:L492): another machine, context only"}
+        for name, o in (("reuse_nbrs", {}), ("no_reuse", dict(reuse_nbrs=-1))):
+            ctx.update_sites(d_sites)
+            ctx.set_options(**o)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ctx.lloyd(args.lloyd)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            lloyd[name] = {"seconds": dt, "ms_per_iteration": 1e3 * dt / (args.lloyd + 1), "computes": args.lloyd + 1}
     ctx.destroy()
 
     # end to end through the C ABI with host buffers: create, set_domain, compute, copy back, destroy
@@ -349,6 +363,7 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
                      "clips": cnt["clips"] / w.n, "pieces": cnt["pieces"] / w.n},
         "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
         "dissolve_mode": dissolve,
+        "lloyd": lloyd,
         "roofline": {"bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x max SM clock (DESIGN.md); no FP64 peak in MEASURED_PEAKS.json",
@@ -374,6 +389,7 @@ def main():
                     "1..5: only that config")
     ap.add_argument("--box", type=int, default=0, help="instead of a BASELINE config: N white-noise sites in the unit cube, the cube itself "
                     "as a simple domain (VD_BOX_3D; the setting of the paper's Fig. 1 / Table VI)")
+    ap.add_argument("--lloyd", type=int, default=0, help="also time vd_lloyd with this many iterations (with --box: the paper's CVT setting)")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -148,6 +148,30 @@ __global__ void __launch_bounds__(kBlock) k_move_sites(const double* __restrict_
   }
 }
 
+// Lloyd iterations, whole-cell kinds (vd_options.reuse_nbrs): the neighbours of cell i in this iteration are the
+// first clips of its cell in the next one -- sites move little between iterations, so nearly all of them bound the new cell
+// too, and any B_ij is a valid clip of Omega_i anyway (Eq. 1; reading U19).  Up to K of them per site, nearest first (the
+// clips of near sites shrink the polytope fastest), -1 padded; replaces the nearest-site lookup of k_near.
+__global__ void __launch_bounds__(kBlock) k_near_from_nbrs(const int64_t* __restrict__ nbrOff, const int* __restrict__ nbr,
+                                                            const double* __restrict__ sites3, int64_t n, int K, int* __restrict__ list) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double x = sites3[i * 3 + 0], y = sites3[i * 3 + 1], z = sites3[i * 3 + 2];
+    int ids[32];
+    double ds[32];
+    int cnt = 0;
+    for (int64_t k = nbrOff[i]; k < nbrOff[i + 1]; ++k) {
+      const int j = nbr[k];
+      const double dx = sites3[(int64_t)j * 3 + 0] - x, dy = sites3[(int64_t)j * 3 + 1] - y, dz = sites3[(int64_t)j * 3 + 2] - z;
+      const double d2 = dx * dx + dy * dy + dz * dz;
+      int t = cnt < K ? cnt++ : K;          // insertion into the K nearest so far
+      if (t == K) { if (!(d2 < ds[K - 1])) continue; t = K - 1; }
+      while (t > 0 && ds[t - 1] > d2) { ds[t] = ds[t - 1]; ids[t] = ids[t - 1]; --t; }
+      ds[t] = d2; ids[t] = j;
+    }
+    for (int t = 0; t < K; ++t) list[i * K + t] = t < cnt ? ids[t] : -1;
+  }
+}
+
 __global__ void __launch_bounds__(kBlock) k_unpad3(const double* __restrict__ in3, int64_t n, int dim, double* __restrict__ out) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     for (int a = 0; a < dim; ++a) out[i * dim + a] = in3[i * 3 + a];
@@ -497,6 +521,15 @@ vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) 
   if (blocks > sm_count() * 16) blocks = sm_count() * 16;
   for (int it = 0; it < iterations; ++it) {
     if ((s = vd_compute(c, out))) return s;
+    if (c->opt.reuse_nbrs >= 0 && c->kind == VD_BOX_3D && !c->weighted && c->nearList.p) {
+      int K = c->opt.near_clips == 0 ? 20 : c->opt.near_clips;
+      if (K > kLanes) K = kLanes;
+      if (K > 0) {
+        VD_LAUNCH(k_near_from_nbrs, blocks, kBlock, 0, c->stream)(c->oNbrOff.as<int64_t>(), c->oNbr.as<int>(), c->sites.as<double>(), c->n, K,
+                                                                  c->nearList.as<int>());
+        c->nearReady = true;
+      }
+    }
     VD_LAUNCH(k_move_sites, blocks, kBlock, 0, c->stream)(c->oMeasure.as<double>(), c->oCentroid.as<double>(), c->n, c->dim,
                                                          c->sites.as<double>());
     c->indexValid = false;

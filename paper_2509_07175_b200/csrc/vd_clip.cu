@@ -303,7 +303,8 @@ vd_status stage_seed(vd_ctx* c) {
         A, b.measure, b.piece_off, b.piece_simplex, b.vert_off, b.vert_xyz, c->bTet.as<int>(), c->bPlanes.as<double4>(), c->nBPlanes, 1e-12);
     return cuda_check(c, cudaGetLastError(), "seed (dissolve)");
   }
-  if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+  if (K > 0 && !c->nearReady) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+  c->nearReady = false;   // (set by vd_lloyd: the list holds the previous iteration's neighbours)
   VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
   const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;
   const int64_t mLocal = A.aEnd - A.aBegin;

@@ -55,6 +55,7 @@ struct vd_ctx {
   bool weighted = false;   // vd_create_weighted: dim 2 -> sites lifted to R^3, VD_TRI_2D runs as a flat surface;
                            //                     dim 3 -> siteW holds the additive term eta - w_i of every site
   int64_t syncs = 0;       // host waits on the stream inside the current vd_compute
+  bool nearReady = false;  // nearList already holds the first clips of the next compute (vd_lloyd: the previous neighbours)
   int heavyKnown = -1;     // refined cells of the site index as last built, while sites and grid options are unchanged; else -1
   bool haveDomain = false, haveResult = false, indexValid = false;
   cudaStream_t stream = nullptr;
