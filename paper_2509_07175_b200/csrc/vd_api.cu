@@ -6,6 +6,8 @@
 
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>   // header-only: ranges cost nothing unless a profiler is attached
+
 #include "vd_internal.h"
 
 namespace vd {
@@ -448,14 +450,16 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     if ((s = alloc_pools(c))) return s;
     if ((s = ensure(c, c->control, sizeof(Control)))) return s;
     cudaMemsetAsync(c->control.p, 0, sizeof(Control), st);
+    // NVTX ranges per stage: host-side brackets of where each stage is enqueued / waited for
+    struct Range { explicit Range(const char* name) { nvtxRangePushA(name); } ~Range() { nvtxRangePop(); } };
     cudaEventRecord(c->ev[0], st);
-    if ((s = stage_index(c))) return s;
+    { Range r("vd S1 site index"); if ((s = stage_index(c))) return s; }
     cudaEventRecord(c->ev[1], st);
     // the full kernels only where a feature they alone carry is in use (header of vd_clip.cu)
     const bool ext = (c->weighted && c->dim == 3) || c->opt.step_out > 0 || c->opt.count_alg > 0;
-    if ((s = ext ? full::stage_seed(c) : lean::stage_seed(c))) return s;
+    { Range r("vd S3 seeds"); if ((s = ext ? full::stage_seed(c) : lean::stage_seed(c))) return s; }
     cudaEventRecord(c->ev[2], st);
-    if ((s = ext ? full::stage_clip(c) : lean::stage_clip(c))) return s;
+    { Range r("vd S4+S5 clip and propagate"); if ((s = ext ? full::stage_clip(c) : lean::stage_clip(c))) return s; }
     cudaEventRecord(c->ev[3], st);
     const unsigned err = c->hostControl.err;
     if (err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) {
@@ -476,7 +480,10 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     }
     break;
   }
-  if ((s = stage_assemble(c))) return s;
+  nvtxRangePushA("vd S6 assemble");
+  s = stage_assemble(c);
+  nvtxRangePop();
+  if (s) return s;
   cudaEventRecord(c->ev[4], st);
   Control h;
   cudaError_t e = cudaMemcpyAsync(&h, c->control.p, sizeof(Control), cudaMemcpyDeviceToHost, st);
