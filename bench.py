@@ -288,7 +288,7 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
     # Alg. 5's site division (vd_options.dissolve; convex tet meshes, one GPU): interior cells as whole cells.  Reported
     # beside the per-piece number, never instead of it (the per-piece output is what parity with SURVEY 8c.1 is defined on)
     dissolve = None
-    if w.kind == 2 and not sharded and cfg in (2, 5):
+    if w.kind == 2 and not sharded and cfg == 2:
         ctx.set_options(dissolve=1)
         for _ in range(2):
             ctx.compute()

@@ -560,7 +560,7 @@ void vd_destroy(vd_ctx* c) {
   dissolve_release(c);
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->scanTmp, &c->sortKeys, &c->sortVals, &c->sortHist, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
                    &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
@@ -582,7 +582,7 @@ vd_status vd_set_stream(vd_ctx* c, void* stream) {
 
 vd_status vd_set_allocator(vd_ctx* c, void* (*alloc)(size_t, void*, void*), void (*rel)(void*, void*), void* user) {
   if (!c || ((alloc == nullptr) != (rel == nullptr))) return VD_E_ARG;
-  if (c->pairs.p || c->sorted.p) { c->lastError = "vd_set_allocator must be called before the first vd_compute"; return VD_E_STATE; }
+  if (c->pairs.p || c->sorted2.p) { c->lastError = "vd_set_allocator must be called before the first vd_compute"; return VD_E_STATE; }
   c->allocFn = alloc; c->freeFn = rel; c->allocUser = user;
   return VD_OK;
 }

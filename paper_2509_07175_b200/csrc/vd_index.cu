@@ -110,21 +110,6 @@ __global__ void __launch_bounds__(kBlock) k_cell_count(const double* __restrict_
   }
 }
 
-__global__ void __launch_bounds__(kBlock) k_cell_scatter(const double* __restrict__ sites, int64_t n, const int* __restrict__ cellOf,
-                                                          const int* __restrict__ cellStart, int* __restrict__ cellFill,
-                                                          double4* __restrict__ sorted) {
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    const int c = cellOf[i];
-    const int pos = cellStart[c] + atomicSub(&cellFill[c], 1) - 1;
-    double4 p;
-    p.x = sites[i * 3 + 0];
-    p.y = sites[i * 3 + 1];
-    p.z = sites[i * 3 + 2];
-    p.w = __longlong_as_double((long long)i);
-    sorted[pos] = p;
-  }
-}
-
 // ---- second level: cells with more than kHeavy sites get a K^3 sub-grid (clustered site sets: a uniform
 // grid at the paper's density leaves thousands of sites in one cell).  K is chosen so that a sub-cell holds
 // `density` sites on average; the cell's sites are re-sorted by sub-cell key.
@@ -176,40 +161,93 @@ __device__ __forceinline__ int sub_key(const GridIndex& g, int c, int K, double 
   return (kz * Ky + ky) * Kx + kx;
 }
 
-// sites are in top-cell order in `sorted`; p = position there
-__global__ void __launch_bounds__(kBlock) k_sub_count(const GridIndex* __restrict__ gp, const double4* __restrict__ sorted, int64_t n,
-                                                       const int* __restrict__ cellOf, const int* __restrict__ subOff,
-                                                       int* __restrict__ subKey, int* __restrict__ subCount) {
+// ---- sort: ONE stable radix sort of the sites by their finest bucket ("Morton/cell-key radix sort + counting-sort bucketing",
+// BASELINE north_star (1)).  The key of site i is c + subOffRaw[c] + k: c its top cell (row-major: a run of cells along x stays
+// one contiguous range), k its sub-cell inside a refined cell (0 in a plain one); subOffRaw[c] = the sub-cells of all refined
+// cells before c, so the key is monotone in (c, k).  Input order is the site id and the sort is stable: inside a bucket the
+// sites end up in ascending id, the same in every run (the first build scattered through atomic cursors: arrival order).
+__global__ void __launch_bounds__(kBlock) k_site_keys(const GridIndex* __restrict__ gp, const double* __restrict__ sites, int64_t n,
+                                                       const int* __restrict__ cellOf, const int* __restrict__ subOff, const int* __restrict__ subOffRaw,
+                                                       unsigned* __restrict__ key, int* __restrict__ val, int* __restrict__ subCount) {
   const GridIndex g = *gp;
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-    const double4 s = sorted[p];
-    const int id = (int)(__double_as_longlong(s.w) & 0x7fffffff);
-    const int c = cellOf[id];
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int c = cellOf[i];
     const int so = subOff[c];
-    int key = -1;
+    int k = 0;
     if (so >= 0) {
-      key = sub_key(g, c, so >> 26, s.x, s.y, s.z);
-      atomicAdd(&subCount[(so & 0x3ffffff) + key], 1);
+      k = sub_key(g, c, so >> 26, sites[i * 3 + 0], sites[i * 3 + 1], sites[i * 3 + 2]);
+      atomicAdd(&subCount[(so & 0x3ffffff) + k], 1);   // (a count: the same whatever the arrival order)
     }
-    subKey[p] = key;
+    key[i] = (unsigned)(c + subOffRaw[c] + k);
+    val[i] = (int)i;
   }
 }
 
-__global__ void __launch_bounds__(kBlock) k_sub_scatter(const double4* __restrict__ sorted, int64_t n, const int* __restrict__ cellOf,
-                                                         const int* __restrict__ cellStart, const int* __restrict__ subOff,
-                                                         const int* __restrict__ subKey, const int* __restrict__ subScan,
-                                                         int* __restrict__ subCount, double4* __restrict__ sorted2) {
-  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-    const double4 s = sorted[p];
-    const int key = subKey[p];
-    int64_t dst = p;
-    if (key >= 0) {
-      const int id = (int)(__double_as_longlong(s.w) & 0x7fffffff);
-      const int c = cellOf[id];
-      const int off = subOff[c] & 0x3ffffff;
-      dst = cellStart[c] + (subScan[off + key] - subScan[off]) + (atomicSub(&subCount[off + key], 1) - 1);
+// LSD radix sort, up to 11 bits per pass (22-bit keys -- two million sites -- take two passes), one WARP per segment of kSortSeg consecutive elements (stable: segments in order, chunks of
+// 32 in order, lanes in order).  Pass = histogram per (digit, segment) -> exclusive scan in digit-major order -> scatter.
+constexpr int kSortSeg = 2048;
+constexpr int kSortWarps = 4, kSortDigits = 2048;   // per block: 4 warps x 2048 counters = 32 KB of shared memory
+
+__device__ __forceinline__ unsigned match_digit(unsigned active, unsigned d) { return __match_any_sync(active, d); }
+
+__global__ void __launch_bounds__(kSortWarps * kLanes) k_radix_hist(const unsigned* __restrict__ key, int64_t n, int shift, int dbits, int nseg, int* __restrict__ hist) {
+  __shared__ int cnt[kSortWarps][kSortDigits];
+  const int nd = 1 << dbits;
+  const unsigned dmask = (unsigned)nd - 1u;
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  const int64_t seg = (int64_t)blockIdx.x * kSortWarps + w;
+  for (int d = lane; d < nd; d += kLanes) cnt[w][d] = 0;
+  __syncwarp();
+  if (seg < nseg) {
+    const int64_t b = seg * kSortSeg, e = b + kSortSeg < n ? b + kSortSeg : n;
+    for (int64_t p0 = b; p0 < e; p0 += kLanes) {
+      const int64_t p = p0 + lane;
+      const unsigned active = __ballot_sync(kFull, p < e);
+      if (p < e) {
+        const unsigned d = (key[p] >> shift) & dmask;
+        const unsigned m = match_digit(active, d);
+        if ((int)(__ffs((int)m) - 1) == lane) cnt[w][d] += __popc(m);   // one lane per distinct digit
+      }
+      __syncwarp();
     }
-    sorted2[dst] = s;
+    for (int d = lane; d < nd; d += kLanes) hist[(int64_t)d * nseg + seg] = cnt[w][d];
+  }
+}
+
+__global__ void __launch_bounds__(kSortWarps * kLanes) k_radix_scatter(const unsigned* __restrict__ key, const int* __restrict__ val, int64_t n, int shift, int dbits, int nseg,
+                                                           const int* __restrict__ scanned, unsigned* __restrict__ keyOut, int* __restrict__ valOut) {
+  __shared__ int off[kSortWarps][kSortDigits];
+  const int nd = 1 << dbits;
+  const unsigned dmask = (unsigned)nd - 1u;
+  const int w = (int)threadIdx.x / kLanes, lane = lane_id();
+  const int64_t seg = (int64_t)blockIdx.x * kSortWarps + w;
+  if (seg >= nseg) return;
+  for (int d = lane; d < nd; d += kLanes) off[w][d] = scanned[(int64_t)d * nseg + seg];
+  __syncwarp();
+  const int64_t b = seg * kSortSeg, e = b + kSortSeg < n ? b + kSortSeg : n;
+  for (int64_t p0 = b; p0 < e; p0 += kLanes) {
+    const int64_t p = p0 + lane;
+    const unsigned active = __ballot_sync(kFull, p < e);
+    unsigned k = 0, d = 0, m = 0;
+    int v = 0, dst = 0;
+    if (p < e) {
+      k = key[p]; v = val[p];
+      d = (k >> shift) & dmask;
+      m = match_digit(active, d);
+      dst = off[w][d] + __popc(m & ((1u << lane) - 1u));   // earlier lanes with the same digit go first
+    }
+    __syncwarp();
+    if (p < e && (int)(__ffs((int)m) - 1) == lane) off[w][d] += __popc(m);
+    __syncwarp();
+    if (p < e) { keyOut[dst] = k; valOut[dst] = v; }
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) k_gather_sorted(const double* __restrict__ sites, const int* __restrict__ order, int64_t n,
+                                                           double4* __restrict__ sorted) {
+  for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+    const int i = order[p];
+    sorted[p] = make_double4(sites[(int64_t)i * 3 + 0], sites[(int64_t)i * 3 + 1], sites[(int64_t)i * 3 + 2], __longlong_as_double((long long)i));
   }
 }
 
@@ -328,7 +366,7 @@ vd_status stage_index(vd_ctx* c) {
   if ((s = ensure(c, c->cellOf, sizeof(int) * n))) return s;
   if ((s = ensure(c, c->cellStart, sizeof(int) * (gridCap + 2)))) return s;
   if ((s = ensure(c, c->cellFill, sizeof(int) * (gridCap + 2)))) return s;
-  if ((s = ensure(c, c->sorted, sizeof(double4) * n))) return s;
+  if ((s = ensure(c, c->sorted2, sizeof(double4) * n))) return s;
   if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(n > gridCap ? n : gridCap) * 2))) return s;
   if ((s = ensure(c, c->control, sizeof(Control)))) return s;
   const int stepMode = c->opt.step_out > 0 ? (c->opt.step_out > 2 ? 2 : c->opt.step_out) : 0;
@@ -339,7 +377,7 @@ vd_status stage_index(vd_ctx* c) {
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
-                                         c->sorted.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
+                                         c->sorted2.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
                                          stepMode ? c->delta.as<double>() : nullptr, stepMode,
                                          lifted4 ? c->sortedW.as<double>() : nullptr, lifted4 ? c->siteW.as<double>() : nullptr, c->grid.as<GridIndex>(),
                                          &c->control.as<Control>()->err);
@@ -347,8 +385,6 @@ vd_status stage_index(vd_ctx* c) {
   VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
                                                               c->cellFill.as<int>());
   exclusive_scan<int, int>(c->cellFill.as<int>(), gridCap + 1, c->cellStart.as<int>(), c->scanTmp.as<int>(), st);
-  VD_LAUNCH(k_cell_scatter, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->cellOf.as<int>(), c->cellStart.as<int>(),
-                                                                c->cellFill.as<int>(), c->sorted.as<double4>());
   // second level
   const int64_t subCap = (int64_t)(4.0 * (double)n / density) + gridCap + 64;
   c->subCap = subCap;
@@ -359,8 +395,6 @@ vd_status stage_index(vd_ctx* c) {
   if ((s = ensure(c, c->subOff, sizeof(int) * (gridCap + 2)))) return s;
   if ((s = ensure(c, c->subCount, sizeof(int) * (subCap + 2)))) return s;
   if ((s = ensure(c, c->subStart, sizeof(int) * (subCap + 3)))) return s;
-  if ((s = ensure(c, c->subKey, sizeof(int) * n))) return s;
-  if ((s = ensure(c, c->sorted2, sizeof(double4) * n))) return s;
   if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(subCap > n ? subCap : n) * 2))) return s;
   GridIndex* gp = c->grid.as<GridIndex>();
   const int gb = grid_for(gridCap + 1, kBlock);
@@ -369,13 +403,33 @@ vd_status stage_index(vd_ctx* c) {
   exclusive_scan<int, int>(c->subNeed.as<int>(), gridCap + 1, c->subOffRaw.as<int>(), c->scanTmp.as<int>(), st);
   VD_LAUNCH(k_sub_pack, gb, kBlock, 0, st)(gp, density, c->subOffRaw.as<int>(), subCap, c->subOff.as<int>());
   cudaMemsetAsync(c->subCount.p, 0, sizeof(int) * (subCap + 2), st);
-  VD_LAUNCH(k_sub_count, grid_for(n, kBlock), kBlock, 0, st)(gp, c->sorted.as<double4>(), n, c->cellOf.as<int>(), c->subOff.as<int>(),
-                                                             c->subKey.as<int>(), c->subCount.as<int>());
+  // the stable radix sort by finest bucket (header of k_site_keys): keys / values ping-pong in two halves of one buffer each
+  const int nseg = (int)((n + kSortSeg - 1) / kSortSeg);
+  if ((s = ensure(c, c->sortKeys, sizeof(unsigned) * 2 * n))) return s;
+  if ((s = ensure(c, c->sortVals, sizeof(int) * 2 * n))) return s;
+  if ((s = ensure(c, c->sortHist, sizeof(int) * (kSortDigits * (size_t)nseg + 2)))) return s;
+  if ((s = ensure(c, c->scanTmp, sizeof(int64_t) * scan_scratch_elems(kSortDigits * (int64_t)nseg) * 2))) return s;
+  unsigned* keyA = c->sortKeys.as<unsigned>();
+  unsigned* keyB = keyA + n;
+  int* valA = c->sortVals.as<int>();
+  int* valB = valA + n;
+  VD_LAUNCH(k_site_keys, grid_for(n, kBlock), kBlock, 0, st)(gp, c->sites.as<double>(), n, c->cellOf.as<int>(), c->subOff.as<int>(),
+                                                             c->subOffRaw.as<int>(), keyA, valA, c->subCount.as<int>());
   exclusive_scan<int, int>(c->subCount.as<int>(), subCap + 1, c->subStart.as<int>(), c->scanTmp.as<int>(), st);
-  // subStart holds the scan for now; the scatter consumes subCount as a cursor, then the scan is rebased in place
-  VD_LAUNCH(k_sub_scatter, grid_for(n, kBlock), kBlock, 0, st)(c->sorted.as<double4>(), n, c->cellOf.as<int>(), c->cellStart.as<int>(),
-                                                               c->subOff.as<int>(), c->subKey.as<int>(), c->subStart.as<int>(),
-                                                               c->subCount.as<int>(), c->sorted2.as<double4>());
+  int bits = 1;
+  while (bits < 32 && ((int64_t)1 << bits) <= gridCap + subCap + 2) ++bits;   // keys are below gridCap + subCap
+  const int sb = (nseg + kSortWarps - 1) / kSortWarps;
+  const int npass = bits <= 11 ? 1 : (bits <= 22 ? 2 : 3);
+  const int dbits = (bits + npass - 1) / npass;
+  for (int shift = 0; shift < bits; shift += dbits) {
+    VD_LAUNCH(k_radix_hist, sb, kSortWarps * kLanes, 0, st)(keyA, n, shift, dbits, nseg, c->sortHist.as<int>());
+    exclusive_scan<int, int>(c->sortHist.as<int>(), ((int64_t)nseg << dbits), c->sortHist.as<int>(), c->scanTmp.as<int>(), st);
+    VD_LAUNCH(k_radix_scatter, sb, kSortWarps * kLanes, 0, st)(keyA, valA, n, shift, dbits, nseg, c->sortHist.as<int>(), keyB, valB);
+    unsigned* tk = keyA; keyA = keyB; keyB = tk;
+    int* tv = valA; valA = valB; valB = tv;
+  }
+  VD_LAUNCH(k_gather_sorted, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), valA, n, c->sorted2.as<double4>());
+  // subStart holds the scan of the sub-cell counts for now; it is rebased to absolute positions in place
   VD_LAUNCH(k_sub_finalize, grid_for(gridCap, kWarpsPerBlock), kBlock, 0, st)(gp, c->subOff.as<int>(), c->subStart.as<int>(),
                                                                                c->subStart.as<int>());
   VD_LAUNCH(k_grid_finish, 1, 1, 0, st)(gp, c->sorted2.as<double4>(), c->heavyPrefix.as<int>(), c->subOff.as<int>(),
