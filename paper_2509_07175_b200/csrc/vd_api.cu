@@ -89,6 +89,9 @@ void release(vd_ctx* c, DevBuf& b) {
 vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
   if (bytes < 256) bytes = 256;
   if (b.cap >= bytes) return VD_OK;
+  // a buffer that grows again gets a quarter of slack: the assemble stage sizes its buffers from pool cursors that differ
+  // by a few entries from run to run, and re-allocating a gigabyte for them costs hundreds of milliseconds
+  if (b.p) bytes += bytes / 4;
   // pending kernels may still use the old block
   if (b.p) sync_stream(c, "buffer grows");
   release(c, b);

@@ -21,6 +21,12 @@ namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
 #ifndef VD_PH_BLOCKS
 #define VD_PH_BLOCKS 4   // resident blocks per SM of the verify / fix kernels (plain index)
 #endif
+#ifndef VD_PH_BLOCKS_HV
+#define VD_PH_BLOCKS_HV 4   // the same for the kernels that know the refined index (measured on C3: 2 blocks 451 ms, 3 blocks 416 ms, 4 blocks 405 ms)
+#endif
+#ifndef VD_PH_TAIL_BLOCKS
+#define VD_PH_TAIL_BLOCKS 3
+#endif
 #ifndef VD_PHV_BLOCKS
 #define VD_PHV_BLOCKS VD_PH_BLOCKS   // the verify kernel's own (its shared memory would allow more than fix's)
 #endif
@@ -143,7 +149,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 // the wave; round r > 0 the pairs that round r-1's k_ph_fix clipped -- it runs only if that kernel ran.  A negative list
 // entry is a pair that left the path.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
+__global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
                                                      int* __restrict__ doneList, PhaseCtl* pc, int r, int tailPairs) {
   if (pc->mode != WAVE_PHASED) return;
   if (r > 0 && (int)pc->nClip[r - 1] <= tailPairs) return;
@@ -203,7 +209,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PHV_BLOCKS) k_ph_verify(Cl
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
 // Runs when round r's tests left more than tailPairs pairs with a corner outside (fewer: k_ph_tail finishes them).
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
+__global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
                                                      PhaseCtl* pc, int r, int tailPairs) {
   if (pc->mode != WAVE_PHASED || (int)pc->nClip[r] <= tailPairs) return;
   int* list = lists + (r & 1) * (int64_t)cap;
@@ -255,7 +261,7 @@ __global__ void __launch_bounds__(kBlock, HV ? 3 : VD_PH_BLOCKS) k_ph_fix(ClipAr
 // a corner outside: those pairs (tested, not clipped) are taken to completion here.  If every round ran its clips, the last
 // round's pairs (clipped, not yet re-tested) are -- so a wave always ends, whatever the number of rounds in the program.
 template <bool HV>
-__global__ void __launch_bounds__(kBlock, 3) k_ph_tail(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ lists, int cap,
+__global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs A, CellState* __restrict__ cells, const int* __restrict__ lists, int cap,
                                                        int* __restrict__ doneList, PhaseCtl* pc, int rounds, int tailPairs) {
   if (pc->mode != WAVE_PHASED) return;
   int r = 0;
