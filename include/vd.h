@@ -131,9 +131,11 @@ typedef struct vd_options {
                              get their WHOLE cell as one piece (piece_simplex = m, no simplex flags) from the whole-cell
                              kernel against the bounding box; the other (boundary) cells are clipped tet by tet as usual.
                              0 (default): every cell as per-simplex pieces.  VD_E_ARG when the mesh is not convex.        */
-  int32_t fp32_filter;    /* 1: candidate sites are first tested in fp32 (16-byte records, an error bound on the squared
-                             distance), fp64 only for the survivors -- the paper's GPU runs are fp32.  Decisions
-                             and results stay fp64-exact.  0 (default): fp64 throughout.  3D kinds, plain index.           */
+  int32_t fp32_filter;    /* 1: mixed precision -- every candidate site of a nearest-site query is first tested in fp32
+                             (16-byte float records, a rigorous error bound on the squared distance from the coordinates'
+                             magnitude); only the survivors are loaded and evaluated in fp64.  The paper's GPU runs are
+                             fp32 throughout; here decisions and results stay fp64-exact (same cells, bit for bit in
+                             structure).  0 (default): fp64 throughout.  Not combined with weighted 3-D sites.              */
   int32_t count_alg;      /* 1: also count D_alg (vd_counters.alg_evals): after every nearest-site query the sites of the
                              grid cells that meet the ball (q, |q - N_q|) -- the least an exact grid search must examine
                              (SURVEY 8d).  Slower; for measurement runs.                                                   */
@@ -164,7 +166,9 @@ typedef struct vd_counters {
   int64_t alg_evals;      /* D_alg (vd_options.count_alg), else 0                                      */
   int64_t syncs;          /* host waits on the stream inside the last vd_compute                       */
   int64_t step_probes;    /* step-out probes of section VI-A (vd_options.step_out)                     */
-  int64_t reserved[2];
+  int64_t f32_survivors;  /* vd_options.fp32_filter: candidates that passed the fp32 filter and were
+                             evaluated in fp64 (the others of dist_evals cost 16 bytes and fp32 only)  */
+  int64_t reserved[1];
 } vd_counters;
 
 /* vd_create: copy n sites of dimension dim (row-major [n][dim], fp64).  Builds nothing heavy: the

@@ -54,7 +54,7 @@ class vd_options(ctypes.Structure):
 class vd_counters(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips",
                                                "waves", "overflow_pairs", "reruns", "launches", "row_evals", "search_evals", "pre_clips",
-                                               "clip_corners", "new_corners", "fan_simplices", "alg_evals", "syncs", "step_probes")] + [("reserved", ctypes.c_int64 * 2)]
+                                               "clip_corners", "new_corners", "fan_simplices", "alg_evals", "syncs", "step_probes", "f32_survivors")] + [("reserved", ctypes.c_int64 * 1)]
 
 
 def load():

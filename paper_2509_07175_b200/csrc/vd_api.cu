@@ -459,7 +459,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     { Range r("vd S1 site index"); if ((s = stage_index(c))) return s; }
     cudaEventRecord(c->ev[1], st);
     // the full kernels only where a feature they alone carry is in use (header of vd_clip.cu)
-    const bool ext = (c->weighted && c->dim == 3) || c->opt.step_out > 0 || c->opt.count_alg > 0;
+    const bool ext = (c->weighted && c->dim == 3) || c->opt.step_out > 0 || c->opt.count_alg > 0 || c->opt.fp32_filter > 0;
     { Range r("vd S3 seeds"); if ((s = ext ? full::stage_seed(c) : lean::stage_seed(c))) return s; }
     cudaEventRecord(c->ev[2], st);
     { Range r("vd S4+S5 clip and propagate"); if ((s = ext ? full::stage_clip(c) : lean::stage_clip(c))) return s; }
@@ -503,7 +503,7 @@ vd_status vd_compute(vd_ctx* c, vd_cells* out) {
     o.row_evals = (int64_t)k.rows; o.search_iters = (int64_t)k.search_iters; o.clips = (int64_t)k.clips;
     o.search_evals = (int64_t)k.search_evals; o.pre_clips = (int64_t)k.pre_clips; o.clip_corners = (int64_t)k.clip_corners;
     o.new_corners = (int64_t)k.new_corners; o.fan_simplices = (int64_t)k.fan_simplices; o.alg_evals = (int64_t)k.alg_evals;
-    o.step_probes = (int64_t)k.step_probes;
+    o.step_probes = (int64_t)k.step_probes; o.f32_survivors = (int64_t)k.f32_survivors;
   };
   fill(c->counters, counters_total(h));
   for (int k = 0; k < kCntKinds; ++k) { memset(&c->phaseCounters[k], 0, sizeof(vd_counters)); fill(c->phaseCounters[k], h.cnt[k]); }
@@ -563,7 +563,7 @@ void vd_destroy(vd_ctx* c) {
   dissolve_release(c);
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill, &c->sorted,
-                   &c->scanTmp, &c->sortKeys, &c->sortVals, &c->sortHist, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
+                   &c->scanTmp, &c->sorted32, &c->sortKeys, &c->sortVals, &c->sortHist, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
                    &c->subKey, &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,

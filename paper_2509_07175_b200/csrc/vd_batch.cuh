@@ -22,6 +22,7 @@ struct QBatch {
   int base[kLanes];     // per packed row: first site index minus first candidate index
   unsigned char qid[kLanes];
   unsigned char flag[kQB];   // refined index: the query met a refined cell in the row pass
+  float qf[kQB][4];          // fp32 filter: the query in float, and the fp32 threshold of its current bound
 };
 
 // One pass of the batch over ONE grid view g (the top grid, the sub-grid of a refined cell, or a single plain cell seen as a
@@ -34,6 +35,12 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
   const int lane = lane_id();
   int myRows = 0;
   bool loose = false;
+  const bool f32 = has_f32(g) && !has_weights(g);
+  if (f32 && lane < nq) {
+    const double qx = B.qx[lane], qy = B.qy[lane], qz = B.qz[lane];
+    B.qf[lane][0] = (float)qx; B.qf[lane][1] = (float)qy; B.qf[lane][2] = (float)qz;
+    B.qf[lane][3] = f32_threshold(B.best[lane], f32_magnitude(g, qx, qy, qz));
+  }
   if (lane < nq && ((active >> lane) & 1u)) {
     const double b = B.best[lane];
     if (!(b < 1e300)) {
@@ -96,13 +103,23 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
       }
       __syncwarp();
       const int t = t0 + lane;
-      const bool valid = t < total;
+      bool valid = t < total;
       double d2 = 0.0;
-      int id = 0x7fffffff, cu = 0;
+      int id = 0x7fffffff, cu = 0, owner = 0;
       bool better = false;
       if (valid) {
-        const int owner = __popc(starts & ((2u << lane) - 1u)) - 1;
+        owner = __popc(starts & ((2u << lane) - 1u)) - 1;
         cu = B.qid[owner];
+      }
+      if (f32) {
+        if (valid) {
+          const float4 pf = g.sites32[B.base[owner] + t];
+          const float fx = B.qf[cu][0] - pf.x, fy = B.qf[cu][1] - pf.y, fz = B.qf[cu][2] - pf.z;
+          valid = fx * fx + fy * fy + fz * fz <= B.qf[cu][3];   // else: farther than its query's bound, whatever fp64 would say
+        }
+        extra_cnt_add(5, (unsigned)__popc(__ballot_sync(kFull, valid)));
+      }
+      if (valid) {
         const double4 p = g.sites[B.base[owner] + t];
         const double dx = B.qx[cu] - p.x, dy = B.qy[cu] - p.y, dz = B.qz[cu] - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
@@ -115,7 +132,10 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
         const int src = __ffs(m) - 1;
         const int bu = shfl(cu, src), bi = shfl(id, src);
         const double bd = shfl(d2, src);
-        if (lane == 0 && closer(bd, bi, B.best[bu], B.bestId[bu])) { B.best[bu] = bd; B.bestId[bu] = bi; }
+        if (lane == 0 && closer(bd, bi, B.best[bu], B.bestId[bu])) {
+          B.best[bu] = bd; B.bestId[bu] = bi;
+          if (f32) B.qf[bu][3] = f32_threshold(bd, f32_magnitude(g, B.qx[bu], B.qy[bu], B.qz[bu]));
+        }
         __syncwarp();
         better = better && lane != src && closer(d2, id, B.best[cu], B.bestId[cu]);
         m = __ballot_sync(kFull, better);
@@ -188,7 +208,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
                   }
                   v.n = 0; v.cellStart = gTop.cellStart + c; v.sites = gTop.sites;
                   v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
-                  v.sitesW = gTop.sitesW; v.siteWid = gTop.siteWid;
+                  v.sitesW = gTop.sitesW; v.siteWid = gTop.siteWid; v.sites32 = gTop.sites32; v.f32M = gTop.f32M;
                 }
               }
               __syncwarp();

@@ -26,7 +26,7 @@ struct alignas(16) Poly3 {
   double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   unsigned short cp[C][3];                // the corner's three planes, cyclically ordered
   unsigned short cadj[C][3];              // corner across the polytope edge (cp[t], cp[t+1])
-  int key[C][3];                          // scratch from here on: flag triple of a corner (output order); rim points during a clip
+  int key[C + 8][3];                      // scratch from here on (sized for the query batch: static_assert in classify_unknown_3d): flag triple of a corner (output order); rim points during a clip
   unsigned short remap[C];                // index of a surviving corner after the clip
   unsigned short pa[P], pb[P];            // new corner whose rim edge starts / ends at a plane
   unsigned short be[P][4];                // rim edges of R_p: (a, b, inside neighbour, flags)

@@ -81,6 +81,7 @@ __device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& s
     if (x[2]) atomicAdd(&cnt->fan_simplices, (unsigned long long)x[2]);
     if (x[3]) atomicAdd(&cnt->step_probes, (unsigned long long)x[3]);
     if (x[4]) atomicAdd(&cnt->alg_evals, (unsigned long long)x[4]);
+    if (x[5]) atomicAdd(&cnt->f32_survivors, (unsigned long long)x[5]);
   }
 }
 

@@ -60,6 +60,10 @@ struct GridIndex {
   // grid's plain box distances stay lower bounds.
   const double* __restrict__ sitesW;
   const double* __restrict__ siteWid;
+  // fp32 filter (vd_options.fp32_filter; the paper's GPU runs are fp32): the sorted sites once more as 16-byte
+  // float4 records (x, y, z, id bits), and the largest coordinate magnitude of the grid box (for the error bound)
+  const float4* __restrict__ sites32;
+  double f32M;
 };
 
 // The optional features of a query (weighted sites, step-out, D_alg counting) behind three predicates: the kernels exist in
@@ -71,6 +75,21 @@ struct GridIndex {
 __device__ __forceinline__ bool has_weights(const GridIndex& g) { return VD_EXT && g.sitesW != nullptr; }
 __device__ __forceinline__ bool has_step_out(const GridIndex& g) { return VD_EXT && g.stepMode != 0; }
 __device__ __forceinline__ bool counts_alg(const GridIndex& g) { return VD_EXT && g.countAlg != 0; }
+__device__ __forceinline__ bool has_f32(const GridIndex& g) { return VD_EXT && g.sites32 != nullptr; }
+
+// fp32 filter: a candidate whose squared distance to q, evaluated in fp32 from the float-rounded operands, exceeds this
+// threshold cannot be closer than `best` in exact arithmetic, so its fp64 record is never loaded.  Error budget: q and the
+// site are rounded to float (2^-24 relative each, coordinates up to M), the difference is rounded once more:
+// |dx_f - dx| <= delta = 2.5e-7 M per coordinate; then |d2_f - d2| <= 2 sqrt(3) delta |d| + 3 delta^2 plus the rounding of
+// three products and two sums (< 4e-6 relative).  With |d| <= sqrt(best) for every candidate that matters:
+__device__ __forceinline__ float f32_threshold(double best, double M) {
+  if (!(best < 1e300)) return __int_as_float(0x7f800000);
+  const double delta = 2.5e-7 * M;
+  return __double2float_ru((best + 3.5 * sqrt(best) * delta + 3.0 * delta * delta) * (1.0 + 4e-6));
+}
+__device__ __forceinline__ double f32_magnitude(const GridIndex& g, double qx, double qy, double qz) {
+  return fmax(fmax(g.f32M, fabs(qx)), fmax(fabs(qy), fabs(qz)));
+}
 __device__ __forceinline__ double site_w(const GridIndex& g, int id) { return has_weights(g) ? __ldg(&g.siteWid[id]) : 0.0; }
 
 constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
@@ -102,7 +121,7 @@ struct Piece {
 struct Counters {
   unsigned long long pairs, pieces, queries, dist_evals, search_iters, clips, overflow_pairs, rows;
   unsigned long long search_evals, pre_clips;   // distance evaluations inside bisector searches; clips by nearest-site bisectors (U19)
-  unsigned long long clip_corners, new_corners, fan_simplices, alg_evals, step_probes;
+  unsigned long long clip_corners, new_corners, fan_simplices, alg_evals, step_probes, f32_survivors;
 };
 
 // which kernel a counter block belongs to (vd_get_phase_counters): the step kernels of the phased schedule, the rest

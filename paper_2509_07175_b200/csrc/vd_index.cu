@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(kBlock) k_bbox_partial(const double* __restric
 // average over all cells of the sites' box -- reading U9), header written to device memory.
 __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64_t n, double density, int64_t gridCap,
                               const int* cellStart, const double4* sorted, int countAlg, const double* delta, int stepMode,
-                              const double* sitesW, const double* siteWid, GridIndex* g, unsigned int* err) {
+                              const double* sitesW, const double* siteWid, const float4* sites32, GridIndex* g, unsigned int* err) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
   for (int k = 0; k < nparts; ++k)
@@ -96,6 +96,9 @@ __global__ void k_grid_params(const double* __restrict__ part, int nparts, int64
   out.stepMode = stepMode;
   out.sitesW = sitesW;
   out.siteWid = siteWid;
+  out.sites32 = sites32;
+  out.f32M = 0.0;
+  for (int a = 0; a < 3; ++a) out.f32M = fmax(out.f32M, fmax(fabs(lo[a]), fabs(hi[a])));
   *g = out;
 }
 
@@ -244,10 +247,12 @@ __global__ void __launch_bounds__(kSortWarps * kLanes) k_radix_scatter(const uns
 }
 
 __global__ void __launch_bounds__(kBlock) k_gather_sorted(const double* __restrict__ sites, const int* __restrict__ order, int64_t n,
-                                                           double4* __restrict__ sorted) {
+                                                           double4* __restrict__ sorted, float4* __restrict__ sorted32) {
   for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
     const int i = order[p];
-    sorted[p] = make_double4(sites[(int64_t)i * 3 + 0], sites[(int64_t)i * 3 + 1], sites[(int64_t)i * 3 + 2], __longlong_as_double((long long)i));
+    const double x = sites[(int64_t)i * 3 + 0], y = sites[(int64_t)i * 3 + 1], z = sites[(int64_t)i * 3 + 2];
+    sorted[p] = make_double4(x, y, z, __longlong_as_double((long long)i));
+    if (sorted32) sorted32[p] = make_float4((float)x, (float)y, (float)z, __int_as_float(i));   // fp32 filter records
   }
 }
 
@@ -373,13 +378,16 @@ vd_status stage_index(vd_ctx* c) {
   if (stepMode && (s = ensure(c, c->delta, sizeof(double) * n))) return s;
   const bool lifted4 = c->weighted && c->dim == 3;   // power diagram of 3-D sites: additive terms travel with the sorted records
   if (lifted4 && (s = ensure(c, c->sortedW, sizeof(double) * n))) return s;
+  const bool f32 = c->opt.fp32_filter > 0 && !lifted4;
+  if (f32 && (s = ensure(c, c->sorted32, sizeof(float4) * n))) return s;
   cudaStream_t st = c->stream;
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
                                          c->sorted2.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
                                          stepMode ? c->delta.as<double>() : nullptr, stepMode,
-                                         lifted4 ? c->sortedW.as<double>() : nullptr, lifted4 ? c->siteW.as<double>() : nullptr, c->grid.as<GridIndex>(),
+                                         lifted4 ? c->sortedW.as<double>() : nullptr, lifted4 ? c->siteW.as<double>() : nullptr,
+                                         f32 ? c->sorted32.as<float4>() : nullptr, c->grid.as<GridIndex>(),
                                          &c->control.as<Control>()->err);
   cudaMemsetAsync(c->cellFill.p, 0, sizeof(int) * (gridCap + 2), st);
   VD_LAUNCH(k_cell_count, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), n, c->grid.as<GridIndex>(), c->cellOf.as<int>(),
@@ -428,7 +436,7 @@ vd_status stage_index(vd_ctx* c) {
     unsigned* tk = keyA; keyA = keyB; keyB = tk;
     int* tv = valA; valA = valB; valB = tv;
   }
-  VD_LAUNCH(k_gather_sorted, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), valA, n, c->sorted2.as<double4>());
+  VD_LAUNCH(k_gather_sorted, grid_for(n, kBlock), kBlock, 0, st)(c->sites.as<double>(), valA, n, c->sorted2.as<double4>(), f32 ? c->sorted32.as<float4>() : nullptr);
   // subStart holds the scan of the sub-cell counts for now; it is rebased to absolute positions in place
   VD_LAUNCH(k_sub_finalize, grid_for(gridCap, kWarpsPerBlock), kBlock, 0, st)(gp, c->subOff.as<int>(), c->subStart.as<int>(),
                                                                                c->subStart.as<int>());

@@ -14,7 +14,7 @@ struct QueryStats {
 // Work counters that are bumped rarely (per clip, per piece, per measurement-mode query) live in shared memory, one row
 // per warp, instead of in registers of kernels that run at their register cap: [0] corners side-tested by clips,
 // [1] corners created by clips, [2] fan simplices of finished pieces, [3] step-out probes, [4] D_alg.
-constexpr int kExtraCnt = 5;
+constexpr int kExtraCnt = 6;   // [5] candidates that passed the fp32 filter (evaluated in fp64)
 static __shared__ unsigned sExtraCnt[kWarpsPerBlock][kExtraCnt + 3];
 
 __device__ __forceinline__ void extra_cnt_reset() {
@@ -60,6 +60,11 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
   const int ny = y1 - y0 + 1;
   const int nrows = ny * (z1 - z0 + 1);
   st.rows += (unsigned)nrows;
+  // fp32 filter: the query in float, and the fp32 threshold of the current bound (recomputed when the bound moves)
+  const bool f32 = has_f32(g) && !has_weights(g);
+  float qxf = 0.f, qyf = 0.f, qzf = 0.f, thr = 0.f;
+  double fM = 0.0;
+  if (f32) { qxf = (float)qx; qyf = (float)qy; qzf = (float)qz; fM = f32_magnitude(g, qx, qy, qz); thr = f32_threshold(best, fM); }
   for (int r0 = 0; r0 < nrows; r0 += kLanes) {
     const int r = r0 + lane;
     int s = 0, cnt = 0;
@@ -104,9 +109,19 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
       const int t = t0 + lane;
       double d2 = best;
       int id = 0x7fffffff;
-      const bool valid = t < total;
+      bool valid = t < total;
+      int owner = 0;
+      if (valid) owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
+      if (f32) {
+        if (valid) {
+          const float4 pf = g.sites32[base[owner] + t];
+          const float fx = qxf - pf.x, fy = qyf - pf.y, fz = qzf - pf.z;
+          valid = fx * fx + fy * fy + fz * fz <= thr;   // else: farther than the bound, whatever fp64 would say
+        }
+        const unsigned pass = __ballot_sync(kFull, valid);
+        extra_cnt_add(5, (unsigned)__popc(pass));
+      }
       if (valid) {
-        const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
         const double4 p = g.sites[base[owner] + t];
         const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
@@ -119,6 +134,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         warp_argmin(d2, id);
         best = d2;
         bestId = id;
+        if (f32) thr = f32_threshold(best, fM);
       }
       __syncwarp();
     }
@@ -175,7 +191,7 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
   v.cellStart = g.subStart + (so & 0x3ffffff);
   v.sites = g.sites;
   v.heavyPrefix = nullptr; v.subOff = nullptr; v.subStart = nullptr; v.countAlg = 0; v.delta = nullptr; v.stepMode = 0;
-  v.sitesW = g.sitesW; v.siteWid = g.siteWid;
+  v.sitesW = g.sitesW; v.siteWid = g.siteWid; v.sites32 = g.sites32; v.f32M = g.f32M;
 }
 
 // One cell of the top grid: a plain cell is scanned directly, a refined cell through its sub-grid,

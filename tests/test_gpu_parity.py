@@ -147,6 +147,28 @@ def test_step_out_of_section_vi_a(idx):
         assert c["step_probes"] > 0 and c0["step_probes"] == 0
 
 
+@pytest.mark.parametrize("idx,opts", [(1, {}), (2, {}), (2, dict(small_wave=-1)), (3, {}), (3, dict(small_wave=-1)), (4, {}), (5, dict(small_wave=-1))])
+def test_fp32_filter_mode_gives_the_same_cells(idx, opts):
+    """vd_options.fp32_filter (the paper's GPU runs are fp32): candidates are first tested in fp32 against a rigorous
+    bound, only the survivors in fp64 -- the cells must be the oracle's, and the nearest sites brute force's, as without it;
+    the counter says how few candidates reach fp64."""
+    w = inputs.config(idx, "small")
+    g, cnt, _ = _gpu(w, fp32_filter=1, **opts)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+    assert 0 < cnt["f32_survivors"] < 0.5 * cnt["dist_evals"]
+    _, c0, _ = _gpu(w, **opts)
+    assert c0["f32_survivors"] == 0
+    rng = np.random.default_rng(300 + idx)
+    dim = w.sites.shape[1]
+    q = np.concatenate([rng.random((1500, dim)), rng.random((300, dim)) * 4.0 - 1.5, w.sites[rng.integers(0, w.n, 200)] + 1e-9])
+    with binding.Context(w.sites) as ctx:
+        ctx.set_options(fp32_filter=1)
+        got = ctx.nearest(q)
+    ref = np.array([np.argmin(((w.sites - x) ** 2).sum(1)) for x in q]) if w.n > 5000 else ((q[:, None, :] - w.sites[None, :, :]) ** 2).sum(-1).argmin(1)
+    assert np.array_equal(got, ref)
+
+
 def test_nearest_site_kernel_against_brute_force():
     for idx in (2, 3, 5):
         w = inputs.config(idx, "small")
