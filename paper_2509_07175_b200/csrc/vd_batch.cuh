@@ -156,8 +156,13 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
 // its sub-grid, a plain one as a 1 x 1 x 1 grid, each as a view that the same batched pass runs on, for the queries
 // whose ball meets that cell.  Only a query whose ball spans many rows (a corner in the void between clusters) takes the
 // single-query path.
-template <bool HV>
-static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
+//
+// FALLBACK = false: the queries that would take the single-query path are NOT answered; their mask is returned (bit u = query
+// u) and the routine carries no call of nearest(): the refined-index step kernels exist in a fast form without that code --
+// the expanding-shell search is a third of their instructions and half of their executed code, and they are bound by
+// instruction fetch -- and a second pass of the same kernels (with the fallback) takes what the fast pass left.
+template <bool HV, bool FALLBACK = true>
+static __device__ __noinline__ unsigned batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
   const int lane = lane_id();
   if (lane < kQB) B.flag[lane] = 0;
   __syncwarp();
@@ -229,6 +234,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
 #ifdef VD_COUNT_LOOSE
   extra_cnt_add(3, (unsigned)__popc(looseMask));   // (experiment: reported as step_probes)
 #endif
+  if constexpr (!FALLBACK) return looseMask;
   while (looseMask) {
     const int u = __ffs(looseMask) - 1;
     looseMask &= looseMask - 1;
@@ -239,6 +245,7 @@ static __device__ __noinline__ void batch_nearest(const GridIndex& gTop, QBatch&
     if (lane == 0) { B.best[u] = best; B.bestId[u] = bestId; }
     __syncwarp();
   }
+  return 0u;
 }
 
 }  // namespace vd

@@ -345,8 +345,8 @@ __global__ void k_wave_begin(ClipArgs A, PhaseCtl* pc, int allowPhased, int smal
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   Control* ctl = A.ctl;
   pc->mode = WAVE_NONE; pc->count = 0; pc->nDone = 0;
-  for (int k = 0; k < kMaxRounds + 2; ++k) pc->nClip[k] = 0;
-  for (int k = 0; k < 2 * kMaxRounds + 4; ++k) pc->ticket[k] = 0;
+  for (int k = 0; k < kMaxRounds + 2; ++k) { pc->nClip[k] = 0; pc->nLoose[k] = 0; pc->nLooseFix[k] = 0; }
+  for (int k = 0; k < 4 * kMaxRounds + 4; ++k) pc->ticket[k] = 0;
   if (ctl->err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP | ERR_DUPLICATE | ERR_INPUT)) return;   // the host reruns / reports
   const unsigned long long begin = ctl->waveEnd;
   unsigned long long tail = ctl->pairTail;

@@ -734,8 +734,10 @@ __device__ __forceinline__ int select_out_3d(const Poly3<P, C>& S, const ClipArg
 // Point-in-cell tests of the unclassified corners (section IV-A), up to kQB at a time in one batched
 // pass (vd_batch.cuh); the batch state lives in the scratch area S.key.  Returns whether there were any.
 // PolyT: Poly3<P, C>, or PolyTest3<P, C> (the members the tests touch, nothing else: k_ph_verify)
-template <class PolyT, bool HV>
-__device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st) {
+// DEFER (refined index, fast pass): corners whose test needs the single-query path are marked ST_LOOSE and left alone;
+// *deferred tells whether there were any.  Without DEFER such marks count as unclassified.
+template <class PolyT, bool HV, bool DEFER = false>
+__device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st, bool* deferred = nullptr) {
   const int lane = lane_id();
   VD_POLY_REFS;
   static_assert(sizeof(QBatch) + 40 <= sizeof(S.key), "the batch state (and a plane behind it) must fit the scratch area");
@@ -745,7 +747,7 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
     int nq = 0;
     for (int c0 = 0; c0 < nc && nq < kQB; c0 += kLanes) {
       const int c = c0 + lane;
-      const bool unk = c < nc && S.cstate[c] == ST_UNKNOWN;
+      const bool unk = c < nc && (S.cstate[c] == ST_UNKNOWN || (!DEFER && S.cstate[c] == ST_LOOSE));
       const unsigned m = __ballot_sync(kFull, unk);
       const int slot = nq + __popc(m & ((1u << lane) - 1u));
       if (unk && slot < kQB) {
@@ -761,8 +763,12 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
     if (nq == 0) break;
     any = true;
     __syncwarp();
-    batch_nearest<HV>(g, Q, nq, st);
-    if (lane < nq) {
+    const unsigned unanswered = batch_nearest<HV, !DEFER>(g, Q, nq, st);
+    if (DEFER && unanswered) {
+      if (lane < nq && ((unanswered >> lane) & 1u)) S.cstate[Q.item[lane]] = ST_LOOSE;
+      *deferred = true;
+    }
+    if (lane < nq && !((unanswered >> lane) & 1u)) {
       const int c = Q.item[lane], id = Q.bestId[lane];
       // q in Omega_i iff no site is nearer than v_i (Eq. 1: the cell is closed).  A tie up to rounding (1e-13
       // relative in the squared distance) counts as inside; a near tie (1e-9) does when the other site already
@@ -786,7 +792,8 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
 
 // One clipping from the known-outside corner p (Alg. 3 lines 3-4): bisector search on the real edge p_s p or on the
 // virtual edge w p, then the clip.  Returns 0 ok, 1 capacity, 2 topology, 3 search cap.
-template <int P, int C, bool HV>
+// Returns 0 ok, 1 capacity, 2 topology, 3 search cap, 4 (DEFER only) the search needs the single-query path: nothing changed.
+template <int P, int C, bool HV, bool DEFER = false>
 __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int i, int p, int s, int& np,
                                             int& nc, QueryStats& st, LocalCnt& lc) {
   const int lane = lane_id();
@@ -798,8 +805,9 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
   double psx = wx, psy = wy, psz = wz;
   if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
   double nx, ny, nz, d;
-  const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
-                                  nx, ny, nz, d, st, lc, reinterpret_cast<double*>(&S.key[0][0]));
+  const int j = find_bisector<HV, DEFER>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.pflag, np,
+                                         nx, ny, nz, d, st, lc, reinterpret_cast<double*>(&S.key[0][0]));
+  if (DEFER && j == -2) return 4;
   if (j < 0) return 3;
   bool own = false;
   for (int f = lane; f < np; f += kLanes) own |= (S.pflag[f] == j);

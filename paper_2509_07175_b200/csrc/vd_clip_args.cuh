@@ -41,7 +41,8 @@ struct ClipArgs {
   int* siteNbrRaw;
 };
 
-enum { ST_UNKNOWN = 0, ST_IN = 1, ST_OUT = 2 };
+enum { ST_UNKNOWN = 0, ST_IN = 1, ST_OUT = 2,
+       ST_LOOSE = 3 };   // unclassified, and its point-in-cell test needs the single-query path (left for the second pass)
 
 // State of one WAVE PROGRAM (vd_clip.cu): the fixed sequence of launches that processes one wavefront of pairs with no
 // host in between.  Its first kernel (k_wave_begin) looks at the pair list and decides what the wave is; every other
@@ -56,7 +57,9 @@ struct PhaseCtl {
   unsigned long long begin;         // first pair of the wave in the pair list
   unsigned nDone, pad;
   unsigned nClip[kMaxRounds + 2];   // pairs with a corner outside after the tests of round r
-  unsigned ticket[2 * kMaxRounds + 4];   // one work cursor per launch of the program
+  unsigned nLoose[kMaxRounds + 2];  // refined index: pairs whose tests / searches of round r need the single-query path
+  unsigned nLooseFix[kMaxRounds + 2];
+  unsigned ticket[4 * kMaxRounds + 4];   // one work cursor per launch of the program
 };
 
 struct LocalCnt {
@@ -384,7 +387,8 @@ static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, c
 // the segment lies in P, and P is inside H_ik for every site k that owns one of them, so N_q = v_k can
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
-template <bool HV>
+template <bool HV, bool DEFER = false>
+// DEFER (refined index, fast pass): a query that needs the single-query path ends the search with -2, nothing changed.
 // The arguments are scalars and pointers on purpose: a struct passed by reference to this (not inlined) function
 // would be copied into every thread's local memory, and so would by-reference results -- the plane comes back
 // through out4 (the caller's shared-memory scratch, or a local array), the iteration count as the return's pair.
@@ -443,7 +447,8 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
       // general single-query search
       if (lane_id() == 0) { qb->qx[0] = ax; qb->qy[0] = ay; qb->qz[0] = az; qb->best[0] = best; qb->bestId[0] = bestId; }
       __syncwarp();
-      batch_nearest<HV>(g, *qb, 1, st);
+      const unsigned unanswered = batch_nearest<HV, !DEFER>(g, *qb, 1, st);
+      if (DEFER && unanswered) return -2;
       __syncwarp();
       best = qb->best[0]; bestId = qb->bestId[0];
       __syncwarp();
@@ -472,7 +477,7 @@ found:
 }
 
 // scratch4: four doubles of the warp's shared-memory scratch (3D kinds); nullptr: a local array
-template <bool HV>
+template <bool HV, bool DEFER = false>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
                                              double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch4 = nullptr) {
@@ -483,7 +488,7 @@ __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex&
     // the scratch area holds the batch state of the point-in-cell tests; the plane comes back through its last 32 bytes
     QBatch* qb = reinterpret_cast<QBatch*>(scratch4);
     double* out4 = scratch4 + (sizeof(QBatch) + 7) / 8;
-    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out4, qb, st, iters);
+    r = find_bisector_impl<HV, DEFER>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out4, qb, st, iters);
     scratch4 = out4;
     nx = scratch4[0]; ny = scratch4[1]; nz = scratch4[2]; d = scratch4[3];
   } else {

@@ -89,13 +89,13 @@ struct vd_ctx {
   vd::DevBuf cellOf;      // int [n]
   vd::DevBuf cellStart;   // int [gridCap+1]
   vd::DevBuf cellFill;    // int [gridCap+1]
-  vd::DevBuf sorted;      // (unused since the radix sort of round 2)
   vd::DevBuf sorted32;    // float4 [n]  the sorted sites in fp32 (vd_options.fp32_filter)
   vd::DevBuf sortKeys, sortVals, sortHist;   // S1 radix sort: keys / site ids (two halves each), per-(digit, segment) counts
   vd::DevBuf sortedW;     // double [n]  additive terms of weighted 3-D sites in index order
   vd::DevBuf delta;       // double [n]  S1b: half the distance to the nearest other site (vd_options.step_out)
   vd::DevBuf scanTmp;     // scan scratch
-  vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart, subKey, sorted2;   // second level
+  vd::DevBuf heavyFlag, heavyPrefix, subNeed, subOffRaw, subOff, subCount, subStart;   // second level
+  vd::DevBuf sorted2;     // double4 [n]  the sites in index order (x, y, z, id bits)
   int64_t subCap = 0;
   // dissolve mode (Alg. 5 lines 2-6, vd_options.dissolve): prepared once per domain (vd_domain.cu)
   bool dissolveReady = false;

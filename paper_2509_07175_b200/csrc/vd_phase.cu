@@ -148,15 +148,20 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 // Round r of a phased wave (lists[r & 1] receives the pairs that still have a corner outside).  Round 0 tests every pair of
 // the wave; round r > 0 the pairs that round r-1's k_ph_fix clipped -- it runs only if that kernel ran.  A negative list
 // entry is a pair that left the path.
-template <bool HV>
+// MODE 0: the whole step.  Refined index: MODE 1 = the fast pass (batched tests only; a pair with a corner whose test needs the
+// single-query path goes to the loose list, those corners marked ST_LOOSE), MODE 2 = the second pass over the loose list with
+// the complete test code.  Both passes feed the same clip / done lists.
+template <bool HV, int MODE>
 __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
                                                      int* __restrict__ doneList, PhaseCtl* pc, int r, int tailPairs) {
   if (pc->mode != WAVE_PHASED) return;
   if (r > 0 && (int)pc->nClip[r - 1] <= tailPairs) return;
-  const int* list = r > 0 ? lists + ((r - 1) & 1) * (int64_t)cap : nullptr;
-  const int count = r > 0 ? (int)pc->nClip[r - 1] : (int)pc->count;
+  int* looseList = lists + 3 * (int64_t)cap;
+  const int* list = MODE == 2 ? looseList : (r > 0 ? lists + ((r - 1) & 1) * (int64_t)cap : nullptr);
+  const int count = MODE == 2 ? (int)pc->nLoose[r] : (r > 0 ? (int)pc->nClip[r - 1] : (int)pc->count);
+  if (count == 0) return;
   int* clipList = lists + (r & 1) * (int64_t)cap;
-  const int slot = 4 + 2 * r;
+  const int slot = 4 + 4 * r + (MODE == 2 ? 1 : 0);
   __shared__ GridIndex g;
   __shared__ PolyT S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -174,12 +179,14 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) 
     CellState* c = &cells[item];
     const int np = c->np, nc = c->nc;
     if (np < 0) continue;
-    bool out = false;
+    bool out = false, loose = false;
     if (!c->failed && nc > 0) {
       unpark(&S[w], &c->S, kTestBytes, bar, parity);
-      const bool any = classify_unknown_3d<PolyT, HV>(S[w], g, c->i, np, nc, st);
+      bool deferred = false;
+      const bool any = classify_unknown_3d<PolyT, HV, MODE == 1>(S[w], g, c->i, np, nc, st, &deferred);
       for (int k = lane; k < nc; k += kLanes) out |= (S[w].cstate[k] == ST_OUT);
       out = __any_sync(kFull, out);
+      if (MODE == 1 && deferred) loose = true;
       if (any) {
 #ifdef VD_NO_TMA
         copy_words(c->S.cnn, S[w].cnn, (nc * 4 + 15) & ~15);
@@ -197,7 +204,8 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) 
       }
     }
     if (lane == 0) {
-      if (out) clipList[atomicAdd(&pc->nClip[r], 1u)] = item;
+      if (MODE == 1 && loose) looseList[atomicAdd(&pc->nLoose[r], 1u)] = item;
+      else if (out) clipList[atomicAdd(&pc->nClip[r], 1u)] = item;
       else doneList[atomicAdd(&pc->nDone, 1u)] = item;
     }
     __syncwarp();
@@ -208,14 +216,18 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) 
 // every corner known to be outside is clipped away (its search, its clip); the new corners wait for the next
 // round of tests.  The list is rewritten in place: the slot, or -1 when the pair left the path.
 // Runs when round r's tests left more than tailPairs pairs with a corner outside (fewer: k_ph_tail finishes them).
-template <bool HV>
+// MODE as in k_ph_verify: the fast pass (1) stops at a search that needs the single-query path -- the pair is parked as it is
+// and its position in the clip list goes to the loose list --, the second pass (2) takes those pairs to the end of the step.
+template <bool HV, int MODE>
 __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k_ph_fix(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
                                                      PhaseCtl* pc, int r, int tailPairs) {
   if (pc->mode != WAVE_PHASED || (int)pc->nClip[r] <= tailPairs) return;
   int* list = lists + (r & 1) * (int64_t)cap;
-  const int count = (int)pc->nClip[r];
+  int* looseList = lists + 3 * (int64_t)cap;
+  const int count = MODE == 2 ? (int)pc->nLooseFix[r] : (int)pc->nClip[r];
+  if (count == 0) return;
   const int64_t begin = (int64_t)pc->begin;
-  const int tslot = 5 + 2 * r;
+  const int tslot = 6 + 4 * r + (MODE == 2 ? 1 : 0);
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -226,8 +238,9 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k
   extra_cnt_reset();
   VD_WARP_BAR;
   for (;;) {
-    const int t = next_item(pc, tslot, count);
+    int t = next_item(pc, tslot, count);
     if (t < 0) break;
+    if (MODE == 2) t = looseList[t];   // the pair's position in the clip list
     const int slot = list[t];
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
@@ -238,7 +251,11 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k
       int s;
       const int p = select_out_3d(S[w], A, nc, s);
       if (p < 0) break;
-      const int rc = clip_from_3d<P3, C3, HV>(S[w], g, A, i, p, s, np, nc, st, lc);
+      const int rc = clip_from_3d<P3, C3, HV, MODE == 1>(S[w], g, A, i, p, s, np, nc, st, lc);
+      if (MODE == 1 && rc == 4) {   // this search is for the second pass; what was clipped so far stays
+        if (lane == 0) looseList[atomicAdd(&pc->nLooseFix[r], 1u)] = t;
+        break;
+      }
       if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
       if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
     }
@@ -270,7 +287,7 @@ __global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs 
   if (count == 0) return;
   const int* list = lists + (r & 1) * (int64_t)cap;
   const int64_t begin = (int64_t)pc->begin;
-  const int tslot = 3;
+  const int tslot = 3;   // (cursors 4 ..: four per round -- tests, their second pass, clips, their second pass)
   __shared__ GridIndex g;
   __shared__ PolyF S[kWarpsPerBlock];
   if (threadIdx.x == 0) g = *A.grid;
@@ -342,7 +359,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
 vd_status phase_buffers(vd_ctx* c, int64_t cap) {
   vd_status s;
   if ((s = ensure(c, c->phaseCells, sizeof(CellState) * (size_t)cap))) return s;
-  return ensure(c, c->phaseLists, sizeof(PhaseCtl) + sizeof(int) * 3 * (size_t)cap);   // the control block first (8-byte members)
+  return ensure(c, c->phaseLists, sizeof(PhaseCtl) + sizeof(int) * 4 * (size_t)cap);   // to verify / to clip, done, loose   // the control block first (8-byte members)
 }
 
 void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int rounds, int tailPairs) {
@@ -357,12 +374,21 @@ void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int roun
   if (c->kind == KIND_BOX_3D) VD_LAUNCH(k_ph_init<true>, grid, kBlock, 0, st)(A, cells, pc);
   else VD_LAUNCH(k_ph_init<false>, grid, kBlock, 0, st)(A, cells, pc);
   for (int r = 0; r < rounds; ++r) {
+    // refined index: a fast pass without the single-query search code, then a second pass for what it left (MODE)
     phase_mark(c, 1);
-    if (hv) VD_LAUNCH(k_ph_verify<true>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
-    else VD_LAUNCH(k_ph_verify<false>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    if (hv) {
+      VD_LAUNCH((k_ph_verify<true, 1>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+      VD_LAUNCH((k_ph_verify<true, 2>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    } else {
+      VD_LAUNCH((k_ph_verify<false, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    }
     phase_mark(c, 2);
-    if (hv) VD_LAUNCH(k_ph_fix<true>, grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
-    else VD_LAUNCH(k_ph_fix<false>, grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+    if (hv) {
+      VD_LAUNCH((k_ph_fix<true, 1>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+      VD_LAUNCH((k_ph_fix<true, 2>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+    } else {
+      VD_LAUNCH((k_ph_fix<false, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+    }
   }
   phase_mark(c, 4);
   if (hv) VD_LAUNCH(k_ph_tail<true>, grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, rounds, tailPairs);
