@@ -92,6 +92,7 @@ vd_status ensure(vd_ctx* c, DevBuf& b, size_t bytes) {
   // a buffer that grows again gets a quarter of slack: the assemble stage sizes its buffers from pool cursors that differ
   // by a few entries from run to run, and re-allocating a gigabyte for them costs hundreds of milliseconds
   if (b.p) bytes += bytes / 4;
+  else if (bytes > ((size_t)1 << 20)) bytes += bytes / 8;   // (large buffers: also the first time)
   // pending kernels may still use the old block
   if (b.p) sync_stream(c, "buffer grows");
   release(c, b);
