@@ -91,13 +91,15 @@ typedef struct vd_options {
   int32_t real_edges;     /* 1 (default): search on a real edge p_s p_t when the outside corner has
                              a known-inside neighbour (Alg. 1); 0: always the virtual
                              edge from the pair's witness point (Alg. 3)               */
-  int32_t persistent;     /* how S4 is scheduled (P:L257's wavefronts):
+  int32_t persistent;     /* how S4 is scheduled (P:L257's wavefronts).  In every mode the wavefront loop runs on the
+                             device ("wave programs": a fixed sequence of launches per wavefront, each kernel reading
+                             from device memory whether it has work; the host looks once per batch of programs):
                              1 (default): 3D kinds "phased" -- every step of Alg. 3 is its own small kernel
                                 over a whole wave, polytopes parked in HBM between steps (the one-kernel form is
                                 bound by instruction fetch); 2D / surface kinds: one launch per wavefront;
                              2: phased (3D kinds), device-side queue (2D / surface kinds);
-                             3: device-side work queue, one persistent kernel;
-                             0: one launch of the one-kernel form per wave                               */
+                             3: device-side work queue: one launch of the one-kernel form drains everything;
+                             0: one launch of the one-kernel form per wavefront                          */
   int64_t pair_capacity;  /* initial capacity of the (simplex, site) pair list; grows on demand     */
   int64_t vert_capacity;  /* initial capacity of the corner pool; grows on demand                   */
   int32_t near_clips;     /* every piece of cell i is first clipped by the bisectors of this many of the
@@ -111,16 +113,16 @@ typedef struct vd_options {
                              measure x centroid by one sum.  0, 0 (default) = all of M.  Meshed kinds only.            */
   int32_t tail_pairs;     /* phased schedule: a round that leaves at most this many pairs with a corner outside hands
                              them to one kernel that tests and clips them to completion (no further rounds for the
-                             wave); 0 = default (65536); < 0: never                                                */
+                             wave); 0 = default (65536); < 0: only what the program's five rounds leave             */
   int32_t first_clip;     /* 0 / 1 (default): a pair (T_a, v_i) discovered through the face of P_{a,u} on B_ui is first
                              clipped by that bisector, without a search -- the first clip of G_{a,j};
                              < 0: every clip is found by a search (Alg. 3 as printed).  3D kinds.                   */
   int32_t seed_corners;   /* corners of every simplex whose nearest site seeds a pair (Alg. 2 line 4): 0 = default
                              (1: the first corner, as in Alg. 2); >= 3 / 4: all of them.  The result does not depend
                              on it; discovered pairs are cheaper than seeds (first_clip).  Meshed kinds.             */
-  int32_t small_wave;     /* phased schedule: a wavefront of fewer pairs than this runs as ONE launch of the one-kernel
-                             form (the last wavefronts of a step hold a few hundred pairs: a dozen launches and three
-                             counter reads each otherwise); 0 = default (8192); < 0: never                          */
+  int32_t small_wave;     /* phased schedule: a wavefront of fewer pairs than this is drained -- with every pair it sets
+                             off -- by ONE launch of the one-kernel form as a device-side queue (the last wavefronts of a
+                             step hold a few hundred pairs); 0 = default (8192); < 0: never (every wavefront phased)  */
   int32_t step_out;       /* improved bisector search of section VI-A: before the search on a segment p_s p_t
                              longer than 2 delta_i (delta_i = half the distance from v_i to its nearest other site, computed
                              for every site by S1b), step out from p_s: g = p_s + lambda delta_i dir, while N_g = v_i, then

@@ -576,3 +576,22 @@ def test_dissolve_mode_follows_moving_sites():
     assert np.abs(a - b).max() <= 1e-11
     o = oracle.compute(b, w.verts, w.simplices, w.kind, dissolve=True, tier="B")
     parity.assert_parity(g, o, w.diameter)
+
+
+def test_counters_per_step_kernel_add_up():
+    """vd_get_phase_counters: the work counters split by the kernel that did the work (bench.py derives each step kernel's
+    algorithmic flop from them) add up to vd_get_counters; tests are counted under verify / tail, searches and clips under
+    init (no search) / fix / tail, fan simplices under finish."""
+    w = inputs.config(2, "small")
+    with binding.Context(w.sites) as ctx:
+        ctx.set_options(small_wave=-1)
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        ctx.compute()
+        tot, ph = ctx.counters(), ctx.phase_counters()
+    for f in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips", "clip_corners", "new_corners", "fan_simplices"):
+        assert sum(ph[k][f] for k in ph) == tot[f], f
+    assert ph["verify"]["queries"] > 0 and ph["verify"]["clips"] == 0 and ph["verify"]["search_iters"] == 0
+    assert ph["fix"]["search_iters"] + ph["tail"]["search_iters"] == tot["search_iters"] > 0
+    assert ph["init"]["clips"] == tot["pre_clips"] > 0 and ph["init"]["queries"] == 0
+    assert ph["finish"]["fan_simplices"] == tot["fan_simplices"] > 0 and ph["finish"]["pieces"] == tot["pieces"]
+    assert tot["clip_corners"] > tot["clips"] * 4 and tot["new_corners"] >= tot["clips"] * 3
