@@ -12,7 +12,8 @@ namespace vd {
 constexpr int kQB = 8;          // queries per batch
 // rows of a query's ball above which it takes the single-query path: 32, and 64 on the top grid of a refined index (measured:
 // 8 / 16 / 32 / 64 rows: C3 405 / 324 / 311 / 306 ms, C5 16.2 / 16.3 / 16.2 / 18.1 ms, C2 21.1 / 20.2 / 20.2 / 20.2 ms)
-constexpr int kQBMaxRows = 32, kQBMaxRowsRefined = 64;
+constexpr int kQBMaxRows = 32, kQBMaxRowsPlanar = 16, kQBMaxRowsRefined = 64;   // (planar grid, C1: 16 rows 1.05 ms, 32 rows 1.23 ms --
+// the batched pass has no early exit, and a bare triangle's corners have loose bounds in a dense grid)
 
 struct QBatch {
   double qx[kQB], qy[kQB], qz[kQB];
@@ -55,7 +56,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
       const int z0 = cell_of(g, 2, qz - r - 1e-6 * g.h[2]), z1 = cell_of(g, 2, qz + r + 1e-6 * g.h[2]);
       myRows = (y1 - y0 + 1) * (z1 - z0 + 1);
       B.x0[lane] = x0; B.x1[lane] = x1; B.y0[lane] = y0; B.ny[lane] = y1 - y0 + 1; B.z0[lane] = z0;
-      if (myRows > (SKIP_REFINED ? kQBMaxRowsRefined : kQBMaxRows)) { loose = true; myRows = 0; }
+      if (myRows > (SKIP_REFINED ? kQBMaxRowsRefined : (g.h[2] > 0 ? kQBMaxRows : kQBMaxRowsPlanar))) { loose = true; myRows = 0; }
     }
   }
   const int incl = warp_incl_scan(myRows);

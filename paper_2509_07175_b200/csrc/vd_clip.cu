@@ -11,6 +11,9 @@
 // This file (and vd_phase.cu) is compiled TWICE (build.py): as namespace vd::lean with VD_EXT = 0 -- the kernels without the code
 // of the optional query features (weighted 3-D sites, step-out, D_alg counting) -- and as vd::full with VD_EXT = 1.  The kernels
 // are bound by instruction fetch: the lean ones are 4-7 % faster on the BASELINE configs.  vd_compute picks per call.
+#ifndef VD_CLIP2D_BLOCKS
+#define VD_CLIP2D_BLOCKS 3   // resident blocks per SM of the one-kernel form on the triangle kinds
+#endif
 namespace vd {
 namespace VD_VARIANT {
 
@@ -139,7 +142,7 @@ constexpr int K2 = 32, K2B = 256;
 // (k_wave_begin): fast tier -- the wave [pc->begin, + pc->count) (WAVE_SINGLE), or the whole list from the wave's first pair
 // on as a device-side queue (WAVE_QUEUE); large tier (BIG) -- the deferred pairs ovf[ovfBegin .. ovfEnd).
 template <int KIND, bool BIG, bool HV>
-__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : 3) k_clip(ClipArgs A, const int* __restrict__ list, const PhaseCtl* __restrict__ pc) {
+__global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : ((KIND == KIND_TRI_2D || KIND == KIND_BOX_2D) ? VD_CLIP2D_BLOCKS : 3)) k_clip(ClipArgs A, const int* __restrict__ list, const PhaseCtl* __restrict__ pc) {
   constexpr int W = BIG ? 1 : kWarpsPerBlock;
   int64_t begin, end;
   bool persist = false;
@@ -392,7 +395,7 @@ template <int KIND>
 static void launch_kind(vd_ctx* c, const ClipArgs& A, bool hv, bool big, const PhaseCtl* pc) {
   cudaStream_t st = c->stream;
   if (!big) {
-    const int blocks = sm_count() * 3;
+    const int blocks = sm_count() * ((KIND == KIND_TRI_2D || KIND == KIND_BOX_2D) ? VD_CLIP2D_BLOCKS : 3);
     if (hv) VD_LAUNCH((k_clip<KIND, false, true>), blocks, kBlock, 0, st)(A, nullptr, pc);
     else VD_LAUNCH((k_clip<KIND, false, false>), blocks, kBlock, 0, st)(A, nullptr, pc);
   } else {

@@ -4,6 +4,9 @@
 #include "vd_nearest.cuh"
 #include "vd_batch.cuh"
 
+#ifndef VD_ONE_SHOT_HV
+#define VD_ONE_SHOT_HV 0
+#endif
 namespace vd {
 
 struct ClipArgs {
@@ -421,7 +424,7 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
     const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
     const double di2 = dix * dix + diy * diy + diz * diz + wi, dj2 = djx * djx + djy * djy + djz * djz + wj;
-    if (!HV && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
+    if ((!HV || VD_ONE_SHOT_HV) && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
       // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
       double tb = 2.0;
       int jb = 0x7fffffff;

@@ -24,6 +24,9 @@ namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
 #ifndef VD_PH_BLOCKS_HV
 #define VD_PH_BLOCKS_HV 4   // the same for the kernels that know the refined index (measured on C3: 2 blocks 451 ms, 3 blocks 416 ms, 4 blocks 405 ms)
 #endif
+#ifndef VD_TWO_PASS
+#define VD_TWO_PASS 1   // refined index: fast pass + second pass of the verify / fix kernels (0: one complete pass)
+#endif
 #ifndef VD_PH_TAIL_BLOCKS
 #define VD_PH_TAIL_BLOCKS 3
 #endif
@@ -376,16 +379,20 @@ void enqueue_phased(vd_ctx* c, const ClipArgs& A, bool hv, int64_t cap, int roun
   for (int r = 0; r < rounds; ++r) {
     // refined index: a fast pass without the single-query search code, then a second pass for what it left (MODE)
     phase_mark(c, 1);
-    if (hv) {
+    if (hv && VD_TWO_PASS) {
       VD_LAUNCH((k_ph_verify<true, 1>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
       VD_LAUNCH((k_ph_verify<true, 2>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
+    } else if (hv) {
+      VD_LAUNCH((k_ph_verify<true, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
     } else {
       VD_LAUNCH((k_ph_verify<false, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, done, pc, r, tailPairs);
     }
     phase_mark(c, 2);
-    if (hv) {
+    if (hv && VD_TWO_PASS) {
       VD_LAUNCH((k_ph_fix<true, 1>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
       VD_LAUNCH((k_ph_fix<true, 2>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
+    } else if (hv) {
+      VD_LAUNCH((k_ph_fix<true, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
     } else {
       VD_LAUNCH((k_ph_fix<false, 0>), grid, kBlock, 0, st)(A, cells, lists, icap, pc, r, tailPairs);
     }
