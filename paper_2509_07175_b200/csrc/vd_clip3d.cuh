@@ -637,16 +637,18 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
                wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
   const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
   const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (((VD_EXT && A.siteW) ? __ldg(&A.siteW[j]) : 0.0) - S.u[12]));
-  // the corner farthest beyond the plane starts R_p
-  double far = 0.0;
-  int p = 0x7fffffff;
+  // any corner clearly beyond the plane starts R_p: the corners of a convex polytope beyond a plane are connected over its
+  // edges, so the flood of apply_clip_3d reaches the same set from each of them (a ballot instead of a warp argmin of the
+  // farthest one)
+  int p = -1;
   const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
-  for (int c = lane; c < nc; c += kLanes) {
-    const double sd = nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d;
-    if (sd > tol && S.cstate[c] != ST_IN && closer(-sd, c, far, p)) { far = -sd; p = c; }
+  for (int c0 = 0; c0 < nc && p < 0; c0 += kLanes) {
+    const int c = c0 + lane;
+    const bool beyond = c < nc && (nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d > tol) && S.cstate[c] != ST_IN;
+    const unsigned m = __ballot_sync(kFull, beyond);
+    if (m) p = c0 + __ffs((int)m) - 1;
   }
-  warp_argmin(far, p);
-  if (p == 0x7fffffff) return -1;   // the plane does not cut P
+  if (p < 0) return -1;   // the plane does not cut P
   if (np >= P) {
     compact_planes_3d(S, np, nc);
     if (np >= P) return 1;
