@@ -595,3 +595,14 @@ def test_counters_per_step_kernel_add_up():
     assert ph["init"]["clips"] == tot["pre_clips"] > 0 and ph["init"]["queries"] == 0
     assert ph["finish"]["fan_simplices"] == tot["fan_simplices"] > 0 and ph["finish"]["pieces"] == tot["pieces"]
     assert tot["clip_corners"] > tot["clips"] * 4 and tot["new_corners"] >= tot["clips"] * 3
+
+
+@pytest.mark.parametrize("idx,opts", [(2, {}), (2, dict(small_wave=-1)), (2, dict(persistent=3)), (4, {}), (1, {}), (2, dict(dissolve=1))])
+def test_pools_that_start_too_small_grow_and_rerun(idx, opts):
+    """vd_options.pair_capacity / vert_capacity far below what the diagram needs: the wave programs stop at the sticky
+    capacity bit, vd_compute doubles the pools and reruns (counters.reruns), and the result is the oracle's."""
+    w = inputs.config(idx, "small")
+    g, cnt, _ = _gpu(w, pair_capacity=2000 if idx != 1 else 64, vert_capacity=20000 if idx != 1 else 256, **opts)   # about three doublings each
+    assert cnt["reruns"] >= 2
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, dissolve=bool(opts.get("dissolve")))
+    parity.assert_parity(g, o, w.diameter)
