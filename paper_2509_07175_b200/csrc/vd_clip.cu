@@ -1,6 +1,7 @@
 // vd_clip.cu -- S3 seeds, S4 clip kernels (one warp per (simplex, site) pair), S5 propagation through
 // the pair list.  Alg. 4 / Alg. 5 lines 15-27 as a wavefront over one growing
-// list: wave k processes the pairs pushed by wave k-1.
+// list: wave k processes the pairs pushed by wave k-1.  The wavefront loop itself runs on the device (wave programs,
+// below: k_wave_begin / k_wave_end around the kernels of a wave); the host enqueues programs in batches.
 #include <string.h>
 
 #include <type_traits>

@@ -1,7 +1,8 @@
 // vd_index.cu -- S1: the site index ("build a structure S of V", line 1 of Alg. 2/4/5, P:L180/L250/L301;
-// grid structure P:L377-383).  Bounding box -> cell key per site -> counting sort (histogram, exclusive
-// scan, scatter) -> sites gathered in cell order as 32-byte records.  Plus the S2 query as a kernel of
-// its own (vd_nearest, and the per-mesh-vertex nearest site used by S3).
+// grid structure P:L377-383).  Bounding box -> cell key per site -> histogram + exclusive scan (bucket starts) -> refined
+// cells planned -> ONE stable radix sort by (cell, sub-cell) key -> sites gathered in that order as 32-byte records ->
+// duplicate check.  Plus S1b (k_delta), the S2 query as a kernel of its own (vd_nearest, and the per-mesh-vertex nearest
+// site used by S3) and its no-allocation variant (vd_nearest_static).
 #include <math.h>
 
 #include "vd_internal.h"

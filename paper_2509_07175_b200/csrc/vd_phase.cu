@@ -1,4 +1,4 @@
-// vd_phase.cu -- S4 as a sequence of small kernels ("phased" mode, vd_options.persistent = 2) for the 3D kinds.
+// vd_phase.cu -- S4 as a sequence of small kernels ("phased" mode, the default of the 3D kinds: vd_options.persistent = 1 / 2).
 //
 // The one-kernel clip path (vd_clip.cu) is bound by instruction fetch: ~100 KB of code whose 24 warps per SM sit
 // in different steps of Alg. 3, against a 32 KB L1.5 instruction cache.  Here every step of Alg. 3 is its own
@@ -8,8 +8,13 @@
 //   k_ph_init    P <- T_a or the box (Alg. 3 line 1), then the clips by the nearest sites (reading U19)
 //   k_ph_verify  point-in-cell tests of all unclassified corners (section IV-A)          --+  rounds, until no
 //   k_ph_fix     per pair with a corner outside: bisector search + clip (Alg. 3 l. 3-4)  --+  corner is outside
+//   k_ph_tail    what the rounds leave: tests and clips to completion in one launch
 //   k_ph_finish  measure, moments, corners, flags, propagation
 //
+// The kernels of a wave are enqueued as one fixed sequence (enqueue_phased, part of a "wave program": vd_clip.cu); each reads
+// from PhaseCtl in device memory whether it has work and how much, so the host does not look between them.  Polytopes move
+// between HBM and shared memory through the TMA unit (vd_tma.cuh).  On the refined index k_ph_verify and k_ph_fix run as a
+// fast pass (without the single-query search code) and a second pass for the pairs it leaves (MODE).
 // Pairs pushed by k_ph_finish form the next wave (Alg. 4's L1/L2 swap).  Pairs that outgrow the fast tier
 // go to the large-capacity kernel of vd_clip.cu, as in the other modes.
 #include "vd_clip3d.cuh"
