@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(kBlock) k_dissolve_seeds(ClipArgs A, const dou
       bool inside = true;
       for (int k = 0; k < np && inside; ++k) {
         const double4 q = planes[k];
-        inside = q.x * x + q.y * y + q.z * z - q.w <= tol;
+        inside = q.x * x + q.y * y + q.z * z - q.w <= tol * fmax(1.0, fmax(fabs(q.w), fabs(x) + fabs(y) + fabs(z)));
       }
       if (inside) push_pair(A, A.m, (int)i, x, y, z);
     }

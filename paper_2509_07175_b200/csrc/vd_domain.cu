@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(kBlock) k_plane_unique(const double4* __restri
     bool uniq = true;
     for (int64_t o = 0; o < t && uniq; ++o) {
       const double4 q = raw[o];
-      if (p.x * q.x + p.y * q.y + p.z * q.z > 1.0 - 1e-12 && fabs(p.w - q.w) <= tol) uniq = false;
+      if (p.x * q.x + p.y * q.y + p.z * q.z > 1.0 - 1e-12 && fabs(p.w - q.w) <= tol * fmax(1.0, fabs(p.w))) uniq = false;   // (relative to the offset's size)
     }
     if (uniq) out[atomicAdd(cursor, 1ull)] = p;
   }
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(kBlock) k_convex_check(const double* __restric
     bool out = false;
     for (int k = 0; k < np; ++k) {
       const double4 p = planes[k];
-      out |= p.x * x + p.y * y + p.z * z - p.w > tol;
+      out |= p.x * x + p.y * y + p.z * z - p.w > tol * fmax(1.0, fmax(fabs(p.w), fabs(x) + fabs(y) + fabs(z)));   // (relative to the coordinates' size)
     }
     if (out) atomicOr(err, ERR_TOPOLOGY);
   }

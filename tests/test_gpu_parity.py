@@ -539,6 +539,20 @@ def test_dissolve_mode_parity(name, opts):
         assert not whole.any()                                      # every site lies outside the cube: no interior site (U13)
 
 
+@pytest.mark.parametrize("scale,shift", [(1e3, 5e3), (1e-3, -2e-3)])
+def test_dissolve_mode_on_scaled_and_shifted_domains(scale, shift):
+    """The convexity check, the plane deduplication and the inside test of dissolve mode are relative to the coordinates'
+    size: the same diagram scaled and shifted gives the same cells (scaled)."""
+    w0 = _dissolve_case("octahedron")
+    w = inputs.custom(inputs.KIND_TET_3D, w0.sites * scale + shift, w0.verts * scale + shift, w0.simplices, "octahedron_scaled")
+    g, cnt, _ = _gpu(w, dissolve=1)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, dissolve=True, tier="B")
+    parity.assert_parity(g, o, w.diameter)
+    g0, _, _ = _gpu(w0, dissolve=1)
+    assert np.array_equal(g.piece_simplex, g0.piece_simplex) and np.array_equal(g.vert_flags, g0.vert_flags)
+    assert np.allclose(g.measure, g0.measure * scale ** 3, rtol=1e-9, atol=0)
+
+
 def test_dissolve_mode_rejects_what_it_cannot_do():
     v, t = inputs.cube_kuhn_mesh(2)
     s = np.random.default_rng(3).random((300, 3))
