@@ -4,6 +4,9 @@
 #include "vd_nearest.cuh"
 #include "vd_batch.cuh"
 
+#ifndef VD_SEARCH_BATCH
+#define VD_SEARCH_BATCH 1   // refined index: a search's queries go through the batched multi-view pass (0: the single-query path)
+#endif
 #ifndef VD_ONE_SHOT_HV
 #define VD_ONE_SHOT_HV 0
 #endif
@@ -445,7 +448,7 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     double best = di2;
     int bestId = i;
     if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
-    if (HV && qb) {
+    if (HV && qb && VD_SEARCH_BATCH) {
       // refined index: the query as a batch of one -- the cell-by-cell pass over sub-grids (vd_batch.cuh) instead of the
       // general single-query search
       if (lane_id() == 0) { qb->qx[0] = ax; qb->qy[0] = ay; qb->qz[0] = az; qb->best[0] = best; qb->bestId[0] = bestId; }
