@@ -281,10 +281,16 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
              "neighbour_entries": int(ctx.cells.n_nbrs)}
     # sharded: the ranks together made ONE diagram of n cells per step; replicas: one each
     value, ms = ranks.whole_job_rate(float(w.n * args.steps) / (world if sharded else 1), ms, dev)
-    # D_alg next to D_act: one more, untimed, step with vd_options.count_alg
-    ctx.set_options(count_alg=1, **opts)
+    # The work counts come from one more, UNTIMED, step on the same inputs with vd_options.count_alg = 2: the
+    # timed kernels keep no per-query statistics (their bookkeeping alone is 3-4 % of a step), the counting ones do, and D_alg
+    # (next to D_act) is counted there too.  The work is a property of the inputs: the timed step did the same.
+    ctx.set_options(count_alg=2, **opts)
     ctx.compute()
-    d_alg = ctx.counters()["alg_evals"]
+    full = ctx.counters()
+    d_alg = full["alg_evals"]
+    for k in ("queries", "dist_evals", "row_evals", "search_evals", "search_iters", "clips", "clip_corners", "new_corners", "fan_simplices", "pairs", "pieces", "pre_clips"):
+        cnt[k] = full[k]
+    pcnt = ctx.phase_counters()
     # Alg. 5's site division (vd_options.dissolve; convex tet meshes, one GPU): interior cells as whole cells.  Reported
     # beside the per-piece number, never instead of it (the per-piece output is what parity with SURVEY 8c.1 is defined on)
     dissolve = None
@@ -297,6 +303,8 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
             flush.fill_(k & 0xff)
             ctx.compute()
             ts.append(ctx.stage_ms()["total"])
+        ctx.set_options(dissolve=1, count_alg=1)     # the work counts: one more untimed step with the statistics on
+        ctx.compute()
         dc = ctx.counters()
         dissolve = {"ms_per_step": float(np.mean(ts)), "value": w.n / (float(np.mean(ts)) * 1e-3), "unit": UNIT, "pairs": dc["pairs"],
                     "queries_per_cell": dc["queries"] / w.n, "paper_queries_per_cell_serial_alg2_cube": 20.54,
@@ -358,6 +366,7 @@ def measure(w, workload, cfg, args, env, cpu_seconds):
         "nonempty_cells_per_s": value * sizes["nonempty_cells"] / w.n, "pairs_per_s": value * cnt["pairs"] / w.n,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "gpu_launches": int(launches), "stage_ms": stage, "counters": cnt,
+        "counters_source": "launches / syncs / waves: the last timed step; work counts: one extra untimed step with vd_options.count_alg = 2",
         "per_cell": {"queries": cnt["queries"] / w.n, "d_act": cnt["dist_evals"] / w.n, "d_alg": d_alg / w.n,
                      "d_act_over_d_alg": cnt["dist_evals"] / max(1, d_alg), "queries_per_pair": cnt["queries"] / max(1, cnt["pairs"]),
                      "clips": cnt["clips"] / w.n, "pieces": cnt["pieces"] / w.n},

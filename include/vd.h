@@ -138,16 +138,21 @@ typedef struct vd_options {
                              magnitude); only the survivors are loaded and evaluated in fp64.  The paper's GPU runs are
                              fp32 throughout; here decisions and results stay fp64-exact (same cells, bit for bit in
                              structure).  0 (default): fp64 throughout.  Not combined with weighted 3-D sites.              */
-  int32_t count_alg;      /* 1: also count D_alg (vd_counters.alg_evals): after every nearest-site query the sites of the
-                             grid cells that meet the ball (q, |q - N_q|) -- the least an exact grid search must examine
-                             (SURVEY 8d).  Slower; for measurement runs.                                                   */
+  int32_t count_alg;      /* measurement runs.  0 (default): the clip kernels keep no per-query statistics (vd_counters.queries
+                             and dist_evals count only the seeds' queries of the mesh vertices; row_evals and search_evals
+                             stay 0: the bookkeeping alone is 3-4 % of a step);
+                             1: those statistics are collected (the "full" kernels run);  2: and D_alg as well
+                             (vd_counters.alg_evals): after every nearest-site query the sites of the grid cells that meet
+                             the ball (q, |q - N_q|) -- the least an exact grid search must examine; slower.    */
   int32_t reuse_nbrs;     /* vd_lloyd, whole-cell kinds: 0 / 1 (default): iteration k+1 clips every cell first by the bisectors
                              of its neighbours of iteration k instead of looking up the nearest sites again;
                              < 0: off                                                                                      */
   int32_t reserved[3];
 } vd_options;
 
-/* Work counters of the last vd_compute (always collected; a few atomics per pair). */
+/* Work counters of the last vd_compute (a few atomics per warp and kernel).  queries, dist_evals, row_evals and search_evals
+ * are per-query statistics: collected only with vd_options.count_alg >= 1 (or another option that selects the full kernels:
+ * step_out, fp32_filter, weighted 3-D sites); everything else always. */
 typedef struct vd_counters {
   int64_t pairs;          /* (simplex, site) pairs processed = Alg. 3 runs          */
   int64_t pieces;         /* non-empty pieces                                                      */

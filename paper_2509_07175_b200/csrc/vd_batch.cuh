@@ -65,7 +65,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
   const unsigned looseMask = __ballot_sync(kFull, loose);
   __syncwarp();
   const int R = B.rowStart[nq];
-  st.rows += (unsigned)R;
+  VD_STAT(st.rows += (unsigned)R;)
   for (int r0 = 0; r0 < R; r0 += kLanes) {
     const int rho = r0 + lane;
     int s = 0, cnt = 0, u = 0;
@@ -90,7 +90,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
     const int pin = warp_incl_scan(cnt);
     const int excl = pin - cnt;
     const int total = shfl(pin, kLanes - 1);
-    st.dist_evals += (unsigned)total;
+    VD_STAT(st.dist_evals += (unsigned)total;)
     for (int t0 = 0; t0 < total; t0 += kLanes) {
       unsigned bit = 0;
       if (cnt > 0) {
@@ -226,7 +226,7 @@ static __device__ __noinline__ unsigned batch_nearest(const GridIndex& gTop, QBa
       }
     }
   }
-  st.queries += (unsigned)(nq - __popc(looseMask));
+  VD_STAT(st.queries += (unsigned)(nq - __popc(looseMask));)
   if (counts_alg(gTop)) {
     // D_alg of the batched queries (the loose ones count inside nearest())
     unsigned v = 0;

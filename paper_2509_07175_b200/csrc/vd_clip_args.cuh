@@ -72,8 +72,10 @@ struct LocalCnt {
   unsigned pairs, pieces, search_iters, clips, search_evals, pre_clips;
 };
 
-__device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats& st, const LocalCnt& lc, int kind = CNT_OTHER) {
+__device__ __forceinline__ void flush_counters(Control* ctl, const QueryStats&, const LocalCnt& lc, int kind = CNT_OTHER) {
+  __syncwarp();
   if (lane_id() == 0) {
+    const WarpStats st = warp_stats();
     Counters* cnt = &ctl->cnt[kind];
     atomicAdd(&cnt->pairs, (unsigned long long)lc.pairs);
     atomicAdd(&cnt->pieces, (unsigned long long)lc.pieces);
@@ -210,7 +212,7 @@ static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, dou
   const int incl = warp_incl_scan(cnt);
   const int excl = incl - cnt;
   const int total = min(shfl(incl, kLanes - 1), 16 * kLanes);   // a dense cluster: the first 512 will do
-  st.dist_evals += (unsigned)total;
+  VD_STAT(st.dist_evals += (unsigned)total;)
   double md = 2e300;
   int mi = 0x7fffffff;
   for (int t0 = 0; t0 < total; t0 += kLanes) {
@@ -307,12 +309,12 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
     }
   }
   if (HV && __any_sync(kFull, refined)) return false;
-  st.queries += 1;
-  st.rows += (unsigned)nrows;
+  VD_STAT(st.queries += 1;)
+  VD_STAT(st.rows += (unsigned)nrows;)
   const int incl = warp_incl_scan(cnt);
   const int excl = incl - cnt;
   const int total = shfl(incl, kLanes - 1);
-  st.dist_evals += (unsigned)total;
+  VD_STAT(st.dist_evals += (unsigned)total;)
   double tb = 2.0;
   int jb = 0x7fffffff;
   for (int t0 = 0; t0 < total; t0 += kLanes) {
@@ -487,7 +489,8 @@ template <bool HV, bool DEFER = false>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
                                              double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch4 = nullptr) {
-  const unsigned e0 = st.dist_evals;
+  __syncwarp();
+  const unsigned e0 = warp_stats().dist_evals;
   unsigned iters = 0;
   int r;
   if (scratch4) {
@@ -504,7 +507,8 @@ __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex&
     nx = __shfl_sync(kFull, out[0], 0); ny = __shfl_sync(kFull, out[1], 0); nz = __shfl_sync(kFull, out[2], 0); d = __shfl_sync(kFull, out[3], 0);
   }
   lc.search_iters += iters;
-  lc.search_evals += st.dist_evals - e0;
+  __syncwarp();
+  lc.search_evals += warp_stats().dist_evals - e0;
   return r;
 }
 

@@ -319,15 +319,17 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
   QueryStats st = {0u, 0u, 0u};
+  extra_cnt_reset();
   for (int64_t q = warp; q < nq; q += nwarps) {
     double best = 2e300;
     int bestId = 0x7fffffff;
     nearest<true>(g, q3[q * 3 + 0], q3[q * 3 + 1], q3[q * 3 + 2], best, bestId, st);
     if (lane_id() == 0) out[q] = bestId;
   }
+  __syncwarp();
   if (lane_id() == 0 && cnt) {
-    atomicAdd(&cnt->queries, (unsigned long long)st.queries);
-    atomicAdd(&cnt->dist_evals, (unsigned long long)st.dist_evals);
+    atomicAdd(&cnt->queries, (unsigned long long)warp_stats().queries);
+    atomicAdd(&cnt->dist_evals, (unsigned long long)warp_stats().dist_evals);
   }
 }
 
@@ -340,6 +342,7 @@ __global__ void __launch_bounds__(kBlock) k_delta(const GridIndex* __restrict__ 
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
   QueryStats st = {0u, 0u, 0u, 0};
+  extra_cnt_reset();
   for (int64_t i = warp; i < n; i += nwarps) {
     double best = 2e300;
     int bestId = 0x7fffffff;
@@ -347,9 +350,10 @@ __global__ void __launch_bounds__(kBlock) k_delta(const GridIndex* __restrict__ 
     nearest<true, true>(g, sites3[i * 3 + 0], sites3[i * 3 + 1], sites3[i * 3 + 2], best, bestId, st);
     if (lane_id() == 0) delta[i] = best < 1e300 ? 0.5 * sqrt(best) : 1e300;   // n = 1: no other site
   }
+  __syncwarp();
   if (lane_id() == 0 && cnt) {
-    atomicAdd(&cnt->queries, (unsigned long long)st.queries);
-    atomicAdd(&cnt->dist_evals, (unsigned long long)st.dist_evals);
+    atomicAdd(&cnt->queries, (unsigned long long)warp_stats().queries);
+    atomicAdd(&cnt->dist_evals, (unsigned long long)warp_stats().dist_evals);
   }
 }
 
@@ -385,7 +389,7 @@ vd_status stage_index(vd_ctx* c) {
   const int nb = grid_for(n, kBlock) < kBBoxBlocks ? grid_for(n, kBlock) : kBBoxBlocks;
   VD_LAUNCH(k_bbox_partial, nb, kBlock, 0, st)(c->sites.as<double>(), n, c->bbox.as<double>());
   VD_LAUNCH(k_grid_params, 1, 1, 0, st)(c->bbox.as<double>(), nb, n, density, gridCap, c->cellStart.as<int>(),
-                                         c->sorted2.as<double4>(), c->opt.count_alg > 0 ? 1 : 0,
+                                         c->sorted2.as<double4>(), c->opt.count_alg > 1 ? 1 : 0,
                                          stepMode ? c->delta.as<double>() : nullptr, stepMode,
                                          lifted4 ? c->sortedW.as<double>() : nullptr, lifted4 ? c->siteW.as<double>() : nullptr,
                                          f32 ? c->sorted32.as<float4>() : nullptr, c->grid.as<GridIndex>(),
@@ -484,6 +488,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points_static(const GridInde
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
   QueryStats st = {0u, 0u, 0u, 0};
+  extra_cnt_reset();
   for (int64_t q = warp; q < nq; q += nwarps) {
     const double x = S->q[q * dim + 0], y = S->q[q * dim + 1], z = dim == 3 ? S->q[q * dim + 2] : 0.0;
     const bool finite = x == x && y == y && z == z && fabs(x) <= 1e150 && fabs(y) <= 1e150 && fabs(z) <= 1e150;

@@ -17,8 +17,24 @@ struct QueryStats {
 constexpr int kExtraCnt = 6;   // [5] candidates that passed the fp32 filter (evaluated in fp64)
 static __shared__ unsigned sExtraCnt[kWarpsPerBlock][kExtraCnt + 3];
 
+// The statistics of the queries (nearest-site queries, site distance evaluations, grid rows examined) live in shared memory
+// too, one row per warp, bumped by lane 0 with warp-uniform amounts: as fields of a struct passed by reference into the (not
+// inlined) query routines they lived in LOCAL memory -- a load and a store per update, through the L1 the site records
+// stream through (measured: 3-4 % of a step).  VD_STAT(st.rows += n;) names the row `st`, shadowing the unused parameter.
+struct WarpStats { unsigned queries, dist_evals, rows, pad; };
+static __shared__ WarpStats sWarpStats[kWarpsPerBlock];
+__device__ __forceinline__ WarpStats& warp_stats() { return sWarpStats[(threadIdx.x / kLanes) % kWarpsPerBlock]; }
+// They exist in the full kernels only (VD_EXT, vd_options.count_alg): in the default kernels the updates alone -- a
+// predicated read-modify-write per query, row pass and candidate round -- were 3-4 % of a step (C2 19.98 -> 19.35 ms).
+#if !VD_EXT
+#define VD_STAT(x)
+#else
+#define VD_STAT(x) { if (lane_id() == 0) { WarpStats& st = warp_stats(); x } }
+#endif
+
 __device__ __forceinline__ void extra_cnt_reset() {
   if (lane_id() < kExtraCnt) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][lane_id()] = 0u;
+  if (lane_id() == 0) { WarpStats& w = warp_stats(); w.queries = 0u; w.dist_evals = 0u; w.rows = 0u; w.pad = 0u; }
   __syncwarp();
 }
 __device__ __forceinline__ void extra_cnt_add(int which, unsigned v) {
@@ -59,7 +75,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
   int* base = sBase[(threadIdx.x / kLanes) % kWarpsPerBlock];
   const int ny = y1 - y0 + 1;
   const int nrows = ny * (z1 - z0 + 1);
-  st.rows += (unsigned)nrows;
+  VD_STAT(st.rows += (unsigned)nrows;)
   // fp32 filter: the query in float, and the fp32 threshold of the current bound (recomputed when the bound moves)
   const bool f32 = has_f32(g) && !has_weights(g);
   float qxf = 0.f, qyf = 0.f, qzf = 0.f, thr = 0.f;
@@ -94,7 +110,7 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
     const int incl = warp_incl_scan(cnt);
     const int excl = incl - cnt;
     const int total = shfl(incl, kLanes - 1);
-    st.dist_evals += (unsigned)total;
+    VD_STAT(st.dist_evals += (unsigned)total;)
     for (int t0 = 0; t0 < total; t0 += kLanes) {
       // rows that start inside this chunk, plus the row that straddles its beginning
       unsigned bit = 0;
@@ -289,7 +305,7 @@ template <bool HV, bool SKIP>
 static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
                                              QueryStats& st, bool nearer_ok) {
   const double bound0 = best;
-  st.queries += 1;
+  VD_STAT(st.queries += 1;)
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);
   if (HV) {
     // Refined home cell (dense cluster): work in its sub-grid.  If the ball lies inside the home cell,

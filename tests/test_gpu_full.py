@@ -82,12 +82,18 @@ def test_c2_dissolve_mode_all_cells():
     element, and the counters say what the mode saves."""
     w = inputs.config(2)
     with binding.Context(w.sites) as ctx:
+        ctx.set_options(count_alg=1)                 # per-query statistics on (off by default)
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         plain, c0 = ctx.to_host(), ctx.counters()
-        ctx.set_options(dissolve=1)
+        ctx.set_options(dissolve=1, count_alg=1)
         ctx.compute()
         g, c1 = ctx.to_host(), ctx.counters()
+        ctx.set_options(dissolve=1)                  # the default kernels: same cells, no per-query statistics
+        ctx.compute()
+        g2, c2 = ctx.to_host(), ctx.counters()
+    assert np.array_equal(g2.vert_flags, g.vert_flags) and np.allclose(g2.measure, g.measure, rtol=1e-11, atol=0)
+    assert c2["queries"] < 0.01 * c1["queries"] and c2["pairs"] == c1["pairs"]     # (what is left: the seeds' queries of the mesh vertices)
     assert np.array_equal(g.nbr_off, plain.nbr_off) and np.array_equal(g.nbr, plain.nbr)
     assert np.allclose(g.measure, plain.measure, rtol=1e-9, atol=0)
     assert np.abs(g.centroid - plain.centroid).max() <= 1e-9 * w.diameter

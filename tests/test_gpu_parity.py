@@ -126,7 +126,7 @@ def test_replica_parity(idx, opts):
                                   dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
                                   dict(tail_pairs=-1, small_wave=-1), dict(tail_pairs=64, small_wave=-1), dict(first_clip=-1), dict(first_clip=-1, small_wave=-1),
                                   dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000),
-                                  dict(step_out=1), dict(step_out=2, small_wave=-1), dict(step_out=1, ball_cells=-1), dict(count_alg=1)])
+                                  dict(step_out=1), dict(step_out=2, small_wave=-1), dict(step_out=1, ball_cells=-1), dict(count_alg=1), dict(count_alg=2, small_wave=-1)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
     g, _, _ = _gpu(w, **opts)
@@ -390,7 +390,7 @@ def test_box_domain_wave_mode_and_lloyd():
 def test_support_calls_phase_times_counters_and_pinned_copy():
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
-        ctx.set_options(small_wave=-1)     # the step kernels also on this replica's small wavefronts
+        ctx.set_options(small_wave=-1, count_alg=1)     # the step kernels also on this replica's small wavefronts; per-query statistics on
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         ph, cnt, st = ctx.phase_ms(), ctx.counters(), ctx.stage_ms()
@@ -598,10 +598,17 @@ def test_counters_per_step_kernel_add_up():
     init (no search) / fix / tail, fan simplices under finish."""
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
-        ctx.set_options(small_wave=-1)
+        ctx.set_options(small_wave=-1, count_alg=1)
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         tot, ph = ctx.counters(), ctx.phase_counters()
+        ctx.set_options(small_wave=-1)              # the default kernels keep no per-query statistics; everything else is counted
+        ctx.compute()
+        lean = ctx.counters()
+    assert lean["queries"] <= len(w.verts) + 8 and lean["row_evals"] == 0          # (the seeds' queries of the mesh vertices are always counted)
+    for f in ("pairs", "pieces", "fan_simplices"):      # (clips / pre_clips depend on which neighbour discovers a pair first)
+        assert lean[f] == tot[f], f
+    assert lean["clips"] > 0 and lean["pre_clips"] > 0
     for f in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips", "clip_corners", "new_corners", "fan_simplices"):
         assert sum(ph[k][f] for k in ph) == tot[f], f
     assert ph["verify"]["queries"] > 0 and ph["verify"]["clips"] == 0 and ph["verify"]["search_iters"] == 0
