@@ -87,46 +87,25 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
         }
       }
     }
-    const int pin = warp_incl_scan(cnt);
-    const int excl = pin - cnt;
-    const int total = shfl(pin, kLanes - 1);
-    VD_STAT(st.dist_evals += (unsigned)total;)
-    for (int t0 = 0; t0 < total; t0 += kLanes) {
-      unsigned bit = 0;
-      if (cnt > 0) {
-        if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
-        else if (excl < t0 && pin > t0) bit = 1u;
-      }
-      const unsigned starts = __reduce_or_sync(kFull, bit);
-      const unsigned owners = __ballot_sync(kFull, bit != 0);
-      if (bit) {
-        const int slot = __popc(owners & ((1u << lane) - 1u));
-        B.base[slot] = s - excl;
-        B.qid[slot] = (unsigned char)u;
-      }
-      __syncwarp();
-      const int t = t0 + lane;
-      bool valid = t < total;
+    const int total = for_each_packed(s, cnt, B.base, 0x7fffffff, [&](int slot) { B.qid[slot] = (unsigned char)u; },
+                                      [&](bool valid, int pos, int owner) {
       double d2 = 0.0;
-      int id = 0x7fffffff, cu = 0, owner = 0;
+      int id = 0x7fffffff, cu = 0;
       bool better = false;
-      if (valid) {
-        owner = __popc(starts & ((2u << lane) - 1u)) - 1;
-        cu = B.qid[owner];
-      }
+      if (valid) cu = B.qid[owner];
       if (f32) {
         if (valid) {
-          const float4 pf = g.sites32[B.base[owner] + t];
+          const float4 pf = g.sites32[pos];
           const float fx = B.qf[cu][0] - pf.x, fy = B.qf[cu][1] - pf.y, fz = B.qf[cu][2] - pf.z;
           valid = fx * fx + fy * fy + fz * fz <= B.qf[cu][3];   // else: farther than its query's bound, whatever fp64 would say
         }
         extra_cnt_add(5, (unsigned)__popc(__ballot_sync(kFull, valid)));
       }
       if (valid) {
-        const double4 p = g.sites[B.base[owner] + t];
+        const double4 p = g.sites[pos];
         const double dx = B.qx[cu] - p.x, dy = B.qy[cu] - p.y, dz = B.qz[cu] - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
-        if (has_weights(g)) d2 += __ldg(&g.sitesW[B.base[owner] + t]);
+        if (has_weights(g)) d2 += __ldg(&g.sitesW[pos]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
         better = closer(d2, id, B.best[cu], B.bestId[cu]);
       }
@@ -143,8 +122,8 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
         better = better && lane != src && closer(d2, id, B.best[cu], B.bestId[cu]);
         m = __ballot_sync(kFull, better);
       }
-      __syncwarp();
-    }
+    });
+    VD_STAT(st.dist_evals += (unsigned)total;)
   }
   return looseMask;
 }

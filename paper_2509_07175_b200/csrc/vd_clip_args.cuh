@@ -209,33 +209,19 @@ static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, dou
     s = __ldg(&g.cellStart[rowBase + x0]);
     cnt = __ldg(&g.cellStart[rowBase + x1 + 1]) - s;
   }
-  const int incl = warp_incl_scan(cnt);
-  const int excl = incl - cnt;
-  const int total = min(shfl(incl, kLanes - 1), 16 * kLanes);   // a dense cluster: the first 512 will do
-  VD_STAT(st.dist_evals += (unsigned)total;)
   double md = 2e300;
   int mi = 0x7fffffff;
-  for (int t0 = 0; t0 < total; t0 += kLanes) {
-    unsigned bit = 0;
-    if (cnt > 0) {
-      if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
-      else if (excl < t0 && incl > t0) bit = 1u;
-    }
-    const unsigned starts = __reduce_or_sync(kFull, bit);
-    const unsigned owners = __ballot_sync(kFull, bit != 0);
-    if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
-    __syncwarp();
-    const int t = t0 + lane;
-    if (t < total) {
-      const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
-      const double4 p = g.sites[base[owner] + t];
+  const int total = for_each_packed(s, cnt, base, 16 * kLanes /* a dense cluster: the first 512 will do */, [](int) {},
+                                    [&](bool valid, int pos, int) {
+    if (valid) {
+      const double4 p = g.sites[pos];
       const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       const double dx = vx - p.x, dy = vy - p.y, dz = vz - p.z;
       const double d2 = dx * dx + dy * dy + dz * dz;
       if (id != i && d2 > 0.0 && closer(d2, id, md, mi)) { md = d2; mi = id; }
     }
-    __syncwarp();
-  }
+  });
+  VD_STAT(st.dist_evals += (unsigned)total;)
   int found = 0;
   for (; found < k; ++found) {
     double bd = md;
@@ -311,29 +297,14 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
   if (HV && __any_sync(kFull, refined)) return false;
   VD_STAT(st.queries += 1;)
   VD_STAT(st.rows += (unsigned)nrows;)
-  const int incl = warp_incl_scan(cnt);
-  const int excl = incl - cnt;
-  const int total = shfl(incl, kLanes - 1);
-  VD_STAT(st.dist_evals += (unsigned)total;)
   double tb = 2.0;
   int jb = 0x7fffffff;
-  for (int t0 = 0; t0 < total; t0 += kLanes) {
-    unsigned bit = 0;
-    if (cnt > 0) {
-      if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
-      else if (excl < t0 && incl > t0) bit = 1u;
-    }
-    const unsigned starts = __reduce_or_sync(kFull, bit);
-    const unsigned owners = __ballot_sync(kFull, bit != 0);
-    if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
-    __syncwarp();
-    const int t = t0 + lane;
-    if (t < total) {
-      const int owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
-      const double4 p = g.sites[base[owner] + t];
+  const int total = for_each_packed(s, cnt, base, 0x7fffffff, [](int) {}, [&](bool valid, int pos, int) {
+    if (valid) {
+      const double4 p = g.sites[pos];
       const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
-      const double pw = has_weights(g) ? __ldg(&g.sitesW[base[owner] + t]) : 0.0;
+      const double pw = has_weights(g) ? __ldg(&g.sitesW[pos]) : 0.0;
       const double dq2 = dx * dx + dy * dy + dz * dz + pw;
       bool cand = id != i && id != j && dq2 < r2 * (1.0 - 1e-13);
       if (cand && !(dq2 < r2 * (1.0 - 1e-9)))
@@ -345,8 +316,8 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
         if (closer(tk, id, tb, jb)) { tb = tk; jb = id; }
       }
     }
-    __syncwarp();
-  }
+  });
+  VD_STAT(st.dist_evals += (unsigned)total;)
   warp_argmin(tb, jb);
   if (closer(tb, jb, tbest, jbest)) { tbest = tb; jbest = jb; }
   if (counts_alg(gTop)) extra_cnt_add(4, lane == 0 ? ball_sites(gTop, qx, qy, qz, r2) : 0u);   // the search needs every site of this ball

@@ -55,6 +55,43 @@ __device__ __forceinline__ double slab_d2(const GridIndex& g, int ax, double q, 
   return d * d;
 }
 
+// The one packing routine of every candidate scan (nearest query, batched tests, nearest-site lists, one-shot search): lane r
+// holds row r of up to 32 grid rows -- `cnt` sites from position `s` of the sorted site array (cnt = 0: none).  Their candidates
+// are handed out 32 per round: body(valid, pos, owner) runs once per round with all lanes converged; lane l gets candidate
+// t0 + l -- `valid`: it exists, `pos`: its position in the site array, `owner`: the index, among the rows that start in or
+// straddle this round (in lane order), of the row it belongs to.  on_row(slot) has run before on the lane that holds row
+// number `slot` of the round (for per-row payloads such as the query a row belongs to).  base: 32 ints of shared scratch of
+// this warp.  At most `limit` candidates are handed out.  Returns how many.
+template <class OnRow, class Body>
+__device__ __forceinline__ int for_each_packed(int s, int cnt, int* base, int limit, OnRow&& on_row, Body&& body) {
+  const int lane = lane_id();
+  const int incl = warp_incl_scan(cnt);
+  const int excl = incl - cnt;
+  const int total = min(shfl(incl, kLanes - 1), limit);
+  for (int t0 = 0; t0 < total; t0 += kLanes) {
+    // rows that start inside this round, plus the row that straddles its beginning
+    unsigned bit = 0;
+    if (cnt > 0) {
+      if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
+      else if (excl < t0 && incl > t0) bit = 1u;
+    }
+    const unsigned starts = __reduce_or_sync(kFull, bit);
+    const unsigned owners = __ballot_sync(kFull, bit != 0);
+    if (bit) {
+      const int slot = __popc(owners & ((1u << lane) - 1u));
+      base[slot] = s - excl;
+      on_row(slot);
+    }
+    __syncwarp();
+    const int t = t0 + lane;
+    const bool valid = t < total;
+    const int owner = valid ? __popc(starts & ((2u << lane) - 1u)) - 1 : 0;
+    body(valid, valid ? base[owner] + t : 0, owner);
+    __syncwarp();
+  }
+  return total;
+}
+
 // Scan every cell of the box [x0..x1]x[y0..y1]x[z0..z1] whose row can hold a site closer than best.
 // One lane per row (y,z): box-distance pruning, x-extent tightened to the ball, one contiguous site
 // range per row.  The candidates of all rows are then packed 32 at a time over the lanes (prefix sum of
@@ -107,30 +144,12 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         }
       }
     }
-    const int incl = warp_incl_scan(cnt);
-    const int excl = incl - cnt;
-    const int total = shfl(incl, kLanes - 1);
-    VD_STAT(st.dist_evals += (unsigned)total;)
-    for (int t0 = 0; t0 < total; t0 += kLanes) {
-      // rows that start inside this chunk, plus the row that straddles its beginning
-      unsigned bit = 0;
-      if (cnt > 0) {
-        if (excl >= t0 && excl < t0 + kLanes) bit = 1u << (excl - t0);
-        else if (excl < t0 && incl > t0) bit = 1u;
-      }
-      const unsigned starts = __reduce_or_sync(kFull, bit);
-      const unsigned owners = __ballot_sync(kFull, bit != 0);
-      if (bit) base[__popc(owners & ((1u << lane) - 1u))] = s - excl;
-      __syncwarp();
-      const int t = t0 + lane;
+    const int total = for_each_packed(s, cnt, base, 0x7fffffff, [](int) {}, [&](bool valid, int pos, int) {
       double d2 = best;
       int id = 0x7fffffff;
-      bool valid = t < total;
-      int owner = 0;
-      if (valid) owner = __popc(starts & (0xffffffffu >> (kLanes - 1 - lane))) - 1;
       if (f32) {
         if (valid) {
-          const float4 pf = g.sites32[base[owner] + t];
+          const float4 pf = g.sites32[pos];
           const float fx = qxf - pf.x, fy = qyf - pf.y, fz = qzf - pf.z;
           valid = fx * fx + fy * fy + fz * fz <= thr;   // else: farther than the bound, whatever fp64 would say
         }
@@ -138,10 +157,10 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         extra_cnt_add(5, (unsigned)__popc(pass));
       }
       if (valid) {
-        const double4 p = g.sites[base[owner] + t];
+        const double4 p = g.sites[pos];
         const double dx = qx - p.x, dy = qy - p.y, dz = qz - p.z;
         d2 = dx * dx + dy * dy + dz * dz;
-        if (has_weights(g)) d2 += __ldg(&g.sitesW[base[owner] + t]);
+        if (has_weights(g)) d2 += __ldg(&g.sitesW[pos]);
         id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       }
       const bool better = valid && closer(d2, id, best, bestId) && !(SKIP && id == st.skip);
@@ -152,8 +171,8 @@ static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, doub
         bestId = id;
         if (f32) thr = f32_threshold(best, fM);
       }
-      __syncwarp();
-    }
+    });
+    VD_STAT(st.dist_evals += (unsigned)total;)
     if (TOP) {
       unsigned hm = __ballot_sync(kFull, hxa <= hxb);
       while (hm) {
