@@ -92,7 +92,10 @@ __device__ __forceinline__ double f32_magnitude(const GridIndex& g, double qx, d
 }
 __device__ __forceinline__ double site_w(const GridIndex& g, int id) { return has_weights(g) ? __ldg(&g.siteWid[id]) : 0.0; }
 
-constexpr int kHeavy = 64;                // sites per cell above which the cell is refined (one warp round)
+#ifndef VD_HEAVY
+#define VD_HEAVY 128   // measured on C3 (round 2): 32 sites 316 ms, 64: 302, 128: 294, 256: 301, 512: 333
+#endif
+constexpr int kHeavy = VD_HEAVY;                // sites per cell above which the cell is refined (one warp round)
 
 // One unit of work: simplex a, site i, and a witness point w in T_a ∩ Ω_i
 // (DESIGN.md "witness"): the start p_s of virtual edges instead of v_i (Alg. 3 line 3).
