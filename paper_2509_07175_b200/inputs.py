@@ -122,6 +122,40 @@ def octahedron_mesh():
     return verts, np.array(tets, dtype=np.int32)
 
 
+def carve(verts: np.ndarray, simplices: np.ndarray, keep: np.ndarray):
+    """The sub-mesh of the simplices flagged in `keep`, its vertices renumbered without gaps."""
+    simp = simplices[keep]
+    used = np.unique(simp)
+    remap = np.full(len(verts), -1, dtype=np.int64)
+    remap[used] = np.arange(len(used))
+    return np.ascontiguousarray(verts[used]), remap[simp].astype(np.int32)
+
+
+def carved_domain(kind: int, k: int = 10, jitter: float = 0.0, seed: int = 5):
+    """A non-convex, disconnected domain (Alg. 4 makes no convexity assumption): the unit square / cube /
+    torus minus a notch (the rest is U-shaped, or an open band with two boundary loops) and minus a strip that detaches
+    an island.  `jitter` > 0 moves every vertex by up to jitter x grid spacing (uneven simplices, all still positively
+    sized for jitter < 0.2); on the square and the cube the outer boundary vertices move too, so the measure is the
+    mesh's own (`mesh_measure`), not a closed form."""
+    rng = np.random.default_rng(seed)
+    if kind == KIND_TRI_SURFACE:
+        verts, simp = torus_mesh(4 * k, 2 * k)
+        c = verts[simp].mean(axis=1)
+        u = np.arctan2(c[:, 1], c[:, 0])                       # angle around the axis, (-pi, pi]
+        keep = ~((u > 0.4) & (u < 1.3)) & ~((u > 2.2) & (u < 2.5)) & ~((u > -2.0) & (u < -1.8) & (c[:, 2] > 0))
+        h = 2.0 * np.pi / (4 * k)
+    else:
+        verts, simp = square_grid_mesh(k) if kind == KIND_TRI_2D else cube_kuhn_mesh(k)
+        c = verts[simp].mean(axis=1)
+        notch = (c[:, 0] > 0.3) & (c[:, 0] < 0.7) & (c[:, 1] > 0.3)
+        strip = (c[:, 0] > 0.8) & (c[:, 0] < 0.9)
+        keep = ~notch & ~strip
+        h = 1.0 / k
+    if jitter > 0.0:
+        verts = verts + (rng.random(verts.shape) * 2.0 - 1.0) * (jitter * h)
+    return carve(verts, simp, keep)
+
+
 def mesh_measure(verts: np.ndarray, simplices: np.ndarray, kind: int) -> float:
     """|M| from the mesh itself (plain determinant / cross-product formulas)."""
     p = verts[simplices]
@@ -220,6 +254,20 @@ def config(idx: int, scale: str = "full") -> Workload:
 
 def custom(kind: int, sites, verts, simplices, name="custom") -> Workload:
     return _wl(name, kind, np.asarray(sites, dtype=np.float64), verts, simplices)
+
+
+def carved(kind: int, n: int, jitter: float = 0.15, seed: int = 31, k: int = 10) -> Workload:
+    """`carved_domain` with sites over its bounding box, the removed parts included (cells that lose pieces to the
+    notch, cells that own nothing, cells split between an arm and the island); surface kind: a shell around the torus as
+    in C4."""
+    v, t = carved_domain(kind, k, jitter)
+    rng = np.random.default_rng(seed)
+    if kind == KIND_TRI_SURFACE:
+        sites = sites_torus_shell(rng, n)
+    else:
+        lo, hi = v.min(0) - 0.03, v.max(0) + 0.03
+        sites = lo + rng.random((n, v.shape[1])) * (hi - lo)
+    return custom(kind, sites, v, t, f"carved{kind}")
 
 
 def box(dim: int, n: int, seed: int = 7, lo=None, hi=None, name=None) -> Workload:

@@ -505,6 +505,39 @@ def test_one_simplex_many_cells(kind):
         assert max(nedges) > 8
 
 
+# ---------------------------------------------------------------------- non-convex, disconnected domains
+def test_golden_carved_square_cases_through_the_abi():
+    import json, os
+    here = os.path.dirname(os.path.abspath(__file__))
+    d = json.load(open(os.path.join(here, "golden", "carved_square_cases.json")))
+    v, t = inputs.carved_domain(d["domain"]["kind"], d["domain"]["k"])
+    for case in d["cases"]:
+        g = binding.compute(np.array(case["sites"], dtype=np.float64), v, t, 0)
+        assert np.allclose(g.measure, case["area"], rtol=0, atol=1e-12)
+        for i, cen in enumerate(case["centroid"]):
+            if cen is not None:
+                assert np.allclose(g.centroid[i], cen, rtol=0, atol=1e-12)
+        for i, nb in enumerate(case["nbr"]):
+            assert g.neighbours(i).tolist() == nb
+
+
+@pytest.mark.parametrize("kind,n,opts", [(0, 3000, {}), (0, 3000, dict(persistent=3)), (1, 3000, {}), (1, 3000, dict(persistent=3)),
+                                         (2, 2500, {}), (2, 2500, dict(small_wave=-1)), (2, 2500, dict(persistent=3)),
+                                         (2, 2500, dict(small_wave=-1, tail_pairs=-1)), (2, 2500, dict(first_clip=-1, real_edges=0))])
+def test_carved_domain_parity(kind, n, opts):
+    """U-shaped domain with a detached island, jittered vertices, sites over the whole bounding box: the simplex seeds and
+    the positive flags must reach every piece although cells are cut apart by the notch and the strip (completeness
+    of S3 + S5; Alg. 4 makes no convexity assumption), boundary faces inside the bounding box carry ~m, and sites in the
+    removed parts own only what reaches across."""
+    w = inputs.carved(kind, n)
+    g, cnt, adj = _gpu(w, **opts)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind, tier="A" if kind != inputs.KIND_TET_3D else "B")
+    parity.assert_parity(g, o, w.diameter)
+    assert np.array_equal(adj, o.simplex_adj)
+    assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
+    assert g.n_nonempty == int((o.measure > 0).sum()) and cnt["pieces"] == len(o.piece_simplex)
+
+
 # ---------------------------------------------------------------------- Alg. 5's site division, dissolved output (P:L296-355)
 def _dissolve_case(name):
     rng = np.random.default_rng(71)
@@ -567,6 +600,13 @@ def test_dissolve_mode_rejects_what_it_cannot_do():
         ctx.set_options()                                            # per-piece mode still works on it
         ctx.compute()
         assert abs(ctx.to_host().measure.sum() - (1.0 - 1.0 / 8)) <= 1e-12
+    w = inputs.carved(inputs.KIND_TET_3D, 500, jitter=0.0)          # U-shaped with an island: neither convex nor connected
+    with binding.Context(w.sites) as ctx:
+        ctx.set_options(dissolve=1)
+        ctx.set_domain(w.verts, w.simplices, w.kind)
+        with pytest.raises(binding.VdError) as e:
+            ctx.compute()
+        assert e.value.status == 1 and "convex" in str(e.value)
     v2, t2 = inputs.unit_square_mesh()
     with binding.Context(s[:, :2]) as ctx:
         ctx.set_options(dissolve=1)

@@ -417,3 +417,39 @@ def test_dissolved_cells_are_the_union_of_their_pieces(domain):
             assert abs(vol - dis.measure[i]) <= 1e-9 * vol
             whole += 1
     assert whole > 30 and whole < (plain.measure > 0).sum()
+
+
+# ---------------------------------------------------------------------- non-convex, disconnected domains
+def _carved_cases():
+    with open(os.path.join(HERE, "golden", "carved_square_cases.json")) as f:
+        d = json.load(f)
+    v, t = inputs.carved_domain(d["domain"]["kind"], d["domain"]["k"])
+    return v, t, d["cases"]
+
+
+def test_golden_carved_square_cases():
+    """Hand-worked cells on the U-shaped square with a detached island: a cell in several connected components, and Voronoi
+    neighbours whose common edge misses the domain are not restricted neighbours."""
+    v, t, cases = _carved_cases()
+    assert abs(inputs.mesh_measure(v, t, inputs.KIND_TRI_2D) - 0.62) < 1e-14
+    for case in cases:
+        s = np.array(case["sites"], dtype=np.float64)
+        c = oracle.compute(s, v, t, inputs.KIND_TRI_2D)
+        assert np.allclose(c.measure, case["area"], rtol=0, atol=1e-12)
+        for i, cen in enumerate(case["centroid"]):
+            if cen is not None:
+                assert np.allclose(c.centroid[i], cen, rtol=0, atol=1e-12)
+        for i, nb in enumerate(case["nbr"]):
+            assert c.neighbours(i).tolist() == nb
+
+
+@pytest.mark.parametrize("kind,n", [(inputs.KIND_TRI_2D, 600), (inputs.KIND_TRI_SURFACE, 800), (inputs.KIND_TET_3D, 700)])
+def test_carved_domain_invariants_and_tiers(kind, n):
+    w = inputs.carved(kind, n)
+    c = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    _check_invariants(w, c, corner_sample=1500)
+    if kind != inputs.KIND_TRI_SURFACE:
+        b = oracle.compute(w.sites, w.verts, w.simplices, w.kind, tier="B")
+        assert np.array_equal(c.piece_off, b.piece_off) and np.array_equal(c.piece_simplex, b.piece_simplex)
+        assert np.array_equal(c.vert_flags, b.vert_flags) and np.array_equal(c.nbr, b.nbr)
+        assert np.allclose(c.measure, b.measure, rtol=1e-11, atol=0)
