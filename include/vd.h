@@ -113,7 +113,7 @@ typedef struct vd_options {
                              measure x centroid by one sum.  0, 0 (default) = all of M.  Meshed kinds only.            */
   int32_t tail_pairs;     /* phased schedule: a round that leaves at most this many pairs with a corner outside hands
                              them to one kernel that tests and clips them to completion (no further rounds for the
-                             wave); 0 = default (65536); < 0: only what the program's five rounds leave             */
+                             wave); 0 = default (65536); < 0: only what the program's rounds (`rounds`) leave             */
   int32_t first_clip;     /* 0 / 1 (default): a pair (T_a, v_i) discovered through the face of P_{a,u} on B_ui is first
                              clipped by that bisector, without a search -- the first clip of G_{a,j};
                              < 0: every clip is found by a search (Alg. 3 as printed).  3D kinds.                   */
@@ -147,7 +147,13 @@ typedef struct vd_options {
   int32_t reuse_nbrs;     /* vd_lloyd, whole-cell kinds: 0 / 1 (default): iteration k+1 clips every cell first by the bisectors
                              of its neighbours of iteration k instead of looking up the nearest sites again;
                              < 0: off                                                                                      */
-  int32_t reserved[3];
+  int32_t rounds;         /* phased schedule: rounds of {point-in-cell tests of all open corners, one search + clip per pair
+                             with a corner outside} a wave program holds before its finishing kernel (which alternates tests
+                             and clips per pair, Alg. 3's loop as printed, without parking the polytope in between).
+                             0 = default, measured per kind: no rounds on tet meshes with the plain site index
+                             (initialise, finishing kernel, emit), 3 in whole-cell mode, 5 on the refined (clustered) index;
+                             1 ... 6: that many; < 0: none                                                                  */
+  int32_t reserved[2];
 } vd_options;
 
 /* Work counters of the last vd_compute (a few atomics per warp and kernel).  queries, dist_evals, row_evals and search_evals

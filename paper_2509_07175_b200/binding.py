@@ -48,7 +48,7 @@ class vd_options(ctypes.Structure):
                 ("tail_pairs", ctypes.c_int32), ("first_clip", ctypes.c_int32),
                 ("seed_corners", ctypes.c_int32), ("small_wave", ctypes.c_int32), ("step_out", ctypes.c_int32),
                 ("dissolve", ctypes.c_int32), ("fp32_filter", ctypes.c_int32), ("count_alg", ctypes.c_int32),
-                ("reuse_nbrs", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
+                ("reuse_nbrs", ctypes.c_int32), ("rounds", ctypes.c_int32), ("reserved", ctypes.c_int32 * 2)]
 
 
 class vd_counters(ctypes.Structure):

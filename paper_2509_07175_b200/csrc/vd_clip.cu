@@ -437,7 +437,6 @@ vd_status stage_clip(vd_ctx* c) {
   const int smallMode = (mode == 3 || (mode == 2 && !solid) || (phased && mode == 1 && c->opt.small_wave >= 0)) ? WAVE_QUEUE : WAVE_SINGLE;
   const int smallWave = !phased ? 0 : (c->opt.small_wave == 0 ? kSmallWave : (c->opt.small_wave < 0 ? 1 : c->opt.small_wave));
   const int tailPairs = c->opt.tail_pairs == 0 ? 65536 : (c->opt.tail_pairs < 0 ? 0 : c->opt.tail_pairs);
-  const int rounds = 5;
   const int64_t chunk = (int64_t)1 << 20;
   const int64_t cap = phased ? (c->pairCap < chunk ? c->pairCap : chunk) : 1;
   vd_status s;
@@ -456,6 +455,11 @@ vd_status stage_clip(vd_ctx* c) {
     if (!(h.err & (ERR_DUPLICATE | ERR_INPUT))) c->heavyKnown = (int)h.nHeavy;
   }
   const bool hv = h.nHeavy > 0;
+  // rounds of {tests, clips} per wave program before k_ph_tail finishes what they leave.  Measured: on tet meshes with
+  // the plain index the finishing kernel's loop alone (no parking between a pair's clips) beats any number of rounds; whole cells (more
+  // clips per pair) and the refined index (long searches, better in kernels of their own) want rounds.
+  int rounds = c->opt.rounds > 0 ? c->opt.rounds : (c->opt.rounds < 0 ? 0 : (hv ? 5 : (c->kind == KIND_BOX_3D ? 3 : 0)));
+  if (rounds > kMaxRounds) rounds = kMaxRounds;
   int batch = (!phased && smallMode == WAVE_SINGLE) ? 8 : 6;   // the seeds' wave and the large ones it sets off
   for (int guard = 0; guard < 4096; ++guard) {
     if (h.err & (ERR_PAIR_CAP | ERR_VERT_CAP | ERR_NBR_CAP)) break;   // caller grows the pools and reruns

@@ -282,6 +282,9 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k
 // instead of one round trip to the host and two nearly empty launches per remaining round.  Finished pairs join the
 // done list.  The whole loop in one kernel is the instruction-fetch-bound form (header of this file); on a few
 // thousand pairs that does not matter.
+// A program without rounds (the default on tet meshes with the plain site index, where it is the fastest form: no parking between a
+// pair's clips; init and finish stay kernels of their own -- fused into this one, its code no longer fits the instruction cache and the
+// step takes 23.8 instead of 17.6 ms on C2) hands every pair of the wave to this kernel straight from k_ph_init.
 // One launch after the program's rounds.  The rounds stop at the first round r whose tests leave at most tailPairs pairs with
 // a corner outside: those pairs (tested, not clipped) are taken to completion here.  If every round ran its clips, the last
 // round's pairs (clipped, not yet re-tested) are -- so a wave always ends, whatever the number of rounds in the program.
@@ -291,9 +294,9 @@ __global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs 
   if (pc->mode != WAVE_PHASED) return;
   int r = 0;
   while (r < rounds - 1 && (int)pc->nClip[r] > tailPairs) ++r;
-  const int count = (int)pc->nClip[r];
+  const int count = rounds == 0 ? (int)pc->count : (int)pc->nClip[r];   // a program without rounds: every pair of the wave, straight from k_ph_init
   if (count == 0) return;
-  const int* list = lists + (r & 1) * (int64_t)cap;
+  const int* list = rounds == 0 ? nullptr : lists + (r & 1) * (int64_t)cap;
   const int64_t begin = (int64_t)pc->begin;
   const int tslot = 3;   // (cursors 4 ..: four per round -- tests, their second pass, clips, their second pass)
   __shared__ GridIndex g;
@@ -308,14 +311,16 @@ __global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs 
   for (;;) {
     const int t = next_item(pc, tslot, count);
     if (t < 0) break;
-    const int slot = list[t];
+    const int slot = list ? list[t] : t;
     if (slot < 0) continue;   // (the fix kernel marked a pair that left the path)
     CellState* c = &cells[slot];
     int np = c->np, nc = c->nc;
+    if (np < 0) continue;     // (k_ph_init sent the pair to the large tier)
     const int i = c->i;
-    unpark(&S[w], &c->S, kPolyBytes, bar, parity);
-    int failed = 0;
-    for (int guard = 0; guard < 8 * P3 + 32 && nc > 0; ++guard) {
+    int failed = c->failed;
+    const bool work = !failed && nc > 0;   // (else: an empty or failed pair from k_ph_init, which stays parked as it is)
+    if (work) unpark(&S[w], &c->S, kPolyBytes, bar, parity);
+    for (int guard = 0; guard < 8 * P3 + 32 && nc > 0 && !failed; ++guard) {
       int s;
       const int p = select_out_3d(S[w], A, nc, s);
       if (p < 0) {
@@ -326,7 +331,7 @@ __global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs 
       if (rc == 1) { defer_pair(A, begin + slot); np = -1; break; }
       if (rc) { failed = 1; atomicOr(&A.ctl->err, rc == 2 ? ERR_TOPOLOGY : ERR_NOCONVERGE); break; }
     }
-    if (np >= 0) park(&c->S, &S[w], kPolyBytes);
+    if (np >= 0 && work) park(&c->S, &S[w], kPolyBytes);
     if (lane == 0) {
       c->np = np; c->nc = nc; c->failed = failed;
       if (np >= 0) doneList[atomicAdd(&pc->nDone, 1u)] = slot;

@@ -108,11 +108,11 @@ def test_c1_full_parity():
 
 
 # small_wave=-1: the step kernels of the phased schedule on every wavefront, however small (the replicas' wavefronts
-# are below the default threshold and would run the one-kernel form); tail_pairs=-1: rounds of k_ph_verify / k_ph_fix only
+# are below the default threshold and would run the one-kernel form); tail_pairs=-1, rounds=5: five rounds of k_ph_verify / k_ph_fix whatever they leave (the default on these meshes is no round: k_ph_init, the finishing kernel, k_ph_finish)
 @pytest.mark.parametrize("idx,opts", [(2, {}), (3, {}), (4, {}), (5, {}),
                                       (2, dict(small_wave=-1)), (3, dict(small_wave=-1)), (5, dict(small_wave=-1)),
-                                      (2, dict(small_wave=-1, tail_pairs=-1)), (3, dict(small_wave=-1, tail_pairs=-1)),
-                                      (5, dict(small_wave=-1, tail_pairs=-1))])
+                                      (2, dict(small_wave=-1, tail_pairs=-1, rounds=5)), (3, dict(small_wave=-1, tail_pairs=-1, rounds=5)),
+                                      (5, dict(small_wave=-1, tail_pairs=-1, rounds=5))])
 def test_replica_parity(idx, opts):
     w = inputs.config(idx, "small")
     g, cnt, adj = _gpu(w, **opts)
@@ -124,8 +124,8 @@ def test_replica_parity(idx, opts):
 
 @pytest.mark.parametrize("opts", [dict(real_edges=0), dict(grid_density=1.5), dict(grid_density=16.0), dict(persistent=0),
                                   dict(ball_cells=-1), dict(ball_cells=8), dict(near_clips=12), dict(persistent=3),
-                                  dict(tail_pairs=-1, small_wave=-1), dict(tail_pairs=64, small_wave=-1), dict(first_clip=-1), dict(first_clip=-1, small_wave=-1),
-                                  dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000),
+                                  dict(tail_pairs=-1, small_wave=-1, rounds=5), dict(tail_pairs=64, small_wave=-1, rounds=4), dict(first_clip=-1), dict(first_clip=-1, small_wave=-1),
+                                  dict(seed_corners=4), dict(seed_corners=2, small_wave=-1), dict(small_wave=100000), dict(rounds=1, small_wave=-1), dict(rounds=2, small_wave=-1), dict(rounds=6, small_wave=-1), dict(rounds=-1, small_wave=-1),
                                   dict(step_out=1), dict(step_out=2, small_wave=-1), dict(step_out=1, ball_cells=-1), dict(count_alg=1), dict(count_alg=2, small_wave=-1)])
 def test_options_do_not_change_the_result(opts):
     w = inputs.config(2, "small")
@@ -390,7 +390,7 @@ def test_box_domain_wave_mode_and_lloyd():
 def test_support_calls_phase_times_counters_and_pinned_copy():
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
-        ctx.set_options(small_wave=-1, count_alg=1)     # the step kernels also on this replica's small wavefronts; per-query statistics on
+        ctx.set_options(small_wave=-1, count_alg=1, rounds=5)     # the step kernels (rounds of tests / clips too) also on this replica's small wavefronts; per-query statistics on
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         ph, cnt, st = ctx.phase_ms(), ctx.counters(), ctx.stage_ms()
@@ -523,7 +523,7 @@ def test_golden_carved_square_cases_through_the_abi():
 
 @pytest.mark.parametrize("kind,n,opts", [(0, 3000, {}), (0, 3000, dict(persistent=3)), (1, 3000, {}), (1, 3000, dict(persistent=3)),
                                          (2, 2500, {}), (2, 2500, dict(small_wave=-1)), (2, 2500, dict(persistent=3)),
-                                         (2, 2500, dict(small_wave=-1, tail_pairs=-1)), (2, 2500, dict(first_clip=-1, real_edges=0))])
+                                         (2, 2500, dict(small_wave=-1, tail_pairs=-1, rounds=5)), (2, 2500, dict(first_clip=-1, real_edges=0))])
 def test_carved_domain_parity(kind, n, opts):
     """U-shaped domain with a detached island, jittered vertices, sites over the whole bounding box: the simplex seeds and
     the positive flags must reach every piece although cells are cut apart by the notch and the strip (completeness
@@ -638,7 +638,7 @@ def test_counters_per_step_kernel_add_up():
     init (no search) / fix / tail, fan simplices under finish."""
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
-        ctx.set_options(small_wave=-1, count_alg=1)
+        ctx.set_options(small_wave=-1, count_alg=1, rounds=5)     # (rounds: the verify / fix kernels run, not only the finishing kernel)
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         tot, ph = ctx.counters(), ctx.phase_counters()
