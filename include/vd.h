@@ -140,8 +140,9 @@ typedef struct vd_options {
                              structure).  0 (default): fp64 throughout.  Not combined with weighted 3-D sites.              */
   int32_t count_alg;      /* measurement runs.  0 (default): the clip kernels keep no per-query statistics (vd_counters.queries
                              and dist_evals count only the seeds' queries of the mesh vertices; row_evals and search_evals
-                             stay 0: the bookkeeping alone is 3-4 % of a step);
-                             1: those statistics are collected (the "full" kernels run);  2: and D_alg as well
+                             stay 0: the bookkeeping alone is 3-4 % of a step) and no work counters of the clip path (clips,
+                             pre_clips, search_iters, clip_corners, new_corners, fan_simplices stay 0: another 2-4 %);
+                             1: statistics and work counters are collected (the "full" kernels run);  2: and D_alg as well
                              (vd_counters.alg_evals): after every nearest-site query the sites of the grid cells that meet
                              the ball (q, |q - N_q|) -- the least an exact grid search must examine; slower.    */
   int32_t reuse_nbrs;     /* vd_lloyd, whole-cell kinds: 0 / 1 (default): iteration k+1 clips every cell first by the bisectors
@@ -156,9 +157,11 @@ typedef struct vd_options {
   int32_t reserved[2];
 } vd_options;
 
-/* Work counters of the last vd_compute (a few atomics per warp and kernel).  queries, dist_evals, row_evals and search_evals
- * are per-query statistics: collected only with vd_options.count_alg >= 1 (or another option that selects the full kernels:
- * step_out, fp32_filter, weighted 3-D sites); everything else always. */
+/* Work counters of the last vd_compute (a few atomics per warp and kernel).  Per-query statistics (queries, dist_evals, row_evals,
+ * search_evals) and the clip path's work counters (search_iters, clips, pre_clips, clip_corners, new_corners, fan_simplices,
+ * step_probes, f32_survivors) are collected only with vd_options.count_alg >= 1 (or another option that selects the full kernels:
+ * step_out, fp32_filter, weighted 3-D sites) -- the default kernels carry no bookkeeping in their inner loops (it was 3-4 % + 2-4 %
+ * of a step) and leave them 0.  pairs, pieces, waves, overflow_pairs, reruns, launches and syncs are counted always. */
 typedef struct vd_counters {
   int64_t pairs;          /* (simplex, site) pairs processed = Alg. 3 runs          */
   int64_t pieces;         /* non-empty pieces                                                      */

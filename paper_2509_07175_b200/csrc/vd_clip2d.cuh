@@ -42,8 +42,7 @@ __device__ __forceinline__ int apply_clip_2d(Poly2<K>& S, int p, int s, double n
   const int lane = lane_id();
   const int nc = S.nc;
   __syncwarp();
-  extra_cnt_add(0, (unsigned)nc);
-  extra_cnt_add(1, 2u);
+  VD_WORK(extra_cnt_add(0, (unsigned)nc); extra_cnt_add(1, 2u);)
   int rc = 0;
   if (lane == 0) {
     // outside run around p (P:L391's R_p for a loop): corners beyond the line, not known inside
@@ -121,8 +120,7 @@ struct Poly2P {
 __device__ __forceinline__ int apply_clip_2d_par(Poly2P& S, int& nc, int p, int s, double nx, double ny, double nz, double d, int j,
                                                  double pnx, double pny, double pnz) {
   const int lane = lane_id();
-  extra_cnt_add(0, (unsigned)nc);
-  extra_cnt_add(1, 2u);
+  VD_WORK(extra_cnt_add(0, (unsigned)nc); extra_cnt_add(1, 2u);)
   // this lane's corner and edge
   double x = 0, y = 0, z = 0, ex = 0, ey = 0, ez = 0, e_d = 0;
   int fl = 0, nn = 0, stt = 0;
@@ -273,8 +271,7 @@ __device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A
       }
       warp_argmin(far, p);   // the corner farthest beyond the line starts the outside run
       if (p == 0x7fffffff || __any_sync(kFull, own)) { complete = false; continue; }   // the line does not cut P
-      lc.clips += 1;
-      lc.pre_clips += 1;
+      VD_WORK(lc.clips += 1; lc.pre_clips += 1;)
       if (apply_clip_2d_par(S, nc, p, -1, nx, ny, nz, d, j, pnx, pny, pnz)) return 1;
     }
     if (complete && nc > 0) {   // P's edge on B_iu is the discovering edge itself: its two end points are in Omega_i
@@ -340,7 +337,7 @@ __device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A
       __syncwarp();
       continue;
     }
-    lc.clips += 1;
+    VD_WORK(lc.clips += 1;)
     if (apply_clip_2d_par(S, nc, p, s, nx, ny, nz, d, j, pnx, pny, pnz)) return 1;
   }
   // ---- finish
@@ -364,7 +361,7 @@ __device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A
     mz = area * (z0 + (uz + vz) * (1.0 / 3.0));
   }
   area = warp_sum(area); mx = warp_sum(mx); my = warp_sum(my); mz = warp_sum(mz);
-  extra_cnt_add(2, (unsigned)(nc - 2));
+  VD_WORK(extra_cnt_add(2, (unsigned)(nc - 2));)
   if (area < 0) { area = -area; mx = -mx; my = -my; mz = -mz; }
   if (!(area > 0)) {
     if (lane == 0) A.pieces[pairIdx] = pc;
@@ -531,8 +528,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
         owned |= (S.eflag[c] == j);
       }
       if (p < 0 || owned) { complete = false; continue; }   // the line does not cut P
-      lc.clips += 1;
-      lc.pre_clips += 1;
+      VD_WORK(lc.clips += 1; lc.pre_clips += 1;)
       if (apply_clip_2d(S, p, -1, nx, ny, nz, d, j, pnx, pny, pnz)) return 1;
     }
     __syncwarp();
@@ -597,7 +593,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
 #ifdef VD_TRACE
     if (lane == 0) printf("pair(%d,%d) clip p=%d s=%d j=%d nc=%d\n", a, i, p, s, j, nc);
 #endif
-    lc.clips += 1;
+    VD_WORK(lc.clips += 1;)
     __syncwarp();
     int rc = apply_clip_2d(S, p, s, nx, ny, nz, d, j, pnx, pny, pnz);
 #ifdef VD_TRACE
@@ -627,7 +623,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     my += ar * (S.cy[0] + (uy + vy) * (1.0 / 3.0));
     mz += ar * (S.cz[0] + (uz + vz) * (1.0 / 3.0));
   }
-  extra_cnt_add(2, (unsigned)(nc - 2));
+  VD_WORK(extra_cnt_add(2, (unsigned)(nc - 2));)
   if (area < 0) { area = -area; mx = -mx; my = -my; mz = -mz; }
   if (!(area > 0)) {
     if (lane == 0) A.pieces[pairIdx] = pc;

@@ -101,8 +101,7 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
     if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
     if (L > P || nc - k + L > C) return 1;
     if (L >= k) {
-      extra_cnt_add(0, (unsigned)nc);
-      extra_cnt_add(1, (unsigned)L);
+      VD_WORK(extra_cnt_add(0, (unsigned)nc); extra_cnt_add(1, (unsigned)L);)
       const int base = __popc(b0 & lt) + 2 * __popc(b1 & lt);
       if (lane == 0) { S.pnx[N] = nx; S.pny[N] = ny; S.pnz[N] = nz; S.pd[N] = d; S.pflag[N] = j; }
       if (rem) S.remap[__popc(R & lt)] = (unsigned short)c;   // slot list: the e-th new corner takes the e-th removed slot
@@ -233,8 +232,7 @@ __device__ int apply_clip_3d(Poly3<P, C>& S, int& np, int& nc, int p, int s, dou
   const int nSurv = nc - nRemoved;
   if (L == 0) { nc = 0; np = N + 1; return 0; }   // nothing of P is left
   if (nSurv + L > C) return 1;
-  extra_cnt_add(0, (unsigned)nc);
-  extra_cnt_add(1, (unsigned)L);
+  VD_WORK(extra_cnt_add(0, (unsigned)nc); extra_cnt_add(1, (unsigned)L);)
   // (2b) where the new corners are: rim edge (a -> b) gives the corner (a, b, N), the solution of its three planes;
   // one lane per rim edge, while the removed corners are still in place for the fallback
   for (int e = lane; e < L; e += kLanes) {
@@ -438,7 +436,7 @@ __device__ int finish_piece_3d(Poly3<P, C>& S, const ClipArgs& A, int64_t pairId
     nnbr += __popc(pm);
   }
   vol = warp_sum(vol); mx = warp_sum(mx); my = warp_sum(my); mz = warp_sum(mz);
-  extra_cnt_add(2, (unsigned)(3 * nc - 2 * nlive));   // fan tetrahedra: every face of k corners gives k - 2; corners lie on 3 faces
+  VD_WORK(extra_cnt_add(2, (unsigned)(3 * nc - 2 * nlive));)   // fan tetrahedra: every face of k corners gives k - 2; corners lie on 3 faces
   if (vol < 0) { vol = -vol; mx = -mx; my = -my; mz = -mz; }
   if (!(vol > 0)) {
 #ifdef VD_TRACE
@@ -653,8 +651,7 @@ __device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A
     compact_planes_3d(S, np, nc);
     if (np >= P) return 1;
   }
-  lc.clips += 1;
-  lc.pre_clips += 1;
+  VD_WORK(lc.clips += 1; lc.pre_clips += 1;)
   return apply_clip_3d(S, np, nc, p, -1, nx, ny, nz, d, j);
 }
 
@@ -821,7 +818,7 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
 #ifdef VD_TRACE
   if (lane == 0) printf("pair(?,%d) clip p=%d(%g,%g,%g) s=%d j=%d nc=%d np=%d\n", i, p, S.cx[p]+ox, S.cy[p]+oy, S.cz[p]+oz, s, j, nc, np);
 #endif
-  lc.clips += 1;
+  VD_WORK(lc.clips += 1;)
   return apply_clip_3d(S, np, nc, p, s, nx, ny, nz, d, j);
 }
 

@@ -477,9 +477,9 @@ __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex&
     r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out, nullptr, st, iters);
     nx = __shfl_sync(kFull, out[0], 0); ny = __shfl_sync(kFull, out[1], 0); nz = __shfl_sync(kFull, out[2], 0); d = __shfl_sync(kFull, out[3], 0);
   }
-  lc.search_iters += iters;
+  VD_WORK(lc.search_iters += iters;)
   __syncwarp();
-  lc.search_evals += warp_stats().dist_evals - e0;
+  VD_WORK(lc.search_evals += warp_stats().dist_evals - e0;)
   return r;
 }
 

@@ -31,6 +31,14 @@ __device__ __forceinline__ WarpStats& warp_stats() { return sWarpStats[(threadId
 #else
 #define VD_STAT(x) { if (lane_id() == 0) { WarpStats& st = warp_stats(); x } }
 #endif
+// Work counters of the clip path (clips, first clips, search iterations, corners tested / created, fan simplices): also the full
+// kernels' only -- the by-reference LocalCnt fields live in local memory and each update waits for its own load (measured: ~4 % of
+// the stall samples of k_ph_tail on C2).  pairs / pieces stay in every build.
+#if !VD_EXT
+#define VD_WORK(x)
+#else
+#define VD_WORK(x) x
+#endif
 
 __device__ __forceinline__ void extra_cnt_reset() {
   if (lane_id() < kExtraCnt) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][lane_id()] = 0u;

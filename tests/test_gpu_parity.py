@@ -407,6 +407,7 @@ def test_support_calls_phase_times_counters_and_pinned_copy():
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
     wb = inputs.box(3, 2000, seed=1)
     with binding.Context(wb.sites) as ctx:
+        ctx.set_options(count_alg=1)           # (work counters are the counting kernels')
         ctx.set_domain(wb.verts, None, wb.kind)
         ctx.compute()
         cnt = ctx.counters()
@@ -491,11 +492,13 @@ def test_one_simplex_many_cells(kind):
         simp = np.array([[0, 1, 2]], np.int32)
         sites = rng.random((4000, 2)) * 1.2 - 0.1
         w = inputs.custom(inputs.KIND_TRI_2D, sites, verts, simp, "one_tri")
-    g, cnt, _ = _gpu(w)
+    g, cnt, _ = _gpu(w, count_alg=1)           # (pre_clips is a work counter: the counting kernels')
     o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
     parity.assert_parity(g, o, w.diameter)
     assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
     assert cnt["waves"] >= 1 and cnt["pre_clips"] > 0
+    g2, cnt2, _ = _gpu(w)                      # the default kernels: the same cells, no work counters
+    assert np.array_equal(g2.vert_flags, g.vert_flags) and np.array_equal(g2.nbr, g.nbr) and cnt2["pre_clips"] == 0 and cnt2["pieces"] == cnt["pieces"]
     if kind == "tet":      # the case this test is for does occur: some finished piece has a face of more than 8 edges
         nedges = []
         for p in range(len(g.piece_simplex)):
@@ -642,13 +645,14 @@ def test_counters_per_step_kernel_add_up():
         ctx.set_domain(w.verts, w.simplices, w.kind)
         ctx.compute()
         tot, ph = ctx.counters(), ctx.phase_counters()
-        ctx.set_options(small_wave=-1)              # the default kernels keep no per-query statistics; everything else is counted
+        ctx.set_options(small_wave=-1)              # the default kernels keep neither per-query statistics nor work counters; pairs and pieces are counted
         ctx.compute()
         lean = ctx.counters()
     assert lean["queries"] <= len(w.verts) + 8 and lean["row_evals"] == 0          # (the seeds' queries of the mesh vertices are always counted)
-    for f in ("pairs", "pieces", "fan_simplices"):      # (clips / pre_clips depend on which neighbour discovers a pair first)
+    for f in ("pairs", "pieces"):
         assert lean[f] == tot[f], f
-    assert lean["clips"] > 0 and lean["pre_clips"] > 0
+    for f in ("clips", "pre_clips", "search_iters", "clip_corners", "new_corners", "fan_simplices"):
+        assert lean[f] == 0 and tot[f] > 0, f
     for f in ("pairs", "pieces", "queries", "dist_evals", "search_iters", "clips", "clip_corners", "new_corners", "fan_simplices"):
         assert sum(ph[k][f] for k in ph) == tot[f], f
     assert ph["verify"]["queries"] > 0 and ph["verify"]["clips"] == 0 and ph["verify"]["search_iters"] == 0
