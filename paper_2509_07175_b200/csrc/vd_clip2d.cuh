@@ -112,7 +112,7 @@ struct Poly2P {
   unsigned char cstate[kLanes];
   int k0[kLanes], k1[kLanes];                           // finish: the ascending flag pair of a corner
   double u[14];                                          // per-pair constants (as Poly2::u)
-  double scratch[(sizeof(QBatch) + 40 + 7) / 8];        // the batch of queries; the search's scratch
+  double scratch[(kSearchScratchBytes + 7) / 8];         // the batch of queries; the search's frame
 };
 
 // P <- P clipped by the line (n, d) with flag j from the outside corner p (s: the known-inside neighbour of p on a searched real

@@ -26,7 +26,7 @@ struct alignas(16) Poly3 {
   double pnx[P], pny[P], pnz[P], pd[P];   // plane f: n.x <= d, coordinates local to the tet's corner 0
   unsigned short cp[C][3];                // the corner's three planes, cyclically ordered
   unsigned short cadj[C][3];              // corner across the polytope edge (cp[t], cp[t+1])
-  int key[C + 8][3];                      // scratch from here on (sized for the query batch: static_assert in classify_unknown_3d): flag triple of a corner (output order); rim points during a clip
+  int key[C + 16][3];                     // scratch from here on (sized for the query batch: static_assert in classify_unknown_3d): flag triple of a corner (output order); rim points during a clip
   unsigned short remap[C];                // index of a surviving corner after the clip
   unsigned short pa[P], pb[P];            // new corner whose rim edge starts / ends at a plane
   unsigned short be[P][4];                // rim edges of R_p: (a, b, inside neighbour, flags)
@@ -43,7 +43,7 @@ struct alignas(16) PolyTest3 {
   double cx[C], cy[C], cz[C];
   unsigned char cstate[C];
   int cnn[C];
-  int key[(sizeof(QBatch) + 40 + 11) / 12 + 1][3];   // scratch: the batch of queries
+  int key[(sizeof(QBatch) + 40 + 11) / 12 + 1][3];   // scratch: the batch of queries (k_ph_verify searches nothing: no frame)
 };
 
 // returns false when the three planes are (numerically) parallel to a common line
@@ -739,7 +739,7 @@ template <class PolyT, bool HV, bool DEFER = false>
 __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st, bool* deferred = nullptr) {
   const int lane = lane_id();
   VD_POLY_REFS;
-  static_assert(sizeof(QBatch) + 40 <= sizeof(S.key), "the batch state (and a plane behind it) must fit the scratch area");
+  static_assert(sizeof(QBatch) + 40 <= sizeof(S.key), "the batch state must fit the scratch area");
   QBatch& Q = *reinterpret_cast<QBatch*>(&S.key[0][0]);
   bool any = false;
   for (;;) {
@@ -801,6 +801,7 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
     compact_planes_3d(S, np, nc);
     if (np >= P) return 1;
   }
+  static_assert(kSearchScratchBytes <= (int)sizeof(S.key), "the batch state and the search frame must fit the scratch area");
   double psx = wx, psy = wy, psz = wz;
   if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
   double nx, ny, nz, d;

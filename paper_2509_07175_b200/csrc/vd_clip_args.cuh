@@ -366,61 +366,78 @@ static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, c
 // the segment lies in P, and P is inside H_ik for every site k that owns one of them, so N_q = v_k can
 // only be a tie and also means q in Omega_i -- the flag rule of P:L109-111 for a point on an edge/face of P
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
+// The state of one search (warp-uniform): it lives in the warp's shared-memory scratch behind the batch of queries, NOT in
+// registers -- the doubles that the loop carries across its calls of the (not inlined) query routines were the largest
+// source of spill loads / stores of the step kernels.  Every lane writes the same values and reads back what it wrote.
+struct SearchFrame {
+  double plane[4];        // out: the bisector (n, d) of the site returned
+  double ps[3], pt[3];    // the segment, local to o
+  double q[3];            // the intersecting point of the current iteration
+  double di2, dj2;
+  unsigned iters, pad;
+};
+constexpr int kSearchScratchBytes = ((int)sizeof(QBatch) + 7) / 8 * 8 + (int)sizeof(SearchFrame);
+
 template <bool HV, bool DEFER = false>
 // DEFER (refined index, fast pass): a query that needs the single-query path ends the search with -2, nothing changed.
 // The arguments are scalars and pointers on purpose: a struct passed by reference to this (not inlined) function
-// would be copied into every thread's local memory, and so would by-reference results -- the plane comes back
-// through out4 (the caller's shared-memory scratch, or a local array), the iteration count as the return's pair.
+// would be copied into every thread's local memory.  The segment comes in and the plane goes out through the frame.
 static __device__ __noinline__ int find_bisector_impl(const double* __restrict__ sites, int ballCells, const GridIndex& g, int i, int j,
                                              const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
-                                             double psx, double psy, double psz, double ptx, double pty, double ptz, const int* flags, int nflags,
-                                             double* out4, QBatch* qb, QueryStats& st, unsigned& iters) {
+                                             SearchFrame* sf, const int* flags, int nflags, QBatch* qb, QueryStats& st) {
   const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
-  double nx, ny, nz, d;
   if (has_step_out(g)) {   // section VI-A (vd_options.step_out): shorten the segment first
-    double pt[3] = {ptx, pty, ptz};
-    const int probes = step_out<HV>(g, i, j, u, psx, psy, psz, pt, flags, nflags, st);
-    if (probes) { ptx = pt[0]; pty = pt[1]; ptz = pt[2]; extra_cnt_add(3, (unsigned)probes); }
+    double pt[3] = {sf->pt[0], sf->pt[1], sf->pt[2]};
+    const int probes = step_out<HV>(g, i, j, u, sf->ps[0], sf->ps[1], sf->ps[2], pt, flags, nflags, st);
+    if (probes) { sf->pt[0] = pt[0]; sf->pt[1] = pt[1]; sf->pt[2] = pt[2]; extra_cnt_add(3, (unsigned)probes); }
   }
   for (int it = 0; it < 96; ++it) {
-    iters += 1;
-    const double vjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
-                 vjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
-    const double wi = u[12], wj = site_w(g, j);   // power diagram: the lifted sites' fourth coordinates, squared (else 0)
-    nx = vjx - vix; ny = vjy - viy; nz = vjz - viz;
-    d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz) + (wj - wi));
-    const double gs = d - (nx * psx + ny * psy + nz * psz);
-    const double gt = d - (nx * ptx + ny * pty + nz * ptz);
-    const double den = gs - gt;
-    double t = den > 0.0 ? gs / den : 1.0;
-    t = fmin(fmax(t, 0.0), 1.0);
-    const double qx = psx + t * (ptx - psx), qy = psy + t * (pty - psy), qz = psz + t * (ptz - psz);
-    // point-in-cell test of the intersecting point: N_q in {i, j} means q is in Omega_i
-    const double ax = qx + ox, ay = qy + oy, az = qz + oz;
-    const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
-    const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
-    const double di2 = dix * dix + diy * diy + diz * diz + wi, dj2 = djx * djx + djy * djy + djz * djz + wj;
-    if ((!HV || VD_ONE_SHOT_HV) && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
-      // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
-      double tb = 2.0;
-      int jb = 0x7fffffff;
-      const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
-      if (scan_ball_min_t<HV>(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz + wi, t, i, j, flags, nflags,
-                          ballCells, tb, jb, st)) {
-        if (jb != 0x7fffffff) {
-          j = jb;
-          const double wjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
-                       wjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
-          nx = wjx - vix; ny = wjy - viy; nz = wjz - viz;
-          d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (site_w(g, j) - wi));
+    double ax, ay, az;
+    {
+      const double psx = sf->ps[0], psy = sf->ps[1], psz = sf->ps[2], ptx = sf->pt[0], pty = sf->pt[1], ptz = sf->pt[2];
+      const double vjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, vjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
+                   vjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
+      const double wi = u[12], wj = site_w(g, j);   // power diagram: the lifted sites' fourth coordinates, squared (else 0)
+      const double nx = vjx - vix, ny = vjy - viy, nz = vjz - viz;
+      const double d = 0.5 * (nx * (vix + vjx) + ny * (viy + vjy) + nz * (viz + vjz) + (wj - wi));
+      const double gs = d - (nx * psx + ny * psy + nz * psz);
+      const double gt = d - (nx * ptx + ny * pty + nz * ptz);
+      const double den = gs - gt;
+      double t = den > 0.0 ? gs / den : 1.0;
+      t = fmin(fmax(t, 0.0), 1.0);
+      const double qx = psx + t * (ptx - psx), qy = psy + t * (pty - psy), qz = psz + t * (ptz - psz);
+      // point-in-cell test of the intersecting point: N_q in {i, j} means q is in Omega_i
+      ax = qx + ox; ay = qy + oy; az = qz + oz;
+      const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
+      const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
+      const double di2 = dix * dix + diy * diy + diz * diz + wi, dj2 = djx * djx + djy * djy + djz * djz + wj;
+      sf->plane[0] = nx; sf->plane[1] = ny; sf->plane[2] = nz; sf->plane[3] = d;
+      sf->q[0] = qx; sf->q[1] = qy; sf->q[2] = qz;
+      sf->di2 = di2; sf->dj2 = dj2;
+      sf->iters = (unsigned)(it + 1);
+      if ((!HV || VD_ONE_SHOT_HV) && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
+        // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
+        double tb = 2.0;
+        int jb = 0x7fffffff;
+        const double sx = psx + ox - u[3], sy = psy + oy - u[4], sz = psz + oz - u[5];
+        if (scan_ball_min_t<HV>(g, ax, ay, az, di2, psx + ox, psy + oy, psz + oz, sx * sx + sy * sy + sz * sz + wi, t, i, j, flags, nflags,
+                            ballCells, tb, jb, st)) {
+          if (jb != 0x7fffffff) {
+            j = jb;
+            const double wjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
+                         wjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
+            const double mx = wjx - vix, my = wjy - viy, mz = wjz - viz;
+            sf->plane[0] = mx; sf->plane[1] = my; sf->plane[2] = mz;
+            sf->plane[3] = 0.5 * (mx * (vix + wjx) + my * (viy + wjy) + mz * (viz + wjz) + (site_w(g, j) - u[12]));
+          }
+          return j;
         }
-        goto found;
+        ax = sf->q[0] + ox; ay = sf->q[1] + oy; az = sf->q[2] + oz;   // (the same sums again, not kept across the call)
       }
     }
-    {
-    double best = di2;
+    double best = sf->di2;
     int bestId = i;
-    if (closer(dj2, j, best, bestId)) { best = dj2; bestId = j; }
+    if (closer(sf->dj2, j, best, bestId)) { best = sf->dj2; bestId = j; }
     if (HV && qb && VD_SEARCH_BATCH) {
       // refined index: the query as a batch of one -- the cell-by-cell pass over sub-grids (vd_batch.cuh) instead of the
       // general single-query search
@@ -434,52 +451,50 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
     } else {
       nearest<HV>(g, ax, ay, az, best, bestId, st, true);
     }
-#ifdef VD_TRACE
-    if (lane_id() == 0) printf("      search i=%d j=%d t=%.17g q=(%g,%g) gs=%g gt=%g -> N_q=%d\n", i, j, t, ax, ay, gs, gt, bestId);
-#endif
-    const double bound = fmin(di2, dj2);
-    if (bestId == i || bestId == j || best >= bound * (1.0 - 1e-13)) goto found;   // nothing nearer, up to rounding
+    const double bound = fmin(sf->di2, sf->dj2);
+    if (bestId == i || bestId == j || best >= bound * (1.0 - 1e-13)) return j;   // nothing nearer, up to rounding
     if (best >= bound * (1.0 - 1e-9)) {   // a (near) tie with a site that owns a plane of P: flag rule
       bool own = false;
       for (int f = lane_id(); f < nflags; f += kLanes) own |= (flags[f] == bestId);
-      if (__any_sync(kFull, own)) goto found;
+      if (__any_sync(kFull, own)) return j;
     }
     j = bestId;
-    ptx = qx; pty = qy; ptz = qz;
-    }
+    sf->pt[0] = sf->q[0]; sf->pt[1] = sf->q[1]; sf->pt[2] = sf->q[2];
   }
   return -1;
-found:
-  if (lane_id() == 0) { out4[0] = nx; out4[1] = ny; out4[2] = nz; out4[3] = d; }
-  __syncwarp();
-  return j;
 }
 
-// scratch4: four doubles of the warp's shared-memory scratch (3D kinds); nullptr: a local array
+// scratch: the warp's shared-memory scratch (kSearchScratchBytes: the batch of queries, then the search frame); nullptr (the
+// large 2D tier): a frame in local memory
 template <bool HV, bool DEFER = false>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
-                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch4 = nullptr) {
+                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch = nullptr) {
   __syncwarp();
   const unsigned e0 = warp_stats().dist_evals;
-  unsigned iters = 0;
   int r;
-  if (scratch4) {
-    // the scratch area holds the batch state of the point-in-cell tests; the plane comes back through its last 32 bytes
-    QBatch* qb = reinterpret_cast<QBatch*>(scratch4);
-    double* out4 = scratch4 + (sizeof(QBatch) + 7) / 8;
-    r = find_bisector_impl<HV, DEFER>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out4, qb, st, iters);
-    scratch4 = out4;
-    nx = scratch4[0]; ny = scratch4[1]; nz = scratch4[2]; d = scratch4[3];
+  unsigned iters;
+  if (scratch) {
+    QBatch* qb = reinterpret_cast<QBatch*>(scratch);
+    SearchFrame* sf = reinterpret_cast<SearchFrame*>(scratch + (sizeof(QBatch) + 7) / 8);
+    sf->ps[0] = psx; sf->ps[1] = psy; sf->ps[2] = psz; sf->pt[0] = ptx; sf->pt[1] = pty; sf->pt[2] = ptz;
+    sf->iters = 0u;
+    r = find_bisector_impl<HV, DEFER>(A.sites, A.ballCells, g, i, j, u, sf, flags, nflags, qb, st);
+    nx = sf->plane[0]; ny = sf->plane[1]; nz = sf->plane[2]; d = sf->plane[3];
+    iters = sf->iters;
   } else {
-    // every lane writes its own copy
-    double out[4] = {0, 0, 0, 0};
-    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, psx, psy, psz, ptx, pty, ptz, flags, nflags, out, nullptr, st, iters);
-    nx = __shfl_sync(kFull, out[0], 0); ny = __shfl_sync(kFull, out[1], 0); nz = __shfl_sync(kFull, out[2], 0); d = __shfl_sync(kFull, out[3], 0);
+    SearchFrame f;   // every lane its own copy
+    f.ps[0] = psx; f.ps[1] = psy; f.ps[2] = psz; f.pt[0] = ptx; f.pt[1] = pty; f.pt[2] = ptz;
+    f.iters = 0u;
+    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, &f, flags, nflags, nullptr, st);
+    nx = f.plane[0]; ny = f.plane[1]; nz = f.plane[2]; d = f.plane[3];
+    iters = f.iters;
   }
   VD_WORK(lc.search_iters += iters;)
+  (void)iters;
   __syncwarp();
   VD_WORK(lc.search_evals += warp_stats().dist_evals - e0;)
+  (void)e0;
   return r;
 }
 
