@@ -21,6 +21,7 @@ struct Poly2 {
   unsigned char tstate[K];
   double u[14];   // per-pair constants: origin, v_i absolute, v_i local, witness local, [12] = 0 (the additive term of 3-D power diagrams)
   int nc;
+  double scratch[(kSearchScratchBytes + 7) / 8];   // the search's batch of one and its frame
 };
 
 // fallback position of a new corner (ill-conditioned planes): where the edge from the removed corner c to
@@ -580,7 +581,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
     if (s >= 0) { psx = S.cx[s]; psy = S.cy[s]; psz = S.cz[s]; }
     double nx, ny, nz, d;
     const int j = find_bisector<HV>(A, g, i, S.cnn[p], S.u, psx, psy, psz, S.cx[p], S.cy[p], S.cz[p], S.eflag, nc,
-                                nx, ny, nz, d, st, lc);
+                                nx, ny, nz, d, st, lc, S.scratch);
     if (j < 0) { failed = true; atomicOr(&A.ctl->err, ERR_NOCONVERGE); break; }
     bool own = false;
     for (int c = 0; c < nc; ++c) own |= (S.eflag[c] == j);

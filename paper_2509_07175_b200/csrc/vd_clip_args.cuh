@@ -368,7 +368,8 @@ static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, c
 // (a real edge, or a virtual edge that runs inside a bisector face).  Returns j, or -1 at the cap.
 // The state of one search (warp-uniform): it lives in the warp's shared-memory scratch behind the batch of queries, NOT in
 // registers -- the doubles that the loop carries across its calls of the (not inlined) query routines were the largest
-// source of spill loads / stores of the step kernels.  Every lane writes the same values and reads back what it wrote.
+// source of spill loads / stores of the step kernels.  Lane 0 writes, the warp synchronises before anyone reads and again
+// before the next write (the lanes of a warp need not be in step after a call).
 struct SearchFrame {
   double plane[4];        // out: the bisector (n, d) of the site returned
   double ps[3], pt[3];    // the segment, local to o
@@ -389,7 +390,9 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
   if (has_step_out(g)) {   // section VI-A (vd_options.step_out): shorten the segment first
     double pt[3] = {sf->pt[0], sf->pt[1], sf->pt[2]};
     const int probes = step_out<HV>(g, i, j, u, sf->ps[0], sf->ps[1], sf->ps[2], pt, flags, nflags, st);
-    if (probes) { sf->pt[0] = pt[0]; sf->pt[1] = pt[1]; sf->pt[2] = pt[2]; extra_cnt_add(3, (unsigned)probes); }
+    __syncwarp();
+    if (probes) { if (lane_id() == 0) { sf->pt[0] = pt[0]; sf->pt[1] = pt[1]; sf->pt[2] = pt[2]; } extra_cnt_add(3, (unsigned)probes); }
+    __syncwarp();
   }
   for (int it = 0; it < 96; ++it) {
     double ax, ay, az;
@@ -411,10 +414,14 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
       const double dix = ax - u[3], diy = ay - u[4], diz = az - u[5];
       const double djx = ax - (vjx + ox), djy = ay - (vjy + oy), djz = az - (vjz + oz);
       const double di2 = dix * dix + diy * diy + diz * diz + wi, dj2 = djx * djx + djy * djy + djz * djz + wj;
-      sf->plane[0] = nx; sf->plane[1] = ny; sf->plane[2] = nz; sf->plane[3] = d;
-      sf->q[0] = qx; sf->q[1] = qy; sf->q[2] = qz;
-      sf->di2 = di2; sf->dj2 = dj2;
-      sf->iters = (unsigned)(it + 1);
+      __syncwarp();   // every lane has read the segment (and, in the previous iteration, q and the bounds)
+      if (lane_id() == 0) {
+        sf->plane[0] = nx; sf->plane[1] = ny; sf->plane[2] = nz; sf->plane[3] = d;
+        sf->q[0] = qx; sf->q[1] = qy; sf->q[2] = qz;
+        sf->di2 = di2; sf->dj2 = dj2;
+        sf->iters = (unsigned)(it + 1);
+      }
+      __syncwarp();
       if ((!HV || VD_ONE_SHOT_HV) && ballCells > 0) {   // (on the refined index the one-shot scan measured slower: C3 583 -> 632 ms)
         // close enough to Omega_i for a complete scan of the ball: the site whose bisector crosses first ends the search
         double tb = 2.0;
@@ -427,9 +434,11 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
             const double wjx = __ldg(&sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&sites[(int64_t)j * 3 + 1]) - oy,
                          wjz = __ldg(&sites[(int64_t)j * 3 + 2]) - oz;
             const double mx = wjx - vix, my = wjy - viy, mz = wjz - viz;
-            sf->plane[0] = mx; sf->plane[1] = my; sf->plane[2] = mz;
-            sf->plane[3] = 0.5 * (mx * (vix + wjx) + my * (viy + wjy) + mz * (viz + wjz) + (site_w(g, j) - u[12]));
+            const double md = 0.5 * (mx * (vix + wjx) + my * (viy + wjy) + mz * (viz + wjz) + (site_w(g, j) - u[12]));
+            __syncwarp();
+            if (lane_id() == 0) { sf->plane[0] = mx; sf->plane[1] = my; sf->plane[2] = mz; sf->plane[3] = md; }
           }
+          __syncwarp();
           return j;
         }
         ax = sf->q[0] + ox; ay = sf->q[1] + oy; az = sf->q[2] + oz;   // (the same sums again, not kept across the call)
@@ -459,37 +468,31 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
       if (__any_sync(kFull, own)) return j;
     }
     j = bestId;
-    sf->pt[0] = sf->q[0]; sf->pt[1] = sf->q[1]; sf->pt[2] = sf->q[2];
+    __syncwarp();   // the bounds have been read by every lane
+    if (lane_id() == 0) { sf->pt[0] = sf->q[0]; sf->pt[1] = sf->q[1]; sf->pt[2] = sf->q[2]; }
+    __syncwarp();
   }
   return -1;
 }
 
-// scratch: the warp's shared-memory scratch (kSearchScratchBytes: the batch of queries, then the search frame); nullptr (the
-// large 2D tier): a frame in local memory
+// scratch: the warp's shared-memory scratch (kSearchScratchBytes: the batch of queries, then the search frame)
 template <bool HV, bool DEFER = false>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
-                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch = nullptr) {
-  __syncwarp();
+                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch) {
   const unsigned e0 = warp_stats().dist_evals;
-  int r;
-  unsigned iters;
-  if (scratch) {
-    QBatch* qb = reinterpret_cast<QBatch*>(scratch);
-    SearchFrame* sf = reinterpret_cast<SearchFrame*>(scratch + (sizeof(QBatch) + 7) / 8);
+  QBatch* qb = reinterpret_cast<QBatch*>(scratch);
+  SearchFrame* sf = reinterpret_cast<SearchFrame*>(scratch + (sizeof(QBatch) + 7) / 8);
+  __syncwarp();
+  if (lane_id() == 0) {
     sf->ps[0] = psx; sf->ps[1] = psy; sf->ps[2] = psz; sf->pt[0] = ptx; sf->pt[1] = pty; sf->pt[2] = ptz;
     sf->iters = 0u;
-    r = find_bisector_impl<HV, DEFER>(A.sites, A.ballCells, g, i, j, u, sf, flags, nflags, qb, st);
-    nx = sf->plane[0]; ny = sf->plane[1]; nz = sf->plane[2]; d = sf->plane[3];
-    iters = sf->iters;
-  } else {
-    SearchFrame f;   // every lane its own copy
-    f.ps[0] = psx; f.ps[1] = psy; f.ps[2] = psz; f.pt[0] = ptx; f.pt[1] = pty; f.pt[2] = ptz;
-    f.iters = 0u;
-    r = find_bisector_impl<HV>(A.sites, A.ballCells, g, i, j, u, &f, flags, nflags, nullptr, st);
-    nx = f.plane[0]; ny = f.plane[1]; nz = f.plane[2]; d = f.plane[3];
-    iters = f.iters;
   }
+  __syncwarp();
+  const int r = find_bisector_impl<HV, DEFER>(A.sites, A.ballCells, g, i, j, u, sf, flags, nflags, qb, st);
+  __syncwarp();
+  nx = sf->plane[0]; ny = sf->plane[1]; nz = sf->plane[2]; d = sf->plane[3];
+  const unsigned iters = sf->iters;
   VD_WORK(lc.search_iters += iters;)
   (void)iters;
   __syncwarp();
