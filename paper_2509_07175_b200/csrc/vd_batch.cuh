@@ -34,7 +34,7 @@ struct QBatch {
 // query is flagged (B.flag) and that row is visited cell by cell afterwards.  A query whose ball spans more than
 // kQBMaxRows rows of g does not take part: it is returned in the mask of loose queries.
 template <bool SKIP_REFINED>
-static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B, int nq, unsigned active, QueryStats& st) {
+static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B, int nq, unsigned active, StRef st) {
   const int lane = lane_id();
   int myRows = 0;
   bool loose = false;
@@ -144,7 +144,7 @@ static __device__ __noinline__ unsigned batch_pass(const GridIndex& g, QBatch& B
 // the expanding-shell search is a third of their instructions and half of their executed code, and they are bound by
 // instruction fetch -- and a second pass of the same kernels (with the fallback) takes what the fast pass left.
 template <bool HV, bool FALLBACK = true>
-static __device__ __noinline__ unsigned batch_nearest(const GridIndex& gTop, QBatch& B, int nq, QueryStats& st) {
+static __device__ __noinline__ unsigned batch_nearest(const GridIndex& gTop, QBatch& B, int nq, StRef st) {
   const int lane = lane_id();
   if (lane < kQB) B.flag[lane] = 0;
   __syncwarp();

@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ l
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   for (int64_t i = (int64_t)blockIdx.x * kWarpsPerBlock + w; i < A.n; i += (int64_t)gridDim.x * kWarpsPerBlock) {
     const int k = near_sites(g, A.sites[i * 3 + 0], A.sites[i * 3 + 1], A.sites[i * 3 + 2], (int)i, K, ids[w], st);
     if (lane < K) list[i * K + lane] = lane < k ? ids[w][lane] : -1;
@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : ((KIND == KIN
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes;
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   constexpr bool BOX = KIND == KIND_BOX_2D || KIND == KIND_BOX_3D;

@@ -182,7 +182,7 @@ __device__ __forceinline__ int apply_clip_2d_par(Poly2P& S, int& nc, int p, int 
 // One (triangle, site) pair on the lane-per-corner structure: Alg. 3 / Alg. 1 as in clip_pair_2d below, step for step.
 // Returns 0 = done, 1 = the polygon outgrew 32 corners (the caller defers the pair to the large tier).
 template <bool HV, bool BOX>
-__device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+__device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, StRef st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
@@ -425,7 +425,7 @@ __device__ int clip_pair_2d_par(Poly2P& S, const GridIndex& g, const ClipArgs& A
 }
 
 template <int K, bool HV, bool BOX>
-__device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+__device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, StRef st, LocalCnt& lc) {
   const int lane = lane_id();
   const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
@@ -496,7 +496,7 @@ __device__ int clip_pair_2d(Poly2<K>& S, const GridIndex& g, const ClipArgs& A, 
   bool failed = false;
 #ifdef VD_TRACE
   {
-    double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0u, 0u, 0u};
+    double b = 2e300; int bi = 0x7fffffff; QueryStats s2 = {0};
     nearest<HV>(g, pr.wx, pr.wy, pr.wz, b, bi, s2);
     const double dx = pr.wx - six, dy = pr.wy - siy, dz = pr.wz - siz;
     const double di = dx * dx + dy * dy + dz * dz;

@@ -736,7 +736,7 @@ __device__ __forceinline__ int select_out_3d(const Poly3<P, C>& S, const ClipArg
 // DEFER (refined index, fast pass): corners whose test needs the single-query path are marked ST_LOOSE and left alone;
 // *deferred tells whether there were any.  Without DEFER such marks count as unclassified.
 template <class PolyT, bool HV, bool DEFER = false>
-__device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, QueryStats& st, bool* deferred = nullptr) {
+__device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g, int i, int np, int nc, StRef st, bool* deferred = nullptr) {
   const int lane = lane_id();
   VD_POLY_REFS;
   static_assert(sizeof(QBatch) + 40 <= sizeof(S.key), "the batch state must fit the scratch area");
@@ -794,7 +794,7 @@ __device__ __forceinline__ bool classify_unknown_3d(PolyT& S, const GridIndex& g
 // Returns 0 ok, 1 capacity, 2 topology, 3 search cap, 4 (DEFER only) the search needs the single-query path: nothing changed.
 template <int P, int C, bool HV, bool DEFER = false>
 __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int i, int p, int s, int& np,
-                                            int& nc, QueryStats& st, LocalCnt& lc) {
+                                            int& nc, StRef st, LocalCnt& lc) {
   const int lane = lane_id();
   VD_POLY_REFS;
   if (np >= P) {
@@ -825,7 +825,7 @@ __device__ __forceinline__ int clip_from_3d(Poly3<P, C>& S, const GridIndex& g, 
 
 // returns 0 = done (piece or empty recorded), 1 = capacity exceeded (caller defers the pair)
 template <int P, int C, bool HV, bool BOX>
-__device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, QueryStats& st, LocalCnt& lc) {
+__device__ int clip_pair_3d(Poly3<P, C>& S, const GridIndex& g, const ClipArgs& A, int64_t pairIdx, StRef st, LocalCnt& lc) {
   const Pair pr = load_pair(A, pairIdx);
   const int a = pr.a, i = pr.i;
   int np, nc;

@@ -193,7 +193,7 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
 // nearest few sites are almost always Voronoi neighbours, so clipping the box by them first costs no search and
 // leaves a small polytope whose corners are all close to the cell.  Selection is approximate on purpose: each
 // lane keeps the nearest of the candidates it saw, the k best lanes win.
-static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, double vy, double vz, int i, int k, int* out, QueryStats& st) {
+static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, double vy, double vz, int i, int k, int* out, StRef st) {
   __shared__ int sBaseN[kWarpsPerBlock][kLanes];
   const int lane = lane_id();
   int* base = sBaseN[(threadIdx.x / kLanes) % kWarpsPerBlock];
@@ -248,7 +248,7 @@ static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, dou
 template <bool HV>
 static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, double qx, double qy, double qz, double r2, double psx,
                                                     double psy, double psz, double dis2, double tq, int i, int j, const int* flags,
-                                                    int nflags, int maxCells, double& tbest, int& jbest, QueryStats& st) {
+                                                    int nflags, int maxCells, double& tbest, int& jbest, StRef st) {
   __shared__ int sBaseT[kWarpsPerBlock][kLanes];
   const int lane = lane_id();
   int* base = sBaseT[(threadIdx.x / kLanes) % kWarpsPerBlock];
@@ -331,7 +331,7 @@ static __device__ __noinline__ bool scan_ball_min_t(const GridIndex& gTop, doubl
 // local to o = u[0..2]; the new end point and its site come back through pt[3] / j.  Returns the number of probes.
 template <bool HV>
 static __device__ __noinline__ int step_out(const GridIndex& g, int i, int& j, const double* u, double psx, double psy, double psz, double* pt,
-                                            const int* flags, int nflags, QueryStats& st) {
+                                            const int* flags, int nflags, StRef st) {
   const double delta = __ldg(&g.delta[i]);
   const double sx = pt[0] - psx, sy = pt[1] - psy, sz = pt[2] - psz;
   const double len = sqrt(sx * sx + sy * sy + sz * sz);
@@ -385,7 +385,7 @@ template <bool HV, bool DEFER = false>
 // would be copied into every thread's local memory.  The segment comes in and the plane goes out through the frame.
 static __device__ __noinline__ int find_bisector_impl(const double* __restrict__ sites, int ballCells, const GridIndex& g, int i, int j,
                                              const double* u,   // per-pair constants (shared memory): origin, v_i absolute, v_i local
-                                             SearchFrame* sf, const int* flags, int nflags, QBatch* qb, QueryStats& st) {
+                                             SearchFrame* sf, const int* flags, int nflags, QBatch* qb, StRef st) {
   const double &ox = u[0], &oy = u[1], &oz = u[2], &vix = u[6], &viy = u[7], &viz = u[8];
   if (has_step_out(g)) {   // section VI-A (vd_options.step_out): shorten the segment first
     double pt[3] = {sf->pt[0], sf->pt[1], sf->pt[2]};
@@ -479,7 +479,7 @@ static __device__ __noinline__ int find_bisector_impl(const double* __restrict__
 template <bool HV, bool DEFER = false>
 __device__ __forceinline__ int find_bisector(const ClipArgs& A, const GridIndex& g, int i, int j, const double* u, double psx, double psy,
                                              double psz, double ptx, double pty, double ptz, const int* flags, int nflags, double& nx,
-                                             double& ny, double& nz, double& d, QueryStats& st, LocalCnt& lc, double* scratch) {
+                                             double& ny, double& nz, double& d, StRef st, LocalCnt& lc, double* scratch) {
   const unsigned e0 = warp_stats().dist_evals;
   QBatch* qb = reinterpret_cast<QBatch*>(scratch);
   SearchFrame* sf = reinterpret_cast<SearchFrame*>(scratch + (sizeof(QBatch) + 7) / 8);

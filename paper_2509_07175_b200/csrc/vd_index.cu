@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points(const GridIndex* __re
   const GridIndex g = *gp;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   extra_cnt_reset();
   for (int64_t q = warp; q < nq; q += nwarps) {
     double best = 2e300;
@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(kBlock) k_delta(const GridIndex* __restrict__ 
   const GridIndex g = *gp;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
-  QueryStats st = {0u, 0u, 0u, 0};
+  QueryStats st = {0};
   extra_cnt_reset();
   for (int64_t i = warp; i < n; i += nwarps) {
     double best = 2e300;
@@ -487,7 +487,7 @@ __global__ void __launch_bounds__(kBlock) k_nearest_points_static(const GridInde
   const GridIndex g = *gp;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / kLanes;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) / kLanes;
-  QueryStats st = {0u, 0u, 0u, 0};
+  QueryStats st = {0};
   extra_cnt_reset();
   for (int64_t q = warp; q < nq; q += nwarps) {
     const double x = S->q[q * dim + 0], y = S->q[q * dim + 1], z = dim == 3 ? S->q[q * dim + 2] : 0.0;

@@ -7,9 +7,16 @@
 namespace vd {
 
 struct QueryStats {
-  unsigned queries, dist_evals, rows;
   int skip;   // SKIP instantiations only (S1b): the site id that does not count as a candidate
 };
+// How the query routines receive it.  The counting fields this struct once had live in shared memory (WarpStats below); what is left
+// is S1b's skip id, which only kernels outside the lean build use -- there the struct travels by value (a dead 4-byte argument)
+// instead of by reference (a pointer that every not-inlined routine keeps alive across its own calls).
+#if VD_EXT
+using StRef = QueryStats&;
+#else
+using StRef = QueryStats;
+#endif
 
 // Work counters that are bumped rarely (per clip, per piece, per measurement-mode query) live in shared memory, one row
 // per warp, instead of in registers of kernels that run at their register cap: [0] corners side-tested by clips,
@@ -107,14 +114,14 @@ __device__ __forceinline__ int for_each_packed(int s, int cnt, int* base, int li
 // query of ~30 candidates in 4-9 rows costs one round of distance evaluations instead of one per row.
 template <bool SKIP>
 static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
-                                              int& bestId, QueryStats& st);
+                                              int& bestId, StRef st);
 
 // TOP = true: g is the site index itself and may hold refined cells (second level); a row that contains
 // one is walked cell by cell afterwards: plain cells are scanned as they are, a refined cell through its
 // own sub-grid (the same routine with TOP = false on a view of that cell).
 template <bool TOP, bool SKIP = false>
 static __device__ __noinline__ void scan_box(const GridIndex& g, double qx, double qy, double qz, int x0, int x1, int y0, int y1,
-                                      int z0, int z1, double& best, int& bestId, QueryStats& st) {
+                                      int z0, int z1, double& best, int& bestId, StRef st) {
   __shared__ int sBase[kWarpsPerBlock][kLanes];
   const int lane = lane_id();
   int* base = sBase[(threadIdx.x / kLanes) % kWarpsPerBlock];
@@ -241,7 +248,7 @@ __device__ __forceinline__ void sub_view(const GridIndex& g, int x, int y, int z
 // restricted to the ball (q, sqrt(best)).
 template <bool SKIP>
 static __device__ __noinline__ void scan_cell(const GridIndex& g, int x, int y, int z, double qx, double qy, double qz, double& best,
-                                              int& bestId, QueryStats& st) {
+                                              int& bestId, StRef st) {
   const int c = (z * g.G[1] + y) * g.G[0] + x;
   if (slab_d2(g, 0, qx, x, x) + slab_d2(g, 1, qy, y, y) + slab_d2(g, 2, qz, z, z) > best) return;
   const int so = __ldg(&g.subOff[c]);
@@ -316,11 +323,11 @@ static __device__ __noinline__ unsigned ball_sites(const GridIndex& g, double qx
 #endif
 template <bool HV, bool SKIP>
 static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
-                                             QueryStats& st, bool nearer_ok);
+                                             StRef st, bool nearer_ok);
 
 template <bool HV, bool SKIP = false>
 __device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
-                                        QueryStats& st, bool nearer_ok = false) {
+                                        StRef st, bool nearer_ok = false) {
   nearest_impl<HV, SKIP>(g, qx, qy, qz, best, bestId, st, nearer_ok);
   if (counts_alg(g)) {
     if (lane_id() == 0) sExtraCnt[(threadIdx.x / kLanes) % kWarpsPerBlock][4] += ball_sites(g, qx, qy, qz, best);
@@ -330,7 +337,7 @@ __device__ __forceinline__ void nearest(const GridIndex& g, double qx, double qy
 
 template <bool HV, bool SKIP>
 static __device__ __noinline__ void nearest_impl(const GridIndex& g, double qx, double qy, double qz, double& best, int& bestId,
-                                             QueryStats& st, bool nearer_ok) {
+                                             StRef st, bool nearer_ok) {
   const double bound0 = best;
   VD_STAT(st.queries += 1;)
   const int cx = cell_of(g, 0, qx), cy = cell_of(g, 1, qy), cz = cell_of(g, 2, qz);

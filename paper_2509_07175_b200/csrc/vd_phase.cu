@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
   const int count = (int)pc->count;
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   for (;;) {
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) 
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   VD_WARP_BAR;
@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   VD_WARP_BAR;
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(kBlock, VD_PH_TAIL_BLOCKS) k_ph_tail(ClipArgs 
   if (threadIdx.x == 0) g = *A.grid;
   __syncthreads();
   const int w = (int)threadIdx.x / kLanes, lane = lane_id();
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   VD_WARP_BAR;
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_finish(ClipArgs A, CellState* 
   const int64_t begin = (int64_t)pc->begin;
   __shared__ PolyF S[kWarpsPerBlock];
   const int w = (int)threadIdx.x / kLanes;
-  QueryStats st = {0u, 0u, 0u};
+  QueryStats st = {0};
   LocalCnt lc = {0u, 0u, 0u, 0u, 0u, 0u};
   extra_cnt_reset();
   VD_WARP_BAR;
