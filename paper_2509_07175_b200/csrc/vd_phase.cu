@@ -38,6 +38,9 @@ namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
 #ifndef VD_PHV_BLOCKS
 #define VD_PHV_BLOCKS VD_PH_BLOCKS   // the verify kernel's own (its shared memory would allow more than fix's)
 #endif
+#ifndef VD_PHV_BLOCKS_HV
+#define VD_PHV_BLOCKS_HV VD_PH_BLOCKS_HV   // (measured on C3, verify alone: 3 blocks 100.0 ms, 4 blocks 91.1, 5 blocks 95.2, 6 blocks 100.4)
+#endif
 constexpr int P3 = 32, C3 = 64;
 constexpr int kTailPairs = 65536;   // a round with at most this many pairs left is finished by k_ph_tail
 using PolyF = Poly3<P3, C3>;
@@ -160,7 +163,7 @@ __global__ void __launch_bounds__(kBlock, 3) k_ph_init(ClipArgs A, CellState* __
 // single-query path goes to the loose list, those corners marked ST_LOOSE), MODE 2 = the second pass over the loose list with
 // the complete test code.  Both passes feed the same clip / done lists.
 template <bool HV, int MODE>
-__global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
+__global__ void __launch_bounds__(kBlock, HV ? VD_PHV_BLOCKS_HV : VD_PHV_BLOCKS) k_ph_verify(ClipArgs A, CellState* __restrict__ cells, int* __restrict__ lists, int cap,
                                                      int* __restrict__ doneList, PhaseCtl* pc, int r, int tailPairs) {
   if (pc->mode != WAVE_PHASED) return;
   if (r > 0 && (int)pc->nClip[r - 1] <= tailPairs) return;
