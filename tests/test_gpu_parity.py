@@ -508,6 +508,27 @@ def test_one_simplex_many_cells(kind):
         assert max(nedges) > 8
 
 
+@pytest.mark.parametrize("kind,opts", [(1, {}), (1, dict(persistent=3)), (1, dict(persistent=0)), (0, {}), (0, dict(persistent=3))])
+def test_triangle_kinds_on_the_refined_index(kind, opts):
+    """Clustered sites (C3's recipe) under the triangle kinds: the refined two-level index, the searches' batch of one and the
+    shared-memory search frame in `k_clip`'s one-kernel form -- per wavefront and as a device-side queue (where the lanes of a
+    warp are least in step).  Surface: the boundary triangles of the C3 replica's cube; 2D: the unit square with the sites'
+    first two coordinates."""
+    w3 = inputs.config(3, "small")
+    if kind == 1:
+        faces = np.concatenate([np.sort(np.delete(w3.simplices, k, axis=1), axis=1) for k in range(4)])
+        u, cnt = np.unique(faces, axis=0, return_counts=True)
+        v, t = inputs.carve(w3.verts, u[cnt == 1].astype(np.int32), np.ones(int((cnt == 1).sum()), bool))
+        w = inputs.custom(inputs.KIND_TRI_SURFACE, w3.sites, v, t, "cube_surface_clustered")
+    else:
+        v, t = inputs.square_grid_mesh(6)
+        w = inputs.custom(inputs.KIND_TRI_2D, np.unique(w3.sites[:, :2], axis=0), v, t, "square_clustered")
+    g, cnt, _ = _gpu(w, **opts)
+    o = oracle.compute(w.sites, w.verts, w.simplices, w.kind)
+    parity.assert_parity(g, o, w.diameter)
+    assert abs(g.measure.sum() - w.measure) <= 1e-11 * w.measure
+
+
 # ---------------------------------------------------------------------- non-convex, disconnected domains (P:L292)
 def test_golden_carved_square_cases_through_the_abi():
     import json, os
