@@ -565,7 +565,7 @@ void vd_destroy(vd_ctx* c) {
   cudaStreamSynchronize(c->stream);
   DevBuf* all[] = {&c->sites, &c->verts, &c->simp, &c->adj, &c->grid, &c->bbox, &c->cellOf, &c->cellStart, &c->cellFill,
                    &c->scanTmp, &c->sorted32, &c->sortKeys, &c->sortVals, &c->sortHist, &c->delta, &c->siteW, &c->sortedW, &c->bTris, &c->bTet, &c->bPlanes, &c->boxVerts, &c->boxVnn, &c->heavyFlag, &c->heavyPrefix, &c->subNeed, &c->subOffRaw, &c->subOff, &c->subCount, &c->subStart,
-                   &c->sorted2, &c->vnn, &c->nearList, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
+                   &c->sorted2, &c->vnn, &c->nearList, &c->nearAuto, &c->phaseCells, &c->phaseLists, &c->control, &c->pairs, &c->pieces, &c->visited, &c->ovf, &c->poolXYZ, &c->poolFlags,
                    &c->poolNbr, &c->siteList, &c->seedPts, &c->seedNN, &c->sitePieces, &c->siteNbrRaw, &c->siteFill, &c->order, &c->nbrRawOff, &c->nbrRaw, &c->nbrCnt,
                    &c->vcount, &c->oMeasure, &c->oCentroid, &c->oNbrOff, &c->oNbr, &c->oPieceOff, &c->oPieceSimplex,
                    &c->oPieceMeasure, &c->oVertOff, &c->oVertXYZ, &c->oVertFlags};

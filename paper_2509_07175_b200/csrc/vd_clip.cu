@@ -113,9 +113,53 @@ __global__ void __launch_bounds__(kBlock) k_dissolve_seeds(ClipArgs A, const dou
   }
 }
 
+// Tet meshes: U19 pays when the cells are about as large as the simplices or smaller and most sites own one -- every pair then
+// faces several of its site's nearest bisectors (C2: 17.0 -> 14.8 ms).  With far sites (C5) or cells that span many simplices
+// nearly all those planes miss the pair's simplex and the list is wasted work.  Decided on the device from two counts: the
+// sites inside the domain's bounding box against n and against m.  auto[0..2] / [3..5]: the box as sortable keys, [6]: the count.
+__device__ __forceinline__ unsigned long long dkey(double v) {
+  const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+  return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double dkey_inv(unsigned long long k) {
+  return __longlong_as_double((long long)((k >> 63) ? (k & 0x7fffffffffffffffull) : ~k));
+}
+__global__ void __launch_bounds__(kBlock) k_near_box(const double* __restrict__ verts, int64_t nv, unsigned long long* __restrict__ au) {
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += (int64_t)gridDim.x * blockDim.x)
+    for (int a = 0; a < 3; ++a) { const double v = verts[i * 3 + a]; lo[a] = fmin(lo[a], v); hi[a] = fmax(hi[a], v); }
+  for (int a = 0; a < 3; ++a) {
+    for (int off = kLanes / 2; off > 0; off >>= 1) {
+      lo[a] = fmin(lo[a], __shfl_xor_sync(kFull, lo[a], off));
+      hi[a] = fmax(hi[a], __shfl_xor_sync(kFull, hi[a], off));
+    }
+    if (lane_id() == 0) { atomicMin(&au[a], dkey(lo[a])); atomicMax(&au[3 + a], dkey(hi[a])); }
+  }
+}
+__global__ void __launch_bounds__(kBlock) k_near_count(const double* __restrict__ sites, int64_t n, unsigned long long* __restrict__ au) {
+  double lo[3], hi[3];
+  for (int a = 0; a < 3; ++a) { lo[a] = dkey_inv(au[a]); hi[a] = dkey_inv(au[3 + a]); }
+  int cnt = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    bool in = true;
+    for (int a = 0; a < 3; ++a) { const double v = sites[i * 3 + a]; in = in && v >= lo[a] && v <= hi[a]; }
+    cnt += in ? 1 : 0;
+  }
+  cnt = warp_sum(cnt);
+  if (lane_id() == 0 && cnt) atomicAdd(&au[6], (unsigned long long)cnt);
+}
+
 // Reading U19: the sites nearest to every site (approximately, from the 3 x 3 x 3 grid cells around it), nearest
 // first; one warp per site.  Their bisectors are the first clips of every piece of that site's cell.
-__global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ list, int K) {
+// au (tet meshes, no explicit vd_options.near_clips): the counts above decide; "no" leaves every list empty.
+__global__ void __launch_bounds__(kBlock) k_near(ClipArgs A, int* __restrict__ list, int K, const unsigned long long* __restrict__ au, long long m) {
+  if (au) {
+    const long long inside = (long long)au[6];
+    if (!(2 * inside >= (long long)A.n && m <= 4 * inside)) {
+      for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < A.n; i += (int64_t)gridDim.x * blockDim.x) list[i * K] = -1;
+      return;
+    }
+  }
   __shared__ GridIndex g;
   __shared__ int ids[kWarpsPerBlock][kLanes];
   if (threadIdx.x == 0) g = *A.grid;
@@ -219,13 +263,14 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : ((KIND == KIN
   flush_counters(A.ctl, st, lc);
 }
 
-// reading U19: by default only the whole-cell kinds start from the bisectors of the nearest sites (measured: on
-// tet meshes the extra plane tests and redundant clips cost more than the searches they save)
+// reading U19: the whole-cell kinds start every cell from the bisectors of its site's 20 nearest sites; tet meshes from 12, where
+// the device-side counts of k_near say it pays (near_auto)
 static int near_clips_of(const vd_ctx* c) {
   const int k = c->opt.near_clips;
-  if (k == 0) return (c->kind == KIND_BOX_3D || (c->kind == KIND_TET_3D && c->opt.dissolve > 0)) ? 20 : 0;
-  return k > kLanes ? kLanes : k;
+  if (k == 0) return (c->kind == KIND_BOX_3D || (c->kind == KIND_TET_3D && c->opt.dissolve > 0)) ? 20 : (c->kind == KIND_TET_3D ? 12 : 0);
+  return k > kLanes ? kLanes : (k < 0 ? 0 : k);
 }
+static bool near_auto(const vd_ctx* c) { return c->opt.near_clips == 0 && c->kind == KIND_TET_3D && !(c->opt.dissolve > 0); }
 
 static ClipArgs make_args(vd_ctx* c) {
   ClipArgs A;
@@ -300,14 +345,23 @@ vd_status stage_seed(vd_ctx* c) {
     // Alg. 5 lines 2-14: classify the sites through the restricted diagram on the boundary, seed boundary sites tet by tet and
     // interior sites as whole cells
     if ((s = stage_nearest_points(c, c->boxVerts.as<double>(), 8, c->boxVnn.as<int>()))) return s;
-    if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+    if (K > 0) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K, nullptr, 0);
     if ((s = stage_dissolve_classify(c))) return s;
     const vd_cells& b = c->boundary->cells;
     VD_LAUNCH(k_dissolve_seeds, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(
         A, b.measure, b.piece_off, b.piece_simplex, b.vert_off, b.vert_xyz, c->bTet.as<int>(), c->bPlanes.as<double4>(), c->nBPlanes, 1e-12);
     return cuda_check(c, cudaGetLastError(), "seed (dissolve)");
   }
-  if (K > 0 && !c->nearReady) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K);
+  const unsigned long long* au = nullptr;
+  if (K > 0 && near_auto(c)) {
+    if ((s = ensure(c, c->nearAuto, sizeof(unsigned long long) * 8))) return s;
+    cudaMemsetAsync(c->nearAuto.p, 0xff, sizeof(unsigned long long) * 3, st);
+    cudaMemsetAsync(c->nearAuto.as<unsigned long long>() + 3, 0, sizeof(unsigned long long) * 5, st);
+    VD_LAUNCH(k_near_box, blocks_for(c->nv, kBlock, sm_count() * 4), kBlock, 0, st)(c->verts.as<double>(), c->nv, c->nearAuto.as<unsigned long long>());
+    VD_LAUNCH(k_near_count, blocks_for(c->n, kBlock, sm_count() * 8), kBlock, 0, st)(c->sites.as<double>(), c->n, c->nearAuto.as<unsigned long long>());
+    au = c->nearAuto.as<unsigned long long>();
+  }
+  if (K > 0 && !c->nearReady) VD_LAUNCH(k_near, blocks_for(c->n, kWarpsPerBlock, sm_count() * 8), kBlock, 0, st)(A, c->nearList.as<int>(), K, au, (long long)c->m);
   c->nearReady = false;   // (set by vd_lloyd: the list holds the previous iteration's neighbours)
   VD_LAUNCH(k_seed, blocks_for(A.aEnd - A.aBegin + 1, kBlock, sm_count() * 8), kBlock, 0, st)(A, c->nc, (boxKind0 || c->opt.seed_corners >= c->nc) ? c->nc : (c->opt.seed_corners > 0 ? c->opt.seed_corners : 1));
   const bool boxKind = c->kind == KIND_BOX_2D || c->kind == KIND_BOX_3D;

@@ -627,14 +627,15 @@ __device__ __forceinline__ void init_poly_3d(Poly3<P, C>& S, const ClipArgs& A, 
 
 // P <- P clipped by the bisector B_ij of a GIVEN site j, no search: any B_ij is a valid clip of Omega_i (Eq. 1).  A
 // plane that does not cut P is skipped.  Returns 0, 1 (capacity), 2 (topology), -1 (skipped).
+// (sx, sy, sz, sw: site j's coordinates and additive term, loaded by the caller -- for a whole list of sites at once, one per lane)
 template <int P, int C>
-__device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A, int j, int& np, int& nc, LocalCnt& lc) {
+__device__ __forceinline__ int clip_by_site_3d(Poly3<P, C>& S, const ClipArgs& A, int j, double sx, double sy, double sz, double sw, int& np, int& nc,
+                                               LocalCnt& lc) {
   const int lane = lane_id();
   VD_POLY_REFS;
-  const double wjx = __ldg(&A.sites[(int64_t)j * 3 + 0]) - ox, wjy = __ldg(&A.sites[(int64_t)j * 3 + 1]) - oy,
-               wjz = __ldg(&A.sites[(int64_t)j * 3 + 2]) - oz;
+  const double wjx = sx - ox, wjy = sy - oy, wjz = sz - oz;
   const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
-  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (((VD_EXT && A.siteW) ? __ldg(&A.siteW[j]) : 0.0) - S.u[12]));
+  const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (sw - S.u[12]));
   // any corner clearly beyond the plane starts R_p: the corners of a convex polytope beyond a plane are connected over its
   // edges, so the flood of apply_clip_3d reaches the same set from each of them (a ballot instead of a warp argmin of the
   // farthest one)
@@ -677,12 +678,18 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
     // they need no point-in-cell test.
     bool complete = true;
     const int pu = np;   // B_iu's plane index, if it cuts
+    // every lane loads its own site: one round trip to L2 for the whole list instead of one per clip
+    double sx = 0.0, sy = 0.0, sz = 0.0, sw = 0.0;
+    if (mine >= 0) {
+      sx = __ldg(&A.sites[(int64_t)mine * 3 + 0]); sy = __ldg(&A.sites[(int64_t)mine * 3 + 1]); sz = __ldg(&A.sites[(int64_t)mine * 3 + 2]);
+      if (VD_EXT && A.siteW) sw = __ldg(&A.siteW[mine]);
+    }
     for (int t = 0; t <= kPairW && nc > 0; ++t) {
       const int j = shfl(mine, t);
       if (j == -2) complete = false;   // f had more adjacent faces than a pair carries
       if (j < 0) break;
       if (j == i) { complete = false; continue; }
-      const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
+      const int rc = clip_by_site_3d(S, A, j, shfl(sx, t), shfl(sy, t), shfl(sz, t), (VD_EXT && A.siteW) ? shfl(sw, t) : 0.0, np, nc, lc);
       if (rc > 0) return rc;
       if (rc < 0) complete = false;
     }
@@ -694,11 +701,20 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
   }
   if (A.nearList && nc > 0 && (!A.dissolve || a == A.wholeA)) {   // (dissolve mode: whole cells only)
     const int K = A.nearClips;
-    const int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
+    int mine = lane < K ? __ldg(&A.nearList[(int64_t)i * K + lane]) : -1;
+    {   // the list ends at its first negative entry (what follows may never have been written)
+      const unsigned neg = __ballot_sync(kFull, mine < 0);
+      if (neg && lane >= __ffs((int)neg) - 1) mine = -1;
+    }
+    double sx = 0.0, sy = 0.0, sz = 0.0, sw = 0.0;
+    if (mine >= 0) {
+      sx = __ldg(&A.sites[(int64_t)mine * 3 + 0]); sy = __ldg(&A.sites[(int64_t)mine * 3 + 1]); sz = __ldg(&A.sites[(int64_t)mine * 3 + 2]);
+      if (VD_EXT && A.siteW) sw = __ldg(&A.siteW[mine]);
+    }
     for (int t = 0; t < K; ++t) {
       const int j = shfl(mine, t);
       if (j < 0) break;
-      const int rc = clip_by_site_3d(S, A, j, np, nc, lc);
+      const int rc = clip_by_site_3d(S, A, j, shfl(sx, t), shfl(sy, t), shfl(sz, t), (VD_EXT && A.siteW) ? shfl(sw, t) : 0.0, np, nc, lc);
       if (rc > 0) return rc;
       if (nc == 0) break;
     }

@@ -111,6 +111,7 @@ struct vd_ctx {
   vd::DevBuf vnn;         // int [nv]   nearest site of every mesh vertex
   vd::DevBuf seedPts, seedNN;   // extra seed points inside the simplices and their nearest sites (few simplices, many sites)
   vd::DevBuf nearList;    // int [n][nearClips]  sites nearest to every site, nearest first, -1 padded (reading U19)
+  vd::DevBuf nearAuto;    // 7 x uint64: the domain's box (sortable keys of lo / hi) and the number of sites inside it (tet meshes: whether U19 pays)
   vd::DevBuf control;     // Control
   vd::DevBuf phaseCells;  // phased mode: polytopes of one wave parked between the step kernels (vd_phase.cu)
   vd::DevBuf phaseLists;  // phased mode: work lists + counters
