@@ -84,7 +84,7 @@ typedef struct vd_cells {
 
 /* Tunables (P:L383 grid density; P:L369 step-out).  Zero / negative fields mean "default". */
 typedef struct vd_options {
-  double grid_density;    /* average sites per grid cell of the site index (default 4.0; paper 2~4) */
+  double grid_density;    /* average sites per grid cell of the site index (default 2.0, measured; paper 2~4) */
   int32_t ball_cells;     /* one-shot bisector search (reading U18): most grid cells its ball
                              scan may cover; 0 = default (64); < 0: only the stepwise search of P:L137.
                              (The step-out of section VI-A, is not needed: U7.)            */

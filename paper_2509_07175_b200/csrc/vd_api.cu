@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kBlock) k_finish_centroids(const double* __res
 
 static void set_default_options(vd_options& o) {
   memset(&o, 0, sizeof(o));
-  o.grid_density = 4.0;
+  o.grid_density = 2.0;
   o.real_edges = 1;
   o.persistent = 1;
 }

@@ -367,7 +367,7 @@ static int grid_for(int64_t items, int perBlock) {
 
 vd_status stage_index(vd_ctx* c) {
   const int64_t n = c->n;
-  const double density = c->opt.grid_density > 0 ? c->opt.grid_density : 4.0;
+  const double density = c->opt.grid_density > 0 ? c->opt.grid_density : 2.0;
   const int64_t gridCap = (int64_t)((double)n / density) * 2 + 64;
   c->gridCap = gridCap;
   vd_status s;
