@@ -12,7 +12,16 @@ namespace vd {
 constexpr int kQB = 8;          // queries per batch
 // rows of a query's ball above which it takes the single-query path: 32, and 64 on the top grid of a refined index (measured:
 // 8 / 16 / 32 / 64 rows: C3 405 / 324 / 311 / 306 ms, C5 16.2 / 16.3 / 16.2 / 18.1 ms, C2 21.1 / 20.2 / 20.2 / 20.2 ms)
-constexpr int kQBMaxRows = 32, kQBMaxRowsPlanar = 16, kQBMaxRowsRefined = 64;   // (planar grid, C1: 16 rows 1.05 ms, 32 rows 1.23 ms --
+#ifndef VD_QB_ROWS
+#define VD_QB_ROWS 32
+#endif
+#ifndef VD_QB_ROWS_REFINED
+#define VD_QB_ROWS_REFINED 64
+#endif
+#ifndef VD_QB_ROWS_PLANAR
+#define VD_QB_ROWS_PLANAR 16
+#endif
+constexpr int kQBMaxRows = VD_QB_ROWS, kQBMaxRowsPlanar = VD_QB_ROWS_PLANAR, kQBMaxRowsRefined = VD_QB_ROWS_REFINED;   // (planar grid, C1: 16 rows 1.05 ms, 32 rows 1.23 ms --
 // the batched pass has no early exit, and a bare triangle's corners have loose bounds in a dense grid)
 
 struct QBatch {
