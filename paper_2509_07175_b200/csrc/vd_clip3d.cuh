@@ -711,9 +711,26 @@ __device__ __forceinline__ int preclip_3d(Poly3<P, C>& S, const ClipArgs& A, int
       sx = __ldg(&A.sites[(int64_t)mine * 3 + 0]); sy = __ldg(&A.sites[(int64_t)mine * 3 + 1]); sz = __ldg(&A.sites[(int64_t)mine * 3 + 2]);
       if (VD_EXT && A.siteW) sw = __ldg(&A.siteW[mine]);
     }
-    for (int t = 0; t < K; ++t) {
+    // which of the listed bisectors cut P as it stands?  One lane per plane, all planes at once (P only shrinks from here on, so a
+    // plane that misses it now misses it for good); only those take their turn in the loop below -- on a mesh whose simplices are
+    // smaller than the cells most of the list misses most pairs
+    unsigned cand;
+    {
+      VD_POLY_REFS;
+      bool cuts = false;
+      if (mine >= 0) {
+        const double wjx = sx - ox, wjy = sy - oy, wjz = sz - oz;
+        const double nx = wjx - vix, ny = wjy - viy, nz = wjz - viz;
+        const double d = 0.5 * (nx * (vix + wjx) + ny * (viy + wjy) + nz * (viz + wjz) + (sw - S.u[12]));
+        const double tol = 1e-9 * (nx * nx + ny * ny + nz * nz);
+        for (int c = 0; c < nc && !cuts; ++c) cuts = (nx * S.cx[c] + ny * S.cy[c] + nz * S.cz[c] - d > tol) && S.cstate[c] != ST_IN;
+      }
+      cand = __ballot_sync(kFull, cuts);
+    }
+    while (cand) {
+      const int t = __ffs((int)cand) - 1;
+      cand &= cand - 1;
       const int j = shfl(mine, t);
-      if (j < 0) break;
       const int rc = clip_by_site_3d(S, A, j, shfl(sx, t), shfl(sy, t), shfl(sz, t), (VD_EXT && A.siteW) ? shfl(sw, t) : 0.0, np, nc, lc);
       if (rc > 0) return rc;
       if (nc == 0) break;
