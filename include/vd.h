@@ -104,7 +104,7 @@ typedef struct vd_options {
   int64_t vert_capacity;  /* initial capacity of the corner pool; grows on demand                   */
   int32_t near_clips;     /* every piece of cell i is first clipped by the bisectors of this many of the
                              sites nearest to v_i (reading U19), so that the point-in-cell loop
-                             starts from a small polytope; 0 = default: 20 for VD_BOX_3D; 12 for VD_TET_3D when at
+                             starts from a small polytope; 0 = default: 24 for VD_BOX_3D; 16 for VD_TET_3D when at
                              least half of the sites lie inside the domain's bounding box and m <= 4 x that count
                              (decided on the device in every compute: cells about as large as the simplices or
                              smaller -- else the lists stay empty); > 0: that many, always; < 0: none; at most 32.

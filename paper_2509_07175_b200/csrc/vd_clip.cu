@@ -263,11 +263,11 @@ __global__ void __launch_bounds__(BIG ? kLanes : kBlock, BIG ? 1 : ((KIND == KIN
   flush_counters(A.ctl, st, lc);
 }
 
-// reading U19: the whole-cell kinds start every cell from the bisectors of its site's 20 nearest sites; tet meshes from 12, where
+// reading U19: the whole-cell kinds start every cell from the bisectors of its site's 24 nearest sites; tet meshes from 16, where
 // the device-side counts of k_near say it pays (near_auto)
 static int near_clips_of(const vd_ctx* c) {
   const int k = c->opt.near_clips;
-  if (k == 0) return (c->kind == KIND_BOX_3D || (c->kind == KIND_TET_3D && c->opt.dissolve > 0)) ? 20 : (c->kind == KIND_TET_3D ? 12 : 0);
+  if (k == 0) return (c->kind == KIND_BOX_3D || (c->kind == KIND_TET_3D && c->opt.dissolve > 0)) ? 24 : (c->kind == KIND_TET_3D ? 16 : 0);
   return k > kLanes ? kLanes : (k < 0 ? 0 : k);
 }
 static bool near_auto(const vd_ctx* c) { return c->opt.near_clips == 0 && c->kind == KIND_TET_3D && !(c->opt.dissolve > 0); }
