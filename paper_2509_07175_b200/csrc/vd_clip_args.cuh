@@ -193,10 +193,25 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
 // nearest few sites are almost always Voronoi neighbours, so clipping the box by them first costs no search and
 // leaves a small polytope whose corners are all close to the cell.  Selection is approximate on purpose: each
 // lane keeps the nearest of the candidates it saw, the k best lanes win.
-static __device__ __noinline__ int near_sites(const GridIndex& g, double vx, double vy, double vz, int i, int k, int* out, StRef st) {
+// A site in a refined cell (clustered sites) looks around in that cell's sub-grid instead: the 27 top cells around it hold
+// thousands of sites there, of which the first 512 in storage order are no one's nearest.
+static __device__ __noinline__ int near_sites(const GridIndex& gTop, double vx, double vy, double vz, int i, int k, int* out, StRef st) {
   __shared__ int sBaseN[kWarpsPerBlock][kLanes];
   const int lane = lane_id();
   int* base = sBaseN[(threadIdx.x / kLanes) % kWarpsPerBlock];
+  const GridIndex* gp = &gTop;
+  if (gTop.subOff) {
+    const int tx = cell_of(gTop, 0, vx), ty = cell_of(gTop, 1, vy), tz = cell_of(gTop, 2, vz);
+    const int so = __ldg(&gTop.subOff[(tz * gTop.G[1] + ty) * gTop.G[0] + tx]);
+    if (so >= 0) {
+      GridIndex& v = warp_view();
+      __syncwarp();
+      if (lane == 0) sub_view(gTop, tx, ty, tz, so, v);
+      __syncwarp();
+      gp = &v;
+    }
+  }
+  const GridIndex& g = *gp;
   const int cx = cell_of(g, 0, vx), cy = cell_of(g, 1, vy), cz = cell_of(g, 2, vz);
   const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.G[0] - 1);
   const int y0 = max(cy - 1, 0), y1 = min(cy + 1, g.G[1] - 1);
