@@ -192,7 +192,10 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
 // nearest first, into out[]; returns how many.  Any bisector B_ij is a valid clip of Omega_i (Eq. 1), and the
 // nearest few sites are almost always Voronoi neighbours, so clipping the box by them first costs no search and
 // leaves a small polytope whose corners are all close to the cell.  Selection is approximate on purpose: each
-// lane keeps the nearest of the candidates it saw, the k best lanes win.
+// lane keeps the two nearest of the candidates it saw, the k best of those 64 win.
+#ifndef VD_NEAR_LIMIT
+#define VD_NEAR_LIMIT 256   // (measured on C3: 16 -> 207 ms, 64 -> 177, 256 -> 174, 1024 -> 174)
+#endif
 // A site in a refined cell (clustered sites) looks around in that cell's sub-grid instead: the 27 top cells around it hold
 // thousands of sites there, of which the first 512 in storage order are no one's nearest.
 static __device__ __noinline__ int near_sites(const GridIndex& gTop, double vx, double vy, double vz, int i, int k, int* out, StRef st) {
@@ -224,16 +227,19 @@ static __device__ __noinline__ int near_sites(const GridIndex& gTop, double vx, 
     s = __ldg(&g.cellStart[rowBase + x0]);
     cnt = __ldg(&g.cellStart[rowBase + x1 + 1]) - s;
   }
-  double md = 2e300;
-  int mi = 0x7fffffff;
-  const int total = for_each_packed(s, cnt, base, 16 * kLanes /* a dense cluster: the first 512 will do */, [](int) {},
+  double md = 2e300, md2 = 2e300;   // the nearest and the second nearest this lane saw
+  int mi = 0x7fffffff, mi2 = 0x7fffffff;
+  const int total = for_each_packed(s, cnt, base, VD_NEAR_LIMIT * kLanes /* a dense neighbourhood: the first VD_NEAR_LIMIT x 32 candidates will do */, [](int) {},
                                     [&](bool valid, int pos, int) {
     if (valid) {
       const double4 p = g.sites[pos];
       const int id = (int)(__double_as_longlong(p.w) & 0x7fffffff);
       const double dx = vx - p.x, dy = vy - p.y, dz = vz - p.z;
       const double d2 = dx * dx + dy * dy + dz * dz;
-      if (id != i && d2 > 0.0 && closer(d2, id, md, mi)) { md = d2; mi = id; }
+      if (id != i && d2 > 0.0) {
+        if (closer(d2, id, md, mi)) { md2 = md; mi2 = mi; md = d2; mi = id; }
+        else if (closer(d2, id, md2, mi2)) { md2 = d2; mi2 = id; }
+      }
     }
   });
   VD_STAT(st.dist_evals += (unsigned)total;)
@@ -244,7 +250,7 @@ static __device__ __noinline__ int near_sites(const GridIndex& gTop, double vx, 
     warp_argmin(bd, bi);
     if (bi == 0x7fffffff) break;
     if (lane == 0) out[found] = bi;
-    if (mi == bi) { md = 2e300; mi = 0x7fffffff; }
+    if (mi == bi) { md = md2; mi = mi2; md2 = 2e300; mi2 = 0x7fffffff; }
   }
   __syncwarp();
   return found;
