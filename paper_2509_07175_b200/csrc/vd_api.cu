@@ -533,8 +533,7 @@ vd_status vd_lloyd(vd_ctx* c, int iterations, vd_cells* out, double* sites_out) 
   for (int it = 0; it < iterations; ++it) {
     if ((s = vd_compute(c, out))) return s;
     if (c->opt.reuse_nbrs >= 0 && c->kind == VD_BOX_3D && !c->weighted && c->nearList.p) {
-      int K = c->opt.near_clips == 0 ? 20 : c->opt.near_clips;
-      if (K > kLanes) K = kLanes;
+      const int K = c->nearK;   // the width the clip kernels read the list with
       if (K > 0) {
         VD_LAUNCH(k_near_from_nbrs, blocks, kBlock, 0, c->stream)(c->oNbrOff.as<int64_t>(), c->oNbr.as<int>(), c->sites.as<double>(), c->n, K,
                                                                   c->nearList.as<int>());

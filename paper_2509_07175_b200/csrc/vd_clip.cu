@@ -334,6 +334,8 @@ vd_status stage_seed(vd_ctx* c) {
   cudaMemsetAsync(c->sitePieces.p, 0, sizeof(int) * c->n, st);
   cudaMemsetAsync(c->siteNbrRaw.p, 0, sizeof(int) * c->n, st);
   const int K = near_clips_of(c);
+  if (K != c->nearK) c->nearReady = false;   // (a list of another width is of no use)
+  c->nearK = K;
   if (K > 0) {
     if ((s = ensure(c, c->nearList, sizeof(int) * c->n * K))) return s;
   } else {

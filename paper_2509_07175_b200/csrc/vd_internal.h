@@ -56,6 +56,7 @@ struct vd_ctx {
                            //                     dim 3 -> siteW holds the additive term eta - w_i of every site
   int64_t syncs = 0;       // host waits on the stream inside the current vd_compute
   bool nearReady = false;  // nearList already holds the first clips of the next compute (vd_lloyd: the previous neighbours)
+  int nearK = 0;           // entries per site of nearList in the last compute (0: no list)
   int heavyKnown = -1;     // refined cells of the site index as last built, while sites and grid options are unchanged; else -1
   bool haveDomain = false, haveResult = false, indexValid = false;
   cudaStream_t stream = nullptr;

@@ -387,6 +387,25 @@ def test_box_domain_wave_mode_and_lloyd():
         parity.assert_parity(g, oracle.compute(got, w.verts, None, w.kind, tier="B"), w.diameter)
 
 
+def test_lloyd_reuses_the_previous_neighbours_as_first_clips():
+    """vd_lloyd, whole cells: iteration k + 1 starts every cell from the bisectors of its neighbours of iteration k (the list the clip
+    kernels read must have the width vd_lloyd writes it with -- a mismatch once made every list garbage: valid clips, five times the
+    time).  With the lists in place nearly every face comes from a first clip, as with fresh lists from k_near -- garbage lists
+    leave most faces to the searches."""
+    w = inputs.box(3, 20000, seed=3)
+    with binding.Context(w.sites) as ctx:
+        ctx.set_options(count_alg=1)
+        ctx.set_domain(w.verts, None, w.kind)
+        ctx.lloyd(3)                                   # (the third compute ran on the second's neighbours)
+        reuse = ctx.counters()
+        ctx.set_options(count_alg=1, reuse_nbrs=-1)
+        ctx.compute()                                  # the same sites, lists from k_near
+        fresh = ctx.counters()
+    assert reuse["pieces"] == fresh["pieces"] == w.n
+    assert reuse["search_iters"] < 1.5 * fresh["search_iters"] < 1.5 * w.n, (reuse["search_iters"], fresh["search_iters"])
+    assert reuse["pre_clips"] > 0.9 * reuse["clips"]
+
+
 def test_support_calls_phase_times_counters_and_pinned_copy():
     w = inputs.config(2, "small")
     with binding.Context(w.sites) as ctx:
