@@ -225,18 +225,21 @@ static __device__ __noinline__ unsigned batch_nearest(const GridIndex& gTop, QBa
 #ifdef VD_COUNT_LOOSE
   extra_cnt_add(3, (unsigned)__popc(looseMask));   // (experiment: reported as step_probes)
 #endif
-  if constexpr (!FALLBACK) return looseMask;
-  while (looseMask) {
-    const int u = __ffs(looseMask) - 1;
-    looseMask &= looseMask - 1;
-    double best = B.best[u];
-    int bestId = B.bestId[u];
-    nearest<HV>(gTop, B.qx[u], B.qy[u], B.qz[u], best, bestId, st, true);
-    __syncwarp();
-    if (lane == 0) { B.best[u] = best; B.bestId[u] = bestId; }
-    __syncwarp();
+  if constexpr (!FALLBACK) {
+    return looseMask;
+  } else {
+    while (looseMask) {
+      const int u = __ffs(looseMask) - 1;
+      looseMask &= looseMask - 1;
+      double best = B.best[u];
+      int bestId = B.bestId[u];
+      nearest<HV>(gTop, B.qx[u], B.qy[u], B.qz[u], best, bestId, st, true);
+      __syncwarp();
+      if (lane == 0) { B.best[u] = best; B.bestId[u] = bestId; }
+      __syncwarp();
+    }
+    return 0u;
   }
-  return 0u;
 }
 
 }  // namespace vd

@@ -181,7 +181,7 @@ PhaseCtl* phase_ctl(vd_ctx* c, int64_t cap);
 constexpr int kSmallWave = 8192;       // phased schedule: a wavefront smaller than this runs as one launch of the one-kernel form
 constexpr int P3 = 32, C3 = 64;        // fast tier: planes / corners per piece held per warp
 constexpr int P3B = 256, C3B = 512;    // large tier (one warp per block)
-constexpr int K2 = 32, K2B = 256;
+constexpr int K2B = 256;                // large 2D tier: corners per polygon
 
 // The one-kernel form: a warp takes a pair through all of Alg. 3.  What it works on comes from the wave program's state
 // (k_wave_begin): fast tier -- the wave [pc->begin, + pc->count) (WAVE_SINGLE), or the whole list from the wave's first pair

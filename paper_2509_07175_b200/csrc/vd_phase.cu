@@ -42,7 +42,6 @@ namespace VD_VARIANT {   // compiled twice: header of vd_clip.cu
 #define VD_PHV_BLOCKS_HV VD_PH_BLOCKS_HV   // (measured on C3, verify alone: 3 blocks 100.0 ms, 4 blocks 91.1, 5 blocks 95.2, 6 blocks 100.4)
 #endif
 constexpr int P3 = 32, C3 = 64;
-constexpr int kTailPairs = 65536;   // a round with at most this many pairs left is finished by k_ph_tail
 using PolyF = Poly3<P3, C3>;
 using PolyT = PolyTest3<P3, C3>;   // k_ph_verify's view of a parked polytope
 
@@ -280,7 +279,7 @@ __global__ void __launch_bounds__(kBlock, HV ? VD_PH_BLOCKS_HV : VD_PH_BLOCKS) k
   flush_counters(A.ctl, st, lc, CNT_FIX);
 }
 
-// The last few pairs of a wave (a verify round left fewer than kTailPairs with a corner outside): tests and clips
+// The last few pairs of a wave (a verify round left at most `tail_pairs` (65 536) pairs with a corner outside): tests and clips
 // alternate inside one launch until every corner is in Omega_i -- Alg. 3's loop as it stands --
 // instead of one round trip to the host and two nearly empty launches per remaining round.  Finished pairs join the
 // done list.  The whole loop in one kernel is the instruction-fetch-bound form (header of this file); on a few
