@@ -193,6 +193,9 @@ __device__ __forceinline__ void pair_done(const ClipArgs& A) {
 // nearest few sites are almost always Voronoi neighbours, so clipping the box by them first costs no search and
 // leaves a small polytope whose corners are all close to the cell.  Selection is approximate on purpose: each
 // lane keeps the two nearest of the candidates it saw, the k best of those 64 win.
+#ifndef VD_NEAR_R
+#define VD_NEAR_R 1   // half width, in cells, of the window near_sites looks around in (at most 2)
+#endif
 #ifndef VD_NEAR_LIMIT
 #define VD_NEAR_LIMIT 256   // (measured on C3: 16 -> 207 ms, 64 -> 177, 256 -> 174, 1024 -> 174)
 #endif
@@ -216,10 +219,10 @@ static __device__ __noinline__ int near_sites(const GridIndex& gTop, double vx, 
   }
   const GridIndex& g = *gp;
   const int cx = cell_of(g, 0, vx), cy = cell_of(g, 1, vy), cz = cell_of(g, 2, vz);
-  const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.G[0] - 1);
-  const int y0 = max(cy - 1, 0), y1 = min(cy + 1, g.G[1] - 1);
-  const int z0 = max(cz - 1, 0), z1 = min(cz + 1, g.G[2] - 1);
-  const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);
+  const int x0 = max(cx - VD_NEAR_R, 0), x1 = min(cx + VD_NEAR_R, g.G[0] - 1);
+  const int y0 = max(cy - VD_NEAR_R, 0), y1 = min(cy + VD_NEAR_R, g.G[1] - 1);
+  const int z0 = max(cz - VD_NEAR_R, 0), z1 = min(cz + VD_NEAR_R, g.G[2] - 1);
+  const int ny = y1 - y0 + 1, nrows = ny * (z1 - z0 + 1);   // (at most 25: one lane per row)
   int s = 0, cnt = 0;
   if (lane < nrows) {
     const int rz = lane / ny;
